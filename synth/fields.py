@@ -1,0 +1,208 @@
+"""Counter-based seeded field generators (numpy only).
+
+Recipe (BASELINE.json configs):
+
+* RNG: splitmix64 finaliser applied to ``key + (counter+1)*GOLDEN`` where
+  ``key = mix(mix(seed) + field_id)``; 53-bit uniforms in (0,1); Box-Muller
+  (cosine branch) on the uniform pair (2c, 2c+1) gives normal number ``c``.
+* SU(3) links: ``G_ij ~ N(0,1)+iN(0,1)``, ``H=(G+G^dag)/2 - tr/3``,
+  ``U=exp(i*eps*H)`` (scaling-and-squaring Taylor), then re-unitarised
+  (normalise row 0, Gram-Schmidt row 1, row 2 = conj(row0 x row1)) so that a
+  12-real reconstruct is exact to rounding.
+* U(1): ``A_mu(x) ~ N(0, sigma^2)`` iid.
+* Spinors: ``eta ~ N(0,1)+iN(0,1)`` per component.
+
+The stand-in status of these inputs (for the CLS G8 / RC* C380 ensembles of
+PAPER.md:155-160, which are not available) is stated in DESIGN.md.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+_GOLDEN = np.uint64(0x9E3779B97F4A7C15)
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+
+FIELD_SU3 = 1
+FIELD_U1 = 2
+FIELD_SPINOR = 3
+FIELD_GAUGE_TRAFO = 4
+FIELD_U1_TRAFO = 5
+
+
+def splitmix64(z):
+    """splitmix64 output function on a uint64 array (wrap-around arithmetic)."""
+    z = np.asarray(z, dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        z = (z ^ (z >> np.uint64(30))) * _M1
+        z = (z ^ (z >> np.uint64(27))) * _M2
+        z = z ^ (z >> np.uint64(31))
+    return z
+
+
+def _key(seed: int, field_id: int) -> np.uint64:
+    with np.errstate(over="ignore"):
+        k = splitmix64(np.uint64(seed) * _GOLDEN + np.uint64(0x1234567))
+        k = splitmix64(k + np.uint64(field_id) * _GOLDEN)
+    return np.uint64(k)
+
+
+def uniform01(seed: int, field_id: int, counter):
+    """Uniform in the open interval (0,1) for each uint64 counter."""
+    c = np.asarray(counter, dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        z = splitmix64(_key(seed, field_id) + (c + np.uint64(1)) * _GOLDEN)
+    return (z >> np.uint64(11)).astype(np.float64) * 2.0**-53 + 2.0**-54
+
+
+def normal(seed: int, field_id: int, counter):
+    """Standard normal number ``counter`` (Box-Muller, cosine branch)."""
+    c = np.asarray(counter, dtype=np.uint64)
+    u1 = uniform01(seed, field_id, c * np.uint64(2))
+    u2 = uniform01(seed, field_id, c * np.uint64(2) + np.uint64(1))
+    return np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)
+
+
+def _mm(A, B):
+    """3x3 complex matrix product on component-major arrays ``[3,3,n]``.
+
+    Pure elementwise vector arithmetic: the result for one matrix does not
+    depend on how the batch is chunked.
+    """
+    C = np.empty_like(A)
+    for i in range(3):
+        for k in range(3):
+            C[i, k] = A[i, 0] * B[0, k] + A[i, 1] * B[1, k] + A[i, 2] * B[2, k]
+    return C
+
+
+_EXP_SQUARINGS = 5
+_EXP_ORDER = 12
+
+
+def _expm_i_herm(H, eps):
+    """exp(i*eps*H) on ``[3,3,n]``: fixed scaling 2^-5, Taylor order 12, 5 squarings."""
+    X = ((1j * eps) / 2.0**_EXP_SQUARINGS) * H
+    E = X.copy()
+    for i in range(3):
+        E[i, i] += 1.0
+    term = X
+    for k in range(2, _EXP_ORDER + 1):
+        term = _mm(term, X) / k
+        E = E + term
+    for _ in range(_EXP_SQUARINGS):
+        E = _mm(E, E)
+    return E
+
+
+def _reunitarise(U):
+    """Rows 0,1 orthonormalised, row 2 = conj(row0 x row1); ``U`` is ``[3,3,n]``."""
+    r0 = U[0]
+    r1 = U[1]
+    r0 = r0 / np.sqrt(np.sum(np.abs(r0) ** 2, axis=0))
+    r1 = r1 - np.sum(np.conj(r0) * r1, axis=0) * r0
+    r1 = r1 / np.sqrt(np.sum(np.abs(r1) ** 2, axis=0))
+    r2 = np.conj(np.stack([r0[1] * r1[2] - r0[2] * r1[1],
+                           r0[2] * r1[0] - r0[0] * r1[2],
+                           r0[0] * r1[1] - r0[1] * r1[0]]))
+    return np.stack([r0, r1, r2])
+
+
+def _su3_from_counter(n0, n, eps, seed, field_id):
+    """SU(3) matrices number n0..n0+n-1 (each uses 18 normals); returns ``[n,3,3]``."""
+    idx = (np.arange(n0, n0 + n, dtype=np.uint64)[None, :] * np.uint64(18)
+           + np.arange(18, dtype=np.uint64)[:, None])
+    g = normal(seed, field_id, idx).reshape(3, 3, 2, n)
+    G = g[:, :, 0] + 1j * g[:, :, 1]
+    H = 0.5 * (G + np.conj(np.swapaxes(G, 0, 1)))
+    tr = (H[0, 0] + H[1, 1] + H[2, 2]).real / 3.0
+    for i in range(3):
+        H[i, i] -= tr
+    U = _reunitarise(_expm_i_herm(H, eps))
+    return np.ascontiguousarray(np.moveaxis(U, -1, 0))
+
+
+def _chunked(n, chunk, fill):
+    """Run ``fill(a, b)`` over [0,n) in chunks on a small thread pool (numpy releases the GIL;
+    results are chunking-independent because every value is a pure function of its counter)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    spans = [(a, min(n, a + chunk)) for a in range(0, n, chunk)]
+    workers = max(1, min(len(spans), os.cpu_count() or 1, 16))
+    if workers == 1:
+        for a, b in spans:
+            fill(a, b)
+        return
+    with ThreadPoolExecutor(workers) as ex:
+        list(ex.map(lambda ab: fill(*ab), spans))
+
+
+def su3_links(dims, eps: float, seed: int = 1, chunk: int = 1 << 14):
+    """SU(3) links on the PHYSICAL lattice: complex128 ``[T,L1,L2,L3,4,3,3]``.
+
+    Matrix number ``Lambda(x)*4 + mu`` (Lambda = Eq. (1) of PAPER.md:93).
+    """
+    T, L1, L2, L3 = dims
+    n = T * L1 * L2 * L3 * 4
+    out = np.empty((n, 3, 3), dtype=np.complex128)
+
+    def fill(a, b):
+        out[a:b] = _su3_from_counter(a, b - a, eps, seed, FIELD_SU3)
+
+    _chunked(n, chunk, fill)
+    return out.reshape(T, L1, L2, L3, 4, 3, 3)
+
+
+def random_su3(n: int, seed: int, eps: float = 1.0):
+    """``n`` random SU(3) matrices (for gauge transformations in tests)."""
+    return _su3_from_counter(0, n, eps, seed, FIELD_GAUGE_TRAFO)
+
+
+def u1_field(dims, sigma: float = 0.3, seed: int = 2, field_id: int = FIELD_U1):
+    """Non-compact U(1) field ``A_mu(x) ~ N(0,sigma^2)``: float64 ``[T,L1,L2,L3,4]``."""
+    T, L1, L2, L3 = dims
+    n = T * L1 * L2 * L3 * 4
+    a = normal(seed, field_id, np.arange(n, dtype=np.uint64)) * sigma
+    return a.reshape(T, L1, L2, L3, 4)
+
+
+def gaussian_spinor(dims_ext, seed: int = 3, chunk: int = 1 << 16):
+    """Gaussian spinor on the EXTENDED lattice: complex128 ``[T,X1,L2,L3,4,3]``."""
+    T, X1, L2, L3 = dims_ext
+    n = T * X1 * L2 * L3 * 12
+    out = np.empty(n, dtype=np.complex128)
+
+    def fill(a, b):
+        c = np.arange(a, b, dtype=np.uint64)
+        out[a:b] = (normal(seed, FIELD_SPINOR, c * np.uint64(2))
+                    + 1j * normal(seed, FIELD_SPINOR, c * np.uint64(2) + np.uint64(1)))
+
+    _chunked(n, chunk, fill)
+    return out.reshape(T, X1, L2, L3, 4, 3)
+
+
+# ---------------------------------------------------------------------------
+# The five BASELINE.json configurations (shapes and couplings only).
+# kappa for c2/c3 is "tuned" (SURVEY.md §8(d) protocol); the values here are the
+# result of that tuning with the fp64 GPU solver and are recorded in DESIGN.md.
+# ---------------------------------------------------------------------------
+CONFIGS = {
+    "c0": dict(dims=(4, 4, 4, 4), cstar=0, antiperiodic=1, eps=0.3, qed=False, q=0.0, qel=1.0,
+               kappa=0.12, csw=1.5, csw_qed=0.0, tol=1e-12),
+    "c1": dict(dims=(8, 8, 8, 8), cstar=3, antiperiodic=1, eps=0.3, qed=True, q=2.0 / 3.0, qel=1.0,
+               kappa=0.12, csw=1.5, csw_qed=1.0, tol=1e-12),
+    "c2": dict(dims=(32, 16, 16, 16), cstar=3, antiperiodic=1, eps=0.15, qed=True, q=2.0 / 3.0, qel=1.0,
+               kappa=0.1315, csw=1.7, csw_qed=1.0, tol=1e-10),
+    "c3": dict(dims=(64, 32, 32, 32), cstar=3, antiperiodic=1, eps=0.15, qed=True, q=2.0 / 3.0, qel=1.0,
+               kappa=0.1315, csw=1.7, csw_qed=1.0, tol=1e-10),
+    "c4": dict(dims=(96, 48, 48, 48), cstar=0, antiperiodic=1, eps=0.15, qed=False, q=0.0, qel=1.0,
+               kappa=0.1315, csw=1.7, csw_qed=0.0, tol=1e-10, nrhs=12),
+}
+
+
+def config(name: str) -> dict:
+    c = dict(CONFIGS[name])
+    T, L1, L2, L3 = c["dims"]
+    c["dims_ext"] = (T, 2 * L1 if c["cstar"] > 0 else L1, L2, L3)
+    c["bc"] = c["cstar"] | (c["antiperiodic"] << 2)
+    return c
