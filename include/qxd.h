@@ -1,0 +1,156 @@
+/* =====================================================================================
+ * qxd.h -- C ABI of the B200-native clover-Wilson QCD+QED Dirac solver with C* boundaries.
+ *
+ * The library solves D_w psi = eta for the O(a)-improved Wilson-Dirac operator
+ * with U(3) hopping links e^{i q A_mu(x)} U_mu(x), the
+ * SU(3)+U(1) Sheikholeslami-Wohlert (clover) term and C* spatial boundary
+ * conditions realised as a lattice doubled in direction 1 with shifted boundaries
+ * (PAPER.md:137).  The operator itself is never written in the paper; the definition used is
+ * recorded in DESIGN.md "Readings" (R1..R18).  The paper's own boundary is
+ * invertQuda(void* h_x, void* h_b, param) on host arrays in application order
+ * (PAPER.md:73-79); this ABI keeps that spirit ("interfacing only a minimal set of
+ * parameters"): plain pointers and sizes, no C++/torch types.
+ *
+ * Conventions common to all calls
+ *  - Every function returns a qxd_status (0 = QXD_OK).  No exceptions, no abort, no stdout.
+ *    qxd_last_error(ctx) gives a human-readable message for the last failing call.
+ *  - Pointers marked DEVICE are CUDA device pointers owned by the caller (PyTorch tensors);
+ *    pointers marked HOST are host pointers.  The library never allocates device memory: the
+ *    caller provides one workspace (qxd_workspace_bytes / qxd_workspace_bind).
+ *  - Calls enqueue work on the bound CUDA stream (qxd_set_stream; default stream 0).  Only
+ *    qxd_solve*, the *_host variants and the qxd_blas_* reductions synchronise that stream.
+ *  - Natural ("application") order, used by every non-packed entry point:
+ *      site index  Lambda(x) = L3 L2 X1 x0 + L3 L2 x1 + L3 x2 + x3        (Eq. (1))
+ *      with x = (t,x,y,z) and X1 = 2*L1 if C* is on (extended lattice) else L1;
+ *      spinor  [V][4 spin][3 colour] complex fp64 (re,im), colour fastest;
+ *      links   [V_phys][4 mu][3][3] complex fp64 row-major, the 4 FORWARD links of every site
+ *              of the PHYSICAL lattice T x L1 x L2 x L3 (the "common convention" of
+ *              PAPER.md:51; row-major a,b as PAPER.md:133);
+ *      A       [V_phys][4 mu] real fp64;
+ *      clover  [V][2 chirality][36] real fp64: 6 diagonal reals, then (re,im) of the 15
+ *              strictly-upper-triangular entries in row-major order;
+ *      even-sublattice fields [V/2][4][3]: the even sites (sum of coordinates even,
+ *              PAPER.md:97) in increasing Lambda order.
+ *  - Packed order is the library's device layout: even-odd,
+ *    tiled, structure-of-arrays in 16-byte chunks.  Packed buffers are opaque; their sizes
+ *    come from qxd_packed_spinor_bytes.
+ * ===================================================================================== */
+#ifndef QXD_H
+#define QXD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qxd_ctx qxd_ctx; /* opaque, host-side; holds borrowed device pointers only */
+
+typedef enum {
+  QXD_OK = 0,
+  QXD_EINVAL = -1,     /* bad argument (odd extent, extent < 2, null pointer, unknown enum ...) */
+  QXD_ESTATE = -2,     /* call out of order (e.g. apply before clover_build)                    */
+  QXD_EWORKSPACE = -3, /* workspace missing, misaligned or too small                            */
+  QXD_ECUDA = -4,      /* a CUDA runtime call or kernel launch failed                            */
+  QXD_ENOCONV = -5     /* solver hit maxiter or broke down; psi and info still hold the best iterate */
+} qxd_status;
+
+typedef enum { QXD_F64 = 0, QXD_F32 = 1, QXD_F16 = 2 } qxd_prec;
+#define QXD_PREC_MASK(p) (1 << (p))
+
+typedef enum { QXD_CGNE = 0, QXD_BICGSTAB = 1 } qxd_algo;
+
+/* Solver controls (in) and report (out).  Zero-initialise for defaults. */
+typedef struct {
+  /* in */
+  int algo;          /* qxd_algo; CG on the normal equations of D-hat, or BiCGstab on D-hat       */
+  int sloppy;        /* qxd_prec of the inner iteration; QXD_F64 = plain double-precision solver   */
+  double delta;      /* reliable-update threshold: true residual recomputed in fp64 whenever the
+                        iterated residual has dropped below delta * (max since last update);
+                        0 -> default 0.1 (ref [4])                                    */
+  int maxiter;       /* 0 -> 10000                                                                  */
+  /* out */
+  int iters;         /* inner iterations done                                                       */
+  int n_reliable;    /* reliable updates done                                                       */
+  double true_res;   /* final fp64 ||eta-hat_e - D-hat psi_e|| / ||eta||  (= ||eta - D_w psi||/||eta||) */
+  double seconds;    /* wall time of the call measured with CUDA events on the bound stream         */
+} qxd_solve_info;
+
+/* ---- geometry --------------------------------
+ * T,L1,L2,L3: PHYSICAL extents, all even and >= 2.  bc = cstar | (antiperiodic_time << 2), with
+ * cstar in 0..3 = number of spatial directions 1..cstar with C* boundary conditions (direction 1
+ * is doubled when cstar > 0; directions 2..cstar wrap with the shift x1 -> x1 + L1 mod 2 L1).
+ * All site indices are computed on the fly by pure inlined functions. */
+int qxd_geometry_create(int T, int L1, int L2, int L3, int bc, qxd_ctx** out);
+int qxd_geometry_destroy(qxd_ctx* ctx);
+/* Optional: tile extents of the device site order (powers of two dividing the extended extents,
+ * b3 >= 2).  Must precede qxd_workspace_bind.  Default: chosen by the library. */
+int qxd_set_tile(qxd_ctx* ctx, int b0, int b1, int b2, int b3);
+/* Number of sites of the extended lattice (V). */
+long qxd_volume(const qxd_ctx* ctx);
+
+/* ---- workspace and stream --------------------------------------------------------------------
+ * prec_mask: OR of QXD_PREC_MASK(p) for every precision that will be used (QXD_F64 is always
+ * included).  nrhs >= 1: right-hand sides of qxd_solve_multi.  The buffer must be 256-byte aligned
+ * DEVICE memory and stay alive until qxd_geometry_destroy. */
+size_t qxd_workspace_bytes(const qxd_ctx* ctx, int prec_mask, int nrhs);
+int qxd_workspace_bind(qxd_ctx* ctx, void* dev /*DEVICE*/, size_t bytes, int prec_mask, int nrhs);
+int qxd_set_stream(qxd_ctx* ctx, void* cuda_stream /* cudaStream_t, e.g. torch stream .cuda_stream */);
+
+/* ---- gauge field (row a2) -------------------------------------------------
+ * U_su3: DEVICE, natural order on the physical lattice; A_u1: DEVICE or NULL (QCD only);
+ * qel: elementary charge unit of the compact U(1) clover term (reading R5), ignored if A_u1 NULL.
+ * The library builds the mirror half (U^*, -A) itself. */
+int qxd_gauge_load(qxd_ctx* ctx, const double* U_su3, const double* A_u1, double qel);
+/* Quark parameters (reading R6): m0 = 1/(2 kappa) - 4, charge q in the hop phase e^{i q A}.
+ * Builds the hopping links W = e^{iqA} U (time-boundary sign folded in) in every bound precision. */
+int qxd_set_quark(qxd_ctx* ctx, double kappa, double q);
+
+/* ---- clover term (row a3) -----------------------------------------
+ * Builds M(x) = (4+m0) + c_sw (i/4) sigma.F-hat + q c_sw_qed (i/4) sigma.A-hat as two Hermitian
+ * 6x6 blocks per site and inverts both blocks, on the device.  Needs gauge + quark. */
+int qxd_clover_build(qxd_ctx* ctx, double csw, double csw_qed);
+/* Copy the fp64 clover field (inverse != 0: the block inverses) to natural order, out: DEVICE
+ * [V][2][36] doubles, packing of PAPER.md:117. */
+int qxd_clover_export(qxd_ctx* ctx, double* out, int inverse);
+
+/* ---- operator applications, natural order (rows a4, a5) -----------------------------------------
+ * psi/out: DEVICE fp64 natural-order spinors on the extended lattice; prec selects the storage
+ * precision of the fields the kernel streams (fp64 arithmetic for QXD_F64, fp32 otherwise). */
+int qxd_apply_Dw(qxd_ctx* ctx, int prec, const double* psi, double* out);
+/* D-hat = A_ee - D_eo A_oo^{-1} D_oe on the even sublattice; dagger != 0 applies D-hat^dagger. */
+int qxd_apply_Dhat_eo(qxd_ctx* ctx, int prec, const double* psi_e, double* out_e, int dagger);
+/* Same as qxd_apply_Dw but psi/out are HOST arrays: H2D copy, pack, apply, unpack, D2H copy. */
+int qxd_apply_Dw_host(qxd_ctx* ctx, int prec, const double* psi_host, double* out_host);
+
+/* ---- solver (rows a7, a8) --------------------------------------------------------
+ * Solves D_w psi = eta to ||eta - D_w psi|| <= tol ||eta|| (checked in fp64 on the even-odd system).
+ * eta, psi: DEVICE natural order (qxd_solve) or HOST (qxd_solve_host).  info may be NULL (defaults).
+ * On QXD_ENOCONV psi holds the best iterate and info->true_res its residual. */
+int qxd_solve(qxd_ctx* ctx, const double* eta, double* psi, double tol, qxd_solve_info* info);
+int qxd_solve_host(qxd_ctx* ctx, const double* eta_host, double* psi_host, double tol, qxd_solve_info* info);
+
+/* ---- packed-layout entry points (row a9; benchmark and building blocks) ---------------------------
+ * Packed spinors: parity 0 (even) half followed by the parity 1 half; `half_only` != 0 gives the size
+ * of one parity.  For QXD_F16 each half is 24 binary16 per site plus one fp32 scale per site. */
+size_t qxd_packed_spinor_bytes(const qxd_ctx* ctx, int prec, int half_only);
+int qxd_spinor_pack(qxd_ctx* ctx, int prec, const double* nat /*DEVICE [V][4][3]*/, void* packed /*DEVICE*/);
+int qxd_spinor_unpack(qxd_ctx* ctx, int prec, const void* packed, double* nat);
+int qxd_apply_Dw_packed(qxd_ctx* ctx, int prec, const void* in, void* out);
+int qxd_apply_Dhat_packed(qxd_ctx* ctx, int prec, const void* in_e, void* out_e, int dagger);
+
+/* ---- BLAS-1 on packed half-lattice spinors (row a6) ---------------------------------------------
+ * y <- a*x + y ;  returns <x,y> = sum conj(x) y  and  |x|^2 (fp64 accumulation, HOST results). */
+int qxd_blas_axpy(qxd_ctx* ctx, int prec, double a, const void* x, void* y);
+int qxd_blas_cdot(qxd_ctx* ctx, int prec, const void* x, const void* y, double* re_im /*HOST [2]*/);
+int qxd_blas_norm2(qxd_ctx* ctx, int prec, const void* x, double* out /*HOST*/);
+
+/* Number of kernel launches issued by this context so far (bench.py's gpu_launches). */
+long qxd_launch_count(const qxd_ctx* ctx);
+const char* qxd_last_error(const qxd_ctx* ctx);
+const char* qxd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QXD_H */

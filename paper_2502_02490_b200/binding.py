@@ -1,0 +1,268 @@
+"""ctypes binding of include/qxd.h -- same names, argument marshalling only.
+
+Every method of :class:`Qxd` forwards to the C entry point of the same name
+(``Qxd.gauge_load`` -> ``qxd_gauge_load`` ...).  Tensors are torch CUDA tensors (or pinned /
+pageable host tensors for the ``*_host`` calls); the library borrows their memory.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+QXD_F64, QXD_F32, QXD_F16 = 0, 1, 2
+QXD_CGNE, QXD_BICGSTAB = 0, 1
+QXD_OK, QXD_EINVAL, QXD_ESTATE, QXD_EWORKSPACE, QXD_ECUDA, QXD_ENOCONV = 0, -1, -2, -3, -4, -5
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+
+class QxdError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"qxd status {status}: {msg}")
+        self.status = status
+
+
+class SolveInfo(C.Structure):
+    _fields_ = [("algo", C.c_int), ("sloppy", C.c_int), ("delta", C.c_double), ("maxiter", C.c_int),
+                ("iters", C.c_int), ("n_reliable", C.c_int), ("true_res", C.c_double), ("seconds", C.c_double)]
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "libqxd.so")
+
+
+# every symbol include/qxd.h declares: name -> (restype, argtypes)
+_vp, _i, _d, _l, _sz = C.c_void_p, C.c_int, C.c_double, C.c_long, C.c_size_t
+SYMBOLS = {
+    "qxd_geometry_create": (_i, [_i, _i, _i, _i, _i, C.POINTER(_vp)]),
+    "qxd_geometry_destroy": (_i, [_vp]),
+    "qxd_set_tile": (_i, [_vp, _i, _i, _i, _i]),
+    "qxd_volume": (_l, [_vp]),
+    "qxd_workspace_bytes": (_sz, [_vp, _i, _i]),
+    "qxd_workspace_bind": (_i, [_vp, _vp, _sz, _i, _i]),
+    "qxd_set_stream": (_i, [_vp, _vp]),
+    "qxd_gauge_load": (_i, [_vp, _vp, _vp, _d]),
+    "qxd_set_quark": (_i, [_vp, _d, _d]),
+    "qxd_clover_build": (_i, [_vp, _d, _d]),
+    "qxd_clover_export": (_i, [_vp, _vp, _i]),
+    "qxd_apply_Dw": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_apply_Dhat_eo": (_i, [_vp, _i, _vp, _vp, _i]),
+    "qxd_apply_Dw_host": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_solve": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
+    "qxd_solve_host": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
+    "qxd_packed_spinor_bytes": (_sz, [_vp, _i, _i]),
+    "qxd_spinor_pack": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_spinor_unpack": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_apply_Dw_packed": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_apply_Dhat_packed": (_i, [_vp, _i, _vp, _vp, _i]),
+    "qxd_blas_axpy": (_i, [_vp, _i, _d, _vp, _vp]),
+    "qxd_blas_cdot": (_i, [_vp, _i, _vp, _vp, _vp]),
+    "qxd_blas_norm2": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_launch_count": (_l, [_vp]),
+    "qxd_last_error": (C.c_char_p, [_vp]),
+    "qxd_version": (C.c_char_p, []),
+}
+
+
+def load_library():
+    """dlopen the in-tree libqxd.so (built by paper_2502_02490_b200/build.py).  Fails loudly if missing."""
+    global _LIB
+    if _LIB is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise QxdError(QXD_ESTATE, f"{path} not built: run `python -m paper_2502_02490_b200.build` "
+                                       "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = C.CDLL(path)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _LIB = lib
+    return _LIB
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+class Qxd:
+    """One solver context (qxd_ctx): geometry, workspace, gauge field, quark, clover term."""
+
+    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise QxdError(QXD_ECUDA, "no CUDA device: the qxd hot path has no CPU fallback")
+        self.torch = torch
+        self.lib = load_library()
+        self.device = torch.device(device)
+        h = C.c_void_p()
+        rc = self.lib.qxd_geometry_create(T, L1, L2, L3, bc, C.byref(h))
+        if rc != QXD_OK:
+            raise QxdError(rc, "qxd_geometry_create: invalid geometry")
+        self.h = h
+        self.dims = (T, L1, L2, L3)
+        self.cstar = bc & 3
+        self.dims_ext = (T, 2 * L1 if self.cstar else L1, L2, L3)
+        self.V = self.lib.qxd_volume(self.h)
+        if tile is not None:
+            self._chk(self.lib.qxd_set_tile(self.h, *tile))
+        self.prec_mask = 0
+        for p in precisions:
+            self.prec_mask |= 1 << p
+        self.prec_mask |= 1
+        nbytes = self.lib.qxd_workspace_bytes(self.h, self.prec_mask, nrhs)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            off = (-self.workspace.data_ptr()) % 256
+            self._chk(self.lib.qxd_set_stream(self.h, C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+            self._chk(self.lib.qxd_workspace_bind(self.h, C.c_void_p(self.workspace.data_ptr() + off), nbytes, self.prec_mask, nrhs))
+        self._keep = []
+
+    # -- plumbing ------------------------------------------------------------------------------
+    def _chk(self, rc, allow=()):
+        if rc != QXD_OK and rc not in allow:
+            raise QxdError(rc, self.lib.qxd_last_error(self.h).decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.torch.cuda.synchronize(self.device)
+            self.lib.qxd_geometry_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev(self, a, dtype=None):
+        torch = self.torch
+        t = torch.as_tensor(a)
+        if dtype is not None and t.dtype != dtype:
+            t = t.to(dtype)
+        return t.to(self.device).contiguous()
+
+    def set_stream(self, stream=None):
+        s = stream if stream is not None else self.torch.cuda.current_stream()
+        self._chk(self.lib.qxd_set_stream(self.h, C.c_void_p(s.cuda_stream)))
+
+    def launch_count(self):
+        return self.lib.qxd_launch_count(self.h)
+
+    # -- setup ---------------------------------------------------------------------------------
+    def gauge_load(self, U_su3, A_u1=None, qel=1.0):
+        torch = self.torch
+        U = self._dev(U_su3, torch.complex128)
+        assert tuple(U.shape) == self.dims + (4, 3, 3), U.shape
+        A = None
+        if A_u1 is not None:
+            A = self._dev(A_u1, torch.float64)
+            assert tuple(A.shape) == self.dims + (4,), A.shape
+        self._chk(self.lib.qxd_gauge_load(self.h, _ptr(U), _ptr(A), float(qel)))
+        torch.cuda.synchronize(self.device)  # inputs may be freed after return
+
+    def set_quark(self, kappa, q=0.0):
+        self._chk(self.lib.qxd_set_quark(self.h, float(kappa), float(q)))
+
+    def clover_build(self, csw, csw_qed=0.0):
+        self._chk(self.lib.qxd_clover_build(self.h, float(csw), float(csw_qed)))
+
+    def clover_export(self, inverse=False):
+        out = self.torch.empty((self.V, 2, 36), dtype=self.torch.float64, device=self.device)
+        self._chk(self.lib.qxd_clover_export(self.h, _ptr(out), int(inverse)))
+        return out
+
+    # -- natural-order operator applications -----------------------------------------------------
+    def apply_Dw(self, psi, prec=QXD_F64, out=None):
+        torch = self.torch
+        psi = self._dev(psi, torch.complex128)
+        assert psi.numel() == self.V * 12
+        if out is None:
+            out = torch.empty_like(psi)
+        self._chk(self.lib.qxd_apply_Dw(self.h, prec, _ptr(psi), _ptr(out)))
+        return out
+
+    def apply_Dhat_eo(self, psi_e, prec=QXD_F64, dagger=False):
+        torch = self.torch
+        psi_e = self._dev(psi_e, torch.complex128)
+        assert psi_e.numel() == self.V * 6
+        out = torch.empty_like(psi_e)
+        self._chk(self.lib.qxd_apply_Dhat_eo(self.h, prec, _ptr(psi_e), _ptr(out), int(dagger)))
+        return out
+
+    def apply_Dw_host(self, psi_host, out_host, prec=QXD_F64):
+        """psi_host/out_host: CPU complex128 tensors (pinned for best throughput)."""
+        assert psi_host.device.type == "cpu" and out_host.device.type == "cpu"
+        self._chk(self.lib.qxd_apply_Dw_host(self.h, prec, _ptr(psi_host), _ptr(out_host)))
+        return out_host
+
+    # -- solver ------------------------------------------------------------------------------------
+    def _info(self, algo, sloppy, delta, maxiter):
+        info = SolveInfo()
+        info.algo, info.sloppy, info.delta, info.maxiter = algo, sloppy, delta, maxiter
+        return info
+
+    @staticmethod
+    def _report(rc, info):
+        return dict(status=rc, iters=info.iters, n_reliable=info.n_reliable, true_res=info.true_res, seconds=info.seconds)
+
+    def solve(self, eta, tol, algo=QXD_CGNE, sloppy=QXD_F64, delta=0.0, maxiter=0, psi=None):
+        torch = self.torch
+        eta = self._dev(eta, torch.complex128)
+        assert eta.numel() == self.V * 12
+        if psi is None:
+            psi = torch.empty_like(eta)
+        info = self._info(algo, sloppy, delta, maxiter)
+        rc = self._chk(self.lib.qxd_solve(self.h, _ptr(eta), _ptr(psi), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
+        return psi, self._report(rc, info)
+
+    def solve_host(self, eta_host, psi_host, tol, algo=QXD_CGNE, sloppy=QXD_F64, delta=0.0, maxiter=0):
+        assert eta_host.device.type == "cpu" and psi_host.device.type == "cpu"
+        info = self._info(algo, sloppy, delta, maxiter)
+        rc = self._chk(self.lib.qxd_solve_host(self.h, _ptr(eta_host), _ptr(psi_host), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
+        return psi_host, self._report(rc, info)
+
+    # -- packed layout -------------------------------------------------------------------------------
+    def packed_spinor_bytes(self, prec, half_only=False):
+        return self.lib.qxd_packed_spinor_bytes(self.h, prec, int(half_only))
+
+    def new_packed(self, prec, half_only=False):
+        return self.torch.zeros(self.packed_spinor_bytes(prec, half_only), dtype=self.torch.uint8, device=self.device)
+
+    def spinor_pack(self, nat, prec, packed=None):
+        nat = self._dev(nat, self.torch.complex128)
+        if packed is None:
+            packed = self.new_packed(prec)
+        self._chk(self.lib.qxd_spinor_pack(self.h, prec, _ptr(nat), _ptr(packed)))
+        return packed
+
+    def spinor_unpack(self, packed, prec):
+        out = self.torch.empty(self.dims_ext + (4, 3), dtype=self.torch.complex128, device=self.device)
+        self._chk(self.lib.qxd_spinor_unpack(self.h, prec, _ptr(packed), _ptr(out)))
+        return out
+
+    def apply_Dw_packed(self, pin, pout, prec):
+        self._chk(self.lib.qxd_apply_Dw_packed(self.h, prec, _ptr(pin), _ptr(pout)))
+        return pout
+
+    def apply_Dhat_packed(self, pin_e, pout_e, prec, dagger=False):
+        self._chk(self.lib.qxd_apply_Dhat_packed(self.h, prec, _ptr(pin_e), _ptr(pout_e), int(dagger)))
+        return pout_e
+
+    # -- BLAS-1 on packed half-lattice spinors ---------------------------------------------------------
+    def blas_axpy(self, a, x, y, prec):
+        self._chk(self.lib.qxd_blas_axpy(self.h, prec, float(a), _ptr(x), _ptr(y)))
+        return y
+
+    def blas_cdot(self, x, y, prec):
+        out = (C.c_double * 2)()
+        self._chk(self.lib.qxd_blas_cdot(self.h, prec, _ptr(x), _ptr(y), C.cast(out, C.c_void_p)))
+        return complex(out[0], out[1])
+
+    def blas_norm2(self, x, prec):
+        out = C.c_double(0.0)
+        self._chk(self.lib.qxd_blas_norm2(self.h, prec, _ptr(x), C.cast(C.byref(out), C.c_void_p)))
+        return out.value

@@ -1,0 +1,307 @@
+// api.cu -- the C-ABI entry points declared in include/qxd.h.  Argument checking,
+// workspace carving and call sequencing only; every step of the path runs in the kernels of this library.
+#include "qxd_ctx.h"
+#include <new>
+#include <cstring>
+
+using namespace qxd;
+
+namespace qxd {
+int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out_e, const SpinorPtr& tmp_o, int dagger, double* norm_slot);
+}
+
+namespace {
+
+int pow2_le_dividing(int extent, int target) {
+  int b = 1;
+  while (b * 2 <= target && extent % (b * 2) == 0) b *= 2;
+  return b;
+}
+int ilog2(int v) { int s = 0; while ((1 << s) < v) s++; return s; }
+
+int set_tile(qxd_ctx* c, const int b[4]) {
+  Geom& g = c->g;
+  for (int mu = 0; mu < 4; mu++) {
+    if (b[mu] < 1 || (b[mu] & (b[mu] - 1)) || g.X[mu] % b[mu]) return fail(c, QXD_EINVAL, "tile extents must be powers of two dividing the extended extents");
+  }
+  if (b[3] < 2) return fail(c, QXD_EINVAL, "tile extent b3 must be >= 2");
+  for (int mu = 0; mu < 4; mu++) { g.sh[mu] = ilog2(b[mu]); g.nt[mu] = g.X[mu] / b[mu]; }
+  g.lo_str[3] = 1; g.lo_str[2] = b[3]; g.lo_str[1] = b[3] * b[2]; g.lo_str[0] = b[3] * b[2] * b[1];
+  const int tv = b[0] * b[1] * b[2] * b[3];
+  g.hi_str[3] = tv; g.hi_str[2] = tv * g.nt[3]; g.hi_str[1] = tv * g.nt[3] * g.nt[2]; g.hi_str[0] = tv * g.nt[3] * g.nt[2] * g.nt[1];
+  return QXD_OK;
+}
+
+struct Carver {
+  size_t off = 0;
+  char* base;
+  explicit Carver(char* b) : base(b) {}
+  void* take(size_t bytes) {
+    void* p = base ? base + off : nullptr;
+    off += (bytes + 255) & ~size_t(255);
+    return p;
+  }
+};
+
+// One layout routine serves both the size query (base == nullptr) and the binding.
+size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
+  (void)nrhs;
+  const size_t Vh = c->g.Vh;
+  Carver k(base);
+  void* Ug[2]; void* Ag[2]; void* W[NPREC][2] = {}; void* M[NPREC][2] = {}; void* Mi[NPREC][2] = {};
+  for (int p = 0; p < 2; p++) { Ug[p] = k.take(Vh * 72 * 8); Ag[p] = k.take(Vh * 4 * 8); }
+  for (int pr = 0; pr < NPREC; pr++) {
+    if (!((prec_mask >> pr) & 1)) continue;
+    for (int p = 0; p < 2; p++) { W[pr][p] = k.take(Vh * 72 * prec_size(pr)); M[pr][p] = k.take(Vh * 72 * prec_size(pr)); Mi[pr][p] = k.take(Vh * 72 * prec_size(pr)); }
+  }
+  void* sp64[12]; void* splo[8];
+  for (int i = 0; i < 12; i++) sp64[i] = k.take(half_bytes(0, Vh));
+  for (int i = 0; i < 8; i++) splo[i] = k.take(half_bytes(0, Vh));  // sized for the widest sloppy type (fp64 when sloppy == hi)
+  void* fa = k.take(2 * half_bytes(0, Vh));
+  void* fb = k.take(2 * half_bytes(0, Vh));
+  void* na = k.take(size_t(c->V) * 24 * 8);
+  void* nb = k.take(size_t(c->V) * 24 * 8);
+  const int max_blocks = int((Vh + 127) / 128) * 2 + 8;
+  void* partials = k.take(size_t(max_blocks) * 4 * 8);
+  void* ticket = k.take(256);
+  void* scal = k.take(64 * 8);
+  if (assign) {
+    for (int p = 0; p < 2; p++) { c->Ug[p] = Ug[p]; c->Ag[p] = Ag[p]; }
+    for (int pr = 0; pr < NPREC; pr++) for (int p = 0; p < 2; p++) { c->W[pr][p] = W[pr][p]; c->M[pr][p] = M[pr][p]; c->Mi[pr][p] = Mi[pr][p]; }
+    for (int i = 0; i < 12; i++) c->sp64[i] = sp64[i];
+    for (int i = 0; i < 8; i++) c->splo[i] = splo[i];
+    c->full_a = fa; c->full_b = fb; c->nat_a = (double*)na; c->nat_b = (double*)nb;
+    c->partials = (double*)partials; c->ticket = (unsigned*)ticket; c->scal = (double*)scal; c->max_blocks = max_blocks;
+  }
+  return k.off;
+}
+
+bool prec_ok(const qxd_ctx* c, int prec) { return prec >= 0 && prec < NPREC && ((c->prec_mask >> prec) & 1); }
+
+}  // namespace
+
+extern "C" {
+
+const char* qxd_version(void) { return "qxd-b200 0.1 (sm_100a)"; }
+
+int qxd_geometry_create(int T, int L1, int L2, int L3, int bc, qxd_ctx** out) {
+  if (!out) return QXD_EINVAL;
+  *out = nullptr;
+  if (T < 2 || L1 < 2 || L2 < 2 || L3 < 2 || ((T | L1 | L2 | L3) & 1) || bc < 0 || bc > 7) return QXD_EINVAL;
+  const int cstar = bc & 3;
+  const long V = long(T) * (cstar ? 2 * L1 : L1) * L2 * L3;
+  if (V / 2 * 72 > 0x7fffffffL) return QXD_EINVAL;  // chunk indices are 32-bit
+  qxd_ctx* c = new (std::nothrow) qxd_ctx;
+  if (!c) return QXD_EINVAL;
+  c->T = T; c->L1 = L1; c->L2 = L2; c->L3 = L3; c->bc = bc; c->V = V;
+  Geom& g = c->g;
+  g.X[0] = T; g.X[1] = cstar ? 2 * L1 : L1; g.X[2] = L2; g.X[3] = L3;
+  g.L1 = L1; g.cstar = cstar; g.antiper = (bc >> 2) & 1; g.Vh = int(V / 2);
+  int b[4] = {pow2_le_dividing(g.X[0], 4), pow2_le_dividing(g.X[1], 4), pow2_le_dividing(g.X[2], 4), pow2_le_dividing(g.X[3], 8)};
+  set_tile(c, b);
+  *out = c;
+  return QXD_OK;
+}
+
+int qxd_geometry_destroy(qxd_ctx* c) {
+  if (!c) return QXD_EINVAL;
+  if (c->h_scal) cudaFreeHost(c->h_scal);
+  if (c->ev0) cudaEventDestroy(c->ev0);
+  if (c->ev1) cudaEventDestroy(c->ev1);
+  delete c;
+  return QXD_OK;
+}
+
+int qxd_set_tile(qxd_ctx* c, int b0, int b1, int b2, int b3) {
+  if (!c) return QXD_EINVAL;
+  if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_tile must precede qxd_workspace_bind");
+  int b[4] = {b0, b1, b2, b3};
+  return set_tile(c, b);
+}
+
+long qxd_volume(const qxd_ctx* c) { return c ? c->V : 0; }
+
+size_t qxd_workspace_bytes(const qxd_ctx* c, int prec_mask, int nrhs) {
+  if (!c || nrhs < 1) return 0;
+  return carve(const_cast<qxd_ctx*>(c), nullptr, (prec_mask | 1) & 7, nrhs, false);
+}
+
+int qxd_workspace_bind(qxd_ctx* c, void* dev, size_t bytes, int prec_mask, int nrhs) {
+  if (!c || nrhs < 1) return QXD_EINVAL;
+  prec_mask = (prec_mask | 1) & 7;
+  if (!dev || (reinterpret_cast<uintptr_t>(dev) & 255)) return fail(c, QXD_EWORKSPACE, "workspace must be a 256-byte aligned device pointer");
+  const size_t need = carve(c, nullptr, prec_mask, nrhs, false);
+  if (bytes < need) return fail(c, QXD_EWORKSPACE, "workspace too small");
+  c->ws = static_cast<char*>(dev); c->ws_bytes = bytes; c->prec_mask = prec_mask; c->nrhs = nrhs;
+  c->ws_used = carve(c, c->ws, prec_mask, nrhs, true);
+  c->have_gauge = c->have_quark = c->have_clover = false;
+  if (!c->h_scal) QXD_CUDA_OK(c, cudaMallocHost((void**)&c->h_scal, 64 * sizeof(double)));
+  if (!c->ev0) QXD_CUDA_OK(c, cudaEventCreate(&c->ev0));
+  if (!c->ev1) QXD_CUDA_OK(c, cudaEventCreate(&c->ev1));
+  QXD_CUDA_OK(c, cudaMemsetAsync(c->ticket, 0, 256, c->stream));
+  QXD_CUDA_OK(c, cudaMemsetAsync(c->scal, 0, 64 * 8, c->stream));
+  return QXD_OK;
+}
+
+int qxd_set_stream(qxd_ctx* c, void* s) {
+  if (!c) return QXD_EINVAL;
+  c->stream = static_cast<cudaStream_t>(s);
+  return QXD_OK;
+}
+
+int qxd_gauge_load(qxd_ctx* c, const double* U, const double* A, double qel) {
+  if (!c || !U) return c ? fail(c, QXD_EINVAL, "gauge_load: U_su3 is null") : QXD_EINVAL;
+  if (!c->ws) return fail(c, QXD_EWORKSPACE, "gauge_load: no workspace bound");
+  if (A && !(qel != 0.0)) return fail(c, QXD_EINVAL, "gauge_load: qel must be non-zero");
+  c->qel = A ? qel : 1.0;
+  c->have_qed = (A != nullptr);
+  int rc = launch_gauge_pack(c, U, A);
+  if (rc) return rc;
+  c->have_gauge = true; c->have_quark = false; c->have_clover = false;
+  return QXD_OK;
+}
+
+int qxd_set_quark(qxd_ctx* c, double kappa, double q) {
+  if (!c) return QXD_EINVAL;
+  if (!c->have_gauge) return fail(c, QXD_ESTATE, "set_quark: load a gauge field first");
+  if (!(kappa > 0.0)) return fail(c, QXD_EINVAL, "set_quark: kappa must be > 0");
+  c->kappa = kappa; c->q = q; c->m0 = 1.0 / (2.0 * kappa) - 4.0;
+  for (int pr = 0; pr < NPREC; pr++)
+    if ((c->prec_mask >> pr) & 1) { int rc = launch_hoplinks(c, pr); if (rc) return rc; }
+  c->have_quark = true; c->have_clover = false;
+  return QXD_OK;
+}
+
+int qxd_clover_build(qxd_ctx* c, double csw, double csw_qed) {
+  if (!c) return QXD_EINVAL;
+  if (!c->have_gauge || !c->have_quark) return fail(c, QXD_ESTATE, "clover_build: needs gauge_load and set_quark");
+  c->csw = csw; c->csw_qed = csw_qed;
+  int rc = launch_clover_build(c);
+  if (rc) return rc;
+  c->have_clover = true;
+  return QXD_OK;
+}
+
+int qxd_clover_export(qxd_ctx* c, double* out, int inverse) {
+  if (!c || !out) return QXD_EINVAL;
+  if (!c->have_clover) return fail(c, QXD_ESTATE, "clover_export: build the clover term first");
+  return launch_clover_export(c, out, inverse);
+}
+
+static int check_apply(qxd_ctx* c, int prec, const void* a, const void* b, const char* who) {
+  if (!c) return QXD_EINVAL;
+  if (!a || !b) return fail(c, QXD_EINVAL, std::string(who) + ": null pointer");
+  if (!c->have_clover) return fail(c, QXD_ESTATE, std::string(who) + ": needs gauge_load, set_quark and clover_build");
+  if (!prec_ok(c, prec)) return fail(c, QXD_EINVAL, std::string(who) + ": precision not bound in the workspace");
+  return QXD_OK;
+}
+
+int qxd_apply_Dw_packed(qxd_ctx* c, int prec, const void* in, void* out) {
+  int rc = check_apply(c, prec, in, out, "apply_Dw_packed");
+  if (rc) return rc;
+  const int Vh = c->g.Vh;
+  DslashCall d{};
+  d.prec = prec; d.mode = DS_DW_FULL; d.flags = 0;
+  d.in[0] = half_view(prec, const_cast<void*>(in), Vh, 0); d.in[1] = half_view(prec, const_cast<void*>(in), Vh, 1);
+  d.out[0] = half_view(prec, out, Vh, 0); d.out[1] = half_view(prec, out, Vh, 1);
+  return launch_dslash(c, d);
+}
+
+int qxd_apply_Dhat_packed(qxd_ctx* c, int prec, const void* in_e, void* out_e, int dagger) {
+  int rc = check_apply(c, prec, in_e, out_e, "apply_Dhat_packed");
+  if (rc) return rc;
+  const int Vh = c->g.Vh;
+  return apply_dhat(c, prec, half_view(prec, const_cast<void*>(in_e), Vh, 0), half_view(prec, out_e, Vh, 0), half_view(prec, c->sp64[11], Vh, 0), dagger,
+                    nullptr);
+}
+
+int qxd_apply_Dw(qxd_ctx* c, int prec, const double* psi, double* out) {
+  int rc = check_apply(c, prec, psi, out, "apply_Dw");
+  if (rc) return rc;
+  if ((rc = launch_spinor_pack(c, prec, psi, c->full_a, 3, 0))) return rc;
+  if ((rc = qxd_apply_Dw_packed(c, prec, c->full_a, c->full_b))) return rc;
+  return launch_spinor_unpack(c, prec, c->full_b, out, 3, 0);
+}
+
+int qxd_apply_Dhat_eo(qxd_ctx* c, int prec, const double* psi_e, double* out_e, int dagger) {
+  int rc = check_apply(c, prec, psi_e, out_e, "apply_Dhat_eo");
+  if (rc) return rc;
+  if ((rc = launch_spinor_pack(c, prec, psi_e, c->full_a, 1, 1))) return rc;
+  if ((rc = qxd_apply_Dhat_packed(c, prec, c->full_a, c->full_b, dagger))) return rc;
+  return launch_spinor_unpack(c, prec, c->full_b, out_e, 1, 1);
+}
+
+int qxd_apply_Dw_host(qxd_ctx* c, int prec, const double* psi_host, double* out_host) {
+  int rc = check_apply(c, prec, psi_host, out_host, "apply_Dw_host");
+  if (rc) return rc;
+  const size_t bytes = size_t(c->V) * 24 * sizeof(double);
+  QXD_CUDA_OK(c, cudaMemcpyAsync(c->nat_a, psi_host, bytes, cudaMemcpyHostToDevice, c->stream));
+  if ((rc = qxd_apply_Dw(c, prec, c->nat_a, c->nat_b))) return rc;
+  QXD_CUDA_OK(c, cudaMemcpyAsync(out_host, c->nat_b, bytes, cudaMemcpyDeviceToHost, c->stream));
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  return QXD_OK;
+}
+
+int qxd_solve(qxd_ctx* c, const double* eta, double* psi, double tol, qxd_solve_info* info) {
+  qxd_solve_info local;
+  if (!info) { std::memset(&local, 0, sizeof(local)); info = &local; }
+  int rc = check_apply(c, info->sloppy, eta, psi, "solve");
+  if (rc) return rc;
+  if (info->algo != QXD_CGNE && info->algo != QXD_BICGSTAB) return fail(c, QXD_EINVAL, "solve: unknown algorithm");
+  return solve_eo(c, eta, psi, tol, info);
+}
+
+int qxd_solve_host(qxd_ctx* c, const double* eta_host, double* psi_host, double tol, qxd_solve_info* info) {
+  if (!c || !eta_host || !psi_host) return c ? fail(c, QXD_EINVAL, "solve_host: null pointer") : QXD_EINVAL;
+  if (!c->ws) return fail(c, QXD_EWORKSPACE, "solve_host: no workspace bound");
+  const size_t bytes = size_t(c->V) * 24 * sizeof(double);
+  QXD_CUDA_OK(c, cudaMemcpyAsync(c->nat_a, eta_host, bytes, cudaMemcpyHostToDevice, c->stream));
+  int rc = qxd_solve(c, c->nat_a, c->nat_b, tol, info);
+  if (rc != QXD_OK && rc != QXD_ENOCONV) return rc;
+  QXD_CUDA_OK(c, cudaMemcpyAsync(psi_host, c->nat_b, bytes, cudaMemcpyDeviceToHost, c->stream));
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  return rc;
+}
+
+size_t qxd_packed_spinor_bytes(const qxd_ctx* c, int prec, int half_only) {
+  if (!c || prec < 0 || prec >= NPREC) return 0;
+  return half_bytes(prec, c->g.Vh) * (half_only ? 1 : 2);
+}
+
+int qxd_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed) {
+  if (!c || !nat || !packed || prec < 0 || prec >= NPREC) return QXD_EINVAL;
+  return launch_spinor_pack(c, prec, nat, packed, 3, 0);
+}
+int qxd_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat) {
+  if (!c || !nat || !packed || prec < 0 || prec >= NPREC) return QXD_EINVAL;
+  return launch_spinor_unpack(c, prec, packed, nat, 3, 0);
+}
+
+static int read_result(qxd_ctx* c, int n, double* out) {
+  QXD_CUDA_OK(c, cudaMemcpyAsync(c->h_scal + 32, c->scal + 32, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < n; i++) out[i] = c->h_scal[32 + i];
+  return QXD_OK;
+}
+
+int qxd_blas_axpy(qxd_ctx* c, int prec, double a, const void* x, void* y) {
+  if (!c || !x || !y || prec < 0 || prec >= NPREC || !c->ws) return QXD_EINVAL;
+  return blas_axpy(c, prec, a, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), half_view(prec, y, c->g.Vh, 0));
+}
+int qxd_blas_cdot(qxd_ctx* c, int prec, const void* x, const void* y, double* re_im) {
+  if (!c || !x || !y || !re_im || prec < 0 || prec >= NPREC || !c->ws) return QXD_EINVAL;
+  int rc = blas_cdot(c, prec, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), half_view(prec, const_cast<void*>(y), c->g.Vh, 0), c->scal + 32);
+  if (rc) return rc;
+  return read_result(c, 2, re_im);
+}
+int qxd_blas_norm2(qxd_ctx* c, int prec, const void* x, double* out) {
+  if (!c || !x || !out || prec < 0 || prec >= NPREC || !c->ws) return QXD_EINVAL;
+  int rc = blas_norm2(c, prec, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), c->scal + 32);
+  if (rc) return rc;
+  return read_result(c, 1, out);
+}
+
+long qxd_launch_count(const qxd_ctx* c) { return c ? c->launches : 0; }
+const char* qxd_last_error(const qxd_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+}  // extern "C"

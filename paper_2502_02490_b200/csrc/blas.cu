@@ -1,0 +1,236 @@
+// blas.cu -- SURVEY.md §8 row a6: BLAS-1 on packed half-lattice spinors (axpy, xpay, complex dot, norm^2
+// and the fused forms the solvers use).  The paper does not describe these kernels; any Krylov solver for
+// D_w psi = eta needs them.  One thread per site (24 reals = 12/6/3 16-byte chunks,
+// coalesced across the warp), fp64 accumulators for every storage precision, warp-shuffle -> block ->
+// single-pass grid reduction (qxd_common.cuh).  Solver scalars (alpha, beta, ...) stay on the device: the
+// kernels read numerator/denominator from device memory, so the inner loop needs no host round trip.
+#include "qxd_ctx.h"
+
+namespace qxd {
+
+namespace {
+
+template <typename S>
+__global__ void __launch_bounds__(128) axpy_k(int Vh, double a, SpinorPtr x, SpinorPtr y) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  C vx[24], vy[24];
+  load_spinor<S>(x, Vh, cb, vx);
+  load_spinor<S>(y, Vh, cb, vy);
+#pragma unroll
+  for (int i = 0; i < 24; i++) vy[i] += (C)a * vx[i];
+  store_spinor<S>(y, Vh, cb, vy);
+}
+
+// z = x + a*y + b*w, complex scalars by value (HASW = false: no w term)
+template <typename S, bool HASW>
+__global__ void __launch_bounds__(128) cxpaypbw_k(int Vh, SpinorPtr x, double ar_, double ai_, SpinorPtr y, double br_, double bi_, SpinorPtr w,
+                                                  SpinorPtr z) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  const C ar = (C)ar_, ai = (C)ai_, br = (C)br_, bi = (C)bi_;
+  C vx[24], vy[24];
+  load_spinor<S>(x, Vh, cb, vx);
+  load_spinor<S>(y, Vh, cb, vy);
+#pragma unroll
+  for (int k = 0; k < 12; k++) {
+    C yr = vy[2 * k], yi = vy[2 * k + 1];
+    vx[2 * k] += ar * yr - ai * yi;
+    vx[2 * k + 1] += ar * yi + ai * yr;
+  }
+  if (HASW) {
+    load_spinor<S>(w, Vh, cb, vy);
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      C yr = vy[2 * k], yi = vy[2 * k + 1];
+      vx[2 * k] += br * yr - bi * yi;
+      vx[2 * k + 1] += br * yi + bi * yr;
+    }
+  }
+  store_spinor<S>(z, Vh, cb, vx);
+}
+
+// CG on the normal equations, step 1:  alpha = num/den ;  x += alpha p ;  r -= alpha t ;  result = |r|^2
+template <typename S>
+__global__ void __launch_bounds__(128) cg_xr_k(int Vh, const double* num, const double* den, SpinorPtr p, SpinorPtr t, SpinorPtr x,
+                                               SpinorPtr r, Reducer R) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  double nrm[1] = {0.0};
+  if (cb < Vh) {
+    const C al = (C)(*num / *den);
+    C vp[24], vx[24];
+    load_spinor<S>(p, Vh, cb, vp);
+    load_spinor<S>(x, Vh, cb, vx);
+#pragma unroll
+    for (int i = 0; i < 24; i++) vx[i] += al * vp[i];
+    store_spinor<S>(x, Vh, cb, vx);
+    load_spinor<S>(t, Vh, cb, vp);
+    load_spinor<S>(r, Vh, cb, vx);
+#pragma unroll
+    for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; nrm[0] += (double)vx[i] * (double)vx[i]; }
+    store_spinor<S>(r, Vh, cb, vx);
+  }
+  grid_reduce<1>(nrm, R);
+}
+// step 2:  beta = num/den ;  p = s + beta p
+template <typename S>
+__global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const double* den, SpinorPtr s, SpinorPtr p) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  const C be = (C)(*num / *den);
+  C vs[24], vp[24];
+  load_spinor<S>(s, Vh, cb, vs);
+  load_spinor<S>(p, Vh, cb, vp);
+#pragma unroll
+  for (int i = 0; i < 24; i++) vp[i] = vs[i] + be * vp[i];
+  store_spinor<S>(p, Vh, cb, vp);
+}
+
+template <typename S>
+__global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  double nrm[1] = {0.0};
+  if (cb < Vh) {
+    C v[24];
+    load_spinor<S>(x, Vh, cb, v);
+#pragma unroll
+    for (int i = 0; i < 24; i++) nrm[0] += (double)v[i] * (double)v[i];
+  }
+  grid_reduce<1>(nrm, R);
+}
+// <x,y> = sum conj(x) y  (re, im) and |y|^2 as a third component
+template <typename S>
+__global__ void __launch_bounds__(128) cdot_k(int Vh, SpinorPtr x, SpinorPtr y, Reducer R) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  double d[3] = {0.0, 0.0, 0.0};
+  if (cb < Vh) {
+    C vx[24], vy[24];
+    load_spinor<S>(x, Vh, cb, vx);
+    load_spinor<S>(y, Vh, cb, vy);
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      double xr = vx[2 * k], xi = vx[2 * k + 1], yr = vy[2 * k], yi = vy[2 * k + 1];
+      d[0] += xr * yr + xi * yi;
+      d[1] += xr * yi - xi * yr;
+      d[2] += yr * yr + yi * yi;
+    }
+  }
+  grid_reduce<3>(d, R);
+}
+
+template <typename S>
+__global__ void __launch_bounds__(128) zero_k(int Vh, SpinorPtr x) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  C v[24];
+#pragma unroll
+  for (int i = 0; i < 24; i++) v[i] = 0;
+  store_spinor<S>(x, Vh, cb, v);
+}
+// reliable update, solution part: x_hi (fp64) += x_lo (S) ; x_lo = 0
+template <typename S>
+__global__ void __launch_bounds__(128) acc_hi_k(int Vh, SpinorPtr xlo, SpinorPtr xhi) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  C v[24];
+  double h[24];
+  load_spinor<S>(xlo, Vh, cb, v);
+  load_spinor<double>(xhi, Vh, cb, h);
+#pragma unroll
+  for (int i = 0; i < 24; i++) { h[i] += (double)v[i]; v[i] = 0; }
+  store_spinor<double>(xhi, Vh, cb, h);
+  store_spinor<S>(xlo, Vh, cb, v);
+}
+// r = b - t ; result = |r|^2
+template <typename S>
+__global__ void __launch_bounds__(128) sub_norm_k(int Vh, SpinorPtr b, SpinorPtr t, SpinorPtr r, Reducer R) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  double nrm[1] = {0.0};
+  if (cb < Vh) {
+    C vb[24], vt[24];
+    load_spinor<S>(b, Vh, cb, vb);
+    load_spinor<S>(t, Vh, cb, vt);
+#pragma unroll
+    for (int i = 0; i < 24; i++) { vb[i] -= vt[i]; nrm[0] += (double)vb[i] * (double)vb[i]; }
+    store_spinor<S>(r, Vh, cb, vb);
+  }
+  grid_reduce<1>(nrm, R);
+}
+
+inline Reducer reducer(qxd_ctx* c, double* result) {
+  Reducer R;
+  R.partials = c->partials; R.ticket = c->ticket; R.result = result;
+  return R;
+}
+
+}  // namespace
+
+#define QXD_BY_PREC(prec, ...)                                 \
+  do {                                                         \
+    if ((prec) == 0) { typedef double S; __VA_ARGS__; }        \
+    else if ((prec) == 1) { typedef float S; __VA_ARGS__; }    \
+    else { typedef __half S; __VA_ARGS__; }                    \
+  } while (0)
+
+#define QXD_GRID dim3((c->g.Vh + 127) / 128), 128, 0, c->stream
+
+int blas_axpy(qxd_ctx* c, int prec, double a, const SpinorPtr& x, const SpinorPtr& y) {
+  QXD_BY_PREC(prec, axpy_k<S><<<QXD_GRID>>>(c->g.Vh, a, x, y));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai, const SpinorPtr& y, double br, double bi,
+                  const SpinorPtr& w, const SpinorPtr& z) {
+  if (br == 0.0 && bi == 0.0) QXD_BY_PREC(prec, cxpaypbw_k<S, false><<<QXD_GRID>>>(c->g.Vh, x, ar, ai, y, br, bi, w, z));
+  else QXD_BY_PREC(prec, cxpaypbw_k<S, true><<<QXD_GRID>>>(c->g.Vh, x, ar, ai, y, br, bi, w, z));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
+               const SpinorPtr& r, double* rr) {
+  QXD_BY_PREC(prec, cg_xr_k<S><<<QXD_GRID>>>(c->g.Vh, num, den, p, t, x, r, reducer(c, rr)));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p) {
+  QXD_BY_PREC(prec, cg_p_k<S><<<QXD_GRID>>>(c->g.Vh, num, den, s, p));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* res) {
+  QXD_BY_PREC(prec, norm2_k<S><<<QXD_GRID>>>(c->g.Vh, x, reducer(c, res)));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* res3) {
+  QXD_BY_PREC(prec, cdot_k<S><<<QXD_GRID>>>(c->g.Vh, x, y, reducer(c, res3)));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x) {
+  QXD_BY_PREC(prec, zero_k<S><<<QXD_GRID>>>(c->g.Vh, x));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y) { return launch_convert_spinor(c, prec, x, prec, y); }
+int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi) {
+  QXD_BY_PREC(prec, acc_hi_k<S><<<QXD_GRID>>>(c->g.Vh, xlo, xhi));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_sub_norm(qxd_ctx* c, int prec, const SpinorPtr& b, const SpinorPtr& t, const SpinorPtr& r, double* res) {
+  QXD_BY_PREC(prec, sub_norm_k<S><<<QXD_GRID>>>(c->g.Vh, b, t, r, reducer(c, res)));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+}  // namespace qxd

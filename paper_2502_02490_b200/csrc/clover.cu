@@ -1,0 +1,290 @@
+// clover.cu -- SURVEY.md §8 row a3: on-device construction and inversion of the QCD+QED clover term.
+// The paper computes this term on the CPU and uploads it and names its generation
+// on the GPU as the next step; this file is that step.
+//
+//   M(x) = (4+m0) + c_sw (i/4) sum_{mu,nu} sigma_{mu nu} F-hat_{mu nu}(x)
+//                 + q c_sw^{U(1)} (i/4) sum_{mu,nu} sigma_{mu nu} A-hat_{mu nu}(x)      (R1,R4,R5)
+//
+// In the chiral basis of reading R3 the term is block diagonal in chirality:
+//   M_+- = (4+m0) + sum_k sigma_k (x) C^{+-}_k ,   C^{+-}_k = (i/2)(+-E_k - B_k),
+//   E_k = X_{0k},  B_1 = X_{23}, B_2 = X_{31}, B_3 = X_{12},  X = c_sw F-hat + q c_sw^{U(1)} A-hat 1.
+// Each block is stored as 36 reals in the order of PAPER.md:117.
+#include "qxd_ctx.h"
+
+namespace qxd {
+
+namespace {
+
+typedef double m3[18];  // 3x3 complex, row-major (re,im)
+
+__device__ __forceinline__ void m3_mul(const double* a, const double* b, double* c) {  // c = a b
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      double re = 0, im = 0;
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        double ar = a[2 * (3 * i + k)], ai = a[2 * (3 * i + k) + 1], br = b[2 * (3 * k + j)], bi = b[2 * (3 * k + j) + 1];
+        re += ar * br - ai * bi; im += ar * bi + ai * br;
+      }
+      c[2 * (3 * i + j)] = re; c[2 * (3 * i + j) + 1] = im;
+    }
+}
+__device__ __forceinline__ void m3_mul_adj(const double* a, const double* b, double* c) {  // c = a b^dag
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      double re = 0, im = 0;
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        double ar = a[2 * (3 * i + k)], ai = a[2 * (3 * i + k) + 1], br = b[2 * (3 * j + k)], bi = -b[2 * (3 * j + k) + 1];
+        re += ar * br - ai * bi; im += ar * bi + ai * br;
+      }
+      c[2 * (3 * i + j)] = re; c[2 * (3 * i + j) + 1] = im;
+    }
+}
+__device__ __forceinline__ void m3_adj_mul(const double* a, const double* b, double* c) {  // c = a^dag b
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      double re = 0, im = 0;
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        double ar = a[2 * (3 * k + i)], ai = -a[2 * (3 * k + i) + 1], br = b[2 * (3 * k + j)], bi = b[2 * (3 * k + j) + 1];
+        re += ar * br - ai * bi; im += ar * bi + ai * br;
+      }
+      c[2 * (3 * i + j)] = re; c[2 * (3 * i + j) + 1] = im;
+    }
+}
+
+struct GaugePtrs { const void* U[2]; const void* A[2]; };
+
+template <int MU>
+__device__ __forceinline__ void link_at(const GaugePtrs& P, const Geom& g, const Site& s, double* m) {
+  load_reals<double, 18 * MU, 18>(P.U[site_parity(s)], g.Vh, s.idx2 >> 1, m);
+}
+template <int MU>
+__device__ __forceinline__ double a_at(const GaugePtrs& P, const Geom& g, const Site& s) {
+  double a;
+  load_reals<double, MU, 1>(P.A[site_parity(s)], g.Vh, s.idx2 >> 1, &a);
+  return a;
+}
+template <int MU, int NU>
+__device__ __forceinline__ double phi_at(const GaugePtrs& P, const Geom& g, const Site& y) {
+  Site ypm, ypn;
+  site_step(g, y, MU, +1, ypm);
+  site_step(g, y, NU, +1, ypn);
+  return a_at<MU>(P, g, y) + a_at<NU>(P, g, ypm) - a_at<MU>(P, g, ypn) - a_at<NU>(P, g, y);
+}
+
+// X_{mu nu}(x) = csw F-hat_{mu nu} + q csw_qed A-hat_{mu nu} 1   (anti-Hermitian 3x3)
+template <int MU, int NU>
+__device__ void plane_X(const GaugePtrs& P, const Geom& g, const Site& x, double csw, double qcq, double qel, int use_a, double* X) {
+  Site xpm, xpn, xmm, xmn, xmmpn, xmmmn, xpmmn;
+  site_step(g, x, MU, +1, xpm); site_step(g, x, NU, +1, xpn);
+  site_step(g, x, MU, -1, xmm); site_step(g, x, NU, -1, xmn);
+  site_step(g, xmm, NU, +1, xmmpn); site_step(g, xmm, NU, -1, xmmmn); site_step(g, xpm, NU, -1, xpmmn);
+  double Q[18];
+#pragma unroll
+  for (int i = 0; i < 18; i++) Q[i] = 0.0;
+  if (csw != 0.0) {
+    m3 a, b, t1, t2, t3;
+    // leaf 1: U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
+    link_at<MU>(P, g, x, a); link_at<NU>(P, g, xpm, b); m3_mul(a, b, t1);
+    link_at<MU>(P, g, xpn, a); m3_mul_adj(t1, a, t2);
+    link_at<NU>(P, g, x, a); m3_mul_adj(t2, a, t3);
+#pragma unroll
+    for (int i = 0; i < 18; i++) Q[i] += t3[i];
+    // leaf 2: U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
+    link_at<NU>(P, g, x, a); link_at<MU>(P, g, xmmpn, b); m3_mul_adj(a, b, t1);
+    link_at<NU>(P, g, xmm, a); m3_mul_adj(t1, a, t2);
+    link_at<MU>(P, g, xmm, a); m3_mul(t2, a, t3);
+#pragma unroll
+    for (int i = 0; i < 18; i++) Q[i] += t3[i];
+    // leaf 3: U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
+    link_at<NU>(P, g, xmmmn, a); link_at<MU>(P, g, xmm, b); m3_mul(a, b, t1);   // (U_nu(x-mu-nu) U_mu(x-mu))
+    link_at<MU>(P, g, xmmmn, a); m3_adj_mul(t1, a, t2);                          // ^dag * U_mu(x-mu-nu)
+    link_at<NU>(P, g, xmn, a); m3_mul(t2, a, t3);
+#pragma unroll
+    for (int i = 0; i < 18; i++) Q[i] += t3[i];
+    // leaf 4: U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
+    link_at<NU>(P, g, xmn, a); link_at<MU>(P, g, xmn, b); m3_adj_mul(a, b, t1);
+    link_at<NU>(P, g, xpmmn, a); m3_mul(t1, a, t2);
+    link_at<MU>(P, g, x, a); m3_mul_adj(t2, a, t3);
+#pragma unroll
+    for (int i = 0; i < 18; i++) Q[i] += t3[i];
+  }
+  // F-hat = (Q - Q^dag)/8
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      X[2 * (3 * i + j)] = csw * 0.125 * (Q[2 * (3 * i + j)] - Q[2 * (3 * j + i)]);
+      X[2 * (3 * i + j) + 1] = csw * 0.125 * (Q[2 * (3 * i + j) + 1] + Q[2 * (3 * j + i) + 1]);
+    }
+  if (use_a && qcq != 0.0) {
+    // A-hat = (i/(4 qel)) sum over the four leaves of sin(qel Phi)
+    double s = sin(qel * phi_at<MU, NU>(P, g, x)) + sin(qel * phi_at<MU, NU>(P, g, xmm)) + sin(qel * phi_at<MU, NU>(P, g, xmn)) +
+               sin(qel * phi_at<MU, NU>(P, g, xmmmn));
+    double ah = qcq * s / (4.0 * qel);
+    X[1] += ah; X[9] += ah; X[17] += ah;  // imaginary parts of the diagonal
+  }
+}
+
+// add sign_p*(i/2) X to Cp and sign_m*(i/2) X to Cm
+__device__ __forceinline__ void acc_C(const double* X, double sp, double sm, double* Cp, double* Cm) {
+#pragma unroll
+  for (int k = 0; k < 9; k++) {
+    double re = -0.5 * X[2 * k + 1], im = 0.5 * X[2 * k];  // (i/2) X
+    Cp[2 * k] += sp * re; Cp[2 * k + 1] += sp * im;
+    Cm[2 * k] += sm * re; Cm[2 * k + 1] += sm * im;
+  }
+}
+
+// write sigma_k (x) C contributions into a packed block (PAPER.md:117 order)
+__device__ __forceinline__ int upper_index(int i, int j) {  // i<j, position among the 15 pairs, row-major
+  return i * 6 - (i * (i + 1)) / 2 + (j - i - 1);
+}
+__device__ __forceinline__ void block_from_C(double diag, const double* C1, const double* C2, const double* C3, double* blk) {
+  // block = diag + [[C3, C1 - i C2],[C1 + i C2, -C3]]
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    blk[a] = diag + C3[2 * (3 * a + a)];
+    blk[3 + a] = diag - C3[2 * (3 * a + a)];
+  }
+#pragma unroll
+  for (int a = 0; a < 3; a++)
+#pragma unroll
+    for (int b = 0; b < 3; b++) {
+      if (b > a) {
+        int k0 = 6 + 2 * upper_index(a, b);
+        blk[k0] = C3[2 * (3 * a + b)]; blk[k0 + 1] = C3[2 * (3 * a + b) + 1];
+        int k1 = 6 + 2 * upper_index(3 + a, 3 + b);
+        blk[k1] = -C3[2 * (3 * a + b)]; blk[k1 + 1] = -C3[2 * (3 * a + b) + 1];
+      }
+      // (C1 - i C2)[a][b]
+      int k2 = 6 + 2 * upper_index(a, 3 + b);
+      blk[k2] = C1[2 * (3 * a + b)] + C2[2 * (3 * a + b) + 1];
+      blk[k2 + 1] = C1[2 * (3 * a + b) + 1] - C2[2 * (3 * a + b)];
+    }
+}
+
+__global__ void __launch_bounds__(64) clover_build_k(Geom g, GaugePtrs P, double diag, double csw, double qcq, double qel, int use_a,
+                                                     void* M0, void* M1) {
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  int parity = blockIdx.y;
+  if (cb >= g.Vh) return;
+  Site x;
+  site_init(g, cb, parity, x);
+  double out[72];
+  double Cp[3][18], Cm[3][18];
+#pragma unroll
+  for (int k = 0; k < 3; k++)
+#pragma unroll
+    for (int i = 0; i < 18; i++) { Cp[k][i] = 0.0; Cm[k][i] = 0.0; }
+  double X[18];
+  // E_k = X_{0k}:  C^+ += (i/2) E, C^- -= (i/2) E ;  B_k:  C^+- -= (i/2) B
+  plane_X<0, 1>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, -1.0, Cp[0], Cm[0]);
+  plane_X<2, 3>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, -1.0, -1.0, Cp[0], Cm[0]);   // B_1 = X_23
+  plane_X<0, 2>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, -1.0, Cp[1], Cm[1]);
+  plane_X<1, 3>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, +1.0, Cp[1], Cm[1]);   // B_2 = X_31 = -X_13
+  plane_X<0, 3>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, -1.0, Cp[2], Cm[2]);
+  plane_X<1, 2>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, -1.0, -1.0, Cp[2], Cm[2]);   // B_3 = X_12
+  block_from_C(diag, Cp[0], Cp[1], Cp[2], out);
+  block_from_C(diag, Cm[0], Cm[1], Cm[2], out + 36);
+  store_record<double, 72>(parity ? M1 : M0, g.Vh, cb, out);
+}
+
+// Inverse of both Hermitian 6x6 blocks of every site: Gauss-Jordan with partial pivoting in fp64,
+// one thread per (site, chirality).  flag[0] is set if a block is numerically singular.
+__global__ void __launch_bounds__(64) clover_invert_k(int Vh, const void* M, void* Mi, int* flag) {
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  double in[72], out[72];
+  load_reals<double, 0, 72>(M, Vh, cb, in);
+  for (int c = 0; c < 2; c++) {
+    double ar[6][6], ai[6][6], br[6][6], bi[6][6];
+    const double* p = in + 36 * c;
+    for (int i = 0; i < 6; i++) {
+      for (int j = 0; j < 6; j++) { br[i][j] = (i == j) ? 1.0 : 0.0; bi[i][j] = 0.0; }
+      ar[i][i] = p[i]; ai[i][i] = 0.0;
+      for (int j = i + 1; j < 6; j++) {
+        int k = 6 + 2 * upper_index(i, j);
+        ar[i][j] = p[k]; ai[i][j] = p[k + 1];
+        ar[j][i] = p[k]; ai[j][i] = -p[k + 1];
+      }
+    }
+    for (int col = 0; col < 6; col++) {
+      int piv = col; double best = ar[col][col] * ar[col][col] + ai[col][col] * ai[col][col];
+      for (int r = col + 1; r < 6; r++) { double m = ar[r][col] * ar[r][col] + ai[r][col] * ai[r][col]; if (m > best) { best = m; piv = r; } }
+      if (!(best > 1e-300)) { atomicExch(flag, 1); best = 1.0; }
+      if (piv != col)
+        for (int j = 0; j < 6; j++) {
+          double t;
+          t = ar[piv][j]; ar[piv][j] = ar[col][j]; ar[col][j] = t; t = ai[piv][j]; ai[piv][j] = ai[col][j]; ai[col][j] = t;
+          t = br[piv][j]; br[piv][j] = br[col][j]; br[col][j] = t; t = bi[piv][j]; bi[piv][j] = bi[col][j]; bi[col][j] = t;
+        }
+      double dr = ar[col][col] / best, di = -ai[col][col] / best;  // 1/pivot
+      for (int j = 0; j < 6; j++) {
+        double xr = ar[col][j], xi = ai[col][j];
+        ar[col][j] = xr * dr - xi * di; ai[col][j] = xr * di + xi * dr;
+        xr = br[col][j]; xi = bi[col][j];
+        br[col][j] = xr * dr - xi * di; bi[col][j] = xr * di + xi * dr;
+      }
+      for (int r = 0; r < 6; r++) {
+        if (r == col) continue;
+        double fr = ar[r][col], fi = ai[r][col];
+        for (int j = 0; j < 6; j++) {
+          ar[r][j] -= fr * ar[col][j] - fi * ai[col][j]; ai[r][j] -= fr * ai[col][j] + fi * ar[col][j];
+          br[r][j] -= fr * br[col][j] - fi * bi[col][j]; bi[r][j] -= fr * bi[col][j] + fi * br[col][j];
+        }
+      }
+    }
+    double* o = out + 36 * c;
+    for (int i = 0; i < 6; i++) {
+      o[i] = br[i][i];
+      for (int j = i + 1; j < 6; j++) {
+        int k = 6 + 2 * upper_index(i, j);
+        // Hermitian average of the (i,j) and (j,i) entries
+        o[k] = 0.5 * (br[i][j] + br[j][i]); o[k + 1] = 0.5 * (bi[i][j] - bi[j][i]);
+      }
+    }
+  }
+  store_record<double, 72>(Mi, Vh, cb, out);
+}
+
+}  // namespace
+
+int launch_clover_build(qxd_ctx* c) {
+  GaugePtrs P;
+  P.U[0] = c->Ug[0]; P.U[1] = c->Ug[1]; P.A[0] = c->Ag[0]; P.A[1] = c->Ag[1];
+  dim3 gr((c->g.Vh + 63) / 64, 2);
+  double diag = 4.0 + c->m0;
+  clover_build_k<<<gr, 64, 0, c->stream>>>(c->g, P, diag, c->csw, c->q * c->csw_qed, c->qel, c->have_qed ? 1 : 0, c->M[0][0], c->M[0][1]);
+  QXD_LAUNCH_CHECK(c);
+  int* flag = reinterpret_cast<int*>(c->scal + 60);
+  QXD_CUDA_OK(c, cudaMemsetAsync(flag, 0, sizeof(int), c->stream));
+  for (int p = 0; p < 2; p++) {
+    clover_invert_k<<<(c->g.Vh + 63) / 64, 64, 0, c->stream>>>(c->g.Vh, c->M[0][p], c->Mi[0][p], flag);
+    QXD_LAUNCH_CHECK(c);
+  }
+  int hflag = 0;
+  QXD_CUDA_OK(c, cudaMemcpyAsync(&hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  if (hflag) return fail(c, QXD_EINVAL, "clover_build: a clover block is singular");
+  for (int pr = 1; pr < NPREC; pr++) {
+    if (!((c->prec_mask >> pr) & 1)) continue;
+    for (int p = 0; p < 2; p++) {
+      int rc = launch_convert_record72(c, c->M[0][p], pr, c->M[pr][p]);
+      if (rc) return rc;
+      rc = launch_convert_record72(c, c->Mi[0][p], pr, c->Mi[pr][p]);
+      if (rc) return rc;
+    }
+  }
+  return QXD_OK;
+}
+
+}  // namespace qxd

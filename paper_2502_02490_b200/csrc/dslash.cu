@@ -1,0 +1,286 @@
+// dslash.cu -- SURVEY.md §8 rows a4 (D_w apply), a5 (D-hat even-odd passes) and the dslash-shaped parts
+// of a8: the hand-written sm_100a stencil kernel.
+//
+//   (D_w psi)(x) = M(x) psi(x) - 1/2 sum_mu [ (1-gamma_mu) W_mu(x) psi(x+mu) + (1+gamma_mu) W_mu(x-mu)^dag psi(x-mu) ]
+//
+// (readings R1-R3; "connects nearest neighbor points ... indices for Dirac spin,
+// color charge, and space-time"; W = e^{iqA} U; M = clover term.)
+// One thread per output site: for each of the 8 neighbours the spinor is spin-projected to a half spinor
+// (2 spin x 3 colour), multiplied by the link (or its adjoint), reconstructed and accumulated; the clover
+// or inverse-clover multiplication is fused into the epilogue.  The path is bandwidth bound:
+// all field accesses are 16-byte vector loads on chunk-major SoA records, coalesced across the warp.
+//
+// In the chiral basis of reading R3 (gamma_0 = [[0,-1],[-1,0]], gamma_k = [[0,-i s_k],[i s_k,0]]):
+//   (1 -+ gamma_0) psi = (h, +-h),            h = psi_u +- psi_l
+//   (1 -+ gamma_k) psi = (h, -+ i s_k h),     h = psi_u +- i s_k psi_l
+// with the upper sign for the forward hop.
+#include "qxd_ctx.h"
+
+namespace qxd {
+
+namespace {
+
+struct DslashArgs {
+  Geom g;
+  SpinorPtr in[2];
+  SpinorPtr phi;
+  SpinorPtr out[2];
+  const void* W[2];
+  const void* CL[2];
+  int parity_out;
+  Reducer R;
+};
+
+// h = psi_u + SGN * (proj_lower), for direction MU; psi: 24 reals, h: 12 reals
+template <int MU, int SGN, typename C>
+__device__ __forceinline__ void project(const C* psi, C* h) {
+  const C s = (C)SGN;
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const C u0r = psi[2 * a], u0i = psi[2 * a + 1], u1r = psi[6 + 2 * a], u1i = psi[6 + 2 * a + 1];
+    const C l0r = psi[12 + 2 * a], l0i = psi[12 + 2 * a + 1], l1r = psi[18 + 2 * a], l1i = psi[18 + 2 * a + 1];
+    if (MU == 0) {        // + s * (l0, l1)
+      h[2 * a] = u0r + s * l0r; h[2 * a + 1] = u0i + s * l0i;
+      h[6 + 2 * a] = u1r + s * l1r; h[6 + 2 * a + 1] = u1i + s * l1i;
+    } else if (MU == 1) { // + s * (i l1, i l0)
+      h[2 * a] = u0r - s * l1i; h[2 * a + 1] = u0i + s * l1r;
+      h[6 + 2 * a] = u1r - s * l0i; h[6 + 2 * a + 1] = u1i + s * l0r;
+    } else if (MU == 2) { // + s * (l1, -l0)
+      h[2 * a] = u0r + s * l1r; h[2 * a + 1] = u0i + s * l1i;
+      h[6 + 2 * a] = u1r - s * l0r; h[6 + 2 * a + 1] = u1i - s * l0i;
+    } else {              // + s * (i l0, -i l1)
+      h[2 * a] = u0r - s * l0i; h[2 * a + 1] = u0i + s * l0r;
+      h[6 + 2 * a] = u1r + s * l1i; h[6 + 2 * a + 1] = u1i - s * l1r;
+    }
+  }
+}
+// acc_u += r ; acc_l += lower part reconstructed from r
+template <int MU, int SGN, typename C>
+__device__ __forceinline__ void reconstruct(const C* r, C* acc) {
+  const C s = (C)SGN;
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const C r0r = r[2 * a], r0i = r[2 * a + 1], r1r = r[6 + 2 * a], r1i = r[6 + 2 * a + 1];
+    acc[2 * a] += r0r; acc[2 * a + 1] += r0i;
+    acc[6 + 2 * a] += r1r; acc[6 + 2 * a + 1] += r1i;
+    if (MU == 0) {        // lower = s * (r0, r1)
+      acc[12 + 2 * a] += s * r0r; acc[12 + 2 * a + 1] += s * r0i;
+      acc[18 + 2 * a] += s * r1r; acc[18 + 2 * a + 1] += s * r1i;
+    } else if (MU == 1) { // lower = -s * (i r1, i r0)
+      acc[12 + 2 * a] += s * r1i; acc[12 + 2 * a + 1] -= s * r1r;
+      acc[18 + 2 * a] += s * r0i; acc[18 + 2 * a + 1] -= s * r0r;
+    } else if (MU == 2) { // lower = -s * (r1, -r0)
+      acc[12 + 2 * a] -= s * r1r; acc[12 + 2 * a + 1] -= s * r1i;
+      acc[18 + 2 * a] += s * r0r; acc[18 + 2 * a + 1] += s * r0i;
+    } else {              // lower = -s * (i r0, -i r1)
+      acc[12 + 2 * a] += s * r0i; acc[12 + 2 * a + 1] -= s * r0r;
+      acc[18 + 2 * a] -= s * r1i; acc[18 + 2 * a + 1] += s * r1r;
+    }
+  }
+}
+// r[s][a] = sum_b W[a][b] h[s][b]   (ADJ: sum_b conj(W[b][a]) h[s][b])
+template <bool ADJ, typename C>
+__device__ __forceinline__ void link_mul(const C* w, const C* h, C* r) {
+#pragma unroll
+  for (int s = 0; s < 2; s++)
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      C re = 0, im = 0;
+#pragma unroll
+      for (int b = 0; b < 3; b++) {
+        const C wr = ADJ ? w[2 * (3 * b + a)] : w[2 * (3 * a + b)];
+        const C wi = ADJ ? -w[2 * (3 * b + a) + 1] : w[2 * (3 * a + b) + 1];
+        const C hr = h[6 * s + 2 * b], hi = h[6 * s + 2 * b + 1];
+        re += wr * hr - wi * hi;
+        im += wr * hi + wi * hr;
+      }
+      r[6 * s + 2 * a] = re; r[6 * s + 2 * a + 1] = im;
+    }
+}
+
+// out(12 reals: one chirality) = Hermitian 6x6 block (36 packed reals) times in
+template <typename C>
+__device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
+#pragma unroll
+  for (int i = 0; i < 6; i++) { out[2 * i] = b[i] * in[2 * i]; out[2 * i + 1] = b[i] * in[2 * i + 1]; }
+  int k = 6;
+#pragma unroll
+  for (int i = 0; i < 6; i++)
+#pragma unroll
+    for (int j = i + 1; j < 6; j++) {
+      const C ur = b[k], ui = b[k + 1];
+      k += 2;
+      // out_i += u in_j ; out_j += conj(u) in_i
+      out[2 * i] += ur * in[2 * j] - ui * in[2 * j + 1];
+      out[2 * i + 1] += ur * in[2 * j + 1] + ui * in[2 * j];
+      out[2 * j] += ur * in[2 * i] + ui * in[2 * i + 1];
+      out[2 * j + 1] += ur * in[2 * i + 1] - ui * in[2 * i];
+    }
+}
+template <typename S>
+__device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const typename PT<S>::C* in, typename PT<S>::C* out) {
+  typename PT<S>::C b[36];
+  load_reals<S, 0, 36>(CL, Vh, cb, b);
+  block_mul(b, in, out);
+  load_reals<S, 36, 36>(CL, Vh, cb, b);
+  block_mul(b, in + 12, out + 12);
+}
+
+template <typename S, int MU, bool G5IN>
+__device__ __forceinline__ void hop_pair(const DslashArgs& a, const Site& s, int cb, int parity, typename PT<S>::C* acc) {
+  typedef typename PT<S>::C C;
+  const int Vh = a.g.Vh;
+  {  // forward: (1 - gamma_mu) W_mu(x) psi(x+mu)
+    const int nb = neighbour_cb<MU, +1>(a.g, s);
+    C psi[24], h[12], w[18], r[12];
+    load_spinor<S>(a.in[1 - parity], Vh, nb, psi);
+    if (G5IN) {
+#pragma unroll
+      for (int i = 12; i < 24; i++) psi[i] = -psi[i];
+    }
+    project<MU, +1>(psi, h);
+    load_reals<S, 18 * MU, 18>(a.W[parity], Vh, cb, w);
+    link_mul<false>(w, h, r);
+    reconstruct<MU, +1>(r, acc);
+  }
+  {  // backward: (1 + gamma_mu) W_mu(x-mu)^dag psi(x-mu)
+    const int nb = neighbour_cb<MU, -1>(a.g, s);
+    C psi[24], h[12], w[18], r[12];
+    load_spinor<S>(a.in[1 - parity], Vh, nb, psi);
+    if (G5IN) {
+#pragma unroll
+      for (int i = 12; i < 24; i++) psi[i] = -psi[i];
+    }
+    project<MU, -1>(psi, h);
+    load_reals<S, 18 * MU, 18>(a.W[1 - parity], Vh, nb, w);
+    link_mul<true>(w, h, r);
+    reconstruct<MU, -1>(r, acc);
+  }
+}
+
+// PHI: 0 none, 1 phi, 2 M*phi (FULL: phi = in on the own parity).  POST: 1 = multiply the result by M^{-1}.
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL>
+__global__ void __launch_bounds__(128) dslash_k(const __grid_constant__ DslashArgs a) {
+  typedef typename PT<S>::C C;
+  const int Vh = a.g.Vh;
+  const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  const int parity = FULL ? blockIdx.y : a.parity_out;
+  double nrm[1] = {0.0};
+  if (cb < Vh) {
+    Site s;
+    site_init(a.g, cb, parity, s);
+    C acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] = 0;
+    hop_pair<S, 0, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
+    hop_pair<S, 1, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
+    hop_pair<S, 2, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
+    hop_pair<S, 3, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
+    const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] *= ((FLAGS & DSF_G5HOP) && i >= 12) ? -hs : hs;
+    if (PHI != 0) {
+      C phi[24];
+      load_spinor<S>(FULL ? a.in[parity] : a.phi, Vh, cb, phi);
+      if (PHI == 2) {
+        C mphi[24];
+        clover_mul<S>(a.CL[parity], Vh, cb, phi, mphi);
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] += mphi[i];
+      } else {
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[i] += phi[i];
+      }
+    }
+    if (POST) {
+      C t[24];
+      clover_mul<S>(a.CL[parity], Vh, cb, acc, t);
+#pragma unroll
+      for (int i = 0; i < 24; i++) acc[i] = t[i];
+    }
+    if (FLAGS & DSF_NORM) {
+#pragma unroll
+      for (int i = 0; i < 24; i++) nrm[0] += (double)acc[i] * (double)acc[i];
+    }
+    store_spinor<S>(a.out[parity], Vh, cb, acc);
+  }
+  if (FLAGS & DSF_NORM) grid_reduce<1>(nrm, a.R);
+}
+
+template <typename S, int INV_DUMMY>
+__global__ void __launch_bounds__(128) clover_apply_k(int Vh, const void* CL, SpinorPtr in, SpinorPtr out) {
+  typedef typename PT<S>::C C;
+  const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  C v[24], w[24];
+  load_spinor<S>(in, Vh, cb, v);
+  clover_mul<S>(CL, Vh, cb, v, w);
+  store_spinor<S>(out, Vh, cb, w);
+}
+
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL>
+void launch_one(qxd_ctx* c, const DslashArgs& a) {
+  dim3 gr((c->g.Vh + 127) / 128, FULL ? 2 : 1);
+  dslash_k<S, PHI, POST, NEG, FLAGS, FULL><<<gr, 128, 0, c->stream>>>(a);
+}
+
+template <typename S>
+int dispatch(qxd_ctx* c, const DslashCall& d, const DslashArgs& a) {
+  const int f = d.flags;
+  switch (d.mode) {
+    case DS_DW_FULL:
+      if (f != 0) break;
+      launch_one<S, 2, 0, false, 0, true>(c, a); return QXD_OK;
+    case DS_HOP_AINV:
+      if (f == 0) { launch_one<S, 0, 1, false, 0, false>(c, a); return QXD_OK; }
+      if (f == DSF_G5IN) { launch_one<S, 0, 1, false, DSF_G5IN, false>(c, a); return QXD_OK; }
+      break;
+    case DS_A_XMHOP:
+      if (f == 0) { launch_one<S, 2, 0, true, 0, false>(c, a); return QXD_OK; }
+      if (f == DSF_NORM) { launch_one<S, 2, 0, true, DSF_NORM, false>(c, a); return QXD_OK; }
+      if (f == DSF_G5HOP) { launch_one<S, 2, 0, true, DSF_G5HOP, false>(c, a); return QXD_OK; }
+      if (f == (DSF_G5HOP | DSF_NORM)) { launch_one<S, 2, 0, true, DSF_G5HOP | DSF_NORM, false>(c, a); return QXD_OK; }
+      break;
+    case DS_X_MHOP:
+      if (f == 0) { launch_one<S, 1, 0, true, 0, false>(c, a); return QXD_OK; }
+      break;
+    case DS_AINV_X_MHOP:
+      if (f == 0) { launch_one<S, 1, 1, true, 0, false>(c, a); return QXD_OK; }
+      break;
+    default: break;
+  }
+  return fail(c, QXD_EINVAL, "dslash: unsupported mode/flags combination");
+}
+
+}  // namespace
+
+int launch_dslash(qxd_ctx* c, const DslashCall& d) {
+  if (d.prec < 0 || d.prec >= NPREC || !((c->prec_mask >> d.prec) & 1)) return fail(c, QXD_EINVAL, "dslash: precision not bound");
+  DslashArgs a;
+  a.g = c->g;
+  a.in[0] = d.in[0]; a.in[1] = d.in[1];
+  a.phi = d.phi;
+  a.out[0] = d.out[0]; a.out[1] = d.out[1];
+  a.W[0] = c->W[d.prec][0]; a.W[1] = c->W[d.prec][1];
+  const bool inv = (d.mode == DS_HOP_AINV || d.mode == DS_AINV_X_MHOP);
+  a.CL[0] = inv ? c->Mi[d.prec][0] : c->M[d.prec][0];
+  a.CL[1] = inv ? c->Mi[d.prec][1] : c->M[d.prec][1];
+  a.parity_out = d.parity_out;
+  a.R.partials = c->partials; a.R.ticket = c->ticket; a.R.result = d.norm_result;
+  int rc = d.prec == 0 ? dispatch<double>(c, d, a) : d.prec == 1 ? dispatch<float>(c, d, a) : dispatch<__half>(c, d, a);
+  if (rc) return rc;
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+int launch_clover_apply(qxd_ctx* c, int prec, int inverse, int parity, const SpinorPtr& in, const SpinorPtr& out) {
+  const void* CL = inverse ? c->Mi[prec][parity] : c->M[prec][parity];
+  dim3 gr((c->g.Vh + 127) / 128);
+  if (prec == 0) clover_apply_k<double, 0><<<gr, 128, 0, c->stream>>>(c->g.Vh, CL, in, out);
+  else if (prec == 1) clover_apply_k<float, 0><<<gr, 128, 0, c->stream>>>(c->g.Vh, CL, in, out);
+  else clover_apply_k<__half, 0><<<gr, 128, 0, c->stream>>>(c->g.Vh, CL, in, out);
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+}  // namespace qxd

@@ -1,0 +1,262 @@
+// qxd_common.cuh -- geometry, precision traits and 16-byte-chunk SoA record access.
+//
+// Site order on the device: the paper's host code orders sites in cache
+// blocks, lexicographic inside a block, even sites first (Eq. (2)); we keep that idea
+// with power-of-two tiles sized for the B200 L1/L2 and compute every index on the fly as a pure
+// inlined function, as PAPER.md:105 advises (no lookup tables).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+namespace qxd {
+
+struct Geom {
+  int X[4];        // extended extents T, X1, L2, L3
+  int L1;          // physical extent of direction 1 (the C* shift)
+  int cstar;       // 0..3
+  int antiper;     // fermions antiperiodic in time
+  int Vh;          // V/2 = sites per parity = stride of every SoA record
+  int sh[4];       // log2 of the tile extents b_mu (sh[3] >= 1)
+  int lo_str[4];   // stride of the in-tile digit of direction mu (full-index units)
+  int hi_str[4];   // stride of the tile digit of direction mu
+  int nt[4];       // tiles per direction
+};
+
+// full index idx2(x) = sum_mu g_mu(x_mu); checkerboard index cb = idx2 >> 1; parity = sum x_mu & 1.
+__host__ __device__ __forceinline__ int gmu(const Geom& g, int mu, int c) {
+  return (c & ((1 << g.sh[mu]) - 1)) * g.lo_str[mu] + (c >> g.sh[mu]) * g.hi_str[mu];
+}
+__host__ __device__ __forceinline__ int idx2_of(const Geom& g, const int x[4]) {
+  return gmu(g, 0, x[0]) + gmu(g, 1, x[1]) + gmu(g, 2, x[2]) + gmu(g, 3, x[3]);
+}
+// inverse: (cb, parity) -> coordinates
+__host__ __device__ __forceinline__ void coords_of(const Geom& g, int cb, int parity, int x[4]) {
+  const int tsh = g.sh[0] + g.sh[1] + g.sh[2] + g.sh[3] - 1;  // log2(tile volume / 2)
+  int tile = cb >> tsh;
+  int r = cb & ((1 << tsh) - 1);
+  int zh = r & ((1 << (g.sh[3] - 1)) - 1); r >>= (g.sh[3] - 1);
+  int yl = r & ((1 << g.sh[2]) - 1); r >>= g.sh[2];
+  int xl = r & ((1 << g.sh[1]) - 1); r >>= g.sh[1];
+  int tl = r;
+  int tz = tile % g.nt[3]; tile /= g.nt[3];
+  int ty = tile % g.nt[2]; tile /= g.nt[2];
+  int tx = tile % g.nt[1];
+  int tt = tile / g.nt[1];
+  x[0] = (tt << g.sh[0]) | tl;
+  x[1] = (tx << g.sh[1]) | xl;
+  x[2] = (ty << g.sh[2]) | yl;
+  int zb = (parity + x[0] + x[1] + x[2]) & 1;
+  x[3] = (tz << g.sh[3]) | (zh << 1) | zb;
+}
+// natural (application) order, Eq. (1) PAPER.md:93 with L1 -> X1
+__host__ __device__ __forceinline__ long lex_of(const Geom& g, const int x[4]) {
+  return ((long(x[0]) * g.X[1] + x[1]) * g.X[2] + x[2]) * g.X[3] + x[3];
+}
+
+// Per-thread site context: coordinates and their index contributions (separable index).
+struct Site {
+  int x[4];
+  int gx[4];
+  int idx2;
+};
+__device__ __forceinline__ void site_init(const Geom& g, int cb, int parity, Site& s) {
+  coords_of(g, cb, parity, s.x);
+#pragma unroll
+  for (int mu = 0; mu < 4; mu++) s.gx[mu] = gmu(g, mu, s.x[mu]);
+  s.idx2 = s.gx[0] + s.gx[1] + s.gx[2] + s.gx[3];
+}
+// checkerboard index of x + dir*mu-hat with the boundary rules of reading R8: time and direction 1
+// periodic (X1 = 2 L1 under C*), directions k in 2..cstar wrap with the shift x1 -> x1 + L1 mod 2 L1
+// ("shifted boundaries").  The neighbour has the opposite parity.
+template <int MU, int DIR>
+__device__ __forceinline__ int neighbour_cb(const Geom& g, const Site& s) {
+  int c = s.x[MU] + DIR;
+  bool wrap = false;
+  if (DIR > 0) { if (c >= g.X[MU]) { c = 0; wrap = true; } }
+  else         { if (c < 0) { c = g.X[MU] - 1; wrap = true; } }
+  int n = s.idx2 - s.gx[MU] + gmu(g, MU, c);
+  if (MU >= 2) {
+    if (wrap && MU <= g.cstar) {
+      int y1 = s.x[1] + g.L1;
+      if (y1 >= g.X[1]) y1 -= g.X[1];
+      n += gmu(g, 1, y1) - s.gx[1];
+    }
+  }
+  return n >> 1;
+}
+// run-time (mu,dir) version for the one-off kernels (clover build); also moves the Site.
+__device__ __forceinline__ void site_step(const Geom& g, const Site& s, int mu, int dir, Site& o) {
+  o = s;
+  int c = s.x[mu] + dir;
+  bool wrap = false;
+  if (c >= g.X[mu]) { c = 0; wrap = true; }
+  if (c < 0) { c = g.X[mu] - 1; wrap = true; }
+  o.x[mu] = c; o.gx[mu] = gmu(g, mu, c);
+  if (wrap && mu >= 2 && mu <= g.cstar) {
+    int y1 = s.x[1] + g.L1;
+    if (y1 >= g.X[1]) y1 -= g.X[1];
+    o.x[1] = y1; o.gx[1] = gmu(g, 1, y1);
+  }
+  o.idx2 = o.gx[0] + o.gx[1] + o.gx[2] + o.gx[3];
+}
+__device__ __forceinline__ int site_parity(const Site& s) { return (s.x[0] + s.x[1] + s.x[2] + s.x[3]) & 1; }
+
+// ---------------------------------------------------------------------------------------------
+// Storage precisions.  A "record" of NR reals per site is stored as ceil(NR/RPC) 16-byte chunks,
+// chunk-major: element (chunk c, site cb) at vector index c*Vh + cb, so that consecutive threads
+// (consecutive cb) issue one coalesced 128-bit access per chunk.
+// ---------------------------------------------------------------------------------------------
+template <typename S> struct PT;
+template <> struct PT<double> { typedef double2 V; typedef double C; static constexpr int RPC = 2; static constexpr int ID = 0; };
+template <> struct PT<float>  { typedef float4 V;  typedef float C;  static constexpr int RPC = 4; static constexpr int ID = 1; };
+template <> struct PT<__half> { typedef uint4 V;   typedef float C;  static constexpr int RPC = 8; static constexpr int ID = 2; };
+
+__device__ __forceinline__ void unpack_vec(const double2& v, double* o) { o[0] = v.x; o[1] = v.y; }
+__device__ __forceinline__ void unpack_vec(const float4& v, float* o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+__device__ __forceinline__ void unpack_vec(const uint4& v, float* o) {
+  const __half2* h = reinterpret_cast<const __half2*>(&v);
+#pragma unroll
+  for (int i = 0; i < 4; i++) { float2 f = __half22float2(h[i]); o[2 * i] = f.x; o[2 * i + 1] = f.y; }
+}
+__device__ __forceinline__ double2 pack_vec(const double* o, double2*) { return make_double2(o[0], o[1]); }
+__device__ __forceinline__ float4 pack_vec(const float* o, float4*) { return make_float4(o[0], o[1], o[2], o[3]); }
+__device__ __forceinline__ uint4 pack_vec(const float* o, uint4*) {
+  uint4 v;
+  __half2* h = reinterpret_cast<__half2*>(&v);
+#pragma unroll
+  for (int i = 0; i < 4; i++) h[i] = __floats2half2_rn(o[2 * i], o[2 * i + 1]);
+  return v;
+}
+
+// load reals [R0, R0+N) of the record of site cb (read-only path)
+template <typename S, int R0, int N>
+__device__ __forceinline__ void load_reals(const void* __restrict__ base, int Vh, int cb, typename PT<S>::C* out) {
+  typedef typename PT<S>::V V;
+  typedef typename PT<S>::C C;
+  constexpr int RPC = PT<S>::RPC;
+  constexpr int C0 = R0 / RPC, C1 = (R0 + N - 1) / RPC;
+  const V* p = reinterpret_cast<const V*>(base);
+#pragma unroll
+  for (int c = C0; c <= C1; c++) {
+    V v = __ldg(p + size_t(c) * Vh + cb);
+    C tmp[RPC];
+    unpack_vec(v, tmp);
+#pragma unroll
+    for (int k = 0; k < RPC; k++) {
+      constexpr int dummy = 0; (void)dummy;
+      int r = c * RPC + k;
+      if (r >= R0 && r < R0 + N) out[r - R0] = tmp[k];
+    }
+  }
+}
+// store a whole record of NR reals (NR % RPC == 0)
+template <typename S, int NR>
+__device__ __forceinline__ void store_record(void* __restrict__ base, int Vh, int cb, const typename PT<S>::C* in) {
+  typedef typename PT<S>::V V;
+  constexpr int RPC = PT<S>::RPC;
+  static_assert(NR % RPC == 0, "record must fill whole chunks");
+  V* p = reinterpret_cast<V*>(base);
+#pragma unroll
+  for (int c = 0; c < NR / RPC; c++) p[size_t(c) * Vh + cb] = pack_vec(in + c * RPC, (V*)nullptr);
+}
+
+// A packed half-lattice spinor: 24 reals per site; fp16 adds one fp32 scale per site (block-float,
+// reading R12): stored halves = value / scale, scale = max |component| of the site.
+struct SpinorPtr {
+  void* data;
+  float* scale;  // fp16 only
+};
+template <typename S> __host__ __device__ inline size_t spinor_half_bytes(int Vh) {
+  return size_t(Vh) * 24 * sizeof(S) + (PT<S>::ID == 2 ? size_t(Vh) * 4 : 0);
+}
+template <typename S> __host__ __device__ inline SpinorPtr spinor_view(void* base, int Vh, int parity) {
+  char* b = static_cast<char*>(base) + size_t(parity) * spinor_half_bytes<S>(Vh);
+  SpinorPtr p;
+  p.data = b;
+  p.scale = (PT<S>::ID == 2) ? reinterpret_cast<float*>(b + size_t(Vh) * 24 * sizeof(S)) : nullptr;
+  return p;
+}
+template <typename S>
+__device__ __forceinline__ void load_spinor(const SpinorPtr& p, int Vh, int cb, typename PT<S>::C* out) {
+  load_reals<S, 0, 24>(p.data, Vh, cb, out);
+  if (PT<S>::ID == 2) {
+    float sc = __ldg(p.scale + cb);
+#pragma unroll
+    for (int i = 0; i < 24; i++) out[i] *= sc;
+  }
+}
+template <typename S>
+__device__ __forceinline__ void store_spinor(const SpinorPtr& p, int Vh, int cb, typename PT<S>::C* v) {
+  if (PT<S>::ID == 2) {
+    float m = 0.f;
+#pragma unroll
+    for (int i = 0; i < 24; i++) m = fmaxf(m, fabsf((float)v[i]));
+    float inv = m > 0.f ? 1.0f / m : 0.f;
+#pragma unroll
+    for (int i = 0; i < 24; i++) v[i] *= inv;
+    p.scale[cb] = m;
+  }
+  store_record<S, 24>(p.data, Vh, cb, v);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Reductions (row a6): warp shuffle -> block -> single-pass grid reduction.  Every block writes its
+// partial sums, the last block to finish (atomic ticket) adds the partials in a fixed order, so the
+// result is deterministic for a fixed launch configuration.  fp64 accumulators for every storage type.
+// ---------------------------------------------------------------------------------------------
+struct Reducer {
+  double* partials;    // [N][gridDim.x]
+  unsigned* ticket;
+  double* result;      // [N]
+};
+template <int N>
+__device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R) {
+  __shared__ double sm[N][32];
+  __shared__ bool last;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int k = 0; k < N; k++) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+    if (lane == 0) sm[k][w] = v[k];
+  }
+  __syncthreads();
+  if (w == 0) {
+#pragma unroll
+    for (int k = 0; k < N; k++) {
+      double t = lane < nw ? sm[k][lane] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+      if (lane == 0) R.partials[size_t(k) * gridDim.x + blockIdx.x] = t;
+    }
+  }
+  if (threadIdx.x == 0) {
+    __threadfence();
+    unsigned t = atomicAdd(R.ticket, 1u);
+    last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (last) {
+    __threadfence();
+#pragma unroll
+    for (int k = 0; k < N; k++) {
+      double t = 0.0;
+      for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) t += __ldcg(R.partials + size_t(k) * gridDim.x + i);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+      __syncthreads();
+      if (lane == 0) sm[k][w] = t;
+      __syncthreads();
+      if (w == 0) {
+        double u = lane < nw ? sm[k][lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
+        if (lane == 0) R.result[k] = u;
+      }
+    }
+    if (threadIdx.x == 0) *R.ticket = 0u;
+  }
+}
+
+}  // namespace qxd

@@ -1,0 +1,135 @@
+// qxd_ctx.h -- host-side context of the C-ABI library and the internal launcher prototypes.
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include <cstdio>
+#include "../../include/qxd.h"
+#include "qxd_common.cuh"
+
+namespace qxd {
+
+enum { NPREC = 3 };
+inline size_t prec_size(int p) { return p == 0 ? 8 : (p == 1 ? 4 : 2); }
+
+// dslash epilogue selection:  tmp = PHI-term + (NEG ? -1 : +1) * hop(in);
+// out = POST applied to tmp, where hop(in) = -1/2 sum_mu [...] is the off-diagonal part of D_w.
+enum DslashMode {
+  DS_DW_FULL = 0,   // out = M in(x) + hop(in)                      both parities in one launch   (row a4)
+  DS_HOP_AINV,      // out_p = M^{-1} hop(in)                       pass 1 of D-hat               (row a5)
+  DS_A_XMHOP,       // out_p = M phi - hop(in)                      pass 2 of D-hat               (row a5)
+  DS_X_MHOP,        // out_p = phi - hop(in)                        source preparation            (row a8)
+  DS_AINV_X_MHOP,   // out_p = M^{-1} (phi - hop(in))               odd-site reconstruction       (row a8)
+  DS_NMODES
+};
+enum { DSF_G5IN = 1, DSF_G5HOP = 2, DSF_NORM = 4 };
+
+struct Scalars;  // device-resident solver scalars (solver.cu)
+
+}  // namespace qxd
+
+struct qxd_ctx {
+  qxd::Geom g;
+  int T, L1, L2, L3, bc;
+  long V;
+  cudaStream_t stream = 0;
+  // workspace
+  char* ws = nullptr;
+  size_t ws_bytes = 0, ws_used = 0;
+  int prec_mask = 0, nrhs = 1;
+  // state
+  bool have_gauge = false, have_qed = false, have_quark = false, have_clover = false;
+  double qel = 1.0, kappa = 0, q = 0, m0 = 0, csw = 0, csw_qed = 0;
+  // fields (device, carved from the workspace); [parity]
+  void* Ug[2] = {nullptr, nullptr};              // fp64 SU(3) links, record of 72 reals (4 links x 18)
+  void* Ag[2] = {nullptr, nullptr};              // fp64 U(1) field, record of 4 reals
+  void* W[qxd::NPREC][2] = {};                   // hopping links e^{iqA} U (time-BC sign folded in), 72 reals
+  void* M[qxd::NPREC][2] = {};                   // clover blocks, 72 reals (PAPER.md:117 order)
+  void* Mi[qxd::NPREC][2] = {};                  // inverse blocks
+  // scratch spinors
+  void* sp64[12] = {};                           // fp64 half-lattice spinors
+  void* splo[8] = {};                            // sloppy half-lattice spinors (sized for fp32)
+  void* full_a = nullptr;                        // packed full-lattice spinors (sized for fp64)
+  void* full_b = nullptr;
+  double* nat_a = nullptr;                       // natural-order staging (host-pointer entry points)
+  double* nat_b = nullptr;
+  // reductions
+  double* partials = nullptr;
+  unsigned* ticket = nullptr;
+  double* scal = nullptr;                        // device scalars [64]
+  double* h_scal = nullptr;                      // pinned host mirror [64]
+  int max_blocks = 0;
+  long launches = 0;
+  std::string err;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+};
+
+namespace qxd {
+
+inline int fail(qxd_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+#define QXD_CUDA_OK(ctx, expr)                                                                   \
+  do {                                                                                           \
+    cudaError_t e__ = (expr);                                                                    \
+    if (e__ != cudaSuccess) return qxd::fail(ctx, QXD_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e__)); \
+  } while (0)
+
+#define QXD_LAUNCH_CHECK(c)                                                                                    \
+  do {                                                                                                         \
+    (c)->launches++;                                                                                           \
+    cudaError_t e__ = cudaGetLastError();                                                                      \
+    if (e__ != cudaSuccess) return qxd::fail((c), QXD_ECUDA, std::string(__func__) + ": " + cudaGetErrorString(e__)); \
+  } while (0)
+
+inline SpinorPtr half_view(int prec, void* base, int Vh, int parity) {
+  return prec == 0 ? spinor_view<double>(base, Vh, parity) : prec == 1 ? spinor_view<float>(base, Vh, parity) : spinor_view<__half>(base, Vh, parity);
+}
+inline size_t half_bytes(int prec, int Vh) {
+  return prec == 0 ? spinor_half_bytes<double>(Vh) : prec == 1 ? spinor_half_bytes<float>(Vh) : spinor_half_bytes<__half>(Vh);
+}
+
+// ---- launchers (each returns a qxd_status and bumps ctx->launches) ----
+// pack.cu
+int launch_gauge_pack(qxd_ctx* c, const double* U, const double* A);
+int launch_hoplinks(qxd_ctx* c, int prec);
+int launch_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed, int parity_mask /*1 even,2 odd,3 both*/, int compact_even);
+int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, int parity_mask, int compact_even);
+int launch_convert_spinor(qxd_ctx* c, int prec_from, const SpinorPtr& from, int prec_to, const SpinorPtr& to);
+int launch_convert_record72(qxd_ctx* c, const void* from64, int prec_to, void* to);
+int launch_clover_export(qxd_ctx* c, double* out, int inverse);
+// clover.cu
+int launch_clover_build(qxd_ctx* c);
+// dslash.cu
+struct DslashCall {
+  int prec;
+  int mode;         // DslashMode
+  int flags;        // DSF_*
+  int parity_out;   // parity of the output sites (ignored for DS_DW_FULL)
+  SpinorPtr in[2];  // input spinor per parity (hop reads in[1-p]; DS_DW_FULL also in[p])
+  SpinorPtr phi;    // PHI-term input on the output parity (modes with phi)
+  SpinorPtr out[2]; // output per parity (only [parity_out] used unless DS_DW_FULL)
+  double* norm_result;  // DSF_NORM: device slot receiving |out|^2
+};
+int launch_dslash(qxd_ctx* c, const DslashCall& d);
+int launch_clover_apply(qxd_ctx* c, int prec, int inverse, int parity, const SpinorPtr& in, const SpinorPtr& out);
+// blas.cu
+int blas_axpy(qxd_ctx* c, int prec, double a, const SpinorPtr& x, const SpinorPtr& y);            // y += a x
+int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* dev_result3);  // Re<x,y>, Im<x,y>, |y|^2
+int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* dev_result);
+int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x);
+// z = x + a*y + b*w with complex scalars by value (w may be unused when b == 0); BiCGstab building block
+int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai, const SpinorPtr& y, double br, double bi,
+                  const SpinorPtr& w, const SpinorPtr& z);
+// alpha = *num / *den (device scalars): x += alpha p ; r -= alpha t ; *rr = |r|^2
+int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
+               const SpinorPtr& r, double* rr);
+// beta = *num / *den : p = s + beta p
+int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p);
+int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi);                  // x_hi += x_lo ; x_lo = 0
+int blas_sub_norm(qxd_ctx* c, int prec, const SpinorPtr& b, const SpinorPtr& t, const SpinorPtr& r, double* res);  // r = b - t
+int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y);                       // y = x
+// solver.cu
+int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+
+}  // namespace qxd
