@@ -1,0 +1,300 @@
+"""GPU parity: the CUDA path (through the C-ABI, paper_2502_02490_b200.binding) against the fp64 CPU
+oracle, element by element on the same seeded inputs (SURVEY.md §8(d) "Parity").
+
+Tolerances (BASELINE.json north_star):
+  fp64 operator: relative L2 error <= 1e-13;  fp32: <= 1e-6;  fp16 (reading R13): <= 2e-3;
+  solves: ||eta - D_ref psi|| / ||eta|| <= tol with the ORACLE's D (1e-12 for c0/c1, 1e-10 mixed).
+Integer / layout work (pack -> unpack) is bit-exact.
+"""
+import numpy as np
+import pytest
+
+import synth
+from oracle import qxd_ref as R
+
+pytestmark = pytest.mark.gpu
+
+F64, F32, F16 = 0, 1, 2
+TOL = {F64: 1e-13, F32: 1e-6, F16: 2e-3}
+
+
+def relerr(a, b):
+    a = np.ravel(a)
+    b = np.ravel(b)
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def to_np(t):
+    return t.detach().cpu().numpy()
+
+
+class Case:
+    """Oracle context + CUDA context on identical seeded fields."""
+
+    def __init__(self, dims, cstar, ap, qed, q=2 / 3, kappa=0.12, csw=1.5, csw_qed=1.0, qel=1.0, eps=0.3,
+                 precisions=(F64, F32, F16), tile=None, oracle_clover=True):
+        from paper_2502_02490_b200 import binding as B
+        self.B = B
+        bc = cstar | (ap << 2)
+        self.dims = dims
+        self.U = synth.su3_links(dims, eps, 1)
+        self.A = synth.u1_field(dims, 0.3, 2) if qed else None
+        self.q = q if qed else 0.0
+        self.csw_qed = csw_qed if qed else 0.0
+        self.ref = R.Ref(*dims, bc)
+        self.ref.gauge_load(self.U, self.A, qel)
+        self.ref.set_quark(kappa, self.q)
+        if oracle_clover:
+            self.ref.clover_build(csw, self.csw_qed)
+        else:
+            self.ref.set_csw(csw, self.csw_qed)
+        self.gpu = B.Qxd(*dims, bc, precisions=precisions, tile=tile)
+        self.gpu.gauge_load(self.U, self.A, qel)
+        self.gpu.set_quark(kappa, self.q)
+        self.gpu.clover_build(csw, self.csw_qed)
+        self.dims_ext = self.ref.dims_ext
+        self.V = self.ref.V
+
+    def close(self):
+        self.gpu.close()
+
+
+# dims (physical), cstar, antiperiodic, qed  -- several tiles, ragged tails (Vh % 128 != 0), L=2 edge cases
+SMALL = [
+    ((4, 4, 4, 4), 0, 1, False),      # BASELINE config c0
+    ((4, 4, 4, 4), 0, 0, True),
+    ((6, 4, 6, 10), 0, 1, True),      # Vh = 720: ragged tail, non power-of-two extents
+    ((4, 2, 4, 4), 1, 1, True),
+    ((4, 4, 2, 6), 2, 1, True),
+    ((6, 4, 4, 6), 3, 1, True),
+    ((2, 2, 2, 2), 3, 1, True),       # degenerate: forward and backward neighbour coincide
+    ((8, 8, 8, 8), 3, 1, True),       # BASELINE config c1 (q = +2/3)
+]
+
+
+@pytest.fixture(scope="module", params=SMALL, ids=lambda p: "x".join(map(str, p[0])) + f"-cstar{p[1]}ap{p[2]}{'qed' if p[3] else 'qcd'}")
+def case(request):
+    c = Case(*request.param)
+    yield c
+    c.close()
+
+
+def test_clover_blocks_match_oracle(case):
+    """Row a3: M and M^{-1} in the PAPER.md:117 packing, fp64."""
+    got = to_np(case.gpu.clover_export(False))
+    exp = case.ref.clover_packed(False)
+    assert relerr(got, exp) < 1e-13
+    got = to_np(case.gpu.clover_export(True))
+    exp = case.ref.clover_packed(True)
+    assert relerr(got, exp) < 1e-12  # inverse of a 6x6 block with cond ~ 10
+
+
+@pytest.mark.parametrize("prec", [F64, F32, F16])
+def test_apply_Dw(case, prec):
+    """Row a4, element by element over the whole extended lattice."""
+    psi = synth.gaussian_spinor(case.dims_ext, 3)
+    exp = case.ref.apply_Dw(psi)
+    got = to_np(case.gpu.apply_Dw(psi, prec)).reshape(exp.shape)
+    assert relerr(got, exp) < TOL[prec]
+    if prec == F64:
+        assert np.max(np.abs(got - exp)) < 1e-12 * np.max(np.abs(exp))
+
+
+@pytest.mark.parametrize("prec", [F64, F32, F16])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_apply_Dhat(case, prec, dagger):
+    """Row a5: both fused passes of the even-odd operator and its adjoint."""
+    pe = synth.gaussian_spinor(case.dims_ext, 6).reshape(-1, 4, 3)[: case.V // 2]
+    exp = case.ref.apply_Dhat(pe, dagger=dagger)
+    got = to_np(case.gpu.apply_Dhat_eo(pe, prec, dagger=dagger)).reshape(exp.shape)
+    assert relerr(got, exp) < 2 * TOL[prec]
+
+
+def test_pack_unpack_bit_exact(case):
+    """Row a9: natural -> packed -> natural is the identity in fp64 (index work is bit-exact)."""
+    psi = synth.gaussian_spinor(case.dims_ext, 7)
+    p = case.gpu.spinor_pack(psi, F64)
+    back = to_np(case.gpu.spinor_unpack(p, F64))
+    assert np.array_equal(back.view(np.float64), psi.view(np.float64))
+    # fp32 storage rounds each real once
+    p = case.gpu.spinor_pack(psi, F32)
+    back = to_np(case.gpu.spinor_unpack(p, F32))
+    assert np.array_equal(back.view(np.float64), psi.view(np.float64).astype(np.float32).astype(np.float64))
+
+
+def test_packed_apply_equals_natural_apply(case):
+    psi = synth.gaussian_spinor(case.dims_ext, 3)
+    g = case.gpu
+    pin = g.spinor_pack(psi, F64)
+    pout = g.new_packed(F64)
+    g.apply_Dw_packed(pin, pout, F64)
+    a = to_np(g.spinor_unpack(pout, F64))
+    b = to_np(g.apply_Dw(psi, F64)).reshape(a.shape)
+    assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("prec", [F64, F32, F16])
+def test_blas(case, prec):
+    """Row a6: axpy, complex dot, norm^2 on packed half-lattice spinors against numpy in fp64."""
+    g = case.gpu
+    x = synth.gaussian_spinor(case.dims_ext, 8)
+    y = synth.gaussian_spinor(case.dims_ext, 9)
+    px, py = g.spinor_pack(x, prec), g.spinor_pack(y, prec)
+    # what the device actually holds (after storage rounding), even half first
+    xs = to_np(g.spinor_unpack(px, prec)).reshape(-1, 12)
+    ys = to_np(g.spinor_unpack(py, prec)).reshape(-1, 12)
+    lat_par = np.indices(case.dims_ext).sum(axis=0).ravel() & 1
+    xe, ye = xs[lat_par == 0], ys[lat_par == 0]
+    hb = g.packed_spinor_bytes(prec, half_only=True)
+    n2 = g.blas_norm2(px[:hb], prec)
+    assert abs(n2 - np.vdot(xe, xe).real) / n2 < 1e-13
+    d = g.blas_cdot(px[:hb], py[:hb], prec)
+    expd = np.vdot(xe, ye)
+    assert abs(d - expd) / abs(expd) < 1e-12
+    g.blas_axpy(0.37, px[:hb], py[:hb], prec)
+    got = to_np(g.spinor_unpack(py, prec)).reshape(-1, 12)[lat_par == 0]
+    assert relerr(got, ye + 0.37 * xe) < {F64: 1e-15, F32: 2e-7, F16: 1e-3}[prec]
+
+
+def test_tiling_does_not_change_results():
+    """Row a1: the tile shape only permutes sites in memory; results are identical for any legal tile."""
+    dims = (4, 4, 4, 8)
+    outs = []
+    psi = synth.gaussian_spinor((4, 8, 4, 8), 3)
+    for tile in [(1, 1, 1, 2), (2, 2, 2, 2), (4, 8, 4, 8), (1, 2, 4, 8), None]:
+        c = Case(dims, 3, 1, True, precisions=(F64,), tile=tile, oracle_clover=False)
+        outs.append(to_np(c.gpu.apply_Dw(psi, F64)))
+        c.close()
+    for o in outs[1:]:
+        assert np.array_equal(o, outs[0])
+
+
+# ---- solves ------------------------------------------------------------------------------------------------
+def true_residual(ref, eta, psi):
+    return np.linalg.norm(np.ravel(eta) - np.ravel(ref.apply_Dw(psi))) / np.linalg.norm(np.ravel(eta))
+
+
+@pytest.mark.parametrize("name,q", [("c0", 0.0), ("c1", 2 / 3), ("c1", -1 / 3)])
+@pytest.mark.parametrize("algo", [0, 1])
+def test_solve_fp64_configs_c0_c1(name, q, algo):
+    """BASELINE configs 0 and 1: fp64 even-odd CGNE / BiCGstab to 1e-12, residual checked with the oracle's D."""
+    cfg = synth.config(name)
+    c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=q, kappa=cfg["kappa"], csw=cfg["csw"],
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64,))
+    eta = synth.gaussian_spinor(c.dims_ext, 3)
+    psi, info = c.gpu.solve(eta, cfg["tol"], algo=algo, sloppy=F64)
+    assert info["status"] == 0, info
+    psi = to_np(psi).reshape(eta.shape)
+    assert true_residual(c.ref, eta, psi) <= cfg["tol"] * 1.05
+    assert abs(info["true_res"] - true_residual(c.ref, eta, psi)) < 0.2 * cfg["tol"]
+    # the solution is unique: compare with the oracle's own solve
+    ps_ref, iref = c.ref.solve(eta, cfg["tol"])
+    assert iref["status"] == 0
+    assert relerr(psi, ps_ref) < 1e-10
+    if algo == 0:
+        assert abs(info["iters"] - iref["iters"]) <= 3
+    c.close()
+
+
+@pytest.mark.parametrize("sloppy,algo", [(F32, 0), (F16, 0), (F32, 1), (F16, 1)])
+def test_solve_mixed_precision_reliable_updates(sloppy, algo):
+    """Row a7: sloppy inner iteration + fp64 reliable updates reaches the fp64 residual target."""
+    dims = (8, 4, 4, 8)
+    c = Case(dims, 3, 1, True, q=-1 / 3, kappa=0.125, csw=1.5, csw_qed=1.0, eps=0.2)
+    eta = synth.gaussian_spinor(c.dims_ext, 5)
+    psi, info = c.gpu.solve(eta, 1e-10, algo=algo, sloppy=sloppy, delta=0.1)
+    assert info["status"] == 0, info
+    assert info["n_reliable"] >= 2
+    assert true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05e-10
+    c.close()
+
+
+def test_solve_host_pointers_and_zero_source():
+    import torch
+    c = Case((4, 4, 4, 4), 0, 1, False, precisions=(F64,))
+    eta = synth.gaussian_spinor(c.dims_ext, 3)
+    eh = torch.from_numpy(eta.copy()).pin_memory()
+    ph = torch.empty_like(eh).pin_memory()
+    _, info = c.gpu.solve_host(eh, ph, 1e-12)
+    assert info["status"] == 0
+    assert true_residual(c.ref, eta, ph.numpy()) <= 1.05e-12
+    # D_w through host pointers
+    oh = torch.empty_like(eh).pin_memory()
+    c.gpu.apply_Dw_host(eh, oh, F64)
+    assert relerr(oh.numpy(), c.ref.apply_Dw(eta)) < 1e-13
+    # eta = 0 -> psi = 0, zero iterations
+    z = torch.zeros_like(eh)
+    _, info = c.gpu.solve_host(z, ph, 1e-12)
+    assert info["status"] == 0 and info["iters"] == 0
+    assert float(ph.abs().max()) == 0.0
+    c.close()
+
+
+def test_maxiter_reports_noconv_with_best_iterate():
+    c = Case((4, 4, 4, 4), 0, 1, False, precisions=(F64,))
+    eta = synth.gaussian_spinor(c.dims_ext, 3)
+    psi, info = c.gpu.solve(eta, 1e-12, maxiter=3)
+    assert info["status"] == c.B.QXD_ENOCONV and info["iters"] == 3
+    res = true_residual(c.ref, eta, to_np(psi).reshape(eta.shape))
+    assert 1e-12 < res < 1.0
+    assert abs(info["true_res"] - res) < 1e-10
+    c.close()
+
+
+def test_error_codes():
+    import torch
+    from paper_2502_02490_b200 import binding as B
+    with pytest.raises(B.QxdError):
+        B.Qxd(4, 3, 4, 4, 0)           # odd extent
+    g = B.Qxd(4, 4, 4, 4, 4, precisions=(F64,))
+    psi = torch.zeros(g.V * 12, dtype=torch.complex128, device="cuda")
+    with pytest.raises(B.QxdError) as e:
+        g.apply_Dw(psi)                 # no gauge / clover yet
+    assert e.value.status == B.QXD_ESTATE
+    g.gauge_load(synth.su3_links((4, 4, 4, 4), 0.3, 1))
+    with pytest.raises(B.QxdError) as e:
+        g.clover_build(1.5)             # no quark yet
+    assert e.value.status == B.QXD_ESTATE
+    g.set_quark(0.12)
+    g.clover_build(1.5)
+    with pytest.raises(B.QxdError) as e:
+        g.apply_Dw(psi, F32)            # precision not bound
+    assert e.value.status == B.QXD_EINVAL
+    g.close()
+
+
+# ---- full-size checks (the configuration bench.py times) ---------------------------------------------------
+@pytest.fixture(scope="module")
+def full_c3_case():
+    cfg = synth.config("c3")
+    c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32, F16), oracle_clover=False)
+    c.psi = synth.gaussian_spinor(c.dims_ext, 3)
+    yield c
+    c.close()
+
+
+@pytest.mark.parametrize("prec", [F64, F32, F16])
+def test_full_c3__size_sampled_sites(full_c3_case, prec):
+    """BASELINE config 3 (64x32^3, C*, QCD+QED; 4.19 M sites) in bench.py's launch configuration: outputs at
+    sampled sites (corners, C* boundaries, tile edges, random interior) against the oracle's per-site definition."""
+    c = full_c3_case
+    T, X1, L2, L3 = c.dims_ext
+    rng = np.random.default_rng(17)
+    coords = [(0, 0, 0, 0), (T - 1, X1 - 1, L2 - 1, L3 - 1), (T - 1, 0, 0, 0), (0, X1 // 2, 0, 0), (0, X1 // 2 - 1, L2 - 1, 0),
+              (5, X1 - 1, 0, L3 - 1), (7, 3, L2 - 1, L3 - 1), (T // 2, X1 // 2, L2 // 2, L3 // 2)]
+    coords += [tuple(int(rng.integers(0, n)) for n in c.dims_ext) for _ in range(120)]
+    sites = np.array([((x0 * X1 + x1) * L2 + x2) * L3 + x3 for x0, x1, x2, x3 in coords], dtype=np.int64)
+    exp = c.ref.apply_Dw_sites(c.psi, sites)
+    got = to_np(c.gpu.apply_Dw(c.psi, prec)).reshape(-1, 4, 3)[sites]
+    assert relerr(got, exp) < TOL[prec]
+
+
+def test_full_c3_gamma5_hermiticity_property(full_c3_case):
+    """Property that holds at any size: <phi, D psi> = <g5 D g5 phi, psi> on the full 64x64x32x32 lattice."""
+    c = full_c3_case
+    phi = synth.gaussian_spinor(c.dims_ext, 4)
+    g5 = np.array([1, 1, -1, -1])[:, None]
+    lhs = np.vdot(phi, to_np(c.gpu.apply_Dw(c.psi, F64)).reshape(phi.shape))
+    rhs = np.vdot(g5 * to_np(c.gpu.apply_Dw(g5 * phi, F64)).reshape(phi.shape), c.psi)
+    assert abs(lhs - rhs) / abs(lhs) < 1e-12
