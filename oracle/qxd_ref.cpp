@@ -89,6 +89,8 @@ struct Ref {
   std::vector<double> A;  // [V][4]     extended U(1) field
   std::vector<cd> Mb;     // [V][2][36] chirality blocks of the site matrix, row-major 6x6
   std::vector<cd> Mi;     // [V][2][36] their inverses
+  std::vector<cd> Mb_range;  // blocks of the site range [range_lo, range_hi) only (bounded-sample timing)
+  long range_lo = 0, range_hi = 0;
   double max_offdiag = 0; // largest |entry| found outside the two chirality blocks (must be ~0)
   double max_antiherm = 0;// largest |M - M^dag| entry (must be ~0)
 
@@ -472,6 +474,44 @@ int qxd_ref_apply_Dw_sites(void* h, const double* psi, long n, const long* sites
     }
   }
   return bad ? -1 : 0;
+}
+
+// ---- bounded-sample variants (bench.py cpu_baseline / --impl reference): the same per-site arithmetic as
+// qxd_ref_clover_build / qxd_ref_apply_Dw, restricted to the natural-order site range [lo, hi) so that a
+// slab of a large lattice can be timed in seconds.  The blocks are kept in a range-sized array.
+int qxd_ref_clover_build_range(void* h, double csw, double csw_qed, long lo, long hi) {
+  Ref& g = *(Ref*)h;
+  if (!g.have_gauge || !g.have_quark) return -2;
+  if (lo < 0 || hi > g.V || lo >= hi) return -1;
+  qxd_ref_set_csw(h, csw, csw_qed);
+  g.range_lo = lo; g.range_hi = hi;
+  g.Mb_range.assign((hi - lo) * 72, 0.0);
+#pragma omp parallel for schedule(static)
+  for (long s = lo; s < hi; s++) {
+    int x[4]; g.coords(s, x);
+    cd M[144]; g.site_matrix(x, M);
+    for (int c = 0; c < 2; c++) {
+      cd* b = &g.Mb_range[(s - lo) * 72 + c * 36];
+      for (int i = 0; i < 6; i++) for (int j = 0; j < 6; j++) b[i * 6 + j] = M[(6 * c + i) * 12 + 6 * c + j];
+    }
+  }
+  return 0;
+}
+// out: [(hi-lo)][4][3] complex = (D_w psi)(x) for the sites of the range built above; psi is the full field.
+int qxd_ref_apply_Dw_range(void* h, const double* psi, double* out) {
+  Ref& g = *(Ref*)h;
+  if (g.Mb_range.empty()) return -2;
+  const cd* p = (const cd*)psi; cd* o = (cd*)out;
+  const long lo = g.range_lo, hi = g.range_hi;
+#pragma omp parallel for schedule(static)
+  for (long s = lo; s < hi; s++) {
+    int x[4]; g.coords(s, x);
+    cd hp[12], dg[12];
+    hop_site(g, p, x, hp);
+    diag_site(&g.Mb_range[(s - lo) * 72], p + s * 12, dg);
+    for (int i = 0; i < 12; i++) o[(s - lo) * 12 + i] = dg[i] + hp[i];
+  }
+  return 0;
 }
 
 // Even-sublattice fields: [V/2][4][3] complex, the even sites in increasing Lambda order

@@ -43,6 +43,8 @@ def lib():
         L.qxd_ref_apply_Dw.argtypes = [vp, vp, vp]
         L.qxd_ref_apply_Dw_sites.argtypes = [vp, vp, l, vp, vp]
         L.qxd_ref_apply_Dhat.argtypes = [vp, vp, vp, i]
+        L.qxd_ref_clover_build_range.argtypes = [vp, d, d, l, l]
+        L.qxd_ref_apply_Dw_range.argtypes = [vp, vp, vp]
         L.qxd_ref_solve.argtypes = [vp, vp, vp, d, i, vp, vp]
         L.qxd_ref_num_threads.restype = i
         _lib = L
@@ -129,6 +131,19 @@ class Ref:
         sites = np.ascontiguousarray(sites, dtype=np.int64)
         out = np.empty((sites.size, 4, 3), dtype=np.complex128)
         _chk(lib().qxd_ref_apply_Dw_sites(self.h, _p(psi), sites.size, _p(sites), _p(out)), "apply_Dw_sites")
+        return out
+
+    def clover_build_range(self, csw, csw_qed, lo, hi):
+        """Clover blocks for the natural-order site range [lo, hi) only (bounded-sample timing)."""
+        _chk(lib().qxd_ref_clover_build_range(self.h, csw, csw_qed, int(lo), int(hi)), "clover_build_range")
+        self._range = (int(lo), int(hi))
+
+    def apply_Dw_range(self, psi, out=None):
+        psi = self._spinor(psi)
+        lo, hi = self._range
+        if out is None:
+            out = np.empty((hi - lo, 4, 3), dtype=np.complex128)
+        _chk(lib().qxd_ref_apply_Dw_range(self.h, _p(psi), _p(out)), "apply_Dw_range")
         return out
 
     def apply_Dhat(self, psi_e, dagger=False):

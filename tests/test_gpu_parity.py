@@ -275,7 +275,7 @@ def full_c3_case():
 
 
 @pytest.mark.parametrize("prec", [F64, F32, F16])
-def test_full_c3__size_sampled_sites(full_c3_case, prec):
+def test_full_c3_sampled_sites(full_c3_case, prec):
     """BASELINE config 3 (64x32^3, C*, QCD+QED; 4.19 M sites) in bench.py's launch configuration: outputs at
     sampled sites (corners, C* boundaries, tile edges, random interior) against the oracle's per-site definition."""
     c = full_c3_case

@@ -299,3 +299,13 @@ def test_invalid_geometry_rejected():
         R.Ref(4, 3, 4, 4, 0)
     with pytest.raises(R.RefError):
         R.Ref(4, 4, 4, 0, 0)
+
+
+def test_range_apply_equals_full_apply():
+    """The bounded-sample entry points (bench.py cpu_baseline) reproduce the full apply on their site range."""
+    r, U, A = setup_case((4, 2, 4, 4), 3, 1, True)
+    psi = synth.gaussian_spinor(r.dims_ext, 3)
+    full = r.apply_Dw(psi).reshape(-1, 4, 3)
+    lo, hi = 37, 201
+    r.clover_build_range(1.5, 1.0, lo, hi)
+    assert np.array_equal(r.apply_Dw_range(psi), full[lo:hi])
