@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the D_w hot path on seeded synthetic fields.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl reference] [--no-solve]
+
+Headline (BASELINE.json `metric`): algorithmic GB/s of one fp32 D_w apply (row a4) on BASELINE config 3
+(64x32^3 QCD+QED with C* boundaries = 64x64x32x32 extended sites).  One "step" = one D_w apply on the packed
+device layout; `value` = 768 B/site x V / time.  The same JSON line carries the fp64/fp32/fp16 sweep for D_w and
+D-hat, BLAS-1 streams, the mixed-precision solves, the end-to-end number through the host-pointer C-ABI call,
+the roofline object for the dominant kernel and the oracle timed on the host cores.
+
+Multi-GPU (torchrun): the path shards by right-hand side -- every rank holds the (replicated) gauge field and
+applies D_w to its own spinor; there is no data-path collective (weak scaling).  Only timing uses
+torch.distributed (barrier, max over ranks).
+
+`--impl reference` times the fp64 CPU oracle (oracle/, test infrastructure) on a bounded slab of the same
+workload on the host cores; it is the base contract's reference arm for this tier.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 1824                    # 1320 hopping + 504 clover
+REALS_DW = 192                          # psi 24 + 4 links x 18 + clover 72 + out 24 (row a4, 18-real links)
+REALS_DHAT = 276                        # both passes, per FULL-lattice site (row a5)
+PREC_NAME = {0: "fp64", 1: "fp32", 2: "fp16"}
+PREC_BYTES = {0: 8, 1: 4, 2: 2}
+FALLBACK_HBM_GBS = 6650.0               # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fp32 D_w kernel at c3, from the committed
+# `ncu --set full` capture (profiles/r1_dslash_fp32_full.md); None until a capture exists.
+NCU_TRAFFIC_BYTES_FP32_C3 = None
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def dw_bytes_per_site(prec):
+    b = REALS_DW * PREC_BYTES[prec]
+    if prec == 2:
+        b += 8                          # fp32 block-float scale, read with psi and written with out
+    return b
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(self.index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1]))
+                mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_fields(cfg, rank):
+    import synth
+    U = synth.su3_links(cfg["dims"], cfg["eps"], 1)
+    A = synth.u1_field(cfg["dims"], 0.3, 2) if cfg["qed"] else None
+    eta = synth.gaussian_spinor(cfg["dims_ext"], 3 + rank)   # each rank: its own right-hand side
+    return U, A, eta
+
+
+# ---------------------------------------------------------------------------------------------------------
+# reference arm: the oracle, as it stands, on the host cores
+# ---------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, U, A, psi, steps, warmup, budget_s=25.0):
+    """Times oracle D_w applies on a slab (leading time slices, natural order) of the workload.
+    Returns (sites_per_s, cores, sample description, seconds per step)."""
+    from oracle import qxd_ref as R
+    ref = R.Ref(*cfg["dims"], cfg["bc"])
+    ref.gauge_load(U, A, cfg["qel"])
+    ref.set_quark(cfg["kappa"], cfg["q"])
+    T, X1, L2, L3 = cfg["dims_ext"]
+    slice_sites = X1 * L2 * L3
+    nslices = max(1, min(T, (1 << 18) // slice_sites))    # ~262k sites per step (~0.5 s on 8 cores)
+    n = nslices * slice_sites
+    ref.clover_build_range(cfg["csw"], cfg["csw_qed"], 0, n)
+    import numpy as np
+    out = np.empty((n, 4, 3), dtype=np.complex128)
+    for _ in range(warmup):
+        ref.apply_Dw_range(psi, out)
+    times = []
+    t_start = time.perf_counter()
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        ref.apply_Dw_range(psi, out)
+        times.append(time.perf_counter() - t0)
+        if time.perf_counter() - t_start > budget_s and len(times) >= 3:
+            break
+    dt = sum(times) / len(times)
+    desc = (f"oracle qxd_ref_apply_Dw_range on the first {nslices} time slices ({n} of {ref.V} sites) of {cfg['name']}, "
+            f"{len(times)} applies, fp64, OpenMP over sites")
+    return n / dt, R.num_threads(), desc, dt, len(times)
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    U, A, psi = make_fields(cfg, 0)
+    rate, cores, desc, dt, done = oracle_sample(cfg, U, A, psi, args.steps, min(args.warmup, 2))
+    gbs = rate * dw_bytes_per_site(1) / 1e9
+    line = {
+        "impl": "reference", "metric": "Dw_apply_fp32_GBps", "value": gbs, "unit": "GB/s", "n_gpus": args.gpus, "steps": done,
+        "warmup": min(args.warmup, 2), "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["label"], "note": "sites/s of the fp64 oracle x 768 B/site (the fp32 algorithmic bytes of the CUDA arm)"},
+        "gflops": rate * FLOP_PER_SITE / 1e9,
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# CUDA arm
+# ---------------------------------------------------------------------------------------------------------
+def run_cuda(args, cfg):
+    import numpy as np
+    import torch
+    from paper_2502_02490_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the qxd hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    t_setup = time.perf_counter()
+    U, A, eta = make_fields(cfg, rank)
+    precs = (B.QXD_F64, B.QXD_F32, B.QXD_F16)
+    g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, device=f"cuda:{local}")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, n):
+        """n calls between two events on the library's stream (torch's current stream); ms per call."""
+        e0, e1 = ev(), ev()
+        torch.cuda.synchronize(dev)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        e1.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    e0, e1, e2, e3 = ev(), ev(), ev(), ev()
+    Ud = torch.from_numpy(U).to(dev)
+    Ad = torch.from_numpy(A).to(dev) if A is not None else None
+    e0.record()
+    g.gauge_load(Ud, Ad, cfg["qel"])                   # row a2
+    e1.record()
+    g.set_quark(cfg["kappa"], cfg["q"])                # hop links in 3 precisions
+    e2.record()
+    g.clover_build(cfg["csw"], cfg["csw_qed"])         # row a3
+    e3.record()
+    torch.cuda.synchronize(dev)
+    setup_ms = {"gauge_load": e0.elapsed_time(e1), "set_quark_hoplinks_x3": e1.elapsed_time(e2), "clover_build_invert": e2.elapsed_time(e3)}
+    del Ud, Ad
+    V = g.V
+    eta_d = torch.from_numpy(eta).to(dev)
+    packed = {p: (g.spinor_pack(eta_d, p), g.new_packed(p)) for p in precs}
+    setup_s = time.perf_counter() - t_setup
+
+    # ---- headline: K fp32 D_w applies, barrier + synchronize on both sides, max over ranks ---------------
+    hp = B.QXD_F32
+    pin, pout = packed[hp]
+    step = lambda: g.apply_Dw_packed(pin, pout, hp)
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = g.launch_count()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    e1.synchronize()
+    barrier()
+    launches = g.launch_count() - l0
+    ms_step = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    # keep the sampler running through the sweep below so that it sees >= a few samples under load
+    sites_per_s = world * V / (ms_step * 1e-3)
+    value = sites_per_s * dw_bytes_per_site(hp) / 1e9
+    peak, peak_src = measured_peak()
+    per_gpu_gbs = value / world
+
+    # ---- sweep: D_w and D-hat in the three storage precisions, BLAS streams (rank-local numbers) ----------
+    sweep = {}
+    nrep = max(10, min(args.steps, 50))
+    for p in precs:
+        a, b = packed[p]
+        for _ in range(3):
+            g.apply_Dw_packed(a, b, p)
+        ms = timed(lambda: g.apply_Dw_packed(a, b, p), nrep)
+        hb = g.packed_spinor_bytes(p, half_only=True)
+        for _ in range(3):
+            g.apply_Dhat_packed(a[:hb], b[:hb], p)
+        ms_hat = timed(lambda: g.apply_Dhat_packed(a[:hb], b[:hb], p), nrep)
+        ms_axpy = timed(lambda: g.blas_axpy(1e-3, a[:hb], b[:hb], p), nrep)
+        bytes_dw = dw_bytes_per_site(p) * V
+        bytes_hat = REALS_DHAT * PREC_BYTES[p] * V + (16 * V // 2 if p == 2 else 0)
+        sweep[PREC_NAME[p]] = {
+            "Dw_ms": ms, "Dw_GBps": bytes_dw / ms / 1e6, "Dw_Gflops": FLOP_PER_SITE * V / ms / 1e6, "Dw_frac_of_peak": bytes_dw / ms / 1e6 / peak,
+            "Dhat_ms": ms_hat, "Dhat_GBps": bytes_hat / ms_hat / 1e6, "Dhat_Gflops": FLOP_PER_SITE * V / ms_hat / 1e6,
+            "axpy_GBps": 3 * 24 * PREC_BYTES[p] * (V // 2) / ms_axpy / 1e6,
+        }
+    clocks = sampler.stop()
+
+    # ---- solves (rows a7, a8): fp64/fp16 and fp64/fp32 mixed CGNE, BiCGstab ------------------------------
+    solves = {}
+    if not args.no_solve:
+        psi_d = torch.empty_like(eta_d)
+        for name, algo, sl in (("cgne_fp64_fp16", B.QXD_CGNE, B.QXD_F16), ("cgne_fp64_fp32", B.QXD_CGNE, B.QXD_F32),
+                               ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32)):
+            l0 = g.launch_count()
+            _, info = g.solve(eta_d, cfg["tol"], algo=algo, sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psi_d)
+            info["launches"] = g.launch_count() - l0
+            info["tol"] = cfg["tol"]
+            solves[name] = info
+
+    # ---- end to end through the host-pointer C-ABI call (H2D + pack + apply + unpack + D2H every step) ------
+    eh = torch.from_numpy(eta).pin_memory()
+    oh = torch.empty_like(eh).pin_memory()
+    g.apply_Dw_host(eh, oh, hp)
+    n_e2e = 3
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        g.apply_Dw_host(eh, oh, hp)
+    torch.cuda.synchronize(dev)
+    barrier()
+    e2e_s = max_over_ranks((time.perf_counter() - t0) / n_e2e)
+    e2e_val = world * V * dw_bytes_per_site(hp) / e2e_s / 1e9
+    io_bytes = V * 24 * 8
+
+    # ---- CPU baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----------------------------
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rate, cores, desc, dt, done = oracle_sample(cfg, U, A, eta, 40, 1, budget_s=15.0)
+        cpu_baseline = {"value": rate * dw_bytes_per_site(hp) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": desc,
+                        "sites_per_s": rate, "gflops": rate * FLOP_PER_SITE / 1e9}
+
+    if rank == 0:
+        line = {
+            "metric": "Dw_apply_fp32_GBps", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["label"], "sites_per_gpu": V, "layout": "even-odd tiled SoA, 16-byte chunks, 18-real links",
+                       "l2": "inputs larger than L2 (fp32 working set 3.2 GB vs 126 MB), no flush", "sharding": "by right-hand side, replicated gauge field"},
+            "gflops": sites_per_s * FLOP_PER_SITE / 1e9,
+            "roofline": {"bound": "hbm", "achieved": per_gpu_gbs, "peak": peak, "unit": "GB/s", "frac": per_gpu_gbs / peak,
+                         "traffic": NCU_TRAFFIC_BYTES_FP32_C3, "peak_source": peak_src, "frac_of_nominal_8000": per_gpu_gbs / 8000.0,
+                         "kernel": "dslash_k<float, DW_FULL>", "algorithmic_bytes_per_launch": dw_bytes_per_site(hp) * V},
+            "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes, "ms_per_step": e2e_s * 1e3,
+                    "call": "qxd_apply_Dw_host (pinned host fp64 in/out)"},
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "cpu_baseline": cpu_baseline,
+            "sweep": sweep,
+            "solve": solves,
+            "setup_ms": setup_ms,
+            "setup_s_total": setup_s,
+        }
+        print(json.dumps(line), flush=True)
+    g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", default="c3")
+    ap.add_argument("--maxiter", type=int, default=20000)
+    ap.add_argument("--no-solve", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    import synth
+    cfg = synth.config(args.config)
+    cfg["name"] = args.config
+    T, L1, L2, L3 = cfg["dims"]
+    cfg["label"] = (f"{args.config}: {T}x{L1}x{L2}x{L3} {'QCD+QED' if cfg['qed'] else 'QCD'} Wilson-clover, cstar={cfg['cstar']} "
+                    f"(extended {'x'.join(map(str, cfg['dims_ext']))}), eps={cfg['eps']}, kappa={cfg['kappa']}, csw={cfg['csw']}, "
+                    f"csw_qed={cfg['csw_qed']}, q={cfg['q']:.4f}")
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_cuda(args, cfg)
+
+
+if __name__ == "__main__":
+    main()
