@@ -263,7 +263,7 @@ def run_cuda(args, cfg):
     # ---- sweep: D_w and D-hat in the three storage precisions, BLAS streams (rank-local numbers) ----------
     sweep = {}
     nrep = max(10, min(args.steps, 50))
-    for p in precs:
+    for p in (() if args.no_sweep else precs):
         a, b = packed[p]
         for _ in range(3):
             g.apply_Dw_packed(a, b, p)
@@ -297,16 +297,16 @@ def run_cuda(args, cfg):
     # ---- end to end through the host-pointer C-ABI call (H2D + pack + apply + unpack + D2H every step) ------
     eh = torch.from_numpy(eta).pin_memory()
     oh = torch.empty_like(eh).pin_memory()
+    n_e2e = 0 if args.no_e2e else 3
     g.apply_Dw_host(eh, oh, hp)
-    n_e2e = 3
     barrier()
     t0 = time.perf_counter()
     for _ in range(n_e2e):
         g.apply_Dw_host(eh, oh, hp)
     torch.cuda.synchronize(dev)
     barrier()
-    e2e_s = max_over_ranks((time.perf_counter() - t0) / n_e2e)
-    e2e_val = world * V * dw_bytes_per_site(hp) / e2e_s / 1e9
+    e2e_s = max_over_ranks((time.perf_counter() - t0) / max(n_e2e, 1))
+    e2e_val = None if args.no_e2e else world * V * dw_bytes_per_site(hp) / e2e_s / 1e9
     io_bytes = V * 24 * 8
 
     # ---- CPU baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----------------------------
@@ -352,6 +352,8 @@ def main():
     ap.add_argument("--maxiter", type=int, default=20000)
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the precision sweep (short runs under ncu)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-pointer end-to-end loop (short runs under ncu)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

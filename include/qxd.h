@@ -83,9 +83,14 @@ typedef struct {
  * All site indices are computed on the fly by pure inlined functions. */
 int qxd_geometry_create(int T, int L1, int L2, int L3, int bc, qxd_ctx** out);
 int qxd_geometry_destroy(qxd_ctx* ctx);
-/* Optional: tile extents of the device site order (powers of two dividing the extended extents,
- * b3 >= 2).  Must precede qxd_workspace_bind.  Default: chosen by the library. */
+/* Optional: the device site order (the paper's host code orders sites in cache
+ * blocks).  Tile extents b (powers of two dividing the extended extents, b3 >= 2): the
+ * sites one CTA works on.  Block extents B (powers of two, multiples of b, dividing the extents): tiles
+ * are visited block by block, blocks lexicographically with direction 0 slowest.  qxd_set_tile keeps the
+ * current block where it is still a multiple of the tile, else sets B = b.  Both must precede
+ * qxd_workspace_bind.  Default: chosen by the library.  The order only permutes sites in memory. */
 int qxd_set_tile(qxd_ctx* ctx, int b0, int b1, int b2, int b3);
+int qxd_set_block(qxd_ctx* ctx, int B0, int B1, int B2, int B3);
 /* Number of sites of the extended lattice (V). */
 long qxd_volume(const qxd_ctx* ctx);
 

@@ -38,6 +38,7 @@ SYMBOLS = {
     "qxd_geometry_create": (_i, [_i, _i, _i, _i, _i, C.POINTER(_vp)]),
     "qxd_geometry_destroy": (_i, [_vp]),
     "qxd_set_tile": (_i, [_vp, _i, _i, _i, _i]),
+    "qxd_set_block": (_i, [_vp, _i, _i, _i, _i]),
     "qxd_volume": (_l, [_vp]),
     "qxd_workspace_bytes": (_sz, [_vp, _i, _i]),
     "qxd_workspace_bind": (_i, [_vp, _vp, _sz, _i, _i]),
@@ -89,7 +90,7 @@ def _ptr(t):
 class Qxd:
     """One solver context (qxd_ctx): geometry, workspace, gauge field, quark, clover term."""
 
-    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, device="cuda:0"):
+    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0"):
         import torch
         if not torch.cuda.is_available():
             raise QxdError(QXD_ECUDA, "no CUDA device: the qxd hot path has no CPU fallback")
@@ -107,6 +108,8 @@ class Qxd:
         self.V = self.lib.qxd_volume(self.h)
         if tile is not None:
             self._chk(self.lib.qxd_set_tile(self.h, *tile))
+        if block is not None:
+            self._chk(self.lib.qxd_set_block(self.h, *block))
         self.prec_mask = 0
         for p in precisions:
             self.prec_mask |= 1 << p

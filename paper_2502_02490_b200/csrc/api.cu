@@ -19,16 +19,20 @@ int pow2_le_dividing(int extent, int target) {
 }
 int ilog2(int v) { int s = 0; while ((1 << s) < v) s++; return s; }
 
-int set_tile(qxd_ctx* c, const int b[4]) {
+int set_order(qxd_ctx* c, const int b[4], const int B[4]) {
   Geom& g = c->g;
   for (int mu = 0; mu < 4; mu++) {
     if (b[mu] < 1 || (b[mu] & (b[mu] - 1)) || g.X[mu] % b[mu]) return fail(c, QXD_EINVAL, "tile extents must be powers of two dividing the extended extents");
+    if (B[mu] < b[mu] || (B[mu] & (B[mu] - 1)) || g.X[mu] % B[mu]) return fail(c, QXD_EINVAL, "block extents must be powers of two, multiples of the tile extents, dividing the extended extents");
   }
   if (b[3] < 2) return fail(c, QXD_EINVAL, "tile extent b3 must be >= 2");
-  for (int mu = 0; mu < 4; mu++) { g.sh[mu] = ilog2(b[mu]); g.nt[mu] = g.X[mu] / b[mu]; }
-  g.lo_str[3] = 1; g.lo_str[2] = b[3]; g.lo_str[1] = b[3] * b[2]; g.lo_str[0] = b[3] * b[2] * b[1];
-  const int tv = b[0] * b[1] * b[2] * b[3];
-  g.hi_str[3] = tv; g.hi_str[2] = tv * g.nt[3]; g.hi_str[1] = tv * g.nt[3] * g.nt[2]; g.hi_str[0] = tv * g.nt[3] * g.nt[2] * g.nt[1];
+  int tv = 1, mv = 1;  // sites per tile, tiles per block
+  for (int mu = 0; mu < 4; mu++) { g.sh[mu] = ilog2(b[mu]); g.shB[mu] = ilog2(B[mu]); g.nB[mu] = g.X[mu] / B[mu]; tv *= b[mu]; mv *= B[mu] / b[mu]; }
+  g.s0[3] = 1; g.s0[2] = b[3]; g.s0[1] = b[3] * b[2]; g.s0[0] = b[3] * b[2] * b[1];
+  g.s1[3] = tv; g.s1[2] = g.s1[3] * (B[3] / b[3]); g.s1[1] = g.s1[2] * (B[2] / b[2]); g.s1[0] = g.s1[1] * (B[1] / b[1]);
+  const int bv = tv * mv;
+  g.s2[3] = bv; g.s2[2] = bv * g.nB[3]; g.s2[1] = bv * g.nB[3] * g.nB[2]; g.s2[0] = bv * g.nB[3] * g.nB[2] * g.nB[1];
+  for (int mu = 0; mu < 4; mu++) { c->tile[mu] = b[mu]; c->block[mu] = B[mu]; }
   return QXD_OK;
 }
 
@@ -97,8 +101,11 @@ int qxd_geometry_create(int T, int L1, int L2, int L3, int bc, qxd_ctx** out) {
   Geom& g = c->g;
   g.X[0] = T; g.X[1] = cstar ? 2 * L1 : L1; g.X[2] = L2; g.X[3] = L3;
   g.L1 = L1; g.cstar = cstar; g.antiper = (bc >> 2) & 1; g.Vh = int(V / 2);
-  int b[4] = {pow2_le_dividing(g.X[0], 4), pow2_le_dividing(g.X[1], 4), pow2_le_dividing(g.X[2], 4), pow2_le_dividing(g.X[3], 8)};
-  set_tile(c, b);
+  // default order: 4x4x4x4 tiles (256 sites = one CTA of the full-lattice kernel), blocks of 4 tiles stacked in time and
+  // time slabs 16 thick, so that only 1/8 of the sites have a neighbour in another slab
+  int b[4] = {pow2_le_dividing(g.X[0], 4), pow2_le_dividing(g.X[1], 4), pow2_le_dividing(g.X[2], 4), pow2_le_dividing(g.X[3], 4)};
+  int B[4] = {pow2_le_dividing(g.X[0], 16), b[1], b[2], b[3]};
+  set_order(c, b, B);
   *out = c;
   return QXD_OK;
 }
@@ -116,7 +123,16 @@ int qxd_set_tile(qxd_ctx* c, int b0, int b1, int b2, int b3) {
   if (!c) return QXD_EINVAL;
   if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_tile must precede qxd_workspace_bind");
   int b[4] = {b0, b1, b2, b3};
-  return set_tile(c, b);
+  int B[4];
+  for (int mu = 0; mu < 4; mu++) B[mu] = c->block[mu] > b[mu] && b[mu] > 0 && c->block[mu] % b[mu] == 0 ? c->block[mu] : b[mu];
+  return set_order(c, b, B);
+}
+
+int qxd_set_block(qxd_ctx* c, int B0, int B1, int B2, int B3) {
+  if (!c) return QXD_EINVAL;
+  if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_block must precede qxd_workspace_bind");
+  int B[4] = {B0, B1, B2, B3};
+  return set_order(c, c->tile, B);
 }
 
 long qxd_volume(const qxd_ctx* c) { return c ? c->V : 0; }

@@ -15,6 +15,7 @@
 //   (1 -+ gamma_k) psi = (h, -+ i s_k h),     h = psi_u +- i s_k psi_l
 // with the upper sign for the forward hop.
 #include "qxd_ctx.h"
+#include <cstdlib>
 
 namespace qxd {
 
@@ -28,6 +29,7 @@ struct DslashArgs {
   const void* W[2];
   const void* CL[2];
   int parity_out;
+  int prefetch;
   Reducer R;
 };
 
@@ -126,45 +128,130 @@ __device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const
   block_mul(b, in + 12, out + 12);
 }
 
-template <typename S, int MU, bool G5IN>
-__device__ __forceinline__ void hop_pair(const DslashArgs& a, const Site& s, int cb, int parity, typename PT<S>::C* acc) {
-  typedef typename PT<S>::C C;
+// One hop in flight: the raw 16-byte chunks of the neighbour spinor and of the link, exactly as loaded.  Keeping the
+// packed vectors (not the unpacked reals) in registers between issue and use lets two hops be in flight per thread
+// (software pipeline in hop_all below): the kernel is bound by memory latency x bytes in flight, not by arithmetic.
+template <typename S>
+struct HopRegs {
+  typedef typename PT<S>::V V;
+  static constexpr int RPC = PT<S>::RPC;
+  static constexpr int NPSI = 24 / RPC;
+  V psi[NPSI];
+  static constexpr int NWC = RPC == 2 ? 9 : RPC == 4 ? 5 : 3;
+  V w[NWC];      // chunks covering the 18 reals of one link
+  float scale;   // fp16 block-float scale of the neighbour spinor
+};
+template <int MU, typename S> struct LinkChunks {
+  static constexpr int RPC = PT<S>::RPC;
+  static constexpr int C0 = (18 * MU) / RPC, C1 = (18 * MU + 17) / RPC, N = C1 - C0 + 1, OFF = 18 * MU - C0 * RPC;
+};
+template <typename S, int MU, int DIR>
+__device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, int cb, int parity, HopRegs<S>& d) {
+  typedef typename PT<S>::V V;
+  typedef LinkChunks<MU, S> LC;
   const int Vh = a.g.Vh;
-  {  // forward: (1 - gamma_mu) W_mu(x) psi(x+mu)
-    const int nb = neighbour_cb<MU, +1>(a.g, s);
-    C psi[24], h[12], w[18], r[12];
-    load_spinor<S>(a.in[1 - parity], Vh, nb, psi);
-    if (G5IN) {
+  const int nb = neighbour_cb<MU, DIR>(a.g, s);
+  const V* p = reinterpret_cast<const V*>(a.in[1 - parity].data);
 #pragma unroll
-      for (int i = 12; i < 24; i++) psi[i] = -psi[i];
-    }
-    project<MU, +1>(psi, h);
-    load_reals<S, 18 * MU, 18>(a.W[parity], Vh, cb, w);
-    link_mul<false>(w, h, r);
-    reconstruct<MU, +1>(r, acc);
+  for (int c = 0; c < HopRegs<S>::NPSI; c++) d.psi[c] = ldg_pinned(p + size_t(c) * Vh + nb);
+  if (PT<S>::ID == 2) d.scale = ldg_pinned(a.in[1 - parity].scale + nb);
+  // forward: W_mu(x) of the own parity; backward: W_mu(x-mu) of the other parity at the neighbour
+  const V* w = reinterpret_cast<const V*>(DIR > 0 ? a.W[parity] : a.W[1 - parity]);
+  const int wi = DIR > 0 ? cb : nb;
+#pragma unroll
+  for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * Vh + wi);
+}
+template <typename S, int MU, int DIR, bool G5IN>
+__device__ __forceinline__ void hop_use(const HopRegs<S>& d, typename PT<S>::C* acc) {
+  typedef typename PT<S>::C C;
+  typedef LinkChunks<MU, S> LC;
+  constexpr int RPC = PT<S>::RPC;
+  C psi[24], h[12], wv[HopRegs<S>::NWC * RPC], r[12];
+#pragma unroll
+  for (int c = 0; c < HopRegs<S>::NPSI; c++) unpack_vec(d.psi[c], psi + c * RPC);
+  if (PT<S>::ID == 2) {
+#pragma unroll
+    for (int i = 0; i < 24; i++) psi[i] *= d.scale;
   }
-  {  // backward: (1 + gamma_mu) W_mu(x-mu)^dag psi(x-mu)
-    const int nb = neighbour_cb<MU, -1>(a.g, s);
-    C psi[24], h[12], w[18], r[12];
-    load_spinor<S>(a.in[1 - parity], Vh, nb, psi);
-    if (G5IN) {
+  if (G5IN) {
 #pragma unroll
-      for (int i = 12; i < 24; i++) psi[i] = -psi[i];
+    for (int i = 12; i < 24; i++) psi[i] = -psi[i];
+  }
+  project<MU, DIR>(psi, h);
+#pragma unroll
+  for (int c = 0; c < LC::N; c++) unpack_vec(d.w[c], wv + c * RPC);
+  link_mul<(DIR < 0)>(wv + LC::OFF, h, r);
+  reconstruct<MU, DIR>(r, acc);
+}
+// all eight hops, two in flight
+template <typename S, bool G5IN>
+__device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int cb, int parity, typename PT<S>::C* acc) {
+  HopRegs<S> d0, d1;
+  hop_issue<S, 0, +1>(a, s, cb, parity, d0);
+  hop_issue<S, 0, -1>(a, s, cb, parity, d1);
+  hop_use<S, 0, +1, G5IN>(d0, acc);
+  hop_issue<S, 1, +1>(a, s, cb, parity, d0);
+  hop_use<S, 0, -1, G5IN>(d1, acc);
+  hop_issue<S, 1, -1>(a, s, cb, parity, d1);
+  hop_use<S, 1, +1, G5IN>(d0, acc);
+  hop_issue<S, 2, +1>(a, s, cb, parity, d0);
+  hop_use<S, 1, -1, G5IN>(d1, acc);
+  hop_issue<S, 2, -1>(a, s, cb, parity, d1);
+  hop_use<S, 2, +1, G5IN>(d0, acc);
+  hop_issue<S, 3, +1>(a, s, cb, parity, d0);
+  hop_use<S, 2, -1, G5IN>(d1, acc);
+  hop_issue<S, 3, -1>(a, s, cb, parity, d1);
+  hop_use<S, 3, +1, G5IN>(d0, acc);
+  hop_use<S, 3, -1, G5IN>(d1, acc);
+}
+
+// Bulk L2 prefetch (cp.async.bulk.prefetch.L2, sm_90+): the compulsory DRAM streams of a CTA -- its own links, its
+// clover blocks and its own spinors -- are contiguous 16 B x 128-site rows of the chunk-major SoA records.  One thread per
+// row asks the L2 for the whole row when the CTA starts, so the per-thread 16-byte loads that follow (one hop after the
+// other, bounded by registers) find their lines in L2 or already in flight instead of paying one DRAM latency per hop.
+__device__ __forceinline__ void bulk_prefetch_l2(const void* p, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+template <typename S, int PHI, bool FULL>
+__device__ __forceinline__ void cta_prefetch(const DslashArgs& a, int cb0) {
+  constexpr int NW = 72 / PT<S>::RPC, NS = 24 / PT<S>::RPC;   // rows per parity: links, clover (NW each), spinor (NS)
+  const int Vh = a.g.Vh;
+  const int n = min(128, Vh - cb0);
+  if (n <= 0) return;
+  const unsigned bytes = unsigned(n) * 16u;
+  const int t = threadIdx.x;
+  if (FULL) {
+    // rows: [parity][W NW | CL NW | psi NS]
+    constexpr int PER = 2 * NW + NS;
+    if (t < 2 * PER) {
+      const int p = t / PER, r = t % PER;
+      const char* base = r < NW ? (const char*)a.W[p] : r < 2 * NW ? (const char*)a.CL[p] : (const char*)a.in[p].data;
+      const int c = r < NW ? r : r < 2 * NW ? r - NW : r - 2 * NW;
+      bulk_prefetch_l2(base + (size_t(c) * Vh + cb0) * 16, bytes);
     }
-    project<MU, -1>(psi, h);
-    load_reals<S, 18 * MU, 18>(a.W[1 - parity], Vh, nb, w);
-    link_mul<true>(w, h, r);
-    reconstruct<MU, -1>(r, acc);
+  } else {
+    // own forward links, clover (or inverse) block, phi
+    constexpr int PER = 2 * NW + (PHI ? NS : 0);
+    if (t < PER) {
+      const int p = a.parity_out;
+      const char* base = t < NW ? (const char*)a.W[p] : t < 2 * NW ? (const char*)a.CL[p] : (const char*)a.phi.data;
+      const int c = t < NW ? t : t < 2 * NW ? t - NW : t - 2 * NW;
+      bulk_prefetch_l2(base + (size_t(c) * Vh + cb0) * 16, bytes);
+    }
   }
 }
 
 // PHI: 0 none, 1 phi, 2 M*phi (FULL: phi = in on the own parity).  POST: 1 = multiply the result by M^{-1}.
+// Full-lattice launches (row a4) put both parities of 128 consecutive checkerboard indices -- one 4x4x4x4 tile with
+// the default order -- into one CTA of 256 threads (warps 0-3 even, 4-7 odd): every link is then used twice by the same
+// CTA (forward hop of x, backward hop of x+mu) and 3/4 of the neighbour spinors belong to the CTA's own tile.
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL>
-__global__ void __launch_bounds__(128) dslash_k(const __grid_constant__ DslashArgs a) {
+__global__ void __launch_bounds__(FULL ? 256 : 128, sizeof(S) == 8 ? 1 : (FULL ? 2 : 4)) dslash_k(const __grid_constant__ DslashArgs a) {
   typedef typename PT<S>::C C;
   const int Vh = a.g.Vh;
-  const int cb = blockIdx.x * blockDim.x + threadIdx.x;
-  const int parity = FULL ? blockIdx.y : a.parity_out;
+  const int cb = blockIdx.x * 128 + (threadIdx.x & 127);
+  const int parity = FULL ? (threadIdx.x >> 7) : a.parity_out;
+  if (a.prefetch) cta_prefetch<S, PHI, FULL>(a, blockIdx.x * 128);
   double nrm[1] = {0.0};
   if (cb < Vh) {
     Site s;
@@ -172,10 +259,7 @@ __global__ void __launch_bounds__(128) dslash_k(const __grid_constant__ DslashAr
     C acc[24];
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[i] = 0;
-    hop_pair<S, 0, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
-    hop_pair<S, 1, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
-    hop_pair<S, 2, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
-    hop_pair<S, 3, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
+    hop_all<S, (FLAGS & DSF_G5IN) != 0>(a, s, cb, parity, acc);
     const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[i] *= ((FLAGS & DSF_G5HOP) && i >= 12) ? -hs : hs;
@@ -220,8 +304,8 @@ __global__ void __launch_bounds__(128) clover_apply_k(int Vh, const void* CL, Sp
 
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL>
 void launch_one(qxd_ctx* c, const DslashArgs& a) {
-  dim3 gr((c->g.Vh + 127) / 128, FULL ? 2 : 1);
-  dslash_k<S, PHI, POST, NEG, FLAGS, FULL><<<gr, 128, 0, c->stream>>>(a);
+  dim3 gr((c->g.Vh + 127) / 128);
+  dslash_k<S, PHI, POST, NEG, FLAGS, FULL><<<gr, FULL ? 256 : 128, 0, c->stream>>>(a);
 }
 
 template <typename S>
@@ -266,6 +350,7 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.CL[0] = inv ? c->Mi[d.prec][0] : c->M[d.prec][0];
   a.CL[1] = inv ? c->Mi[d.prec][1] : c->M[d.prec][1];
   a.parity_out = d.parity_out;
+  { static const int pf = getenv("QXD_PREFETCH") ? atoi(getenv("QXD_PREFETCH")) : 0; a.prefetch = pf; }
   a.R.partials = c->partials; a.R.ticket = c->ticket; a.R.result = d.norm_result;
   int rc = d.prec == 0 ? dispatch<double>(c, d, a) : d.prec == 1 ? dispatch<float>(c, d, a) : dispatch<__half>(c, d, a);
   if (rc) return rc;

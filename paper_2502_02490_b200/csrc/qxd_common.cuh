@@ -17,37 +17,49 @@ struct Geom {
   int cstar;       // 0..3
   int antiper;     // fermions antiperiodic in time
   int Vh;          // V/2 = sites per parity = stride of every SoA record
-  int sh[4];       // log2 of the tile extents b_mu (sh[3] >= 1)
-  int lo_str[4];   // stride of the in-tile digit of direction mu (full-index units)
-  int hi_str[4];   // stride of the tile digit of direction mu
-  int nt[4];       // tiles per direction
+  // Three-level site order (all extents powers of two except the number of blocks per direction):
+  //   level 0  tile  b_mu  -- the sites one CTA works on (both parities), lexicographic, x3 fastest;
+  //   level 1  block B_mu  -- B/b tiles, lexicographic; consecutive CTAs stay inside one block, so that
+  //                           neighbour spinors and the second use of every link are L2 hits;
+  //   level 2  blocks      -- lexicographic over X/B blocks, direction 0 slowest.
+  int sh[4];       // log2 b_mu (sh[3] >= 1)
+  int shB[4];      // log2 B_mu (>= sh)
+  int s0[4];       // stride of the in-tile digit of direction mu (full-index units)
+  int s1[4];       // stride of the tile-in-block digit
+  int s2[4];       // stride of the block digit
+  int nB[4];       // blocks per direction
 };
 
 // full index idx2(x) = sum_mu g_mu(x_mu); checkerboard index cb = idx2 >> 1; parity = sum x_mu & 1.
 __host__ __device__ __forceinline__ int gmu(const Geom& g, int mu, int c) {
-  return (c & ((1 << g.sh[mu]) - 1)) * g.lo_str[mu] + (c >> g.sh[mu]) * g.hi_str[mu];
+  return (c & ((1 << g.sh[mu]) - 1)) * g.s0[mu] + ((c & ((1 << g.shB[mu]) - 1)) >> g.sh[mu]) * g.s1[mu] + (c >> g.shB[mu]) * g.s2[mu];
 }
 __host__ __device__ __forceinline__ int idx2_of(const Geom& g, const int x[4]) {
   return gmu(g, 0, x[0]) + gmu(g, 1, x[1]) + gmu(g, 2, x[2]) + gmu(g, 3, x[3]);
 }
 // inverse: (cb, parity) -> coordinates
 __host__ __device__ __forceinline__ void coords_of(const Geom& g, int cb, int parity, int x[4]) {
-  const int tsh = g.sh[0] + g.sh[1] + g.sh[2] + g.sh[3] - 1;  // log2(tile volume / 2)
-  int tile = cb >> tsh;
+  const int tsh = g.sh[0] + g.sh[1] + g.sh[2] + g.sh[3] - 1;                            // log2(tile volume / 2)
+  const int d3 = g.shB[3] - g.sh[3], d2 = g.shB[2] - g.sh[2], d1 = g.shB[1] - g.sh[1], d0 = g.shB[0] - g.sh[0];
   int r = cb & ((1 << tsh) - 1);
+  int n = cb >> tsh;                                                                     // tile number
   int zh = r & ((1 << (g.sh[3] - 1)) - 1); r >>= (g.sh[3] - 1);
   int yl = r & ((1 << g.sh[2]) - 1); r >>= g.sh[2];
   int xl = r & ((1 << g.sh[1]) - 1); r >>= g.sh[1];
   int tl = r;
-  int tz = tile % g.nt[3]; tile /= g.nt[3];
-  int ty = tile % g.nt[2]; tile /= g.nt[2];
-  int tx = tile % g.nt[1];
-  int tt = tile / g.nt[1];
-  x[0] = (tt << g.sh[0]) | tl;
-  x[1] = (tx << g.sh[1]) | xl;
-  x[2] = (ty << g.sh[2]) | yl;
+  int mz = n & ((1 << d3) - 1); n >>= d3;
+  int my = n & ((1 << d2) - 1); n >>= d2;
+  int mx = n & ((1 << d1) - 1); n >>= d1;
+  int mt = n & ((1 << d0) - 1); n >>= d0;                                                // n = block number
+  int bz = n % g.nB[3]; n /= g.nB[3];
+  int by = n % g.nB[2]; n /= g.nB[2];
+  int bx = n % g.nB[1];
+  int bt = n / g.nB[1];
+  x[0] = (bt << g.shB[0]) | (mt << g.sh[0]) | tl;
+  x[1] = (bx << g.shB[1]) | (mx << g.sh[1]) | xl;
+  x[2] = (by << g.shB[2]) | (my << g.sh[2]) | yl;
   int zb = (parity + x[0] + x[1] + x[2]) & 1;
-  x[3] = (tz << g.sh[3]) | (zh << 1) | zb;
+  x[3] = (bz << g.shB[3]) | (mz << g.sh[3]) | (zh << 1) | zb;
 }
 // natural (application) order, Eq. (1) PAPER.md:93 with L1 -> X1
 __host__ __device__ __forceinline__ long lex_of(const Geom& g, const int x[4]) {
@@ -126,6 +138,29 @@ __device__ __forceinline__ uint4 pack_vec(const float* o, uint4*) {
   __half2* h = reinterpret_cast<__half2*>(&v);
 #pragma unroll
   for (int i = 0; i < 4; i++) h[i] = __floats2half2_rn(o[2 * i], o[2 * i + 1]);
+  return v;
+}
+
+// Read-only 16-byte loads as volatile asm: the issue order written in the kernels (software-pipelined batches)
+// is the order the compiler keeps; plain __ldg loads get sunk towards their use to save registers.
+__device__ __forceinline__ double2 ldg_pinned(const double2* p) {
+  double2 v;
+  asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ float4 ldg_pinned(const float4* p) {
+  float4 v;
+  asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint4 ldg_pinned(const uint4* p) {
+  uint4 v;
+  asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ float ldg_pinned(const float* p) {
+  float v;
+  asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
   return v;
 }
 

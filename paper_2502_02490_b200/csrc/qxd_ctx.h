@@ -30,6 +30,7 @@ struct Scalars;  // device-resident solver scalars (solver.cu)
 struct qxd_ctx {
   qxd::Geom g;
   int T, L1, L2, L3, bc;
+  int tile[4] = {1, 1, 1, 2}, block[4] = {1, 1, 1, 2};
   long V;
   cudaStream_t stream = 0;
   // workspace
