@@ -93,6 +93,14 @@ int qxd_set_tile(qxd_ctx* ctx, int b0, int b1, int b2, int b3);
 int qxd_set_block(qxd_ctx* ctx, int B0, int B1, int B2, int B3);
 /* Number of sites of the extended lattice (V). */
 long qxd_volume(const qxd_ctx* ctx);
+/* Introspection of the device site order (host-only, no GPU needed; used by the CPU tests of row a1).
+ * qxd_site_index: extended coordinates x[4] -> checkerboard index cb in [0,V/2) and parity (sum of coordinates mod 2).
+ * qxd_site_coords: the inverse.  qxd_site_neighbour: checkerboard index (of the opposite parity) of x + dir*mu-hat,
+ * dir = +1/-1, with the boundary rules of reading R8 (shifted C* boundaries); the same inlined
+ * function the kernels use.  All return QXD_EINVAL on out-of-range arguments. */
+int qxd_site_index(const qxd_ctx* ctx, const int x[4], int* cb, int* parity);
+int qxd_site_coords(const qxd_ctx* ctx, int cb, int parity, int x[4]);
+int qxd_site_neighbour(const qxd_ctx* ctx, int cb, int parity, int mu, int dir, int* cb_nb);
 
 /* ---- workspace and stream --------------------------------------------------------------------
  * prec_mask: OR of QXD_PREC_MASK(p) for every precision that will be used (QXD_F64 is always

@@ -40,6 +40,9 @@ SYMBOLS = {
     "qxd_set_tile": (_i, [_vp, _i, _i, _i, _i]),
     "qxd_set_block": (_i, [_vp, _i, _i, _i, _i]),
     "qxd_volume": (_l, [_vp]),
+    "qxd_site_index": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)]),
+    "qxd_site_coords": (_i, [_vp, _i, _i, C.POINTER(_i)]),
+    "qxd_site_neighbour": (_i, [_vp, _i, _i, _i, _i, C.POINTER(_i)]),
     "qxd_workspace_bytes": (_sz, [_vp, _i, _i]),
     "qxd_workspace_bind": (_i, [_vp, _vp, _sz, _i, _i]),
     "qxd_set_stream": (_i, [_vp, _vp]),

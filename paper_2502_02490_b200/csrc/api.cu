@@ -137,6 +137,35 @@ int qxd_set_block(qxd_ctx* c, int B0, int B1, int B2, int B3) {
 
 long qxd_volume(const qxd_ctx* c) { return c ? c->V : 0; }
 
+int qxd_site_index(const qxd_ctx* c, const int x[4], int* cb, int* parity) {
+  if (!c || !x || !cb || !parity) return QXD_EINVAL;
+  for (int mu = 0; mu < 4; mu++) if (x[mu] < 0 || x[mu] >= c->g.X[mu]) return QXD_EINVAL;
+  *cb = idx2_of(c->g, x) >> 1;
+  *parity = (x[0] + x[1] + x[2] + x[3]) & 1;
+  return QXD_OK;
+}
+int qxd_site_coords(const qxd_ctx* c, int cb, int parity, int x[4]) {
+  if (!c || !x || cb < 0 || cb >= c->g.Vh || parity < 0 || parity > 1) return QXD_EINVAL;
+  coords_of(c->g, cb, parity, x);
+  return QXD_OK;
+}
+int qxd_site_neighbour(const qxd_ctx* c, int cb, int parity, int mu, int dir, int* cb_nb) {
+  if (!c || !cb_nb || cb < 0 || cb >= c->g.Vh || parity < 0 || parity > 1 || mu < 0 || mu > 3 || (dir != 1 && dir != -1)) return QXD_EINVAL;
+  Site s;
+  site_init(c->g, cb, parity, s);
+  switch (mu * 2 + (dir > 0 ? 0 : 1)) {
+    case 0: *cb_nb = neighbour_cb<0, +1>(c->g, s); break;
+    case 1: *cb_nb = neighbour_cb<0, -1>(c->g, s); break;
+    case 2: *cb_nb = neighbour_cb<1, +1>(c->g, s); break;
+    case 3: *cb_nb = neighbour_cb<1, -1>(c->g, s); break;
+    case 4: *cb_nb = neighbour_cb<2, +1>(c->g, s); break;
+    case 5: *cb_nb = neighbour_cb<2, -1>(c->g, s); break;
+    case 6: *cb_nb = neighbour_cb<3, +1>(c->g, s); break;
+    default: *cb_nb = neighbour_cb<3, -1>(c->g, s); break;
+  }
+  return QXD_OK;
+}
+
 size_t qxd_workspace_bytes(const qxd_ctx* c, int prec_mask, int nrhs) {
   if (!c || nrhs < 1) return 0;
   return carve(const_cast<qxd_ctx*>(c), nullptr, (prec_mask | 1) & 7, nrhs, false);

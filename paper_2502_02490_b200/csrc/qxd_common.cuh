@@ -72,7 +72,7 @@ struct Site {
   int gx[4];
   int idx2;
 };
-__device__ __forceinline__ void site_init(const Geom& g, int cb, int parity, Site& s) {
+__host__ __device__ __forceinline__ void site_init(const Geom& g, int cb, int parity, Site& s) {
   coords_of(g, cb, parity, s.x);
 #pragma unroll
   for (int mu = 0; mu < 4; mu++) s.gx[mu] = gmu(g, mu, s.x[mu]);
@@ -82,7 +82,7 @@ __device__ __forceinline__ void site_init(const Geom& g, int cb, int parity, Sit
 // periodic (X1 = 2 L1 under C*), directions k in 2..cstar wrap with the shift x1 -> x1 + L1 mod 2 L1
 // ("shifted boundaries").  The neighbour has the opposite parity.
 template <int MU, int DIR>
-__device__ __forceinline__ int neighbour_cb(const Geom& g, const Site& s) {
+__host__ __device__ __forceinline__ int neighbour_cb(const Geom& g, const Site& s) {
   int c = s.x[MU] + DIR;
   bool wrap = false;
   if (DIR > 0) { if (c >= g.X[MU]) { c = 0; wrap = true; } }

@@ -1,0 +1,96 @@
+"""CPU-only checks of the C-ABI library (no compute calls, no GPU): it loads, exports every symbol that
+include/qxd.h declares, rejects bad geometry, and its on-the-fly site order (PAPER.md:97,105,
+137-139) is a bijection whose neighbour function agrees with an independent numpy neighbour table."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import lattice_np as LN
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2502_02490_b200 import build, binding
+    build.build()
+    return binding.load_library()
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "qxd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(qxd_[a-z0-9_A-Z]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported_and_bound(lib):
+    from paper_2502_02490_b200 import binding
+    names = declared_functions()
+    assert len(names) >= 25
+    for n in names:
+        assert hasattr(lib, n), f"libqxd.so does not export {n}"
+        assert n in binding.SYMBOLS, f"binding.py does not declare {n}"
+    assert set(binding.SYMBOLS) == set(names)
+    assert lib.qxd_version().decode().startswith("qxd-b200")
+
+
+def test_geometry_argument_checks(lib):
+    h = C.c_void_p()
+    for bad in ((3, 4, 4, 4, 0), (4, 4, 4, 0, 0), (4, 2, 4, 5, 1), (4, 4, 4, 4, 8), (4, 4, 4, 4, -1)):
+        assert lib.qxd_geometry_create(*bad, C.byref(h)) == -1 and not h.value
+    assert lib.qxd_geometry_create(4, 2, 2, 6, 3 | 4, C.byref(h)) == 0
+    assert lib.qxd_volume(h) == 4 * 4 * 2 * 6
+    assert lib.qxd_set_tile(h, 2, 2, 2, 1) == -1           # b3 must be >= 2
+    assert lib.qxd_set_tile(h, 3, 2, 2, 2) == -1           # not a power of two
+    assert lib.qxd_set_tile(h, 2, 2, 2, 2) == 0
+    assert lib.qxd_workspace_bytes(h, 1, 1) > 0
+    assert lib.qxd_workspace_bytes(h, 7, 1) > lib.qxd_workspace_bytes(h, 1, 1)
+    # state errors need no GPU: nothing is bound yet
+    assert lib.qxd_set_quark(h, 0.12, 0.0) == -2
+    assert lib.qxd_clover_build(h, 1.0, 0.0) == -2
+    assert lib.qxd_geometry_destroy(h) == 0
+
+
+@pytest.mark.parametrize("dims,cstar,tile,block", [
+    ((4, 4, 4, 4), 0, None, None),
+    ((8, 4, 4, 8), 3, None, None),
+    ((8, 2, 6, 4), 2, (2, 2, 2, 4), (4, 4, 2, 4)),
+    ((16, 4, 4, 4), 1, (4, 4, 4, 4), (16, 4, 4, 4)),
+    ((6, 2, 2, 2), 3, None, None),
+])
+def test_site_order_bijection_and_neighbours(lib, dims, cstar, tile, block):
+    h = C.c_void_p()
+    assert lib.qxd_geometry_create(*dims, cstar | 4, C.byref(h)) == 0
+    if tile:
+        assert lib.qxd_set_tile(h, *tile) == 0
+    if block:
+        assert lib.qxd_set_block(h, *block) == 0
+    lat = LN.Lattice(*dims, cstar=cstar)
+    V = lat.V
+    assert lib.qxd_volume(h) == V
+    I4 = C.c_int * 4
+    cb, par, nb = C.c_int(), C.c_int(), C.c_int()
+    index = np.empty((V, 2), dtype=np.int64)
+    for s in range(V):
+        x = I4(*[int(v) for v in lat.coords[s]])
+        assert lib.qxd_site_index(h, x, C.byref(cb), C.byref(par)) == 0
+        index[s] = (cb.value, par.value)
+        y = I4()
+        assert lib.qxd_site_coords(h, cb.value, par.value, y) == 0
+        assert list(y) == list(x)
+    assert np.array_equal(index[:, 1], lat.parity)                       # parity from extended coordinates
+    for p in (0, 1):                                                     # each parity fills [0, V/2) exactly once
+        assert sorted(index[index[:, 1] == p, 0]) == list(range(V // 2))
+    for s in range(V):
+        for mu in range(4):
+            for d, step in enumerate((+1, -1)):
+                assert lib.qxd_site_neighbour(h, int(index[s, 0]), int(index[s, 1]), mu, step, C.byref(nb)) == 0
+                t = lat.nbr[mu, d, s]
+                assert index[t, 1] == 1 - index[s, 1]
+                assert nb.value == index[t, 0], (s, mu, step)
+    assert lib.qxd_site_neighbour(h, 0, 0, 4, 1, C.byref(nb)) == -1
+    assert lib.qxd_site_coords(h, V // 2, 0, I4()) == -1
+    lib.qxd_geometry_destroy(h)
