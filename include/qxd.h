@@ -143,6 +143,16 @@ int qxd_apply_Dw_host(qxd_ctx* ctx, int prec, const double* psi_host, double* ou
 int qxd_solve(qxd_ctx* ctx, const double* eta, double* psi, double tol, qxd_solve_info* info);
 int qxd_solve_host(qxd_ctx* ctx, const double* eta_host, double* psi_host, double tol, qxd_solve_info* info);
 
+/* ---- batched solve (rows a7 + a10; "for many right-hand sides"; BASELINE config 4) -------------------
+ * nrhs (<= the nrhs the workspace was bound with, <= 64) systems with the same operator: eta, psi are DEVICE arrays
+ * [nrhs][V][4][3] complex fp64 in natural order (psi may be the same buffer as eta).  The CG iterations on the normal
+ * equations run in lockstep so that every sloppy operator application is ONE multi-RHS dslash launch that reads each
+ * link and clover block once for all right-hand sides; each system has its own scalars and reliable updates and is
+ * frozen once its fp64 residual meets tol.  info: array of nrhs entries; algo (QXD_CGNE only), sloppy, delta, maxiter
+ * are read from info[0]; every entry receives that system's iters, n_reliable, true_res (seconds = whole call).
+ * Returns QXD_ENOCONV if any system missed tol (its best iterate and true residual are still returned). */
+int qxd_solve_multi(qxd_ctx* ctx, int nrhs, const double* eta, double* psi, double tol, qxd_solve_info* info);
+
 /* ---- packed-layout entry points (row a9; benchmark and building blocks) ---------------------------
  * Packed spinors: parity 0 (even) half followed by the parity 1 half; `half_only` != 0 gives the size
  * of one parity.  For QXD_F16 each half is 24 binary16 per site plus one fp32 scale per site. */
@@ -151,6 +161,11 @@ int qxd_spinor_pack(qxd_ctx* ctx, int prec, const double* nat /*DEVICE [V][4][3]
 int qxd_spinor_unpack(qxd_ctx* ctx, int prec, const void* packed, double* nat);
 int qxd_apply_Dw_packed(qxd_ctx* ctx, int prec, const void* in, void* out);
 int qxd_apply_Dhat_packed(qxd_ctx* ctx, int prec, const void* in_e, void* out_e, int dagger);
+/* Multi-RHS D_w (row a10): in/out hold nrhs packed full-lattice spinors back to back, qxd_packed_spinor_bytes(prec,0)
+ * apart.  One launch; every thread applies its site's links and clover blocks to r right-hand sides
+ * (qxd_set_rhs_per_thread: 0 = library default, 1..3; fp64 always runs one right-hand side per thread). */
+int qxd_apply_Dw_multi_packed(qxd_ctx* ctx, int prec, int nrhs, const void* in, void* out);
+int qxd_set_rhs_per_thread(qxd_ctx* ctx, int r);
 
 /* ---- BLAS-1 on packed half-lattice spinors (row a6) ---------------------------------------------
  * y <- a*x + y ;  returns <x,y> = sum conj(x) y  and  |x|^2 (fp64 accumulation, HOST results). */

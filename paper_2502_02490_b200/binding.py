@@ -55,6 +55,9 @@ SYMBOLS = {
     "qxd_apply_Dw_host": (_i, [_vp, _i, _vp, _vp]),
     "qxd_solve": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_solve_host": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
+    "qxd_solve_multi": (_i, [_vp, _i, _vp, _vp, _d, C.POINTER(SolveInfo)]),
+    "qxd_apply_Dw_multi_packed": (_i, [_vp, _i, _i, _vp, _vp]),
+    "qxd_set_rhs_per_thread": (_i, [_vp, _i]),
     "qxd_packed_spinor_bytes": (_sz, [_vp, _i, _i]),
     "qxd_spinor_pack": (_i, [_vp, _i, _vp, _vp]),
     "qxd_spinor_unpack": (_i, [_vp, _i, _vp, _vp]),
@@ -224,6 +227,26 @@ class Qxd:
         info = self._info(algo, sloppy, delta, maxiter)
         rc = self._chk(self.lib.qxd_solve(self.h, _ptr(eta), _ptr(psi), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
         return psi, self._report(rc, info)
+
+    def solve_multi(self, eta, tol, sloppy=QXD_F32, delta=0.0, maxiter=0, psi=None):
+        """eta: [nrhs, T, X1, L2, L3, 4, 3] complex128 (device).  Returns psi and one report per right-hand side."""
+        torch = self.torch
+        eta = self._dev(eta, torch.complex128)
+        nrhs = eta.numel() // (self.V * 12)
+        assert nrhs * self.V * 12 == eta.numel() and nrhs >= 1
+        if psi is None:
+            psi = torch.empty_like(eta)
+        infos = (SolveInfo * nrhs)()
+        infos[0].algo, infos[0].sloppy, infos[0].delta, infos[0].maxiter = QXD_CGNE, sloppy, delta, maxiter
+        rc = self._chk(self.lib.qxd_solve_multi(self.h, nrhs, _ptr(eta), _ptr(psi), float(tol), infos), allow=(QXD_ENOCONV,))
+        return psi, [self._report(rc, infos[k]) for k in range(nrhs)]
+
+    def set_rhs_per_thread(self, r):
+        self._chk(self.lib.qxd_set_rhs_per_thread(self.h, int(r)))
+
+    def apply_Dw_multi_packed(self, pin, pout, prec, nrhs):
+        self._chk(self.lib.qxd_apply_Dw_multi_packed(self.h, prec, int(nrhs), _ptr(pin), _ptr(pout)))
+        return pout
 
     def solve_host(self, eta_host, psi_host, tol, algo=QXD_CGNE, sloppy=QXD_F64, delta=0.0, maxiter=0):
         assert eta_host.device.type == "cpu" and psi_host.device.type == "cpu"

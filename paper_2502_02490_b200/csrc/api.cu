@@ -49,7 +49,6 @@ struct Carver {
 
 // One layout routine serves both the size query (base == nullptr) and the binding.
 size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
-  (void)nrhs;
   const size_t Vh = c->g.Vh;
   Carver k(base);
   void* Ug[2]; void* Ag[2]; void* W[NPREC][2] = {}; void* M[NPREC][2] = {}; void* Mi[NPREC][2] = {};
@@ -66,10 +65,26 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
   void* na = k.take(size_t(c->V) * 24 * 8);
   void* nb = k.take(size_t(c->V) * 24 * 8);
   const int max_blocks = int((Vh + 127) / 128) * 2 + 8;
-  void* partials = k.take(size_t(max_blocks) * 4 * 8);
+  void* partials = k.take(size_t(max_blocks) * 4 * 8 * nrhs);
   void* ticket = k.take(256);
   void* scal = k.take(64 * 8);
+  // batch vectors (row a10): fp64 b, x and five sloppy vectors per right-hand side; the sloppy ones are sized for the
+  // widest bound precision below fp64 (fp64 itself if no other is bound)
+  void* mhi[2] = {}; void* mlo[5] = {};
+  const size_t mlo_size = (prec_mask & 2) ? 4 : (prec_mask & 4) ? 2 : 8;
+  void* mscal = nullptr; void* mact = nullptr;
+  if (nrhs > 1) {
+    const int plo = mlo_size == 8 ? 0 : mlo_size == 4 ? 1 : 2;
+    const size_t lo = (half_bytes(plo, Vh) + 255) & ~size_t(255);
+    for (int i = 0; i < 2; i++) mhi[i] = k.take(half_bytes(0, Vh) * nrhs);
+    for (int i = 0; i < 5; i++) mlo[i] = k.take(lo * nrhs);
+    mscal = k.take(64 * 8 * 8);
+    mact = k.take(64 * 8);
+  }
   if (assign) {
+    for (int i = 0; i < 2; i++) c->mhi[i] = mhi[i];
+    for (int i = 0; i < 5; i++) c->mlo[i] = mlo[i];
+    c->mlo_size = nrhs > 1 ? mlo_size : 0; c->mscal = (double*)mscal; c->mact = (double*)mact;
     for (int p = 0; p < 2; p++) { c->Ug[p] = Ug[p]; c->Ag[p] = Ag[p]; }
     for (int pr = 0; pr < NPREC; pr++) for (int p = 0; p < 2; p++) { c->W[pr][p] = W[pr][p]; c->M[pr][p] = M[pr][p]; c->Mi[pr][p] = Mi[pr][p]; }
     for (int i = 0; i < 12; i++) c->sp64[i] = sp64[i];
@@ -167,12 +182,12 @@ int qxd_site_neighbour(const qxd_ctx* c, int cb, int parity, int mu, int dir, in
 }
 
 size_t qxd_workspace_bytes(const qxd_ctx* c, int prec_mask, int nrhs) {
-  if (!c || nrhs < 1) return 0;
+  if (!c || nrhs < 1 || nrhs > 64) return 0;
   return carve(const_cast<qxd_ctx*>(c), nullptr, (prec_mask | 1) & 7, nrhs, false);
 }
 
 int qxd_workspace_bind(qxd_ctx* c, void* dev, size_t bytes, int prec_mask, int nrhs) {
-  if (!c || nrhs < 1) return QXD_EINVAL;
+  if (!c || nrhs < 1 || nrhs > 64) return QXD_EINVAL;
   prec_mask = (prec_mask | 1) & 7;
   if (!dev || (reinterpret_cast<uintptr_t>(dev) & 255)) return fail(c, QXD_EWORKSPACE, "workspace must be a 256-byte aligned device pointer");
   const size_t need = carve(c, nullptr, prec_mask, nrhs, false);
@@ -180,7 +195,11 @@ int qxd_workspace_bind(qxd_ctx* c, void* dev, size_t bytes, int prec_mask, int n
   c->ws = static_cast<char*>(dev); c->ws_bytes = bytes; c->prec_mask = prec_mask; c->nrhs = nrhs;
   c->ws_used = carve(c, c->ws, prec_mask, nrhs, true);
   c->have_gauge = c->have_quark = c->have_clover = false;
-  if (!c->h_scal) QXD_CUDA_OK(c, cudaMallocHost((void**)&c->h_scal, 64 * sizeof(double)));
+  if (!c->h_scal) {
+    QXD_CUDA_OK(c, cudaMallocHost((void**)&c->h_scal, (64 + 64 * 8 + 64) * sizeof(double)));
+    c->h_mscal = c->h_scal + 64; c->h_mact = c->h_mscal + 64 * 8;
+  }
+  if (c->mscal) QXD_CUDA_OK(c, cudaMemsetAsync(c->mscal, 0, 64 * 8 * 8, c->stream));
   if (!c->ev0) QXD_CUDA_OK(c, cudaEventCreate(&c->ev0));
   if (!c->ev1) QXD_CUDA_OK(c, cudaEventCreate(&c->ev1));
   QXD_CUDA_OK(c, cudaMemsetAsync(c->ticket, 0, 256, c->stream));
@@ -252,6 +271,26 @@ int qxd_apply_Dw_packed(qxd_ctx* c, int prec, const void* in, void* out) {
   return launch_dslash(c, d);
 }
 
+int qxd_apply_Dw_multi_packed(qxd_ctx* c, int prec, int nrhs, const void* in, void* out) {
+  int rc = check_apply(c, prec, in, out, "apply_Dw_multi_packed");
+  if (rc) return rc;
+  if (nrhs < 1 || nrhs > 64) return fail(c, QXD_EINVAL, "apply_Dw_multi_packed: nrhs must be in 1..64");
+  if (size_t(c->max_blocks) * 4 * c->nrhs < size_t(nrhs)) return fail(c, QXD_EINVAL, "apply_Dw_multi_packed: nrhs exceeds the bound workspace");
+  const int Vh = c->g.Vh;
+  DslashCall d{};
+  d.prec = prec; d.mode = DS_DW_FULL; d.flags = 0;
+  d.in[0] = half_view(prec, const_cast<void*>(in), Vh, 0); d.in[1] = half_view(prec, const_cast<void*>(in), Vh, 1);
+  d.out[0] = half_view(prec, out, Vh, 0); d.out[1] = half_view(prec, out, Vh, 1);
+  d.nrhs = nrhs; d.rs_in = d.rs_phi = d.rs_out = 2 * half_bytes(prec, Vh);
+  return launch_dslash(c, d);
+}
+
+int qxd_set_rhs_per_thread(qxd_ctx* c, int r) {
+  if (!c || r < 0 || r > 3) return c ? fail(c, QXD_EINVAL, "set_rhs_per_thread: 0 (default), 1, 2 or 3") : QXD_EINVAL;
+  c->rhs_per_thread = r;
+  return QXD_OK;
+}
+
 int qxd_apply_Dhat_packed(qxd_ctx* c, int prec, const void* in_e, void* out_e, int dagger) {
   int rc = check_apply(c, prec, in_e, out_e, "apply_Dhat_packed");
   if (rc) return rc;
@@ -294,6 +333,14 @@ int qxd_solve(qxd_ctx* c, const double* eta, double* psi, double tol, qxd_solve_
   if (rc) return rc;
   if (info->algo != QXD_CGNE && info->algo != QXD_BICGSTAB) return fail(c, QXD_EINVAL, "solve: unknown algorithm");
   return solve_eo(c, eta, psi, tol, info);
+}
+
+int qxd_solve_multi(qxd_ctx* c, int nrhs, const double* eta, double* psi, double tol, qxd_solve_info* info) {
+  if (!c || !info) return c ? fail(c, QXD_EINVAL, "solve_multi: info array is null") : QXD_EINVAL;
+  int rc = check_apply(c, info[0].sloppy, eta, psi, "solve_multi");
+  if (rc) return rc;
+  if (c->nrhs < 2 || !c->mscal) return fail(c, QXD_EWORKSPACE, "solve_multi: bind the workspace with nrhs > 1");
+  return solve_eo_multi(c, nrhs, eta, psi, tol, info);
 }
 
 int qxd_solve_host(qxd_ctx* c, const double* eta_host, double* psi_host, double tol, qxd_solve_info* info) {

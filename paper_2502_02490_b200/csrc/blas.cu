@@ -53,14 +53,19 @@ __global__ void __launch_bounds__(128) cxpaypbw_k(int Vh, SpinorPtr x, double ar
 }
 
 // CG on the normal equations, step 1:  alpha = num/den ;  x += alpha p ;  r -= alpha t ;  result = |r|^2
+// Batched form (row a10): blockIdx.y = right-hand side; vectors rs bytes apart, scalars ss doubles apart; act (may be null)
+// holds 1.0 / 0.0 per right-hand side: a converged system is frozen (alpha = beta = 0).
 template <typename S>
 __global__ void __launch_bounds__(128) cg_xr_k(int Vh, const double* num, const double* den, SpinorPtr p, SpinorPtr t, SpinorPtr x,
-                                               SpinorPtr r, Reducer R) {
+                                               SpinorPtr r, Reducer R, size_t rs, int ss, const double* act) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   double nrm[1] = {0.0};
+  const int k = blockIdx.y;
+  p = rhs_view(p, rs, k); t = rhs_view(t, rs, k); x = rhs_view(x, rs, k); r = rhs_view(r, rs, k);
   if (cb < Vh) {
-    const C al = (C)(*num / *den);
+    const double dn = den[k * ss];
+    const C al = (act && act[k] == 0.0) || dn == 0.0 ? (C)0 : (C)(num[k * ss] / dn);
     C vp[24], vx[24];
     load_spinor<S>(p, Vh, cb, vp);
     load_spinor<S>(x, Vh, cb, vx);
@@ -77,11 +82,15 @@ __global__ void __launch_bounds__(128) cg_xr_k(int Vh, const double* num, const 
 }
 // step 2:  beta = num/den ;  p = s + beta p
 template <typename S>
-__global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const double* den, SpinorPtr s, SpinorPtr p) {
+__global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const double* den, SpinorPtr s, SpinorPtr p, size_t rs, int ss,
+                                              const double* act) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   if (cb >= Vh) return;
-  const C be = (C)(*num / *den);
+  const int k = blockIdx.y;
+  s = rhs_view(s, rs, k); p = rhs_view(p, rs, k);
+  const double dn = den[k * ss];
+  const C be = (act && act[k] == 0.0) || dn == 0.0 ? (C)0 : (C)(num[k * ss] / dn);
   C vs[24], vp[24];
   load_spinor<S>(s, Vh, cb, vs);
   load_spinor<S>(p, Vh, cb, vp);
@@ -91,10 +100,11 @@ __global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const d
 }
 
 template <typename S>
-__global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R) {
+__global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R, size_t rs) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   double nrm[1] = {0.0};
+  x = rhs_view(x, rs, blockIdx.y);
   if (cb < Vh) {
     C v[24];
     load_spinor<S>(x, Vh, cb, v);
@@ -125,10 +135,11 @@ __global__ void __launch_bounds__(128) cdot_k(int Vh, SpinorPtr x, SpinorPtr y, 
 }
 
 template <typename S>
-__global__ void __launch_bounds__(128) zero_k(int Vh, SpinorPtr x) {
+__global__ void __launch_bounds__(128) zero_k(int Vh, SpinorPtr x, size_t rs) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   if (cb >= Vh) return;
+  x = rhs_view(x, rs, blockIdx.y);
   C v[24];
 #pragma unroll
   for (int i = 0; i < 24; i++) v[i] = 0;
@@ -166,9 +177,9 @@ __global__ void __launch_bounds__(128) sub_norm_k(int Vh, SpinorPtr b, SpinorPtr
   grid_reduce<1>(nrm, R);
 }
 
-inline Reducer reducer(qxd_ctx* c, double* result) {
+inline Reducer reducer(qxd_ctx* c, double* result, int rstride = 0) {
   Reducer R;
-  R.partials = c->partials; R.ticket = c->ticket; R.result = result;
+  R.partials = c->partials; R.ticket = c->ticket; R.result = result; R.rstride = rstride;
   return R;
 }
 
@@ -182,6 +193,7 @@ inline Reducer reducer(qxd_ctx* c, double* result) {
   } while (0)
 
 #define QXD_GRID dim3((c->g.Vh + 127) / 128), 128, 0, c->stream
+#define QXD_GRID_N(n) dim3((c->g.Vh + 127) / 128, (n)), 128, 0, c->stream
 
 int blas_axpy(qxd_ctx* c, int prec, double a, const SpinorPtr& x, const SpinorPtr& y) {
   QXD_BY_PREC(prec, axpy_k<S><<<QXD_GRID>>>(c->g.Vh, a, x, y));
@@ -196,18 +208,18 @@ int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai
   return QXD_OK;
 }
 int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
-               const SpinorPtr& r, double* rr) {
-  QXD_BY_PREC(prec, cg_xr_k<S><<<QXD_GRID>>>(c->g.Vh, num, den, p, t, x, r, reducer(c, rr)));
+               const SpinorPtr& r, double* rr, const Batch& b) {
+  QXD_BY_PREC(prec, cg_xr_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, num, den, p, t, x, r, reducer(c, rr, b.ss), b.rs, b.ss, b.act));
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p) {
-  QXD_BY_PREC(prec, cg_p_k<S><<<QXD_GRID>>>(c->g.Vh, num, den, s, p));
+int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const Batch& b) {
+  QXD_BY_PREC(prec, cg_p_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, num, den, s, p, b.rs, b.ss, b.act));
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* res) {
-  QXD_BY_PREC(prec, norm2_k<S><<<QXD_GRID>>>(c->g.Vh, x, reducer(c, res)));
+int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* res, const Batch& b) {
+  QXD_BY_PREC(prec, norm2_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, x, reducer(c, res, b.ss), b.rs));
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
@@ -216,12 +228,14 @@ int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, doub
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x) {
-  QXD_BY_PREC(prec, zero_k<S><<<QXD_GRID>>>(c->g.Vh, x));
+int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x, const Batch& b) {
+  QXD_BY_PREC(prec, zero_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, x, b.rs));
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y) { return launch_convert_spinor(c, prec, x, prec, y); }
+int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, const Batch& b) {
+  return launch_convert_spinor(c, prec, x, prec, y, b.n, b.rs, b.rs);
+}
 int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi) {
   QXD_BY_PREC(prec, acc_hi_k<S><<<QXD_GRID>>>(c->g.Vh, xlo, xhi));
   QXD_LAUNCH_CHECK(c);

@@ -1,0 +1,28 @@
+// dslash_args.h -- kernel argument block of the dslash kernels (dslash_kernel.cuh) and the per-precision dispatchers.
+#pragma once
+#include "qxd_ctx.h"
+
+namespace qxd {
+
+struct DslashArgs {
+  Geom g;
+  SpinorPtr in[2];
+  SpinorPtr phi;
+  SpinorPtr out[2];
+  const void* W[2];
+  const void* CL[2];
+  int parity_out;
+  int prefetch;
+  int nrhs;            // right-hand sides in this launch (row a10); 1 for the single-spinor entry points
+  int ngroups;         // ceil(nrhs / R): consecutive CTAs work on the same tile for different groups of R right-hand sides
+  size_t rs_in, rs_phi, rs_out;   // byte distance between consecutive right-hand sides
+  Reducer R;
+};
+
+
+// one translation unit per storage precision (dslash_f64.cu, dslash_f32.cu, dslash_f16.cu)
+int dslash_dispatch_f64(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+
+}  // namespace qxd

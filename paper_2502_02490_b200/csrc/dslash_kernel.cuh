@@ -1,0 +1,416 @@
+// dslash.cu -- SURVEY.md §8 rows a4 (D_w apply), a5 (D-hat even-odd passes) and the dslash-shaped parts
+// of a8: the hand-written sm_100a stencil kernel.
+//
+//   (D_w psi)(x) = M(x) psi(x) - 1/2 sum_mu [ (1-gamma_mu) W_mu(x) psi(x+mu) + (1+gamma_mu) W_mu(x-mu)^dag psi(x-mu) ]
+//
+// (readings R1-R3; "connects nearest neighbor points ... indices for Dirac spin,
+// color charge, and space-time"; W = e^{iqA} U; M = clover term.)
+// One thread per output site: for each of the 8 neighbours the spinor is spin-projected to a half spinor
+// (2 spin x 3 colour), multiplied by the link (or its adjoint), reconstructed and accumulated; the clover
+// or inverse-clover multiplication is fused into the epilogue.  The path is bandwidth bound:
+// all field accesses are 16-byte vector loads on chunk-major SoA records, coalesced across the warp.
+//
+// In the chiral basis of reading R3 (gamma_0 = [[0,-1],[-1,0]], gamma_k = [[0,-i s_k],[i s_k,0]]):
+//   (1 -+ gamma_0) psi = (h, +-h),            h = psi_u +- psi_l
+//   (1 -+ gamma_k) psi = (h, -+ i s_k h),     h = psi_u +- i s_k psi_l
+// with the upper sign for the forward hop.
+#pragma once
+#include "dslash_args.h"
+
+namespace qxd {
+
+namespace {
+
+// h = psi_u + SGN * (proj_lower), for direction MU; psi: 24 reals, h: 12 reals
+template <int MU, int SGN, typename C>
+__device__ __forceinline__ void project(const C* psi, C* h) {
+  const C s = (C)SGN;
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const C u0r = psi[2 * a], u0i = psi[2 * a + 1], u1r = psi[6 + 2 * a], u1i = psi[6 + 2 * a + 1];
+    const C l0r = psi[12 + 2 * a], l0i = psi[12 + 2 * a + 1], l1r = psi[18 + 2 * a], l1i = psi[18 + 2 * a + 1];
+    if (MU == 0) {        // + s * (l0, l1)
+      h[2 * a] = u0r + s * l0r; h[2 * a + 1] = u0i + s * l0i;
+      h[6 + 2 * a] = u1r + s * l1r; h[6 + 2 * a + 1] = u1i + s * l1i;
+    } else if (MU == 1) { // + s * (i l1, i l0)
+      h[2 * a] = u0r - s * l1i; h[2 * a + 1] = u0i + s * l1r;
+      h[6 + 2 * a] = u1r - s * l0i; h[6 + 2 * a + 1] = u1i + s * l0r;
+    } else if (MU == 2) { // + s * (l1, -l0)
+      h[2 * a] = u0r + s * l1r; h[2 * a + 1] = u0i + s * l1i;
+      h[6 + 2 * a] = u1r - s * l0r; h[6 + 2 * a + 1] = u1i - s * l0i;
+    } else {              // + s * (i l0, -i l1)
+      h[2 * a] = u0r - s * l0i; h[2 * a + 1] = u0i + s * l0r;
+      h[6 + 2 * a] = u1r + s * l1i; h[6 + 2 * a + 1] = u1i - s * l1r;
+    }
+  }
+}
+// acc_u += r ; acc_l += lower part reconstructed from r
+template <int MU, int SGN, typename C>
+__device__ __forceinline__ void reconstruct(const C* r, C* acc) {
+  const C s = (C)SGN;
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const C r0r = r[2 * a], r0i = r[2 * a + 1], r1r = r[6 + 2 * a], r1i = r[6 + 2 * a + 1];
+    acc[2 * a] += r0r; acc[2 * a + 1] += r0i;
+    acc[6 + 2 * a] += r1r; acc[6 + 2 * a + 1] += r1i;
+    if (MU == 0) {        // lower = s * (r0, r1)
+      acc[12 + 2 * a] += s * r0r; acc[12 + 2 * a + 1] += s * r0i;
+      acc[18 + 2 * a] += s * r1r; acc[18 + 2 * a + 1] += s * r1i;
+    } else if (MU == 1) { // lower = -s * (i r1, i r0)
+      acc[12 + 2 * a] += s * r1i; acc[12 + 2 * a + 1] -= s * r1r;
+      acc[18 + 2 * a] += s * r0i; acc[18 + 2 * a + 1] -= s * r0r;
+    } else if (MU == 2) { // lower = -s * (r1, -r0)
+      acc[12 + 2 * a] -= s * r1r; acc[12 + 2 * a + 1] -= s * r1i;
+      acc[18 + 2 * a] += s * r0r; acc[18 + 2 * a + 1] += s * r0i;
+    } else {              // lower = -s * (i r0, -i r1)
+      acc[12 + 2 * a] += s * r0i; acc[12 + 2 * a + 1] -= s * r0r;
+      acc[18 + 2 * a] -= s * r1i; acc[18 + 2 * a + 1] += s * r1r;
+    }
+  }
+}
+// r[s][a] = sum_b W[a][b] h[s][b]   (ADJ: sum_b conj(W[b][a]) h[s][b])
+template <bool ADJ, typename C>
+__device__ __forceinline__ void link_mul(const C* w, const C* h, C* r) {
+#pragma unroll
+  for (int s = 0; s < 2; s++)
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      C re = 0, im = 0;
+#pragma unroll
+      for (int b = 0; b < 3; b++) {
+        const C wr = ADJ ? w[2 * (3 * b + a)] : w[2 * (3 * a + b)];
+        const C wi = ADJ ? -w[2 * (3 * b + a) + 1] : w[2 * (3 * a + b) + 1];
+        const C hr = h[6 * s + 2 * b], hi = h[6 * s + 2 * b + 1];
+        re += wr * hr - wi * hi;
+        im += wr * hi + wi * hr;
+      }
+      r[6 * s + 2 * a] = re; r[6 * s + 2 * a + 1] = im;
+    }
+}
+
+// out(12 reals: one chirality) = Hermitian 6x6 block (36 packed reals) times in
+template <typename C>
+__device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
+#pragma unroll
+  for (int i = 0; i < 6; i++) { out[2 * i] = b[i] * in[2 * i]; out[2 * i + 1] = b[i] * in[2 * i + 1]; }
+  int k = 6;
+#pragma unroll
+  for (int i = 0; i < 6; i++)
+#pragma unroll
+    for (int j = i + 1; j < 6; j++) {
+      const C ur = b[k], ui = b[k + 1];
+      k += 2;
+      // out_i += u in_j ; out_j += conj(u) in_i
+      out[2 * i] += ur * in[2 * j] - ui * in[2 * j + 1];
+      out[2 * i + 1] += ur * in[2 * j + 1] + ui * in[2 * j];
+      out[2 * j] += ur * in[2 * i] + ui * in[2 * i + 1];
+      out[2 * j + 1] += ur * in[2 * i + 1] - ui * in[2 * i];
+    }
+}
+template <typename S>
+__device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const typename PT<S>::C* in, typename PT<S>::C* out) {
+  typename PT<S>::C b[36];
+  load_reals<S, 0, 36>(CL, Vh, cb, b);
+  block_mul(b, in, out);
+  load_reals<S, 36, 36>(CL, Vh, cb, b);
+  block_mul(b, in + 12, out + 12);
+}
+// the same blocks applied to R spinors (multi-RHS, row a10): each block is loaded once
+template <typename S, int R>
+__device__ __forceinline__ void clover_mul_multi(const void* CL, int Vh, int cb, const typename PT<S>::C (*in)[24], typename PT<S>::C (*out)[24]) {
+  typename PT<S>::C b[36];
+  load_reals<S, 0, 36>(CL, Vh, cb, b);
+#pragma unroll
+  for (int r = 0; r < R; r++) block_mul(b, in[r], out[r]);
+  load_reals<S, 36, 36>(CL, Vh, cb, b);
+#pragma unroll
+  for (int r = 0; r < R; r++) block_mul(b, in[r] + 12, out[r] + 12);
+}
+
+// One hop in flight: the raw 16-byte chunks of the neighbour spinor and of the link, exactly as loaded.  Keeping the
+// packed vectors (not the unpacked reals) in registers between issue and use lets two hops be in flight per thread
+// (software pipeline in hop_all below): the kernel is bound by memory latency x bytes in flight, not by arithmetic.
+template <typename S, int R>
+struct HopRegs {
+  typedef typename PT<S>::V V;
+  static constexpr int RPC = PT<S>::RPC;
+  static constexpr int NPSI = 24 / RPC;
+  V psi[R][NPSI];
+  static constexpr int NWC = RPC == 2 ? 9 : RPC == 4 ? 5 : 3;
+  V w[NWC];        // chunks covering the 18 reals of one link (loaded once for all R right-hand sides)
+  float scale[R];  // fp16 block-float scale of the neighbour spinor
+};
+template <int MU, typename S> struct LinkChunks {
+  static constexpr int RPC = PT<S>::RPC;
+  static constexpr int C0 = (18 * MU) / RPC, C1 = (18 * MU + 17) / RPC, N = C1 - C0 + 1, OFF = 18 * MU - C0 * RPC;
+};
+template <typename S, int MU, int DIR, int R>
+__device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, HopRegs<S, R>& d) {
+  typedef typename PT<S>::V V;
+  typedef LinkChunks<MU, S> LC;
+  const int Vh = a.g.Vh;
+  const int nb = neighbour_cb<MU, DIR>(a.g, s);
+#pragma unroll
+  for (int r = 0; r < R; r++) {
+    if (R > 1 && rhs0 + r >= a.nrhs) break;
+    const V* p = reinterpret_cast<const V*>(static_cast<const char*>(a.in[1 - parity].data) + a.rs_in * (rhs0 + r));
+#pragma unroll
+    for (int c = 0; c < HopRegs<S, R>::NPSI; c++) d.psi[r][c] = ldg_pinned(p + size_t(c) * Vh + nb);
+    if (PT<S>::ID == 2) d.scale[r] = ldg_pinned(reinterpret_cast<const float*>(reinterpret_cast<const char*>(a.in[1 - parity].scale) + a.rs_in * (rhs0 + r)) + nb);
+  }
+  // forward: W_mu(x) of the own parity; backward: W_mu(x-mu) of the other parity at the neighbour
+  const V* w = reinterpret_cast<const V*>(DIR > 0 ? a.W[parity] : a.W[1 - parity]);
+  const int wi = DIR > 0 ? cb : nb;
+#pragma unroll
+  for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * Vh + wi);
+}
+template <typename S, int MU, int DIR, bool G5IN, int R>
+__device__ __forceinline__ void hop_use(const HopRegs<S, R>& d, typename PT<S>::C (*acc)[24]) {
+  typedef typename PT<S>::C C;
+  typedef LinkChunks<MU, S> LC;
+  constexpr int RPC = PT<S>::RPC;
+  C wv[HopRegs<S, R>::NWC * RPC];
+#pragma unroll
+  for (int c = 0; c < LC::N; c++) unpack_vec(d.w[c], wv + c * RPC);
+#pragma unroll
+  for (int r = 0; r < R; r++) {
+    C psi[24], h[12], t[12];
+#pragma unroll
+    for (int c = 0; c < HopRegs<S, R>::NPSI; c++) unpack_vec(d.psi[r][c], psi + c * RPC);
+    if (PT<S>::ID == 2) {
+#pragma unroll
+      for (int i = 0; i < 24; i++) psi[i] *= d.scale[r];
+    }
+    if (G5IN) {
+#pragma unroll
+      for (int i = 12; i < 24; i++) psi[i] = -psi[i];
+    }
+    project<MU, DIR>(psi, h);
+    link_mul<(DIR < 0)>(wv + LC::OFF, h, t);
+    reconstruct<MU, DIR>(t, acc[r]);
+  }
+}
+// all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one
+template <typename S, bool G5IN, int R, int PIPE>
+__device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, typename PT<S>::C (*acc)[24]) {
+  if (PIPE == 2) {
+    HopRegs<S, R> d0, d1;
+    hop_issue<S, 0, +1, R>(a, s, cb, parity, rhs0, d0);
+    hop_issue<S, 0, -1, R>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 0, +1, G5IN, R>(d0, acc);
+    hop_issue<S, 1, +1, R>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 0, -1, G5IN, R>(d1, acc);
+    hop_issue<S, 1, -1, R>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 1, +1, G5IN, R>(d0, acc);
+    hop_issue<S, 2, +1, R>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 1, -1, G5IN, R>(d1, acc);
+    hop_issue<S, 2, -1, R>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 2, +1, G5IN, R>(d0, acc);
+    hop_issue<S, 3, +1, R>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 2, -1, G5IN, R>(d1, acc);
+    hop_issue<S, 3, -1, R>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 3, +1, G5IN, R>(d0, acc);
+    hop_use<S, 3, -1, G5IN, R>(d1, acc);
+  } else {
+    HopRegs<S, R> d;
+    hop_issue<S, 0, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 0, +1, G5IN, R>(d, acc);
+    hop_issue<S, 0, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 0, -1, G5IN, R>(d, acc);
+    hop_issue<S, 1, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 1, +1, G5IN, R>(d, acc);
+    hop_issue<S, 1, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 1, -1, G5IN, R>(d, acc);
+    hop_issue<S, 2, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 2, +1, G5IN, R>(d, acc);
+    hop_issue<S, 2, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 2, -1, G5IN, R>(d, acc);
+    hop_issue<S, 3, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 3, +1, G5IN, R>(d, acc);
+    hop_issue<S, 3, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 3, -1, G5IN, R>(d, acc);
+  }
+}
+
+// Bulk L2 prefetch (cp.async.bulk.prefetch.L2, sm_90+): the compulsory DRAM streams of a CTA -- its own links, its
+// clover blocks and its own spinors -- are contiguous 16 B x 128-site rows of the chunk-major SoA records.  One thread per
+// row asks the L2 for the whole row when the CTA starts, so the per-thread 16-byte loads that follow (one hop after the
+// other, bounded by registers) find their lines in L2 or already in flight instead of paying one DRAM latency per hop.
+__device__ __forceinline__ void bulk_prefetch_l2(const void* p, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+template <typename S, int PHI, bool FULL>
+__device__ __forceinline__ void cta_prefetch(const DslashArgs& a, int cb0) {
+  constexpr int NW = 72 / PT<S>::RPC, NS = 24 / PT<S>::RPC;   // rows per parity: links, clover (NW each), spinor (NS)
+  const int Vh = a.g.Vh;
+  const int n = min(128, Vh - cb0);
+  if (n <= 0) return;
+  const unsigned bytes = unsigned(n) * 16u;
+  const int t = threadIdx.x;
+  if (FULL) {
+    // rows: [parity][W NW | CL NW | psi NS]
+    constexpr int PER = 2 * NW + NS;
+    if (t < 2 * PER) {
+      const int p = t / PER, r = t % PER;
+      const char* base = r < NW ? (const char*)a.W[p] : r < 2 * NW ? (const char*)a.CL[p] : (const char*)a.in[p].data;
+      const int c = r < NW ? r : r < 2 * NW ? r - NW : r - 2 * NW;
+      bulk_prefetch_l2(base + (size_t(c) * Vh + cb0) * 16, bytes);
+    }
+  } else {
+    // own forward links, clover (or inverse) block, phi
+    constexpr int PER = 2 * NW + (PHI ? NS : 0);
+    if (t < PER) {
+      const int p = a.parity_out;
+      const char* base = t < NW ? (const char*)a.W[p] : t < 2 * NW ? (const char*)a.CL[p] : (const char*)a.phi.data;
+      const int c = t < NW ? t : t < 2 * NW ? t - NW : t - 2 * NW;
+      bulk_prefetch_l2(base + (size_t(c) * Vh + cb0) * 16, bytes);
+    }
+  }
+}
+
+// PHI: 0 none, 1 phi, 2 M*phi (FULL: phi = in on the own parity).  POST: 1 = multiply the result by M^{-1}.
+// Full-lattice launches (row a4) put both parities of 128 consecutive checkerboard indices -- one 4x4x4x4 tile with
+// the default order -- into one CTA of 256 threads (warps 0-3 even, 4-7 odd): every link is then used twice by the same
+// CTA (forward hop of x, backward hop of x+mu) and 3/4 of the neighbour spinors belong to the CTA's own tile.
+// R > 1 (row a10, multi-RHS): every thread applies the operator of its site to R right-hand sides, loading each link
+// and clover block once; ngroups consecutive CTAs cover all right-hand sides of one tile, so the links of a tile are
+// read from DRAM once and from L2 by the other groups.
+template <typename S, int R, bool FULL> struct KernelShape {
+  static constexpr int THREADS = FULL ? 256 : 128;
+  // CTAs per SM the register budget is sized for
+  static constexpr int MINB = sizeof(S) == 8 ? 1 : (R == 1 ? (FULL ? 2 : 4) : (R == 2 ? (FULL ? 1 : 3) : (FULL ? 1 : 2)));
+  static constexpr int PIPE = (R == 1) ? 2 : 1;
+};
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R>
+__global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<S, R, FULL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
+  typedef typename PT<S>::C C;
+  const int Vh = a.g.Vh;
+  const int tile = R > 1 ? blockIdx.x / a.ngroups : blockIdx.x;
+  const int rhs0 = R > 1 ? (blockIdx.x - tile * a.ngroups) * R : 0;
+  const int cb = tile * 128 + (threadIdx.x & 127);
+  const int parity = FULL ? (threadIdx.x >> 7) : a.parity_out;
+  if (a.prefetch) cta_prefetch<S, PHI, FULL>(a, tile * 128);
+  double nrm[R];
+#pragma unroll
+  for (int r = 0; r < R; r++) nrm[r] = 0.0;
+  if (cb < Vh) {
+    Site s;
+    site_init(a.g, cb, parity, s);
+    C acc[R][24];
+#pragma unroll
+    for (int r = 0; r < R; r++)
+#pragma unroll
+      for (int i = 0; i < 24; i++) acc[r][i] = 0;
+    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL>::PIPE>(a, s, cb, parity, rhs0, acc);
+    const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
+#pragma unroll
+    for (int r = 0; r < R; r++)
+#pragma unroll
+      for (int i = 0; i < 24; i++) acc[r][i] *= ((FLAGS & DSF_G5HOP) && i >= 12) ? -hs : hs;
+    if (PHI != 0) {
+      C phi[R][24];
+#pragma unroll
+      for (int r = 0; r < R; r++) {
+        if (R > 1 && rhs0 + r >= a.nrhs) break;
+        load_spinor<S>(FULL ? rhs_view(a.in[parity], a.rs_in, rhs0 + r) : rhs_view(a.phi, a.rs_phi, rhs0 + r), Vh, cb, phi[r]);
+      }
+      if (PHI == 2) {
+        C mphi[R][24];
+        clover_mul_multi<S, R>(a.CL[parity], Vh, cb, phi, mphi);
+#pragma unroll
+        for (int r = 0; r < R; r++)
+#pragma unroll
+          for (int i = 0; i < 24; i++) acc[r][i] += mphi[r][i];
+      } else {
+#pragma unroll
+        for (int r = 0; r < R; r++)
+#pragma unroll
+          for (int i = 0; i < 24; i++) acc[r][i] += phi[r][i];
+      }
+    }
+    if (POST) {
+      C t[R][24];
+      clover_mul_multi<S, R>(a.CL[parity], Vh, cb, acc, t);
+#pragma unroll
+      for (int r = 0; r < R; r++)
+#pragma unroll
+        for (int i = 0; i < 24; i++) acc[r][i] = t[r][i];
+    }
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+      if (R > 1 && rhs0 + r >= a.nrhs) break;
+      if (FLAGS & DSF_NORM) {
+#pragma unroll
+        for (int i = 0; i < 24; i++) nrm[r] += (double)acc[r][i] * (double)acc[r][i];
+      }
+      store_spinor<S>(rhs_view(a.out[parity], a.rs_out, rhs0 + r), Vh, cb, acc[r]);
+    }
+  }
+  if (FLAGS & DSF_NORM) {
+    const int ntiles = R > 1 ? gridDim.x / a.ngroups : gridDim.x;
+#pragma unroll
+    for (int r = 0; r < R; r++) {
+      if (R > 1 && rhs0 + r >= a.nrhs) break;   // uniform over the CTA
+      double v[1] = {nrm[r]};
+      grid_reduce<1>(v, a.R, tile, ntiles, rhs0 + r);
+    }
+  }
+}
+
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R>
+void launch_r(qxd_ctx* c, DslashArgs& a) {
+  a.ngroups = (a.nrhs + R - 1) / R;
+  dim3 gr(unsigned((c->g.Vh + 127) / 128) * unsigned(a.ngroups));
+  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R><<<gr, KernelShape<S, R, FULL>::THREADS, 0, c->stream>>>(a);
+}
+// right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 3)
+// MULTI: instantiate the R = 2, 3 kernels for this mode (only the modes the batched solver and bench use)
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, bool MULTI>
+int launch_one(qxd_ctx* c, DslashArgs& a) {
+  int R = 1;
+  if (a.nrhs > 1) {
+    R = c->rhs_per_thread > 0 ? c->rhs_per_thread : 3;
+    if (R > a.nrhs) R = a.nrhs;
+  }
+  if (MULTI && sizeof(S) < 8) {   // fp64: the accumulators of two spinors do not fit the register file
+    if (R == 2) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 2 : 1>(c, a); return QXD_OK; }
+    if (R >= 3) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 3 : 1>(c, a); return QXD_OK; }
+  }
+  // one launch per right-hand side
+  const int n = a.nrhs;
+  const SpinorPtr in0 = a.in[0], in1 = a.in[1], phi = a.phi, out0 = a.out[0], out1 = a.out[1];
+  double* res = a.R.result;
+  for (int r = 0; r < n; r++) {
+    a.nrhs = 1;
+    a.in[0] = rhs_view(in0, a.rs_in, r); a.in[1] = rhs_view(in1, a.rs_in, r); a.phi = rhs_view(phi, a.rs_phi, r);
+    a.out[0] = rhs_view(out0, a.rs_out, r); a.out[1] = rhs_view(out1, a.rs_out, r);
+    a.R.result = res ? res + size_t(r) * a.R.rstride : nullptr;
+    launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1>(c, a);
+    if (r + 1 < n) c->launches++;
+  }
+  return QXD_OK;
+}
+
+template <typename S>
+int dispatch(qxd_ctx* c, const DslashCall& d, DslashArgs& a) {
+  const int f = d.flags;
+  switch (d.mode) {
+    case DS_DW_FULL:
+      if (f != 0) break;
+      return launch_one<S, 2, 0, false, 0, true, true>(c, a);
+    case DS_HOP_AINV:
+      if (f == 0) { return launch_one<S, 0, 1, false, 0, false, true>(c, a); }
+      if (f == DSF_G5IN) { return launch_one<S, 0, 1, false, DSF_G5IN, false, true>(c, a); }
+      break;
+    case DS_A_XMHOP:
+      if (f == 0) { return launch_one<S, 2, 0, true, 0, false, true>(c, a); }
+      if (f == DSF_NORM) { return launch_one<S, 2, 0, true, DSF_NORM, false, true>(c, a); }
+      if (f == DSF_G5HOP) { return launch_one<S, 2, 0, true, DSF_G5HOP, false, true>(c, a); }
+      if (f == (DSF_G5HOP | DSF_NORM)) { return launch_one<S, 2, 0, true, DSF_G5HOP | DSF_NORM, false, true>(c, a); }
+      break;
+    case DS_X_MHOP:
+      if (f == 0) { return launch_one<S, 1, 0, true, 0, false, false>(c, a); }
+      break;
+    case DS_AINV_X_MHOP:
+      if (f == 0) { return launch_one<S, 1, 1, true, 0, false, false>(c, a); }
+      break;
+    default: break;
+  }
+  return fail(c, QXD_EINVAL, "dslash: unsupported mode/flags combination");
+}
+
+}  // namespace
+
+}  // namespace qxd

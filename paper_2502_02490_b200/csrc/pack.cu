@@ -101,9 +101,10 @@ __global__ void __launch_bounds__(128) spinor_unpack_k(Geom g, SpinorPtr p0, Spi
 }
 
 template <typename SF, typename ST>
-__global__ void __launch_bounds__(128) convert_spinor_k(int Vh, SpinorPtr from, SpinorPtr to) {
+__global__ void __launch_bounds__(128) convert_spinor_k(int Vh, SpinorPtr from, SpinorPtr to, size_t rs_from, size_t rs_to) {
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   if (cb >= Vh) return;
+  from = rhs_view(from, rs_from, blockIdx.y); to = rhs_view(to, rs_to, blockIdx.y);
   typename PT<SF>::C v[24];
   typename PT<ST>::C w[24];
   load_spinor<SF>(from, Vh, cb, v);
@@ -175,16 +176,16 @@ int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, 
 }
 
 template <typename SF>
-static void convert_from(qxd_ctx* c, const SpinorPtr& from, int pt, const SpinorPtr& to) {
-  dim3 gr = grid_for(c->g.Vh, 1);
-  if (pt == 0) convert_spinor_k<SF, double><<<gr, 128, 0, c->stream>>>(c->g.Vh, from, to);
-  else if (pt == 1) convert_spinor_k<SF, float><<<gr, 128, 0, c->stream>>>(c->g.Vh, from, to);
-  else convert_spinor_k<SF, __half><<<gr, 128, 0, c->stream>>>(c->g.Vh, from, to);
+static void convert_from(qxd_ctx* c, const SpinorPtr& from, int pt, const SpinorPtr& to, int n, size_t rf, size_t rt) {
+  dim3 gr = grid_for(c->g.Vh, n);
+  if (pt == 0) convert_spinor_k<SF, double><<<gr, 128, 0, c->stream>>>(c->g.Vh, from, to, rf, rt);
+  else if (pt == 1) convert_spinor_k<SF, float><<<gr, 128, 0, c->stream>>>(c->g.Vh, from, to, rf, rt);
+  else convert_spinor_k<SF, __half><<<gr, 128, 0, c->stream>>>(c->g.Vh, from, to, rf, rt);
 }
-int launch_convert_spinor(qxd_ctx* c, int pf, const SpinorPtr& from, int pt, const SpinorPtr& to) {
-  if (pf == 0) convert_from<double>(c, from, pt, to);
-  else if (pf == 1) convert_from<float>(c, from, pt, to);
-  else convert_from<__half>(c, from, pt, to);
+int launch_convert_spinor(qxd_ctx* c, int pf, const SpinorPtr& from, int pt, const SpinorPtr& to, int n, size_t rf, size_t rt) {
+  if (pf == 0) convert_from<double>(c, from, pt, to, n, rf, rt);
+  else if (pf == 1) convert_from<float>(c, from, pt, to, n, rf, rt);
+  else convert_from<__half>(c, from, pt, to, n, rf, rt);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

@@ -241,15 +241,20 @@ __device__ __forceinline__ void store_spinor(const SpinorPtr& p, int Vh, int cb,
 // result is deterministic for a fixed launch configuration.  fp64 accumulators for every storage type.
 // ---------------------------------------------------------------------------------------------
 struct Reducer {
-  double* partials;    // [N][gridDim.x]
-  unsigned* ticket;
-  double* result;      // [N]
+  double* partials;    // [slot][N][nparts]
+  unsigned* ticket;    // [slot]
+  double* result;      // [slot * rstride + N]
+  int rstride;         // distance (in doubles) between the results of consecutive slots (right-hand sides)
 };
+// part / nparts: this block's index among the blocks that contribute to `slot` and their number.
 template <int N>
-__device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R) {
+__device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R, int part, int nparts, int slot) {
   __shared__ double sm[N][32];
   __shared__ bool last;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  double* partials = R.partials + size_t(slot) * N * nparts;
+  unsigned* ticket = R.ticket + slot;
+  __syncthreads();  // sm may still be read by a previous call
 #pragma unroll
   for (int k = 0; k < N; k++) {
 #pragma unroll
@@ -263,13 +268,13 @@ __device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R) {
       double t = lane < nw ? sm[k][lane] : 0.0;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-      if (lane == 0) R.partials[size_t(k) * gridDim.x + blockIdx.x] = t;
+      if (lane == 0) partials[size_t(k) * nparts + part] = t;
     }
   }
   if (threadIdx.x == 0) {
     __threadfence();
-    unsigned t = atomicAdd(R.ticket, 1u);
-    last = (t == gridDim.x - 1);
+    unsigned t = atomicAdd(ticket, 1u);
+    last = (t == unsigned(nparts) - 1u);
   }
   __syncthreads();
   if (last) {
@@ -277,7 +282,7 @@ __device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R) {
 #pragma unroll
     for (int k = 0; k < N; k++) {
       double t = 0.0;
-      for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) t += __ldcg(R.partials + size_t(k) * gridDim.x + i);
+      for (int i = threadIdx.x; i < nparts; i += blockDim.x) t += __ldcg(partials + size_t(k) * nparts + i);
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
       __syncthreads();
@@ -287,11 +292,24 @@ __device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R) {
         double u = lane < nw ? sm[k][lane] : 0.0;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
-        if (lane == 0) R.result[k] = u;
+        if (lane == 0) R.result[size_t(slot) * R.rstride + k] = u;
       }
     }
-    if (threadIdx.x == 0) *R.ticket = 0u;
+    if (threadIdx.x == 0) *ticket = 0u;
   }
+}
+// one slot per blockIdx.y (batched BLAS: blockIdx.y = right-hand side)
+template <int N>
+__device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R) {
+  grid_reduce<N>(v, R, blockIdx.x, gridDim.x, blockIdx.y);
+}
+
+// Right-hand side r of a batch: consecutive right-hand sides are `stride` bytes apart (data and fp16 scales alike).
+__host__ __device__ __forceinline__ SpinorPtr rhs_view(const SpinorPtr& p, size_t stride, int r) {
+  SpinorPtr q;
+  q.data = static_cast<char*>(p.data) + stride * r;
+  q.scale = p.scale ? reinterpret_cast<float*>(reinterpret_cast<char*>(p.scale) + stride * r) : nullptr;
+  return q;
 }
 
 }  // namespace qxd

@@ -37,6 +37,7 @@ struct qxd_ctx {
   char* ws = nullptr;
   size_t ws_bytes = 0, ws_used = 0;
   int prec_mask = 0, nrhs = 1;
+  int rhs_per_thread = 0;                        // multi-RHS dslash: right-hand sides per thread (0 = default)
   // state
   bool have_gauge = false, have_qed = false, have_quark = false, have_clover = false;
   double qel = 1.0, kappa = 0, q = 0, m0 = 0, csw = 0, csw_qed = 0;
@@ -53,6 +54,14 @@ struct qxd_ctx {
   void* full_b = nullptr;
   double* nat_a = nullptr;                       // natural-order staging (host-pointer entry points)
   double* nat_b = nullptr;
+  // batch (multi-RHS) vectors, present when the workspace was bound with nrhs > 1: nrhs half-lattice spinors each
+  void* mhi[2] = {};                             // fp64: b, x
+  void* mlo[5] = {};                             // sloppy: x, r, p, t(=s), odd-site scratch; mlo_size bytes per real
+  size_t mlo_size = 0;
+  double* mscal = nullptr;                       // device scalars [64 systems][8]
+  double* mact = nullptr;                        // device activity mask [64]
+  double* h_mscal = nullptr;                     // pinned host mirrors
+  double* h_mact = nullptr;
   // reductions
   double* partials = nullptr;
   unsigned* ticket = nullptr;
@@ -96,7 +105,8 @@ int launch_gauge_pack(qxd_ctx* c, const double* U, const double* A);
 int launch_hoplinks(qxd_ctx* c, int prec);
 int launch_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed, int parity_mask /*1 even,2 odd,3 both*/, int compact_even);
 int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, int parity_mask, int compact_even);
-int launch_convert_spinor(qxd_ctx* c, int prec_from, const SpinorPtr& from, int prec_to, const SpinorPtr& to);
+int launch_convert_spinor(qxd_ctx* c, int prec_from, const SpinorPtr& from, int prec_to, const SpinorPtr& to, int n = 1, size_t rs_from = 0,
+                          size_t rs_to = 0);
 int launch_convert_record72(qxd_ctx* c, const void* from64, int prec_to, void* to);
 int launch_clover_export(qxd_ctx* c, double* out, int inverse);
 // clover.cu
@@ -110,27 +120,40 @@ struct DslashCall {
   SpinorPtr in[2];  // input spinor per parity (hop reads in[1-p]; DS_DW_FULL also in[p])
   SpinorPtr phi;    // PHI-term input on the output parity (modes with phi)
   SpinorPtr out[2]; // output per parity (only [parity_out] used unless DS_DW_FULL)
-  double* norm_result;  // DSF_NORM: device slot receiving |out|^2
+  double* norm_result;  // DSF_NORM: device slot receiving |out|^2 (right-hand side r: norm_result[r * norm_stride])
+  // multi-RHS launches (row a10): nrhs > 1 right-hand sides, rs_* bytes apart in in / phi / out
+  int nrhs;
+  size_t rs_in, rs_phi, rs_out;
+  int norm_stride;
 };
 int launch_dslash(qxd_ctx* c, const DslashCall& d);
 int launch_clover_apply(qxd_ctx* c, int prec, int inverse, int parity, const SpinorPtr& in, const SpinorPtr& out);
 // blas.cu
+// A batch of right-hand sides (row a10): n vectors rs bytes apart, per-system scalars ss doubles apart, optional
+// activity mask act[n] (1.0 = iterate, 0.0 = frozen).  The default is a single vector.
+struct Batch {
+  int n = 1;
+  size_t rs = 0;
+  int ss = 0;
+  const double* act = nullptr;
+};
 int blas_axpy(qxd_ctx* c, int prec, double a, const SpinorPtr& x, const SpinorPtr& y);            // y += a x
 int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* dev_result3);  // Re<x,y>, Im<x,y>, |y|^2
-int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* dev_result);
-int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x);
+int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* dev_result, const Batch& b = Batch());
+int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x, const Batch& b = Batch());
 // z = x + a*y + b*w with complex scalars by value (w may be unused when b == 0); BiCGstab building block
 int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai, const SpinorPtr& y, double br, double bi,
                   const SpinorPtr& w, const SpinorPtr& z);
 // alpha = *num / *den (device scalars): x += alpha p ; r -= alpha t ; *rr = |r|^2
 int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
-               const SpinorPtr& r, double* rr);
+               const SpinorPtr& r, double* rr, const Batch& b = Batch());
 // beta = *num / *den : p = s + beta p
-int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p);
+int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const Batch& b = Batch());
 int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi);                  // x_hi += x_lo ; x_lo = 0
 int blas_sub_norm(qxd_ctx* c, int prec, const SpinorPtr& b, const SpinorPtr& t, const SpinorPtr& r, double* res);  // r = b - t
-int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y);                       // y = x
+int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, const Batch& b = Batch());   // y = x
 // solver.cu
 int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
 
 }  // namespace qxd

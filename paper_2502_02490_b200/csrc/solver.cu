@@ -40,17 +40,24 @@ int read_scal(qxd_ctx* c, int idx, int n, double* out) {
 
 }  // namespace
 
-// out_e = D-hat in_e (dagger: D-hat^dag in_e); tmp_o: odd-site scratch of the same precision.
-int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out_e, const SpinorPtr& tmp_o, int dagger, double* norm_slot) {
+// out_e = D-hat in_e (dagger: D-hat^dag in_e); tmp_o: odd-site scratch of the same precision.  A batch b applies the
+// operator to b.n right-hand sides b.rs bytes apart with the multi-RHS kernels (row a10); norms go to norm_slot[k * b.ss].
+int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out_e, const SpinorPtr& tmp_o, int dagger, double* norm_slot,
+               const Batch& b) {
   DslashCall d1{};
   d1.prec = prec; d1.mode = DS_HOP_AINV; d1.flags = dagger ? DSF_G5IN : 0; d1.parity_out = 1;
   d1.in[0] = in_e; d1.out[1] = tmp_o;
+  d1.nrhs = b.n; d1.rs_in = d1.rs_phi = d1.rs_out = b.rs;
   QXD_TRY(launch_dslash(c, d1));
   DslashCall d2{};
   d2.prec = prec; d2.mode = DS_A_XMHOP; d2.flags = (dagger ? DSF_G5HOP : 0) | (norm_slot ? DSF_NORM : 0); d2.parity_out = 0;
-  d2.in[1] = tmp_o; d2.phi = in_e; d2.out[0] = out_e; d2.norm_result = norm_slot;
+  d2.in[1] = tmp_o; d2.phi = in_e; d2.out[0] = out_e; d2.norm_result = norm_slot; d2.norm_stride = b.ss;
+  d2.nrhs = b.n; d2.rs_in = d2.rs_phi = d2.rs_out = b.rs;
   QXD_TRY(launch_dslash(c, d2));
   return QXD_OK;
+}
+int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out_e, const SpinorPtr& tmp_o, int dagger, double* norm_slot) {
+  return apply_dhat(c, prec, in_e, out_e, tmp_o, dagger, norm_slot, Batch());
 }
 
 namespace {
@@ -246,6 +253,146 @@ int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd
   QXD_CUDA_OK(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
   info->seconds = ms * 1e-3;
   if (status == QXD_ENOCONV) c->err = "solve: not converged (maxiter or breakdown); psi holds the best iterate";
+  return status;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// Batched solve (rows a7 + a10, BASELINE config 4): nrhs independent CG iterations on the normal equations of D-hat
+// run in lockstep, so that every sloppy operator application is one multi-RHS dslash launch (links and clover blocks
+// read once for all right-hand sides, "solution of this system for many right-hand sides").  Every system
+// keeps its own scalars (device arrays, SS doubles apart) and its own reliable-update schedule; a system that has met
+// the fp64 residual target is frozen (alpha = beta = 0) until all are done.  Source preparation, reliable updates and
+// reconstruction run per right-hand side through the single-RHS fp64 kernels.
+// ---------------------------------------------------------------------------------------------------------------
+int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info) {
+  const int Vh = c->g.Vh;
+  const int plo = info[0].sloppy;
+  if (nrhs < 1 || nrhs > c->nrhs) return fail(c, QXD_EINVAL, "solve_multi: nrhs exceeds the value the workspace was bound for");
+  if (plo < 0 || plo >= NPREC || !((c->prec_mask >> plo) & 1)) return fail(c, QXD_EINVAL, "solve_multi: sloppy precision not bound");
+  if (prec_size(plo) > c->mlo_size) return fail(c, QXD_EINVAL, "solve_multi: the batch workspace is sized for a narrower sloppy precision");
+  if (info[0].algo != QXD_CGNE) return fail(c, QXD_EINVAL, "solve_multi: only QXD_CGNE is batched");
+  if (!(tol > 0.0)) return fail(c, QXD_EINVAL, "solve_multi: tol must be > 0");
+  const double delta = info[0].delta > 0.0 ? info[0].delta : 0.1;
+  const int maxiter = info[0].maxiter > 0 ? info[0].maxiter : 10000;
+  enum { SS = 8, M_GAM0 = 0, M_GAM1 = 1, M_TT = 2, M_RR = 3, M_RRT = 4 };
+  const size_t rs_hi = half_bytes(0, Vh), rs_lo = (half_bytes(plo, Vh) + 255) & ~size_t(255);
+  const size_t vnat = size_t(c->V) * 24;
+  // single-RHS scratch (fp64)
+  SpinorPtr eta_e = half_view(0, c->full_a, Vh, 0), eta_o = half_view(0, c->full_a, Vh, 1);
+  SpinorPtr out_e = half_view(0, c->full_b, Vh, 0), out_o = half_view(0, c->full_b, Vh, 1);
+  SpinorPtr thi = hv(0, c->sp64[3], Vh), tmp_o_hi = hv(0, c->sp64[4], Vh), rhi = hv(0, c->sp64[2], Vh);
+  // batch vectors
+  SpinorPtr B = hv(0, c->mhi[0], Vh), X = hv(0, c->mhi[1], Vh);
+  SpinorPtr xlo = hv(plo, c->mlo[0], Vh), rlo = hv(plo, c->mlo[1], Vh), p = hv(plo, c->mlo[2], Vh), t = hv(plo, c->mlo[3], Vh),
+            tmp_o = hv(plo, c->mlo[4], Vh);
+  double* ms = c->mscal;
+  double* hs = c->h_mscal;
+  Batch bl; bl.n = nrhs; bl.rs = rs_lo; bl.ss = SS; bl.act = c->mact;
+  Batch bh; bh.n = nrhs; bh.rs = rs_hi; bh.ss = SS;
+
+  QXD_CUDA_OK(c, cudaEventRecord(c->ev0, c->stream));
+  double eta2[64], stop2[64], maxr[64], rr_true[64];
+  int done[64], nrel[64], iters[64];
+  // ---- per right-hand side: pack, |eta|^2, source preparation b_k = eta_e - D_eo A_oo^{-1} eta_o (row a8) ----
+  for (int k = 0; k < nrhs; k++) {
+    QXD_TRY(launch_spinor_pack(c, 0, eta_nat + vnat * k, c->full_a, 3, 0));
+    QXD_TRY(blas_norm2(c, 0, eta_e, c->scal + SC_NE));
+    QXD_TRY(blas_norm2(c, 0, eta_o, c->scal + SC_NO));
+    double nn[2];
+    QXD_TRY(read_scal(c, SC_NE, 2, nn));
+    eta2[k] = nn[0] + nn[1];
+    stop2[k] = tol * tol * eta2[k];
+    QXD_TRY(launch_clover_apply(c, 0, 1, 1, eta_o, tmp_o_hi));
+    DslashCall d{};
+    d.prec = 0; d.mode = DS_X_MHOP; d.parity_out = 0; d.in[1] = tmp_o_hi; d.phi = eta_e; d.out[0] = rhs_view(B, rs_hi, k);
+    QXD_TRY(launch_dslash(c, d));
+  }
+  QXD_TRY(blas_zero(c, 0, X, bh));
+  QXD_TRY(blas_zero(c, plo, xlo, bl));
+  QXD_TRY(blas_norm2(c, 0, B, ms + M_RRT, bh));
+  QXD_TRY(launch_convert_spinor(c, 0, B, plo, rlo, nrhs, rs_hi, rs_lo));
+  QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  int nactive = 0;
+  for (int k = 0; k < nrhs; k++) {
+    rr_true[k] = hs[k * SS + M_RRT];
+    maxr[k] = std::sqrt(rr_true[k]);
+    done[k] = (rr_true[k] <= stop2[k]) ? 1 : 0;   // includes eta_k = 0
+    nrel[k] = 0; iters[k] = 0;
+    c->h_mact[k] = done[k] ? 0.0 : 1.0;
+    nactive += !done[k];
+  }
+  QXD_CUDA_OK(c, cudaMemcpyAsync(c->mact, c->h_mact, sizeof(double) * nrhs, cudaMemcpyHostToDevice, c->stream));
+  // fp64 true residual of system k:  x_hi += x_lo; x_lo = 0; r = b - D-hat x_hi; r_lo = r
+  auto reliable = [&](int k) -> int {
+    SpinorPtr xk = rhs_view(X, rs_hi, k);
+    QXD_TRY(blas_acc_hi(c, plo, rhs_view(xlo, rs_lo, k), xk));
+    QXD_TRY(apply_dhat(c, 0, xk, thi, tmp_o_hi, 0, nullptr));
+    QXD_TRY(blas_sub_norm(c, 0, rhs_view(B, rs_hi, k), thi, rhi, c->scal + SC_RRT));
+    QXD_TRY(launch_convert_spinor(c, 0, rhi, plo, rhs_view(rlo, rs_lo, k)));
+    QXD_TRY(read_scal(c, SC_RRT, 1, &rr_true[k]));
+    nrel[k]++;
+    return QXD_OK;
+  };
+  int it = 0;
+  if (nactive) {
+    QXD_TRY(apply_dhat(c, plo, rlo, t, tmp_o, 1, ms + M_GAM0, bl));   // s = A^dag r (s shares the buffer of t)
+    QXD_TRY(blas_copy(c, plo, t, p, bl));
+  }
+  while (nactive && it < maxiter) {
+    double* gam = ms + M_GAM0 + (it & 1);
+    double* gam_next = ms + M_GAM0 + ((it + 1) & 1);
+    QXD_TRY(apply_dhat(c, plo, p, t, tmp_o, 0, ms + M_TT, bl));
+    QXD_TRY(blas_cg_xr(c, plo, gam, ms + M_TT, p, t, xlo, rlo, ms + M_RR, bl));
+    QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
+    QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    it++;
+    bool changed = false;
+    for (int k = 0; k < nrhs; k++) {
+      if (done[k]) continue;
+      iters[k] = it;
+      const double rr = hs[k * SS + M_RR];
+      if (!(rr == rr)) { done[k] = 2; c->h_mact[k] = 0.0; changed = true; nactive--; continue; }  // breakdown
+      const double rn = std::sqrt(rr);
+      if (rn > maxr[k]) maxr[k] = rn;
+      if (rn < delta * maxr[k] || rr <= stop2[k]) {
+        QXD_TRY(reliable(k));
+        maxr[k] = std::sqrt(rr_true[k]);
+        if (rr_true[k] <= stop2[k]) { done[k] = 1; c->h_mact[k] = 0.0; changed = true; nactive--; }
+      }
+    }
+    if (changed) QXD_CUDA_OK(c, cudaMemcpyAsync(c->mact, c->h_mact, sizeof(double) * nrhs, cudaMemcpyHostToDevice, c->stream));
+    if (!nactive) break;
+    QXD_TRY(apply_dhat(c, plo, rlo, t, tmp_o, 1, gam_next, bl));
+    QXD_TRY(blas_cg_p(c, plo, gam_next, gam, t, p, bl));
+  }
+  int status = QXD_OK;
+  for (int k = 0; k < nrhs; k++) {
+    if (done[k] != 1) {   // leave the best iterate with its true residual
+      QXD_TRY(reliable(k));
+      if (rr_true[k] <= stop2[k]) done[k] = 1;
+    }
+    if (done[k] != 1) status = QXD_ENOCONV;
+    // reconstruction (row a8): psi_o = A_oo^{-1}(eta_o - D_oe psi_e)
+    QXD_TRY(launch_spinor_pack(c, 0, eta_nat + vnat * k, c->full_a, 2, 0));
+    DslashCall r{};
+    r.prec = 0; r.mode = DS_AINV_X_MHOP; r.parity_out = 1; r.in[0] = rhs_view(X, rs_hi, k); r.phi = eta_o; r.out[1] = out_o;
+    QXD_TRY(launch_dslash(c, r));
+    QXD_TRY(blas_copy(c, 0, rhs_view(X, rs_hi, k), out_e));
+    QXD_TRY(launch_spinor_unpack(c, 0, c->full_b, psi_nat + vnat * k, 3, 0));
+  }
+  QXD_CUDA_OK(c, cudaEventRecord(c->ev1, c->stream));
+  QXD_CUDA_OK(c, cudaEventSynchronize(c->ev1));
+  float ms_el = 0.f;
+  QXD_CUDA_OK(c, cudaEventElapsedTime(&ms_el, c->ev0, c->ev1));
+  for (int k = 0; k < nrhs; k++) {
+    info[k].algo = info[0].algo; info[k].sloppy = plo; info[k].delta = delta; info[k].maxiter = maxiter;
+    info[k].iters = iters[k]; info[k].n_reliable = nrel[k];
+    info[k].true_res = eta2[k] > 0.0 ? std::sqrt(rr_true[k] / eta2[k]) : 0.0;
+    info[k].seconds = ms_el * 1e-3;
+  }
+  if (status == QXD_ENOCONV) c->err = "solve_multi: at least one system not converged (maxiter or breakdown); psi holds the best iterates";
   return status;
 }
 

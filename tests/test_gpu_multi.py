@@ -1,0 +1,85 @@
+"""GPU parity of the multi-RHS path (BASELINE config 4): the batched D_w and the batched
+mixed-precision solve against the fp64 CPU oracle, right-hand side by right-hand side.  Tolerances as in
+test_gpu_parity.py (fp64 1e-13, fp32 1e-6, fp16 2e-3; solves: true residual with the oracle's D)."""
+import numpy as np
+import pytest
+
+import synth
+from test_gpu_parity import Case, relerr, to_np, TOL, F64, F32, F16
+
+pytestmark = pytest.mark.gpu
+
+
+def true_residual(ref, eta, psi):
+    return np.linalg.norm(np.ravel(eta - ref.apply_Dw(psi))) / np.linalg.norm(np.ravel(eta))
+
+
+# nrhs chosen to be ragged against 2 and 3 right-hand sides per thread; Vh = 720 has a ragged tile tail
+@pytest.mark.parametrize("dims,cstar,qed,nrhs", [((6, 4, 6, 10), 0, False, 5), ((6, 4, 4, 6), 3, True, 4), ((4, 4, 4, 4), 0, True, 1)])
+@pytest.mark.parametrize("prec", [F64, F32, F16])
+@pytest.mark.parametrize("rpt", [0, 1, 2, 3])
+def test_apply_Dw_multi(dims, cstar, qed, nrhs, prec, rpt):
+    import torch
+    c = Case(dims, cstar, 1, qed, nrhs=max(nrhs, 2))
+    g = c.gpu
+    g.set_rhs_per_thread(rpt)
+    etas = [synth.gaussian_spinor(c.dims_ext, 11 + k) for k in range(nrhs)]
+    nb = g.packed_spinor_bytes(prec)
+    pin = torch.zeros(nrhs * nb, dtype=torch.uint8, device="cuda")
+    pout = torch.zeros_like(pin)
+    for k in range(nrhs):
+        g.spinor_pack(etas[k], prec, packed=pin[k * nb:(k + 1) * nb])
+    g.apply_Dw_multi_packed(pin, pout, prec, nrhs)
+    for k in range(nrhs):
+        got = to_np(g.spinor_unpack(pout[k * nb:(k + 1) * nb], prec))
+        assert relerr(got, c.ref.apply_Dw(etas[k])) < TOL[prec], (k, prec, rpt)
+    # the batched launch must agree bit for bit with nrhs single launches (same arithmetic per site)
+    single = torch.zeros(nb, dtype=torch.uint8, device="cuda")
+    g.apply_Dw_packed(pin[:nb], single, prec)
+    assert torch.equal(single, pout[:nb])
+    c.close()
+
+
+@pytest.mark.parametrize("sloppy", [F32, F16])
+@pytest.mark.parametrize("rpt", [0, 2])
+def test_solve_multi(sloppy, rpt):
+    """Five systems (one of them with a zero source, one a multiple of another) to 1e-10 in lockstep."""
+    dims = (8, 4, 4, 8)
+    c = Case(dims, 3, 1, True, q=-1 / 3, kappa=0.125, csw=1.5, csw_qed=1.0, eps=0.2, nrhs=5)
+    c.gpu.set_rhs_per_thread(rpt)
+    etas = np.stack([synth.gaussian_spinor(c.dims_ext, 21 + k) for k in range(5)])
+    etas[2] = 0.0
+    etas[4] = 1e-3 * etas[0]
+    psi, infos = c.gpu.solve_multi(etas, 1e-10, sloppy=sloppy, delta=0.1)
+    psi = to_np(psi).reshape(etas.shape)
+    for k in range(5):
+        assert infos[k]["status"] == 0, infos[k]
+        if k == 2:
+            assert np.all(psi[k] == 0) and infos[k]["iters"] == 0
+            continue
+        assert true_residual(c.ref, etas[k], psi[k]) <= 1.05e-10, (k, infos[k])
+        assert infos[k]["n_reliable"] >= 2
+    # in-place (psi aliases eta) gives the same solutions
+    import torch
+    buf = torch.from_numpy(etas).cuda()
+    c.gpu.solve_multi(buf, 1e-10, sloppy=sloppy, delta=0.1, psi=buf)
+    assert relerr(to_np(buf).reshape(etas.shape)[[0, 1, 3, 4]], psi[[0, 1, 3, 4]]) < 1e-8
+    c.close()
+
+
+def test_solve_multi_argument_errors():
+    c = Case((4, 4, 4, 4), 0, 1, False, precisions=(F64, F32), nrhs=2)
+    B = c.B
+    etas = np.stack([synth.gaussian_spinor(c.dims_ext, 31 + k) for k in range(3)])
+    with pytest.raises(B.QxdError) as e:
+        c.gpu.solve_multi(etas, 1e-10, sloppy=F32)            # 3 systems, workspace bound for 2
+    assert e.value.status == B.QXD_EINVAL
+    with pytest.raises(B.QxdError) as e:
+        c.gpu.solve_multi(etas[:2], 1e-10, sloppy=F64)        # batch vectors sized for fp32
+    assert e.value.status == B.QXD_EINVAL
+    c.close()
+    c1 = Case((4, 4, 4, 4), 0, 1, False, precisions=(F64, F32), nrhs=1)
+    with pytest.raises(B.QxdError) as e:
+        c1.gpu.solve_multi(etas[:1], 1e-10, sloppy=F32)       # workspace bound without a batch
+    assert e.value.status == B.QXD_EWORKSPACE
+    c1.close()
