@@ -61,7 +61,6 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.nrhs = d.nrhs > 1 ? d.nrhs : 1; a.ngroups = 1;
   a.rs_in = d.rs_in; a.rs_phi = d.rs_phi; a.rs_out = d.rs_out;
   if (a.nrhs > 64) return fail(c, QXD_EINVAL, "dslash: at most 64 right-hand sides per launch");
-  { static const int pf = getenv("QXD_PREFETCH") ? atoi(getenv("QXD_PREFETCH")) : 0; a.prefetch = pf; }
   a.R.partials = c->partials; a.R.ticket = c->ticket; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
   int rc = d.prec == 0 ? dslash_dispatch_f64(c, d, a) : d.prec == 1 ? dslash_dispatch_f32(c, d, a) : dslash_dispatch_f16(c, d, a);
   if (rc) return rc;

@@ -12,7 +12,6 @@ struct DslashArgs {
   const void* W[2];
   const void* CL[2];
   int parity_out;
-  int prefetch;
   int nrhs;            // right-hand sides in this launch (row a10); 1 for the single-spinor entry points
   int ngroups;         // ceil(nrhs / R): consecutive CTAs work on the same tile for different groups of R right-hand sides
   size_t rs_in, rs_phi, rs_out;   // byte distance between consecutive right-hand sides

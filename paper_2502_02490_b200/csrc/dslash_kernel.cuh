@@ -44,31 +44,34 @@ __device__ __forceinline__ void project(const C* psi, C* h) {
     }
   }
 }
-// acc_u += r ; acc_l += lower part reconstructed from r
-template <int MU, int SGN, typename C>
-__device__ __forceinline__ void reconstruct(const C* r, C* acc) {
-  const C s = (C)SGN;
+// acc_u += sc * r ; acc_l += sc * (lower part reconstructed from r).  sc = 1 except for fp16 storage, where it is the
+// block-float scale of the neighbour spinor: folding it into these FMAs costs nothing (the link multiply is linear).
+template <int MU, int SGN, bool SCALED, typename C>
+__device__ __forceinline__ void reconstruct(const C* r, C* acc, C sc) {
+  const C p = SCALED ? sc : (C)1, sp = (C)SGN * p, sm = -sp;   // +-scale with the sign of the hop direction
 #pragma unroll
   for (int a = 0; a < 3; a++) {
     const C r0r = r[2 * a], r0i = r[2 * a + 1], r1r = r[6 + 2 * a], r1i = r[6 + 2 * a + 1];
-    acc[2 * a] += r0r; acc[2 * a + 1] += r0i;
-    acc[6 + 2 * a] += r1r; acc[6 + 2 * a + 1] += r1i;
+    acc[2 * a] += p * r0r; acc[2 * a + 1] += p * r0i;
+    acc[6 + 2 * a] += p * r1r; acc[6 + 2 * a + 1] += p * r1i;
     if (MU == 0) {        // lower = s * (r0, r1)
-      acc[12 + 2 * a] += s * r0r; acc[12 + 2 * a + 1] += s * r0i;
-      acc[18 + 2 * a] += s * r1r; acc[18 + 2 * a + 1] += s * r1i;
+      acc[12 + 2 * a] += sp * r0r; acc[12 + 2 * a + 1] += sp * r0i;
+      acc[18 + 2 * a] += sp * r1r; acc[18 + 2 * a + 1] += sp * r1i;
     } else if (MU == 1) { // lower = -s * (i r1, i r0)
-      acc[12 + 2 * a] += s * r1i; acc[12 + 2 * a + 1] -= s * r1r;
-      acc[18 + 2 * a] += s * r0i; acc[18 + 2 * a + 1] -= s * r0r;
+      acc[12 + 2 * a] += sp * r1i; acc[12 + 2 * a + 1] += sm * r1r;
+      acc[18 + 2 * a] += sp * r0i; acc[18 + 2 * a + 1] += sm * r0r;
     } else if (MU == 2) { // lower = -s * (r1, -r0)
-      acc[12 + 2 * a] -= s * r1r; acc[12 + 2 * a + 1] -= s * r1i;
-      acc[18 + 2 * a] += s * r0r; acc[18 + 2 * a + 1] += s * r0i;
+      acc[12 + 2 * a] += sm * r1r; acc[12 + 2 * a + 1] += sm * r1i;
+      acc[18 + 2 * a] += sp * r0r; acc[18 + 2 * a + 1] += sp * r0i;
     } else {              // lower = -s * (i r0, -i r1)
-      acc[12 + 2 * a] += s * r0i; acc[12 + 2 * a + 1] -= s * r0r;
-      acc[18 + 2 * a] -= s * r1i; acc[18 + 2 * a + 1] += s * r1r;
+      acc[12 + 2 * a] += sp * r0i; acc[12 + 2 * a + 1] += sm * r0r;
+      acc[18 + 2 * a] += sm * r1i; acc[18 + 2 * a + 1] += sp * r1r;
     }
   }
 }
 // r[s][a] = sum_b W[a][b] h[s][b]   (ADJ: sum_b conj(W[b][a]) h[s][b])
+// Written as chains of single multiply-adds so that every product is one FMA (re += a*b - c*d would cost three
+// instructions: multiply, FMA, add).
 template <bool ADJ, typename C>
 __device__ __forceinline__ void link_mul(const C* w, const C* h, C* r) {
 #pragma unroll
@@ -79,10 +82,10 @@ __device__ __forceinline__ void link_mul(const C* w, const C* h, C* r) {
 #pragma unroll
       for (int b = 0; b < 3; b++) {
         const C wr = ADJ ? w[2 * (3 * b + a)] : w[2 * (3 * a + b)];
-        const C wi = ADJ ? -w[2 * (3 * b + a) + 1] : w[2 * (3 * a + b) + 1];
+        const C wi = ADJ ? w[2 * (3 * b + a) + 1] : w[2 * (3 * a + b) + 1];
         const C hr = h[6 * s + 2 * b], hi = h[6 * s + 2 * b + 1];
-        re += wr * hr - wi * hi;
-        im += wr * hi + wi * hr;
+        if (b == 0) { re = wr * hr; im = wr * hi; } else { re += wr * hr; im += wr * hi; }
+        if (ADJ) { re += wi * hi; im -= wi * hr; } else { re -= wi * hi; im += wi * hr; }
       }
       r[6 * s + 2 * a] = re; r[6 * s + 2 * a + 1] = im;
     }
@@ -100,11 +103,11 @@ __device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
     for (int j = i + 1; j < 6; j++) {
       const C ur = b[k], ui = b[k + 1];
       k += 2;
-      // out_i += u in_j ; out_j += conj(u) in_i
-      out[2 * i] += ur * in[2 * j] - ui * in[2 * j + 1];
-      out[2 * i + 1] += ur * in[2 * j + 1] + ui * in[2 * j];
-      out[2 * j] += ur * in[2 * i] + ui * in[2 * i + 1];
-      out[2 * j + 1] += ur * in[2 * i + 1] - ui * in[2 * i];
+      // out_i += u in_j ; out_j += conj(u) in_i   (one FMA per product)
+      out[2 * i] += ur * in[2 * j]; out[2 * i] -= ui * in[2 * j + 1];
+      out[2 * i + 1] += ur * in[2 * j + 1]; out[2 * i + 1] += ui * in[2 * j];
+      out[2 * j] += ur * in[2 * i]; out[2 * j] += ui * in[2 * i + 1];
+      out[2 * j + 1] += ur * in[2 * i + 1]; out[2 * j + 1] -= ui * in[2 * i];
     }
 }
 template <typename S>
@@ -156,6 +159,7 @@ __device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, in
     const V* p = reinterpret_cast<const V*>(static_cast<const char*>(a.in[1 - parity].data) + a.rs_in * (rhs0 + r));
 #pragma unroll
     for (int c = 0; c < HopRegs<S, R>::NPSI; c++) d.psi[r][c] = ldg_pinned(p + size_t(c) * Vh + nb);
+    d.scale[r] = 1.f;
     if (PT<S>::ID == 2) d.scale[r] = ldg_pinned(reinterpret_cast<const float*>(reinterpret_cast<const char*>(a.in[1 - parity].scale) + a.rs_in * (rhs0 + r)) + nb);
   }
   // forward: W_mu(x) of the own parity; backward: W_mu(x-mu) of the other parity at the neighbour
@@ -177,17 +181,13 @@ __device__ __forceinline__ void hop_use(const HopRegs<S, R>& d, typename PT<S>::
     C psi[24], h[12], t[12];
 #pragma unroll
     for (int c = 0; c < HopRegs<S, R>::NPSI; c++) unpack_vec(d.psi[r][c], psi + c * RPC);
-    if (PT<S>::ID == 2) {
-#pragma unroll
-      for (int i = 0; i < 24; i++) psi[i] *= d.scale[r];
-    }
     if (G5IN) {
 #pragma unroll
       for (int i = 12; i < 24; i++) psi[i] = -psi[i];
     }
     project<MU, DIR>(psi, h);
     link_mul<(DIR < 0)>(wv + LC::OFF, h, t);
-    reconstruct<MU, DIR>(t, acc[r]);
+    reconstruct<MU, DIR, PT<S>::ID == 2>(t, acc[r], (C)d.scale[r]);
   }
 }
 // all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one
@@ -224,42 +224,6 @@ __device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int 
   }
 }
 
-// Bulk L2 prefetch (cp.async.bulk.prefetch.L2, sm_90+): the compulsory DRAM streams of a CTA -- its own links, its
-// clover blocks and its own spinors -- are contiguous 16 B x 128-site rows of the chunk-major SoA records.  One thread per
-// row asks the L2 for the whole row when the CTA starts, so the per-thread 16-byte loads that follow (one hop after the
-// other, bounded by registers) find their lines in L2 or already in flight instead of paying one DRAM latency per hop.
-__device__ __forceinline__ void bulk_prefetch_l2(const void* p, unsigned bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
-template <typename S, int PHI, bool FULL>
-__device__ __forceinline__ void cta_prefetch(const DslashArgs& a, int cb0) {
-  constexpr int NW = 72 / PT<S>::RPC, NS = 24 / PT<S>::RPC;   // rows per parity: links, clover (NW each), spinor (NS)
-  const int Vh = a.g.Vh;
-  const int n = min(128, Vh - cb0);
-  if (n <= 0) return;
-  const unsigned bytes = unsigned(n) * 16u;
-  const int t = threadIdx.x;
-  if (FULL) {
-    // rows: [parity][W NW | CL NW | psi NS]
-    constexpr int PER = 2 * NW + NS;
-    if (t < 2 * PER) {
-      const int p = t / PER, r = t % PER;
-      const char* base = r < NW ? (const char*)a.W[p] : r < 2 * NW ? (const char*)a.CL[p] : (const char*)a.in[p].data;
-      const int c = r < NW ? r : r < 2 * NW ? r - NW : r - 2 * NW;
-      bulk_prefetch_l2(base + (size_t(c) * Vh + cb0) * 16, bytes);
-    }
-  } else {
-    // own forward links, clover (or inverse) block, phi
-    constexpr int PER = 2 * NW + (PHI ? NS : 0);
-    if (t < PER) {
-      const int p = a.parity_out;
-      const char* base = t < NW ? (const char*)a.W[p] : t < 2 * NW ? (const char*)a.CL[p] : (const char*)a.phi.data;
-      const int c = t < NW ? t : t < 2 * NW ? t - NW : t - 2 * NW;
-      bulk_prefetch_l2(base + (size_t(c) * Vh + cb0) * 16, bytes);
-    }
-  }
-}
-
 // PHI: 0 none, 1 phi, 2 M*phi (FULL: phi = in on the own parity).  POST: 1 = multiply the result by M^{-1}.
 // Full-lattice launches (row a4) put both parities of 128 consecutive checkerboard indices -- one 4x4x4x4 tile with
 // the default order -- into one CTA of 256 threads (warps 0-3 even, 4-7 odd): every link is then used twice by the same
@@ -281,7 +245,6 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
   const int rhs0 = R > 1 ? (blockIdx.x - tile * a.ngroups) * R : 0;
   const int cb = tile * 128 + (threadIdx.x & 127);
   const int parity = FULL ? (threadIdx.x >> 7) : a.parity_out;
-  if (a.prefetch) cta_prefetch<S, PHI, FULL>(a, tile * 128);
   double nrm[R];
 #pragma unroll
   for (int r = 0; r < R; r++) nrm[r] = 0.0;
@@ -293,8 +256,8 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
     for (int r = 0; r < R; r++)
 #pragma unroll
       for (int i = 0; i < 24; i++) acc[r][i] = 0;
-    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL>::PIPE>(a, s, cb, parity, rhs0, acc);
     const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
+    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL>::PIPE>(a, s, cb, parity, rhs0, acc);
 #pragma unroll
     for (int r = 0; r < R; r++)
 #pragma unroll
