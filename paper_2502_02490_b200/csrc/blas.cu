@@ -99,6 +99,47 @@ __global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const d
   store_spinor<S>(p, Vh, cb, vp);
 }
 
+// fp16 sloppy operator with fp32 Krylov vectors (reading R12): the CG vectors x, r, p are kept in float,
+// only the operator's inputs (p, r) and outputs (t, s) are binary16.  Rounding x, r and p themselves to 11-bit
+// mantissas every iteration was measured to cost 2.8x the iterations of the fp32 solver at config c3.
+//   x += alpha p ; r -= alpha t(half) ; r16 = half(r) ; result = |r|^2
+__global__ void __launch_bounds__(128) cg_xr_h_k(int Vh, const double* num, const double* den, SpinorPtr p, SpinorPtr t, SpinorPtr x,
+                                                 SpinorPtr r, SpinorPtr r16, Reducer R) {
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  double nrm[1] = {0.0};
+  if (cb < Vh) {
+    const double dn = den[0];
+    const float al = dn == 0.0 ? 0.f : (float)(num[0] / dn);
+    float vp[24], vx[24];
+    load_spinor<float>(p, Vh, cb, vp);
+    load_spinor<float>(x, Vh, cb, vx);
+#pragma unroll
+    for (int i = 0; i < 24; i++) vx[i] += al * vp[i];
+    store_spinor<float>(x, Vh, cb, vx);
+    load_spinor<__half>(t, Vh, cb, vp);
+    load_spinor<float>(r, Vh, cb, vx);
+#pragma unroll
+    for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; nrm[0] += (double)vx[i] * (double)vx[i]; }
+    store_spinor<float>(r, Vh, cb, vx);
+    store_spinor<__half>(r16, Vh, cb, vx);
+  }
+  grid_reduce<1>(nrm, R);
+}
+//   p = s(half) + beta p ; p16 = half(p)
+__global__ void __launch_bounds__(128) cg_p_h_k(int Vh, const double* num, const double* den, SpinorPtr s, SpinorPtr p, SpinorPtr p16) {
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  const double dn = den[0];
+  const float be = dn == 0.0 ? 0.f : (float)(num[0] / dn);
+  float vs[24], vp[24];
+  load_spinor<__half>(s, Vh, cb, vs);
+  load_spinor<float>(p, Vh, cb, vp);
+#pragma unroll
+  for (int i = 0; i < 24; i++) vp[i] = vs[i] + be * vp[i];
+  store_spinor<float>(p, Vh, cb, vp);
+  store_spinor<__half>(p16, Vh, cb, vp);
+}
+
 template <typename S>
 __global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R, size_t rs) {
   typedef typename PT<S>::C C;
@@ -215,6 +256,17 @@ int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const
 }
 int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const Batch& b) {
   QXD_BY_PREC(prec, cg_p_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, num, den, s, p, b.rs, b.ss, b.act));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_cg_xr_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
+                 const SpinorPtr& r, const SpinorPtr& r16, double* rr) {
+  cg_xr_h_k<<<QXD_GRID>>>(c->g.Vh, num, den, p, t, x, r, r16, reducer(c, rr));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const SpinorPtr& p16) {
+  cg_p_h_k<<<QXD_GRID>>>(c->g.Vh, num, den, s, p, p16);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

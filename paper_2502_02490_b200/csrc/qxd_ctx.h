@@ -149,6 +149,10 @@ int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const
                const SpinorPtr& r, double* rr, const Batch& b = Batch());
 // beta = *num / *den : p = s + beta p
 int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const Batch& b = Batch());
+// fp16 operator with fp32 vectors: x, r, p in float; t, s and the operator inputs r16, p16 in binary16
+int blas_cg_xr_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
+                 const SpinorPtr& r, const SpinorPtr& r16, double* rr);
+int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const SpinorPtr& p16);
 int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi);                  // x_hi += x_lo ; x_lo = 0
 int blas_sub_norm(qxd_ctx* c, int prec, const SpinorPtr& b, const SpinorPtr& t, const SpinorPtr& r, double* res);  // r = b - t
 int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, const Batch& b = Batch());   // y = x

@@ -63,11 +63,12 @@ int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out
 namespace {
 
 // fp64 true residual: x_hi += x_lo; x_lo = 0; r_hi = b - D-hat x_hi; r_lo = r_hi; returns |r_hi|^2
-int reliable_update(qxd_ctx* c, int plo, Ws& w, double* rr_true) {
+int reliable_update(qxd_ctx* c, int plo, Ws& w, double* rr_true, const SpinorPtr* r16 = nullptr) {
   QXD_TRY(blas_acc_hi(c, plo, w.xlo, w.xhi));
   QXD_TRY(apply_dhat(c, 0, w.xhi, w.thi, w.tmp_o_hi, 0, nullptr));
   QXD_TRY(blas_sub_norm(c, 0, w.b, w.thi, w.rhi, c->scal + SC_RRT));
   QXD_TRY(launch_convert_spinor(c, 0, w.rhi, plo, w.rlo));
+  if (r16) QXD_TRY(launch_convert_spinor(c, 0, w.rhi, 2, *r16));
   QXD_TRY(read_scal(c, SC_RRT, 1, rr_true));
   return QXD_OK;
 }
@@ -75,7 +76,16 @@ int reliable_update(qxd_ctx* c, int plo, Ws& w, double* rr_true) {
 // CG on the normal equations of D-hat keeping the system residual (reading R11):
 //   s = A^dag r, p = s, gam = |s|^2; loop: t = A p; al = gam/|t|^2; x += al p; r -= al t; s = A^dag r;
 //   gam' = |s|^2; p = s + (gam'/gam) p.
-int cgne(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter, qxd_solve_info* info) {
+int cgne(qxd_ctx* c, int pop, Ws& w0, double stop2, double delta, int maxiter, qxd_solve_info* info) {
+  // pop: precision of the sloppy operator; plo: precision of the Krylov vectors x, r, p.  With a binary16 operator the
+  // vectors stay in float and the operator reads binary16 copies r16 (slot v) and p16 (slot r0), see blas.cu.
+  const bool h16 = (pop == 2);
+  const int plo = h16 ? 1 : pop;
+  Ws w = w0;
+  SpinorPtr r16 = w0.v, p16 = w0.r0;
+  if (h16) { w.xlo.scale = nullptr; w.rlo.scale = nullptr; w.p.scale = nullptr; }
+  const SpinorPtr& rin = h16 ? r16 : w.rlo;   // operator inputs
+  const SpinorPtr& pin = h16 ? p16 : w.p;
   double rr = 0;
   QXD_TRY(blas_zero(c, 0, w.xhi));
   QXD_TRY(blas_zero(c, plo, w.xlo));
@@ -83,31 +93,35 @@ int cgne(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter, qx
   QXD_TRY(blas_norm2(c, 0, w.rhi, c->scal + SC_RRT));
   QXD_TRY(read_scal(c, SC_RRT, 1, &rr));
   QXD_TRY(launch_convert_spinor(c, 0, w.rhi, plo, w.rlo));
+  if (h16) QXD_TRY(launch_convert_spinor(c, 0, w.rhi, 2, r16));
   int it = 0, nrel = 0, status = QXD_ENOCONV;
   double maxr = std::sqrt(rr), rr_true = rr;
   if (rr <= stop2) status = QXD_OK;
   if (status != QXD_OK) {
-    QXD_TRY(apply_dhat(c, plo, w.rlo, w.s, w.tmp_o_lo, 1, c->scal + SC_GAM0));
-    QXD_TRY(blas_copy(c, plo, w.s, w.p));
+    QXD_TRY(apply_dhat(c, pop, rin, w.s, w.tmp_o_lo, 1, c->scal + SC_GAM0));
+    QXD_TRY(launch_convert_spinor(c, pop, w.s, plo, w.p));
+    if (h16) QXD_TRY(blas_copy(c, 2, w.s, p16));
   }
   while (status != QXD_OK && it < maxiter) {
     double* gam = c->scal + SC_GAM0 + (it & 1);
     double* gam_next = c->scal + SC_GAM0 + ((it + 1) & 1);
-    QXD_TRY(apply_dhat(c, plo, w.p, w.t, w.tmp_o_lo, 0, c->scal + SC_TT));
-    QXD_TRY(blas_cg_xr(c, plo, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, c->scal + SC_RR));
+    QXD_TRY(apply_dhat(c, pop, pin, w.t, w.tmp_o_lo, 0, c->scal + SC_TT));
+    if (h16) QXD_TRY(blas_cg_xr_h(c, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, r16, c->scal + SC_RR));
+    else QXD_TRY(blas_cg_xr(c, plo, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, c->scal + SC_RR));
     QXD_TRY(read_scal(c, SC_RR, 1, &rr));
     it++;
     if (!(rr == rr)) break;  // NaN: breakdown
     double rn = std::sqrt(rr);
     if (rn > maxr) maxr = rn;
     if (rn < delta * maxr || rr <= stop2) {
-      QXD_TRY(reliable_update(c, plo, w, &rr_true));
+      QXD_TRY(reliable_update(c, plo, w, &rr_true, h16 ? &r16 : nullptr));
       nrel++;
       maxr = std::sqrt(rr_true);
       if (rr_true <= stop2) { status = QXD_OK; break; }
     }
-    QXD_TRY(apply_dhat(c, plo, w.rlo, w.s, w.tmp_o_lo, 1, gam_next));
-    QXD_TRY(blas_cg_p(c, plo, gam_next, gam, w.s, w.p));
+    QXD_TRY(apply_dhat(c, pop, rin, w.s, w.tmp_o_lo, 1, gam_next));
+    if (h16) QXD_TRY(blas_cg_p_h(c, gam_next, gam, w.s, w.p, p16));
+    else QXD_TRY(blas_cg_p(c, plo, gam_next, gam, w.s, w.p));
   }
   if (status != QXD_OK) {  // leave the best iterate in x_hi with its true residual
     QXD_TRY(reliable_update(c, plo, w, &rr_true));
