@@ -123,6 +123,15 @@ int qxd_set_quark(qxd_ctx* ctx, double kappa, double q);
  * Builds M(x) = (4+m0) + c_sw (i/4) sigma.F-hat + q c_sw_qed (i/4) sigma.A-hat as two Hermitian
  * 6x6 blocks per site and inverts both blocks, on the device.  Needs gauge + quark. */
 int qxd_clover_build(qxd_ctx* ctx, double csw, double csw_qed);
+/* Storage format of the hopping links W = e^{iqA} U (north_star "12-real SU(3) reconstruct and the U(1)
+ * phase fused into the link multiply").  QXD_RECON_NONE: all 18 reals of W.  QXD_RECON_12: rows 0 and 1 of W (12 reals)
+ * plus det W = e^{3iqA} det U (x -1 on the antiperiodic time boundary) as (re, im) = 14 reals per link; the dslash rebuilds
+ * row 2 = det W * conj(row0 x row1), which holds for every unitary W, so the phase costs no separate multiply.  Traffic per
+ * D_w site drops from 192 to 176 reals.  The input links must be unitary to the working precision (they are only used
+ * through this identity); det U is computed, not assumed to be 1.  May be called at any time; if a quark is set the links
+ * of every bound precision are rewritten in the new format.  Other values -> QXD_EINVAL. */
+enum { QXD_RECON_NONE = 18, QXD_RECON_12 = 12 };
+int qxd_set_gauge_reconstruct(qxd_ctx* ctx, int recon);
 /* Copy the fp64 clover field (inverse != 0: the block inverses) to natural order, out: DEVICE
  * [V][2][36] doubles, packing of PAPER.md:117. */
 int qxd_clover_export(qxd_ctx* ctx, double* out, int inverse);

@@ -11,6 +11,7 @@ import os
 
 QXD_F64, QXD_F32, QXD_F16 = 0, 1, 2
 QXD_CGNE, QXD_BICGSTAB = 0, 1
+QXD_RECON_NONE, QXD_RECON_12 = 18, 12
 QXD_OK, QXD_EINVAL, QXD_ESTATE, QXD_EWORKSPACE, QXD_ECUDA, QXD_ENOCONV = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -49,6 +50,7 @@ SYMBOLS = {
     "qxd_gauge_load": (_i, [_vp, _vp, _vp, _d]),
     "qxd_set_quark": (_i, [_vp, _d, _d]),
     "qxd_clover_build": (_i, [_vp, _d, _d]),
+    "qxd_set_gauge_reconstruct": (_i, [_vp, _i]),
     "qxd_clover_export": (_i, [_vp, _vp, _i]),
     "qxd_apply_Dw": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dhat_eo": (_i, [_vp, _i, _vp, _vp, _i]),
@@ -240,6 +242,9 @@ class Qxd:
         infos[0].algo, infos[0].sloppy, infos[0].delta, infos[0].maxiter = QXD_CGNE, sloppy, delta, maxiter
         rc = self._chk(self.lib.qxd_solve_multi(self.h, nrhs, _ptr(eta), _ptr(psi), float(tol), infos), allow=(QXD_ENOCONV,))
         return psi, [self._report(rc, infos[k]) for k in range(nrhs)]
+
+    def set_gauge_reconstruct(self, recon):
+        self._chk(self.lib.qxd_set_gauge_reconstruct(self.h, int(recon)))
 
     def set_rhs_per_thread(self, r):
         self._chk(self.lib.qxd_set_rhs_per_thread(self.h, int(r)))

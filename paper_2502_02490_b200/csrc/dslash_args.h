@@ -19,9 +19,12 @@ struct DslashArgs {
 };
 
 
-// one translation unit per storage precision (dslash_f64.cu, dslash_f32.cu, dslash_f16.cu)
-int dslash_dispatch_f64(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f32(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f16(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+// one translation unit per storage precision and link format (dslash_f64_l18.cu, ..., dslash_f16_l14.cu)
+int dslash_dispatch_f64_l18(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32_l18(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16_l18(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f64_l14(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32_l14(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16_l14(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
 
 }  // namespace qxd

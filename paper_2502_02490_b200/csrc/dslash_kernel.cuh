@@ -133,24 +133,44 @@ __device__ __forceinline__ void clover_mul_multi(const void* CL, int Vh, int cb,
 // One hop in flight: the raw 16-byte chunks of the neighbour spinor and of the link, exactly as loaded.  Keeping the
 // packed vectors (not the unpacked reals) in registers between issue and use lets two hops be in flight per thread
 // (software pipeline in hop_all below): the kernel is bound by memory latency x bytes in flight, not by arithmetic.
-template <typename S, int R>
+// NL = stored reals per link: 18 (full 3x3) or 14 (rows 0 and 1 + det W = e^{3iqA} (-1)^{bc}: "12-real reconstruct with
+// the U(1) phase fused", row 2 = det W * conj(row0 x row1) for any U(3) matrix W; north_star).
+template <typename S, int R, int NL>
 struct HopRegs {
   typedef typename PT<S>::V V;
   static constexpr int RPC = PT<S>::RPC;
   static constexpr int NPSI = 24 / RPC;
   V psi[R][NPSI];
-  static constexpr int NWC = RPC == 2 ? 9 : RPC == 4 ? 5 : 3;
-  V w[NWC];        // chunks covering the 18 reals of one link (loaded once for all R right-hand sides)
+  static constexpr int NWC = NL == 18 ? (RPC == 2 ? 9 : RPC == 4 ? 5 : 3) : (RPC == 2 ? 7 : RPC == 4 ? 4 : 3);
+  V w[NWC];        // chunks covering the NL reals of one link (loaded once for all R right-hand sides)
   float scale[R];  // fp16 block-float scale of the neighbour spinor
 };
-template <int MU, typename S> struct LinkChunks {
+template <int MU, typename S, int NL> struct LinkChunks {
   static constexpr int RPC = PT<S>::RPC;
-  static constexpr int C0 = (18 * MU) / RPC, C1 = (18 * MU + 17) / RPC, N = C1 - C0 + 1, OFF = 18 * MU - C0 * RPC;
+  static constexpr int C0 = (NL * MU) / RPC, C1 = (NL * MU + NL - 1) / RPC, N = C1 - C0 + 1, OFF = NL * MU - C0 * RPC;
 };
-template <typename S, int MU, int DIR, int R>
-__device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, HopRegs<S, R>& d) {
+// row 2 of a U(3) matrix from rows 0, 1 and its determinant: w[12..17] = det * conj(row0 x row1); in: w[0..11], det = (w[12], w[13])
+template <typename C>
+__device__ __forceinline__ void reconstruct_row2(const C* in, C* w) {
+#pragma unroll
+  for (int i = 0; i < 12; i++) w[i] = in[i];
+  const C dr = in[12], di = in[13];
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    const int a = (c + 1) % 3, b = (c + 2) % 3;
+    const C ar = in[2 * a], ai = in[2 * a + 1], br = in[2 * b], bi = in[2 * b + 1];                    // row 0
+    const C pr = in[6 + 2 * a], pi = in[6 + 2 * a + 1], qr = in[6 + 2 * b], qi = in[6 + 2 * b + 1];    // row 1
+    C zr = ar * qr; zr -= ai * qi; zr -= br * pr; zr += bi * pi;                                       // z = r0[a] r1[b] - r0[b] r1[a]
+    C zi = ar * qi; zi += ai * qr; zi -= br * pi; zi -= bi * pr;
+    C rr = dr * zr; rr += di * zi;                                                                     // det * conj(z)
+    C ri = di * zr; ri -= dr * zi;
+    w[12 + 2 * c] = rr; w[12 + 2 * c + 1] = ri;
+  }
+}
+template <typename S, int MU, int DIR, int R, int NL>
+__device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, HopRegs<S, R, NL>& d) {
   typedef typename PT<S>::V V;
-  typedef LinkChunks<MU, S> LC;
+  typedef LinkChunks<MU, S, NL> LC;
   const int Vh = a.g.Vh;
   const int nb = neighbour_cb<MU, DIR>(a.g, s);
 #pragma unroll
@@ -158,7 +178,7 @@ __device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, in
     if (R > 1 && rhs0 + r >= a.nrhs) break;
     const V* p = reinterpret_cast<const V*>(static_cast<const char*>(a.in[1 - parity].data) + a.rs_in * (rhs0 + r));
 #pragma unroll
-    for (int c = 0; c < HopRegs<S, R>::NPSI; c++) d.psi[r][c] = ldg_pinned(p + size_t(c) * Vh + nb);
+    for (int c = 0; c < HopRegs<S, R, NL>::NPSI; c++) d.psi[r][c] = ldg_pinned(p + size_t(c) * Vh + nb);
     d.scale[r] = 1.f;
     if (PT<S>::ID == 2) d.scale[r] = ldg_pinned(reinterpret_cast<const float*>(reinterpret_cast<const char*>(a.in[1 - parity].scale) + a.rs_in * (rhs0 + r)) + nb);
   }
@@ -168,59 +188,62 @@ __device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, in
 #pragma unroll
   for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * Vh + wi);
 }
-template <typename S, int MU, int DIR, bool G5IN, int R>
-__device__ __forceinline__ void hop_use(const HopRegs<S, R>& d, typename PT<S>::C (*acc)[24]) {
+template <typename S, int MU, int DIR, bool G5IN, int R, int NL>
+__device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<S>::C (*acc)[24]) {
   typedef typename PT<S>::C C;
-  typedef LinkChunks<MU, S> LC;
+  typedef LinkChunks<MU, S, NL> LC;
   constexpr int RPC = PT<S>::RPC;
-  C wv[HopRegs<S, R>::NWC * RPC];
+  C wv[HopRegs<S, R, NL>::NWC * RPC];
 #pragma unroll
   for (int c = 0; c < LC::N; c++) unpack_vec(d.w[c], wv + c * RPC);
+  C w18[18];
+  if (NL == 14) reconstruct_row2(wv + LC::OFF, w18);
+  const C* wl = NL == 14 ? w18 : wv + LC::OFF;
 #pragma unroll
   for (int r = 0; r < R; r++) {
     C psi[24], h[12], t[12];
 #pragma unroll
-    for (int c = 0; c < HopRegs<S, R>::NPSI; c++) unpack_vec(d.psi[r][c], psi + c * RPC);
+    for (int c = 0; c < HopRegs<S, R, NL>::NPSI; c++) unpack_vec(d.psi[r][c], psi + c * RPC);
     if (G5IN) {
 #pragma unroll
       for (int i = 12; i < 24; i++) psi[i] = -psi[i];
     }
     project<MU, DIR>(psi, h);
-    link_mul<(DIR < 0)>(wv + LC::OFF, h, t);
+    link_mul<(DIR < 0)>(wl, h, t);
     reconstruct<MU, DIR, PT<S>::ID == 2>(t, acc[r], (C)d.scale[r]);
   }
 }
 // all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one
-template <typename S, bool G5IN, int R, int PIPE>
+template <typename S, bool G5IN, int R, int PIPE, int NL>
 __device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, typename PT<S>::C (*acc)[24]) {
   if (PIPE == 2) {
-    HopRegs<S, R> d0, d1;
-    hop_issue<S, 0, +1, R>(a, s, cb, parity, rhs0, d0);
-    hop_issue<S, 0, -1, R>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 0, +1, G5IN, R>(d0, acc);
-    hop_issue<S, 1, +1, R>(a, s, cb, parity, rhs0, d0);
-    hop_use<S, 0, -1, G5IN, R>(d1, acc);
-    hop_issue<S, 1, -1, R>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 1, +1, G5IN, R>(d0, acc);
-    hop_issue<S, 2, +1, R>(a, s, cb, parity, rhs0, d0);
-    hop_use<S, 1, -1, G5IN, R>(d1, acc);
-    hop_issue<S, 2, -1, R>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 2, +1, G5IN, R>(d0, acc);
-    hop_issue<S, 3, +1, R>(a, s, cb, parity, rhs0, d0);
-    hop_use<S, 2, -1, G5IN, R>(d1, acc);
-    hop_issue<S, 3, -1, R>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 3, +1, G5IN, R>(d0, acc);
-    hop_use<S, 3, -1, G5IN, R>(d1, acc);
+    HopRegs<S, R, NL> d0, d1;
+    hop_issue<S, 0, +1, R, NL>(a, s, cb, parity, rhs0, d0);
+    hop_issue<S, 0, -1, R, NL>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 0, +1, G5IN, R, NL>(d0, acc);
+    hop_issue<S, 1, +1, R, NL>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 0, -1, G5IN, R, NL>(d1, acc);
+    hop_issue<S, 1, -1, R, NL>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 1, +1, G5IN, R, NL>(d0, acc);
+    hop_issue<S, 2, +1, R, NL>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 1, -1, G5IN, R, NL>(d1, acc);
+    hop_issue<S, 2, -1, R, NL>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 2, +1, G5IN, R, NL>(d0, acc);
+    hop_issue<S, 3, +1, R, NL>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 2, -1, G5IN, R, NL>(d1, acc);
+    hop_issue<S, 3, -1, R, NL>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 3, +1, G5IN, R, NL>(d0, acc);
+    hop_use<S, 3, -1, G5IN, R, NL>(d1, acc);
   } else {
-    HopRegs<S, R> d;
-    hop_issue<S, 0, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 0, +1, G5IN, R>(d, acc);
-    hop_issue<S, 0, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 0, -1, G5IN, R>(d, acc);
-    hop_issue<S, 1, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 1, +1, G5IN, R>(d, acc);
-    hop_issue<S, 1, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 1, -1, G5IN, R>(d, acc);
-    hop_issue<S, 2, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 2, +1, G5IN, R>(d, acc);
-    hop_issue<S, 2, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 2, -1, G5IN, R>(d, acc);
-    hop_issue<S, 3, +1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 3, +1, G5IN, R>(d, acc);
-    hop_issue<S, 3, -1, R>(a, s, cb, parity, rhs0, d); hop_use<S, 3, -1, G5IN, R>(d, acc);
+    HopRegs<S, R, NL> d;
+    hop_issue<S, 0, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 0, +1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 0, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 0, -1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 1, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 1, +1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 1, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 1, -1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 2, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 2, +1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 2, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 2, -1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 3, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 3, +1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 3, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 3, -1, G5IN, R, NL>(d, acc);
   }
 }
 
@@ -237,7 +260,7 @@ template <typename S, int R, bool FULL> struct KernelShape {
   static constexpr int MINB = sizeof(S) == 8 ? 1 : (R == 1 ? (FULL ? 2 : 4) : (R == 2 ? (FULL ? 1 : 3) : (FULL ? 1 : 2)));
   static constexpr int PIPE = (R == 1) ? 2 : 1;
 };
-template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R>
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
 __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<S, R, FULL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
   typedef typename PT<S>::C C;
   const int Vh = a.g.Vh;
@@ -257,7 +280,7 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
 #pragma unroll
       for (int i = 0; i < 24; i++) acc[r][i] = 0;
     const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
-    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL>::PIPE>(a, s, cb, parity, rhs0, acc);
+    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL>::PIPE, NL>(a, s, cb, parity, rhs0, acc);
 #pragma unroll
     for (int r = 0; r < R; r++)
 #pragma unroll
@@ -312,15 +335,15 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
   }
 }
 
-template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R>
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
 void launch_r(qxd_ctx* c, DslashArgs& a) {
   a.ngroups = (a.nrhs + R - 1) / R;
   dim3 gr(unsigned((c->g.Vh + 127) / 128) * unsigned(a.ngroups));
-  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R><<<gr, KernelShape<S, R, FULL>::THREADS, 0, c->stream>>>(a);
+  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL><<<gr, KernelShape<S, R, FULL>::THREADS, 0, c->stream>>>(a);
 }
 // right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 3)
 // MULTI: instantiate the R = 2, 3 kernels for this mode (only the modes the batched solver and bench use)
-template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, bool MULTI>
+template <typename S, int NL, int PHI, int POST, bool NEG, int FLAGS, bool FULL, bool MULTI>
 int launch_one(qxd_ctx* c, DslashArgs& a) {
   int R = 1;
   if (a.nrhs > 1) {
@@ -328,8 +351,8 @@ int launch_one(qxd_ctx* c, DslashArgs& a) {
     if (R > a.nrhs) R = a.nrhs;
   }
   if (MULTI && sizeof(S) < 8) {   // fp64: the accumulators of two spinors do not fit the register file
-    if (R == 2) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 2 : 1>(c, a); return QXD_OK; }
-    if (R >= 3) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 3 : 1>(c, a); return QXD_OK; }
+    if (R == 2) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 2 : 1, NL>(c, a); return QXD_OK; }
+    if (R >= 3) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 3 : 1, NL>(c, a); return QXD_OK; }
   }
   // one launch per right-hand side
   const int n = a.nrhs;
@@ -340,34 +363,34 @@ int launch_one(qxd_ctx* c, DslashArgs& a) {
     a.in[0] = rhs_view(in0, a.rs_in, r); a.in[1] = rhs_view(in1, a.rs_in, r); a.phi = rhs_view(phi, a.rs_phi, r);
     a.out[0] = rhs_view(out0, a.rs_out, r); a.out[1] = rhs_view(out1, a.rs_out, r);
     a.R.result = res ? res + size_t(r) * a.R.rstride : nullptr;
-    launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1>(c, a);
+    launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1, NL>(c, a);
     if (r + 1 < n) c->launches++;
   }
   return QXD_OK;
 }
 
-template <typename S>
+template <typename S, int NL>
 int dispatch(qxd_ctx* c, const DslashCall& d, DslashArgs& a) {
   const int f = d.flags;
   switch (d.mode) {
     case DS_DW_FULL:
       if (f != 0) break;
-      return launch_one<S, 2, 0, false, 0, true, true>(c, a);
+      return launch_one<S, NL, 2, 0, false, 0, true, true>(c, a);
     case DS_HOP_AINV:
-      if (f == 0) { return launch_one<S, 0, 1, false, 0, false, true>(c, a); }
-      if (f == DSF_G5IN) { return launch_one<S, 0, 1, false, DSF_G5IN, false, true>(c, a); }
+      if (f == 0) { return launch_one<S, NL, 0, 1, false, 0, false, true>(c, a); }
+      if (f == DSF_G5IN) { return launch_one<S, NL, 0, 1, false, DSF_G5IN, false, true>(c, a); }
       break;
     case DS_A_XMHOP:
-      if (f == 0) { return launch_one<S, 2, 0, true, 0, false, true>(c, a); }
-      if (f == DSF_NORM) { return launch_one<S, 2, 0, true, DSF_NORM, false, true>(c, a); }
-      if (f == DSF_G5HOP) { return launch_one<S, 2, 0, true, DSF_G5HOP, false, true>(c, a); }
-      if (f == (DSF_G5HOP | DSF_NORM)) { return launch_one<S, 2, 0, true, DSF_G5HOP | DSF_NORM, false, true>(c, a); }
+      if (f == 0) { return launch_one<S, NL, 2, 0, true, 0, false, true>(c, a); }
+      if (f == DSF_NORM) { return launch_one<S, NL, 2, 0, true, DSF_NORM, false, true>(c, a); }
+      if (f == DSF_G5HOP) { return launch_one<S, NL, 2, 0, true, DSF_G5HOP, false, true>(c, a); }
+      if (f == (DSF_G5HOP | DSF_NORM)) { return launch_one<S, NL, 2, 0, true, DSF_G5HOP | DSF_NORM, false, true>(c, a); }
       break;
     case DS_X_MHOP:
-      if (f == 0) { return launch_one<S, 1, 0, true, 0, false, false>(c, a); }
+      if (f == 0) { return launch_one<S, NL, 1, 0, true, 0, false, false>(c, a); }
       break;
     case DS_AINV_X_MHOP:
-      if (f == 0) { return launch_one<S, 1, 1, true, 0, false, false>(c, a); }
+      if (f == 0) { return launch_one<S, NL, 1, 1, true, 0, false, false>(c, a); }
       break;
     default: break;
   }

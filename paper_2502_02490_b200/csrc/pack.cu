@@ -36,7 +36,9 @@ __global__ void __launch_bounds__(128) gauge_pack_k(Geom g, const double* __rest
 
 // ---- hopping links W_mu(x) = e^{i q A_mu(x)} U_mu(x), fermion time-boundary sign folded
 // into W_0 at x0 = T-1 (reading R9; the clover term is built from Ug and is unaffected).
-template <typename S>
+// NL = 14: rows 0 and 1 of W and det W = e^{3 i q A} det U (-1 at the antiperiodic time boundary); the dslash rebuilds
+// row 2 = det W * conj(row0 x row1).  det U is computed (not assumed 1), so U(3) input links are represented exactly.
+template <typename S, int NL>
 __global__ void __launch_bounds__(128) hoplinks_k(Geom g, double q, int use_a, const void* Ug0, const void* Ug1, const void* Ag0,
                                                   const void* Ag1, void* W0, void* W1) {
   typedef typename PT<S>::C C;
@@ -48,20 +50,39 @@ __global__ void __launch_bounds__(128) hoplinks_k(Geom g, double q, int use_a, c
   double u[72], a[4];
   load_reals<double, 0, 72>(parity ? Ug1 : Ug0, g.Vh, cb, u);
   load_reals<double, 0, 4>(parity ? Ag1 : Ag0, g.Vh, cb, a);
-  C w[72];
+  C w[4 * NL];
 #pragma unroll
   for (int mu = 0; mu < 4; mu++) {
     double c = 1.0, s = 0.0;
     if (use_a) sincos(q * a[mu], &s, &c);
     if (mu == 0 && g.antiper && x[0] == g.X[0] - 1) { c = -c; s = -s; }
+    const double* m = u + 18 * mu;
 #pragma unroll
-    for (int k = 0; k < 9; k++) {
-      double re = u[18 * mu + 2 * k], im = u[18 * mu + 2 * k + 1];
-      w[18 * mu + 2 * k] = (C)(c * re - s * im);
-      w[18 * mu + 2 * k + 1] = (C)(c * im + s * re);
+    for (int k = 0; k < NL / 2 && k < 9; k++) {
+      double re = m[2 * k], im = m[2 * k + 1];
+      if (NL == 18 || k < 6) {
+        w[NL * mu + 2 * k] = (C)(c * re - s * im);
+        w[NL * mu + 2 * k + 1] = (C)(c * im + s * re);
+      }
+    }
+    if (NL == 14) {
+      // det U = sum_c row2[c] * (row0 x row1)[c]
+      double dr = 0.0, di = 0.0;
+#pragma unroll
+      for (int cc = 0; cc < 3; cc++) {
+        const int a0 = (cc + 1) % 3, b0 = (cc + 2) % 3;
+        double zr = m[2 * a0] * m[6 + 2 * b0] - m[2 * a0 + 1] * m[6 + 2 * b0 + 1] - m[2 * b0] * m[6 + 2 * a0] + m[2 * b0 + 1] * m[6 + 2 * a0 + 1];
+        double zi = m[2 * a0] * m[6 + 2 * b0 + 1] + m[2 * a0 + 1] * m[6 + 2 * b0] - m[2 * b0] * m[6 + 2 * a0 + 1] - m[2 * b0 + 1] * m[6 + 2 * a0];
+        dr += m[12 + 2 * cc] * zr - m[12 + 2 * cc + 1] * zi;
+        di += m[12 + 2 * cc] * zi + m[12 + 2 * cc + 1] * zr;
+      }
+      // (c + i s)^3 det U
+      const double c3 = c * (c * c - 3.0 * s * s), s3 = s * (3.0 * c * c - s * s);
+      w[NL * mu + 12] = (C)(c3 * dr - s3 * di);
+      w[NL * mu + 13] = (C)(c3 * di + s3 * dr);
     }
   }
-  store_record<S, 72>(parity ? W1 : W0, g.Vh, cb, w);
+  store_record<S, 4 * NL>(parity ? W1 : W0, g.Vh, cb, w);
 }
 
 // ---- spinors: natural AoS fp64 <-> packed SoA in precision S
@@ -149,9 +170,10 @@ int launch_gauge_pack(qxd_ctx* c, const double* U, const double* A) {
 int launch_hoplinks(qxd_ctx* c, int prec) {
   dim3 gr = grid_for(c->g.Vh, 2);
   int ua = c->have_qed ? 1 : 0;
-  if (prec == 0) hoplinks_k<double><<<gr, 128, 0, c->stream>>>(c->g, c->q, ua, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1], c->W[0][0], c->W[0][1]);
-  else if (prec == 1) hoplinks_k<float><<<gr, 128, 0, c->stream>>>(c->g, c->q, ua, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1], c->W[1][0], c->W[1][1]);
-  else hoplinks_k<__half><<<gr, 128, 0, c->stream>>>(c->g, c->q, ua, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1], c->W[2][0], c->W[2][1]);
+#define QXD_HOPLINKS(S, NL) hoplinks_k<S, NL><<<gr, 128, 0, c->stream>>>(c->g, c->q, ua, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1], c->W[prec][0], c->W[prec][1])
+  if (c->link_reals == 14) { if (prec == 0) QXD_HOPLINKS(double, 14); else if (prec == 1) QXD_HOPLINKS(float, 14); else QXD_HOPLINKS(__half, 14); }
+  else { if (prec == 0) QXD_HOPLINKS(double, 18); else if (prec == 1) QXD_HOPLINKS(float, 18); else QXD_HOPLINKS(__half, 18); }
+#undef QXD_HOPLINKS
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

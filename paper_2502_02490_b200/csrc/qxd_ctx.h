@@ -37,6 +37,7 @@ struct qxd_ctx {
   char* ws = nullptr;
   size_t ws_bytes = 0, ws_used = 0;
   int prec_mask = 0, nrhs = 1;
+  int link_reals = 18;                           // stored reals per hopping link: 18, or 14 = rows 0,1 + det (qxd_set_gauge_reconstruct)
   int rhs_per_thread = 0;                        // multi-RHS dslash: right-hand sides per thread (0 = default)
   // state
   bool have_gauge = false, have_qed = false, have_quark = false, have_clover = false;
@@ -44,7 +45,7 @@ struct qxd_ctx {
   // fields (device, carved from the workspace); [parity]
   void* Ug[2] = {nullptr, nullptr};              // fp64 SU(3) links, record of 72 reals (4 links x 18)
   void* Ag[2] = {nullptr, nullptr};              // fp64 U(1) field, record of 4 reals
-  void* W[qxd::NPREC][2] = {};                   // hopping links e^{iqA} U (time-BC sign folded in), 72 reals
+  void* W[qxd::NPREC][2] = {};                   // hopping links e^{iqA} U (time-BC sign folded in), 4 x link_reals (buffer: 72 reals)
   void* M[qxd::NPREC][2] = {};                   // clover blocks, 72 reals (PAPER.md:117 order)
   void* Mi[qxd::NPREC][2] = {};                  // inverse blocks
   // scratch spinors

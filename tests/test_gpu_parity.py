@@ -101,6 +101,43 @@ def test_apply_Dw(case, prec):
 
 
 @pytest.mark.parametrize("prec", [F64, F32, F16])
+def test_apply_Dw_and_Dhat_reconstruct12(case, prec):
+    """Rows a2/a4/a5 with the 14-real link format (rows 0, 1 + det W: 12-real reconstruct, U(1) phase and the
+    antiperiodic sign carried by det W); switching the format rewrites the links and must not change any result."""
+    B = case.B
+    psi = synth.gaussian_spinor(case.dims_ext, 3)
+    pe = synth.gaussian_spinor(case.dims_ext, 6).reshape(-1, 4, 3)[: case.V // 2]
+    exp = case.ref.apply_Dw(psi)
+    case.gpu.set_gauge_reconstruct(B.QXD_RECON_12)
+    try:
+        got = to_np(case.gpu.apply_Dw(psi, prec)).reshape(exp.shape)
+        assert relerr(got, exp) < TOL[prec]
+        for dagger in (False, True):
+            e2 = case.ref.apply_Dhat(pe, dagger=dagger)
+            g2 = to_np(case.gpu.apply_Dhat_eo(pe, prec, dagger=dagger)).reshape(e2.shape)
+            assert relerr(g2, e2) < 2 * TOL[prec]
+    finally:
+        case.gpu.set_gauge_reconstruct(B.QXD_RECON_NONE)
+    got = to_np(case.gpu.apply_Dw(psi, prec)).reshape(exp.shape)
+    assert relerr(got, exp) < TOL[prec]
+
+
+def test_reconstruct12_solve_and_bad_value(case):
+    B = case.B
+    eta = synth.gaussian_spinor(case.dims_ext, 4)
+    case.gpu.set_gauge_reconstruct(B.QXD_RECON_12)
+    try:
+        psi, info = case.gpu.solve(eta, 1e-10, algo=B.QXD_CGNE, sloppy=F32)
+        assert info["status"] == 0
+        res = relerr(case.ref.apply_Dw(to_np(psi).reshape(eta.shape)), eta)
+        assert res <= 1.05e-10
+        with pytest.raises(B.QxdError):
+            case.gpu.set_gauge_reconstruct(8)
+    finally:
+        case.gpu.set_gauge_reconstruct(B.QXD_RECON_NONE)
+
+
+@pytest.mark.parametrize("prec", [F64, F32, F16])
 @pytest.mark.parametrize("dagger", [False, True])
 def test_apply_Dhat(case, prec, dagger):
     """Row a5: both fused passes of the even-odd operator and its adjoint."""
