@@ -50,8 +50,9 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def dw_bytes_per_site(prec):
-    b = REALS_DW * PREC_BYTES[prec]
+def dw_bytes_per_site(prec, link_reals=18):
+    """Algorithmic bytes of one D_w site: psi 24 + 4 links x link_reals (18, or 14 = 12-real reconstruct + det) + clover 72 + out 24."""
+    b = (REALS_DW - 72 + 4 * link_reals) * PREC_BYTES[prec]
     if prec == 2:
         b += 8                          # fp32 block-float scale, read with psi and written with out
     return b
@@ -174,6 +175,7 @@ def run_reference(args, cfg):
 def run_cuda(args, cfg):
     import numpy as np
     import torch
+    import synth as synth_mod
     from paper_2502_02490_b200 import binding as B
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -203,7 +205,7 @@ def run_cuda(args, cfg):
     t_setup = time.perf_counter()
     U, A, eta = make_fields(cfg, rank)
     precs = (B.QXD_F64, B.QXD_F32, B.QXD_F16)
-    g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, device=f"cuda:{local}")
+    g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=max(1, args.nrhs), device=f"cuda:{local}")
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
     def timed(fn, n):
@@ -261,30 +263,55 @@ def run_cuda(args, cfg):
     per_gpu_gbs = value / world
 
     # ---- sweep: D_w and D-hat in the three storage precisions, BLAS streams (rank-local numbers) ----------
+    # link formats: 18 stored reals (full) and 14 (12-real reconstruct + det W, qxd_set_gauge_reconstruct)
     sweep = {}
     nrep = max(10, min(args.steps, 50))
-    for p in (() if args.no_sweep else precs):
-        a, b = packed[p]
-        for _ in range(3):
-            g.apply_Dw_packed(a, b, p)
-        ms = timed(lambda: g.apply_Dw_packed(a, b, p), nrep)
-        hb = g.packed_spinor_bytes(p, half_only=True)
-        for _ in range(3):
-            g.apply_Dhat_packed(a[:hb], b[:hb], p)
-        ms_hat = timed(lambda: g.apply_Dhat_packed(a[:hb], b[:hb], p), nrep)
-        ms_axpy = timed(lambda: g.blas_axpy(1e-3, a[:hb], b[:hb], p), nrep)
-        bytes_dw = dw_bytes_per_site(p) * V
-        bytes_hat = REALS_DHAT * PREC_BYTES[p] * V + (16 * V // 2 if p == 2 else 0)
-        sweep[PREC_NAME[p]] = {
-            "Dw_ms": ms, "Dw_GBps": bytes_dw / ms / 1e6, "Dw_Gflops": FLOP_PER_SITE * V / ms / 1e6, "Dw_frac_of_peak": bytes_dw / ms / 1e6 / peak,
-            "Dhat_ms": ms_hat, "Dhat_GBps": bytes_hat / ms_hat / 1e6, "Dhat_Gflops": FLOP_PER_SITE * V / ms_hat / 1e6,
-            "axpy_GBps": 3 * 24 * PREC_BYTES[p] * (V // 2) / ms_axpy / 1e6,
-        }
+    for nl, tag in ((18, ""), (14, "_recon12")):
+        if args.no_sweep:
+            break
+        g.set_gauge_reconstruct(B.QXD_RECON_12 if nl == 14 else B.QXD_RECON_NONE)
+        for p in precs:
+            a, b = packed[p]
+            for _ in range(3):
+                g.apply_Dw_packed(a, b, p)
+            ms = timed(lambda: g.apply_Dw_packed(a, b, p), nrep)
+            hb = g.packed_spinor_bytes(p, half_only=True)
+            for _ in range(3):
+                g.apply_Dhat_packed(a[:hb], b[:hb], p)
+            ms_hat = timed(lambda: g.apply_Dhat_packed(a[:hb], b[:hb], p), nrep)
+            bytes_dw = dw_bytes_per_site(p, nl) * V
+            # D-hat, both passes, per full-lattice site: 276 reals with 18-real links, 8 x (18 - nl) fewer per even site
+            bytes_hat = (REALS_DHAT - 4 * (18 - nl)) * PREC_BYTES[p] * V + (16 * V // 2 if p == 2 else 0)
+            e = {"link_reals": nl, "Dw_ms": ms, "Dw_GBps": bytes_dw / ms / 1e6, "Dw_Gflops": FLOP_PER_SITE * V / ms / 1e6,
+                 "Dw_frac_of_peak": bytes_dw / ms / 1e6 / peak, "Dhat_ms": ms_hat, "Dhat_GBps": bytes_hat / ms_hat / 1e6,
+                 "Dhat_Gflops": FLOP_PER_SITE * V / ms_hat / 1e6}
+            if nl == 18:
+                ms_axpy = timed(lambda: g.blas_axpy(1e-3, a[:hb], b[:hb], p), nrep)
+                e["axpy_GBps"] = 3 * 24 * PREC_BYTES[p] * (V // 2) / ms_axpy / 1e6
+            sweep[PREC_NAME[p] + tag] = e
+    g.set_gauge_reconstruct(B.QXD_RECON_NONE)
     clocks = sampler.stop()
+
+    # ---- multi-RHS D_w (row a10): links and clover blocks read once for a batch of right-hand sides --------
+    multi = {}
+    if args.nrhs > 1 and not args.no_sweep:
+        n = args.nrhs
+        for p in (B.QXD_F32, B.QXD_F16):
+            nb = g.packed_spinor_bytes(p)
+            pin = packed[p][0].repeat(n)
+            pout = torch.empty_like(pin)
+            for _ in range(2):
+                g.apply_Dw_multi_packed(pin, pout, p, n)
+            ms = timed(lambda: g.apply_Dw_multi_packed(pin, pout, p, n), max(3, nrep // 5))
+            reals = 48 + 144.0 / n
+            multi[PREC_NAME[p]] = {"nrhs": n, "ms_per_rhs": ms / n, "GBps": reals * PREC_BYTES[p] * V * n / ms / 1e6,
+                                   "Gflops": FLOP_PER_SITE * V * n / ms / 1e6, "speedup_vs_single": sweep[PREC_NAME[p]]["Dw_ms"] * n / ms}
+            del pin, pout
 
     # ---- solves (rows a7, a8): fp64/fp16 and fp64/fp32 mixed CGNE, BiCGstab ------------------------------
     solves = {}
     if not args.no_solve:
+        g.set_gauge_reconstruct(B.QXD_RECON_12)   # the solves run on the 14-real link format (less traffic per D-hat)
         psi_d = torch.empty_like(eta_d)
         for name, algo, sl in (("cgne_fp64_fp16", B.QXD_CGNE, B.QXD_F16), ("cgne_fp64_fp32", B.QXD_CGNE, B.QXD_F32),
                                ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32)):
@@ -292,7 +319,20 @@ def run_cuda(args, cfg):
             _, info = g.solve(eta_d, cfg["tol"], algo=algo, sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psi_d)
             info["launches"] = g.launch_count() - l0
             info["tol"] = cfg["tol"]
+            info["links"] = "recon12"
             solves[name] = info
+        if args.nrhs > 1:
+            etas = torch.stack([eta_d] + [torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + k)).to(dev) for k in range(1, args.nrhs)])
+            l0 = g.launch_count()
+            t0 = time.perf_counter()
+            _, infos = g.solve_multi(etas, cfg["tol"], sloppy=B.QXD_F32, delta=0.1, maxiter=args.maxiter)
+            torch.cuda.synchronize(dev)
+            solves[f"cgne_multi{args.nrhs}_fp64_fp32"] = {
+                "status": max(abs(i["status"]) for i in infos), "iters_max": max(i["iters"] for i in infos),
+                "true_res_max": max(i["true_res"] for i in infos), "seconds": time.perf_counter() - t0,
+                "seconds_per_rhs": (time.perf_counter() - t0) / args.nrhs, "launches": g.launch_count() - l0, "tol": cfg["tol"], "links": "recon12"}
+            del etas
+        g.set_gauge_reconstruct(B.QXD_RECON_NONE)
 
     # ---- end to end through the host-pointer C-ABI call (H2D + pack + apply + unpack + D2H every step) ------
     eh = torch.from_numpy(eta).pin_memory()
@@ -332,6 +372,7 @@ def run_cuda(args, cfg):
             "clocks": clocks,
             "cpu_baseline": cpu_baseline,
             "sweep": sweep,
+            "multi_rhs": multi,
             "solve": solves,
             "setup_ms": setup_ms,
             "setup_s_total": setup_s,
@@ -350,6 +391,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", default="c3")
     ap.add_argument("--maxiter", type=int, default=20000)
+    ap.add_argument("--nrhs", type=int, default=12, help="right-hand sides of the multi-RHS D_w / batched solve lines (row a10; 1 = skip)")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the precision sweep (short runs under ncu)")

@@ -171,8 +171,9 @@ int qxd_spinor_unpack(qxd_ctx* ctx, int prec, const void* packed, double* nat);
 int qxd_apply_Dw_packed(qxd_ctx* ctx, int prec, const void* in, void* out);
 int qxd_apply_Dhat_packed(qxd_ctx* ctx, int prec, const void* in_e, void* out_e, int dagger);
 /* Multi-RHS D_w (row a10): in/out hold nrhs packed full-lattice spinors back to back, qxd_packed_spinor_bytes(prec,0)
- * apart.  One launch; every thread applies its site's links and clover blocks to r right-hand sides
- * (qxd_set_rhs_per_thread: 0 = library default, 1..3; fp64 always runs one right-hand side per thread). */
+ * apart.  One launch: the CTAs working on the same tile for different right-hand sides are consecutive, so the links
+ * and clover blocks of a tile come from DRAM once and from L2 afterwards; every thread applies its site's links and
+ * clover blocks to r right-hand sides (qxd_set_rhs_per_thread: 0 = library default (1), 1..3; fp64 always 1). */
 int qxd_apply_Dw_multi_packed(qxd_ctx* ctx, int prec, int nrhs, const void* in, void* out);
 int qxd_set_rhs_per_thread(qxd_ctx* ctx, int r);
 

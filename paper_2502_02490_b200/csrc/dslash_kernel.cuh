@@ -270,10 +270,13 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
   typedef typename PT<S>::C C;
   const int Vh = a.g.Vh;
   constexpr bool SPLIT = KernelShape<S, R, FULL>::SPLIT;
-  const int tile = R > 1 ? blockIdx.x / a.ngroups : SPLIT ? (blockIdx.x >> 1) : blockIdx.x;
-  const int rhs0 = R > 1 ? (blockIdx.x - tile * a.ngroups) * R : 0;
+  // block index -> (tile, parity, group of R right-hand sides), groups fastest: the CTAs that need the links and clover
+  // blocks of a tile run at the same time, so a batch reads them from DRAM once and from L2 afterwards
+  const int bt = blockIdx.x / a.ngroups;
+  const int rhs0 = (blockIdx.x - bt * a.ngroups) * R;
+  const int tile = SPLIT ? (bt >> 1) : bt;
   const int cb = tile * 128 + (threadIdx.x & 127);
-  const int parity = FULL ? (SPLIT ? (blockIdx.x & 1) : (threadIdx.x >> 7)) : a.parity_out;
+  const int parity = FULL ? (SPLIT ? (bt & 1) : (threadIdx.x >> 7)) : a.parity_out;
   double nrm[R];
 #pragma unroll
   for (int r = 0; r < R; r++) nrm[r] = 0.0;
@@ -331,7 +334,7 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
     }
   }
   if (FLAGS & DSF_NORM) {
-    const int ntiles = R > 1 ? gridDim.x / a.ngroups : gridDim.x;
+    const int ntiles = gridDim.x / a.ngroups;
 #pragma unroll
     for (int r = 0; r < R; r++) {
       if (R > 1 && rhs0 + r >= a.nrhs) break;   // uniform over the CTA
@@ -347,31 +350,22 @@ void launch_r(qxd_ctx* c, DslashArgs& a) {
   dim3 gr(unsigned((c->g.Vh + 127) / 128) * unsigned(a.ngroups) * (KernelShape<S, R, FULL>::SPLIT ? 2u : 1u));
   dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL><<<gr, KernelShape<S, R, FULL>::THREADS, 0, c->stream>>>(a);
 }
-// right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 3)
+// right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 1:
+// measured at c3 with 12 right-hand sides, fp32: 0.43 ms per right-hand side against 0.59 (R = 2) and 0.50 (R = 3))
 // MULTI: instantiate the R = 2, 3 kernels for this mode (only the modes the batched solver and bench use)
 template <typename S, int NL, int PHI, int POST, bool NEG, int FLAGS, bool FULL, bool MULTI>
 int launch_one(qxd_ctx* c, DslashArgs& a) {
   int R = 1;
   if (a.nrhs > 1) {
-    R = c->rhs_per_thread > 0 ? c->rhs_per_thread : 3;
+    R = c->rhs_per_thread > 0 ? c->rhs_per_thread : 1;
     if (R > a.nrhs) R = a.nrhs;
   }
   if (MULTI && sizeof(S) < 8) {   // fp64: the accumulators of two spinors do not fit the register file
     if (R == 2) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 2 : 1, NL>(c, a); return QXD_OK; }
     if (R >= 3) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 3 : 1, NL>(c, a); return QXD_OK; }
   }
-  // one launch per right-hand side
-  const int n = a.nrhs;
-  const SpinorPtr in0 = a.in[0], in1 = a.in[1], phi = a.phi, out0 = a.out[0], out1 = a.out[1];
-  double* res = a.R.result;
-  for (int r = 0; r < n; r++) {
-    a.nrhs = 1;
-    a.in[0] = rhs_view(in0, a.rs_in, r); a.in[1] = rhs_view(in1, a.rs_in, r); a.phi = rhs_view(phi, a.rs_phi, r);
-    a.out[0] = rhs_view(out0, a.rs_out, r); a.out[1] = rhs_view(out1, a.rs_out, r);
-    a.R.result = res ? res + size_t(r) * a.R.rstride : nullptr;
-    launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1, NL>(c, a);
-    if (r + 1 < n) c->launches++;
-  }
+  // one right-hand side per thread, the right-hand sides of a tile in consecutive CTAs
+  launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1, NL>(c, a);
   return QXD_OK;
 }
 
