@@ -112,7 +112,8 @@ def make_fields(cfg, rank):
     import synth
     U = synth.su3_links(cfg["dims"], cfg["eps"], 1)
     A = synth.u1_field(cfg["dims"], 0.3, 2) if cfg["qed"] else None
-    eta = synth.gaussian_spinor(cfg["dims_ext"], 3 + rank)   # each rank: its own right-hand side
+    from paper_2502_02490_b200 import sharding
+    eta = synth.gaussian_spinor(cfg["dims_ext"], sharding.rhs_seed(rank))   # each rank: its own right-hand side (global index = rank)
     return U, A, eta
 
 
@@ -195,12 +196,10 @@ def run_cuda(args, cfg):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    from paper_2502_02490_b200 import sharding
+
     def max_over_ranks(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return sharding.max_over_ranks(x, dist, dev)
 
     t_setup = time.perf_counter()
     U, A, eta = make_fields(cfg, rank)

@@ -263,7 +263,7 @@ template <typename S, int R, bool FULL> struct KernelShape {
   static constexpr int THREADS = (FULL && !SPLIT) ? 256 : 128;
   // CTAs per SM the register budget is sized for
   static constexpr int MINB = SPLIT ? (sizeof(S) == 8 ? 2 : 4) : sizeof(S) == 8 ? 1 : (R == 1 ? (FULL ? 2 : 4) : (R == 2 ? (FULL ? 1 : 3) : (FULL ? 1 : 2)));
-  static constexpr int PIPE = (R == 1) ? 2 : 1;
+  static constexpr int PIPE = (R == 1) ? 2 : 1;   // hops in flight per thread
 };
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
 __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<S, R, FULL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
