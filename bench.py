@@ -37,8 +37,8 @@ PREC_NAME = {0: "fp64", 1: "fp32", 2: "fp16"}
 PREC_BYTES = {0: 8, 1: 4, 2: 2}
 FALLBACK_HBM_GBS = 6650.0               # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fp32 D_w kernel at c3, from the committed
-# `ncu --set full` capture (profiles/r1_dslash_fp32_c3.md); None until a capture exists.
-NCU_TRAFFIC_BYTES_FP32_C3 = 3662338024   # 3.257889 GB read + 0.404449 GB write (profiles/r1_dslash_fp32_c3.md)
+# `ncu --set full` capture (profiles/r1b_dslash_fp32_c3.md).
+NCU_TRAFFIC_BYTES_FP32_C3 = 3737077912   # 3.267887 GB read + 0.469191 GB write (profiles/r1b_dslash_fp32_c3.md)
 
 
 def measured_peak():
