@@ -177,6 +177,26 @@ int qxd_apply_Dhat_packed(qxd_ctx* ctx, int prec, const void* in_e, void* out_e,
 int qxd_apply_Dw_multi_packed(qxd_ctx* ctx, int prec, int nrhs, const void* in, void* out);
 int qxd_set_rhs_per_thread(qxd_ctx* ctx, int r);
 
+/* ---- openQxD field orders (§2, §4.1) ---------------------------------
+ * The paper's host code keeps its fields in its own order; these calls convert between that order and the natural
+ * order of this header, so that its arrays can be passed as they are (the load()/save() pair of PAPER.md:107).
+ *   site index  xhat = floor((V_B Lambda(n,N_B) + Lambda(b,B)) / 2) + P(x) V/2     (Eq. (2); R14)
+ *               for cache blocks of extent block[mu], even points first, on the EXTENDED
+ *               lattice; computed on the fly, no ipt[] table.  block[mu] must divide the extent, block[3] even.
+ *   qxd_openqxd_index    xs: DEVICE [n][4] int coordinates (t,x,y,z) -> out: DEVICE [n] long xhat.
+ *   qxd_openqxd_reorder  records of reals_per_site doubles per site (24 = spinor (x,alpha,a), PAPER.md:49,111;
+ *                        72 = clover (x,+-,i)): to_openqxd != 0: out[xhat] = in[Lambda(x)], else the
+ *                        inverse.  in, out: DEVICE [V][reals_per_site], must not alias.
+ *   qxd_openqxd_gauge    reals_per_link = 18: SU(3) links, = 1: U(1) field A.  openQxD side: DEVICE [V/2][8][reals], the 8
+ *                        links of every odd point of the extended lattice in the order +0,-0,+1,-1,+2,-2,+3,-3, entry +mu =
+ *                        U_mu(x), entry -mu = U_mu(x-mu) (R20).  Natural side: DEVICE
+ *                        [V_phys][4][reals] as qxd_gauge_load takes it.  to_openqxd != 0 builds the mirror half
+ *                        (conjugate links, -A) and applies the shifted boundaries; the inverse reads the physical half only.
+ * All three enqueue on the bound stream and return QXD_EINVAL for a bad block, reals count or null / aliased pointers. */
+int qxd_openqxd_index(qxd_ctx* ctx, const int block[4], const int* xs, long n, long* out);
+int qxd_openqxd_reorder(qxd_ctx* ctx, const int block[4], int reals_per_site, int to_openqxd, const double* in, double* out);
+int qxd_openqxd_gauge(qxd_ctx* ctx, const int block[4], int reals_per_link, int to_openqxd, const double* in, double* out);
+
 /* ---- BLAS-1 on packed half-lattice spinors (row a6) ---------------------------------------------
  * y <- a*x + y ;  returns <x,y> = sum conj(x) y  and  |x|^2 (fp64 accumulation, HOST results). */
 int qxd_blas_axpy(qxd_ctx* ctx, int prec, double a, const void* x, void* y);

@@ -65,6 +65,9 @@ SYMBOLS = {
     "qxd_spinor_unpack": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dw_packed": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dhat_packed": (_i, [_vp, _i, _vp, _vp, _i]),
+    "qxd_openqxd_index": (_i, [_vp, C.POINTER(_i), _vp, _l, _vp]),
+    "qxd_openqxd_reorder": (_i, [_vp, C.POINTER(_i), _i, _i, _vp, _vp]),
+    "qxd_openqxd_gauge": (_i, [_vp, C.POINTER(_i), _i, _i, _vp, _vp]),
     "qxd_blas_axpy": (_i, [_vp, _i, _d, _vp, _vp]),
     "qxd_blas_cdot": (_i, [_vp, _i, _vp, _vp, _vp]),
     "qxd_blas_norm2": (_i, [_vp, _i, _vp, _vp]),
@@ -242,6 +245,36 @@ class Qxd:
         infos[0].algo, infos[0].sloppy, infos[0].delta, infos[0].maxiter = QXD_CGNE, sloppy, delta, maxiter
         rc = self._chk(self.lib.qxd_solve_multi(self.h, nrhs, _ptr(eta), _ptr(psi), float(tol), infos), allow=(QXD_ENOCONV,))
         return psi, [self._report(rc, infos[k]) for k in range(nrhs)]
+
+    # -- openQxD field orders (row f1) ---------------------------------------------------------------
+    def openqxd_index(self, xs, block):
+        torch = self.torch
+        x = self._dev(xs, torch.int32).reshape(-1, 4)
+        out = torch.empty(x.shape[0], dtype=torch.int64, device=self.device)
+        self._chk(self.lib.qxd_openqxd_index(self.h, (C.c_int * 4)(*block), _ptr(x), x.shape[0], _ptr(out)))
+        return out.cpu().numpy()
+
+    def openqxd_reorder(self, field, reals_per_site, to_openqxd, block):
+        torch = self.torch
+        f = self._dev(field, torch.float64).reshape(-1)
+        assert f.numel() == self.V * reals_per_site, (f.numel(), self.V, reals_per_site)
+        out = torch.empty_like(f)
+        self._chk(self.lib.qxd_openqxd_reorder(self.h, (C.c_int * 4)(*block), int(reals_per_site), int(bool(to_openqxd)), _ptr(f), _ptr(out)))
+        return out.reshape(self.V, reals_per_site)
+
+    def openqxd_gauge(self, field, to_openqxd, block, phase=False):
+        torch = self.torch
+        f = self._dev(field, torch.float64 if phase else torch.complex128).reshape(-1)
+        nr = 1 if phase else 18
+        vphys = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        n_in, n_out = (vphys * 4, self.V // 2 * 8) if to_openqxd else (self.V // 2 * 8, vphys * 4)
+        per = 1 if phase else 9
+        assert f.numel() == n_in * per, (f.numel(), n_in * per)
+        out = torch.empty(n_out * per, dtype=f.dtype, device=self.device)
+        self._chk(self.lib.qxd_openqxd_gauge(self.h, (C.c_int * 4)(*block), nr, int(bool(to_openqxd)), _ptr(f), _ptr(out)))
+        if to_openqxd:
+            return out.reshape((self.V // 2, 8) + (() if phase else (3, 3)))
+        return out.reshape(self.dims + (4,) + (() if phase else (3, 3)))
 
     def set_gauge_reconstruct(self, recon):
         self._chk(self.lib.qxd_set_gauge_reconstruct(self.h, int(recon)))

@@ -134,7 +134,7 @@ def test_cuda_openqxd_orders_bit_exact(dims, cstar, blk):
     assert np.array_equal(g.openqxd_gauge(ad, to_openqxd=False, block=blk, phase=True).cpu().numpy().reshape(A.shape), A)
     # bad block -> QXD_EINVAL
     with pytest.raises(B.QxdError):
-        g.openqxd_reorder(np.zeros((V, 24)), 24, to_openqxd=True, block=(3, 2, 2, 2))
+        g.openqxd_reorder(np.zeros((V, 24)), 24, to_openqxd=True, block=(5, 2, 2, 2))
     g.close()
 
 
