@@ -310,7 +310,10 @@ def run_cuda(args, cfg):
     # ---- solves (rows a7, a8): fp64/fp16 and fp64/fp32 mixed CGNE, BiCGstab ------------------------------
     solves = {}
     if not args.no_solve:
-        g.set_gauge_reconstruct(B.QXD_RECON_12)   # the solves run on the 14-real link format (less traffic per D-hat)
+        # link format per storage precision as measured best: 14 reals (12-real reconstruct) where the dslash is bandwidth
+        # bound (fp64, fp32), 18 reals in fp16 (issue bound)
+        g.set_gauge_reconstruct(B.QXD_RECON_12)
+        g.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=B.QXD_F16)
         psi_d = torch.empty_like(eta_d)
         for name, algo, sl in (("cgne_fp64_fp16", B.QXD_CGNE, B.QXD_F16), ("cgne_fp64_fp32", B.QXD_CGNE, B.QXD_F32),
                                ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32)):
@@ -318,7 +321,7 @@ def run_cuda(args, cfg):
             _, info = g.solve(eta_d, cfg["tol"], algo=algo, sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psi_d)
             info["launches"] = g.launch_count() - l0
             info["tol"] = cfg["tol"]
-            info["links"] = "recon12"
+            info["links"] = "fp64/fp32: recon12, fp16: 18 reals"
             solves[name] = info
         if args.nrhs > 1:
             etas = torch.stack([eta_d] + [torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + k)).to(dev) for k in range(1, args.nrhs)])

@@ -129,9 +129,12 @@ int qxd_clover_build(qxd_ctx* ctx, double csw, double csw_qed);
  * row 2 = det W * conj(row0 x row1), which holds for every unitary W, so the phase costs no separate multiply.  Traffic per
  * D_w site drops from 192 to 176 reals.  The input links must be unitary to the working precision (they are only used
  * through this identity); det U is computed, not assumed to be 1.  May be called at any time; if a quark is set the links
- * of every bound precision are rewritten in the new format.  Other values -> QXD_EINVAL. */
+ * of every bound precision are rewritten in the new format.  Other values -> QXD_EINVAL.  The _prec form sets the
+ * format of one storage precision only (measured on B200: the 14-real format is faster in fp64 and fp32, where the
+ * dslash is bandwidth bound, and slower in fp16, where it is bound by instruction issue). */
 enum { QXD_RECON_NONE = 18, QXD_RECON_12 = 12 };
 int qxd_set_gauge_reconstruct(qxd_ctx* ctx, int recon);
+int qxd_set_gauge_reconstruct_prec(qxd_ctx* ctx, int prec, int recon);
 /* Copy the fp64 clover field (inverse != 0: the block inverses) to natural order, out: DEVICE
  * [V][2][36] doubles, packing of PAPER.md:117. */
 int qxd_clover_export(qxd_ctx* ctx, double* out, int inverse);

@@ -51,6 +51,7 @@ SYMBOLS = {
     "qxd_set_quark": (_i, [_vp, _d, _d]),
     "qxd_clover_build": (_i, [_vp, _d, _d]),
     "qxd_set_gauge_reconstruct": (_i, [_vp, _i]),
+    "qxd_set_gauge_reconstruct_prec": (_i, [_vp, _i, _i]),
     "qxd_clover_export": (_i, [_vp, _vp, _i]),
     "qxd_apply_Dw": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dhat_eo": (_i, [_vp, _i, _vp, _vp, _i]),
@@ -276,8 +277,11 @@ class Qxd:
             return out.reshape((self.V // 2, 8) + (() if phase else (3, 3)))
         return out.reshape(self.dims + (4,) + (() if phase else (3, 3)))
 
-    def set_gauge_reconstruct(self, recon):
-        self._chk(self.lib.qxd_set_gauge_reconstruct(self.h, int(recon)))
+    def set_gauge_reconstruct(self, recon, prec=None):
+        if prec is None:
+            self._chk(self.lib.qxd_set_gauge_reconstruct(self.h, int(recon)))
+        else:
+            self._chk(self.lib.qxd_set_gauge_reconstruct_prec(self.h, int(prec), int(recon)))
 
     def set_rhs_per_thread(self, r):
         self._chk(self.lib.qxd_set_rhs_per_thread(self.h, int(r)))

@@ -236,15 +236,20 @@ int qxd_set_quark(qxd_ctx* c, double kappa, double q) {
   return QXD_OK;
 }
 
-int qxd_set_gauge_reconstruct(qxd_ctx* c, int recon) {
+int qxd_set_gauge_reconstruct_prec(qxd_ctx* c, int prec, int recon) {
   if (!c) return QXD_EINVAL;
+  if (prec < 0 || prec >= NPREC) return fail(c, QXD_EINVAL, "set_gauge_reconstruct: unknown precision");
   if (recon != QXD_RECON_NONE && recon != QXD_RECON_12) return fail(c, QXD_EINVAL, "set_gauge_reconstruct: QXD_RECON_NONE (18) or QXD_RECON_12 (12)");
   const int nl = recon == QXD_RECON_12 ? 14 : 18;
-  if (nl == c->link_reals) return QXD_OK;
-  c->link_reals = nl;
-  if (c->have_quark)   // the hopping links are derived data: rewrite them in the new format (the clover term is unaffected)
-    for (int pr = 0; pr < NPREC; pr++)
-      if ((c->prec_mask >> pr) & 1) { int rc = launch_hoplinks(c, pr); if (rc) return rc; }
+  if (nl == c->link_reals[prec]) return QXD_OK;
+  c->link_reals[prec] = nl;
+  // the hopping links are derived data: rewrite them in the new format (the clover term is unaffected)
+  if (c->have_quark && ((c->prec_mask >> prec) & 1)) return launch_hoplinks(c, prec);
+  return QXD_OK;
+}
+int qxd_set_gauge_reconstruct(qxd_ctx* c, int recon) {
+  if (!c) return QXD_EINVAL;
+  for (int pr = 0; pr < NPREC; pr++) { int rc = qxd_set_gauge_reconstruct_prec(c, pr, recon); if (rc) return rc; }
   return QXD_OK;
 }
 

@@ -63,7 +63,7 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   if (a.nrhs > 64) return fail(c, QXD_EINVAL, "dslash: at most 64 right-hand sides per launch");
   a.R.partials = c->partials; a.R.ticket = c->ticket; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
   int rc;
-  if (c->link_reals == 14) rc = d.prec == 0 ? dslash_dispatch_f64_l14(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l14(c, d, a) : dslash_dispatch_f16_l14(c, d, a);
+  if (c->link_reals[d.prec] == 14) rc = d.prec == 0 ? dslash_dispatch_f64_l14(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l14(c, d, a) : dslash_dispatch_f16_l14(c, d, a);
   else rc = d.prec == 0 ? dslash_dispatch_f64_l18(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l18(c, d, a) : dslash_dispatch_f16_l18(c, d, a);
   if (rc) return rc;
   QXD_LAUNCH_CHECK(c);

@@ -171,7 +171,7 @@ int launch_hoplinks(qxd_ctx* c, int prec) {
   dim3 gr = grid_for(c->g.Vh, 2);
   int ua = c->have_qed ? 1 : 0;
 #define QXD_HOPLINKS(S, NL) hoplinks_k<S, NL><<<gr, 128, 0, c->stream>>>(c->g, c->q, ua, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1], c->W[prec][0], c->W[prec][1])
-  if (c->link_reals == 14) { if (prec == 0) QXD_HOPLINKS(double, 14); else if (prec == 1) QXD_HOPLINKS(float, 14); else QXD_HOPLINKS(__half, 14); }
+  if (c->link_reals[prec] == 14) { if (prec == 0) QXD_HOPLINKS(double, 14); else if (prec == 1) QXD_HOPLINKS(float, 14); else QXD_HOPLINKS(__half, 14); }
   else { if (prec == 0) QXD_HOPLINKS(double, 18); else if (prec == 1) QXD_HOPLINKS(float, 18); else QXD_HOPLINKS(__half, 18); }
 #undef QXD_HOPLINKS
   QXD_LAUNCH_CHECK(c);

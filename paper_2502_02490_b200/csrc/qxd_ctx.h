@@ -37,7 +37,7 @@ struct qxd_ctx {
   char* ws = nullptr;
   size_t ws_bytes = 0, ws_used = 0;
   int prec_mask = 0, nrhs = 1;
-  int link_reals = 18;                           // stored reals per hopping link: 18, or 14 = rows 0,1 + det (qxd_set_gauge_reconstruct)
+  int link_reals[qxd::NPREC] = {18, 18, 18};     // per storage precision: stored reals per hopping link, 18 or 14 = rows 0,1 + det (qxd_set_gauge_reconstruct)
   int rhs_per_thread = 0;                        // multi-RHS dslash: right-hand sides per thread (0 = default)
   // state
   bool have_gauge = false, have_qed = false, have_quark = false, have_clover = false;

@@ -133,6 +133,11 @@ def test_reconstruct12_solve_and_bad_value(case):
         assert res <= 1.05e-10
         with pytest.raises(B.QxdError):
             case.gpu.set_gauge_reconstruct(8)
+        # per-precision format: fp16 back to 18 reals while fp64 / fp32 stay reconstructed; mixed fp64/fp16 solve
+        case.gpu.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=F16)
+        psi, info = case.gpu.solve(eta, 1e-10, algo=B.QXD_CGNE, sloppy=F16)
+        assert info["status"] == 0
+        assert relerr(case.ref.apply_Dw(to_np(psi).reshape(eta.shape)), eta) <= 1.05e-10
     finally:
         case.gpu.set_gauge_reconstruct(B.QXD_RECON_NONE)
 
