@@ -340,3 +340,51 @@ def test_full_c3_gamma5_hermiticity_property(full_c3_case):
     lhs = np.vdot(phi, to_np(c.gpu.apply_Dw(c.psi, F64)).reshape(phi.shape))
     rhs = np.vdot(g5 * to_np(c.gpu.apply_Dw(g5 * phi, F64)).reshape(phi.shape), c.psi)
     assert abs(lhs - rhs) / abs(lhs) < 1e-12
+
+
+def _c3_sample_sites(c, n_random, seed):
+    T, X1, L2, L3 = c.dims_ext
+    rng = np.random.default_rng(seed)
+    coords = [(0, 0, 0, 0), (T - 1, X1 - 1, L2 - 1, L3 - 1), (0, X1 // 2, 0, 0), (3, X1 // 2 - 1, L2 - 1, L3 - 1)]
+    coords += [tuple(int(rng.integers(0, n)) for n in c.dims_ext) for _ in range(n_random)]
+    return np.array([((x0 * X1 + x1) * L2 + x2) * L3 + x3 for x0, x1, x2, x3 in coords], dtype=np.int64)
+
+
+def test_full_c3_mixed_solve_sampled_residual(full_c3_case):
+    """The solve bench.py times (fp64/fp16 CGNE, 14-real links in fp64, 18-real in fp16) on the full c3 lattice: the
+    returned psi must satisfy (eta - D psi)(x) ~ 0 with the ORACLE's D at sampled sites: with ||r|| <= tol ||eta|| the
+    RMS of r over any sample is <= tol * RMS(eta) up to sampling noise (factor 5 allowed for 200 sites)."""
+    c = full_c3_case
+    B = c.B
+    c.gpu.set_gauge_reconstruct(B.QXD_RECON_12)
+    c.gpu.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=F16)
+    try:
+        psi, info = c.gpu.solve(c.psi, 1e-10, algo=B.QXD_CGNE, sloppy=F16, delta=0.1, maxiter=3000)
+    finally:
+        c.gpu.set_gauge_reconstruct(B.QXD_RECON_NONE)
+    assert info["status"] == 0 and info["true_res"] <= 1e-10
+    sites = _c3_sample_sites(c, 196, 23)
+    sol = to_np(psi).reshape(c.psi.shape)
+    r = c.ref.apply_Dw_sites(sol, sites) - c.psi.reshape(-1, 4, 3)[sites]
+    rms_r = np.sqrt(np.mean(np.abs(r) ** 2))
+    rms_eta = np.sqrt(np.mean(np.abs(c.psi) ** 2))
+    assert rms_r <= 5e-10 * rms_eta, (rms_r, rms_eta, info)
+
+
+@pytest.mark.parametrize("prec", [F32, F16])
+def test_full_c3_multi_rhs_sampled_sites(full_c3_case, prec):
+    """Row a10 at full size: three right-hand sides in one batched launch, sampled sites of each against the oracle."""
+    import torch
+    c = full_c3_case
+    g = c.gpu
+    etas = [c.psi, synth.gaussian_spinor(c.dims_ext, 31), synth.gaussian_spinor(c.dims_ext, 32)]
+    nb = g.packed_spinor_bytes(prec)
+    pin = torch.empty(3 * nb, dtype=torch.uint8, device="cuda")
+    pout = torch.zeros_like(pin)
+    for k in range(3):
+        g.spinor_pack(etas[k], prec, packed=pin[k * nb:(k + 1) * nb])
+    g.apply_Dw_multi_packed(pin, pout, prec, 3)
+    sites = _c3_sample_sites(c, 60, 29)
+    for k in range(3):
+        got = to_np(g.spinor_unpack(pout[k * nb:(k + 1) * nb], prec)).reshape(-1, 4, 3)[sites]
+        assert relerr(got, c.ref.apply_Dw_sites(etas[k], sites)) < TOL[prec], k
