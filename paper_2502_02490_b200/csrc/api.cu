@@ -66,7 +66,6 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
   void* nb = k.take(size_t(c->V) * 24 * 8);
   const int max_blocks = int((Vh + 127) / 128) * 2 + 8;
   void* partials = k.take(size_t(max_blocks) * 4 * 8 * nrhs);
-  void* ticket = k.take(256);
   void* scal = k.take(64 * 8);
   // batch vectors (row a10): fp64 b, x and five sloppy vectors per right-hand side; the sloppy ones are sized for the
   // widest bound precision below fp64 (fp64 itself if no other is bound)
@@ -90,7 +89,7 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
     for (int i = 0; i < 12; i++) c->sp64[i] = sp64[i];
     for (int i = 0; i < 8; i++) c->splo[i] = splo[i];
     c->full_a = fa; c->full_b = fb; c->nat_a = (double*)na; c->nat_b = (double*)nb;
-    c->partials = (double*)partials; c->ticket = (unsigned*)ticket; c->scal = (double*)scal; c->max_blocks = max_blocks;
+    c->partials = (double*)partials; c->scal = (double*)scal; c->max_blocks = max_blocks;
   }
   return k.off;
 }
@@ -202,7 +201,6 @@ int qxd_workspace_bind(qxd_ctx* c, void* dev, size_t bytes, int prec_mask, int n
   if (c->mscal) QXD_CUDA_OK(c, cudaMemsetAsync(c->mscal, 0, 64 * 8 * 8, c->stream));
   if (!c->ev0) QXD_CUDA_OK(c, cudaEventCreate(&c->ev0));
   if (!c->ev1) QXD_CUDA_OK(c, cudaEventCreate(&c->ev1));
-  QXD_CUDA_OK(c, cudaMemsetAsync(c->ticket, 0, 256, c->stream));
   QXD_CUDA_OK(c, cudaMemsetAsync(c->scal, 0, 64 * 8, c->stream));
   return QXD_OK;
 }
@@ -399,13 +397,13 @@ int qxd_blas_axpy(qxd_ctx* c, int prec, double a, const void* x, void* y) {
 }
 int qxd_blas_cdot(qxd_ctx* c, int prec, const void* x, const void* y, double* re_im) {
   if (!c || !x || !y || !re_im || prec < 0 || prec >= NPREC || !c->ws) return QXD_EINVAL;
-  int rc = blas_cdot(c, prec, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), half_view(prec, const_cast<void*>(y), c->g.Vh, 0), c->scal + 32);
+  int rc = blas_cdot(c, prec, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), half_view(prec, const_cast<void*>(y), c->g.Vh, 0), c->scal + 32, true);
   if (rc) return rc;
   return read_result(c, 2, re_im);
 }
 int qxd_blas_norm2(qxd_ctx* c, int prec, const void* x, double* out) {
   if (!c || !x || !out || prec < 0 || prec >= NPREC || !c->ws) return QXD_EINVAL;
-  int rc = blas_norm2(c, prec, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), c->scal + 32);
+  int rc = blas_norm2(c, prec, half_view(prec, const_cast<void*>(x), c->g.Vh, 0), c->scal + 32, Batch(), true);
   if (rc) return rc;
   return read_result(c, 1, out);
 }

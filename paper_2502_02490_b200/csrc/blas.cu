@@ -75,7 +75,11 @@ __global__ void __launch_bounds__(128) cg_xr_k(int Vh, const double* num, const 
     load_spinor<S>(t, Vh, cb, vp);
     load_spinor<S>(r, Vh, cb, vx);
 #pragma unroll
-    for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; nrm[0] += (double)vx[i] * (double)vx[i]; }
+    C part = 0;   // per-site sum in the arithmetic type (fp32 for fp32/fp16 storage), fp64 across sites: the float->double
+                  // conversions and DFMAs of a per-element fp64 sum cost more than the memory traffic of this kernel
+#pragma unroll
+    for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; part += vx[i] * vx[i]; }
+    nrm[0] = (double)part;
     store_spinor<S>(r, Vh, cb, vx);
   }
   grid_reduce<1>(nrm, R);
@@ -119,7 +123,10 @@ __global__ void __launch_bounds__(128) cg_xr_h_k(int Vh, const double* num, cons
     load_spinor<__half>(t, Vh, cb, vp);
     load_spinor<float>(r, Vh, cb, vx);
 #pragma unroll
-    for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; nrm[0] += (double)vx[i] * (double)vx[i]; }
+    float part = 0.f;
+#pragma unroll
+    for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; part += vx[i] * vx[i]; }
+    nrm[0] = (double)part;
     store_spinor<float>(r, Vh, cb, vx);
     store_spinor<__half>(r16, Vh, cb, vx);
   }
@@ -140,7 +147,9 @@ __global__ void __launch_bounds__(128) cg_p_h_k(int Vh, const double* num, const
   store_spinor<__half>(p16, Vh, cb, vp);
 }
 
-template <typename S>
+// EXACT: every product and sum in fp64 (the public qxd_blas_* entry points); otherwise the per-site sum runs in the
+// arithmetic type of the storage precision and only the sum over sites is fp64 (solver-internal calls).
+template <typename S, bool EXACT>
 __global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R, size_t rs) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
@@ -149,13 +158,20 @@ __global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R, s
   if (cb < Vh) {
     C v[24];
     load_spinor<S>(x, Vh, cb, v);
+    if (EXACT) {
 #pragma unroll
-    for (int i = 0; i < 24; i++) nrm[0] += (double)v[i] * (double)v[i];
+      for (int i = 0; i < 24; i++) nrm[0] += (double)v[i] * (double)v[i];
+    } else {
+      C part = 0;
+#pragma unroll
+      for (int i = 0; i < 24; i++) part += v[i] * v[i];
+      nrm[0] = (double)part;
+    }
   }
   grid_reduce<1>(nrm, R);
 }
 // <x,y> = sum conj(x) y  (re, im) and |y|^2 as a third component
-template <typename S>
+template <typename S, bool EXACT>
 __global__ void __launch_bounds__(128) cdot_k(int Vh, SpinorPtr x, SpinorPtr y, Reducer R) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
@@ -164,12 +180,24 @@ __global__ void __launch_bounds__(128) cdot_k(int Vh, SpinorPtr x, SpinorPtr y, 
     C vx[24], vy[24];
     load_spinor<S>(x, Vh, cb, vx);
     load_spinor<S>(y, Vh, cb, vy);
+    if (EXACT) {
 #pragma unroll
-    for (int k = 0; k < 12; k++) {
-      double xr = vx[2 * k], xi = vx[2 * k + 1], yr = vy[2 * k], yi = vy[2 * k + 1];
-      d[0] += xr * yr + xi * yi;
-      d[1] += xr * yi - xi * yr;
-      d[2] += yr * yr + yi * yi;
+      for (int k = 0; k < 12; k++) {
+        double xr = vx[2 * k], xi = vx[2 * k + 1], yr = vy[2 * k], yi = vy[2 * k + 1];
+        d[0] += xr * yr + xi * yi;
+        d[1] += xr * yi - xi * yr;
+        d[2] += yr * yr + yi * yi;
+      }
+    } else {
+      C p0 = 0, p1 = 0, p2 = 0;
+#pragma unroll
+      for (int k = 0; k < 12; k++) {
+        const C xr = vx[2 * k], xi = vx[2 * k + 1], yr = vy[2 * k], yi = vy[2 * k + 1];
+        p0 += xr * yr; p0 += xi * yi;
+        p1 += xr * yi; p1 -= xi * yr;
+        p2 += yr * yr; p2 += yi * yi;
+      }
+      d[0] = (double)p0; d[1] = (double)p1; d[2] = (double)p2;
     }
   }
   grid_reduce<3>(d, R);
@@ -220,7 +248,7 @@ __global__ void __launch_bounds__(128) sub_norm_k(int Vh, SpinorPtr b, SpinorPtr
 
 inline Reducer reducer(qxd_ctx* c, double* result, int rstride = 0) {
   Reducer R;
-  R.partials = c->partials; R.ticket = c->ticket; R.result = result; R.rstride = rstride;
+  R.partials = c->partials; R.result = result; R.rstride = rstride;
   return R;
 }
 
@@ -231,6 +259,13 @@ inline Reducer reducer(qxd_ctx* c, double* result, int rstride = 0) {
     if ((prec) == 0) { typedef double S; __VA_ARGS__; }        \
     else if ((prec) == 1) { typedef float S; __VA_ARGS__; }    \
     else { typedef __half S; __VA_ARGS__; }                    \
+  } while (0)
+
+// second kernel of every reduction: adds the per-block partials of the launch before it (qxd_common.cuh)
+#define QXD_FINALIZE(N, res, rstride, nslots)                                                                           \
+  do {                                                                                                                  \
+    QXD_LAUNCH_CHECK(c);                                                                                                \
+    reduce_finalize_k<N><<<dim3(1, (nslots)), 256, 0, c->stream>>>(reducer(c, (res), (rstride)), (c->g.Vh + 127) / 128); \
   } while (0)
 
 #define QXD_GRID dim3((c->g.Vh + 127) / 128), 128, 0, c->stream
@@ -251,6 +286,7 @@ int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai
 int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
                const SpinorPtr& r, double* rr, const Batch& b) {
   QXD_BY_PREC(prec, cg_xr_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, num, den, p, t, x, r, reducer(c, rr, b.ss), b.rs, b.ss, b.act));
+  QXD_FINALIZE(1, rr, b.ss, b.n);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
@@ -262,6 +298,7 @@ int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const 
 int blas_cg_xr_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
                  const SpinorPtr& r, const SpinorPtr& r16, double* rr) {
   cg_xr_h_k<<<QXD_GRID>>>(c->g.Vh, num, den, p, t, x, r, r16, reducer(c, rr));
+  QXD_FINALIZE(1, rr, 0, 1);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
@@ -270,13 +307,17 @@ int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPt
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* res, const Batch& b) {
-  QXD_BY_PREC(prec, norm2_k<S><<<QXD_GRID_N(b.n)>>>(c->g.Vh, x, reducer(c, res, b.ss), b.rs));
+int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* res, const Batch& b, bool exact) {
+  if (exact) QXD_BY_PREC(prec, norm2_k<S, true><<<QXD_GRID_N(b.n)>>>(c->g.Vh, x, reducer(c, res, b.ss), b.rs));
+  else QXD_BY_PREC(prec, norm2_k<S, false><<<QXD_GRID_N(b.n)>>>(c->g.Vh, x, reducer(c, res, b.ss), b.rs));
+  QXD_FINALIZE(1, res, b.ss, b.n);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* res3) {
-  QXD_BY_PREC(prec, cdot_k<S><<<QXD_GRID>>>(c->g.Vh, x, y, reducer(c, res3)));
+int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* res3, bool exact) {
+  if (exact) QXD_BY_PREC(prec, cdot_k<S, true><<<QXD_GRID>>>(c->g.Vh, x, y, reducer(c, res3)));
+  else QXD_BY_PREC(prec, cdot_k<S, false><<<QXD_GRID>>>(c->g.Vh, x, y, reducer(c, res3)));
+  QXD_FINALIZE(3, res3, 0, 1);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
@@ -295,6 +336,7 @@ int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi
 }
 int blas_sub_norm(qxd_ctx* c, int prec, const SpinorPtr& b, const SpinorPtr& t, const SpinorPtr& r, double* res) {
   QXD_BY_PREC(prec, sub_norm_k<S><<<QXD_GRID>>>(c->g.Vh, b, t, r, reducer(c, res)));
+  QXD_FINALIZE(1, res, 0, 1);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

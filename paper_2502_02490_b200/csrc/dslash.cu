@@ -61,12 +61,16 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.nrhs = d.nrhs > 1 ? d.nrhs : 1; a.ngroups = 1;
   a.rs_in = d.rs_in; a.rs_phi = d.rs_phi; a.rs_out = d.rs_out;
   if (a.nrhs > 64) return fail(c, QXD_EINVAL, "dslash: at most 64 right-hand sides per launch");
-  a.R.partials = c->partials; a.R.ticket = c->ticket; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
+  a.R.partials = c->partials; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
   int rc;
   if (c->link_reals[d.prec] == 14) rc = d.prec == 0 ? dslash_dispatch_f64_l14(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l14(c, d, a) : dslash_dispatch_f16_l14(c, d, a);
   else rc = d.prec == 0 ? dslash_dispatch_f64_l18(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l18(c, d, a) : dslash_dispatch_f16_l18(c, d, a);
   if (rc) return rc;
   QXD_LAUNCH_CHECK(c);
+  if (d.flags & DSF_NORM) {   // second kernel of the fused norm: add the per-tile partials (qxd_common.cuh)
+    reduce_finalize_k<1><<<dim3(1, a.nrhs), 256, 0, c->stream>>>(a.R, (c->g.Vh + 127) / 128);
+    QXD_LAUNCH_CHECK(c);
+  }
   return QXD_OK;
 }
 

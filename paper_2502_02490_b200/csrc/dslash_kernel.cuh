@@ -326,9 +326,11 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
 #pragma unroll
     for (int r = 0; r < R; r++) {
       if (R > 1 && rhs0 + r >= a.nrhs) break;
-      if (FLAGS & DSF_NORM) {
+      if (FLAGS & DSF_NORM) {   // per-site sum in the arithmetic type, fp64 across sites (see blas.cu)
+        C part = 0;
 #pragma unroll
-        for (int i = 0; i < 24; i++) nrm[r] += (double)acc[r][i] * (double)acc[r][i];
+        for (int i = 0; i < 24; i++) part += acc[r][i] * acc[r][i];
+        nrm[r] = (double)part;
       }
       store_spinor<S>(rhs_view(a.out[parity], a.rs_out, rhs0 + r), Vh, cb, acc[r]);
     }

@@ -65,7 +65,6 @@ struct qxd_ctx {
   double* h_mact = nullptr;
   // reductions
   double* partials = nullptr;
-  unsigned* ticket = nullptr;
   double* scal = nullptr;                        // device scalars [64]
   double* h_scal = nullptr;                      // pinned host mirror [64]
   int max_blocks = 0;
@@ -139,8 +138,9 @@ struct Batch {
   const double* act = nullptr;
 };
 int blas_axpy(qxd_ctx* c, int prec, double a, const SpinorPtr& x, const SpinorPtr& y);            // y += a x
-int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* dev_result3);  // Re<x,y>, Im<x,y>, |y|^2
-int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* dev_result, const Batch& b = Batch());
+// exact: every product and sum in fp64; default: per-site sums in the arithmetic type, fp64 across sites (solver calls)
+int blas_cdot(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, double* dev_result3, bool exact = false);  // Re<x,y>, Im<x,y>, |y|^2
+int blas_norm2(qxd_ctx* c, int prec, const SpinorPtr& x, double* dev_result, const Batch& b = Batch(), bool exact = false);
 int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x, const Batch& b = Batch());
 // z = x + a*y + b*w with complex scalars by value (w may be unused when b == 0); BiCGstab building block
 int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai, const SpinorPtr& y, double br, double bi,
