@@ -129,6 +129,7 @@ int qxd_geometry_destroy(qxd_ctx* c) {
   if (c->h_scal) cudaFreeHost(c->h_scal);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);
+  if (c->ev_scal) cudaEventDestroy(c->ev_scal);
   delete c;
   return QXD_OK;
 }
@@ -201,6 +202,7 @@ int qxd_workspace_bind(qxd_ctx* c, void* dev, size_t bytes, int prec_mask, int n
   if (c->mscal) QXD_CUDA_OK(c, cudaMemsetAsync(c->mscal, 0, 64 * 8 * 8, c->stream));
   if (!c->ev0) QXD_CUDA_OK(c, cudaEventCreate(&c->ev0));
   if (!c->ev1) QXD_CUDA_OK(c, cudaEventCreate(&c->ev1));
+  if (!c->ev_scal) QXD_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_scal, cudaEventDisableTiming));
   QXD_CUDA_OK(c, cudaMemsetAsync(c->scal, 0, 64 * 8, c->stream));
   return QXD_OK;
 }

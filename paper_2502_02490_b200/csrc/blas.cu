@@ -265,7 +265,7 @@ inline Reducer reducer(qxd_ctx* c, double* result, int rstride = 0) {
 #define QXD_FINALIZE(N, res, rstride, nslots)                                                                           \
   do {                                                                                                                  \
     QXD_LAUNCH_CHECK(c);                                                                                                \
-    reduce_finalize_k<N><<<dim3(1, (nslots)), 256, 0, c->stream>>>(reducer(c, (res), (rstride)), (c->g.Vh + 127) / 128); \
+    reduce_finalize_k<N><<<dim3(1, (nslots)), FINALIZE_THREADS, 0, c->stream>>>(reducer(c, (res), (rstride)), (c->g.Vh + 127) / 128); \
   } while (0)
 
 #define QXD_GRID dim3((c->g.Vh + 127) / 128), 128, 0, c->stream

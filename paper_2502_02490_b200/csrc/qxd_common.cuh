@@ -271,24 +271,35 @@ __device__ __forceinline__ void grid_reduce(double (&v)[N], const Reducer& R, in
     }
   }
 }
-// grid (1, nslots), 256 threads: result[slot * rstride + k] = sum_i partials[slot][k][i], fixed order
+// grid (1, nslots), FINALIZE_THREADS threads: result[slot * rstride + k] = sum_i partials[slot][k][i], fixed order
+constexpr int FINALIZE_THREADS = 1024;
 template <int N>
-__global__ void __launch_bounds__(256) reduce_finalize_k(Reducer R, int nparts) {
-  __shared__ double sm[8];
+__global__ void __launch_bounds__(FINALIZE_THREADS) reduce_finalize_k(Reducer R, int nparts) {
+  __shared__ double sm[N][32];
   const int slot = blockIdx.y, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const double* partials = R.partials + size_t(slot) * N * nparts;
+  double t[N];
+#pragma unroll
   for (int k = 0; k < N; k++) {
-    double t = 0.0;
-    for (int i = threadIdx.x; i < nparts; i += 256) t += partials[size_t(k) * nparts + i];
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;   // four independent loads in flight per thread
+    int i = threadIdx.x;
+    for (; i + 3 * FINALIZE_THREADS < nparts; i += 4 * FINALIZE_THREADS) {
+      t0 += partials[size_t(k) * nparts + i]; t1 += partials[size_t(k) * nparts + i + FINALIZE_THREADS];
+      t2 += partials[size_t(k) * nparts + i + 2 * FINALIZE_THREADS]; t3 += partials[size_t(k) * nparts + i + 3 * FINALIZE_THREADS];
+    }
+    for (; i < nparts; i += FINALIZE_THREADS) t0 += partials[size_t(k) * nparts + i];
+    t[k] = (t0 + t1) + (t2 + t3);
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    __syncthreads();
-    if (lane == 0) sm[w] = t;
-    __syncthreads();
-    if (w == 0) {
-      double u = lane < 8 ? sm[lane] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) t[k] += __shfl_xor_sync(0xffffffffu, t[k], o);
+    if (lane == 0) sm[k][w] = t[k];
+  }
+  __syncthreads();
+  if (w == 0) {
 #pragma unroll
-      for (int o = 4; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
+    for (int k = 0; k < N; k++) {
+      double u = sm[k][lane];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
       if (lane == 0) R.result[size_t(slot) * R.rstride + k] = u;
     }
   }

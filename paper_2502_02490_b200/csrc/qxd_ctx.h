@@ -71,6 +71,7 @@ struct qxd_ctx {
   long launches = 0;
   std::string err;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  cudaEvent_t ev_scal = nullptr;                 // marks the device->host copy of solver scalars (solver.cu: post_scal / wait_scal)
 };
 
 namespace qxd {

@@ -32,6 +32,19 @@ int read_scal(qxd_ctx* c, int idx, int n, double* out) {
   return QXD_OK;
 }
 
+// Split form of read_scal: post_scal enqueues the copy and marks it with an event; work enqueued afterwards keeps the GPU
+// busy while wait_scal blocks the host on that event only (not on the whole stream).
+int post_scal(qxd_ctx* c, int idx, int n) {
+  QXD_CUDA_OK(c, cudaMemcpyAsync(c->h_scal + idx, c->scal + idx, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+  QXD_CUDA_OK(c, cudaEventRecord(c->ev_scal, c->stream));
+  return QXD_OK;
+}
+int wait_scal(qxd_ctx* c, int idx, int n, double* out) {
+  QXD_CUDA_OK(c, cudaEventSynchronize(c->ev_scal));
+  for (int i = 0; i < n; i++) out[i] = c->h_scal[idx + i];
+  return QXD_OK;
+}
+
 #define QXD_TRY(expr)        \
   do {                       \
     int rc__ = (expr);       \
@@ -108,7 +121,12 @@ int cgne(qxd_ctx* c, int pop, Ws& w0, double stop2, double delta, int maxiter, q
     QXD_TRY(apply_dhat(c, pop, pin, w.t, w.tmp_o_lo, 0, c->scal + SC_TT));
     if (h16) QXD_TRY(blas_cg_xr_h(c, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, r16, c->scal + SC_RR));
     else QXD_TRY(blas_cg_xr(c, plo, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, c->scal + SC_RR));
-    QXD_TRY(read_scal(c, SC_RR, 1, &rr));
+    // |r|^2 decides on the host whether to stop or to do a reliable update.  s = A^dag r is enqueued BEFORE the host waits
+    // for it, so the GPU never idles on the round trip; it is only wasted (recomputed from the corrected r) in the
+    // iterations that do a reliable update.
+    QXD_TRY(post_scal(c, SC_RR, 1));
+    QXD_TRY(apply_dhat(c, pop, rin, w.s, w.tmp_o_lo, 1, gam_next));
+    QXD_TRY(wait_scal(c, SC_RR, 1, &rr));
     it++;
     if (!(rr == rr)) break;  // NaN: breakdown
     double rn = std::sqrt(rr);
@@ -118,8 +136,8 @@ int cgne(qxd_ctx* c, int pop, Ws& w0, double stop2, double delta, int maxiter, q
       nrel++;
       maxr = std::sqrt(rr_true);
       if (rr_true <= stop2) { status = QXD_OK; break; }
+      QXD_TRY(apply_dhat(c, pop, rin, w.s, w.tmp_o_lo, 1, gam_next));
     }
-    QXD_TRY(apply_dhat(c, pop, rin, w.s, w.tmp_o_lo, 1, gam_next));
     if (h16) QXD_TRY(blas_cg_p_h(c, gam_next, gam, w.s, w.p, p16));
     else QXD_TRY(blas_cg_p(c, plo, gam_next, gam, w.s, w.p));
   }
