@@ -256,20 +256,23 @@ __device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int 
 // R > 1 (row a10, multi-RHS): every thread applies the operator of its site to R right-hand sides, loading each link
 // and clover block once; ngroups consecutive CTAs cover all right-hand sides of one tile, so the links of a tile are
 // read from DRAM once and from L2 by the other groups.
-template <typename S, int R, bool FULL> struct KernelShape {
-  // single right-hand side, full lattice: one CTA of 128 threads per (tile, parity), the two parities of a tile in
-  // consecutive CTAs (measured 4.5 % faster at c3 fp32 than one 256-thread CTA per tile: 534 vs 559 us under ncu)
-  static constexpr bool SPLIT = FULL && R == 1;
+template <typename S, int R, bool FULL, int NL> struct KernelShape {
+  // Full lattice, single right-hand side: either one 256-thread CTA per tile (both parities: the second use of every link
+  // hits L1) or one 128-thread CTA per (tile, parity) in consecutive CTAs (links shared through L2).  Timed alone (ncu, 1.83
+  // GHz) the split form is 4.5 % faster (534 vs 559 us, 18-real links); in a long run the GPU sits on its power cap and
+  // the time follows the energy per apply: the extra 0.8 GB of L2 -> SM traffic of the split form costs 6 % (0.68 vs 0.64
+  // ms sustained) with 18-real links, while with the 14-real format the split form stays ahead (0.61 vs 0.62 ms).
+  static constexpr bool SPLIT = FULL && R == 1 && NL == 14;
   static constexpr int THREADS = (FULL && !SPLIT) ? 256 : 128;
   // CTAs per SM the register budget is sized for
   static constexpr int MINB = SPLIT ? (sizeof(S) == 8 ? 2 : 4) : sizeof(S) == 8 ? 1 : (R == 1 ? (FULL ? 2 : 4) : (R == 2 ? (FULL ? 1 : 3) : (FULL ? 1 : 2)));
   static constexpr int PIPE = (R == 1) ? 2 : 1;   // hops in flight per thread
 };
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
-__global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<S, R, FULL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
+__global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelShape<S, R, FULL, NL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
   typedef typename PT<S>::C C;
   const int Vh = a.g.Vh;
-  constexpr bool SPLIT = KernelShape<S, R, FULL>::SPLIT;
+  constexpr bool SPLIT = KernelShape<S, R, FULL, NL>::SPLIT;
   // block index -> (tile, parity, group of R right-hand sides), groups fastest: the CTAs that need the links and clover
   // blocks of a tile run at the same time, so a batch reads them from DRAM once and from L2 afterwards
   const int bt = blockIdx.x / a.ngroups;
@@ -289,7 +292,7 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
 #pragma unroll
       for (int i = 0; i < 24; i++) acc[r][i] = 0;
     const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
-    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL>::PIPE, NL>(a, s, cb, parity, rhs0, acc);
+    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL, NL>::PIPE, NL>(a, s, cb, parity, rhs0, acc);
 #pragma unroll
     for (int r = 0; r < R; r++)
 #pragma unroll
@@ -349,8 +352,8 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL>::THREADS, KernelShape<
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
 void launch_r(qxd_ctx* c, DslashArgs& a) {
   a.ngroups = (a.nrhs + R - 1) / R;
-  dim3 gr(unsigned((c->g.Vh + 127) / 128) * unsigned(a.ngroups) * (KernelShape<S, R, FULL>::SPLIT ? 2u : 1u));
-  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL><<<gr, KernelShape<S, R, FULL>::THREADS, 0, c->stream>>>(a);
+  dim3 gr(unsigned((c->g.Vh + 127) / 128) * unsigned(a.ngroups) * (KernelShape<S, R, FULL, NL>::SPLIT ? 2u : 1u));
+  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL><<<gr, KernelShape<S, R, FULL, NL>::THREADS, 0, c->stream>>>(a);
 }
 // right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 1:
 // measured at c3 with 12 right-hand sides, fp32: 0.43 ms per right-hand side against 0.59 (R = 2) and 0.50 (R = 3))
