@@ -328,14 +328,16 @@ def run_cuda(args, cfg):
             solves[name] = info
         if args.nrhs > 1:
             etas = torch.stack([eta_d] + [torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + k)).to(dev) for k in range(1, args.nrhs)])
-            l0 = g.launch_count()
-            t0 = time.perf_counter()
-            _, infos = g.solve_multi(etas, cfg["tol"], sloppy=B.QXD_F32, delta=0.1, maxiter=args.maxiter)
-            torch.cuda.synchronize(dev)
-            solves[f"cgne_multi{args.nrhs}_fp64_fp32"] = {
-                "status": max(abs(i["status"]) for i in infos), "iters_max": max(i["iters"] for i in infos),
-                "true_res_max": max(i["true_res"] for i in infos), "seconds": time.perf_counter() - t0,
-                "seconds_per_rhs": (time.perf_counter() - t0) / args.nrhs, "launches": g.launch_count() - l0, "tol": cfg["tol"], "links": "recon12"}
+            for sl, tag, links in ((B.QXD_F32, "fp32", "recon12"), (B.QXD_F16, "fp16", "fp64: recon12, fp16: 18 reals")):
+                l0 = g.launch_count()
+                t0 = time.perf_counter()
+                _, infos = g.solve_multi(etas, cfg["tol"], sloppy=sl, delta=0.1, maxiter=args.maxiter)
+                torch.cuda.synchronize(dev)
+                dt = time.perf_counter() - t0
+                solves[f"cgne_multi{args.nrhs}_fp64_{tag}"] = {
+                    "status": max(abs(i["status"]) for i in infos), "iters_max": max(i["iters"] for i in infos),
+                    "true_res_max": max(i["true_res"] for i in infos), "seconds": dt, "seconds_per_rhs": dt / args.nrhs,
+                    "launches": g.launch_count() - l0, "tol": cfg["tol"], "links": links}
             del etas
         g.set_gauge_reconstruct(B.QXD_RECON_NONE)
 

@@ -69,20 +69,20 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
   void* scal = k.take(64 * 8);
   // batch vectors (row a10): fp64 b, x and five sloppy vectors per right-hand side; the sloppy ones are sized for the
   // widest bound precision below fp64 (fp64 itself if no other is bound)
-  void* mhi[2] = {}; void* mlo[5] = {};
+  void* mhi[2] = {}; void* mlo[7] = {};
   const size_t mlo_size = (prec_mask & 2) ? 4 : (prec_mask & 4) ? 2 : 8;
   void* mscal = nullptr; void* mact = nullptr;
   if (nrhs > 1) {
     const int plo = mlo_size == 8 ? 0 : mlo_size == 4 ? 1 : 2;
     const size_t lo = (half_bytes(plo, Vh) + 255) & ~size_t(255);
     for (int i = 0; i < 2; i++) mhi[i] = k.take(half_bytes(0, Vh) * nrhs);
-    for (int i = 0; i < 5; i++) mlo[i] = k.take(lo * nrhs);
+    for (int i = 0; i < 7; i++) mlo[i] = k.take(lo * nrhs);
     mscal = k.take(64 * 8 * 8);
     mact = k.take(64 * 8);
   }
   if (assign) {
     for (int i = 0; i < 2; i++) c->mhi[i] = mhi[i];
-    for (int i = 0; i < 5; i++) c->mlo[i] = mlo[i];
+    for (int i = 0; i < 7; i++) c->mlo[i] = mlo[i];
     c->mlo_size = nrhs > 1 ? mlo_size : 0; c->mscal = (double*)mscal; c->mact = (double*)mact;
     for (int p = 0; p < 2; p++) { c->Ug[p] = Ug[p]; c->Ag[p] = Ag[p]; }
     for (int pr = 0; pr < NPREC; pr++) for (int p = 0; p < 2; p++) { c->W[pr][p] = W[pr][p]; c->M[pr][p] = M[pr][p]; c->Mi[pr][p] = Mi[pr][p]; }

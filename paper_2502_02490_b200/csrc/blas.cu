@@ -108,12 +108,14 @@ __global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const d
 // mantissas every iteration was measured to cost 2.8x the iterations of the fp32 solver at config c3.
 //   x += alpha p ; r -= alpha t(half) ; r16 = half(r) ; result = |r|^2
 __global__ void __launch_bounds__(128) cg_xr_h_k(int Vh, const double* num, const double* den, SpinorPtr p, SpinorPtr t, SpinorPtr x,
-                                                 SpinorPtr r, SpinorPtr r16, Reducer R) {
+                                                 SpinorPtr r, SpinorPtr r16, Reducer R, size_t rs_v, size_t rs_o, int ss, const double* act) {
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   double nrm[1] = {0.0};
+  const int k = blockIdx.y;   // right-hand side (batched form, row a10): fp32 vectors rs_v bytes apart, binary16 ones rs_o
+  p = rhs_view(p, rs_v, k); x = rhs_view(x, rs_v, k); r = rhs_view(r, rs_v, k); t = rhs_view(t, rs_o, k); r16 = rhs_view(r16, rs_o, k);
   if (cb < Vh) {
-    const double dn = den[0];
-    const float al = dn == 0.0 ? 0.f : (float)(num[0] / dn);
+    const double dn = den[k * ss];
+    const float al = (act && act[k] == 0.0) || dn == 0.0 ? 0.f : (float)(num[k * ss] / dn);
     float vp[24], vx[24];
     load_spinor<float>(p, Vh, cb, vp);
     load_spinor<float>(x, Vh, cb, vx);
@@ -122,7 +124,6 @@ __global__ void __launch_bounds__(128) cg_xr_h_k(int Vh, const double* num, cons
     store_spinor<float>(x, Vh, cb, vx);
     load_spinor<__half>(t, Vh, cb, vp);
     load_spinor<float>(r, Vh, cb, vx);
-#pragma unroll
     float part = 0.f;
 #pragma unroll
     for (int i = 0; i < 24; i++) { vx[i] -= al * vp[i]; part += vx[i] * vx[i]; }
@@ -133,11 +134,14 @@ __global__ void __launch_bounds__(128) cg_xr_h_k(int Vh, const double* num, cons
   grid_reduce<1>(nrm, R);
 }
 //   p = s(half) + beta p ; p16 = half(p)
-__global__ void __launch_bounds__(128) cg_p_h_k(int Vh, const double* num, const double* den, SpinorPtr s, SpinorPtr p, SpinorPtr p16) {
+__global__ void __launch_bounds__(128) cg_p_h_k(int Vh, const double* num, const double* den, SpinorPtr s, SpinorPtr p, SpinorPtr p16,
+                                                size_t rs_v, size_t rs_o, int ss, const double* act) {
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   if (cb >= Vh) return;
-  const double dn = den[0];
-  const float be = dn == 0.0 ? 0.f : (float)(num[0] / dn);
+  const int k = blockIdx.y;
+  s = rhs_view(s, rs_o, k); p16 = rhs_view(p16, rs_o, k); p = rhs_view(p, rs_v, k);
+  const double dn = den[k * ss];
+  const float be = (act && act[k] == 0.0) || dn == 0.0 ? 0.f : (float)(num[k * ss] / dn);
   float vs[24], vp[24];
   load_spinor<__half>(s, Vh, cb, vs);
   load_spinor<float>(p, Vh, cb, vp);
@@ -147,8 +151,6 @@ __global__ void __launch_bounds__(128) cg_p_h_k(int Vh, const double* num, const
   store_spinor<__half>(p16, Vh, cb, vp);
 }
 
-// EXACT: every product and sum in fp64 (the public qxd_blas_* entry points); otherwise the per-site sum runs in the
-// arithmetic type of the storage precision and only the sum over sites is fp64 (solver-internal calls).
 template <typename S, bool EXACT>
 __global__ void __launch_bounds__(128) norm2_k(int Vh, SpinorPtr x, Reducer R, size_t rs) {
   typedef typename PT<S>::C C;
@@ -296,14 +298,15 @@ int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const 
   return QXD_OK;
 }
 int blas_cg_xr_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
-                 const SpinorPtr& r, const SpinorPtr& r16, double* rr) {
-  cg_xr_h_k<<<QXD_GRID>>>(c->g.Vh, num, den, p, t, x, r, r16, reducer(c, rr));
-  QXD_FINALIZE(1, rr, 0, 1);
+                 const SpinorPtr& r, const SpinorPtr& r16, double* rr, const Batch& b, size_t rs_o) {
+  cg_xr_h_k<<<QXD_GRID_N(b.n)>>>(c->g.Vh, num, den, p, t, x, r, r16, reducer(c, rr, b.ss), b.rs, rs_o, b.ss, b.act);
+  QXD_FINALIZE(1, rr, b.ss, b.n);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const SpinorPtr& p16) {
-  cg_p_h_k<<<QXD_GRID>>>(c->g.Vh, num, den, s, p, p16);
+int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const SpinorPtr& p16,
+                const Batch& b, size_t rs_o) {
+  cg_p_h_k<<<QXD_GRID_N(b.n)>>>(c->g.Vh, num, den, s, p, p16, b.rs, rs_o, b.ss, b.act);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

@@ -57,7 +57,7 @@ struct qxd_ctx {
   double* nat_b = nullptr;
   // batch (multi-RHS) vectors, present when the workspace was bound with nrhs > 1: nrhs half-lattice spinors each
   void* mhi[2] = {};                             // fp64: b, x
-  void* mlo[5] = {};                             // sloppy: x, r, p, t(=s), odd-site scratch; mlo_size bytes per real
+  void* mlo[7] = {};                             // sloppy: x, r, p, t(=s), odd-site scratch, r16, p16 (fp16 operator with fp32 vectors); mlo_size bytes per real
   size_t mlo_size = 0;
   double* mscal = nullptr;                       // device scalars [64 systems][8]
   double* mact = nullptr;                        // device activity mask [64]
@@ -152,9 +152,11 @@ int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const
 // beta = *num / *den : p = s + beta p
 int blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const Batch& b = Batch());
 // fp16 operator with fp32 vectors: x, r, p in float; t, s and the operator inputs r16, p16 in binary16
+// (batch b: fp32 vectors b.rs bytes apart, binary16 vectors rs_o bytes apart)
 int blas_cg_xr_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
-                 const SpinorPtr& r, const SpinorPtr& r16, double* rr);
-int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const SpinorPtr& p16);
+                 const SpinorPtr& r, const SpinorPtr& r16, double* rr, const Batch& b = Batch(), size_t rs_o = 0);
+int blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const SpinorPtr& s, const SpinorPtr& p, const SpinorPtr& p16,
+                const Batch& b = Batch(), size_t rs_o = 0);
 int blas_acc_hi(qxd_ctx* c, int prec, const SpinorPtr& xlo, const SpinorPtr& xhi);                  // x_hi += x_lo ; x_lo = 0
 int blas_sub_norm(qxd_ctx* c, int prec, const SpinorPtr& b, const SpinorPtr& t, const SpinorPtr& r, double* res);  // r = b - t
 int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, const Batch& b = Batch());   // y = x

@@ -299,9 +299,12 @@ int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd
 // ---------------------------------------------------------------------------------------------------------------
 int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info) {
   const int Vh = c->g.Vh;
-  const int plo = info[0].sloppy;
+  const int pop = info[0].sloppy;   // precision of the sloppy operator
+  // binary16 operator: the Krylov vectors x, r, p stay in fp32 (reading R12) when the batch workspace is sized for fp32
+  const bool h16 = (pop == 2 && c->mlo_size >= 4);
+  const int plo = h16 ? 1 : pop;    // precision of the Krylov vectors
   if (nrhs < 1 || nrhs > c->nrhs) return fail(c, QXD_EINVAL, "solve_multi: nrhs exceeds the value the workspace was bound for");
-  if (plo < 0 || plo >= NPREC || !((c->prec_mask >> plo) & 1)) return fail(c, QXD_EINVAL, "solve_multi: sloppy precision not bound");
+  if (pop < 0 || pop >= NPREC || !((c->prec_mask >> pop) & 1)) return fail(c, QXD_EINVAL, "solve_multi: sloppy precision not bound");
   if (prec_size(plo) > c->mlo_size) return fail(c, QXD_EINVAL, "solve_multi: the batch workspace is sized for a narrower sloppy precision");
   if (info[0].algo != QXD_CGNE) return fail(c, QXD_EINVAL, "solve_multi: only QXD_CGNE is batched");
   if (!(tol > 0.0)) return fail(c, QXD_EINVAL, "solve_multi: tol must be > 0");
@@ -309,6 +312,7 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
   const int maxiter = info[0].maxiter > 0 ? info[0].maxiter : 10000;
   enum { SS = 8, M_GAM0 = 0, M_GAM1 = 1, M_TT = 2, M_RR = 3, M_RRT = 4 };
   const size_t rs_hi = half_bytes(0, Vh), rs_lo = (half_bytes(plo, Vh) + 255) & ~size_t(255);
+  const size_t rs_op = (half_bytes(pop, Vh) + 255) & ~size_t(255);   // operator inputs / outputs
   const size_t vnat = size_t(c->V) * 24;
   // single-RHS scratch (fp64)
   SpinorPtr eta_e = half_view(0, c->full_a, Vh, 0), eta_o = half_view(0, c->full_a, Vh, 1);
@@ -316,11 +320,15 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
   SpinorPtr thi = hv(0, c->sp64[3], Vh), tmp_o_hi = hv(0, c->sp64[4], Vh), rhi = hv(0, c->sp64[2], Vh);
   // batch vectors
   SpinorPtr B = hv(0, c->mhi[0], Vh), X = hv(0, c->mhi[1], Vh);
-  SpinorPtr xlo = hv(plo, c->mlo[0], Vh), rlo = hv(plo, c->mlo[1], Vh), p = hv(plo, c->mlo[2], Vh), t = hv(plo, c->mlo[3], Vh),
-            tmp_o = hv(plo, c->mlo[4], Vh);
+  SpinorPtr xlo = hv(plo, c->mlo[0], Vh), rlo = hv(plo, c->mlo[1], Vh), p = hv(plo, c->mlo[2], Vh), t = hv(pop, c->mlo[3], Vh),
+            tmp_o = hv(pop, c->mlo[4], Vh);
+  SpinorPtr r16 = hv(pop, c->mlo[5], Vh), p16 = hv(pop, c->mlo[6], Vh);   // binary16 copies the operator reads (h16 only)
+  const SpinorPtr& rin = h16 ? r16 : rlo;
+  const SpinorPtr& pin = h16 ? p16 : p;
   double* ms = c->mscal;
   double* hs = c->h_mscal;
   Batch bl; bl.n = nrhs; bl.rs = rs_lo; bl.ss = SS; bl.act = c->mact;
+  Batch bo = bl; bo.rs = rs_op;
   Batch bh; bh.n = nrhs; bh.rs = rs_hi; bh.ss = SS;
 
   QXD_CUDA_OK(c, cudaEventRecord(c->ev0, c->stream));
@@ -344,6 +352,7 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
   QXD_TRY(blas_zero(c, plo, xlo, bl));
   QXD_TRY(blas_norm2(c, 0, B, ms + M_RRT, bh));
   QXD_TRY(launch_convert_spinor(c, 0, B, plo, rlo, nrhs, rs_hi, rs_lo));
+  if (h16) QXD_TRY(launch_convert_spinor(c, 0, B, pop, r16, nrhs, rs_hi, rs_op));
   QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
   QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
   int nactive = 0;
@@ -363,20 +372,23 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
     QXD_TRY(apply_dhat(c, 0, xk, thi, tmp_o_hi, 0, nullptr));
     QXD_TRY(blas_sub_norm(c, 0, rhs_view(B, rs_hi, k), thi, rhi, c->scal + SC_RRT));
     QXD_TRY(launch_convert_spinor(c, 0, rhi, plo, rhs_view(rlo, rs_lo, k)));
+    if (h16) QXD_TRY(launch_convert_spinor(c, 0, rhi, pop, rhs_view(r16, rs_op, k)));
     QXD_TRY(read_scal(c, SC_RRT, 1, &rr_true[k]));
     nrel[k]++;
     return QXD_OK;
   };
   int it = 0;
   if (nactive) {
-    QXD_TRY(apply_dhat(c, plo, rlo, t, tmp_o, 1, ms + M_GAM0, bl));   // s = A^dag r (s shares the buffer of t)
-    QXD_TRY(blas_copy(c, plo, t, p, bl));
+    QXD_TRY(apply_dhat(c, pop, rin, t, tmp_o, 1, ms + M_GAM0, bo));   // s = A^dag r (s shares the buffer of t)
+    QXD_TRY(launch_convert_spinor(c, pop, t, plo, p, nrhs, rs_op, rs_lo));
+    if (h16) QXD_TRY(blas_copy(c, pop, t, p16, bo));
   }
   while (nactive && it < maxiter) {
     double* gam = ms + M_GAM0 + (it & 1);
     double* gam_next = ms + M_GAM0 + ((it + 1) & 1);
-    QXD_TRY(apply_dhat(c, plo, p, t, tmp_o, 0, ms + M_TT, bl));
-    QXD_TRY(blas_cg_xr(c, plo, gam, ms + M_TT, p, t, xlo, rlo, ms + M_RR, bl));
+    QXD_TRY(apply_dhat(c, pop, pin, t, tmp_o, 0, ms + M_TT, bo));
+    if (h16) QXD_TRY(blas_cg_xr_h(c, gam, ms + M_TT, p, t, xlo, rlo, r16, ms + M_RR, bl, rs_op));
+    else QXD_TRY(blas_cg_xr(c, plo, gam, ms + M_TT, p, t, xlo, rlo, ms + M_RR, bl));
     QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
     QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     it++;
@@ -396,8 +408,9 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
     }
     if (changed) QXD_CUDA_OK(c, cudaMemcpyAsync(c->mact, c->h_mact, sizeof(double) * nrhs, cudaMemcpyHostToDevice, c->stream));
     if (!nactive) break;
-    QXD_TRY(apply_dhat(c, plo, rlo, t, tmp_o, 1, gam_next, bl));
-    QXD_TRY(blas_cg_p(c, plo, gam_next, gam, t, p, bl));
+    QXD_TRY(apply_dhat(c, pop, rin, t, tmp_o, 1, gam_next, bo));
+    if (h16) QXD_TRY(blas_cg_p_h(c, gam_next, gam, t, p, p16, bl, rs_op));
+    else QXD_TRY(blas_cg_p(c, plo, gam_next, gam, t, p, bl));
   }
   int status = QXD_OK;
   for (int k = 0; k < nrhs; k++) {
@@ -419,7 +432,7 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
   float ms_el = 0.f;
   QXD_CUDA_OK(c, cudaEventElapsedTime(&ms_el, c->ev0, c->ev1));
   for (int k = 0; k < nrhs; k++) {
-    info[k].algo = info[0].algo; info[k].sloppy = plo; info[k].delta = delta; info[k].maxiter = maxiter;
+    info[k].algo = info[0].algo; info[k].sloppy = pop; info[k].delta = delta; info[k].maxiter = maxiter;
     info[k].iters = iters[k]; info[k].n_reliable = nrel[k];
     info[k].true_res = eta2[k] > 0.0 ? std::sqrt(rr_true[k] / eta2[k]) : 0.0;
     info[k].seconds = ms_el * 1e-3;

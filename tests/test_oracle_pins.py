@@ -309,3 +309,19 @@ def test_range_apply_equals_full_apply():
     lo, hi = 37, 201
     r.clover_build_range(1.5, 1.0, lo, hi)
     assert np.array_equal(r.apply_Dw_range(psi), full[lo:hi])
+
+
+def test_reconstruct_identity_for_u3_links():
+    """Reading R19: for every unitary W (here W = e^{i theta} U with U in SU(3), optionally times -1 for the
+    antiperiodic time boundary) row 2 equals det W * conj(row 0 x row 1), and det W = e^{3 i theta} det U.  This is the
+    identity the 14-real link format of the CUDA path relies on; checked here with numpy only."""
+    U = synth.random_su3(64, 11)
+    rng = np.random.default_rng(5)
+    theta = rng.normal(0.0, 0.7, size=64)
+    sign = np.where(rng.integers(0, 2, size=64) == 1, -1.0, 1.0)
+    W = (sign * np.exp(1j * theta))[:, None, None] * U
+    det = np.linalg.det(W)
+    assert np.allclose(det, sign * np.exp(3j * theta) * np.linalg.det(U), atol=1e-13)
+    assert np.allclose(np.linalg.det(U), 1.0, atol=1e-13)
+    row2 = det[:, None] * np.conj(np.cross(W[:, 0, :], W[:, 1, :]))
+    assert np.max(np.abs(row2 - W[:, 2, :])) < 1e-13
