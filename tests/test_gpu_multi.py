@@ -121,3 +121,17 @@ def test_full_c4_twelve_rhs_batched_dslash_and_solve():
         r = c.ref.apply_Dw_sites(psi[k], sites) - src[k].reshape(-1, 4, 3)[sites]
         assert np.sqrt(np.mean(np.abs(r) ** 2)) <= 5e-10 * np.sqrt(np.mean(np.abs(src[k]) ** 2))
     c.close()
+
+
+def test_solve_multi_fp16_only_workspace():
+    """Only fp64 and binary16 bound: the batch workspace has no room for fp32 Krylov vectors, so the batched solver runs
+    with binary16 vectors throughout (more iterations, same acceptance on the fp64 true residual)."""
+    dims = (8, 4, 4, 8)
+    c = Case(dims, 3, 1, True, q=-1 / 3, kappa=0.125, csw=1.5, csw_qed=1.0, eps=0.2, precisions=(F64, F16), nrhs=3)
+    etas = np.stack([synth.gaussian_spinor(c.dims_ext, 61 + k) for k in range(3)])
+    psi, infos = c.gpu.solve_multi(etas, 1e-10, sloppy=F16, delta=0.1)
+    psi = to_np(psi).reshape(etas.shape)
+    for k in range(3):
+        assert infos[k]["status"] == 0, infos[k]
+        assert true_residual(c.ref, etas[k], psi[k]) <= 1.05e-10
+    c.close()
