@@ -374,7 +374,7 @@ def run_cuda(args, cfg):
                          "traffic": NCU_TRAFFIC_BYTES_FP32_C3, "peak_source": peak_src, "frac_of_nominal_8000": per_gpu_gbs / 8000.0,
                          "kernel": "dslash_k<float, DW_FULL>", "algorithmic_bytes_per_launch": dw_bytes_per_site(hp) * V},
             "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes, "ms_per_step": e2e_s * 1e3,
-                    "call": "qxd_apply_Dw_host (pinned host fp64 in/out)"},
+                    "call": "qxd_apply_Dw_host (pinned host fp64 in/out, pipelined over time slabs)"},
             "gpu_launches": launches,
             "clocks": clocks,
             "cpu_baseline": cpu_baseline,

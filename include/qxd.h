@@ -145,7 +145,9 @@ int qxd_clover_export(qxd_ctx* ctx, double* out, int inverse);
 int qxd_apply_Dw(qxd_ctx* ctx, int prec, const double* psi, double* out);
 /* D-hat = A_ee - D_eo A_oo^{-1} D_oe on the even sublattice; dagger != 0 applies D-hat^dagger. */
 int qxd_apply_Dhat_eo(qxd_ctx* ctx, int prec, const double* psi_e, double* out_e, int dagger);
-/* Same as qxd_apply_Dw but psi/out are HOST arrays: H2D copy, pack, apply, unpack, D2H copy. */
+/* Same as qxd_apply_Dw but psi/out are HOST arrays (pinned memory for full speed; the paper's boundary).
+ * The lattice is processed in time slabs of one tile thickness: copy-in, pack, apply, unpack and copy-out of different
+ * slabs overlap on three streams, so the two PCIe directions run at the same time.  Synchronises before returning. */
 int qxd_apply_Dw_host(qxd_ctx* ctx, int prec, const double* psi_host, double* out_host);
 
 /* ---- solver (rows a7, a8) --------------------------------------------------------

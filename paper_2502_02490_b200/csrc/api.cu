@@ -3,6 +3,7 @@
 #include "qxd_ctx.h"
 #include <new>
 #include <cstring>
+#include <vector>
 
 using namespace qxd;
 
@@ -130,6 +131,9 @@ int qxd_geometry_destroy(qxd_ctx* c) {
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);
   if (c->ev_scal) cudaEventDestroy(c->ev_scal);
+  for (int io = 0; io < 2; io++) for (int k = 0; k < 64; k++) if (c->ev_slab[io][k]) cudaEventDestroy(c->ev_slab[io][k]);
+  if (c->s_in) cudaStreamDestroy(c->s_in);
+  if (c->s_out) cudaStreamDestroy(c->s_out);
   delete c;
   return QXD_OK;
 }
@@ -332,13 +336,85 @@ int qxd_apply_Dhat_eo(qxd_ctx* c, int prec, const double* psi_e, double* out_e, 
   return launch_spinor_unpack(c, prec, c->full_b, out_e, 1, 1);
 }
 
+// Time slabs of one tile thickness as tile subsets (TileMap, qxd_common.cuh): inside a block the t digit of the tile index
+// is the slowest one, and the blocks are lexicographic with direction 0 slowest, so slab (bt, mt) is
+// { (bt NBsp + i) mv + mt q + j : i < NBsp, j < q } with mv tiles per block and q = mv / (tiles per block in t).
+static bool time_slabs(const qxd_ctx* c, std::vector<TileMap>& maps, size_t& slab_sites) {
+  const Geom& g = c->g;
+  long tv = 1, mv = 1;
+  for (int mu = 0; mu < 4; mu++) { tv *= c->tile[mu]; mv *= c->block[mu] / c->tile[mu]; }
+  if (tv != 256 || g.Vh % 128) return false;   // the kernels' 128-index tiles must be the geometric tiles
+  const int ntt = c->block[0] / c->tile[0], q = int(mv / ntt), NBsp = g.nB[1] * g.nB[2] * g.nB[3];
+  const int S = g.nB[0] * ntt;
+  if (S < 3 || S > 64) return false;
+  int lq = 0;
+  while ((1 << lq) < q) lq++;
+  maps.clear();
+  for (int bt = 0; bt < g.nB[0]; bt++)
+    for (int mt = 0; mt < ntt; mt++) {
+      TileMap m;
+      m.lq = lq; m.qm = q - 1; m.mv = int(mv); m.base = bt * NBsp * int(mv) + mt * q; m.count = NBsp * q;
+      maps.push_back(m);
+    }
+  slab_sites = size_t(c->tile[0]) * g.X[1] * g.X[2] * g.X[3];
+  return true;
+}
+
+// Host-pointer D_w (the shape of the paper's boundary: host arrays in, host arrays out).  The lattice is cut
+// into time slabs of one tile thickness; slab k is copied in on its own stream, packed as soon as it has arrived, the operator
+// is applied to a slab as soon as its two time neighbours are packed, and its result is unpacked and copied out on a third
+// stream -- so the device->host copy of the first slabs overlaps the host->device copy of the last ones (PCIe is full duplex)
+// and only the copies of about three slabs are exposed.  Orders without such slabs fall back to copy - apply - copy.
 int qxd_apply_Dw_host(qxd_ctx* c, int prec, const double* psi_host, double* out_host) {
   int rc = check_apply(c, prec, psi_host, out_host, "apply_Dw_host");
   if (rc) return rc;
   const size_t bytes = size_t(c->V) * 24 * sizeof(double);
-  QXD_CUDA_OK(c, cudaMemcpyAsync(c->nat_a, psi_host, bytes, cudaMemcpyHostToDevice, c->stream));
-  if ((rc = qxd_apply_Dw(c, prec, c->nat_a, c->nat_b))) return rc;
-  QXD_CUDA_OK(c, cudaMemcpyAsync(out_host, c->nat_b, bytes, cudaMemcpyDeviceToHost, c->stream));
+  std::vector<TileMap> maps;
+  size_t slab_sites = 0;
+  if (!time_slabs(c, maps, slab_sites)) {
+    QXD_CUDA_OK(c, cudaMemcpyAsync(c->nat_a, psi_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    if ((rc = qxd_apply_Dw(c, prec, c->nat_a, c->nat_b))) return rc;
+    QXD_CUDA_OK(c, cudaMemcpyAsync(out_host, c->nat_b, bytes, cudaMemcpyDeviceToHost, c->stream));
+    QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return QXD_OK;
+  }
+  const int S = int(maps.size());
+  if (!c->s_in) QXD_CUDA_OK(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+  if (!c->s_out) QXD_CUDA_OK(c, cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+  for (int k = 0; k < S; k++)
+    for (int io = 0; io < 2; io++)
+      if (!c->ev_slab[io][k]) QXD_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_slab[io][k], cudaEventDisableTiming));
+  // the copy streams start after whatever is queued on the compute stream (it may still read the staging buffers)
+  QXD_CUDA_OK(c, cudaEventRecord(c->ev_scal, c->stream));
+  QXD_CUDA_OK(c, cudaStreamWaitEvent(c->s_in, c->ev_scal, 0));
+  QXD_CUDA_OK(c, cudaStreamWaitEvent(c->s_out, c->ev_scal, 0));
+  const size_t slab_reals = slab_sites * 24, slab_bytes = slab_reals * sizeof(double);
+  for (int k = 0; k < S; k++) {
+    QXD_CUDA_OK(c, cudaMemcpyAsync(c->nat_a + k * slab_reals, psi_host + k * slab_reals, slab_bytes, cudaMemcpyHostToDevice, c->s_in));
+    QXD_CUDA_OK(c, cudaEventRecord(c->ev_slab[0][k], c->s_in));
+  }
+  const int Vh = c->g.Vh;
+  bool packed[64] = {}, applied[64] = {};
+  for (int k = 0; k < S; k++) {
+    QXD_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_slab[0][k], 0));
+    if ((rc = launch_spinor_pack(c, prec, c->nat_a, c->full_a, 3, 0, maps[k]))) return rc;
+    packed[k] = true;
+    for (int j = 0; j < S; j++) {
+      if (applied[j] || !(packed[(j + S - 1) % S] && packed[j] && packed[(j + 1) % S])) continue;
+      DslashCall d{};
+      d.prec = prec; d.mode = DS_DW_FULL; d.flags = 0;
+      d.in[0] = half_view(prec, c->full_a, Vh, 0); d.in[1] = half_view(prec, c->full_a, Vh, 1);
+      d.out[0] = half_view(prec, c->full_b, Vh, 0); d.out[1] = half_view(prec, c->full_b, Vh, 1);
+      d.tm = maps[j];
+      if ((rc = launch_dslash(c, d))) return rc;
+      if ((rc = launch_spinor_unpack(c, prec, c->full_b, c->nat_b, 3, 0, maps[j]))) return rc;
+      QXD_CUDA_OK(c, cudaEventRecord(c->ev_slab[1][j], c->stream));
+      QXD_CUDA_OK(c, cudaStreamWaitEvent(c->s_out, c->ev_slab[1][j], 0));
+      QXD_CUDA_OK(c, cudaMemcpyAsync(out_host + j * slab_reals, c->nat_b + j * slab_reals, slab_bytes, cudaMemcpyDeviceToHost, c->s_out));
+      applied[j] = true;
+    }
+  }
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->s_out));
   QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
   return QXD_OK;
 }

@@ -60,6 +60,7 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.parity_out = d.parity_out;
   a.nrhs = d.nrhs > 1 ? d.nrhs : 1; a.ngroups = 1;
   a.rs_in = d.rs_in; a.rs_phi = d.rs_phi; a.rs_out = d.rs_out;
+  a.tm = d.tm;
   if (a.nrhs > 64) return fail(c, QXD_EINVAL, "dslash: at most 64 right-hand sides per launch");
   a.R.partials = c->partials; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
   int rc;

@@ -16,6 +16,7 @@ struct DslashArgs {
   int ngroups;         // ceil(nrhs / R): consecutive CTAs work on the same tile for different groups of R right-hand sides
   size_t rs_in, rs_phi, rs_out;   // byte distance between consecutive right-hand sides
   Reducer R;
+  TileMap tm;          // subset of tiles this launch works on (identity unless count > 0)
 };
 
 

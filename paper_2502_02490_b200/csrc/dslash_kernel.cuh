@@ -277,7 +277,7 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
   // blocks of a tile run at the same time, so a batch reads them from DRAM once and from L2 afterwards
   const int bt = blockIdx.x / a.ngroups;
   const int rhs0 = (blockIdx.x - bt * a.ngroups) * R;
-  const int tile = SPLIT ? (bt >> 1) : bt;
+  const int tile = tile_of(a.tm, SPLIT ? (bt >> 1) : bt);
   const int cb = tile * 128 + (threadIdx.x & 127);
   const int parity = FULL ? (SPLIT ? (bt & 1) : (threadIdx.x >> 7)) : a.parity_out;
   double nrm[R];
@@ -352,7 +352,8 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
 void launch_r(qxd_ctx* c, DslashArgs& a) {
   a.ngroups = (a.nrhs + R - 1) / R;
-  dim3 gr(unsigned((c->g.Vh + 127) / 128) * unsigned(a.ngroups) * (KernelShape<S, R, FULL, NL>::SPLIT ? 2u : 1u));
+  const unsigned ntiles = a.tm.count > 0 ? unsigned(a.tm.count) : unsigned((c->g.Vh + 127) / 128);
+  dim3 gr(ntiles * unsigned(a.ngroups) * (KernelShape<S, R, FULL, NL>::SPLIT ? 2u : 1u));
   dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL><<<gr, KernelShape<S, R, FULL, NL>::THREADS, 0, c->stream>>>(a);
 }
 // right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 1:

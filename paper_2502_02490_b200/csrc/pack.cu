@@ -88,9 +88,9 @@ __global__ void __launch_bounds__(128) hoplinks_k(Geom g, double q, int use_a, c
 // ---- spinors: natural AoS fp64 <-> packed SoA in precision S
 template <typename S>
 __global__ void __launch_bounds__(128) spinor_pack_k(Geom g, const double* __restrict__ nat, SpinorPtr p0, SpinorPtr p1, int pmask,
-                                                     int compact_even) {
+                                                     int compact_even, TileMap tm) {
   typedef typename PT<S>::C C;
-  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  int cb = tile_of(tm, blockIdx.x) * 128 + threadIdx.x;
   int parity = blockIdx.y;
   if (cb >= g.Vh || !((pmask >> parity) & 1)) return;
   int x[4];
@@ -105,9 +105,9 @@ __global__ void __launch_bounds__(128) spinor_pack_k(Geom g, const double* __res
 }
 template <typename S>
 __global__ void __launch_bounds__(128) spinor_unpack_k(Geom g, SpinorPtr p0, SpinorPtr p1, double* __restrict__ nat, int pmask,
-                                                       int compact_even) {
+                                                       int compact_even, TileMap tm) {
   typedef typename PT<S>::C C;
-  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  int cb = tile_of(tm, blockIdx.x) * 128 + threadIdx.x;
   int parity = blockIdx.y;
   if (cb >= g.Vh || !((pmask >> parity) & 1)) return;
   int x[4];
@@ -178,21 +178,21 @@ int launch_hoplinks(qxd_ctx* c, int prec) {
   return QXD_OK;
 }
 
-int launch_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed, int pmask, int compact_even) {
-  dim3 gr = grid_for(c->g.Vh, 2);
+int launch_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed, int pmask, int compact_even, const TileMap& tm) {
+  dim3 gr = tm.count > 0 ? dim3(tm.count, 2) : grid_for(c->g.Vh, 2);
   SpinorPtr p0 = half_view(prec, packed, c->g.Vh, 0), p1 = half_view(prec, packed, c->g.Vh, 1);
-  if (prec == 0) spinor_pack_k<double><<<gr, 128, 0, c->stream>>>(c->g, nat, p0, p1, pmask, compact_even);
-  else if (prec == 1) spinor_pack_k<float><<<gr, 128, 0, c->stream>>>(c->g, nat, p0, p1, pmask, compact_even);
-  else spinor_pack_k<__half><<<gr, 128, 0, c->stream>>>(c->g, nat, p0, p1, pmask, compact_even);
+  if (prec == 0) spinor_pack_k<double><<<gr, 128, 0, c->stream>>>(c->g, nat, p0, p1, pmask, compact_even, tm);
+  else if (prec == 1) spinor_pack_k<float><<<gr, 128, 0, c->stream>>>(c->g, nat, p0, p1, pmask, compact_even, tm);
+  else spinor_pack_k<__half><<<gr, 128, 0, c->stream>>>(c->g, nat, p0, p1, pmask, compact_even, tm);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, int pmask, int compact_even) {
-  dim3 gr = grid_for(c->g.Vh, 2);
+int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, int pmask, int compact_even, const TileMap& tm) {
+  dim3 gr = tm.count > 0 ? dim3(tm.count, 2) : grid_for(c->g.Vh, 2);
   SpinorPtr p0 = half_view(prec, const_cast<void*>(packed), c->g.Vh, 0), p1 = half_view(prec, const_cast<void*>(packed), c->g.Vh, 1);
-  if (prec == 0) spinor_unpack_k<double><<<gr, 128, 0, c->stream>>>(c->g, p0, p1, nat, pmask, compact_even);
-  else if (prec == 1) spinor_unpack_k<float><<<gr, 128, 0, c->stream>>>(c->g, p0, p1, nat, pmask, compact_even);
-  else spinor_unpack_k<__half><<<gr, 128, 0, c->stream>>>(c->g, p0, p1, nat, pmask, compact_even);
+  if (prec == 0) spinor_unpack_k<double><<<gr, 128, 0, c->stream>>>(c->g, p0, p1, nat, pmask, compact_even, tm);
+  else if (prec == 1) spinor_unpack_k<float><<<gr, 128, 0, c->stream>>>(c->g, p0, p1, nat, pmask, compact_even, tm);
+  else spinor_unpack_k<__half><<<gr, 128, 0, c->stream>>>(c->g, p0, p1, nat, pmask, compact_even, tm);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

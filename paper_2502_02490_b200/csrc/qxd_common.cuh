@@ -66,6 +66,14 @@ __host__ __device__ __forceinline__ long lex_of(const Geom& g, const int x[4]) {
   return ((long(x[0]) * g.X[1] + x[1]) * g.X[2] + x[2]) * g.X[3] + x[3];
 }
 
+// A subset of the tiles (128 checkerboard indices each) in launch order: tile(k) = base + (k >> lq) * mv + (k & qm), k < count.
+// The identity map (count == 0) is the whole lattice.  A time slab of one tile thickness is such a subset for every site
+// order (the t digit is the slowest one inside a block and over the blocks); qxd_apply_Dw_host pipelines over these slabs.
+struct TileMap {
+  int lq = 0, qm = 0, mv = 1, base = 0, count = 0;
+};
+__host__ __device__ __forceinline__ int tile_of(const TileMap& m, int k) { return m.base + (k >> m.lq) * m.mv + (k & m.qm); }
+
 // Per-thread site context: coordinates and their index contributions (separable index).
 struct Site {
   int x[4];

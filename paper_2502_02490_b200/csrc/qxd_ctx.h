@@ -71,6 +71,8 @@ struct qxd_ctx {
   long launches = 0;
   std::string err;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of the pipelined host-pointer apply (created on first use)
+  cudaEvent_t ev_slab[2][64] = {};               // [in/out][slab]
   cudaEvent_t ev_scal = nullptr;                 // marks the device->host copy of solver scalars (solver.cu: post_scal / wait_scal)
 };
 
@@ -104,8 +106,10 @@ inline size_t half_bytes(int prec, int Vh) {
 // pack.cu
 int launch_gauge_pack(qxd_ctx* c, const double* U, const double* A);
 int launch_hoplinks(qxd_ctx* c, int prec);
-int launch_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed, int parity_mask /*1 even,2 odd,3 both*/, int compact_even);
-int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, int parity_mask, int compact_even);
+int launch_spinor_pack(qxd_ctx* c, int prec, const double* nat, void* packed, int parity_mask /*1 even,2 odd,3 both*/, int compact_even,
+                       const TileMap& tm = TileMap());
+int launch_spinor_unpack(qxd_ctx* c, int prec, const void* packed, double* nat, int parity_mask, int compact_even,
+                         const TileMap& tm = TileMap());
 int launch_convert_spinor(qxd_ctx* c, int prec_from, const SpinorPtr& from, int prec_to, const SpinorPtr& to, int n = 1, size_t rs_from = 0,
                           size_t rs_to = 0);
 int launch_convert_record72(qxd_ctx* c, const void* from64, int prec_to, void* to);
@@ -126,6 +130,7 @@ struct DslashCall {
   int nrhs;
   size_t rs_in, rs_phi, rs_out;
   int norm_stride;
+  TileMap tm;       // launch on a subset of the tiles (time slab); default: whole lattice
 };
 int launch_dslash(qxd_ctx* c, const DslashCall& d);
 int launch_clover_apply(qxd_ctx* c, int prec, int inverse, int parity, const SpinorPtr& in, const SpinorPtr& out);
