@@ -408,3 +408,17 @@ def test_apply_Dw_host_pipelined_equals_device_apply(dims, cstar, prec):
         assert np.array_equal(oh.numpy().reshape(dev.shape), dev)
     assert relerr(oh.numpy().reshape(psi.shape), c.ref.apply_Dw(psi)) < TOL[prec]
     c.close()
+
+
+@pytest.mark.parametrize("sloppy", [F32, F16])
+def test_solve_config_c2_full_size(sloppy):
+    """BASELINE config 2 at its full size (32x16^3 QCD+QED C*, 262144 extended sites, eps 0.15, csw 1.7): mixed-precision
+    even-odd CG with reliable updates to 1e-10; the true residual is recomputed with the oracle's D on the whole lattice."""
+    cfg = synth.config("c2")
+    c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32, F16))
+    eta = synth.gaussian_spinor(c.dims_ext, 3)
+    psi, info = c.gpu.solve(eta, cfg["tol"], algo=0, sloppy=sloppy, delta=0.1)
+    assert info["status"] == 0 and info["n_reliable"] >= 1, info
+    assert true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05 * cfg["tol"]
+    c.close()
