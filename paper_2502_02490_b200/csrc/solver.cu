@@ -172,6 +172,10 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
   if (rr <= stop2) status = QXD_OK;
   cplx rho = {rr, 0.0};
   const double tiny = 1e-290;
+  // stagnation guard: BiCGstab on D-hat can stall near / beyond the critical kappa (it did at config c4); if the iterated
+  // residual has not improved on its best value for 500 iterations the solve is reported as not converged (R11)
+  double best_rr = rr;
+  int since_best = 0;
   while (status != QXD_OK && it < maxiter) {
     QXD_TRY(apply_dhat(c, plo, w.p, w.v, w.tmp_o_lo, 0, nullptr));                 // v = A p
     QXD_TRY(blas_cdot(c, plo, w.r0, w.v, c->scal + SC_DOT));
@@ -202,6 +206,7 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
     cplx rho_new = {d3[0], d3[1]};
     rr = d3[2];
     if (!(rr == rr)) break;
+    if (rr < best_rr) { best_rr = rr; since_best = 0; } else if (++since_best >= 500) break;
     double rn = std::sqrt(rr);
     if (rn > maxr) maxr = rn;
     bool updated = false;
