@@ -19,7 +19,7 @@ enum { SC_GAM0 = 0, SC_GAM1 = 1, SC_TT = 2, SC_RR = 3, SC_RRT = 4, SC_NE = 5, SC
 
 struct Ws {
   int Vh;
-  SpinorPtr eta_e, eta_o, b, xhi, rhi, thi, tmp_o_hi, out_e, out_o;
+  SpinorPtr eta_e, eta_o, b, xhi, rhi, thi, tmp_o_hi, out_e, out_o, xbest;
   SpinorPtr xlo, rlo, p, t, s, tmp_o_lo, v, r0;
 };
 
@@ -176,6 +176,10 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
   // residual has not improved on its best value for 500 iterations the solve is reported as not converged (R11)
   double best_rr = rr;
   int since_best = 0;
+  // BiCGstab's residual is not monotonic: keep the fp64 iterate with the smallest TRUE residual seen at a reliable update
+  // (x = 0 to begin with), so that a solve that fails still returns its best iterate (include/qxd.h, QXD_ENOCONV)
+  double best_true = rr;
+  QXD_TRY(blas_zero(c, 0, w.xbest));
   while (status != QXD_OK && it < maxiter) {
     QXD_TRY(apply_dhat(c, plo, w.p, w.v, w.tmp_o_lo, 0, nullptr));                 // v = A p
     QXD_TRY(blas_cdot(c, plo, w.r0, w.v, c->scal + SC_DOT));
@@ -213,6 +217,7 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
     if (rn < delta * maxr || rr <= stop2) {
       QXD_TRY(reliable_update(c, plo, w, &rr_true));
       nrel++; updated = true;
+      if (rr_true < best_true) { best_true = rr_true; QXD_TRY(blas_copy(c, 0, w.xhi, w.xbest)); }
       maxr = std::sqrt(rr_true);
       if (rr_true <= stop2) { status = QXD_OK; break; }
     }
@@ -231,6 +236,7 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
     QXD_TRY(reliable_update(c, plo, w, &rr_true));
     nrel++;
     if (rr_true <= stop2) status = QXD_OK;
+    else if (rr_true > best_true) { QXD_TRY(blas_copy(c, 0, w.xbest, w.xhi)); rr_true = best_true; }
   }
   info->iters = it; info->n_reliable = nrel; info->true_res = rr_true;
   return status;
@@ -250,7 +256,7 @@ int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd
   w.eta_e = half_view(0, c->full_a, Vh, 0); w.eta_o = half_view(0, c->full_a, Vh, 1);
   w.out_e = half_view(0, c->full_b, Vh, 0); w.out_o = half_view(0, c->full_b, Vh, 1);
   w.b = hv(0, c->sp64[0], Vh); w.xhi = hv(0, c->sp64[1], Vh); w.rhi = hv(0, c->sp64[2], Vh); w.thi = hv(0, c->sp64[3], Vh);
-  w.tmp_o_hi = hv(0, c->sp64[4], Vh);
+  w.tmp_o_hi = hv(0, c->sp64[4], Vh); w.xbest = hv(0, c->sp64[5], Vh);
   w.xlo = hv(plo, c->splo[0], Vh); w.rlo = hv(plo, c->splo[1], Vh); w.p = hv(plo, c->splo[2], Vh); w.t = hv(plo, c->splo[3], Vh);
   w.s = hv(plo, c->splo[4], Vh); w.tmp_o_lo = hv(plo, c->splo[5], Vh); w.v = hv(plo, c->splo[6], Vh); w.r0 = hv(plo, c->splo[7], Vh);
 

@@ -272,14 +272,28 @@ def test_solve_host_pointers_and_zero_source():
     c.close()
 
 
-def test_maxiter_reports_noconv_with_best_iterate():
+@pytest.mark.parametrize("algo", [0, 1])
+def test_maxiter_reports_noconv_with_best_iterate(algo):
     c = Case((4, 4, 4, 4), 0, 1, False, precisions=(F64,))
     eta = synth.gaussian_spinor(c.dims_ext, 3)
-    psi, info = c.gpu.solve(eta, 1e-12, maxiter=3)
+    psi, info = c.gpu.solve(eta, 1e-12, algo=algo, maxiter=3)
     assert info["status"] == c.B.QXD_ENOCONV and info["iters"] == 3
     res = true_residual(c.ref, eta, to_np(psi).reshape(eta.shape))
-    assert 1e-12 < res < 1.0
+    assert 1e-12 < res <= 1.0          # never worse than the zero vector (BiCGstab returns its best iterate)
     assert abs(info["true_res"] - res) < 1e-10
+    c.close()
+
+
+def test_bicgstab_supercritical_returns_best_iterate():
+    """Beyond the critical kappa BiCGstab on D-hat stalls or diverges: the call must end with QXD_ENOCONV (stagnation guard or
+    maxiter), and the psi it returns must be the iterate with the smallest true residual it saw, reported truthfully."""
+    c = Case((8, 4, 4, 4), 0, 1, False, kappa=0.20, csw=1.7, eps=0.3, precisions=(F64, F32))
+    eta = synth.gaussian_spinor(c.dims_ext, 3)
+    psi, info = c.gpu.solve(eta, 1e-10, algo=1, sloppy=F32, maxiter=1500)
+    res = true_residual(c.ref, eta, to_np(psi).reshape(eta.shape))
+    assert abs(info["true_res"] - res) <= 1e-9 * max(1.0, res)
+    if info["status"] != 0:
+        assert info["status"] == c.B.QXD_ENOCONV and res <= 1.0 + 1e-12
     c.close()
 
 
