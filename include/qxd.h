@@ -19,6 +19,7 @@
  *    caller provides one workspace (qxd_workspace_bytes / qxd_workspace_bind).
  *  - Calls enqueue work on the bound CUDA stream (qxd_set_stream; default stream 0).  Only
  *    qxd_solve*, the *_host variants and the qxd_blas_* reductions synchronise that stream.
+ *  - A context is not thread-safe: use it from one host thread at a time (different contexts are independent).
  *  - Natural ("application") order, used by every non-packed entry point:
  *      site index  Lambda(x) = L3 L2 X1 x0 + L3 L2 x1 + L3 x2 + x3        (Eq. (1))
  *      with x = (t,x,y,z) and X1 = 2*L1 if C* is on (extended lattice) else L1;
