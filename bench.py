@@ -319,7 +319,7 @@ def run_cuda(args, cfg):
         g.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=B.QXD_F16)
         psi_d = torch.empty_like(eta_d)
         for name, algo, sl in (("cgne_fp64_fp16", B.QXD_CGNE, B.QXD_F16), ("cgne_fp64_fp32", B.QXD_CGNE, B.QXD_F32),
-                               ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32)):
+                               ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32), ("bicgstab_fp64_fp16", B.QXD_BICGSTAB, B.QXD_F16)):
             l0 = g.launch_count()
             _, info = g.solve(eta_d, cfg["tol"], algo=algo, sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psi_d)
             info["launches"] = g.launch_count() - l0

@@ -52,6 +52,46 @@ __global__ void __launch_bounds__(128) cxpaypbw_k(int Vh, SpinorPtr x, double ar
   store_spinor<S>(z, Vh, cb, vx);
 }
 
+// BiCGstab, end of an iteration in one pass:  x += alpha p + omega s ;  r = s - omega t ;  result = (<r0,r>, |r|^2)
+template <typename S>
+__global__ void __launch_bounds__(128) bicg_xr_k(int Vh, double ar_, double ai_, double wr_, double wi_, SpinorPtr p, SpinorPtr s, SpinorPtr t,
+                                                 SpinorPtr r0, SpinorPtr x, SpinorPtr r, Reducer R) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  double d[3] = {0.0, 0.0, 0.0};
+  if (cb < Vh) {
+    const C ar = (C)ar_, ai = (C)ai_, wr = (C)wr_, wi = (C)wi_;
+    C vx[24], va[24], vs[24];
+    load_spinor<S>(x, Vh, cb, vx);
+    load_spinor<S>(p, Vh, cb, va);
+    load_spinor<S>(s, Vh, cb, vs);
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      vx[2 * k] += ar * va[2 * k] - ai * va[2 * k + 1] + wr * vs[2 * k] - wi * vs[2 * k + 1];
+      vx[2 * k + 1] += ar * va[2 * k + 1] + ai * va[2 * k] + wr * vs[2 * k + 1] + wi * vs[2 * k];
+    }
+    store_spinor<S>(x, Vh, cb, vx);
+    load_spinor<S>(t, Vh, cb, va);
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      vs[2 * k] -= wr * va[2 * k] - wi * va[2 * k + 1];
+      vs[2 * k + 1] -= wr * va[2 * k + 1] + wi * va[2 * k];
+    }
+    load_spinor<S>(r0, Vh, cb, va);
+    C p0 = 0, p1 = 0, p2 = 0;
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      const C xr = va[2 * k], xi = va[2 * k + 1], yr = vs[2 * k], yi = vs[2 * k + 1];
+      p0 += xr * yr; p0 += xi * yi;
+      p1 += xr * yi; p1 -= xi * yr;
+      p2 += yr * yr; p2 += yi * yi;
+    }
+    d[0] = (double)p0; d[1] = (double)p1; d[2] = (double)p2;
+    store_spinor<S>(r, Vh, cb, vs);
+  }
+  grid_reduce<3>(d, R);
+}
+
 // CG on the normal equations, step 1:  alpha = num/den ;  x += alpha p ;  r -= alpha t ;  result = |r|^2
 // Batched form (row a10): blockIdx.y = right-hand side; vectors rs bytes apart, scalars ss doubles apart; act (may be null)
 // holds 1.0 / 0.0 per right-hand side: a converged system is frozen (alpha = beta = 0).
@@ -282,6 +322,13 @@ int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai
                   const SpinorPtr& w, const SpinorPtr& z) {
   if (br == 0.0 && bi == 0.0) QXD_BY_PREC(prec, cxpaypbw_k<S, false><<<QXD_GRID>>>(c->g.Vh, x, ar, ai, y, br, bi, w, z));
   else QXD_BY_PREC(prec, cxpaypbw_k<S, true><<<QXD_GRID>>>(c->g.Vh, x, ar, ai, y, br, bi, w, z));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_bicg_xr(qxd_ctx* c, int prec, double ar, double ai, double wr, double wi, const SpinorPtr& p, const SpinorPtr& s,
+                 const SpinorPtr& t, const SpinorPtr& r0, const SpinorPtr& x, const SpinorPtr& r, double* res3) {
+  QXD_BY_PREC(prec, bicg_xr_k<S><<<QXD_GRID>>>(c->g.Vh, ar, ai, wr, wi, p, s, t, r0, x, r, reducer(c, res3)));
+  QXD_FINALIZE(3, res3, 0, 1);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

@@ -189,12 +189,11 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
     cplx alpha = cdiv(rho, r0v);
     QXD_TRY(blas_cxpaypbw(c, plo, w.rlo, -alpha.re, -alpha.im, w.v, 0, 0, w.v, w.s));   // s = r - alpha v
     QXD_TRY(apply_dhat(c, plo, w.s, w.t, w.tmp_o_lo, 0, nullptr));                 // t = A s
-    QXD_TRY(blas_cdot(c, plo, w.t, w.s, c->scal + SC_DOT));                         // <t,s>, |s|^2
-    QXD_TRY(blas_norm2(c, plo, w.t, c->scal + SC_DOT2));
-    double d5[5];
-    QXD_TRY(read_scal(c, SC_DOT, 5, d5));  // slots SC_DOT..SC_DOT2
-    cplx ts = {d5[0], d5[1]};
-    double tt = d5[SC_DOT2 - SC_DOT];
+    QXD_TRY(blas_cdot(c, plo, w.s, w.t, c->scal + SC_DOT));                         // <s,t> = conj <t,s>, |t|^2 in one pass
+    double d5[3];
+    QXD_TRY(read_scal(c, SC_DOT, 3, d5));
+    cplx ts = {d5[0], -d5[1]};
+    double tt = d5[2];
     if (!(tt > tiny)) {  // t = 0: s is already the exact residual update
       QXD_TRY(blas_cxpaypbw(c, plo, w.xlo, alpha.re, alpha.im, w.p, 0, 0, w.p, w.xlo));
       QXD_TRY(blas_copy(c, plo, w.s, w.rlo));
@@ -202,9 +201,8 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
       break;
     }
     cplx omega = {ts.re / tt, ts.im / tt};
-    QXD_TRY(blas_cxpaypbw(c, plo, w.xlo, alpha.re, alpha.im, w.p, omega.re, omega.im, w.s, w.xlo));  // x += alpha p + omega s
-    QXD_TRY(blas_cxpaypbw(c, plo, w.s, -omega.re, -omega.im, w.t, 0, 0, w.t, w.rlo));                // r = s - omega t
-    QXD_TRY(blas_cdot(c, plo, w.r0, w.rlo, c->scal + SC_DOT));                                       // rho' , |r|^2
+    // x += alpha p + omega s ; r = s - omega t ; rho' = <r0,r>, |r|^2 -- one kernel
+    QXD_TRY(blas_bicg_xr(c, plo, alpha.re, alpha.im, omega.re, omega.im, w.p, w.s, w.t, w.r0, w.xlo, w.rlo, c->scal + SC_DOT));
     QXD_TRY(read_scal(c, SC_DOT, 3, d3));
     it++;
     cplx rho_new = {d3[0], d3[1]};
