@@ -310,6 +310,65 @@ def run_cuda(args, cfg):
                                    "Gflops": FLOP_PER_SITE * V * n / ms / 1e6, "speedup_vs_single": sweep[PREC_NAME[p]]["Dw_ms"] * n / ms}
             del pin, pout
 
+    # ---- end to end through the host-pointer C-ABI call (H2D + pack + apply + unpack + D2H every step) ------
+    eh = torch.from_numpy(eta).pin_memory()
+    oh = torch.empty_like(eh).pin_memory()
+    n_e2e = 0 if args.no_e2e else 3
+    g.apply_Dw_host(eh, oh, hp)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        g.apply_Dw_host(eh, oh, hp)
+    torch.cuda.synchronize(dev)
+    barrier()
+    e2e_s = max_over_ranks((time.perf_counter() - t0) / max(n_e2e, 1))
+    e2e_val = None if args.no_e2e else world * V * dw_bytes_per_site(hp) / e2e_s / 1e9
+    io_bytes = V * 24 * 8
+
+    # ---- C*-paired device layout (qxd_set_cstar_pairing): links and clover once per physical site, a site and its mirror
+    # image in neighbouring threads.  A different scheme with fewer algorithmic bytes (D_w 120 / 112 reals per site instead
+    # of 192 / 176; D-hat 168 / 152 per full-lattice site instead of 276 / 244), reported beside the headline scheme and
+    # used for the solves below.
+    pairing = cfg["cstar"] > 0 and not args.no_pairing
+    if pairing:
+        g.close()
+        del packed
+        torch.cuda.empty_cache()
+        g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=max(1, args.nrhs), device=f"cuda:{local}", pairing=True)
+        Ud = torch.from_numpy(U).to(dev)
+        Ad = torch.from_numpy(A).to(dev) if A is not None else None
+        g.gauge_load(Ud, Ad, cfg["qel"])
+        g.set_quark(cfg["kappa"], cfg["q"])
+        ep0, ep1 = ev(), ev()
+        ep0.record()
+        g.clover_build(cfg["csw"], cfg["csw_qed"])
+        ep1.record()
+        torch.cuda.synchronize(dev)
+        setup_ms["clover_build_invert_paired"] = ep0.elapsed_time(ep1)
+        del Ud, Ad
+        for nl, tag in ((18, "_paired"), (14, "_paired_recon12")):
+            if args.no_sweep:
+                break
+            g.set_gauge_reconstruct(B.QXD_RECON_12 if nl == 14 else B.QXD_RECON_NONE)
+            for p in precs:
+                a, b = g.spinor_pack(eta_d, p), g.new_packed(p)
+                for _ in range(3):
+                    g.apply_Dw_packed(a, b, p)
+                ms = timed(lambda: g.apply_Dw_packed(a, b, p), nrep)
+                hb = g.packed_spinor_bytes(p, half_only=True)
+                for _ in range(3):
+                    g.apply_Dhat_packed(a[:hb], b[:hb], p)
+                ms_hat = timed(lambda: g.apply_Dhat_packed(a[:hb], b[:hb], p), nrep)
+                reals_dw = 48 + (4 * nl + 72) / 2.0                     # psi + out + half of (links + clover)
+                reals_hat = (120 + (8 * nl + 72 + 8 * nl + 72) / 2.0) / 2.0   # per FULL-lattice site: 5 spinor streams + half the gauge data
+                bytes_dw = reals_dw * PREC_BYTES[p] * V + (8 * V if p == 2 else 0)
+                bytes_hat = reals_hat * PREC_BYTES[p] * V + (16 * V // 2 if p == 2 else 0)
+                sweep[PREC_NAME[p] + tag] = {"link_reals": nl, "layout": "C*-paired", "Dw_ms": ms, "Dw_GBps": bytes_dw / ms / 1e6,
+                                             "Dw_Gflops": FLOP_PER_SITE * V / ms / 1e6, "Dw_frac_of_peak": bytes_dw / ms / 1e6 / peak,
+                                             "Dhat_ms": ms_hat, "Dhat_GBps": bytes_hat / ms_hat / 1e6, "Dhat_Gflops": FLOP_PER_SITE * V / ms_hat / 1e6}
+                del a, b
+        g.set_gauge_reconstruct(B.QXD_RECON_NONE)
+
     # ---- solves (rows a7, a8): fp64/fp16 and fp64/fp32 mixed CGNE, BiCGstab ------------------------------
     solves = {}
     if not args.no_solve:
@@ -325,6 +384,7 @@ def run_cuda(args, cfg):
             info["launches"] = g.launch_count() - l0
             info["tol"] = cfg["tol"]
             info["links"] = "fp64/fp32: recon12, fp16: 18 reals"
+            info["layout"] = "C*-paired" if pairing else "extended lattice"
             solves[name] = info
         if args.nrhs > 1:
             etas = torch.stack([eta_d] + [torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + k)).to(dev) for k in range(1, args.nrhs)])
@@ -340,21 +400,6 @@ def run_cuda(args, cfg):
                     "launches": g.launch_count() - l0, "tol": cfg["tol"], "links": links}
             del etas
         g.set_gauge_reconstruct(B.QXD_RECON_NONE)
-
-    # ---- end to end through the host-pointer C-ABI call (H2D + pack + apply + unpack + D2H every step) ------
-    eh = torch.from_numpy(eta).pin_memory()
-    oh = torch.empty_like(eh).pin_memory()
-    n_e2e = 0 if args.no_e2e else 3
-    g.apply_Dw_host(eh, oh, hp)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(n_e2e):
-        g.apply_Dw_host(eh, oh, hp)
-    torch.cuda.synchronize(dev)
-    barrier()
-    e2e_s = max_over_ranks((time.perf_counter() - t0) / max(n_e2e, 1))
-    e2e_val = None if args.no_e2e else world * V * dw_bytes_per_site(hp) / e2e_s / 1e9
-    io_bytes = V * 24 * 8
 
     # ---- CPU baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----------------------------
     cpu_baseline = None
@@ -399,6 +444,7 @@ def main():
     ap.add_argument("--config", default="c3")
     ap.add_argument("--maxiter", type=int, default=20000)
     ap.add_argument("--nrhs", type=int, default=12, help="right-hand sides of the multi-RHS D_w / batched solve lines (row a10; 1 = skip)")
+    ap.add_argument("--no-pairing", action="store_true", help="keep the extended-lattice layout for the solves (C* configs)")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the precision sweep (short runs under ncu)")

@@ -40,6 +40,7 @@ SYMBOLS = {
     "qxd_geometry_destroy": (_i, [_vp]),
     "qxd_set_tile": (_i, [_vp, _i, _i, _i, _i]),
     "qxd_set_block": (_i, [_vp, _i, _i, _i, _i]),
+    "qxd_set_cstar_pairing": (_i, [_vp, _i]),
     "qxd_volume": (_l, [_vp]),
     "qxd_site_index": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)]),
     "qxd_site_coords": (_i, [_vp, _i, _i, C.POINTER(_i)]),
@@ -102,7 +103,7 @@ def _ptr(t):
 class Qxd:
     """One solver context (qxd_ctx): geometry, workspace, gauge field, quark, clover term."""
 
-    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0"):
+    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=False):
         import torch
         if not torch.cuda.is_available():
             raise QxdError(QXD_ECUDA, "no CUDA device: the qxd hot path has no CPU fallback")
@@ -118,6 +119,8 @@ class Qxd:
         self.cstar = bc & 3
         self.dims_ext = (T, 2 * L1 if self.cstar else L1, L2, L3)
         self.V = self.lib.qxd_volume(self.h)
+        if pairing:
+            self._chk(self.lib.qxd_set_cstar_pairing(self.h, 1))
         if tile is not None:
             self._chk(self.lib.qxd_set_tile(self.h, *tile))
         if block is not None:

@@ -50,13 +50,13 @@ struct Carver {
 
 // One layout routine serves both the size query (base == nullptr) and the binding.
 size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
-  const size_t Vh = c->g.Vh;
+  const size_t Vh = c->g.Vh, Vg = c->g.Vg;
   Carver k(base);
   void* Ug[2]; void* Ag[2]; void* W[NPREC][2] = {}; void* M[NPREC][2] = {}; void* Mi[NPREC][2] = {};
-  for (int p = 0; p < 2; p++) { Ug[p] = k.take(Vh * 72 * 8); Ag[p] = k.take(Vh * 4 * 8); }
+  for (int p = 0; p < 2; p++) { Ug[p] = k.take(Vg * 72 * 8); Ag[p] = k.take(Vg * 4 * 8); }
   for (int pr = 0; pr < NPREC; pr++) {
     if (!((prec_mask >> pr) & 1)) continue;
-    for (int p = 0; p < 2; p++) { W[pr][p] = k.take(Vh * 72 * prec_size(pr)); M[pr][p] = k.take(Vh * 72 * prec_size(pr)); Mi[pr][p] = k.take(Vh * 72 * prec_size(pr)); }
+    for (int p = 0; p < 2; p++) { W[pr][p] = k.take(Vg * 72 * prec_size(pr)); M[pr][p] = k.take(Vg * 72 * prec_size(pr)); Mi[pr][p] = k.take(Vg * 72 * prec_size(pr)); }
   }
   void* sp64[12]; void* splo[8];
   for (int i = 0; i < 12; i++) sp64[i] = k.take(half_bytes(0, Vh));
@@ -116,6 +116,8 @@ int qxd_geometry_create(int T, int L1, int L2, int L3, int bc, qxd_ctx** out) {
   Geom& g = c->g;
   g.X[0] = T; g.X[1] = cstar ? 2 * L1 : L1; g.X[2] = L2; g.X[3] = L3;
   g.L1 = L1; g.cstar = cstar; g.antiper = (bc >> 2) & 1; g.Vh = int(V / 2);
+  for (int mu = 0; mu < 4; mu++) g.XE[mu] = g.X[mu];
+  g.pair = 0; g.Vg = g.Vh;
   // default order: 4x4x4x4 tiles (256 sites = one CTA of the full-lattice kernel), blocks of 4 tiles stacked in time and
   // time slabs 16 thick, so that only 1/8 of the sites have a neighbour in another slab
   int b[4] = {pow2_le_dividing(g.X[0], 4), pow2_le_dividing(g.X[1], 4), pow2_le_dividing(g.X[2], 4), pow2_le_dividing(g.X[3], 4)};
@@ -154,13 +156,31 @@ int qxd_set_block(qxd_ctx* c, int B0, int B1, int B2, int B3) {
   return set_order(c, c->tile, B);
 }
 
+int qxd_set_cstar_pairing(qxd_ctx* c, int on) {
+  if (!c) return QXD_EINVAL;
+  if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_cstar_pairing must precede qxd_workspace_bind");
+  Geom& g = c->g;
+  if (on && g.cstar == 0) return fail(c, QXD_EINVAL, "set_cstar_pairing: the geometry has no C* direction");
+  g.pair = on ? 1 : 0;
+  g.X[1] = g.pair ? g.L1 : g.XE[1];
+  g.Vg = g.pair ? g.Vh / 2 : g.Vh;
+  // default site order on the indexed lattice (as in qxd_geometry_create)
+  int b[4] = {pow2_le_dividing(g.X[0], 4), pow2_le_dividing(g.X[1], 4), pow2_le_dividing(g.X[2], 4), pow2_le_dividing(g.X[3], 4)};
+  int B[4] = {pow2_le_dividing(g.X[0], 16), b[1], b[2], b[3]};
+  return set_order(c, b, B);
+}
+
 long qxd_volume(const qxd_ctx* c) { return c ? c->V : 0; }
 
 int qxd_site_index(const qxd_ctx* c, const int x[4], int* cb, int* parity) {
   if (!c || !x || !cb || !parity) return QXD_EINVAL;
-  for (int mu = 0; mu < 4; mu++) if (x[mu] < 0 || x[mu] >= c->g.X[mu]) return QXD_EINVAL;
-  *cb = idx2_of(c->g, x) >> 1;
+  for (int mu = 0; mu < 4; mu++) if (x[mu] < 0 || x[mu] >= c->g.XE[mu]) return QXD_EINVAL;
   *parity = (x[0] + x[1] + x[2] + x[3]) & 1;
+  if (c->g.pair) {   // (physical site, mirror bit)
+    const int m = x[1] >= c->g.L1 ? 1 : 0;
+    const int xp[4] = {x[0], x[1] - m * c->g.L1, x[2], x[3]};
+    *cb = ((idx2_of(c->g, xp) >> 1) << 1) | m;
+  } else *cb = idx2_of(c->g, x) >> 1;
   return QXD_OK;
 }
 int qxd_site_coords(const qxd_ctx* c, int cb, int parity, int x[4]) {
@@ -343,7 +363,7 @@ static bool time_slabs(const qxd_ctx* c, std::vector<TileMap>& maps, size_t& sla
   const Geom& g = c->g;
   long tv = 1, mv = 1;
   for (int mu = 0; mu < 4; mu++) { tv *= c->tile[mu]; mv *= c->block[mu] / c->tile[mu]; }
-  if (tv != 256 || g.Vh % 128) return false;   // the kernels' 128-index tiles must be the geometric tiles
+  if (tv != 256 || g.Vh % 128 || g.pair) return false;   // the kernels' 128-index tiles must be the geometric tiles
   const int ntt = c->block[0] / c->tile[0], q = int(mv / ntt), NBsp = g.nB[1] * g.nB[2] * g.nB[3];
   const int S = g.nB[0] * ntt;
   if (S < 3 || S > 64) return false;

@@ -62,15 +62,21 @@ __device__ __forceinline__ void m3_adj_mul(const double* a, const double* b, dou
 
 struct GaugePtrs { const void* U[2]; const void* A[2]; };
 
+// links and A of the site s; in the paired layout the records are those of the physical site and the mirror image
+// (s.m = 1) takes U^* and -A (reading R8)
 template <int MU>
 __device__ __forceinline__ void link_at(const GaugePtrs& P, const Geom& g, const Site& s, double* m) {
-  load_reals<double, 18 * MU, 18>(P.U[site_parity(s)], g.Vh, s.idx2 >> 1, m);
+  load_reals<double, 18 * MU, 18>(P.U[site_parity(s)], g.Vg, s.idx2 >> 1, m);
+  if (s.m) {
+#pragma unroll
+    for (int k = 0; k < 9; k++) m[2 * k + 1] = -m[2 * k + 1];
+  }
 }
 template <int MU>
 __device__ __forceinline__ double a_at(const GaugePtrs& P, const Geom& g, const Site& s) {
   double a;
-  load_reals<double, MU, 1>(P.A[site_parity(s)], g.Vh, s.idx2 >> 1, &a);
-  return a;
+  load_reals<double, MU, 1>(P.A[site_parity(s)], g.Vg, s.idx2 >> 1, &a);
+  return s.m ? -a : a;
 }
 template <int MU, int NU>
 __device__ __forceinline__ double phi_at(const GaugePtrs& P, const Geom& g, const Site& y) {
@@ -174,11 +180,11 @@ __device__ __forceinline__ void block_from_C(double diag, const double* C1, cons
 
 __global__ void __launch_bounds__(64) clover_build_k(Geom g, GaugePtrs P, double diag, double csw, double qcq, double qel, int use_a,
                                                      void* M0, void* M1) {
-  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;   // index of the clover record (physical site in the paired layout)
   int parity = blockIdx.y;
-  if (cb >= g.Vh) return;
+  if (cb >= g.Vg) return;
   Site x;
-  site_init(g, cb, parity, x);
+  site_init(g, g.pair ? 2 * cb : cb, parity, x);
   double out[72];
   double Cp[3][18], Cm[3][18];
 #pragma unroll
@@ -195,7 +201,7 @@ __global__ void __launch_bounds__(64) clover_build_k(Geom g, GaugePtrs P, double
   plane_X<1, 2>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, -1.0, -1.0, Cp[2], Cm[2]);   // B_3 = X_12
   block_from_C(diag, Cp[0], Cp[1], Cp[2], out);
   block_from_C(diag, Cm[0], Cm[1], Cm[2], out + 36);
-  store_record<double, 72>(parity ? M1 : M0, g.Vh, cb, out);
+  store_record<double, 72>(parity ? M1 : M0, g.Vg, cb, out);
 }
 
 // Fast path of the block inversion: in-place Gauss-Jordan WITHOUT pivoting, fully unrolled so that the 6x6 complex matrix
@@ -326,14 +332,14 @@ __global__ void __launch_bounds__(64) clover_invert_k(int Vh, const void* M, voi
 int launch_clover_build(qxd_ctx* c) {
   GaugePtrs P;
   P.U[0] = c->Ug[0]; P.U[1] = c->Ug[1]; P.A[0] = c->Ag[0]; P.A[1] = c->Ag[1];
-  dim3 gr((c->g.Vh + 63) / 64, 2);
+  dim3 gr((c->g.Vg + 63) / 64, 2);
   double diag = 4.0 + c->m0;
   clover_build_k<<<gr, 64, 0, c->stream>>>(c->g, P, diag, c->csw, c->q * c->csw_qed, c->qel, c->have_qed ? 1 : 0, c->M[0][0], c->M[0][1]);
   QXD_LAUNCH_CHECK(c);
   int* flag = reinterpret_cast<int*>(c->scal + 60);
   QXD_CUDA_OK(c, cudaMemsetAsync(flag, 0, 2 * sizeof(int), c->stream));
   for (int p = 0; p < 2; p++) {
-    clover_invert_fast_k<<<(2 * c->g.Vh + 127) / 128, 128, 0, c->stream>>>(c->g.Vh, c->M[0][p], c->Mi[0][p], flag);
+    clover_invert_fast_k<<<(2 * c->g.Vg + 127) / 128, 128, 0, c->stream>>>(c->g.Vg, c->M[0][p], c->Mi[0][p], flag);
     QXD_LAUNCH_CHECK(c);
   }
   int hflag[2] = {0, 0};
@@ -341,7 +347,7 @@ int launch_clover_build(qxd_ctx* c) {
   QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
   if (hflag[1]) {   // a small pivot somewhere: redo with partial pivoting
     for (int p = 0; p < 2; p++) {
-      clover_invert_k<<<(c->g.Vh + 63) / 64, 64, 0, c->stream>>>(c->g.Vh, c->M[0][p], c->Mi[0][p], flag);
+      clover_invert_k<<<(c->g.Vg + 63) / 64, 64, 0, c->stream>>>(c->g.Vg, c->M[0][p], c->Mi[0][p], flag);
       QXD_LAUNCH_CHECK(c);
     }
     QXD_CUDA_OK(c, cudaMemcpyAsync(hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));

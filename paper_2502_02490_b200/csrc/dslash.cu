@@ -24,23 +24,43 @@ __device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
       out[2 * j + 1] += ur * in[2 * i + 1] - ui * in[2 * i];
     }
 }
+// M v or M^{-1} v for one site; in the C*-paired layout the record is that of the physical site and the mirror image uses
+// sigma2 M^* sigma2, applied as sigma2 conj(M conj(sigma2 v)) (see dslash_kernel.cuh)
 template <typename S>
-__device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const typename PT<S>::C* in, typename PT<S>::C* out) {
-  typename PT<S>::C b[36];
-  load_reals<S, 0, 36>(CL, Vh, cb, b);
-  block_mul(b, in, out);
-  load_reals<S, 36, 36>(CL, Vh, cb, b);
-  block_mul(b, in + 12, out + 12);
+__device__ __forceinline__ void clover_mul(const void* CL, const Geom& g, int cb, const typename PT<S>::C* in, typename PT<S>::C* out) {
+  typedef typename PT<S>::C C;
+  const bool mir = g.pair && (cb & 1);
+  const int rec = g.pair ? (cb >> 1) : cb;
+  C b[36];
+#pragma unroll
+  for (int blk = 0; blk < 2; blk++) {
+    if (blk == 0) load_reals<S, 0, 36>(CL, g.Vg, rec, b); else load_reals<S, 36, 36>(CL, g.Vg, rec, b);
+    const C* v = in + 12 * blk;
+    C a[12], w[12];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      a[2 * c] = mir ? v[6 + 2 * c + 1] : v[2 * c];        a[2 * c + 1] = mir ? v[6 + 2 * c] : v[2 * c + 1];
+      a[6 + 2 * c] = mir ? -v[2 * c + 1] : v[6 + 2 * c];   a[6 + 2 * c + 1] = mir ? -v[2 * c] : v[6 + 2 * c + 1];
+    }
+    block_mul(b, a, w);
+    C* y = out + 12 * blk;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      y[2 * c] = mir ? -w[6 + 2 * c + 1] : w[2 * c];       y[2 * c + 1] = mir ? -w[6 + 2 * c] : w[2 * c + 1];
+      y[6 + 2 * c] = mir ? w[2 * c + 1] : w[6 + 2 * c];    y[6 + 2 * c + 1] = mir ? w[2 * c] : w[6 + 2 * c + 1];
+    }
+  }
 }
 
 template <typename S, int INV_DUMMY>
-__global__ void __launch_bounds__(128) clover_apply_k(int Vh, const void* CL, SpinorPtr in, SpinorPtr out) {
+__global__ void __launch_bounds__(128) clover_apply_k(Geom g, const void* CL, SpinorPtr in, SpinorPtr out) {
   typedef typename PT<S>::C C;
+  const int Vh = g.Vh;
   const int cb = blockIdx.x * blockDim.x + threadIdx.x;
   if (cb >= Vh) return;
   C v[24], w[24];
   load_spinor<S>(in, Vh, cb, v);
-  clover_mul<S>(CL, Vh, cb, v, w);
+  clover_mul<S>(CL, g, cb, v, w);
   store_spinor<S>(out, Vh, cb, w);
 }
 
@@ -63,9 +83,12 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.tm = d.tm;
   if (a.nrhs > 64) return fail(c, QXD_EINVAL, "dslash: at most 64 right-hand sides per launch");
   a.R.partials = c->partials; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
-  int rc;
-  if (c->link_reals[d.prec] == 14) rc = d.prec == 0 ? dslash_dispatch_f64_l14(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l14(c, d, a) : dslash_dispatch_f16_l14(c, d, a);
-  else rc = d.prec == 0 ? dslash_dispatch_f64_l18(c, d, a) : d.prec == 1 ? dslash_dispatch_f32_l18(c, d, a) : dslash_dispatch_f16_l18(c, d, a);
+  typedef int (*Dispatch)(qxd_ctx*, const DslashCall&, DslashArgs&);
+  static const Dispatch table[3][2][2] = {   // [precision][14-real links][paired layout]
+      {{dslash_dispatch_f64_l18_p0, dslash_dispatch_f64_l18_p1}, {dslash_dispatch_f64_l14_p0, dslash_dispatch_f64_l14_p1}},
+      {{dslash_dispatch_f32_l18_p0, dslash_dispatch_f32_l18_p1}, {dslash_dispatch_f32_l14_p0, dslash_dispatch_f32_l14_p1}},
+      {{dslash_dispatch_f16_l18_p0, dslash_dispatch_f16_l18_p1}, {dslash_dispatch_f16_l14_p0, dslash_dispatch_f16_l14_p1}}};
+  int rc = table[d.prec][c->link_reals[d.prec] == 14 ? 1 : 0][c->g.pair ? 1 : 0](c, d, a);
   if (rc) return rc;
   QXD_LAUNCH_CHECK(c);
   if (d.flags & DSF_NORM) {   // second kernel of the fused norm: add the per-tile partials (qxd_common.cuh)
@@ -78,9 +101,9 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
 int launch_clover_apply(qxd_ctx* c, int prec, int inverse, int parity, const SpinorPtr& in, const SpinorPtr& out) {
   const void* CL = inverse ? c->Mi[prec][parity] : c->M[prec][parity];
   dim3 gr((c->g.Vh + 127) / 128);
-  if (prec == 0) clover_apply_k<double, 0><<<gr, 128, 0, c->stream>>>(c->g.Vh, CL, in, out);
-  else if (prec == 1) clover_apply_k<float, 0><<<gr, 128, 0, c->stream>>>(c->g.Vh, CL, in, out);
-  else clover_apply_k<__half, 0><<<gr, 128, 0, c->stream>>>(c->g.Vh, CL, in, out);
+  if (prec == 0) clover_apply_k<double, 0><<<gr, 128, 0, c->stream>>>(c->g, CL, in, out);
+  else if (prec == 1) clover_apply_k<float, 0><<<gr, 128, 0, c->stream>>>(c->g, CL, in, out);
+  else clover_apply_k<__half, 0><<<gr, 128, 0, c->stream>>>(c->g, CL, in, out);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }

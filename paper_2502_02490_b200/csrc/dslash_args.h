@@ -20,12 +20,18 @@ struct DslashArgs {
 };
 
 
-// one translation unit per storage precision and link format (dslash_f64_l18.cu, ..., dslash_f16_l14.cu)
-int dslash_dispatch_f64_l18(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f32_l18(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f16_l18(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f64_l14(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f32_l14(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
-int dslash_dispatch_f16_l14(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+// one translation unit per storage precision, link format and layout (dslash_f64_l18_p0.cu, ..., dslash_f16_l14_p1.cu)
+int dslash_dispatch_f64_l18_p0(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f64_l18_p1(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f64_l14_p0(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f64_l14_p1(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32_l18_p0(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32_l18_p1(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32_l14_p0(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f32_l14_p1(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16_l18_p0(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16_l18_p1(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16_l14_p0(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
+int dslash_dispatch_f16_l14_p1(qxd_ctx* c, const DslashCall& d, DslashArgs& a);
 
 }  // namespace qxd

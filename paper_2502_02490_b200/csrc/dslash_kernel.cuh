@@ -118,16 +118,46 @@ __device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const
   load_reals<S, 36, 36>(CL, Vh, cb, b);
   block_mul(b, in + 12, out + 12);
 }
+// Paired layout: the clover block of the mirror site is sigma2 M^* sigma2, so (M' v) = sigma2 conj(M conj(sigma2 v)): the
+// stored block is applied to a = conj(sigma2 v) = (i conj v1, -i conj v0) and the result w is mapped to (-i conj w1, i conj w0).
+// In (re, im) pairs these are swaps and sign changes only; `mir` differs between neighbouring lanes, hence selects.
+template <typename C>
+__device__ __forceinline__ void mirror_in(const C* v, C* a, bool mir) {
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    a[2 * c] = mir ? v[6 + 2 * c + 1] : v[2 * c];            a[2 * c + 1] = mir ? v[6 + 2 * c] : v[2 * c + 1];
+    a[6 + 2 * c] = mir ? -v[2 * c + 1] : v[6 + 2 * c];       a[6 + 2 * c + 1] = mir ? -v[2 * c] : v[6 + 2 * c + 1];
+  }
+}
+template <typename C>
+__device__ __forceinline__ void mirror_out(const C* w, C* y, bool mir) {
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    y[2 * c] = mir ? -w[6 + 2 * c + 1] : w[2 * c];           y[2 * c + 1] = mir ? -w[6 + 2 * c] : w[2 * c + 1];
+    y[6 + 2 * c] = mir ? w[2 * c + 1] : w[6 + 2 * c];        y[6 + 2 * c + 1] = mir ? w[2 * c] : w[6 + 2 * c + 1];
+  }
+}
 // the same blocks applied to R spinors (multi-RHS, row a10): each block is loaded once
-template <typename S, int R>
-__device__ __forceinline__ void clover_mul_multi(const void* CL, int Vh, int cb, const typename PT<S>::C (*in)[24], typename PT<S>::C (*out)[24]) {
-  typename PT<S>::C b[36];
-  load_reals<S, 0, 36>(CL, Vh, cb, b);
+template <typename S, int R, bool PAIR>
+__device__ __forceinline__ void clover_mul_multi(const void* CL, const Geom& g, int cb, const typename PT<S>::C (*in)[24], typename PT<S>::C (*out)[24]) {
+  typedef typename PT<S>::C C;
+  C b[36];
+  constexpr bool paired = PAIR;
+  const bool mir = paired && (cb & 1);
+  const int rec = paired ? (cb >> 1) : cb;
 #pragma unroll
-  for (int r = 0; r < R; r++) block_mul(b, in[r], out[r]);
-  load_reals<S, 36, 36>(CL, Vh, cb, b);
+  for (int blk = 0; blk < 2; blk++) {
+    if (blk == 0) load_reals<S, 0, 36>(CL, g.Vg, rec, b); else load_reals<S, 36, 36>(CL, g.Vg, rec, b);
 #pragma unroll
-  for (int r = 0; r < R; r++) block_mul(b, in[r] + 12, out[r] + 12);
+    for (int r = 0; r < R; r++) {
+      if (paired) {
+        C a[12], w[12];
+        mirror_in(in[r] + 12 * blk, a, mir);
+        block_mul(b, a, w);
+        mirror_out(w, out[r] + 12 * blk, mir);
+      } else block_mul(b, in[r] + 12 * blk, out[r] + 12 * blk);
+    }
+  }
 }
 
 // One hop in flight: the raw 16-byte chunks of the neighbour spinor and of the link, exactly as loaded.  Keeping the
@@ -144,6 +174,7 @@ struct HopRegs {
   static constexpr int NWC = NL == 18 ? (RPC == 2 ? 9 : RPC == 4 ? 5 : 3) : (RPC == 2 ? 7 : RPC == 4 ? 4 : 3);
   V w[NWC];        // chunks covering the NL reals of one link (loaded once for all R right-hand sides)
   float scale[R];  // fp16 block-float scale of the neighbour spinor
+  float wsgn;      // paired layout: -1 if the link belongs to a mirror site (W^* = conj W), else +1
 };
 template <int MU, typename S, int NL> struct LinkChunks {
   static constexpr int RPC = PT<S>::RPC;
@@ -167,12 +198,12 @@ __device__ __forceinline__ void reconstruct_row2(const C* in, C* w) {
     w[12 + 2 * c] = rr; w[12 + 2 * c + 1] = ri;
   }
 }
-template <typename S, int MU, int DIR, int R, int NL>
+template <typename S, int MU, int DIR, int R, int NL, bool PAIR>
 __device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, HopRegs<S, R, NL>& d) {
   typedef typename PT<S>::V V;
   typedef LinkChunks<MU, S, NL> LC;
   const int Vh = a.g.Vh;
-  const int nb = neighbour_cb<MU, DIR>(a.g, s);
+  const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
 #pragma unroll
   for (int r = 0; r < R; r++) {
     if (R > 1 && rhs0 + r >= a.nrhs) break;
@@ -184,12 +215,14 @@ __device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, in
   }
   // forward: W_mu(x) of the own parity; backward: W_mu(x-mu) of the other parity at the neighbour
   const V* w = reinterpret_cast<const V*>(DIR > 0 ? a.W[parity] : a.W[1 - parity]);
-  const int wi = DIR > 0 ? cb : nb;
+  int wi = DIR > 0 ? cb : nb;
+  d.wsgn = 1.f;
+  if (PAIR) { d.wsgn = (wi & 1) ? -1.f : 1.f; wi >>= 1; }   // the record of the physical site; conjugate for the mirror image
 
 #pragma unroll
-  for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * Vh + wi);
+  for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * a.g.Vg + wi);
 }
-template <typename S, int MU, int DIR, bool G5IN, int R, int NL>
+template <typename S, int MU, int DIR, bool G5IN, int R, int NL, bool PAIR>
 __device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<S>::C (*acc)[24]) {
   typedef typename PT<S>::C C;
   typedef LinkChunks<MU, S, NL> LC;
@@ -197,6 +230,10 @@ __device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<
   C wv[HopRegs<S, R, NL>::NWC * RPC];
 #pragma unroll
   for (int c = 0; c < LC::N; c++) unpack_vec(d.w[c], wv + c * RPC);
+  if (PAIR) {   // links of mirror sites are the complex conjugates (rows, and det W with them)
+#pragma unroll
+    for (int i = 1; i < NL; i += 2) wv[LC::OFF + i] *= (C)d.wsgn;
+  }
   C w18[18];
   if (NL == 14) reconstruct_row2(wv + LC::OFF, w18);
   const C* wl = NL == 14 ? w18 : wv + LC::OFF;
@@ -215,36 +252,36 @@ __device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<
   }
 }
 // all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one
-template <typename S, bool G5IN, int R, int PIPE, int NL>
+template <typename S, bool G5IN, int R, int PIPE, int NL, bool PAIR>
 __device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, typename PT<S>::C (*acc)[24]) {
   if (PIPE == 2) {
     HopRegs<S, R, NL> d0, d1;
-    hop_issue<S, 0, +1, R, NL>(a, s, cb, parity, rhs0, d0);
-    hop_issue<S, 0, -1, R, NL>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 0, +1, G5IN, R, NL>(d0, acc);
-    hop_issue<S, 1, +1, R, NL>(a, s, cb, parity, rhs0, d0);
-    hop_use<S, 0, -1, G5IN, R, NL>(d1, acc);
-    hop_issue<S, 1, -1, R, NL>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 1, +1, G5IN, R, NL>(d0, acc);
-    hop_issue<S, 2, +1, R, NL>(a, s, cb, parity, rhs0, d0);
-    hop_use<S, 1, -1, G5IN, R, NL>(d1, acc);
-    hop_issue<S, 2, -1, R, NL>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 2, +1, G5IN, R, NL>(d0, acc);
-    hop_issue<S, 3, +1, R, NL>(a, s, cb, parity, rhs0, d0);
-    hop_use<S, 2, -1, G5IN, R, NL>(d1, acc);
-    hop_issue<S, 3, -1, R, NL>(a, s, cb, parity, rhs0, d1);
-    hop_use<S, 3, +1, G5IN, R, NL>(d0, acc);
-    hop_use<S, 3, -1, G5IN, R, NL>(d1, acc);
+    hop_issue<S, 0, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d0);
+    hop_issue<S, 0, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 0, +1, G5IN, R, NL, PAIR>(d0, acc);
+    hop_issue<S, 1, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 0, -1, G5IN, R, NL, PAIR>(d1, acc);
+    hop_issue<S, 1, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 1, +1, G5IN, R, NL, PAIR>(d0, acc);
+    hop_issue<S, 2, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 1, -1, G5IN, R, NL, PAIR>(d1, acc);
+    hop_issue<S, 2, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 2, +1, G5IN, R, NL, PAIR>(d0, acc);
+    hop_issue<S, 3, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d0);
+    hop_use<S, 2, -1, G5IN, R, NL, PAIR>(d1, acc);
+    hop_issue<S, 3, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d1);
+    hop_use<S, 3, +1, G5IN, R, NL, PAIR>(d0, acc);
+    hop_use<S, 3, -1, G5IN, R, NL, PAIR>(d1, acc);
   } else {
     HopRegs<S, R, NL> d;
-    hop_issue<S, 0, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 0, +1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 0, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 0, -1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 1, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 1, +1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 1, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 1, -1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 2, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 2, +1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 2, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 2, -1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 3, +1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 3, +1, G5IN, R, NL>(d, acc);
-    hop_issue<S, 3, -1, R, NL>(a, s, cb, parity, rhs0, d); hop_use<S, 3, -1, G5IN, R, NL>(d, acc);
+    hop_issue<S, 0, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 0, +1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 0, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 0, -1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 1, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 1, +1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 1, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 1, -1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 2, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 2, +1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 2, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 2, -1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 3, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 3, +1, G5IN, R, NL, PAIR>(d, acc);
+    hop_issue<S, 3, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d); hop_use<S, 3, -1, G5IN, R, NL, PAIR>(d, acc);
   }
 }
 
@@ -268,7 +305,7 @@ template <typename S, int R, bool FULL, int NL> struct KernelShape {
   static constexpr int MINB = SPLIT ? (sizeof(S) == 8 ? 2 : 4) : sizeof(S) == 8 ? 1 : (R == 1 ? (FULL ? 2 : 4) : (R == 2 ? (FULL ? 1 : 3) : (FULL ? 1 : 2)));
   static constexpr int PIPE = (R == 1) ? 2 : 1;   // hops in flight per thread
 };
-template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL, bool PAIR>
 __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelShape<S, R, FULL, NL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
   typedef typename PT<S>::C C;
   const int Vh = a.g.Vh;
@@ -285,14 +322,14 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
   for (int r = 0; r < R; r++) nrm[r] = 0.0;
   if (cb < Vh) {
     Site s;
-    site_init(a.g, cb, parity, s);
+    site_init<PAIR ? 1 : 0>(a.g, cb, parity, s);
     C acc[R][24];
 #pragma unroll
     for (int r = 0; r < R; r++)
 #pragma unroll
       for (int i = 0; i < 24; i++) acc[r][i] = 0;
     const C hs = NEG ? (C)0.5 : (C)-0.5;  // +-hop = -+1/2 acc
-    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL, NL>::PIPE, NL>(a, s, cb, parity, rhs0, acc);
+    hop_all<S, (FLAGS & DSF_G5IN) != 0, R, KernelShape<S, R, FULL, NL>::PIPE, NL, PAIR>(a, s, cb, parity, rhs0, acc);
 #pragma unroll
     for (int r = 0; r < R; r++)
 #pragma unroll
@@ -306,7 +343,7 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
       }
       if (PHI == 2) {
         C mphi[R][24];
-        clover_mul_multi<S, R>(a.CL[parity], Vh, cb, phi, mphi);
+        clover_mul_multi<S, R, PAIR>(a.CL[parity], a.g, cb, phi, mphi);
 #pragma unroll
         for (int r = 0; r < R; r++)
 #pragma unroll
@@ -320,7 +357,7 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
     }
     if (POST) {
       C t[R][24];
-      clover_mul_multi<S, R>(a.CL[parity], Vh, cb, acc, t);
+      clover_mul_multi<S, R, PAIR>(a.CL[parity], a.g, cb, acc, t);
 #pragma unroll
       for (int r = 0; r < R; r++)
 #pragma unroll
@@ -349,17 +386,17 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
   }
 }
 
-template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL>
+template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL, bool PAIR>
 void launch_r(qxd_ctx* c, DslashArgs& a) {
   a.ngroups = (a.nrhs + R - 1) / R;
   const unsigned ntiles = a.tm.count > 0 ? unsigned(a.tm.count) : unsigned((c->g.Vh + 127) / 128);
   dim3 gr(ntiles * unsigned(a.ngroups) * (KernelShape<S, R, FULL, NL>::SPLIT ? 2u : 1u));
-  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL><<<gr, KernelShape<S, R, FULL, NL>::THREADS, 0, c->stream>>>(a);
+  dslash_k<S, PHI, POST, NEG, FLAGS, FULL, R, NL, PAIR><<<gr, KernelShape<S, R, FULL, NL>::THREADS, 0, c->stream>>>(a);
 }
 // right-hand sides per thread: 1 for a single spinor; for a batch the value chosen by qxd_set_rhs_per_thread (default 1:
 // measured at c3 with 12 right-hand sides, fp32: 0.43 ms per right-hand side against 0.59 (R = 2) and 0.50 (R = 3))
 // MULTI: instantiate the R = 2, 3 kernels for this mode (only the modes the batched solver and bench use)
-template <typename S, int NL, int PHI, int POST, bool NEG, int FLAGS, bool FULL, bool MULTI>
+template <typename S, int NL, bool PAIR, int PHI, int POST, bool NEG, int FLAGS, bool FULL, bool MULTI>
 int launch_one(qxd_ctx* c, DslashArgs& a) {
   int R = 1;
   if (a.nrhs > 1) {
@@ -367,36 +404,36 @@ int launch_one(qxd_ctx* c, DslashArgs& a) {
     if (R > a.nrhs) R = a.nrhs;
   }
   if (MULTI && sizeof(S) < 8) {   // fp64: the accumulators of two spinors do not fit the register file
-    if (R == 2) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 2 : 1, NL>(c, a); return QXD_OK; }
-    if (R >= 3) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 3 : 1, NL>(c, a); return QXD_OK; }
+    if (R == 2) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 2 : 1, NL, PAIR>(c, a); return QXD_OK; }
+    if (R >= 3) { launch_r<S, PHI, POST, NEG, FLAGS, FULL, (MULTI && sizeof(S) < 8) ? 3 : 1, NL, PAIR>(c, a); return QXD_OK; }
   }
   // one right-hand side per thread, the right-hand sides of a tile in consecutive CTAs
-  launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1, NL>(c, a);
+  launch_r<S, PHI, POST, NEG, FLAGS, FULL, 1, NL, PAIR>(c, a);
   return QXD_OK;
 }
 
-template <typename S, int NL>
+template <typename S, int NL, bool PAIR>
 int dispatch(qxd_ctx* c, const DslashCall& d, DslashArgs& a) {
   const int f = d.flags;
   switch (d.mode) {
     case DS_DW_FULL:
       if (f != 0) break;
-      return launch_one<S, NL, 2, 0, false, 0, true, true>(c, a);
+      return launch_one<S, NL, PAIR, 2, 0, false, 0, true, true>(c, a);
     case DS_HOP_AINV:
-      if (f == 0) { return launch_one<S, NL, 0, 1, false, 0, false, true>(c, a); }
-      if (f == DSF_G5IN) { return launch_one<S, NL, 0, 1, false, DSF_G5IN, false, true>(c, a); }
+      if (f == 0) { return launch_one<S, NL, PAIR, 0, 1, false, 0, false, true>(c, a); }
+      if (f == DSF_G5IN) { return launch_one<S, NL, PAIR, 0, 1, false, DSF_G5IN, false, true>(c, a); }
       break;
     case DS_A_XMHOP:
-      if (f == 0) { return launch_one<S, NL, 2, 0, true, 0, false, true>(c, a); }
-      if (f == DSF_NORM) { return launch_one<S, NL, 2, 0, true, DSF_NORM, false, true>(c, a); }
-      if (f == DSF_G5HOP) { return launch_one<S, NL, 2, 0, true, DSF_G5HOP, false, true>(c, a); }
-      if (f == (DSF_G5HOP | DSF_NORM)) { return launch_one<S, NL, 2, 0, true, DSF_G5HOP | DSF_NORM, false, true>(c, a); }
+      if (f == 0) { return launch_one<S, NL, PAIR, 2, 0, true, 0, false, true>(c, a); }
+      if (f == DSF_NORM) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_NORM, false, true>(c, a); }
+      if (f == DSF_G5HOP) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_G5HOP, false, true>(c, a); }
+      if (f == (DSF_G5HOP | DSF_NORM)) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_G5HOP | DSF_NORM, false, true>(c, a); }
       break;
     case DS_X_MHOP:
-      if (f == 0) { return launch_one<S, NL, 1, 0, true, 0, false, false>(c, a); }
+      if (f == 0) { return launch_one<S, NL, PAIR, 1, 0, true, 0, false, false>(c, a); }
       break;
     case DS_AINV_X_MHOP:
-      if (f == 0) { return launch_one<S, NL, 1, 1, true, 0, false, false>(c, a); }
+      if (f == 0) { return launch_one<S, NL, PAIR, 1, 1, true, 0, false, false>(c, a); }
       break;
     default: break;
   }

@@ -10,12 +10,12 @@ namespace qxd {
 // ---- gauge: natural physical AoS -> extended even-odd SoA fp64; mirror half = conj(U), -A (reading R8)
 __global__ void __launch_bounds__(128) gauge_pack_k(Geom g, const double* __restrict__ U, const double* __restrict__ A,
                                                     void* Ug0, void* Ug1, void* Ag0, void* Ag1) {
-  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;   // index of the link record: extended site, or physical site (paired layout)
   int parity = blockIdx.y;
-  if (cb >= g.Vh) return;
+  if (cb >= g.Vg) return;
   int x[4];
-  coords_of(g, cb, parity, x);
-  bool mirror = x[1] >= g.L1;
+  coords_int(g, cb, parity, x);
+  bool mirror = !g.pair && x[1] >= g.L1;
   int x1p = mirror ? x[1] - g.L1 : x[1];
   size_t sp = ((size_t(x[0]) * g.L1 + x1p) * g.X[2] + x[2]) * g.X[3] + x[3];
   double r[72];
@@ -25,13 +25,13 @@ __global__ void __launch_bounds__(128) gauge_pack_k(Geom g, const double* __rest
     r[2 * k] = u[2 * k];
     r[2 * k + 1] = mirror ? -u[2 * k + 1] : u[2 * k + 1];
   }
-  store_record<double, 72>(parity ? Ug1 : Ug0, g.Vh, cb, r);
+  store_record<double, 72>(parity ? Ug1 : Ug0, g.Vg, cb, r);
   double a[4] = {0, 0, 0, 0};
   if (A) {
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) a[mu] = mirror ? -A[sp * 4 + mu] : A[sp * 4 + mu];
   }
-  store_record<double, 4>(parity ? Ag1 : Ag0, g.Vh, cb, a);
+  store_record<double, 4>(parity ? Ag1 : Ag0, g.Vg, cb, a);
 }
 
 // ---- hopping links W_mu(x) = e^{i q A_mu(x)} U_mu(x), fermion time-boundary sign folded
@@ -44,12 +44,12 @@ __global__ void __launch_bounds__(128) hoplinks_k(Geom g, double q, int use_a, c
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   int parity = blockIdx.y;
-  if (cb >= g.Vh) return;
+  if (cb >= g.Vg) return;
   int x[4];
-  coords_of(g, cb, parity, x);
+  coords_int(g, cb, parity, x);
   double u[72], a[4];
-  load_reals<double, 0, 72>(parity ? Ug1 : Ug0, g.Vh, cb, u);
-  load_reals<double, 0, 4>(parity ? Ag1 : Ag0, g.Vh, cb, a);
+  load_reals<double, 0, 72>(parity ? Ug1 : Ug0, g.Vg, cb, u);
+  load_reals<double, 0, 4>(parity ? Ag1 : Ag0, g.Vg, cb, a);
   C w[4 * NL];
 #pragma unroll
   for (int mu = 0; mu < 4; mu++) {
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(128) hoplinks_k(Geom g, double q, int use_a, c
       w[NL * mu + 13] = (C)(c3 * di + s3 * dr);
     }
   }
-  store_record<S, 4 * NL>(parity ? W1 : W0, g.Vh, cb, w);
+  store_record<S, 4 * NL>(parity ? W1 : W0, g.Vg, cb, w);
 }
 
 // ---- spinors: natural AoS fp64 <-> packed SoA in precision S
@@ -146,6 +146,25 @@ __global__ void __launch_bounds__(128) convert72_k(int Vh, const void* from, voi
   store_record<ST, 72>(to, Vh, cb, w);
 }
 
+// Packed 6x6 Hermitian block (PAPER.md:117 order, index i = 3 s + c) of the mirror site: M' = sigma2 M^* sigma2, i.e.
+//   M'_(0c)(0c') = conj M_(1c)(1c'),  M'_(1c)(1c') = conj M_(0c)(0c'),  M'_(0c)(1c') = -conj M_(1c)(0c') = -M_(0c')(1c).
+__host__ __device__ inline int packed_upper_index(int i, int j) { return i * 6 - (i * (i + 1)) / 2 + (j - i - 1); }
+__device__ __forceinline__ void mirror_block(const double* b, double* o) {
+#pragma unroll
+  for (int c = 0; c < 3; c++) { o[c] = b[3 + c]; o[3 + c] = b[c]; }
+#pragma unroll
+  for (int c = 0; c < 3; c++)
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+      if (d > c) {
+        const int k00 = 6 + 2 * packed_upper_index(c, d), k11 = 6 + 2 * packed_upper_index(3 + c, 3 + d);
+        o[k00] = b[k11]; o[k00 + 1] = -b[k11 + 1];
+        o[k11] = b[k00]; o[k11 + 1] = -b[k00 + 1];
+      }
+      const int k01 = 6 + 2 * packed_upper_index(c, 3 + d), k10 = 6 + 2 * packed_upper_index(d, 3 + c);
+      o[k01] = -b[k10]; o[k01 + 1] = -b[k10 + 1];
+    }
+}
 __global__ void __launch_bounds__(128) clover_export_k(Geom g, const void* m0, const void* m1, double* __restrict__ out) {
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   int parity = blockIdx.y;
@@ -154,7 +173,14 @@ __global__ void __launch_bounds__(128) clover_export_k(Geom g, const void* m0, c
   coords_of(g, cb, parity, x);
   size_t s = lex_of(g, x);
   double v[72];
-  load_reals<double, 0, 72>(parity ? m1 : m0, g.Vh, cb, v);
+  load_reals<double, 0, 72>(parity ? m1 : m0, g.Vg, g.pair ? (cb >> 1) : cb, v);
+  if (g.pair && (cb & 1)) {   // mirror site: sigma2 M^* sigma2 of either block
+    double t[72];
+#pragma unroll
+    for (int b = 0; b < 2; b++) mirror_block(v + 36 * b, t + 36 * b);
+#pragma unroll
+    for (int i = 0; i < 72; i++) v[i] = t[i];
+  }
 #pragma unroll
   for (int i = 0; i < 72; i++) out[s * 72 + i] = v[i];
 }
@@ -162,13 +188,13 @@ __global__ void __launch_bounds__(128) clover_export_k(Geom g, const void* m0, c
 static inline dim3 grid_for(int Vh, int ny) { return dim3((Vh + 127) / 128, ny); }
 
 int launch_gauge_pack(qxd_ctx* c, const double* U, const double* A) {
-  gauge_pack_k<<<grid_for(c->g.Vh, 2), 128, 0, c->stream>>>(c->g, U, A, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1]);
+  gauge_pack_k<<<grid_for(c->g.Vg, 2), 128, 0, c->stream>>>(c->g, U, A, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1]);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
 
 int launch_hoplinks(qxd_ctx* c, int prec) {
-  dim3 gr = grid_for(c->g.Vh, 2);
+  dim3 gr = grid_for(c->g.Vg, 2);
   int ua = c->have_qed ? 1 : 0;
 #define QXD_HOPLINKS(S, NL) hoplinks_k<S, NL><<<gr, 128, 0, c->stream>>>(c->g, c->q, ua, c->Ug[0], c->Ug[1], c->Ag[0], c->Ag[1], c->W[prec][0], c->W[prec][1])
   if (c->link_reals[prec] == 14) { if (prec == 0) QXD_HOPLINKS(double, 14); else if (prec == 1) QXD_HOPLINKS(float, 14); else QXD_HOPLINKS(__half, 14); }
@@ -212,9 +238,9 @@ int launch_convert_spinor(qxd_ctx* c, int pf, const SpinorPtr& from, int pt, con
   return QXD_OK;
 }
 int launch_convert_record72(qxd_ctx* c, const void* from64, int pt, void* to) {
-  dim3 gr = grid_for(c->g.Vh, 1);
-  if (pt == 1) convert72_k<float><<<gr, 128, 0, c->stream>>>(c->g.Vh, from64, to);
-  else if (pt == 2) convert72_k<__half><<<gr, 128, 0, c->stream>>>(c->g.Vh, from64, to);
+  dim3 gr = grid_for(c->g.Vg, 1);
+  if (pt == 1) convert72_k<float><<<gr, 128, 0, c->stream>>>(c->g.Vg, from64, to);
+  else if (pt == 2) convert72_k<__half><<<gr, 128, 0, c->stream>>>(c->g.Vg, from64, to);
   else return fail(c, QXD_EINVAL, "convert72: bad precision");
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;

@@ -12,7 +12,14 @@
 namespace qxd {
 
 struct Geom {
-  int X[4];        // extended extents T, X1, L2, L3
+  // C*-paired layout (pair = 1): the index machinery below runs on the PHYSICAL lattice
+  // (X[1] = L1) and an extended site is (physical site, mirror bit m): spinor index cb = 2 * cb_phys + m, so a site and
+  // its mirror image x + L1 e1 are neighbours in memory and in the warp.  Links and clover blocks exist once per
+  // physical site (record stride Vg = Vh / 2); the mirror site uses U^*, -A and sigma2 M^* sigma2 (reading R8).
+  int pair;        // 0: extended-lattice layout, 1: C*-paired layout (cstar > 0 only)
+  int Vg;          // stride of the link / clover records: Vh, or Vh / 2 in the paired layout
+  int XE[4];       // extended extents T, X1 = 2 L1 (C*) or L1, L2, L3 -- the natural order of the ABI
+  int X[4];        // extents of the indexed lattice: = XE, or the physical extents in the paired layout
   int L1;          // physical extent of direction 1 (the C* shift)
   int cstar;       // 0..3
   int antiper;     // fermions antiperiodic in time
@@ -37,8 +44,8 @@ __host__ __device__ __forceinline__ int gmu(const Geom& g, int mu, int c) {
 __host__ __device__ __forceinline__ int idx2_of(const Geom& g, const int x[4]) {
   return gmu(g, 0, x[0]) + gmu(g, 1, x[1]) + gmu(g, 2, x[2]) + gmu(g, 3, x[3]);
 }
-// inverse: (cb, parity) -> coordinates
-__host__ __device__ __forceinline__ void coords_of(const Geom& g, int cb, int parity, int x[4]) {
+// inverse on the indexed lattice: (cb, parity) -> coordinates
+__host__ __device__ __forceinline__ void coords_int(const Geom& g, int cb, int parity, int x[4]) {
   const int tsh = g.sh[0] + g.sh[1] + g.sh[2] + g.sh[3] - 1;                            // log2(tile volume / 2)
   const int d3 = g.shB[3] - g.sh[3], d2 = g.shB[2] - g.sh[2], d1 = g.shB[1] - g.sh[1], d0 = g.shB[0] - g.sh[0];
   int r = cb & ((1 << tsh) - 1);
@@ -61,9 +68,16 @@ __host__ __device__ __forceinline__ void coords_of(const Geom& g, int cb, int pa
   int zb = (parity + x[0] + x[1] + x[2]) & 1;
   x[3] = (bz << g.shB[3]) | (mz << g.sh[3]) | (zh << 1) | zb;
 }
-// natural (application) order, Eq. (1) PAPER.md:93 with L1 -> X1
+// (spinor cb, parity) -> EXTENDED coordinates (x1 in [0, 2 L1) under C*)
+__host__ __device__ __forceinline__ void coords_of(const Geom& g, int cb, int parity, int x[4]) {
+  if (g.pair) {
+    coords_int(g, cb >> 1, parity, x);
+    x[1] += (cb & 1) * g.L1;
+  } else coords_int(g, cb, parity, x);
+}
+// natural (application) order, Eq. (1) PAPER.md:93 with L1 -> X1, extended coordinates
 __host__ __device__ __forceinline__ long lex_of(const Geom& g, const int x[4]) {
-  return ((long(x[0]) * g.X[1] + x[1]) * g.X[2] + x[2]) * g.X[3] + x[3];
+  return ((long(x[0]) * g.XE[1] + x[1]) * g.XE[2] + x[2]) * g.XE[3] + x[3];
 }
 
 // A subset of the tiles (128 checkerboard indices each) in launch order: tile(k) = base + (k >> lq) * mv + (k & qm), k < count.
@@ -76,12 +90,17 @@ __host__ __device__ __forceinline__ int tile_of(const TileMap& m, int k) { retur
 
 // Per-thread site context: coordinates and their index contributions (separable index).
 struct Site {
-  int x[4];
+  int x[4];     // coordinates on the indexed lattice (physical in the paired layout)
   int gx[4];
   int idx2;
+  int m;        // mirror bit (paired layout), else 0
 };
+// PAIR: 0 / 1 = layout known at compile time (the dslash kernels), -1 = read g.pair
+template <int PAIR = -1>
 __host__ __device__ __forceinline__ void site_init(const Geom& g, int cb, int parity, Site& s) {
-  coords_of(g, cb, parity, s.x);
+  const bool pair = PAIR < 0 ? (g.pair != 0) : (PAIR != 0);
+  s.m = pair ? (cb & 1) : 0;
+  coords_int(g, pair ? (cb >> 1) : cb, parity, s.x);
 #pragma unroll
   for (int mu = 0; mu < 4; mu++) s.gx[mu] = gmu(g, mu, s.x[mu]);
   s.idx2 = s.gx[0] + s.gx[1] + s.gx[2] + s.gx[3];
@@ -89,13 +108,20 @@ __host__ __device__ __forceinline__ void site_init(const Geom& g, int cb, int pa
 // checkerboard index of x + dir*mu-hat with the boundary rules of reading R8: time and direction 1
 // periodic (X1 = 2 L1 under C*), directions k in 2..cstar wrap with the shift x1 -> x1 + L1 mod 2 L1
 // ("shifted boundaries").  The neighbour has the opposite parity.
-template <int MU, int DIR>
+template <int MU, int DIR, int PAIR = -1>
 __host__ __device__ __forceinline__ int neighbour_cb(const Geom& g, const Site& s) {
+  const bool pair = PAIR < 0 ? (g.pair != 0) : (PAIR != 0);
   int c = s.x[MU] + DIR;
   bool wrap = false;
   if (DIR > 0) { if (c >= g.X[MU]) { c = 0; wrap = true; } }
   else         { if (c < 0) { c = g.X[MU] - 1; wrap = true; } }
   int n = s.idx2 - s.gx[MU] + gmu(g, MU, c);
+  if (pair) {
+    // paired layout: every direction is periodic on the physical lattice; crossing a C* boundary (direction 1, and
+    // directions 2..cstar) lands on the mirror image: the mirror bit flips
+    const int flip = (wrap && MU >= 1 && MU <= (MU == 1 ? 1 : g.cstar)) ? 1 : 0;
+    return ((n >> 1) << 1) | (s.m ^ flip);
+  }
   if (MU >= 2) {
     if (wrap && MU <= g.cstar) {
       int y1 = s.x[1] + g.L1;
@@ -113,7 +139,9 @@ __device__ __forceinline__ void site_step(const Geom& g, const Site& s, int mu, 
   if (c >= g.X[mu]) { c = 0; wrap = true; }
   if (c < 0) { c = g.X[mu] - 1; wrap = true; }
   o.x[mu] = c; o.gx[mu] = gmu(g, mu, c);
-  if (wrap && mu >= 2 && mu <= g.cstar) {
+  if (g.pair) {
+    if (wrap && mu >= 1 && mu <= (mu == 1 ? 1 : g.cstar)) o.m = s.m ^ 1;
+  } else if (wrap && mu >= 2 && mu <= g.cstar) {
     int y1 = s.x[1] + g.L1;
     if (y1 >= g.X[1]) y1 -= g.X[1];
     o.x[1] = y1; o.gx[1] = gmu(g, 1, y1);

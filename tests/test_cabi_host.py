@@ -37,6 +37,13 @@ def test_every_declared_symbol_is_exported_and_bound(lib):
     assert lib.qxd_version().decode().startswith("qxd-b200")
 
 
+def test_pairing_needs_cstar(lib):
+    h = C.c_void_p()
+    assert lib.qxd_geometry_create(4, 4, 4, 4, 4, C.byref(h)) == 0
+    assert lib.qxd_set_cstar_pairing(h, 1) == -1
+    lib.qxd_geometry_destroy(h)
+
+
 def test_geometry_argument_checks(lib):
     h = C.c_void_p()
     for bad in ((3, 4, 4, 4, 0), (4, 4, 4, 0, 0), (4, 2, 4, 5, 1), (4, 4, 4, 4, 8), (4, 4, 4, 4, -1)):
@@ -54,16 +61,23 @@ def test_geometry_argument_checks(lib):
     assert lib.qxd_geometry_destroy(h) == 0
 
 
-@pytest.mark.parametrize("dims,cstar,tile,block", [
-    ((4, 4, 4, 4), 0, None, None),
-    ((8, 4, 4, 8), 3, None, None),
-    ((8, 2, 6, 4), 2, (2, 2, 2, 4), (4, 4, 2, 4)),
-    ((16, 4, 4, 4), 1, (4, 4, 4, 4), (16, 4, 4, 4)),
-    ((6, 2, 2, 2), 3, None, None),
+@pytest.mark.parametrize("dims,cstar,tile,block,pairing", [
+    ((4, 4, 4, 4), 0, None, None, 0),
+    ((8, 4, 4, 8), 3, None, None, 0),
+    ((8, 2, 6, 4), 2, (2, 2, 2, 4), (4, 4, 2, 4), 0),
+    ((16, 4, 4, 4), 1, (4, 4, 4, 4), (16, 4, 4, 4), 0),
+    ((6, 2, 2, 2), 3, None, None, 0),
+    # C*-paired layout: (physical site, mirror bit); same extended-lattice neighbour relation
+    ((8, 4, 4, 8), 3, None, None, 1),
+    ((8, 2, 6, 4), 2, (2, 2, 2, 4), (4, 2, 2, 4), 1),
+    ((16, 4, 4, 4), 1, None, None, 1),
+    ((6, 2, 2, 2), 3, None, None, 1),
 ])
-def test_site_order_bijection_and_neighbours(lib, dims, cstar, tile, block):
+def test_site_order_bijection_and_neighbours(lib, dims, cstar, tile, block, pairing):
     h = C.c_void_p()
     assert lib.qxd_geometry_create(*dims, cstar | 4, C.byref(h)) == 0
+    if pairing:
+        assert lib.qxd_set_cstar_pairing(h, 1) == 0
     if tile:
         assert lib.qxd_set_tile(h, *tile) == 0
     if block:
@@ -91,6 +105,14 @@ def test_site_order_bijection_and_neighbours(lib, dims, cstar, tile, block):
                 t = lat.nbr[mu, d, s]
                 assert index[t, 1] == 1 - index[s, 1]
                 assert nb.value == index[t, 0], (s, mu, step)
+    if pairing:   # a site and its mirror image x + L1 e1 are consecutive indices of the same parity
+        L1 = dims[1]
+        for s in range(V):
+            x = lat.coords[s]
+            if x[1] < L1:
+                y = I4(int(x[0]), int(x[1]) + L1, int(x[2]), int(x[3]))
+                assert lib.qxd_site_index(h, y, C.byref(cb), C.byref(par)) == 0
+                assert (cb.value, par.value) == (int(index[s, 0]) + 1, int(index[s, 1])) and index[s, 0] % 2 == 0
     assert lib.qxd_site_neighbour(h, 0, 0, 4, 1, C.byref(nb)) == -1
     assert lib.qxd_site_coords(h, V // 2, 0, I4()) == -1
     lib.qxd_geometry_destroy(h)

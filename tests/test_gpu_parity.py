@@ -32,7 +32,7 @@ class Case:
     """Oracle context + CUDA context on identical seeded fields."""
 
     def __init__(self, dims, cstar, ap, qed, q=2 / 3, kappa=0.12, csw=1.5, csw_qed=1.0, qel=1.0, eps=0.3,
-                 precisions=(F64, F32, F16), tile=None, oracle_clover=True, nrhs=1):
+                 precisions=(F64, F32, F16), tile=None, oracle_clover=True, nrhs=1, pairing=False):
         from paper_2502_02490_b200 import binding as B
         self.B = B
         bc = cstar | (ap << 2)
@@ -48,7 +48,7 @@ class Case:
             self.ref.clover_build(csw, self.csw_qed)
         else:
             self.ref.set_csw(csw, self.csw_qed)
-        self.gpu = B.Qxd(*dims, bc, precisions=precisions, tile=tile, nrhs=nrhs)
+        self.gpu = B.Qxd(*dims, bc, precisions=precisions, tile=tile, nrhs=nrhs, pairing=pairing)
         self.gpu.gauge_load(self.U, self.A, qel)
         self.gpu.set_quark(kappa, self.q)
         self.gpu.clover_build(csw, self.csw_qed)
@@ -69,12 +69,21 @@ SMALL = [
     ((6, 4, 4, 6), 3, 1, True),
     ((2, 2, 2, 2), 3, 1, True),       # degenerate: forward and backward neighbour coincide
     ((8, 8, 8, 8), 3, 1, True),       # BASELINE config c1 (q = +2/3)
+    # the same C* cases in the C*-paired device layout (links and clover once per physical site)
+    ((4, 2, 4, 4), 1, 1, True, True),
+    ((4, 4, 2, 6), 2, 1, True, True),
+    ((6, 4, 4, 6), 3, 1, True, True),
+    ((2, 2, 2, 2), 3, 1, True, True),
+    ((8, 8, 8, 8), 3, 1, True, True),
+    ((8, 4, 4, 4), 3, 0, False, True),   # QCD only, periodic in time
 ]
 
 
-@pytest.fixture(scope="module", params=SMALL, ids=lambda p: "x".join(map(str, p[0])) + f"-cstar{p[1]}ap{p[2]}{'qed' if p[3] else 'qcd'}")
+@pytest.fixture(scope="module", params=SMALL,
+                ids=lambda p: "x".join(map(str, p[0])) + f"-cstar{p[1]}ap{p[2]}{'qed' if p[3] else 'qcd'}{'-paired' if len(p) > 4 and p[4] else ''}")
 def case(request):
-    c = Case(*request.param)
+    p = request.param
+    c = Case(*p[:4], pairing=(len(p) > 4 and p[4]))
     yield c
     c.close()
 
