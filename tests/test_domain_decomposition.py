@@ -128,7 +128,7 @@ def test_cuda_contexts_as_rank_local_operators(dims, cstar, ap, qed, world, prec
 
     def make(ts):
         Ul, Al = ts.local_fields(U, A, antiperiodic=bool(ap))
-        g = B.Qxd(*ts.local_dims, D.TimeSlabs.local_bc(cstar), precisions=(B.QXD_F64, B.QXD_F32))
+        g = B.Qxd(*ts.local_dims, D.TimeSlabs.local_bc(cstar), precisions=(B.QXD_F64, B.QXD_F32), pairing=cstar > 0)
         g.gauge_load(Ul, Al, 1.0)
         g.set_quark(KAPPA, Q if qed else 0.0)
         g.set_gauge_reconstruct(B.QXD_RECON_12)     # det W carries the boundary sign of the time links
