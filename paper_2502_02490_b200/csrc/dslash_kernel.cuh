@@ -147,7 +147,7 @@ __device__ __forceinline__ void clover_mul_multi(const void* CL, const Geom& g, 
   const int rec = paired ? (cb >> 1) : cb;
 #pragma unroll
   for (int blk = 0; blk < 2; blk++) {
-    if (blk == 0) load_reals<S, 0, 36>(CL, g.Vg, rec, b); else load_reals<S, 36, 36>(CL, g.Vg, rec, b);
+    if (blk == 0) load_reals<S, 0, 36>(CL, paired ? g.Vg : g.Vh, rec, b); else load_reals<S, 36, 36>(CL, paired ? g.Vg : g.Vh, rec, b);
 #pragma unroll
     for (int r = 0; r < R; r++) {
       if (paired) {
@@ -219,8 +219,9 @@ __device__ __forceinline__ void hop_issue(const DslashArgs& a, const Site& s, in
   d.wsgn = 1.f;
   if (PAIR) { d.wsgn = (wi & 1) ? -1.f : 1.f; wi >>= 1; }   // the record of the physical site; conjugate for the mirror image
 
+  const int Vs = PAIR ? a.g.Vg : Vh;   // stride of the link records (the same register as the spinor stride unless paired)
 #pragma unroll
-  for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * a.g.Vg + wi);
+  for (int c = 0; c < LC::N; c++) d.w[c] = ldg_pinned(w + size_t(LC::C0 + c) * Vs + wi);
 }
 template <typename S, int MU, int DIR, bool G5IN, int R, int NL, bool PAIR>
 __device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<S>::C (*acc)[24]) {
