@@ -363,20 +363,22 @@ static bool time_slabs(const qxd_ctx* c, std::vector<TileMap>& maps, size_t& sla
   const Geom& g = c->g;
   long tv = 1, mv = 1;
   for (int mu = 0; mu < 4; mu++) { tv *= c->tile[mu]; mv *= c->block[mu] / c->tile[mu]; }
-  if (tv != 256 || g.Vh % 128 || g.pair) return false;   // the kernels' 128-index tiles must be the geometric tiles
+  if (tv != 256 || g.Vh % 128) return false;   // the kernels' 128-index tiles must tile the geometric tiles
+  // paired layout: a geometric tile (of the physical lattice) holds two 128-index kernel tiles per parity, (2 n, 2 n + 1)
+  const int f = g.pair ? 2 : 1;
   const int ntt = c->block[0] / c->tile[0], q = int(mv / ntt), NBsp = g.nB[1] * g.nB[2] * g.nB[3];
   const int S = g.nB[0] * ntt;
   if (S < 3 || S > 64) return false;
   int lq = 0;
-  while ((1 << lq) < q) lq++;
+  while ((1 << lq) < q * f) lq++;
   maps.clear();
   for (int bt = 0; bt < g.nB[0]; bt++)
     for (int mt = 0; mt < ntt; mt++) {
       TileMap m;
-      m.lq = lq; m.qm = q - 1; m.mv = int(mv); m.base = bt * NBsp * int(mv) + mt * q; m.count = NBsp * q;
+      m.lq = lq; m.qm = q * f - 1; m.mv = int(mv) * f; m.base = (bt * NBsp * int(mv) + mt * q) * f; m.count = NBsp * q * f;
       maps.push_back(m);
     }
-  slab_sites = size_t(c->tile[0]) * g.X[1] * g.X[2] * g.X[3];
+  slab_sites = size_t(c->tile[0]) * g.XE[1] * g.XE[2] * g.XE[3];
   return true;
 }
 

@@ -413,14 +413,15 @@ def test_full_c3_multi_rhs_sampled_sites(full_c3_case, prec):
         assert relerr(got, c.ref.apply_Dw_sites(etas[k], sites)) < TOL[prec], k
 
 
-@pytest.mark.parametrize("dims,cstar", [((12, 4, 4, 4), 0), ((16, 2, 4, 4), 1), ((16, 4, 4, 8), 3), ((8, 4, 4, 4), 0)])
+@pytest.mark.parametrize("dims,cstar,pairing", [((12, 4, 4, 4), 0, False), ((16, 2, 4, 4), 1, False), ((16, 4, 4, 8), 3, False),
+                                                ((8, 4, 4, 4), 0, False), ((16, 4, 4, 8), 3, True), ((12, 4, 4, 4), 1, True)])
 @pytest.mark.parametrize("prec", [F64, F32])
-def test_apply_Dw_host_pipelined_equals_device_apply(dims, cstar, prec):
+def test_apply_Dw_host_pipelined_equals_device_apply(dims, cstar, pairing, prec):
     """qxd_apply_Dw_host cuts the lattice into time slabs and overlaps host<->device copies with pack / apply / unpack
     (3, 4 and 4 slabs here; the 8x4^3 case has only two and takes the unpipelined path).  Same kernels on the same
     data: the result must equal the device-pointer apply bit for bit, and the oracle within tolerance."""
     import torch
-    c = Case(dims, cstar, 1, cstar > 0, precisions=(F64, F32))
+    c = Case(dims, cstar, 1, cstar > 0, precisions=(F64, F32), pairing=pairing)
     psi = synth.gaussian_spinor(c.dims_ext, 12)
     dev = to_np(c.gpu.apply_Dw(psi, prec))
     eh = torch.from_numpy(psi).pin_memory()
