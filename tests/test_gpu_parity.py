@@ -446,3 +446,38 @@ def test_solve_config_c2_full_size(sloppy):
     assert info["status"] == 0 and info["n_reliable"] >= 1, info
     assert true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05 * cfg["tol"]
     c.close()
+
+
+def _random_geometries(n, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    while len(out) < n:
+        dims = tuple(int(2 * rng.integers(1, 5)) for _ in range(4))          # even extents 2..8
+        cstar = int(rng.integers(0, 4))
+        if np.prod(dims) * (2 if cstar else 1) > 6000:
+            continue
+        ap = int(rng.integers(0, 2))
+        qed = bool(rng.integers(0, 2)) or cstar > 0
+        pairing = bool(cstar > 0 and rng.integers(0, 2))
+        out.append((dims, cstar, ap, qed, pairing))
+    return out
+
+
+@pytest.mark.parametrize("dims,cstar,ap,qed,pairing", _random_geometries(16, 2024),
+                         ids=lambda v: "x".join(map(str, v)) if isinstance(v, tuple) else str(int(v)))
+def test_random_geometries_fp64_operator_and_solve(dims, cstar, ap, qed, pairing):
+    """Seeded random small geometries (even extents 2..8, every cstar, both time boundary conditions, both device layouts,
+    both link formats): fp64 D_w and D-hat element by element against the oracle, and an fp64/fp32 solve to 1e-10."""
+    c = Case(dims, cstar, ap, qed, q=-1 / 3, precisions=(F64, F32), pairing=pairing)
+    psi = synth.gaussian_spinor(c.dims_ext, 3)
+    exp = c.ref.apply_Dw(psi)
+    pe = synth.gaussian_spinor(c.dims_ext, 6).reshape(-1, 4, 3)[: c.V // 2]
+    for recon in (c.B.QXD_RECON_NONE, c.B.QXD_RECON_12):
+        c.gpu.set_gauge_reconstruct(recon)
+        assert relerr(to_np(c.gpu.apply_Dw(psi, F64)).reshape(exp.shape), exp) < 1e-13
+        assert relerr(to_np(c.gpu.apply_Dhat_eo(pe, F64)).reshape(pe.shape), c.ref.apply_Dhat(pe)) < 2e-13
+        assert relerr(to_np(c.gpu.apply_Dw(psi, F32)).reshape(exp.shape), exp) < 1e-6
+    sol, info = c.gpu.solve(psi, 1e-10, algo=0, sloppy=F32)
+    assert info["status"] == 0
+    assert true_residual(c.ref, psi, to_np(sol).reshape(psi.shape)) <= 1.05e-10
+    c.close()
