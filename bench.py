@@ -207,7 +207,7 @@ def run_cuda(args, cfg):
     t_setup = time.perf_counter()
     U, A, eta = make_fields(cfg, rank)
     precs = (B.QXD_F64, B.QXD_F32, B.QXD_F16)
-    g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=max(1, args.nrhs), device=f"cuda:{local}")
+    g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=max(1, args.nrhs), device=f"cuda:{local}", pairing=False)
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
     def timed(fn, n):

@@ -93,7 +93,8 @@ int qxd_geometry_destroy(qxd_ctx* ctx);
 int qxd_set_tile(qxd_ctx* ctx, int b0, int b1, int b2, int b3);
 int qxd_set_block(qxd_ctx* ctx, int B0, int B1, int B2, int B3);
 /* Number of sites of the extended lattice (V). */
-/* C*-paired device layout (C* geometries only; call before qxd_workspace_bind).  A site of the extended lattice and its mirror
+/* C*-paired device layout: the DEFAULT for C* geometries (on = 0 selects the extended-lattice layout; call before
+ * qxd_workspace_bind; on = 1 without a C* direction -> QXD_EINVAL).  A site of the extended lattice and its mirror
  * image x + L1 e1 carry the same gauge information (U^*, -A, R8), so links and clover blocks are stored
  * once per PHYSICAL site and the two sites are processed by neighbouring threads that share every link and clover load: the
  * traffic of the even-odd operator drops from 488 to 248 reals per even site (14-real links).  Results are unchanged (same

@@ -103,7 +103,7 @@ def _ptr(t):
 class Qxd:
     """One solver context (qxd_ctx): geometry, workspace, gauge field, quark, clover term."""
 
-    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=False):
+    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=None):
         import torch
         if not torch.cuda.is_available():
             raise QxdError(QXD_ECUDA, "no CUDA device: the qxd hot path has no CPU fallback")
@@ -119,8 +119,8 @@ class Qxd:
         self.cstar = bc & 3
         self.dims_ext = (T, 2 * L1 if self.cstar else L1, L2, L3)
         self.V = self.lib.qxd_volume(self.h)
-        if pairing:
-            self._chk(self.lib.qxd_set_cstar_pairing(self.h, 1))
+        if pairing is not None and (self.cstar > 0 or pairing):   # None: library default (paired layout for C* geometries)
+            self._chk(self.lib.qxd_set_cstar_pairing(self.h, 1 if pairing else 0))
         if tile is not None:
             self._chk(self.lib.qxd_set_tile(self.h, *tile))
         if block is not None:

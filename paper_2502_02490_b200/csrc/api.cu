@@ -124,6 +124,8 @@ int qxd_geometry_create(int T, int L1, int L2, int L3, int bc, qxd_ctx** out) {
   int B[4] = {pow2_le_dividing(g.X[0], 16), b[1], b[2], b[3]};
   set_order(c, b, B);
   *out = c;
+  // C* geometries use the paired layout by default; qxd_set_cstar_pairing(ctx, 0) selects the extended one
+  if (cstar > 0) qxd_set_cstar_pairing(c, 1);
   return QXD_OK;
 }
 

@@ -124,7 +124,7 @@ int make_geom(qxd_ctx* c, const int B[4], OqxdGeom& o) {
   if (!B) return fail(c, QXD_EINVAL, "openqxd: null block");
   o.V = c->V; o.L1 = c->g.L1; o.cstar = c->g.cstar; o.VB = 1;
   for (int m = 0; m < 4; m++) {
-    o.X[m] = c->g.X[m]; o.B[m] = B[m];
+    o.X[m] = c->g.XE[m]; o.B[m] = B[m];
     if (B[m] < 1 || o.X[m] % B[m]) return fail(c, QXD_EINVAL, "openqxd: cache-block extents must divide the (extended) lattice extents");
     o.NB[m] = o.X[m] / B[m]; o.VB *= B[m];
   }

@@ -76,8 +76,8 @@ def test_geometry_argument_checks(lib):
 def test_site_order_bijection_and_neighbours(lib, dims, cstar, tile, block, pairing):
     h = C.c_void_p()
     assert lib.qxd_geometry_create(*dims, cstar | 4, C.byref(h)) == 0
-    if pairing:
-        assert lib.qxd_set_cstar_pairing(h, 1) == 0
+    if cstar:
+        assert lib.qxd_set_cstar_pairing(h, pairing) == 0     # the paired layout is the default for C* geometries
     if tile:
         assert lib.qxd_set_tile(h, *tile) == 0
     if block:
