@@ -369,6 +369,19 @@ def run_cuda(args, cfg):
                 del a, b
         g.set_gauge_reconstruct(B.QXD_RECON_NONE)
 
+    # ---- row f4: one HMC step's regeneration of the derived fields (new gauge field, same kappa/q/c_sw), lazily -------
+    Ud = torch.from_numpy(U).to(dev)
+    Ad = torch.from_numpy(A).to(dev) if A is not None else None
+    g.set_lazy_refresh(True)
+
+    def new_field():
+        g.gauge_load(Ud, Ad, cfg["qel"])
+        g.refresh()
+    new_field()
+    setup_ms["hmc_step_gauge_load_hoplinks_x3_clover"] = timed(new_field, 5)
+    g.set_lazy_refresh(False)
+    del Ud, Ad
+
     # ---- solves (rows a7, a8): fp64/fp16 and fp64/fp32 mixed CGNE, BiCGstab ------------------------------
     solves = {}
     if not args.no_solve:

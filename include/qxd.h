@@ -127,6 +127,20 @@ int qxd_gauge_load(qxd_ctx* ctx, const double* U_su3, const double* A_u1, double
  * Builds the hopping links W = e^{iqA} U (time-boundary sign folded in) in every bound precision. */
 int qxd_set_quark(qxd_ctx* ctx, double kappa, double q);
 
+/* ---- field-status manager --------------------------------------
+ * Inside an HMC trajectory the gauge field changes while kappa, q, c_sw stay: the hopping links and the clover term
+ * (with its inverse) are DERIVED fields that must follow it.  By default every setter regenerates (qxd_set_quark) or
+ * invalidates (qxd_gauge_load: set_quark and clover_build must be called again, else QXD_ESTATE) what depends on it.
+ * With lazy refresh ON the setters only record their parameters and mark the derived fields stale; the first call that
+ * reads them (any apply, solve, qxd_clover_export, or qxd_refresh) regenerates them on the bound stream, once, from the
+ * recorded parameters -- a trajectory is then  qxd_gauge_load; qxd_solve; qxd_gauge_load; qxd_solve; ...
+ * Turning it OFF regenerates whatever is stale.  qxd_field_status: *status = OR of QXD_FS_*; counts (may be NULL):
+ * [0] hopping-link regenerations, [1] clover build+inversion passes since qxd_geometry_create. */
+enum { QXD_FS_GAUGE = 1, QXD_FS_HOPLINKS = 2, QXD_FS_CLOVER = 4, QXD_FS_HOPLINKS_STALE = 8, QXD_FS_CLOVER_STALE = 16, QXD_FS_LAZY = 32 };
+int qxd_set_lazy_refresh(qxd_ctx* ctx, int on);
+int qxd_refresh(qxd_ctx* ctx);
+int qxd_field_status(const qxd_ctx* ctx, int* status /*HOST*/, long counts[2] /*HOST or NULL*/);
+
 /* ---- clover term (row a3) -----------------------------------------
  * Builds M(x) = (4+m0) + c_sw (i/4) sigma.F-hat + q c_sw_qed (i/4) sigma.A-hat as two Hermitian
  * 6x6 blocks per site and inverts both blocks, on the device.  Needs gauge + quark. */

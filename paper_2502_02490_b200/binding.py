@@ -12,6 +12,7 @@ import os
 QXD_F64, QXD_F32, QXD_F16 = 0, 1, 2
 QXD_CGNE, QXD_BICGSTAB = 0, 1
 QXD_RECON_NONE, QXD_RECON_12 = 18, 12
+QXD_FS_GAUGE, QXD_FS_HOPLINKS, QXD_FS_CLOVER, QXD_FS_HOPLINKS_STALE, QXD_FS_CLOVER_STALE, QXD_FS_LAZY = 1, 2, 4, 8, 16, 32
 QXD_OK, QXD_EINVAL, QXD_ESTATE, QXD_EWORKSPACE, QXD_ECUDA, QXD_ENOCONV = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -51,6 +52,9 @@ SYMBOLS = {
     "qxd_gauge_load": (_i, [_vp, _vp, _vp, _d]),
     "qxd_set_quark": (_i, [_vp, _d, _d]),
     "qxd_clover_build": (_i, [_vp, _d, _d]),
+    "qxd_set_lazy_refresh": (_i, [_vp, _i]),
+    "qxd_refresh": (_i, [_vp]),
+    "qxd_field_status": (_i, [_vp, _vp, _vp]),
     "qxd_set_gauge_reconstruct": (_i, [_vp, _i]),
     "qxd_set_gauge_reconstruct_prec": (_i, [_vp, _i, _i]),
     "qxd_clover_export": (_i, [_vp, _vp, _i]),
@@ -187,6 +191,19 @@ class Qxd:
 
     def clover_build(self, csw, csw_qed=0.0):
         self._chk(self.lib.qxd_clover_build(self.h, float(csw), float(csw_qed)))
+
+    def set_lazy_refresh(self, on=True):
+        self._chk(self.lib.qxd_set_lazy_refresh(self.h, 1 if on else 0))
+
+    def refresh(self):
+        self._chk(self.lib.qxd_refresh(self.h))
+
+    def field_status(self):
+        """(status bits QXD_FS_*, hopping-link regenerations, clover regenerations)"""
+        st = C.c_int(0)
+        cnt = (C.c_long * 2)()
+        self._chk(self.lib.qxd_field_status(self.h, C.byref(st), cnt))
+        return st.value, cnt[0], cnt[1]
 
     def clover_export(self, inverse=False):
         out = self.torch.empty((self.V, 2, 36), dtype=self.torch.float64, device=self.device)

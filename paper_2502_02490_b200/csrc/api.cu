@@ -239,6 +239,42 @@ int qxd_set_stream(qxd_ctx* c, void* s) {
   return QXD_OK;
 }
 
+// ---- field-status manager (row f4) ---------------------------------------------------------------
+static int refresh_hoplinks(qxd_ctx* c) {
+  for (int pr = 0; pr < NPREC; pr++)
+    if ((c->prec_mask >> pr) & 1) { int rc = launch_hoplinks(c, pr); if (rc) return rc; }
+  c->hop_stale = false; c->n_hop_refresh++;
+  return QXD_OK;
+}
+static int refresh_clover(qxd_ctx* c) {
+  int rc = launch_clover_build(c);
+  if (rc) return rc;
+  c->clover_stale = false; c->n_clover_refresh++;
+  return QXD_OK;
+}
+// regenerate what a setter left stale; every entry point that reads derived fields calls it first
+static int ensure_fresh(qxd_ctx* c) {
+  if (c->hop_stale) { int rc = refresh_hoplinks(c); if (rc) return rc; }
+  if (c->clover_stale) { int rc = refresh_clover(c); if (rc) return rc; }
+  return QXD_OK;
+}
+
+int qxd_set_lazy_refresh(qxd_ctx* c, int on) {
+  if (!c) return QXD_EINVAL;
+  if (!on) { int rc = ensure_fresh(c); if (rc) return rc; }
+  c->lazy = on != 0;
+  return QXD_OK;
+}
+int qxd_refresh(qxd_ctx* c) { return c ? ensure_fresh(c) : QXD_EINVAL; }
+int qxd_field_status(const qxd_ctx* c, int* status, long counts[2]) {
+  if (!c || !status) return QXD_EINVAL;
+  *status = (c->have_gauge ? QXD_FS_GAUGE : 0) | (c->have_quark && !c->hop_stale ? QXD_FS_HOPLINKS : 0) |
+            (c->have_clover && !c->clover_stale ? QXD_FS_CLOVER : 0) | (c->hop_stale ? QXD_FS_HOPLINKS_STALE : 0) |
+            (c->clover_stale ? QXD_FS_CLOVER_STALE : 0) | (c->lazy ? QXD_FS_LAZY : 0);
+  if (counts) { counts[0] = c->n_hop_refresh; counts[1] = c->n_clover_refresh; }
+  return QXD_OK;
+}
+
 int qxd_gauge_load(qxd_ctx* c, const double* U, const double* A, double qel) {
   if (!c || !U) return c ? fail(c, QXD_EINVAL, "gauge_load: U_su3 is null") : QXD_EINVAL;
   if (!c->ws) return fail(c, QXD_EWORKSPACE, "gauge_load: no workspace bound");
@@ -247,7 +283,10 @@ int qxd_gauge_load(qxd_ctx* c, const double* U, const double* A, double qel) {
   c->have_qed = (A != nullptr);
   int rc = launch_gauge_pack(c, U, A);
   if (rc) return rc;
-  c->have_gauge = true; c->have_quark = false; c->have_clover = false;
+  c->have_gauge = true;
+  if (c->lazy) {   // the quark and clover parameters stay; what they produced is stale until its next use
+    c->hop_stale = c->have_quark; c->clover_stale = c->have_clover;
+  } else { c->have_quark = false; c->have_clover = false; }
   return QXD_OK;
 }
 
@@ -256,8 +295,12 @@ int qxd_set_quark(qxd_ctx* c, double kappa, double q) {
   if (!c->have_gauge) return fail(c, QXD_ESTATE, "set_quark: load a gauge field first");
   if (!(kappa > 0.0)) return fail(c, QXD_EINVAL, "set_quark: kappa must be > 0");
   c->kappa = kappa; c->q = q; c->m0 = 1.0 / (2.0 * kappa) - 4.0;
-  for (int pr = 0; pr < NPREC; pr++)
-    if ((c->prec_mask >> pr) & 1) { int rc = launch_hoplinks(c, pr); if (rc) return rc; }
+  if (c->lazy) {   // the clover term depends on m0 and q: stale too if its coefficients are known
+    c->have_quark = true; c->hop_stale = true; c->clover_stale = c->have_clover;
+    return QXD_OK;
+  }
+  int rc = refresh_hoplinks(c);
+  if (rc) return rc;
   c->have_quark = true; c->have_clover = false;
   return QXD_OK;
 }
@@ -270,7 +313,7 @@ int qxd_set_gauge_reconstruct_prec(qxd_ctx* c, int prec, int recon) {
   if (nl == c->link_reals[prec]) return QXD_OK;
   c->link_reals[prec] = nl;
   // the hopping links are derived data: rewrite them in the new format (the clover term is unaffected)
-  if (c->have_quark && ((c->prec_mask >> prec) & 1)) return launch_hoplinks(c, prec);
+  if (c->have_quark && !c->hop_stale && ((c->prec_mask >> prec) & 1)) return launch_hoplinks(c, prec);
   return QXD_OK;
 }
 int qxd_set_gauge_reconstruct(qxd_ctx* c, int recon) {
@@ -283,7 +326,8 @@ int qxd_clover_build(qxd_ctx* c, double csw, double csw_qed) {
   if (!c) return QXD_EINVAL;
   if (!c->have_gauge || !c->have_quark) return fail(c, QXD_ESTATE, "clover_build: needs gauge_load and set_quark");
   c->csw = csw; c->csw_qed = csw_qed;
-  int rc = launch_clover_build(c);
+  if (c->lazy) { c->have_clover = true; c->clover_stale = true; return QXD_OK; }
+  int rc = refresh_clover(c);
   if (rc) return rc;
   c->have_clover = true;
   return QXD_OK;
@@ -292,6 +336,8 @@ int qxd_clover_build(qxd_ctx* c, double csw, double csw_qed) {
 int qxd_clover_export(qxd_ctx* c, double* out, int inverse) {
   if (!c || !out) return QXD_EINVAL;
   if (!c->have_clover) return fail(c, QXD_ESTATE, "clover_export: build the clover term first");
+  int rc = ensure_fresh(c);
+  if (rc) return rc;
   return launch_clover_export(c, out, inverse);
 }
 
@@ -300,7 +346,7 @@ static int check_apply(qxd_ctx* c, int prec, const void* a, const void* b, const
   if (!a || !b) return fail(c, QXD_EINVAL, std::string(who) + ": null pointer");
   if (!c->have_clover) return fail(c, QXD_ESTATE, std::string(who) + ": needs gauge_load, set_quark and clover_build");
   if (!prec_ok(c, prec)) return fail(c, QXD_EINVAL, std::string(who) + ": precision not bound in the workspace");
-  return QXD_OK;
+  return ensure_fresh(c);
 }
 
 int qxd_apply_Dw_packed(qxd_ctx* c, int prec, const void* in, void* out) {
