@@ -91,6 +91,74 @@ __device__ __forceinline__ void link_mul(const C* w, const C* h, C* r) {
     }
 }
 
+// ---- packed fp32 arithmetic (sm_100a FFMA2 / FMUL2: two fp32 lanes per issue slot) ----------------------------------
+// The fp32 FMA pipe is no faster with them, but the fp16-storage and C*-paired kernels are bound by instruction issue
+// (profiles/r1c_dslash_family_c3.md), and a packed instruction takes one slot for two results.  ptxas folds lane
+// broadcast (R.F32), lane swap (LO_HI) and negation into the operand, so the packing below costs no instruction where
+// the register allocator can pair the operands.  Same products in the same order as the scalar code: bit-identical.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
+// link multiply with the two spin components of the half spinor in the two lanes
+template <bool ADJ>
+__device__ __forceinline__ void link_mul_x2(const float* w, const float* h, float* r) {
+  f32x2 Xr[3], Xi[3];
+#pragma unroll
+  for (int b = 0; b < 3; b++) { Xr[b] = pk2(h[2 * b], h[6 + 2 * b]); Xi[b] = pk2(h[2 * b + 1], h[6 + 2 * b + 1]); }
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    f32x2 re = 0, im = 0;
+#pragma unroll
+    for (int b = 0; b < 3; b++) {
+      const float wr = ADJ ? w[2 * (3 * b + a)] : w[2 * (3 * a + b)];
+      const float wi = ADJ ? w[2 * (3 * b + a) + 1] : w[2 * (3 * a + b) + 1];
+      const f32x2 Wr = pk2(wr, wr), Wp = pk2(wi, wi), Wn = pk2(-wi, -wi);
+      if (b == 0) { re = mul2(Wr, Xr[0]); im = mul2(Wr, Xi[0]); } else { re = fma2(Wr, Xr[b], re); im = fma2(Wr, Xi[b], im); }
+      re = fma2(ADJ ? Wp : Wn, Xi[b], re);
+      im = fma2(ADJ ? Wn : Wp, Xr[b], im);
+    }
+    upk2(re, r[2 * a], r[6 + 2 * a]);
+    upk2(im, r[2 * a + 1], r[6 + 2 * a + 1]);
+  }
+}
+// reconstruct with the same lanes: (upper spin 0, upper spin 1) and (lower spin 0, lower spin 1) per colour and re/im
+template <int MU, int SGN, bool SCALED>
+__device__ __forceinline__ void reconstruct_x2(const float* r, float* acc, float sc) {
+  const float p = SCALED ? sc : 1.0f, sp = (float)SGN * p, sm = -sp;
+  const f32x2 P = pk2(p, p), PP = pk2(sp, sp), MM = pk2(sm, sm), MP = pk2(sm, sp), PM = pk2(sp, sm);
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const f32x2 Rr = pk2(r[2 * a], r[6 + 2 * a]), Ri = pk2(r[2 * a + 1], r[6 + 2 * a + 1]);
+    const f32x2 Sr = pk2(r[6 + 2 * a], r[2 * a]), Si = pk2(r[6 + 2 * a + 1], r[2 * a + 1]);   // spins swapped
+    f32x2 Ur = pk2(acc[2 * a], acc[6 + 2 * a]), Ui = pk2(acc[2 * a + 1], acc[6 + 2 * a + 1]);
+    f32x2 Lr = pk2(acc[12 + 2 * a], acc[18 + 2 * a]), Li = pk2(acc[12 + 2 * a + 1], acc[18 + 2 * a + 1]);
+    Ur = fma2(P, Rr, Ur); Ui = fma2(P, Ri, Ui);
+    if (MU == 0) { Lr = fma2(PP, Rr, Lr); Li = fma2(PP, Ri, Li); }
+    else if (MU == 1) { Lr = fma2(PP, Si, Lr); Li = fma2(MM, Sr, Li); }
+    else if (MU == 2) { Lr = fma2(MP, Sr, Lr); Li = fma2(MP, Si, Li); }
+    else { Lr = fma2(PM, Ri, Lr); Li = fma2(MP, Rr, Li); }
+    upk2(Ur, acc[2 * a], acc[6 + 2 * a]); upk2(Ui, acc[2 * a + 1], acc[6 + 2 * a + 1]);
+    upk2(Lr, acc[12 + 2 * a], acc[18 + 2 * a]); upk2(Li, acc[12 + 2 * a + 1], acc[18 + 2 * a + 1]);
+  }
+}
+// Which kernels use the packed forms (measured at c3, same box, both layouts): fp16 storage gains 3-8 % (issue bound);
+// fp32 storage loses 0-5 % (bound by DRAM and latency: the pairing constraints on the register allocation cost more
+// than the issue slots bring), fp64 has no packed form.
+#ifndef QXD_X2_F32
+#define QXD_X2_F32 0
+#endif
+#ifndef QXD_X2_F16
+#define QXD_X2_F16 7
+#endif
+// bit 0: link multiply, bit 1: reconstruct, bit 2: clover block multiply
+template <typename S> struct UseX2 {
+  static constexpr int MASK = PT<S>::ID == 2 ? QXD_X2_F16 : PT<S>::ID == 1 ? QXD_X2_F32 : 0;
+  static constexpr bool LINK = (MASK & 1) != 0, RECON = (MASK & 2) != 0, BLOCK = (MASK & 4) != 0;
+};
+
 // out(12 reals: one chirality) = Hermitian 6x6 block (36 packed reals) times in
 template <typename C>
 __device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
@@ -110,13 +178,38 @@ __device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
       out[2 * j + 1] += ur * in[2 * i + 1]; out[2 * j + 1] -= ui * in[2 * i];
     }
 }
+// (re, im) of one component in the two lanes; A = i * in supplies the products with the imaginary part of the block entry
+__device__ __forceinline__ void block_mul_x2(const float* b, const float* in, float* out) {
+  f32x2 I[6], A[6], O[6];
+#pragma unroll
+  for (int k = 0; k < 6; k++) { I[k] = pk2(in[2 * k], in[2 * k + 1]); A[k] = pk2(-in[2 * k + 1], in[2 * k]); }
+#pragma unroll
+  for (int i = 0; i < 6; i++) O[i] = mul2(pk2(b[i], b[i]), I[i]);
+  int k = 6;
+#pragma unroll
+  for (int i = 0; i < 6; i++)
+#pragma unroll
+    for (int j = i + 1; j < 6; j++) {
+      const float ur = b[k], ui = b[k + 1];
+      k += 2;
+      const f32x2 Ur = pk2(ur, ur);
+      O[i] = fma2(Ur, I[j], O[i]); O[i] = fma2(pk2(ui, ui), A[j], O[i]);       // out_i += u in_j
+      O[j] = fma2(Ur, I[i], O[j]); O[j] = fma2(pk2(-ui, -ui), A[i], O[j]);     // out_j += conj(u) in_i
+    }
+#pragma unroll
+  for (int i = 0; i < 6; i++) upk2(O[i], out[2 * i], out[2 * i + 1]);
+}
+template <typename S, typename C>
+__device__ __forceinline__ void block_mul_s(const C* b, const C* in, C* out) {
+  if constexpr (UseX2<S>::BLOCK) block_mul_x2(b, in, out); else block_mul(b, in, out);
+}
 template <typename S>
 __device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const typename PT<S>::C* in, typename PT<S>::C* out) {
   typename PT<S>::C b[36];
   load_reals<S, 0, 36>(CL, Vh, cb, b);
-  block_mul(b, in, out);
+  block_mul_s<S>(b, in, out);
   load_reals<S, 36, 36>(CL, Vh, cb, b);
-  block_mul(b, in + 12, out + 12);
+  block_mul_s<S>(b, in + 12, out + 12);
 }
 // Paired layout: the clover block of the mirror site is sigma2 M^* sigma2, so (M' v) = sigma2 conj(M conj(sigma2 v)): the
 // stored block is applied to a = conj(sigma2 v) = (i conj v1, -i conj v0) and the result w is mapped to (-i conj w1, i conj w0).
@@ -153,9 +246,9 @@ __device__ __forceinline__ void clover_mul_multi(const void* CL, const Geom& g, 
       if (paired) {
         C a[12], w[12];
         mirror_in(in[r] + 12 * blk, a, mir);
-        block_mul(b, a, w);
+        block_mul_s<S>(b, a, w);
         mirror_out(w, out[r] + 12 * blk, mir);
-      } else block_mul(b, in[r] + 12 * blk, out[r] + 12 * blk);
+      } else block_mul_s<S>(b, in[r] + 12 * blk, out[r] + 12 * blk);
     }
   }
 }
@@ -248,8 +341,9 @@ __device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<
       for (int i = 12; i < 24; i++) psi[i] = -psi[i];
     }
     project<MU, DIR>(psi, h);
-    link_mul<(DIR < 0)>(wl, h, t);
-    reconstruct<MU, DIR, PT<S>::ID == 2>(t, acc[r], (C)d.scale[r]);
+    if constexpr (UseX2<S>::LINK) link_mul_x2<(DIR < 0)>(wl, h, t); else link_mul<(DIR < 0)>(wl, h, t);
+    if constexpr (UseX2<S>::RECON) reconstruct_x2<MU, DIR, PT<S>::ID == 2>(t, acc[r], (C)d.scale[r]);
+    else reconstruct<MU, DIR, PT<S>::ID == 2>(t, acc[r], (C)d.scale[r]);
   }
 }
 // all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one
