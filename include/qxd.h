@@ -89,7 +89,9 @@ int qxd_geometry_destroy(qxd_ctx* ctx);
  * sites one CTA works on.  Block extents B (powers of two, multiples of b, dividing the extents): tiles
  * are visited block by block, blocks lexicographically with direction 0 slowest.  qxd_set_tile keeps the
  * current block where it is still a multiple of the tile, else sets B = b.  Both must precede
- * qxd_workspace_bind.  Default: chosen by the library.  The order only permutes sites in memory. */
+ * qxd_workspace_bind.  Default: chosen by the library.  The order only permutes sites in memory.  In the C*-paired
+ * layout (the default for C* geometries, see qxd_set_cstar_pairing) the site order runs over the PHYSICAL lattice, so
+ * b1 and B1 must divide L1; qxd_set_cstar_pairing resets tile and block to the defaults of the layout it selects. */
 int qxd_set_tile(qxd_ctx* ctx, int b0, int b1, int b2, int b3);
 int qxd_set_block(qxd_ctx* ctx, int B0, int B1, int B2, int B3);
 /* Number of sites of the extended lattice (V). */
