@@ -38,7 +38,7 @@ PREC_BYTES = {0: 8, 1: 4, 2: 2}
 FALLBACK_HBM_GBS = 6650.0               # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fp32 D_w kernel at c3, from the committed
 # `ncu --set full` capture (profiles/r1b_dslash_fp32_c3.md).
-NCU_TRAFFIC_BYTES_FP32_C3 = 3681449528   # 3.259251 GB read + 0.422199 GB write (profiles/r1b_dslash_fp32_c3.md)
+NCU_TRAFFIC_BYTES_FP32_C3 = 3688318912   # 3.267128 GB read + 0.421191 GB write (profiles/r1d_dslash_fp32_c3.md)
 
 
 def measured_peak():
