@@ -146,18 +146,20 @@ __global__ void __launch_bounds__(128) cg_p_k(int Vh, const double* num, const d
 // fp16 sloppy operator with fp32 Krylov vectors (reading R12): the CG vectors x, r, p are kept in float,
 // only the operator's inputs (p, r) and outputs (t, s) are binary16.  Rounding x, r and p themselves to 11-bit
 // mantissas every iteration was measured to cost 2.8x the iterations of the fp32 solver at config c3.
-//   x += alpha p ; r -= alpha t(half) ; r16 = half(r) ; result = |r|^2
+//   x += alpha p16 ; r -= alpha t(half) ; r16 = half(r) ; result = |r|^2
+// x takes the binary16 direction the operator was applied to (t = A p16), so that x and r stay consistent (r = b - A x up
+// to fp32 rounding) and the fp32 p need not be read here.
 __global__ void __launch_bounds__(128) cg_xr_h_k(int Vh, const double* num, const double* den, SpinorPtr p, SpinorPtr t, SpinorPtr x,
                                                  SpinorPtr r, SpinorPtr r16, Reducer R, size_t rs_v, size_t rs_o, int ss, const double* act) {
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   double nrm[1] = {0.0};
   const int k = blockIdx.y;   // right-hand side (batched form, row a10): fp32 vectors rs_v bytes apart, binary16 ones rs_o
-  p = rhs_view(p, rs_v, k); x = rhs_view(x, rs_v, k); r = rhs_view(r, rs_v, k); t = rhs_view(t, rs_o, k); r16 = rhs_view(r16, rs_o, k);
+  p = rhs_view(p, rs_o, k); x = rhs_view(x, rs_v, k); r = rhs_view(r, rs_v, k); t = rhs_view(t, rs_o, k); r16 = rhs_view(r16, rs_o, k);
   if (cb < Vh) {
     const double dn = den[k * ss];
     const float al = (act && act[k] == 0.0) || dn == 0.0 ? 0.f : (float)(num[k * ss] / dn);
     float vp[24], vx[24];
-    load_spinor<float>(p, Vh, cb, vp);
+    load_spinor<__half>(p, Vh, cb, vp);
     load_spinor<float>(x, Vh, cb, vx);
 #pragma unroll
     for (int i = 0; i < 24; i++) vx[i] += al * vp[i];

@@ -119,7 +119,7 @@ int cgne(qxd_ctx* c, int pop, Ws& w0, double stop2, double delta, int maxiter, q
     double* gam = c->scal + SC_GAM0 + (it & 1);
     double* gam_next = c->scal + SC_GAM0 + ((it + 1) & 1);
     QXD_TRY(apply_dhat(c, pop, pin, w.t, w.tmp_o_lo, 0, c->scal + SC_TT));
-    if (h16) QXD_TRY(blas_cg_xr_h(c, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, r16, c->scal + SC_RR));
+    if (h16) QXD_TRY(blas_cg_xr_h(c, gam, c->scal + SC_TT, p16, w.t, w.xlo, w.rlo, r16, c->scal + SC_RR));
     else QXD_TRY(blas_cg_xr(c, plo, gam, c->scal + SC_TT, w.p, w.t, w.xlo, w.rlo, c->scal + SC_RR));
     // |r|^2 decides on the host whether to stop or to do a reliable update.  s = A^dag r is enqueued BEFORE the host waits
     // for it, so the GPU never idles on the round trip; it is only wasted (recomputed from the corrected r) in the
@@ -396,7 +396,7 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
     double* gam = ms + M_GAM0 + (it & 1);
     double* gam_next = ms + M_GAM0 + ((it + 1) & 1);
     QXD_TRY(apply_dhat(c, pop, pin, t, tmp_o, 0, ms + M_TT, bo));
-    if (h16) QXD_TRY(blas_cg_xr_h(c, gam, ms + M_TT, p, t, xlo, rlo, r16, ms + M_RR, bl, rs_op));
+    if (h16) QXD_TRY(blas_cg_xr_h(c, gam, ms + M_TT, p16, t, xlo, rlo, r16, ms + M_RR, bl, rs_op));
     else QXD_TRY(blas_cg_xr(c, plo, gam, ms + M_TT, p, t, xlo, rlo, ms + M_RR, bl));
     QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
     QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
