@@ -52,14 +52,52 @@ __global__ void __launch_bounds__(128) cxpaypbw_k(int Vh, SpinorPtr x, double ar
   store_spinor<S>(z, Vh, cb, vx);
 }
 
+// BiCGstab coefficients from the device-resident reduction results, so that the host need not read them back between the
+// kernels of an iteration (one round trip per iteration instead of three):
+//   alpha = rho / <r0,v>   (0 if <r0,v> vanishes: the step degenerates to the minimal-residual half, x and r stay consistent)
+//   omega = <t,s> / |t|^2  (0 if t vanishes; dst = (Re <s,t>, Im <s,t>, |t|^2) as cdot_k leaves it)
+constexpr double BICG_TINY = 1e-290;
+__device__ __forceinline__ void bicg_alpha(double rho_re, double rho_im, const double* r0v, double& ar, double& ai) {
+  const double br = r0v[0], bi = r0v[1], d = br * br + bi * bi;
+  if (d < BICG_TINY) { ar = 0.0; ai = 0.0; return; }
+  ar = (rho_re * br + rho_im * bi) / d; ai = (rho_im * br - rho_re * bi) / d;
+}
+__device__ __forceinline__ void bicg_omega(const double* dst, double& wr, double& wi) {
+  const double tt = dst[2];
+  if (!(tt > BICG_TINY)) { wr = 0.0; wi = 0.0; return; }
+  wr = dst[0] / tt; wi = -dst[1] / tt;
+}
+//   s = r - alpha v
+template <typename S>
+__global__ void __launch_bounds__(128) bicg_s_k(int Vh, double rho_re, double rho_im, const double* r0v, SpinorPtr r, SpinorPtr v, SpinorPtr s) {
+  typedef typename PT<S>::C C;
+  int cb = blockIdx.x * blockDim.x + threadIdx.x;
+  if (cb >= Vh) return;
+  double ar_, ai_;
+  bicg_alpha(rho_re, rho_im, r0v, ar_, ai_);
+  const C ar = (C)(-ar_), ai = (C)(-ai_);
+  C vx[24], vy[24];
+  load_spinor<S>(r, Vh, cb, vx);
+  load_spinor<S>(v, Vh, cb, vy);
+#pragma unroll
+  for (int k = 0; k < 12; k++) {
+    C yr = vy[2 * k], yi = vy[2 * k + 1];
+    vx[2 * k] += ar * yr - ai * yi;
+    vx[2 * k + 1] += ar * yi + ai * yr;
+  }
+  store_spinor<S>(s, Vh, cb, vx);
+}
 // BiCGstab, end of an iteration in one pass:  x += alpha p + omega s ;  r = s - omega t ;  result = (<r0,r>, |r|^2)
 template <typename S>
-__global__ void __launch_bounds__(128) bicg_xr_k(int Vh, double ar_, double ai_, double wr_, double wi_, SpinorPtr p, SpinorPtr s, SpinorPtr t,
-                                                 SpinorPtr r0, SpinorPtr x, SpinorPtr r, Reducer R) {
+__global__ void __launch_bounds__(128) bicg_xr_k(int Vh, double rho_re, double rho_im, const double* r0v, const double* dst, SpinorPtr p, SpinorPtr s,
+                                                 SpinorPtr t, SpinorPtr r0, SpinorPtr x, SpinorPtr r, Reducer R) {
   typedef typename PT<S>::C C;
   int cb = blockIdx.x * blockDim.x + threadIdx.x;
   double d[3] = {0.0, 0.0, 0.0};
   if (cb < Vh) {
+    double ar_, ai_, wr_, wi_;
+    bicg_alpha(rho_re, rho_im, r0v, ar_, ai_);
+    bicg_omega(dst, wr_, wi_);
     const C ar = (C)ar_, ai = (C)ai_, wr = (C)wr_, wi = (C)wi_;
     C vx[24], va[24], vs[24];
     load_spinor<S>(x, Vh, cb, vx);
@@ -327,9 +365,14 @@ int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
-int blas_bicg_xr(qxd_ctx* c, int prec, double ar, double ai, double wr, double wi, const SpinorPtr& p, const SpinorPtr& s,
+int blas_bicg_s(qxd_ctx* c, int prec, double rho_re, double rho_im, const double* r0v, const SpinorPtr& r, const SpinorPtr& v, const SpinorPtr& s) {
+  QXD_BY_PREC(prec, bicg_s_k<S><<<QXD_GRID>>>(c->g.Vh, rho_re, rho_im, r0v, r, v, s));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int blas_bicg_xr(qxd_ctx* c, int prec, double rho_re, double rho_im, const double* r0v, const double* dst, const SpinorPtr& p, const SpinorPtr& s,
                  const SpinorPtr& t, const SpinorPtr& r0, const SpinorPtr& x, const SpinorPtr& r, double* res3) {
-  QXD_BY_PREC(prec, bicg_xr_k<S><<<QXD_GRID>>>(c->g.Vh, ar, ai, wr, wi, p, s, t, r0, x, r, reducer(c, res3)));
+  QXD_BY_PREC(prec, bicg_xr_k<S><<<QXD_GRID>>>(c->g.Vh, rho_re, rho_im, r0v, dst, p, s, t, r0, x, r, reducer(c, res3)));
   QXD_FINALIZE(3, res3, 0, 1);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;

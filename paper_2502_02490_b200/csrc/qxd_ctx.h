@@ -155,8 +155,9 @@ int blas_zero(qxd_ctx* c, int prec, const SpinorPtr& x, const Batch& b = Batch()
 int blas_cxpaypbw(qxd_ctx* c, int prec, const SpinorPtr& x, double ar, double ai, const SpinorPtr& y, double br, double bi,
                   const SpinorPtr& w, const SpinorPtr& z);
 // BiCGstab: x += alpha p + omega s ; r = s - omega t ; res3 = (Re<r0,r>, Im<r0,r>, |r|^2)
-int blas_bicg_xr(qxd_ctx* c, int prec, double ar, double ai, double wr, double wi, const SpinorPtr& p, const SpinorPtr& s,
-                 const SpinorPtr& t, const SpinorPtr& r0, const SpinorPtr& x, const SpinorPtr& r, double* dev_result3);
+int blas_bicg_s(qxd_ctx* c, int prec, double rho_re, double rho_im, const double* r0v, const SpinorPtr& r, const SpinorPtr& v, const SpinorPtr& s);
+int blas_bicg_xr(qxd_ctx* c, int prec, double rho_re, double rho_im, const double* r0v, const double* dst, const SpinorPtr& p, const SpinorPtr& s,
+                 const SpinorPtr& t, const SpinorPtr& r0, const SpinorPtr& x, const SpinorPtr& r, double* res3);
 // alpha = *num / *den (device scalars): x += alpha p ; r -= alpha t ; *rr = |r|^2
 int blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const SpinorPtr& p, const SpinorPtr& t, const SpinorPtr& x,
                const SpinorPtr& r, double* rr, const Batch& b = Batch());

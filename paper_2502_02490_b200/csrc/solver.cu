@@ -15,7 +15,7 @@ namespace qxd {
 
 namespace {
 
-enum { SC_GAM0 = 0, SC_GAM1 = 1, SC_TT = 2, SC_RR = 3, SC_RRT = 4, SC_NE = 5, SC_NO = 6, SC_DOT = 8 /* 3 slots */, SC_DOT2 = 12 };
+enum { SC_GAM0 = 0, SC_GAM1 = 1, SC_TT = 2, SC_RR = 3, SC_RRT = 4, SC_NE = 5, SC_NO = 6, SC_DOT = 8 /* 9 slots: <r0,v>, <s,t> and |t|^2, <r0,r> and |r|^2 of a BiCGstab iteration */ };
 
 struct Ws {
   int Vh;
@@ -181,29 +181,27 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
   double best_true = rr;
   QXD_TRY(blas_zero(c, 0, w.xbest));
   while (status != QXD_OK && it < maxiter) {
+    if (cabs2(rho) < tiny) break;
+    // alpha and omega are formed on the device from the reduction results (blas.cu: bicg_alpha, bicg_omega), so the six
+    // kernels of an iteration are enqueued back to back; the host reads all nine scalars once, at the end
     QXD_TRY(apply_dhat(c, plo, w.p, w.v, w.tmp_o_lo, 0, nullptr));                 // v = A p
-    QXD_TRY(blas_cdot(c, plo, w.r0, w.v, c->scal + SC_DOT));
-    QXD_TRY(read_scal(c, SC_DOT, 3, d3));
-    cplx r0v = {d3[0], d3[1]};
-    if (cabs2(r0v) < tiny || cabs2(rho) < tiny) break;
-    cplx alpha = cdiv(rho, r0v);
-    QXD_TRY(blas_cxpaypbw(c, plo, w.rlo, -alpha.re, -alpha.im, w.v, 0, 0, w.v, w.s));   // s = r - alpha v
+    QXD_TRY(blas_cdot(c, plo, w.r0, w.v, c->scal + SC_DOT));                        // <r0,v>
+    QXD_TRY(blas_bicg_s(c, plo, rho.re, rho.im, c->scal + SC_DOT, w.rlo, w.v, w.s));   // s = r - alpha v
     QXD_TRY(apply_dhat(c, plo, w.s, w.t, w.tmp_o_lo, 0, nullptr));                 // t = A s
-    QXD_TRY(blas_cdot(c, plo, w.s, w.t, c->scal + SC_DOT));                         // <s,t> = conj <t,s>, |t|^2 in one pass
-    double d5[3];
-    QXD_TRY(read_scal(c, SC_DOT, 3, d5));
-    cplx ts = {d5[0], -d5[1]};
-    double tt = d5[2];
-    if (!(tt > tiny)) {  // t = 0: s is already the exact residual update
-      QXD_TRY(blas_cxpaypbw(c, plo, w.xlo, alpha.re, alpha.im, w.p, 0, 0, w.p, w.xlo));
-      QXD_TRY(blas_copy(c, plo, w.s, w.rlo));
-      it++;
-      break;
-    }
-    cplx omega = {ts.re / tt, ts.im / tt};
+    QXD_TRY(blas_cdot(c, plo, w.s, w.t, c->scal + SC_DOT + 3));                     // <s,t> = conj <t,s>, |t|^2 in one pass
     // x += alpha p + omega s ; r = s - omega t ; rho' = <r0,r>, |r|^2 -- one kernel
-    QXD_TRY(blas_bicg_xr(c, plo, alpha.re, alpha.im, omega.re, omega.im, w.p, w.s, w.t, w.r0, w.xlo, w.rlo, c->scal + SC_DOT));
-    QXD_TRY(read_scal(c, SC_DOT, 3, d3));
+    QXD_TRY(blas_bicg_xr(c, plo, rho.re, rho.im, c->scal + SC_DOT, c->scal + SC_DOT + 3, w.p, w.s, w.t, w.r0, w.xlo, w.rlo, c->scal + SC_DOT + 6));
+    double d9[9];
+    QXD_TRY(read_scal(c, SC_DOT, 9, d9));
+    cplx r0v = {d9[0], d9[1]};
+    cplx ts = {d9[3], -d9[4]};
+    const double tt = d9[5];
+    d3[0] = d9[6]; d3[1] = d9[7]; d3[2] = d9[8];
+    // the degenerate steps the device took with alpha = 0 or omega = 0 (x and r consistent either way) end the iteration
+    if (cabs2(r0v) < tiny) { it++; break; }
+    cplx alpha = cdiv(rho, r0v);
+    if (!(tt > tiny)) { it++; break; }   // t = 0: s was already the exact residual update (the device used omega = 0)
+    cplx omega = {ts.re / tt, ts.im / tt};
     it++;
     cplx rho_new = {d3[0], d3[1]};
     rr = d3[2];
