@@ -94,6 +94,9 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   if (d.flags & DSF_NORM) {   // second kernel of the fused norm: add the per-tile partials (qxd_common.cuh)
     reduce_finalize_k<1><<<dim3(1, a.nrhs), FINALIZE_THREADS, 0, c->stream>>>(a.R, (c->g.Vh + 127) / 128);
     QXD_LAUNCH_CHECK(c);
+  } else if (d.flags & DSF_DOT) {
+    reduce_finalize_k<3><<<dim3(1, a.nrhs), FINALIZE_THREADS, 0, c->stream>>>(a.R, (c->g.Vh + 127) / 128);
+    QXD_LAUNCH_CHECK(c);
   }
   return QXD_OK;
 }

@@ -412,9 +412,12 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
   const int tile = tile_of(a.tm, SPLIT ? (bt >> 1) : bt);
   const int cb = tile * 128 + (threadIdx.x & 127);
   const int parity = FULL ? (SPLIT ? (bt & 1) : (threadIdx.x >> 7)) : a.parity_out;
-  double nrm[R];
+  constexpr int NRED = (FLAGS & DSF_DOT) ? 3 : 1;   // fused reductions: |out|^2, or <phi,out> and |out|^2
+  double nrm[R][NRED];
 #pragma unroll
-  for (int r = 0; r < R; r++) nrm[r] = 0.0;
+  for (int r = 0; r < R; r++)
+#pragma unroll
+    for (int k = 0; k < NRED; k++) nrm[r][k] = 0.0;
   if (cb < Vh) {
     Site s;
     site_init<PAIR ? 1 : 0>(a.g, cb, parity, s);
@@ -461,22 +464,33 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
 #pragma unroll
     for (int r = 0; r < R; r++) {
       if (R > 1 && rhs0 + r >= a.nrhs) break;
-      if (FLAGS & DSF_NORM) {   // per-site sum in the arithmetic type, fp64 across sites (see blas.cu)
+      if (FLAGS & DSF_DOT) {    // BiCGstab's <s,t> and |t|^2 for t = A s: phi = s is re-read (L1/L2) rather than kept in registers
+        C ph[24];
+        load_spinor<S>(rhs_view(a.phi, a.rs_phi, rhs0 + r), Vh, cb, ph);
+        C p0 = 0, p1 = 0, p2 = 0;
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+          const C xr = ph[2 * k], xi = ph[2 * k + 1], yr = acc[r][2 * k], yi = acc[r][2 * k + 1];
+          p0 += xr * yr; p0 += xi * yi;
+          p1 += xr * yi; p1 -= xi * yr;
+          p2 += yr * yr; p2 += yi * yi;
+        }
+        nrm[r][0] = (double)p0; nrm[r][NRED > 1 ? 1 : 0] = (double)p1; nrm[r][NRED - 1] = (double)p2;
+      } else if (FLAGS & DSF_NORM) {   // per-site sum in the arithmetic type, fp64 across sites (see blas.cu)
         C part = 0;
 #pragma unroll
         for (int i = 0; i < 24; i++) part += acc[r][i] * acc[r][i];
-        nrm[r] = (double)part;
+        nrm[r][0] = (double)part;
       }
       store_spinor<S>(rhs_view(a.out[parity], a.rs_out, rhs0 + r), Vh, cb, acc[r]);
     }
   }
-  if (FLAGS & DSF_NORM) {
+  if (FLAGS & (DSF_NORM | DSF_DOT)) {
     const int ntiles = gridDim.x / a.ngroups;
 #pragma unroll
     for (int r = 0; r < R; r++) {
       if (R > 1 && rhs0 + r >= a.nrhs) break;   // uniform over the CTA
-      double v[1] = {nrm[r]};
-      grid_reduce<1>(v, a.R, tile, ntiles, rhs0 + r);
+      grid_reduce<NRED>(nrm[r], a.R, tile, ntiles, rhs0 + r);
     }
   }
 }
@@ -521,6 +535,7 @@ int dispatch(qxd_ctx* c, const DslashCall& d, DslashArgs& a) {
     case DS_A_XMHOP:
       if (f == 0) { return launch_one<S, NL, PAIR, 2, 0, true, 0, false, true>(c, a); }
       if (f == DSF_NORM) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_NORM, false, true>(c, a); }
+      if (f == DSF_DOT) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_DOT, false, false>(c, a); }
       if (f == DSF_G5HOP) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_G5HOP, false, true>(c, a); }
       if (f == (DSF_G5HOP | DSF_NORM)) { return launch_one<S, NL, PAIR, 2, 0, true, DSF_G5HOP | DSF_NORM, false, true>(c, a); }
       break;

@@ -21,7 +21,7 @@ enum DslashMode {
   DS_AINV_X_MHOP,   // out_p = M^{-1} (phi - hop(in))               odd-site reconstruction       (row a8)
   DS_NMODES
 };
-enum { DSF_G5IN = 1, DSF_G5HOP = 2, DSF_NORM = 4 };
+enum { DSF_G5IN = 1, DSF_G5HOP = 2, DSF_NORM = 4, DSF_DOT = 8 };
 
 struct Scalars;  // device-resident solver scalars (solver.cu)
 
@@ -128,7 +128,8 @@ struct DslashCall {
   SpinorPtr in[2];  // input spinor per parity (hop reads in[1-p]; DS_DW_FULL also in[p])
   SpinorPtr phi;    // PHI-term input on the output parity (modes with phi)
   SpinorPtr out[2]; // output per parity (only [parity_out] used unless DS_DW_FULL)
-  double* norm_result;  // DSF_NORM: device slot receiving |out|^2 (right-hand side r: norm_result[r * norm_stride])
+  double* norm_result;  // DSF_NORM: device slot receiving |out|^2 (right-hand side r: norm_result[r * norm_stride]);
+                        // DSF_DOT: three slots receiving Re <phi,out>, Im <phi,out>, |out|^2
   // multi-RHS launches (row a10): nrhs > 1 right-hand sides, rs_* bytes apart in in / phi / out
   int nrhs;
   size_t rs_in, rs_phi, rs_out;

@@ -69,6 +69,20 @@ int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out
   QXD_TRY(launch_dslash(c, d2));
   return QXD_OK;
 }
+// out_e = D-hat in_e with the fused reduction dot_slot[0..2] = (Re <in,out>, Im <in,out>, |out|^2)
+int apply_dhat_dot(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out_e, const SpinorPtr& tmp_o, double* dot_slot) {
+  DslashCall d1{};
+  d1.prec = prec; d1.mode = DS_HOP_AINV; d1.flags = 0; d1.parity_out = 1;
+  d1.in[0] = in_e; d1.out[1] = tmp_o;
+  d1.nrhs = 1;
+  QXD_TRY(launch_dslash(c, d1));
+  DslashCall d2{};
+  d2.prec = prec; d2.mode = DS_A_XMHOP; d2.flags = DSF_DOT; d2.parity_out = 0;
+  d2.in[1] = tmp_o; d2.phi = in_e; d2.out[0] = out_e; d2.norm_result = dot_slot; d2.norm_stride = 0;
+  d2.nrhs = 1;
+  QXD_TRY(launch_dslash(c, d2));
+  return QXD_OK;
+}
 int apply_dhat(qxd_ctx* c, int prec, const SpinorPtr& in_e, const SpinorPtr& out_e, const SpinorPtr& tmp_o, int dagger, double* norm_slot) {
   return apply_dhat(c, prec, in_e, out_e, tmp_o, dagger, norm_slot, Batch());
 }
@@ -187,8 +201,7 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
     QXD_TRY(apply_dhat(c, plo, w.p, w.v, w.tmp_o_lo, 0, nullptr));                 // v = A p
     QXD_TRY(blas_cdot(c, plo, w.r0, w.v, c->scal + SC_DOT));                        // <r0,v>
     QXD_TRY(blas_bicg_s(c, plo, rho.re, rho.im, c->scal + SC_DOT, w.rlo, w.v, w.s));   // s = r - alpha v
-    QXD_TRY(apply_dhat(c, plo, w.s, w.t, w.tmp_o_lo, 0, nullptr));                 // t = A s
-    QXD_TRY(blas_cdot(c, plo, w.s, w.t, c->scal + SC_DOT + 3));                     // <s,t> = conj <t,s>, |t|^2 in one pass
+    QXD_TRY(apply_dhat_dot(c, plo, w.s, w.t, w.tmp_o_lo, c->scal + SC_DOT + 3));   // t = A s with <s,t> = conj <t,s> and |t|^2 fused
     // x += alpha p + omega s ; r = s - omega t ; rho' = <r0,r>, |r|^2 -- one kernel
     QXD_TRY(blas_bicg_xr(c, plo, rho.re, rho.im, c->scal + SC_DOT, c->scal + SC_DOT + 3, w.p, w.s, w.t, w.r0, w.xlo, w.rlo, c->scal + SC_DOT + 6));
     double d9[9];
