@@ -22,8 +22,12 @@
 // (apply and solve), gamma5-hermiticity, SU(3)xU(1) gauge covariance, C* charge-conjugation
 // symmetry, csw=0 -> Wilson, uniform abelian background clover closed form, SU(3)-formula
 // on U(3) links -> q*A-hat, dense-matrix brute force with LU on 4^4 (independent numpy
-// assembler).  PARITY UNPINNED: the overall sign of the SW term and the gamma-basis
-// relative to the paper's host code (the paper prints no operator values).
+// assembler); the SIGN of both SW terms by tree-level O(a) improvement: in a uniform abelian
+// background the lowest Landau level of gamma5 D_w sits at (1 - c_sw) B/2 + O(B^2)
+// (test_sw_term_sign_is_the_improving_one; "O(a)-improved").
+// PARITY UNPINNED: only the choice of gamma-basis (ordering of the spin components at the
+// ABI) relative to the paper's host code -- the paper prints no operator values; every
+// chiral basis gives the same operator up to a fixed unitary change of spin components.
 // =====================================================================================
 #include <complex>
 #include <vector>

@@ -325,3 +325,65 @@ def test_reconstruct_identity_for_u3_links():
     assert np.allclose(np.linalg.det(U), 1.0, atol=1e-13)
     row2 = det[:, None] * np.conj(np.cross(W[:, 0, :], W[:, 1, :]))
     assert np.max(np.abs(row2 - W[:, 2, :])) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------
+# Sign of the Sheikholeslami-Wohlert term, pinned by what "O(a)-improved" means (PAPER.md:3 title).
+# Continuum: (gamma.D)^2 = D^2 + (1/2) sigma.F, so in a uniform magnetic field B the massless Dirac operator has exact zero
+# modes (lowest Landau level: |B| from -D^2 cancels against sigma.F).  The Wilson term -(a/2) D^2 = -(a/2)[(gamma.D)^2 -
+# (1/2) sigma.F] lifts them by (a/2)|B|; the SW term with the right sign and c_sw = 1 (tree level) puts them back up to
+# O(a^2).  In lattice units (B = 2 pi k / L^2 on an L x L torus, m0 = 0) the lowest |eigenvalue| of gamma5 D_w must be
+#     c_sw = +1:  O(B^2)  (falls like L^-4: ratio ~16 when L doubles)      c_sw = 0:  B/2        c_sw = -1:  B
+# A flipped sign of the SW term in the oracle (reading R4: +c_sw (i/4) sigma.F-hat with F-hat = (Q - Q^dag)/8) would swap
+# the first and the last line.  Nothing here restates the oracle's formula: the expected values are continuum Landau-level
+# algebra.  Both SW terms are tested: the U(1) one (A-hat, csw_qed) and the SU(3) one on U(3) links e^{iA} 1.
+# ------------------------------------------------------------------------------------------
+def _lowest_landau_level(L, c, mode, k=1):
+    """Lowest |eigenvalues| of gamma5 D_w (kappa = 1/8, i.e. m0 = 0) in the sector of zero momentum in directions 0 and 3,
+    uniform flux 2 pi k through the (1,2) torus of size L x L; returns (sorted |eigenvalues|, B)."""
+    dims = (2, L, L, 2)
+    B = 2 * np.pi * k / L**2
+    A = np.zeros(dims + (4,))
+    x1 = np.arange(L).reshape(1, L, 1, 1)
+    x2 = np.arange(L).reshape(1, 1, L, 1)
+    A[..., 2] = B * x1                                   # A_2 = B x_1
+    A[:, L - 1, :, :, 1] = (-B * L * x2)[:, 0]           # transition function on the last x_1 slice: every plaquette has angle B mod 2 pi
+    one = np.zeros(dims + (4, 3, 3), dtype=complex)
+    one[...] = np.eye(3)
+    r = R.Ref(*dims, 0)                                  # periodic in all directions (zero-momentum sector exists)
+    if mode == "u1":
+        r.gauge_load(one, A, 1.0)
+        r.set_quark(0.125, 1.0)
+        r.clover_build(0.0, c)
+    else:
+        r.gauge_load(np.exp(1j * A)[..., None, None] * np.eye(3), None, 1.0)
+        r.set_quark(0.125, 0.0)
+        r.clover_build(c, 0.0)
+    n = 12 * L * L
+    M = np.zeros((n, n), dtype=complex)
+    for j in range(n):                                   # the operator restricted to fields constant in x0, x3
+        v = np.zeros((L * L, 12), dtype=complex)
+        v[j // 12, j % 12] = 1.0
+        psi = np.ascontiguousarray(np.broadcast_to(v.reshape(1, L, L, 1, 4, 3), dims + (4, 3)))
+        out = r.apply_Dw(psi).reshape(2, L, L, 2, 12)
+        assert np.abs(out - out[:1, :, :, :1]).max() < 1e-13
+        M[:, j] = out[0, :, :, 0].reshape(-1)
+    g5 = np.tile(np.repeat([1.0, 1.0, -1.0, -1.0], 3), L * L)
+    ev = np.linalg.eigvalsh(g5[:, None] * M)
+    return np.sort(np.abs(ev)), B
+
+
+@pytest.mark.parametrize("mode", ["u1", "su3"])
+def test_sw_term_sign_is_the_improving_one(mode):
+    low = {}
+    for L in (6, 12):
+        for c in (1.0, 0.0, -1.0):
+            ev, B = _lowest_landau_level(L, c, mode)
+            low[L, c] = ev[0] / B
+            assert ev[6] / B > 2.0                       # the six lowest-Landau-level modes are separated from the rest
+    for L in (6, 12):
+        assert abs(low[L, 0.0] - 0.5) < 0.02             # Wilson term alone: (a/2)|B|
+        assert abs(low[L, -1.0] - 1.0) < 0.02            # wrong sign: doubled
+        assert low[L, 1.0] < 0.02                        # c_sw = +1: the O(a) shift is gone
+    # what is left at c_sw = +1 is O(a^2): lambda ~ B^2 ~ L^-4  (lambda/B ~ L^-2: ratio 4 when L doubles)
+    assert 3.0 < low[6, 1.0] / low[12, 1.0] < 5.0
