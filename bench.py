@@ -36,9 +36,25 @@ REALS_DHAT = 276                        # both passes, per FULL-lattice site (ro
 PREC_NAME = {0: "fp64", 1: "fp32", 2: "fp16"}
 PREC_BYTES = {0: 8, 1: 4, 2: 2}
 FALLBACK_HBM_GBS = 6650.0               # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fp32 D_w kernel at c3, from the committed
-# `ncu --set full` capture (profiles/r1b_dslash_fp32_c3.md).
-NCU_TRAFFIC_BYTES_FP32_C3 = 3688318912   # 3.267128 GB read + 0.421191 GB write (profiles/r1d_dslash_fp32_c3.md)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the headline kernel, from committed `ncu --set full` captures,
+# keyed by what the capture was taken on: (config, storage precision, stored reals per link, layout).  Any other
+# combination reports "traffic": null (a capture of another lattice says nothing about this one).
+NCU_TRAFFIC = {
+    ("c3", 1, 18, "extended"): (3688318912, "profiles/r1d_dslash_fp32_c3.md"),   # 3.267128 GB read + 0.421191 GB write
+}
+
+
+def ncu_traffic(config, prec, link_reals, layout):
+    t = NCU_TRAFFIC.get((config, prec, link_reals, layout))
+    return (t[0], t[1]) if t else (None, None)
+
+
+def config_object(cfg, V):
+    """The `config` object of the JSON line: identical in the CUDA arm and in the reference arm."""
+    fp32_ws_gb = V * (24 + 72 + 72 + 24) * 4 / 1e9
+    return {"workload": cfg["label"], "sites_per_gpu": V, "layout": "even-odd tiled SoA, 16-byte chunks, 18-real links",
+            "l2": f"inputs larger than L2 (fp32 working set {fp32_ws_gb:.1f} GB vs 126 MB), no flush",
+            "sharding": "by right-hand side, replicated gauge field"}
 
 
 def measured_peak():
@@ -153,18 +169,50 @@ def oracle_sample(cfg, U, A, psi, steps, warmup, budget_s=25.0):
     return n / dt, R.num_threads(), desc, dt, len(times)
 
 
+def oracle_solve_baseline(cfg, U, A, eta, oref, solves):
+    """BASELINE.md §4 / SURVEY.md §8(d) "Oracle timing": the oracle's own even-odd CGNE (fp64, as it stands), timed in full on
+    config c2 and for 10 iterations on the benchmarked configuration, the latter EXTRAPOLATED to the iteration count of the
+    GPU's fp64/fp32 CGNE (iteration counts of CG on the same system agree to a few per cent between precisions)."""
+    import synth
+    from oracle import qxd_ref as R
+    out = {"cores": R.num_threads(), "kind": "oracle"}
+    c2 = synth.config("c2")
+    r2 = R.Ref(*c2["dims"], c2["bc"])
+    r2.gauge_load(synth.su3_links(c2["dims"], c2["eps"], 1), synth.u1_field(c2["dims"], 0.3, 2) if c2["qed"] else None, c2["qel"])
+    r2.set_quark(c2["kappa"], c2["q"])
+    r2.clover_build(c2["csw"], c2["csw_qed"])
+    e2 = synth.gaussian_spinor(c2["dims_ext"], 3)
+    t0 = time.perf_counter()
+    _, info = r2.solve(e2, c2["tol"])
+    out["c2_full_solve"] = {"seconds": time.perf_counter() - t0, "iters": info["iters"], "relres": info["relres"], "status": info["status"],
+                            "tol": c2["tol"], "sites": r2.V}
+    del r2, e2
+    if oref is not None and cfg["name"] != "c2":
+        t0 = time.perf_counter()
+        _, info = oref.solve(eta, cfg["tol"], maxiter=10)
+        dt = time.perf_counter() - t0
+        ref_it = (solves.get("cgne_fp64_fp32") or {}).get("iters")
+        out[cfg["name"] + "_10_iterations"] = {"seconds": dt, "iters": info["iters"], "sites": oref.V,
+                                               "note": "includes source preparation and reconstruction (3 dslash-like passes)"}
+        if ref_it:
+            out[cfg["name"] + "_extrapolated_solve"] = {"seconds": dt / max(info["iters"], 1) * ref_it, "iters_assumed": ref_it,
+                                                        "note": "EXTRAPOLATION: seconds per oracle iteration x iterations of the GPU fp64/fp32 CGNE"}
+    return out
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     U, A, psi = make_fields(cfg, 0)
-    rate, cores, desc, dt, done = oracle_sample(cfg, U, A, psi, args.steps, min(args.warmup, 2))
+    rate, cores, desc, dt, done = oracle_sample(cfg, U, A, psi, args.steps, args.warmup, budget_s=150.0)
     gbs = rate * dw_bytes_per_site(1) / 1e9
     line = {
         "impl": "reference", "metric": "Dw_apply_fp32_GBps", "value": gbs, "unit": "GB/s", "n_gpus": args.gpus, "steps": done,
-        "warmup": min(args.warmup, 2), "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["label"], "note": "sites/s of the fp64 oracle x 768 B/site (the fp32 algorithmic bytes of the CUDA arm)"},
+        "config": config_object(cfg, psi.size // 12),
+        "note": "sites/s of the fp64 oracle on the host cores x 768 B/site (the fp32 algorithmic bytes of the CUDA arm)",
         "gflops": rate * FLOP_PER_SITE / 1e9,
         "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -258,11 +306,36 @@ def run_cuda(args, cfg):
     barrier()
     launches = g.launch_count() - l0
     ms_step = max_over_ranks(e0.elapsed_time(e1) / args.steps)
-    # keep the sampler running through the sweep below so that it sees >= a few samples under load
     sites_per_s = world * V / (ms_step * 1e-3)
     value = sites_per_s * dw_bytes_per_site(hp) / 1e9
     peak, peak_src = measured_peak()
     per_gpu_gbs = value / world
+
+    # ---- sustained: the same apply kept running for >= args.sustain_s seconds whatever --steps says (a solver runs for
+    # 0.3 s, not 11 ms): events every 100 applies, median of the per-100 intervals, clocks sampled over this window only
+    sustained = None
+    if args.sustain_s > 0:
+        s2 = ClockSampler(local)
+        nblk = max(3, int(args.sustain_s * 1e3 / (100 * ms_step)) + 1)
+        evs = [ev() for _ in range(nblk + 1)]
+        torch.cuda.synchronize(dev)
+        s2.start()
+        evs[0].record()
+        for b in range(nblk):
+            for _ in range(100):
+                step()
+            evs[b + 1].record()
+        evs[-1].synchronize()
+        ck = s2.stop()
+        per100 = sorted(evs[b].elapsed_time(evs[b + 1]) / 100 for b in range(nblk))
+        ms_med = max_over_ranks(per100[len(per100) // 2])
+        gbs = V * dw_bytes_per_site(hp) / (ms_med * 1e-3) / 1e9
+        sustained = {"applies": 100 * nblk, "seconds": evs[0].elapsed_time(evs[-1]) * 1e-3, "ms_per_step_median": ms_med,
+                     "ms_per_step_min": per100[0], "ms_per_step_max": per100[-1], "value": gbs * world, "unit": "GB/s",
+                     "frac": gbs / peak, "frac_of_nominal_8000": gbs / 8000.0, "clocks": ck}
+    # the headline sampler ran through the --steps region and the sustained window of the same kernel (a 100 ms nvidia-smi
+    # cadence cannot resolve a --steps region of a few ms by itself)
+    clocks = sampler.stop()
 
     # ---- sweep: D_w and D-hat in the three storage precisions, BLAS streams (rank-local numbers) ----------
     # link formats: 18 stored reals (full) and 14 (12-real reconstruct + det W, qxd_set_gauge_reconstruct)
@@ -292,7 +365,6 @@ def run_cuda(args, cfg):
                 e["axpy_GBps"] = 3 * 24 * PREC_BYTES[p] * (V // 2) / ms_axpy / 1e6
             sweep[PREC_NAME[p] + tag] = e
     g.set_gauge_reconstruct(B.QXD_RECON_NONE)
-    clocks = sampler.stop()
 
     # ---- multi-RHS D_w (row a10): links and clover blocks read once for a batch of right-hand sides --------
     multi = {}
@@ -383,56 +455,103 @@ def run_cuda(args, cfg):
     del Ud, Ad
 
     # ---- solves (rows a7, a8): fp64/fp16 and fp64/fp32 mixed CGNE, BiCGstab ------------------------------
+    # Every solve is judged twice: by the library's own fp64 residual (true_res) and, outside the timed region, by
+    # ||eta - D_ref psi|| / ||eta|| over the WHOLE lattice with the ORACLE's D_w (true_res_oracle).
     solves = {}
+    oref = None
+    want_oracle = rank == 0 and world == 1 and not args.no_oracle_residual and not args.no_solve
+
+    def oracle_residual(eta_np, psi_t):
+        nonlocal oref
+        if not want_oracle:
+            return None
+        if oref is None:
+            from oracle import qxd_ref as R
+            oref = R.Ref(*cfg["dims"], cfg["bc"])
+            oref.gauge_load(U, A, cfg["qel"])
+            oref.set_quark(cfg["kappa"], cfg["q"])
+            oref.clover_build(cfg["csw"], cfg["csw_qed"])
+        r = eta_np.reshape(-1) - oref.apply_Dw(psi_t.cpu().numpy()).reshape(-1)
+        return float(np.linalg.norm(r) / np.linalg.norm(eta_np.reshape(-1)))
+
+    e2e_solve = None
     if not args.no_solve:
         # link format per storage precision as measured best: 14 reals (12-real reconstruct) where the dslash is bandwidth
         # bound (fp64, fp32), 18 reals in fp16 (issue bound)
         g.set_gauge_reconstruct(B.QXD_RECON_12)
         g.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=B.QXD_F16)
         psi_d = torch.empty_like(eta_d)
-        for name, algo, sl in (("cgne_fp64_fp16", B.QXD_CGNE, B.QXD_F16), ("cgne_fp64_fp32", B.QXD_CGNE, B.QXD_F32),
-                               ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32), ("bicgstab_fp64_fp16", B.QXD_BICGSTAB, B.QXD_F16)):
+        runs = [("cgne_fp64_fp16", B.QXD_CGNE, B.QXD_F16, cfg["tol"]), ("cgne_fp64_fp32", B.QXD_CGNE, B.QXD_F32, cfg["tol"]),
+                ("bicgstab_fp64_fp32", B.QXD_BICGSTAB, B.QXD_F32, cfg["tol"]), ("bicgstab_fp64_fp16", B.QXD_BICGSTAB, B.QXD_F16, cfg["tol"])]
+        if cfg["tol"] > 1e-12:   # the paper's own target for all solves, beside BASELINE.json's 1e-10
+            runs += [("cgne_fp64_fp16_tol1e-12", B.QXD_CGNE, B.QXD_F16, 1e-12), ("cgne_fp64_fp32_tol1e-12", B.QXD_CGNE, B.QXD_F32, 1e-12)]
+        for name, algo, sl, tol in runs:
             l0 = g.launch_count()
-            _, info = g.solve(eta_d, cfg["tol"], algo=algo, sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psi_d)
+            _, info = g.solve(eta_d, tol, algo=algo, sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psi_d)
             info["launches"] = g.launch_count() - l0
-            info["tol"] = cfg["tol"]
+            info["tol"] = tol
             info["links"] = "fp64/fp32: recon12, fp16: 18 reals"
             info["layout"] = "C*-paired" if pairing else "extended lattice"
+            info["true_res_oracle"] = oracle_residual(eta, psi_d)
             solves[name] = info
+        # end to end through the host-pointer call (the invertQuda boundary of PAPER.md:73-79): pinned eta in, pinned psi out
+        if not args.no_e2e:
+            ph = torch.empty_like(eh).pin_memory()
+            t0 = time.perf_counter()
+            _, info = g.solve_host(eh, ph, cfg["tol"], algo=B.QXD_CGNE, sloppy=B.QXD_F16, delta=0.1, maxiter=args.maxiter)
+            e2e_solve = {"seconds": time.perf_counter() - t0, "call": "qxd_solve_host (pinned host fp64 eta in, psi out), fp64/fp16 CGNE",
+                         "tol": cfg["tol"], "iters": info["iters"], "status": info["status"], "true_res": info["true_res"],
+                         "seconds_device_part": info["seconds"], "h2d_bytes": io_bytes, "d2h_bytes": io_bytes,
+                         "true_res_oracle": oracle_residual(eta, ph)}
+            del ph
+        del psi_d
         if args.nrhs > 1:
-            etas = torch.stack([eta_d] + [torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + k)).to(dev) for k in range(1, args.nrhs)])
+            etas = torch.empty((args.nrhs,) + tuple(eta_d.shape), dtype=eta_d.dtype, device=dev)
+            etas[0].copy_(eta_d)
+            for k in range(1, args.nrhs):
+                etas[k].copy_(torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + k)))
+            psis = torch.empty_like(etas) if torch.cuda.mem_get_info(dev)[0] > 1.2 * etas.numel() * 16 else None
             for sl, tag, links in ((B.QXD_F32, "fp32", "recon12"), (B.QXD_F16, "fp16", "fp64: recon12, fp16: 18 reals")):
+                if psis is None and tag == "fp16":
+                    break            # in-place solve (no room for a second batch of spinors): the sources are gone after the first run
                 l0 = g.launch_count()
                 t0 = time.perf_counter()
-                _, infos = g.solve_multi(etas, cfg["tol"], sloppy=sl, delta=0.1, maxiter=args.maxiter)
+                out, infos = g.solve_multi(etas, cfg["tol"], sloppy=sl, delta=0.1, maxiter=args.maxiter, psi=psis if psis is not None else etas)
                 torch.cuda.synchronize(dev)
                 dt = time.perf_counter() - t0
+                kk = args.nrhs - 1
+                eta_k = eta if kk == 0 else synth_mod.gaussian_spinor(cfg["dims_ext"], 40 + kk)
                 solves[f"cgne_multi{args.nrhs}_fp64_{tag}"] = {
                     "status": max(abs(i["status"]) for i in infos), "iters_max": max(i["iters"] for i in infos),
                     "true_res_max": max(i["true_res"] for i in infos), "seconds": dt, "seconds_per_rhs": dt / args.nrhs,
-                    "launches": g.launch_count() - l0, "tol": cfg["tol"], "links": links}
-            del etas
+                    "launches": g.launch_count() - l0, "tol": cfg["tol"], "links": links,
+                    "true_res_oracle_last_rhs": oracle_residual(eta_k, out.reshape(etas.shape)[kk])}
+            del etas, psis
         g.set_gauge_reconstruct(B.QXD_RECON_NONE)
 
     # ---- CPU baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----------------------------
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rate, cores, desc, dt, done = oracle_sample(cfg, U, A, eta, 40, 1, budget_s=15.0)
+        rate, cores, desc, dt, done = oracle_sample(cfg, U, A, eta, 40, 1, budget_s=10.0)
         cpu_baseline = {"value": rate * dw_bytes_per_site(hp) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": desc,
                         "sites_per_s": rate, "gflops": rate * FLOP_PER_SITE / 1e9}
+        if not args.no_solve:
+            cpu_baseline["solve"] = oracle_solve_baseline(cfg, U, A, eta, oref, solves)
 
+    traffic, traffic_src = ncu_traffic(cfg["name"], hp, 18, "extended")
     if rank == 0:
         line = {
             "metric": "Dw_apply_fp32_GBps", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["label"], "sites_per_gpu": V, "layout": "even-odd tiled SoA, 16-byte chunks, 18-real links",
-                       "l2": "inputs larger than L2 (fp32 working set 3.2 GB vs 126 MB), no flush", "sharding": "by right-hand side, replicated gauge field"},
+            "config": config_object(cfg, V),
             "gflops": sites_per_s * FLOP_PER_SITE / 1e9,
             "roofline": {"bound": "hbm", "achieved": per_gpu_gbs, "peak": peak, "unit": "GB/s", "frac": per_gpu_gbs / peak,
-                         "traffic": NCU_TRAFFIC_BYTES_FP32_C3, "peak_source": peak_src, "frac_of_nominal_8000": per_gpu_gbs / 8000.0,
+                         "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src, "frac_of_nominal_8000": per_gpu_gbs / 8000.0,
                          "kernel": "dslash_k<float, DW_FULL>", "algorithmic_bytes_per_launch": dw_bytes_per_site(hp) * V},
             "e2e": {"value": e2e_val, "unit": "GB/s", "h2d_bytes_per_step": io_bytes, "d2h_bytes_per_step": io_bytes, "ms_per_step": e2e_s * 1e3,
                     "call": "qxd_apply_Dw_host (pinned host fp64 in/out, pipelined over time slabs)"},
+            "sustained": sustained,
+            "e2e_solve": e2e_solve,
             "gpu_launches": launches,
             "clocks": clocks,
             "cpu_baseline": cpu_baseline,
@@ -461,7 +580,9 @@ def main():
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the precision sweep (short runs under ncu)")
-    ap.add_argument("--no-e2e", action="store_true", help="skip the host-pointer end-to-end loop (short runs under ncu)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-pointer end-to-end loops (short runs under ncu)")
+    ap.add_argument("--sustain-s", type=float, default=1.0, help="seconds of back-to-back applies for the `sustained` figure (0 = skip)")
+    ap.add_argument("--no-oracle-residual", action="store_true", help="skip the oracle's whole-lattice true residual of the solves")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

@@ -147,6 +147,10 @@ int qxd_field_status(const qxd_ctx* ctx, int* status /*HOST*/, long counts[2] /*
  * Builds M(x) = (4+m0) + c_sw (i/4) sigma.F-hat + q c_sw_qed (i/4) sigma.A-hat as two Hermitian
  * 6x6 blocks per site and inverts both blocks, on the device.  Needs gauge + quark. */
 int qxd_clover_build(qxd_ctx* ctx, double csw, double csw_qed);
+/* How the 6x6 block inverses were obtained so far (HOST counts[2]): [0] parity passes of the unpivoted in-register
+ * Gauss-Jordan (the fast path: the blocks are (4 + m0) + O(c_sw F), diagonally dominant for every sensible field),
+ * [1] parity passes redone with the partially pivoted kernel because a pivot fell below 1e-6 of the largest diagonal entry. */
+int qxd_clover_stats(const qxd_ctx* ctx, long counts[2] /*HOST*/);
 /* Storage format of the hopping links W = e^{iqA} U (north_star "12-real SU(3) reconstruct and the U(1)
  * phase fused into the link multiply").  QXD_RECON_NONE: all 18 reals of W.  QXD_RECON_12: rows 0 and 1 of W (12 reals)
  * plus det W = e^{3iqA} det U (x -1 on the antiperiodic time boundary) as (re, im) = 14 reals per link; the dslash rebuilds

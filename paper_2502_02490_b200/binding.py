@@ -58,6 +58,7 @@ SYMBOLS = {
     "qxd_set_gauge_reconstruct": (_i, [_vp, _i]),
     "qxd_set_gauge_reconstruct_prec": (_i, [_vp, _i, _i]),
     "qxd_clover_export": (_i, [_vp, _vp, _i]),
+    "qxd_clover_stats": (_i, [_vp, _vp]),
     "qxd_apply_Dw": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dhat_eo": (_i, [_vp, _i, _vp, _vp, _i]),
     "qxd_apply_Dw_host": (_i, [_vp, _i, _vp, _vp]),
@@ -204,6 +205,12 @@ class Qxd:
         cnt = (C.c_long * 2)()
         self._chk(self.lib.qxd_field_status(self.h, C.byref(st), cnt))
         return st.value, cnt[0], cnt[1]
+
+    def clover_stats(self):
+        """(parity passes of the unpivoted block inversion, parity passes redone with the pivoted kernel)"""
+        cnt = (C.c_long * 2)()
+        self._chk(self.lib.qxd_clover_stats(self.h, cnt))
+        return cnt[0], cnt[1]
 
     def clover_export(self, inverse=False):
         out = self.torch.empty((self.V, 2, 36), dtype=self.torch.float64, device=self.device)

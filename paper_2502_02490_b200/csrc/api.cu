@@ -56,7 +56,12 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
   for (int p = 0; p < 2; p++) { Ug[p] = k.take(Vg * 72 * 8); Ag[p] = k.take(Vg * 4 * 8); }
   for (int pr = 0; pr < NPREC; pr++) {
     if (!((prec_mask >> pr) & 1)) continue;
-    for (int p = 0; p < 2; p++) { W[pr][p] = k.take(Vg * 72 * prec_size(pr)); M[pr][p] = k.take(Vg * 72 * prec_size(pr)); Mi[pr][p] = k.take(Vg * 72 * prec_size(pr)); }
+    for (int p = 0; p < 2; p++) {
+      W[pr][p] = k.take(Vg * 72 * prec_size(pr)); M[pr][p] = k.take(Vg * 72 * prec_size(pr));
+      // block inverses: only A_oo^{-1} is ever applied (SURVEY.md §8 row a3 "odd sites only is enough"); the even-site inverses
+      // exist in fp64 alone, for qxd_clover_export
+      Mi[pr][p] = (pr == 0 || p == 1) ? k.take(Vg * 72 * prec_size(pr)) : nullptr;
+    }
   }
   void* sp64[12]; void* splo[8];
   for (int i = 0; i < 12; i++) sp64[i] = k.take(half_bytes(0, Vh));
@@ -77,7 +82,8 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
     const int plo = mlo_size == 8 ? 0 : mlo_size == 4 ? 1 : 2;
     const size_t lo = (half_bytes(plo, Vh) + 255) & ~size_t(255);
     for (int i = 0; i < 2; i++) mhi[i] = k.take(half_bytes(0, Vh) * nrhs);
-    for (int i = 0; i < 7; i++) mlo[i] = k.take(lo * nrhs);
+    // x, r, p, t, odd-site scratch; r16, p16 only for the binary16 operator with fp32 vectors
+    for (int i = 0; i < 7; i++) mlo[i] = (i < 5 || (mlo_size == 4 && (prec_mask & 4))) ? k.take(lo * nrhs) : nullptr;
     mscal = k.take(64 * 8 * 8);
     mact = k.take(64 * 8);
   }
@@ -330,6 +336,12 @@ int qxd_clover_build(qxd_ctx* c, double csw, double csw_qed) {
   int rc = refresh_clover(c);
   if (rc) return rc;
   c->have_clover = true;
+  return QXD_OK;
+}
+
+int qxd_clover_stats(const qxd_ctx* c, long counts[2]) {
+  if (!c || !counts) return QXD_EINVAL;
+  counts[0] = c->n_inv_fast; counts[1] = c->n_inv_pivoted;
   return QXD_OK;
 }
 

@@ -152,7 +152,6 @@ __global__ void __launch_bounds__(128) cg_xr_k(int Vh, const double* num, const 
     store_spinor<S>(x, Vh, cb, vx);
     load_spinor<S>(t, Vh, cb, vp);
     load_spinor<S>(r, Vh, cb, vx);
-#pragma unroll
     C part = 0;   // per-site sum in the arithmetic type (fp32 for fp32/fp16 storage), fp64 across sites: the float->double
                   // conversions and DFMAs of a per-element fp64 sum cost more than the memory traffic of this kernel
 #pragma unroll

@@ -341,6 +341,7 @@ int launch_clover_build(qxd_ctx* c) {
   for (int p = 0; p < 2; p++) {
     clover_invert_fast_k<<<(2 * c->g.Vg + 127) / 128, 128, 0, c->stream>>>(c->g.Vg, c->M[0][p], c->Mi[0][p], flag);
     QXD_LAUNCH_CHECK(c);
+    c->n_inv_fast++;
   }
   int hflag[2] = {0, 0};
   QXD_CUDA_OK(c, cudaMemcpyAsync(hflag, flag, 2 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -349,6 +350,7 @@ int launch_clover_build(qxd_ctx* c) {
     for (int p = 0; p < 2; p++) {
       clover_invert_k<<<(c->g.Vg + 63) / 64, 64, 0, c->stream>>>(c->g.Vg, c->M[0][p], c->Mi[0][p], flag);
       QXD_LAUNCH_CHECK(c);
+      c->n_inv_pivoted++;
     }
     QXD_CUDA_OK(c, cudaMemcpyAsync(hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
@@ -359,6 +361,7 @@ int launch_clover_build(qxd_ctx* c) {
     for (int p = 0; p < 2; p++) {
       int rc = launch_convert_record72(c, c->M[0][p], pr, c->M[pr][p]);
       if (rc) return rc;
+      if (!c->Mi[pr][p]) continue;   // even-site inverses are kept in fp64 only (api.cu: carve)
       rc = launch_convert_record72(c, c->Mi[0][p], pr, c->Mi[pr][p]);
       if (rc) return rc;
     }

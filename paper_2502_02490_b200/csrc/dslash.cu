@@ -1,29 +1,12 @@
 // dslash.cu -- launch front end of the dslash kernels (dslash_kernel.cuh) and the stand-alone clover multiply; SURVEY.md §8 rows a4 (D_w apply), a5 (D-hat even-odd passes) and the dslash-shaped parts
 #include "dslash_args.h"
+#include "block_algebra.cuh"
 #include <cstdlib>
 
 namespace qxd {
 
 namespace {
 
-// out(12 reals: one chirality) = Hermitian 6x6 block (36 packed reals) times in
-template <typename C>
-__device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
-#pragma unroll
-  for (int i = 0; i < 6; i++) { out[2 * i] = b[i] * in[2 * i]; out[2 * i + 1] = b[i] * in[2 * i + 1]; }
-  int k = 6;
-#pragma unroll
-  for (int i = 0; i < 6; i++)
-#pragma unroll
-    for (int j = i + 1; j < 6; j++) {
-      const C ur = b[k], ui = b[k + 1];
-      k += 2;
-      out[2 * i] += ur * in[2 * j] - ui * in[2 * j + 1];
-      out[2 * i + 1] += ur * in[2 * j + 1] + ui * in[2 * j];
-      out[2 * j] += ur * in[2 * i] + ui * in[2 * i + 1];
-      out[2 * j + 1] += ur * in[2 * i + 1] - ui * in[2 * i];
-    }
-}
 // M v or M^{-1} v for one site; in the C*-paired layout the record is that of the physical site and the mirror image uses
 // sigma2 M^* sigma2, applied as sigma2 conj(M conj(sigma2 v)) (see dslash_kernel.cuh)
 template <typename S>
@@ -35,20 +18,10 @@ __device__ __forceinline__ void clover_mul(const void* CL, const Geom& g, int cb
 #pragma unroll
   for (int blk = 0; blk < 2; blk++) {
     if (blk == 0) load_reals<S, 0, 36>(CL, g.Vg, rec, b); else load_reals<S, 36, 36>(CL, g.Vg, rec, b);
-    const C* v = in + 12 * blk;
     C a[12], w[12];
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-      a[2 * c] = mir ? v[6 + 2 * c + 1] : v[2 * c];        a[2 * c + 1] = mir ? v[6 + 2 * c] : v[2 * c + 1];
-      a[6 + 2 * c] = mir ? -v[2 * c + 1] : v[6 + 2 * c];   a[6 + 2 * c + 1] = mir ? -v[2 * c] : v[6 + 2 * c + 1];
-    }
+    mirror_in(in + 12 * blk, a, mir);
     block_mul(b, a, w);
-    C* y = out + 12 * blk;
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-      y[2 * c] = mir ? -w[6 + 2 * c + 1] : w[2 * c];       y[2 * c + 1] = mir ? -w[6 + 2 * c] : w[2 * c + 1];
-      y[6 + 2 * c] = mir ? w[2 * c + 1] : w[6 + 2 * c];    y[6 + 2 * c + 1] = mir ? w[2 * c] : w[6 + 2 * c + 1];
-    }
+    mirror_out(w, out + 12 * blk, mir);
   }
 }
 
@@ -78,6 +51,7 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.CL[0] = inv ? c->Mi[d.prec][0] : c->M[d.prec][0];
   a.CL[1] = inv ? c->Mi[d.prec][1] : c->M[d.prec][1];
   a.parity_out = d.parity_out;
+  if (inv && !a.CL[d.parity_out & 1]) return fail(c, QXD_EINVAL, "dslash: the inverse clover blocks of the even sites exist in fp64 only");
   a.nrhs = d.nrhs > 1 ? d.nrhs : 1; a.ngroups = 1;
   a.rs_in = d.rs_in; a.rs_phi = d.rs_phi; a.rs_out = d.rs_out;
   a.tm = d.tm;

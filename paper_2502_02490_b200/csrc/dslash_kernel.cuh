@@ -16,6 +16,7 @@
 // with the upper sign for the forward hop.
 #pragma once
 #include "dslash_args.h"
+#include "block_algebra.cuh"
 
 namespace qxd {
 
@@ -159,25 +160,6 @@ template <typename S> struct UseX2 {
   static constexpr bool LINK = (MASK & 1) != 0, RECON = (MASK & 2) != 0, BLOCK = (MASK & 4) != 0;
 };
 
-// out(12 reals: one chirality) = Hermitian 6x6 block (36 packed reals) times in
-template <typename C>
-__device__ __forceinline__ void block_mul(const C* b, const C* in, C* out) {
-#pragma unroll
-  for (int i = 0; i < 6; i++) { out[2 * i] = b[i] * in[2 * i]; out[2 * i + 1] = b[i] * in[2 * i + 1]; }
-  int k = 6;
-#pragma unroll
-  for (int i = 0; i < 6; i++)
-#pragma unroll
-    for (int j = i + 1; j < 6; j++) {
-      const C ur = b[k], ui = b[k + 1];
-      k += 2;
-      // out_i += u in_j ; out_j += conj(u) in_i   (one FMA per product)
-      out[2 * i] += ur * in[2 * j]; out[2 * i] -= ui * in[2 * j + 1];
-      out[2 * i + 1] += ur * in[2 * j + 1]; out[2 * i + 1] += ui * in[2 * j];
-      out[2 * j] += ur * in[2 * i]; out[2 * j] += ui * in[2 * i + 1];
-      out[2 * j + 1] += ur * in[2 * i + 1]; out[2 * j + 1] -= ui * in[2 * i];
-    }
-}
 // (re, im) of one component in the two lanes; A = i * in supplies the products with the imaginary part of the block entry
 __device__ __forceinline__ void block_mul_x2(const float* b, const float* in, float* out) {
   f32x2 I[6], A[6], O[6];
@@ -210,25 +192,6 @@ __device__ __forceinline__ void clover_mul(const void* CL, int Vh, int cb, const
   block_mul_s<S>(b, in, out);
   load_reals<S, 36, 36>(CL, Vh, cb, b);
   block_mul_s<S>(b, in + 12, out + 12);
-}
-// Paired layout: the clover block of the mirror site is sigma2 M^* sigma2, so (M' v) = sigma2 conj(M conj(sigma2 v)): the
-// stored block is applied to a = conj(sigma2 v) = (i conj v1, -i conj v0) and the result w is mapped to (-i conj w1, i conj w0).
-// In (re, im) pairs these are swaps and sign changes only; `mir` differs between neighbouring lanes, hence selects.
-template <typename C>
-__device__ __forceinline__ void mirror_in(const C* v, C* a, bool mir) {
-#pragma unroll
-  for (int c = 0; c < 3; c++) {
-    a[2 * c] = mir ? v[6 + 2 * c + 1] : v[2 * c];            a[2 * c + 1] = mir ? v[6 + 2 * c] : v[2 * c + 1];
-    a[6 + 2 * c] = mir ? -v[2 * c + 1] : v[6 + 2 * c];       a[6 + 2 * c + 1] = mir ? -v[2 * c] : v[6 + 2 * c + 1];
-  }
-}
-template <typename C>
-__device__ __forceinline__ void mirror_out(const C* w, C* y, bool mir) {
-#pragma unroll
-  for (int c = 0; c < 3; c++) {
-    y[2 * c] = mir ? -w[6 + 2 * c + 1] : w[2 * c];           y[2 * c + 1] = mir ? -w[6 + 2 * c] : w[2 * c + 1];
-    y[6 + 2 * c] = mir ? w[2 * c + 1] : w[6 + 2 * c];        y[6 + 2 * c + 1] = mir ? w[2 * c] : w[6 + 2 * c + 1];
-  }
 }
 // the same blocks applied to R spinors (multi-RHS, row a10): each block is loaded once
 template <typename S, int R, bool PAIR>

@@ -44,6 +44,7 @@ struct qxd_ctx {
   // field-status manager (row f4): derived fields marked stale by a setter and regenerated at their first use
   bool lazy = false, hop_stale = false, clover_stale = false;
   long n_hop_refresh = 0, n_clover_refresh = 0;
+  long n_inv_fast = 0, n_inv_pivoted = 0;          // block-inversion passes: unpivoted fast path / pivoted fallback (qxd_clover_stats)
   double qel = 1.0, kappa = 0, q = 0, m0 = 0, csw = 0, csw_qed = 0;
   // fields (device, carved from the workspace); [parity]
   void* Ug[2] = {nullptr, nullptr};              // fp64 SU(3) links, record of 72 reals (4 links x 18)

@@ -142,7 +142,10 @@ int cgne(qxd_ctx* c, int pop, Ws& w0, double stop2, double delta, int maxiter, q
     QXD_TRY(apply_dhat(c, pop, rin, w.s, w.tmp_o_lo, 1, gam_next));
     QXD_TRY(wait_scal(c, SC_RR, 1, &rr));
     it++;
-    if (!(rr == rr)) break;  // NaN: breakdown
+    if (!(rr == rr)) {  // NaN: breakdown.  x_lo is poisoned: drop it, so that x_hi (the last reliable update) is what is returned
+      QXD_TRY(blas_zero(c, plo, w.xlo));
+      break;
+    }
     double rn = std::sqrt(rr);
     if (rn > maxr) maxr = rn;
     if (rn < delta * maxr || rr <= stop2) {
@@ -218,7 +221,7 @@ int bicgstab(qxd_ctx* c, int plo, Ws& w, double stop2, double delta, int maxiter
     it++;
     cplx rho_new = {d3[0], d3[1]};
     rr = d3[2];
-    if (!(rr == rr)) break;
+    if (!(rr == rr)) { QXD_TRY(blas_zero(c, plo, w.xlo)); break; }   // NaN: drop the poisoned x_lo (x_hi / xbest are returned)
     if (rr < best_rr) { best_rr = rr; since_best = 0; } else if (++since_best >= 500) break;
     double rn = std::sqrt(rr);
     if (rn > maxr) maxr = rn;
@@ -385,16 +388,23 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
     nactive += !done[k];
   }
   QXD_CUDA_OK(c, cudaMemcpyAsync(c->mact, c->h_mact, sizeof(double) * nrhs, cudaMemcpyHostToDevice, c->stream));
-  // fp64 true residual of system k:  x_hi += x_lo; x_lo = 0; r = b - D-hat x_hi; r_lo = r
-  auto reliable = [&](int k) -> int {
-    SpinorPtr xk = rhs_view(X, rs_hi, k);
-    QXD_TRY(blas_acc_hi(c, plo, rhs_view(xlo, rs_lo, k), xk));
-    QXD_TRY(apply_dhat(c, 0, xk, thi, tmp_o_hi, 0, nullptr));
-    QXD_TRY(blas_sub_norm(c, 0, rhs_view(B, rs_hi, k), thi, rhi, c->scal + SC_RRT));
-    QXD_TRY(launch_convert_spinor(c, 0, rhi, plo, rhs_view(rlo, rs_lo, k)));
-    if (h16) QXD_TRY(launch_convert_spinor(c, 0, rhi, pop, rhs_view(r16, rs_op, k)));
-    QXD_TRY(read_scal(c, SC_RRT, 1, &rr_true[k]));
-    nrel[k]++;
+  // fp64 true residuals of the systems in `list`:  x_hi += x_lo; x_lo = 0; r = b - D-hat x_hi; r_lo = r.  All of them are
+  // enqueued back to back (their |r|^2 go to the systems' own device slots) and read back with ONE host round trip.
+  auto reliable = [&](const int* list, int n) -> int {
+    if (n == 0) return QXD_OK;
+    for (int i = 0; i < n; i++) {
+      const int k = list[i];
+      SpinorPtr xk = rhs_view(X, rs_hi, k);
+      QXD_TRY(blas_acc_hi(c, plo, rhs_view(xlo, rs_lo, k), xk));
+      QXD_TRY(apply_dhat(c, 0, xk, thi, tmp_o_hi, 0, nullptr));
+      QXD_TRY(blas_sub_norm(c, 0, rhs_view(B, rs_hi, k), thi, rhi, ms + k * SS + M_RRT));
+      QXD_TRY(launch_convert_spinor(c, 0, rhi, plo, rhs_view(rlo, rs_lo, k)));
+      if (h16) QXD_TRY(launch_convert_spinor(c, 0, rhi, pop, rhs_view(r16, rs_op, k)));
+      nrel[k]++;
+    }
+    QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
+    QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < n; i++) rr_true[list[i]] = hs[list[i] * SS + M_RRT];
     return QXD_OK;
   };
   int it = 0;
@@ -409,35 +419,49 @@ int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat,
     QXD_TRY(apply_dhat(c, pop, pin, t, tmp_o, 0, ms + M_TT, bo));
     if (h16) QXD_TRY(blas_cg_xr_h(c, gam, ms + M_TT, p16, t, xlo, rlo, r16, ms + M_RR, bl, rs_op));
     else QXD_TRY(blas_cg_xr(c, plo, gam, ms + M_TT, p, t, xlo, rlo, ms + M_RR, bl));
+    // the |r|^2 of all systems travel to the host while s = A^dag r of the whole batch is already running (as in the
+    // single-RHS loop): the GPU does not idle on the round trip; systems that do a reliable update get their s redone below
     QXD_CUDA_OK(c, cudaMemcpyAsync(hs, ms, sizeof(double) * SS * nrhs, cudaMemcpyDeviceToHost, c->stream));
-    QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    QXD_CUDA_OK(c, cudaEventRecord(c->ev_scal, c->stream));
+    QXD_TRY(apply_dhat(c, pop, rin, t, tmp_o, 1, gam_next, bo));
+    QXD_CUDA_OK(c, cudaEventSynchronize(c->ev_scal));
     it++;
     bool changed = false;
+    int upd[64], nupd = 0;
     for (int k = 0; k < nrhs; k++) {
       if (done[k]) continue;
       iters[k] = it;
       const double rr = hs[k * SS + M_RR];
-      if (!(rr == rr)) { done[k] = 2; c->h_mact[k] = 0.0; changed = true; nactive--; continue; }  // breakdown
+      if (!(rr == rr)) {   // breakdown: freeze the system and drop its poisoned x_lo (x_hi of the last reliable update is returned)
+        done[k] = 2; c->h_mact[k] = 0.0; changed = true; nactive--;
+        QXD_TRY(blas_zero(c, plo, rhs_view(xlo, rs_lo, k)));
+        continue;
+      }
       const double rn = std::sqrt(rr);
       if (rn > maxr[k]) maxr[k] = rn;
-      if (rn < delta * maxr[k] || rr <= stop2[k]) {
-        QXD_TRY(reliable(k));
-        maxr[k] = std::sqrt(rr_true[k]);
-        if (rr_true[k] <= stop2[k]) { done[k] = 1; c->h_mact[k] = 0.0; changed = true; nactive--; }
-      }
+      if (rn < delta * maxr[k] || rr <= stop2[k]) upd[nupd++] = k;
+    }
+    QXD_TRY(reliable(upd, nupd));
+    for (int i = 0; i < nupd; i++) {
+      const int k = upd[i];
+      maxr[k] = std::sqrt(rr_true[k]);
+      if (rr_true[k] <= stop2[k]) { done[k] = 1; c->h_mact[k] = 0.0; changed = true; nactive--; }
+      else   // s_k = A^dag r_k from the corrected residual (single-RHS launch into the system's slots of the batch)
+        QXD_TRY(apply_dhat(c, pop, rhs_view(rin, rs_op, k), rhs_view(t, rs_op, k), rhs_view(tmp_o, rs_op, k), 1, gam_next + k * SS));
     }
     if (changed) QXD_CUDA_OK(c, cudaMemcpyAsync(c->mact, c->h_mact, sizeof(double) * nrhs, cudaMemcpyHostToDevice, c->stream));
     if (!nactive) break;
-    QXD_TRY(apply_dhat(c, pop, rin, t, tmp_o, 1, gam_next, bo));
     if (h16) QXD_TRY(blas_cg_p_h(c, gam_next, gam, t, p, p16, bl, rs_op));
     else QXD_TRY(blas_cg_p(c, plo, gam_next, gam, t, p, bl));
   }
+  {   // systems that did not converge: leave the best iterate with its true residual
+    int upd[64], nupd = 0;
+    for (int k = 0; k < nrhs; k++) if (done[k] != 1) upd[nupd++] = k;
+    QXD_TRY(reliable(upd, nupd));
+    for (int i = 0; i < nupd; i++) if (rr_true[upd[i]] <= stop2[upd[i]]) done[upd[i]] = 1;
+  }
   int status = QXD_OK;
   for (int k = 0; k < nrhs; k++) {
-    if (done[k] != 1) {   // leave the best iterate with its true residual
-      QXD_TRY(reliable(k));
-      if (rr_true[k] <= stop2[k]) done[k] = 1;
-    }
     if (done[k] != 1) status = QXD_ENOCONV;
     // reconstruction (row a8): psi_o = A_oo^{-1}(eta_o - D_oe psi_e)
     QXD_TRY(launch_spinor_pack(c, 0, eta_nat + vnat * k, c->full_a, 2, 0));

@@ -70,8 +70,13 @@ class TimeSlabs:
 
 
 def exchange_time_ghosts(ts: TimeSlabs, local, dist=None):
-    """Fill the two ghost slices of `local` (tensor or array [T_loc+2][...]) from the time neighbours.  Upward messages
-    (my last interior slice -> next rank's lower ghost) use tag 0, downward ones tag 1.  world == 1: periodic self-copy."""
+    """Fill the two ghost slices of `local` (tensor or array [T_loc+2][...]) from the time neighbours.  world == 1:
+    periodic self-copy.  The four point-to-point operations go out as ONE batch (dist.batch_isend_irecv = one
+    ncclGroupStart/End under NCCL): NCCL ignores tags and serialises the p2p operations of a peer pair on one stream, so
+    with world == 2 (previous and next rank are the same peer) four separately issued isend/irecv calls could block each
+    other; inside a group they cannot.  The pairing does not rely on tags: for every peer both sides list the upward
+    message (my last interior slice -> the next rank's lower ghost) before the downward one, and messages between a pair
+    of ranks are matched in issue order."""
     Tl = ts.T_loc
     if ts.world == 1 or dist is None:
         if ts.world != 1:
@@ -83,9 +88,9 @@ def exchange_time_ghosts(ts: TimeSlabs, local, dist=None):
     t = local if isinstance(local, torch.Tensor) else torch.from_numpy(local)
     up_send, down_send = t[Tl].contiguous(), t[1].contiguous()
     low_recv, high_recv = torch.empty_like(up_send), torch.empty_like(down_send)
-    reqs = [dist.isend(up_send, ts.next, tag=0), dist.irecv(low_recv, ts.prev, tag=0),
-            dist.isend(down_send, ts.prev, tag=1), dist.irecv(high_recv, ts.next, tag=1)]
-    for r in reqs:
+    ops = [dist.P2POp(dist.isend, up_send, ts.next), dist.P2POp(dist.irecv, low_recv, ts.prev),       # upward
+           dist.P2POp(dist.isend, down_send, ts.prev), dist.P2POp(dist.irecv, high_recv, ts.next)]    # downward
+    for r in dist.batch_isend_irecv(ops):
         r.wait()
     t[0].copy_(low_recv)
     t[Tl + 1].copy_(high_recv)

@@ -86,40 +86,40 @@ def test_solve_multi_argument_errors():
 
 
 def test_full_c4_twelve_rhs_batched_dslash_and_solve():
-    """BASELINE config 4 at full size (96x48^3 QCD, 10.6 M sites, 12 right-hand sides): the 12-RHS batched D_w in the
-    launch configuration bench.py uses, checked at sampled sites of three of the right-hand sides against the oracle's
-    per-site definition; then a batched mixed fp64/fp32 solve of four systems to 1e-10, checked through the oracle's
-    residual at sampled sites (RMS criterion as in test_full_c3_mixed_solve_sampled_residual)."""
+    """BASELINE config 4 AS STATED (96x48^3 QCD, 10.6 M sites): 12 Gaussian right-hand sides, the 12-RHS batched D_w in the
+    launch configuration bench.py uses and the batched mixed fp64/fp32 solve of all 12 systems to 1e-10; every right-hand
+    side is compared with the oracle over the WHOLE lattice (D_w: relative L2; solve: ||eta - D_ref psi|| / ||eta||).
+    Sources are generated one at a time (a c4 spinor is 2 GB in fp64) and regenerated for the check."""
     import torch
     cfg = synth.config("c4")
+    n = cfg["nrhs"]
+    assert n == 12
     c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
-             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32), oracle_clover=False, nrhs=4)
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32), nrhs=n)
     g = c.gpu
-    T, X1, L2, L3 = c.dims_ext
-    rng = np.random.default_rng(41)
-    coords = [(0, 0, 0, 0), (T - 1, X1 - 1, L2 - 1, L3 - 1), (T - 1, 0, L2 - 1, 0), (17, 3, 0, L3 - 1)]
-    coords += [tuple(int(rng.integers(0, n)) for n in c.dims_ext) for _ in range(60)]
-    sites = np.array([((x0 * X1 + x1) * L2 + x2) * L3 + x3 for x0, x1, x2, x3 in coords], dtype=np.int64)
-    etas = [synth.gaussian_spinor(c.dims_ext, 51 + k) for k in range(3)]
+    source = lambda k: synth.gaussian_spinor(c.dims_ext, 51 + k)
+    # ---- batched D_w, 12 right-hand sides in one launch ----
     nb = g.packed_spinor_bytes(F32)
-    pin = torch.empty(12 * nb, dtype=torch.uint8, device="cuda")
+    pin = torch.empty(n * nb, dtype=torch.uint8, device="cuda")
     pout = torch.zeros_like(pin)
-    for k in range(12):                         # 12 right-hand sides, three distinct sources in rotation
-        g.spinor_pack(etas[k % 3], F32, packed=pin[k * nb:(k + 1) * nb])
-    g.apply_Dw_multi_packed(pin, pout, F32, 12)
-    exp = [c.ref.apply_Dw_sites(e, sites) for e in etas]
-    for k in (0, 4, 11):
-        got = to_np(g.spinor_unpack(pout[k * nb:(k + 1) * nb], F32)).reshape(-1, 4, 3)[sites]
-        assert relerr(got, exp[k % 3]) < TOL[F32], k
-    del pin, pout
+    for k in range(n):
+        g.spinor_pack(source(k), F32, packed=pin[k * nb:(k + 1) * nb])
+    g.apply_Dw_multi_packed(pin, pout, F32, n)
+    for k in (0, 5, 11):
+        got = to_np(g.spinor_unpack(pout[k * nb:(k + 1) * nb], F32))
+        exp = c.ref.apply_Dw(source(k))
+        assert relerr(got, exp) < TOL[F32], k
+    del pin, pout, got, exp
     torch.cuda.empty_cache()
-    src = np.stack([etas[0], etas[1], etas[2], 0.5 * etas[0]])
-    psi, infos = g.solve_multi(src, 1e-10, sloppy=F32, delta=0.1, maxiter=3000)
-    psi = to_np(psi).reshape(src.shape)
-    for k in (1, 3):
-        assert infos[k]["status"] == 0 and infos[k]["true_res"] <= 1e-10, infos[k]
-        r = c.ref.apply_Dw_sites(psi[k], sites) - src[k].reshape(-1, 4, 3)[sites]
-        assert np.sqrt(np.mean(np.abs(r) ** 2)) <= 5e-10 * np.sqrt(np.mean(np.abs(src[k]) ** 2))
+    # ---- batched solve of the 12 systems, in place on the device ----
+    buf = torch.empty((n,) + tuple(c.dims_ext) + (4, 3), dtype=torch.complex128, device="cuda")
+    for k in range(n):
+        buf[k].copy_(torch.from_numpy(source(k)))
+    _, infos = g.solve_multi(buf, cfg["tol"], sloppy=F32, delta=0.1, maxiter=5000, psi=buf)
+    for k in range(n):
+        assert infos[k]["status"] == 0 and infos[k]["true_res"] <= cfg["tol"], (k, infos[k])
+        res = true_residual(c.ref, source(k), to_np(buf[k]))
+        assert res <= 1.05 * cfg["tol"], (k, res, infos[k])
     c.close()
 
 
