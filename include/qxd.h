@@ -59,12 +59,13 @@ typedef enum {
 typedef enum { QXD_F64 = 0, QXD_F32 = 1, QXD_F16 = 2 } qxd_prec;
 #define QXD_PREC_MASK(p) (1 << (p))
 
-typedef enum { QXD_CGNE = 0, QXD_BICGSTAB = 1 } qxd_algo;
+typedef enum { QXD_CGNE = 0, QXD_BICGSTAB = 1, QXD_GCR = 2 } qxd_algo;
 
 /* Solver controls (in) and report (out).  Zero-initialise for defaults. */
 typedef struct {
   /* in */
-  int algo;          /* qxd_algo; CG on the normal equations of D-hat, or BiCGstab on D-hat       */
+  int algo;          /* qxd_algo; CG on the normal equations of D-hat, BiCGstab on D-hat, or SAP-preconditioned
+                        flexible GCR on the full-lattice D_w (needs qxd_set_gcr before qxd_workspace_bind)      */
   int sloppy;        /* qxd_prec of the inner iteration; QXD_F64 = plain double-precision solver   */
   double delta;      /* reliable-update threshold: true residual recomputed in fp64 whenever the
                         iterated residual has dropped below delta * (max since last update);
@@ -184,6 +185,28 @@ int qxd_apply_Dw_host(qxd_ctx* ctx, int prec, const double* psi_host, double* ou
  * On QXD_ENOCONV psi holds the best iterate and info->true_res its residual. */
 int qxd_solve(qxd_ctx* ctx, const double* eta, double* psi, double tol, qxd_solve_info* info);
 int qxd_solve_host(qxd_ctx* ctx, const double* eta_host, double* psi_host, double tol, qxd_solve_info* info);
+
+/* ---- SAP-preconditioned GCR ("heavily preconditioned GCR ... Schwarz alternating
+ * procedure"; precisions PAPER.md:168-170) ---------------------------------------------------------------------------
+ * qxd_solve with algo = QXD_GCR solves the full-lattice system D_w psi = eta by a flexible, restarted GCR(nkv):
+ *   per step  z_k = M_sap r ;  w_k = D_w z_k  (fp32) ;  w_k orthonormalised against w_0..w_{k-1} ;  r -= <w_k, r> w_k
+ *   restart   psi += sum_k y_k z_k in fp64 (y from the triangular system of the orthogonalisation coefficients), and the
+ *             true residual eta - D_w psi is recomputed in fp64 (after nkv steps, or when the fp32 residual has dropped by
+ *             1e-4 within the cycle, or looks converged); convergence is only ever declared on that fp64 residual.
+ * M_sap = ncy cycles of the multiplicative Schwarz alternating procedure over a two-colouring of blocks: a block is one
+ * 128-index tile of both parities (256 sites: 4x4x4x4, or 2x4x4x4 with both C* mirror images in the paired layout) with
+ * Dirichlet boundaries; on each block nmr minimal-residual steps on D_w restricted to the block, run by ONE thread block
+ * entirely out of shared memory (links and clover blocks of the block staged once per visit, storage precision
+ * info->sloppy = QXD_F16 or QXD_F32; residual and correction in fp32); the residual of the neighbouring blocks is
+ * corrected lazily from the stored corrections when they are visited.  info->delta is ignored; info->iters counts GCR
+ * steps, info->n_reliable the fp64 restarts.
+ * qxd_set_gcr: nkv = 0 releases the Krylov space (default; QXD_GCR then returns QXD_EWORKSPACE), else 1 <= nkv <= 32,
+ * ncy >= 1, nmr >= 1 (0 = defaults ncy 4, nmr 4).  Must precede qxd_workspace_bind (the 2 nkv + 3 fp32 full-lattice
+ * vectors are part of the workspace).  Geometries whose tiles admit no two-colouring (an odd number of blocks in a
+ * direction) are rejected with QXD_EINVAL by qxd_solve.
+ * qxd_apply_sap: out = M_sap in on fp32 packed full-lattice spinors (test and bench entry point of the preconditioner). */
+int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
+int qxd_apply_sap(qxd_ctx* ctx, int prec, const void* in /*DEVICE, packed fp32*/, void* out /*DEVICE, packed fp32*/);
 
 /* ---- batched solve (rows a7 + a10; "for many right-hand sides"; BASELINE config 4) -------------------
  * nrhs (<= the nrhs the workspace was bound with, <= 64) systems with the same operator: eta, psi are DEVICE arrays

@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 QXD_F64, QXD_F32, QXD_F16 = 0, 1, 2
-QXD_CGNE, QXD_BICGSTAB = 0, 1
+QXD_CGNE, QXD_BICGSTAB, QXD_GCR = 0, 1, 2
 QXD_RECON_NONE, QXD_RECON_12 = 18, 12
 QXD_FS_GAUGE, QXD_FS_HOPLINKS, QXD_FS_CLOVER, QXD_FS_HOPLINKS_STALE, QXD_FS_CLOVER_STALE, QXD_FS_LAZY = 1, 2, 4, 8, 16, 32
 QXD_OK, QXD_EINVAL, QXD_ESTATE, QXD_EWORKSPACE, QXD_ECUDA, QXD_ENOCONV = 0, -1, -2, -3, -4, -5
@@ -64,6 +64,8 @@ SYMBOLS = {
     "qxd_apply_Dw_host": (_i, [_vp, _i, _vp, _vp]),
     "qxd_solve": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_solve_host": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
+    "qxd_set_gcr": (_i, [_vp, _i, _i, _i]),
+    "qxd_apply_sap": (_i, [_vp, _i, _vp, _vp]),
     "qxd_solve_multi": (_i, [_vp, _i, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_apply_Dw_multi_packed": (_i, [_vp, _i, _i, _vp, _vp]),
     "qxd_set_rhs_per_thread": (_i, [_vp, _i]),
@@ -108,7 +110,7 @@ def _ptr(t):
 class Qxd:
     """One solver context (qxd_ctx): geometry, workspace, gauge field, quark, clover term."""
 
-    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=None):
+    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=None, gcr=None):
         import torch
         if not torch.cuda.is_available():
             raise QxdError(QXD_ECUDA, "no CUDA device: the qxd hot path has no CPU fallback")
@@ -130,6 +132,8 @@ class Qxd:
             self._chk(self.lib.qxd_set_tile(self.h, *tile))
         if block is not None:
             self._chk(self.lib.qxd_set_block(self.h, *block))
+        if gcr is not None:                     # (nkv, ncy, nmr): Krylov space and SAP parameters of QXD_GCR (row f3)
+            self._chk(self.lib.qxd_set_gcr(self.h, *gcr))
         self.prec_mask = 0
         for p in precisions:
             self.prec_mask |= 1 << p
@@ -260,6 +264,11 @@ class Qxd:
         info = self._info(algo, sloppy, delta, maxiter)
         rc = self._chk(self.lib.qxd_solve(self.h, _ptr(eta), _ptr(psi), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
         return psi, self._report(rc, info)
+
+    def apply_sap(self, pin, pout, prec=QXD_F16):
+        """pout = M_sap pin on fp32 packed full-lattice spinors; prec = storage precision of the block operator."""
+        self._chk(self.lib.qxd_apply_sap(self.h, prec, _ptr(pin), _ptr(pout)))
+        return pout
 
     def solve_multi(self, eta, tol, sloppy=QXD_F32, delta=0.0, maxiter=0, psi=None):
         """eta: [nrhs, T, X1, L2, L3, 4, 3] complex128 (device).  Returns psi and one report per right-hand side."""

@@ -87,7 +87,18 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
     mscal = k.take(64 * 8 * 8);
     mact = k.take(64 * 8);
   }
+  // SAP-GCR (row f3): 2 nkv + 3 fp32 full-lattice vectors, 2 fp64 ones, scalars
+  void* gz[32] = {}; void* gw[32] = {}; void* g_r = nullptr; void* g_res = nullptr; void* g_corr = nullptr; void* g_r64 = nullptr; void* g_t64 = nullptr;
+  void* gscal = nullptr;
+  if (c->gcr_nkv > 0) {
+    const size_t f32 = 2 * half_bytes(1, Vh), f64 = 2 * half_bytes(0, Vh);
+    for (int i = 0; i < c->gcr_nkv; i++) { gz[i] = k.take(f32); gw[i] = k.take(f32); }
+    g_r = k.take(f32); g_res = k.take(f32); g_corr = k.take(f32); g_r64 = k.take(f64); g_t64 = k.take(f64);
+    gscal = k.take(4096 * 8);
+  }
   if (assign) {
+    for (int i = 0; i < 32; i++) { c->gz[i] = gz[i]; c->gw[i] = gw[i]; }
+    c->g_r = g_r; c->g_res = g_res; c->g_corr = g_corr; c->g_r64 = g_r64; c->g_t64 = g_t64; c->gscal = (double*)gscal;
     for (int i = 0; i < 2; i++) c->mhi[i] = mhi[i];
     for (int i = 0; i < 7; i++) c->mlo[i] = mlo[i];
     c->mlo_size = nrhs > 1 ? mlo_size : 0; c->mscal = (double*)mscal; c->mact = (double*)mact;
@@ -506,8 +517,25 @@ int qxd_solve(qxd_ctx* c, const double* eta, double* psi, double tol, qxd_solve_
   if (!info) { std::memset(&local, 0, sizeof(local)); info = &local; }
   int rc = check_apply(c, info->sloppy, eta, psi, "solve");
   if (rc) return rc;
+  if (info->algo == QXD_GCR) return solve_gcr(c, eta, psi, tol, info);
   if (info->algo != QXD_CGNE && info->algo != QXD_BICGSTAB) return fail(c, QXD_EINVAL, "solve: unknown algorithm");
   return solve_eo(c, eta, psi, tol, info);
+}
+
+int qxd_set_gcr(qxd_ctx* c, int nkv, int ncy, int nmr) {
+  if (!c) return QXD_EINVAL;
+  if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_gcr must precede qxd_workspace_bind");
+  if (nkv < 0 || nkv > 32 || ncy < 0 || nmr < 0) return fail(c, QXD_EINVAL, "set_gcr: 0 <= nkv <= 32, ncy >= 0, nmr >= 0");
+  c->gcr_nkv = nkv; c->gcr_ncy = ncy > 0 ? ncy : 4; c->gcr_nmr = nmr > 0 ? nmr : 4;
+  return QXD_OK;
+}
+
+int qxd_apply_sap(qxd_ctx* c, int prec, const void* in, void* out) {
+  int rc = check_apply(c, prec, in, out, "apply_sap");
+  if (rc) return rc;
+  if (c->gcr_nkv < 1) return fail(c, QXD_EWORKSPACE, "apply_sap: call qxd_set_gcr before qxd_workspace_bind");
+  if (!prec_ok(c, 1)) return fail(c, QXD_EINVAL, "apply_sap: fp32 must be bound (the preconditioner works on fp32 vectors)");
+  return launch_sap(c, prec, in, out);
 }
 
 int qxd_solve_multi(qxd_ctx* c, int nrhs, const double* eta, double* psi, double tol, qxd_solve_info* info) {

@@ -67,6 +67,16 @@ struct qxd_ctx {
   double* mact = nullptr;                        // device activity mask [64]
   double* h_mscal = nullptr;                     // pinned host mirrors
   double* h_mact = nullptr;
+  // SAP-preconditioned GCR (row f3): Krylov space z_k, w_k and the preconditioner's residual / correction fields, fp32 full lattice
+  int gcr_nkv = 0, gcr_ncy = 4, gcr_nmr = 4;
+  void* gz[32] = {};
+  void* gw[32] = {};
+  void* g_r = nullptr;                           // fp32 residual of the GCR cycle
+  void* g_res = nullptr;                         // SAP: block residuals
+  void* g_corr = nullptr;                        // SAP: latest block corrections
+  void* g_r64 = nullptr;                         // fp64 full-lattice residual / scratch
+  void* g_t64 = nullptr;
+  double* gscal = nullptr;                       // device scalars of the GCR cycle: coefficient matrix b[32][32] (complex), c[32], y[32], norms
   // reductions
   double* partials = nullptr;
   double* scal = nullptr;                        // device scalars [64]
@@ -177,5 +187,9 @@ int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, cons
 // solver.cu
 int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
 int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+// sap.cu / gcr.cu (row f3)
+int sap_check_geometry(qxd_ctx* c);
+int launch_sap(qxd_ctx* c, int prec, const void* in_full32, void* out_full32);   // out = M_sap in (fp32 packed full-lattice vectors)
+int solve_gcr(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
 
 }  // namespace qxd

@@ -1,0 +1,288 @@
+// sap.cu -- SURVEY.md §8(f) row f3, the preconditioner: the Schwarz alternating procedure (SAP) named by the paper as the
+// preconditioner of its CPU solver ("heavily preconditioned GCR ... Schwarz alternating procedure"), re-designed
+// for the B200: a block is the 256 sites of one 128-index tile (both parities) and is solved by ONE thread block that keeps
+// everything the block solve touches in shared memory -- the block residual (fp32, 24 KB) and the hopping links and clover
+// blocks of the block (storage precision S: 36 + 36 KB in binary16, 72 + 72 KB in fp32) -- so that the nmr minimal-residual
+// steps on the Dirichlet block operator D_Lambda = P_Lambda D_w P_Lambda run without touching L2 or HBM.
+//
+//   M_sap:  psi = 0, r = in;  for cy < ncy, for colour in (0, 1):  on every block Lambda of that colour
+//              e = MR_nmr(D_Lambda, r|Lambda);   psi|Lambda += e;   r -= D_w e
+// The update of r outside the block is done lazily: the kernel writes the in-block part (the MR residual) and the correction
+// e; when a neighbouring block (of the other colour) is visited next, its prologue subtracts the hopping terms of the stored
+// corrections across the block boundary.  With a proper two-colouring every correction is applied exactly once.
+#include "dslash_kernel.cuh"
+
+namespace qxd {
+
+namespace {
+
+struct SapArgs {
+  Geom g;
+  const void* W[2];       // hopping links W = e^{iqA} U of the sloppy precision S, NL stored reals per link
+  const void* CL[2];      // clover blocks M (72 reals) of precision S
+  const float4* src[2];   // residual the block solves start from: the preconditioner's input in cycle 0, `res` afterwards
+  float4* res[2];         // block residuals (in-block part kept up to date)
+  float4* corr[2];        // latest correction e of every site
+  float4* psi[2];         // accumulated output
+  int colour, prologue, init_psi, nmr;
+  int boxsh[4];           // log2 of the block extents on the indexed lattice
+  int colmask[4];         // 1 if the direction has more than one block (contributes to the colour)
+};
+
+__device__ __forceinline__ int colour_of(const SapArgs& a, const Site& s) {
+  return ((a.colmask[0] ? (s.x[0] >> a.boxsh[0]) : 0) + (a.colmask[1] ? (s.x[1] >> a.boxsh[1]) : 0) +
+          (a.colmask[2] ? (s.x[2] >> a.boxsh[2]) : 0) + (a.colmask[3] ? (s.x[3] >> a.boxsh[3]) : 0)) & 1;
+}
+
+// reals [R0, R0+N) of the record of local site l from a shared-memory array laid out [chunk][128]
+template <typename S, int R0, int N>
+__device__ __forceinline__ void lds_reals(const typename PT<S>::V* base, int l, float* out) {
+  typedef typename PT<S>::V V;
+  constexpr int RPC = PT<S>::RPC;
+  constexpr int C0 = R0 / RPC, C1 = (R0 + N - 1) / RPC;
+#pragma unroll
+  for (int c = C0; c <= C1; c++) {
+    const V v = base[c * 128 + l];
+    float tmp[RPC];
+    unpack_vec(v, tmp);
+#pragma unroll
+    for (int k = 0; k < RPC; k++) {
+      const int r = c * RPC + k;
+      if (r >= R0 && r < R0 + N) out[r - R0] = tmp[k];
+    }
+  }
+}
+__device__ __forceinline__ void unpack4(const float4& v, float* o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+
+template <typename S> struct SapShape {
+  static constexpr int RPC = PT<S>::RPC;
+  static constexpr int NCH = 72 / RPC;                       // chunks of a 72-real record (links of a site; clover blocks)
+  static constexpr size_t RHO = size_t(2) * 6 * 128 * 16;    // fp32 block residual
+  static constexpr size_t REC = size_t(2) * NCH * 128 * 16;  // one 72-real record per site of the block
+  static constexpr size_t BYTES = RHO + 2 * REC;
+  static constexpr int MINB = sizeof(S) == 2 ? 2 : 1;
+};
+
+// in-block hop from shared memory: acc += (1 -+ gamma_mu) W psi(x +- mu) for a neighbour inside the block, nothing otherwise
+template <typename S, int MU, int DIR, bool PAIR>
+__device__ __forceinline__ void hop_sm(const SapArgs& a, const Site& s, int tile, int par, int l, const float4* rho,
+                                       const typename PT<S>::V* Wsm, float* acc) {
+  const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
+  if ((nb >> 7) != tile) return;
+  const int ln = nb & 127;
+  float psi[24], w[18], h[12], t[12];
+#pragma unroll
+  for (int c = 0; c < 6; c++) unpack4(rho[((1 - par) * 6 + c) * 128 + ln], psi + 4 * c);
+  if (DIR > 0) lds_reals<S, 18 * MU, 18>(Wsm + par * SapShape<S>::NCH * 128, l, w);
+  else lds_reals<S, 18 * MU, 18>(Wsm + (1 - par) * SapShape<S>::NCH * 128, ln, w);
+  project<MU, DIR>(psi, h);
+  link_mul<(DIR < 0)>(w, h, t);
+  reconstruct<MU, DIR, false>(t, acc, 1.0f);
+}
+// hop across the block boundary, from the stored corrections in global memory (prologue)
+template <typename S, int MU, int DIR, int NL, bool PAIR>
+__device__ __forceinline__ void hop_bnd(const SapArgs& a, const Site& s, int tile, int par, int l, const typename PT<S>::V* Wsm, float* acc) {
+  const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
+  if ((nb >> 7) == tile) return;
+  const int Vh = a.g.Vh;
+  float psi[24], w[18], h[12], t[12];
+#pragma unroll
+  for (int c = 0; c < 6; c++) unpack4(__ldg(a.corr[1 - par] + size_t(c) * Vh + nb), psi + 4 * c);
+  if (DIR > 0) lds_reals<S, 18 * MU, 18>(Wsm + par * SapShape<S>::NCH * 128, l, w);
+  else {   // W_mu(x - mu): the forward link of the neighbour, from its global record
+    int wi = nb;
+    float sgn = 1.f;
+    if (PAIR) { sgn = (wi & 1) ? -1.f : 1.f; wi >>= 1; }
+    float wv[NL];
+    load_reals<S, NL * MU, NL>(a.W[1 - par], PAIR ? a.g.Vg : Vh, wi, wv);
+    if (PAIR) {
+#pragma unroll
+      for (int i = 1; i < NL; i += 2) wv[i] *= sgn;
+    }
+    if (NL == 14) reconstruct_row2(wv, w);
+    else {
+#pragma unroll
+      for (int i = 0; i < 18; i++) w[i] = wv[i];
+    }
+  }
+  project<MU, DIR>(psi, h);
+  link_mul<(DIR < 0)>(w, h, t);
+  reconstruct<MU, DIR, false>(t, acc, 1.0f);
+}
+
+// stage the four forward links of the thread's own site as 72 reals (18 per link; conjugated for a C* mirror site, row 2
+// rebuilt from the 14-real format) and its clover record into shared memory
+template <typename S, int NL, bool PAIR>
+__device__ __forceinline__ void stage_site(const SapArgs& a, int cb, int par, int l, typename PT<S>::V* Wsm, typename PT<S>::V* Csm) {
+  typedef typename PT<S>::V V;
+  constexpr int RPC = PT<S>::RPC, NCH = SapShape<S>::NCH;
+  const int rec = PAIR ? (cb >> 1) : cb;
+  const int Vs = PAIR ? a.g.Vg : a.g.Vh;
+  const bool mir = PAIR && (cb & 1);
+  V* wdst = Wsm + par * NCH * 128 + l;
+  if (NL == 18 && !PAIR) {
+    const V* wsrc = reinterpret_cast<const V*>(a.W[par]);
+#pragma unroll
+    for (int c = 0; c < NCH; c++) wdst[c * 128] = __ldg(wsrc + size_t(c) * Vs + rec);
+  } else {
+    float w72[72];
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+      float wv[NL];
+      load_reals<S, NL * mu, NL>(a.W[par], Vs, rec, wv);
+      if (PAIR) {
+#pragma unroll
+        for (int i = 1; i < NL; i += 2) wv[i] = mir ? -wv[i] : wv[i];
+      }
+      if (NL == 14) reconstruct_row2(wv, w72 + 18 * mu);
+      else {
+#pragma unroll
+        for (int i = 0; i < 18; i++) w72[18 * mu + i] = wv[i];
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < NCH; c++) wdst[c * 128] = pack_vec(w72 + c * RPC, (V*)nullptr);
+  }
+  const V* csrc = reinterpret_cast<const V*>(a.CL[par]);
+  V* cdst = Csm + par * NCH * 128 + l;
+#pragma unroll
+  for (int c = 0; c < NCH; c++) cdst[c * 128] = __ldg(csrc + size_t(c) * Vs + rec);
+}
+
+// t = D_Lambda rho at the thread's site, all operands from shared memory
+template <typename S, bool PAIR>
+__device__ __forceinline__ void block_apply(const SapArgs& a, const Site& s, int tile, int cb, int par, int l, const float4* rho,
+                                            const typename PT<S>::V* Wsm, const typename PT<S>::V* Csm, const float* own, float* t) {
+  float acc[24];
+#pragma unroll
+  for (int i = 0; i < 24; i++) acc[i] = 0.f;
+  hop_sm<S, 0, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 0, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 1, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 1, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 2, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 2, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 3, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 3, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  const bool mir = PAIR && (cb & 1);
+  const typename PT<S>::V* cl = Csm + par * SapShape<S>::NCH * 128;
+#pragma unroll
+  for (int blk = 0; blk < 2; blk++) {
+    float b[36], v[12], w[12];
+    if (blk == 0) lds_reals<S, 0, 36>(cl, l, b); else lds_reals<S, 36, 36>(cl, l, b);
+    if (PAIR) mirror_in(own + 12 * blk, v, mir);
+    else {
+#pragma unroll
+      for (int i = 0; i < 12; i++) v[i] = own[12 * blk + i];
+    }
+    block_mul(b, v, w);
+    if (PAIR) mirror_out(w, t + 12 * blk, mir);
+    else {
+#pragma unroll
+      for (int i = 0; i < 12; i++) t[12 * blk + i] = w[i];
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 24; i++) t[i] -= 0.5f * acc[i];
+}
+
+template <typename S, int NL, bool PAIR>
+__global__ void __launch_bounds__(256, SapShape<S>::MINB) sap_mr_k(const __grid_constant__ SapArgs a) {
+  typedef typename PT<S>::V V;
+  extern __shared__ __align__(16) unsigned char smem[];
+  float4* rho = reinterpret_cast<float4*>(smem);                                   // [2 parities][6 chunks][128]
+  V* Wsm = reinterpret_cast<V*>(smem + SapShape<S>::RHO);                          // [2][NCH][128]
+  V* Csm = reinterpret_cast<V*>(smem + SapShape<S>::RHO + SapShape<S>::REC);       // [2][NCH][128]
+  __shared__ float red[8][3];
+  const int l = threadIdx.x & 127, par = threadIdx.x >> 7, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int Vh = a.g.Vh;
+  // tiles 2j and 2j+1 have opposite colours (checked on the host): this block takes the one of the requested colour
+  int tile;
+  {
+    Site s0;
+    site_init<PAIR ? 1 : 0>(a.g, 2 * blockIdx.x * 128, 0, s0);
+    tile = 2 * blockIdx.x + (colour_of(a, s0) != a.colour ? 1 : 0);
+  }
+  const int cb = tile * 128 + l;
+  stage_site<S, NL, PAIR>(a, cb, par, l, Wsm, Csm);
+  Site s;
+  site_init<PAIR ? 1 : 0>(a.g, cb, par, s);
+  float r[24], e[24];
+#pragma unroll
+  for (int c = 0; c < 6; c++) unpack4(__ldg(a.src[par] + size_t(c) * Vh + cb), r + 4 * c);
+  __syncthreads();
+  if (a.prologue) {   // r -= (hopping terms of the neighbouring blocks' latest corrections) = r + 1/2 acc
+    float acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] = 0.f;
+    hop_bnd<S, 0, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 0, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 1, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 1, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 2, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 2, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 3, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 3, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+#pragma unroll
+    for (int i = 0; i < 24; i++) r[i] += 0.5f * acc[i];
+  }
+#pragma unroll
+  for (int c = 0; c < 6; c++) rho[(par * 6 + c) * 128 + l] = make_float4(r[4 * c], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+#pragma unroll
+  for (int i = 0; i < 24; i++) e[i] = 0.f;
+  __syncthreads();
+  for (int it = 0; it < a.nmr; it++) {
+    float t[24];
+    block_apply<S, PAIR>(a, s, tile, cb, par, l, rho, Wsm, Csm, r, t);
+    // alpha = <t, r> / <t, t> over the block (minimal residual step)
+    float p0 = 0.f, p1 = 0.f, p2 = 0.f;
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      p0 += t[2 * k] * r[2 * k]; p0 += t[2 * k + 1] * r[2 * k + 1];
+      p1 += t[2 * k] * r[2 * k + 1]; p1 -= t[2 * k + 1] * r[2 * k];
+      p2 += t[2 * k] * t[2 * k]; p2 += t[2 * k + 1] * t[2 * k + 1];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      p0 += __shfl_xor_sync(0xffffffffu, p0, o); p1 += __shfl_xor_sync(0xffffffffu, p1, o); p2 += __shfl_xor_sync(0xffffffffu, p2, o);
+    }
+    if (lane == 0) { red[warp][0] = p0; red[warp][1] = p1; red[warp][2] = p2; }
+    __syncthreads();   // also: every thread has finished reading its neighbours' rho
+    p0 = 0.f; p1 = 0.f; p2 = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; w++) { p0 += red[w][0]; p1 += red[w][1]; p2 += red[w][2]; }
+    const float ar = p2 > 0.f ? p0 / p2 : 0.f, ai = p2 > 0.f ? p1 / p2 : 0.f;
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+      e[2 * k] += ar * r[2 * k] - ai * r[2 * k + 1]; e[2 * k + 1] += ar * r[2 * k + 1] + ai * r[2 * k];
+      r[2 * k] -= ar * t[2 * k] - ai * t[2 * k + 1]; r[2 * k + 1] -= ar * t[2 * k + 1] + ai * t[2 * k];
+    }
+#pragma unroll
+    for (int c = 0; c < 6; c++) rho[(par * 6 + c) * 128 + l] = make_float4(r[4 * c], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+    __syncthreads();
+  }
+#pragma unroll
+  for (int c = 0; c < 6; c++) {
+    const size_t i = size_t(c) * Vh + cb;
+    a.res[par][i] = make_float4(r[4 * c], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+    float4 ev = make_float4(e[4 * c], e[4 * c + 1], e[4 * c + 2], e[4 * c + 3]);
+    a.corr[par][i] = ev;
+    if (!a.init_psi) { const float4 o = a.psi[par][i]; ev.x += o.x; ev.y += o.y; ev.z += o.z; ev.w += o.w; }
+    a.psi[par][i] = ev;
+  }
+}
+
+template <typename S, int NL, bool PAIR>
+int sap_launch_t(qxd_ctx* c, const SapArgs& a, int nblocks) {
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(sap_mr_k<S, NL, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SapShape<S>::BYTES);
+    if (e != cudaSuccess) return fail(c, QXD_ECUDA, std::string("sap: cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+    configured = true;
+  }
+  sap_mr_k<S, NL, PAIR><<<nblocks, 256, SapShape<S>::BYTES, c->stream>>>(a);
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+}  // namespace
