@@ -1,0 +1,294 @@
+// gcr.cu -- SURVEY.md §8(f) row f3, the outer solver: flexible restarted GCR on the full-lattice D_w with the Schwarz
+// alternating procedure (sap.cu) as preconditioner -- the solver family the paper measures ("heavily preconditioned GCR",
+// PAPER.md:164; mixed half/single/double precision).
+//
+//   cycle:  for k < nkv:  z_k = M_sap r ;  w_k = D_w z_k (fp32) ;  w_k -= sum_{j<k} <w_j, w_k>/|w_j|^2 w_j ;
+//                         r -= <w_k, r>/|w_k|^2 w_k
+//   restart: solve the triangular system b y = c of the orthogonalisation coefficients (device, one thread),
+//            psi += sum_k y_k z_k in fp64, r = eta - D_w psi in fp64 (the only residual convergence is declared on).
+// All coefficients stay on the device; the host reads one scalar (|r|^2) per step to decide about restart and stop.
+// A packed fp32 full-lattice spinor is a flat array of 12 Vh float4 (chunk-major per parity, qxd_common.cuh), so the
+// vector kernels here are flat grid-stride loops; (re, im) pairs never straddle a float4.
+#include "qxd_ctx.h"
+#include <cmath>
+
+namespace qxd {
+
+namespace {
+
+enum { G_BR = 0 /* [32][32][2] raw <w_j, D z_k> */, G_N2 = 2048 /* [32] |w_k|^2 */, G_Q = 2080 /* [32][2] <w_k, r> */, G_Y = 2144 /* [32][2] */,
+       G_RR = 2208, G_RRT = 2209, G_NE = 2210, G_NO = 2211 };
+
+struct VecList {
+  const float4* v[32];
+};
+
+#define QXD_TRY(expr)        \
+  do {                       \
+    int rc__ = (expr);       \
+    if (rc__) return rc__;   \
+  } while (0)
+
+// d_j = <w_j, v> for NJ vectors of the list starting at j0: result[(j0 + j) * rstride2 .. +1] = (re, im)
+template <int NJ>
+__global__ void __launch_bounds__(256) gcr_dots_k(size_t n4, VecList W, int j0, const float4* __restrict__ v, Reducer R) {
+  double acc[2 * NJ];
+#pragma unroll
+  for (int i = 0; i < 2 * NJ; i++) acc[i] = 0.0;
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const float4 y = __ldg(v + i);
+#pragma unroll
+    for (int j = 0; j < NJ; j++) {
+      const float4 x = __ldg(W.v[j0 + j] + i);
+      float re = x.x * y.x; re += x.y * y.y; re += x.z * y.z; re += x.w * y.w;
+      float im = x.x * y.y; im -= x.y * y.x; im += x.z * y.w; im -= x.w * y.z;
+      acc[2 * j] += (double)re; acc[2 * j + 1] += (double)im;
+    }
+  }
+  grid_reduce<2 * NJ>(acc, R, blockIdx.x, gridDim.x, 0);
+}
+
+// v -= sum_{j<k} (braw_j / n2_j) w_j ;  result = (|v|^2, Re <v, r>, Im <v, r>)
+__global__ void __launch_bounds__(256) gcr_orth_k(size_t n4, VecList W, int k, const double* __restrict__ braw /*[j][2], stride 64*/,
+                                                  const double* __restrict__ n2, float4* __restrict__ v, const float4* __restrict__ r, Reducer R) {
+  __shared__ float cr[32], ci[32];
+  if (threadIdx.x < k) {
+    const double d = n2[threadIdx.x];
+    cr[threadIdx.x] = d > 0.0 ? (float)(braw[threadIdx.x * 64] / d) : 0.f;
+    ci[threadIdx.x] = d > 0.0 ? (float)(braw[threadIdx.x * 64 + 1] / d) : 0.f;
+  }
+  __syncthreads();
+  double acc[3] = {0.0, 0.0, 0.0};
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    float4 y = v[i];
+    for (int j = 0; j < k; j++) {
+      const float4 x = __ldg(W.v[j] + i);
+      const float ar = cr[j], ai = ci[j];
+      y.x -= ar * x.x - ai * x.y; y.y -= ar * x.y + ai * x.x;
+      y.z -= ar * x.z - ai * x.w; y.w -= ar * x.w + ai * x.z;
+    }
+    v[i] = y;
+    const float4 q = __ldg(r + i);
+    float nn = y.x * y.x; nn += y.y * y.y; nn += y.z * y.z; nn += y.w * y.w;
+    float re = y.x * q.x; re += y.y * q.y; re += y.z * q.z; re += y.w * q.w;
+    float im = y.x * q.y; im -= y.y * q.x; im += y.z * q.w; im -= y.w * q.z;
+    acc[0] += (double)nn; acc[1] += (double)re; acc[2] += (double)im;
+  }
+  grid_reduce<3>(acc, R, blockIdx.x, gridDim.x, 0);
+}
+// after the finalize of gcr_orth_k the three sums sit in tmp[0..2]: move them to their slots (n2[k], q[k])
+__global__ void gcr_store3_k(const double* tmp, double* n2k, double* qk) { *n2k = tmp[0]; qk[0] = tmp[1]; qk[1] = tmp[2]; }
+
+// r -= (q / n2) w ;  result = |r|^2
+__global__ void __launch_bounds__(256) gcr_update_r_k(size_t n4, const float4* __restrict__ w, const double* __restrict__ q, const double* __restrict__ n2,
+                                                      float4* __restrict__ r, Reducer R) {
+  const double d = *n2;
+  const float ar = d > 0.0 ? (float)(q[0] / d) : 0.f, ai = d > 0.0 ? (float)(q[1] / d) : 0.f;
+  double acc[1] = {0.0};
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const float4 x = __ldg(w + i);
+    float4 y = r[i];
+    y.x -= ar * x.x - ai * x.y; y.y -= ar * x.y + ai * x.x;
+    y.z -= ar * x.z - ai * x.w; y.w -= ar * x.w + ai * x.z;
+    r[i] = y;
+    float nn = y.x * y.x; nn += y.y * y.y; nn += y.z * y.z; nn += y.w * y.w;
+    acc[0] += (double)nn;
+  }
+  grid_reduce<1>(acc, R, blockIdx.x, gridDim.x, 0);
+}
+
+// Back substitution of  sum_k b_jk y_k = c_j  (j <= k < K) with b_jk = braw_jk / sqrt(n2_j) (j < k), b_kk = sqrt(n2_k),
+// c_j = q_j / sqrt(n2_j): the coefficients of the solution update in terms of the z_k.  One thread.
+__global__ void gcr_backsub_k(int K, double* s) {
+  if (threadIdx.x || blockIdx.x) return;
+  for (int k = K - 1; k >= 0; k--) {
+    const double nk = sqrt(s[G_N2 + k]);
+    if (!(nk > 0.0)) { s[G_Y + 2 * k] = 0.0; s[G_Y + 2 * k + 1] = 0.0; continue; }
+    double yr = s[G_Q + 2 * k] / nk, yi = s[G_Q + 2 * k + 1] / nk;
+    for (int l = k + 1; l < K; l++) {
+      const double br = s[G_BR + (k * 32 + l) * 2] / nk, bi = s[G_BR + (k * 32 + l) * 2 + 1] / nk;
+      const double zr = s[G_Y + 2 * l], zi = s[G_Y + 2 * l + 1];
+      yr -= br * zr - bi * zi; yi -= br * zi + bi * zr;
+    }
+    s[G_Y + 2 * k] = yr / nk; s[G_Y + 2 * k + 1] = yi / nk;
+  }
+}
+
+// x (fp64 packed full lattice: 24 Vh double2) += sum_{k<K} y_k z_k (fp32).  fp32 chunk c of a parity holds the reals of the
+// fp64 chunks 2c and 2c+1 of the same parity and site.
+__global__ void __launch_bounds__(256) gcr_update_x_k(int Vh, VecList Z, int K, const double* __restrict__ y, double2* __restrict__ x) {
+  __shared__ double yr[32], yi[32];
+  if (threadIdx.x < K) { yr[threadIdx.x] = y[2 * threadIdx.x]; yi[threadIdx.x] = y[2 * threadIdx.x + 1]; }
+  __syncthreads();
+  const size_t n4 = size_t(12) * Vh;
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const size_t pc = i / Vh, cb = i - pc * Vh;      // pc = parity * 6 + chunk
+    const size_t i64 = (2 * pc) * Vh + cb;
+    double2 a = x[i64], b = x[i64 + Vh];
+    for (int k = 0; k < K; k++) {
+      const float4 z = __ldg(Z.v[k] + i);
+      a.x += yr[k] * z.x - yi[k] * z.y; a.y += yr[k] * z.y + yi[k] * z.x;
+      b.x += yr[k] * z.z - yi[k] * z.w; b.y += yr[k] * z.w + yi[k] * z.z;
+    }
+    x[i64] = a; x[i64 + Vh] = b;
+  }
+}
+// r64 = b - t (t may be null: r64 = b) ;  r32 = float(r64) ;  result = |r64|^2
+__global__ void __launch_bounds__(256) gcr_resid_k(int Vh, const double2* __restrict__ b, const double2* __restrict__ t, double2* __restrict__ r64,
+                                                   float4* __restrict__ r32, Reducer R) {
+  const size_t n4 = size_t(12) * Vh;
+  double acc[1] = {0.0};
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const size_t pc = i / Vh, cb = i - pc * Vh;
+    const size_t i64 = (2 * pc) * Vh + cb;
+    double2 u = b[i64], v = b[i64 + Vh];
+    if (t) { const double2 p = t[i64], q = t[i64 + Vh]; u.x -= p.x; u.y -= p.y; v.x -= q.x; v.y -= q.y; }
+    r64[i64] = u; r64[i64 + Vh] = v;
+    r32[i] = make_float4((float)u.x, (float)u.y, (float)v.x, (float)v.y);
+    acc[0] += u.x * u.x + u.y * u.y + v.x * v.x + v.y * v.y;
+  }
+  grid_reduce<1>(acc, R, blockIdx.x, gridDim.x, 0);
+}
+
+struct Gcr {
+  qxd_ctx* c;
+  int nblk;
+  size_t n4;
+  Reducer red(double* result) const { Reducer R; R.partials = c->partials; R.result = result; R.rstride = 0; return R; }
+  template <int N> int finalize(double* result) {
+    reduce_finalize_k<N><<<dim3(1, 1), FINALIZE_THREADS, 0, c->stream>>>(red(result), nblk);
+    QXD_LAUNCH_CHECK(c);
+    return QXD_OK;
+  }
+  int read(int idx, int n, double* out) {
+    QXD_CUDA_OK(c, cudaMemcpyAsync(c->h_scal, c->gscal + idx, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < n; i++) out[i] = c->h_scal[i];
+    return QXD_OK;
+  }
+};
+
+}  // namespace
+
+int solve_gcr(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info) {
+  const int Vh = c->g.Vh;
+  const int pprec = info->sloppy;   // storage precision of the SAP block operator
+  if (c->gcr_nkv < 1 || !c->gz[0]) return fail(c, QXD_EWORKSPACE, "solve: QXD_GCR needs qxd_set_gcr(nkv > 0) before qxd_workspace_bind");
+  if (pprec != 1 && pprec != 2) return fail(c, QXD_EINVAL, "solve: QXD_GCR takes sloppy = QXD_F32 or QXD_F16 (storage of the SAP block operator)");
+  if (!((c->prec_mask >> 1) & 1)) return fail(c, QXD_EINVAL, "solve: QXD_GCR needs fp32 bound (Krylov vectors and the fp32 D_w)");
+  if (!(tol > 0.0)) return fail(c, QXD_EINVAL, "solve: tol must be > 0");
+  QXD_TRY(sap_check_geometry(c));
+  const int maxiter = info->maxiter > 0 ? info->maxiter : 10000;
+  const int nkv = c->gcr_nkv;
+  Gcr G;
+  G.c = c; G.n4 = size_t(12) * Vh;
+  G.nblk = Vh / 128 < 1 ? 1 : (Vh / 128 > 148 * 8 ? 148 * 8 : Vh / 128);
+  double* S = c->gscal;
+  double* tmp = S + 3000;
+  SpinorPtr b_e = half_view(0, c->full_a, Vh, 0), b_o = half_view(0, c->full_a, Vh, 1);
+  SpinorPtr x_e = half_view(0, c->full_b, Vh, 0), x_o = half_view(0, c->full_b, Vh, 1);
+  const double2* b64 = static_cast<const double2*>(c->full_a);
+  double2* x64 = static_cast<double2*>(c->full_b);
+  double2* r64 = static_cast<double2*>(c->g_r64);
+  double2* t64 = static_cast<double2*>(c->g_t64);
+  float4* r32 = static_cast<float4*>(c->g_r);
+  VecList Z, W;
+  for (int k = 0; k < 32; k++) { Z.v[k] = static_cast<const float4*>(c->gz[k]); W.v[k] = static_cast<const float4*>(c->gw[k]); }
+
+  QXD_CUDA_OK(c, cudaEventRecord(c->ev0, c->stream));
+  QXD_TRY(launch_spinor_pack(c, 0, eta_nat, c->full_a, 3, 0));
+  QXD_TRY(blas_norm2(c, 0, b_e, S + G_NE));
+  QXD_TRY(blas_norm2(c, 0, b_o, S + G_NO));
+  double nn[2];
+  QXD_TRY(G.read(G_NE, 2, nn));
+  const double eta2 = nn[0] + nn[1];
+  const double stop2 = tol * tol * eta2;
+  QXD_TRY(blas_zero(c, 0, x_e));
+  QXD_TRY(blas_zero(c, 0, x_o));
+  int it = 0, nrel = 0, status = QXD_ENOCONV;
+  double rr_true = eta2;
+  if (eta2 == 0.0) status = QXD_OK;
+  else {
+    gcr_resid_k<<<G.nblk, 256, 0, c->stream>>>(Vh, b64, nullptr, r64, r32, G.red(S + G_RRT));
+    QXD_LAUNCH_CHECK(c);
+    QXD_TRY(G.finalize<1>(S + G_RRT));
+  }
+  int stalled = 0;
+  while (status != QXD_OK && it < maxiter) {
+    double rr = rr_true;
+    const double rr0 = rr_true;
+    int K = 0;
+    for (int k = 0; k < nkv && it < maxiter; k++) {
+      QXD_TRY(launch_sap(c, pprec, c->g_r, c->gz[k]));                         // z_k = M_sap r
+      DslashCall d{};                                                           // w_k = D_w z_k (fp32)
+      d.prec = 1; d.mode = DS_DW_FULL; d.flags = 0;
+      d.in[0] = half_view(1, c->gz[k], Vh, 0); d.in[1] = half_view(1, c->gz[k], Vh, 1);
+      d.out[0] = half_view(1, c->gw[k], Vh, 0); d.out[1] = half_view(1, c->gw[k], Vh, 1);
+      QXD_TRY(launch_dslash(c, d));
+      float4* wk = static_cast<float4*>(c->gw[k]);
+      for (int j0 = 0; j0 < k; j0 += 4) {                                       // raw <w_j, w_k>, four at a time
+        const int nj = k - j0 < 4 ? k - j0 : 4;
+        Reducer R = G.red(S + G_BR + (j0 * 32 + k) * 2);
+        R.rstride = 64;
+        if (nj == 4) gcr_dots_k<4><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+        else if (nj == 3) gcr_dots_k<3><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+        else if (nj == 2) gcr_dots_k<2><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+        else gcr_dots_k<1><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+        QXD_LAUNCH_CHECK(c);
+        reduce_finalize_k<2><<<dim3(1, nj), FINALIZE_THREADS, 0, c->stream>>>(R, G.nblk);
+        QXD_LAUNCH_CHECK(c);
+      }
+      gcr_orth_k<<<G.nblk, 256, 0, c->stream>>>(G.n4, W, k, S + G_BR + k * 2, S + G_N2, wk, r32, G.red(tmp));
+      QXD_LAUNCH_CHECK(c);
+      QXD_TRY(G.finalize<3>(tmp));
+      gcr_store3_k<<<1, 1, 0, c->stream>>>(tmp, S + G_N2 + k, S + G_Q + 2 * k);
+      QXD_LAUNCH_CHECK(c);
+      gcr_update_r_k<<<G.nblk, 256, 0, c->stream>>>(G.n4, wk, S + G_Q + 2 * k, S + G_N2 + k, r32, G.red(S + G_RR));
+      QXD_LAUNCH_CHECK(c);
+      QXD_TRY(G.finalize<1>(S + G_RR));
+      QXD_TRY(G.read(G_RR, 1, &rr));
+      it++; K = k + 1;
+      if (!(rr == rr)) break;                         // NaN: leave the cycle, the fp64 restart below decides
+      // restart early when the fp32 recursion cannot be trusted further (residual down by 1e-4 within the cycle) or the
+      // target looks reached (with a margin: the fp64 residual decides)
+      if (rr <= 0.8 * stop2 || rr <= 1e-8 * rr0) break;
+    }
+    if (rr == rr && K > 0) {
+      gcr_backsub_k<<<1, 32, 0, c->stream>>>(K, S);
+      QXD_LAUNCH_CHECK(c);
+      gcr_update_x_k<<<G.nblk, 256, 0, c->stream>>>(Vh, Z, K, S + G_Y, x64);
+      QXD_LAUNCH_CHECK(c);
+    }
+    // true residual in fp64
+    DslashCall d{};
+    d.prec = 0; d.mode = DS_DW_FULL; d.flags = 0;
+    d.in[0] = x_e; d.in[1] = x_o;
+    d.out[0] = half_view(0, c->g_t64, Vh, 0); d.out[1] = half_view(0, c->g_t64, Vh, 1);
+    QXD_TRY(launch_dslash(c, d));
+    gcr_resid_k<<<G.nblk, 256, 0, c->stream>>>(Vh, b64, t64, r64, r32, G.red(S + G_RRT));
+    QXD_LAUNCH_CHECK(c);
+    QXD_TRY(G.finalize<1>(S + G_RRT));
+    double rt;
+    QXD_TRY(G.read(G_RRT, 1, &rt));
+    nrel++;
+    if (!(rt == rt)) break;                           // the iterate itself is poisoned: nothing left to return but the report
+    const double prev = rr_true;
+    rr_true = rt;
+    if (rt <= stop2) { status = QXD_OK; break; }
+    if (!(rr == rr)) break;                           // breakdown inside the cycle: psi holds the iterate of the last restart
+    stalled = rt > 0.9801 * prev ? stalled + 1 : 0;   // less than 1 % gain in a whole cycle, three times in a row: stagnation
+    if (stalled >= 3) break;
+  }
+  info->iters = it; info->n_reliable = nrel;
+  info->true_res = eta2 > 0.0 ? std::sqrt(rr_true / eta2) : 0.0;
+  QXD_TRY(launch_spinor_unpack(c, 0, c->full_b, psi_nat, 3, 0));
+  QXD_CUDA_OK(c, cudaEventRecord(c->ev1, c->stream));
+  QXD_CUDA_OK(c, cudaEventSynchronize(c->ev1));
+  float ms = 0.f;
+  QXD_CUDA_OK(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+  info->seconds = ms * 1e-3;
+  if (status == QXD_ENOCONV) c->err = "solve: GCR not converged (maxiter, stagnation or breakdown); psi holds the last iterate";
+  return status;
+}
+
+}  // namespace qxd

@@ -76,6 +76,7 @@ struct qxd_ctx {
   void* g_corr = nullptr;                        // SAP: latest block corrections
   void* g_r64 = nullptr;                         // fp64 full-lattice residual / scratch
   void* g_t64 = nullptr;
+  int sap_ok = -1, sap_boxsh[4] = {}, sap_colmask[4] = {};   // two-colouring of the SAP blocks (-1: not yet checked for the current site order)
   double* gscal = nullptr;                       // device scalars of the GCR cycle: coefficient matrix b[32][32] (complex), c[32], y[32], norms
   // reductions
   double* partials = nullptr;

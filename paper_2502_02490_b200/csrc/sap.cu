@@ -110,6 +110,20 @@ __device__ __forceinline__ void hop_bnd(const SapArgs& a, const Site& s, int til
   reconstruct<MU, DIR, false>(t, acc, 1.0f);
 }
 
+template <typename S, int NL, bool PAIR, int MU>
+__device__ __forceinline__ void stage_link(const SapArgs& a, int par, int Vs, int rec, bool mir, float* w72) {
+  float wv[NL];
+  load_reals<S, NL * MU, NL>(a.W[par], Vs, rec, wv);
+  if (PAIR) {
+#pragma unroll
+    for (int i = 1; i < NL; i += 2) wv[i] = mir ? -wv[i] : wv[i];
+  }
+  if (NL == 14) reconstruct_row2(wv, w72 + 18 * MU);
+  else {
+#pragma unroll
+    for (int i = 0; i < 18; i++) w72[18 * MU + i] = wv[i];
+  }
+}
 // stage the four forward links of the thread's own site as 72 reals (18 per link; conjugated for a C* mirror site, row 2
 // rebuilt from the 14-real format) and its clover record into shared memory
 template <typename S, int NL, bool PAIR>
@@ -126,20 +140,8 @@ __device__ __forceinline__ void stage_site(const SapArgs& a, int cb, int par, in
     for (int c = 0; c < NCH; c++) wdst[c * 128] = __ldg(wsrc + size_t(c) * Vs + rec);
   } else {
     float w72[72];
-#pragma unroll
-    for (int mu = 0; mu < 4; mu++) {
-      float wv[NL];
-      load_reals<S, NL * mu, NL>(a.W[par], Vs, rec, wv);
-      if (PAIR) {
-#pragma unroll
-        for (int i = 1; i < NL; i += 2) wv[i] = mir ? -wv[i] : wv[i];
-      }
-      if (NL == 14) reconstruct_row2(wv, w72 + 18 * mu);
-      else {
-#pragma unroll
-        for (int i = 0; i < 18; i++) w72[18 * mu + i] = wv[i];
-      }
-    }
+    stage_link<S, NL, PAIR, 0>(a, par, Vs, rec, mir, w72); stage_link<S, NL, PAIR, 1>(a, par, Vs, rec, mir, w72);
+    stage_link<S, NL, PAIR, 2>(a, par, Vs, rec, mir, w72); stage_link<S, NL, PAIR, 3>(a, par, Vs, rec, mir, w72);
 #pragma unroll
     for (int c = 0; c < NCH; c++) wdst[c * 128] = pack_vec(w72 + c * RPC, (V*)nullptr);
   }
@@ -286,3 +288,96 @@ int sap_launch_t(qxd_ctx* c, const SapArgs& a, int nblocks) {
 }
 
 }  // namespace
+
+// The SAP blocks are the 128-index tiles the kernels work on anyway: a run of 256 (128 in the paired layout) consecutive full
+// indices idx2, which is a box of the indexed lattice as long as it is made of in-tile and tile-in-block digits (powers of
+// two).  A two-colouring needs an even number of boxes in every direction that has more than one, and tiles 2j, 2j+1 must
+// have opposite colours (the kernel picks its tile that way).  Host-only; the result is cached in the context.
+int sap_check_geometry(qxd_ctx* c) {
+  if (c->sap_ok == 1) return QXD_OK;
+  const Geom& g = c->g;
+  const char* why = nullptr;
+  if (g.Vh % 128 || (g.Vh / 128) % 2) why = "the number of 128-index tiles must be even";
+  int boxsh[4] = {0, 0, 0, 0};
+  if (!why) {
+    int bits = g.pair ? 7 : 8;
+    const int order[8] = {3, 2, 1, 0, 3, 2, 1, 0};
+    for (int k = 0; k < 8 && bits > 0; k++) {
+      const int mu = order[k];
+      const int avail = k < 4 ? g.sh[mu] : g.shB[mu] - g.sh[mu];
+      const int take = bits < avail ? bits : avail;
+      boxsh[mu] += take; bits -= take;
+    }
+    if (bits > 0) why = "a 128-index tile spans several blocks of the site order";
+  }
+  int colmask[4] = {0, 0, 0, 0};
+  for (int mu = 0; mu < 4 && !why; mu++) {
+    const int nb = g.X[mu] >> boxsh[mu];
+    if (nb > 1) {
+      colmask[mu] = 1;
+      if (nb & 1) why = "odd number of SAP blocks in a direction";
+    } else if (!g.pair && mu >= 2 && mu <= g.cstar && (g.X[1] >> boxsh[1]) > 1) {
+      why = "a single SAP block in a C* direction whose shifted wrap leaves the block";
+    }
+    // extended-lattice layout: a hop across a C* boundary also shifts x1 by L1; the colour must flip exactly once
+    if (!why && !g.pair && mu >= 2 && mu <= g.cstar && nb > 1 && ((g.L1 >> boxsh[1]) & 1))
+      why = "the C* shift by L1 is an odd number of blocks in direction 1";
+  }
+  if (!why) {   // tiles 2j and 2j+1 must differ in colour
+    const int ntiles = g.Vh / 128;
+    for (int j = 0; j < ntiles / 2 && !why; j++) {
+      int col[2];
+      for (int k = 0; k < 2; k++) {
+        int x[4];
+        const int cb = (2 * j + k) * 128;
+        coords_int(g, g.pair ? (cb >> 1) : cb, 0, x);
+        col[k] = 0;
+        for (int mu = 0; mu < 4; mu++) if (colmask[mu]) col[k] += x[mu] >> boxsh[mu];
+        col[k] &= 1;
+      }
+      if (col[0] == col[1]) why = "consecutive tiles have the same colour in this site order";
+    }
+  }
+  if (why) { c->sap_ok = 0; return fail(c, QXD_EINVAL, std::string("SAP: the geometry admits no two-colouring of the blocks (") + why + ")"); }
+  for (int mu = 0; mu < 4; mu++) { c->sap_boxsh[mu] = boxsh[mu]; c->sap_colmask[mu] = colmask[mu]; }
+  c->sap_ok = 1;
+  return QXD_OK;
+}
+
+// out = M_sap in: 2 ncy half-steps of sap_mr_k; in, out: fp32 packed full-lattice spinors (parity 1 half_bytes after parity 0)
+int launch_sap(qxd_ctx* c, int prec, const void* in, void* out) {
+  if (prec != 1 && prec != 2) return fail(c, QXD_EINVAL, "SAP: the block operator is stored in fp32 or binary16");
+  int rc = sap_check_geometry(c);
+  if (rc) return rc;
+  const int Vh = c->g.Vh;
+  const size_t hb = half_bytes(1, Vh);
+  SapArgs a;
+  a.g = c->g;
+  for (int p = 0; p < 2; p++) {
+    a.W[p] = c->W[prec][p]; a.CL[p] = c->M[prec][p];
+    a.res[p] = reinterpret_cast<float4*>(static_cast<char*>(c->g_res) + p * hb);
+    a.corr[p] = reinterpret_cast<float4*>(static_cast<char*>(c->g_corr) + p * hb);
+    a.psi[p] = reinterpret_cast<float4*>(static_cast<char*>(out) + p * hb);
+  }
+  for (int mu = 0; mu < 4; mu++) { a.boxsh[mu] = c->sap_boxsh[mu]; a.colmask[mu] = c->sap_colmask[mu]; }
+  a.nmr = c->gcr_nmr;
+  const int nblocks = Vh / 256;
+  const int nl = c->link_reals[prec];
+  for (int cy = 0; cy < c->gcr_ncy; cy++)
+    for (int col = 0; col < 2; col++) {
+      a.colour = col; a.prologue = (cy > 0 || col > 0) ? 1 : 0; a.init_psi = cy == 0 ? 1 : 0;
+      for (int p = 0; p < 2; p++)
+        a.src[p] = cy == 0 ? reinterpret_cast<const float4*>(static_cast<const char*>(in) + p * hb) : a.res[p];
+      if (prec == 1) {
+        if (nl == 14) rc = c->g.pair ? sap_launch_t<float, 14, true>(c, a, nblocks) : sap_launch_t<float, 14, false>(c, a, nblocks);
+        else rc = c->g.pair ? sap_launch_t<float, 18, true>(c, a, nblocks) : sap_launch_t<float, 18, false>(c, a, nblocks);
+      } else {
+        if (nl == 14) rc = c->g.pair ? sap_launch_t<__half, 14, true>(c, a, nblocks) : sap_launch_t<__half, 14, false>(c, a, nblocks);
+        else rc = c->g.pair ? sap_launch_t<__half, 18, true>(c, a, nblocks) : sap_launch_t<__half, 18, false>(c, a, nblocks);
+      }
+      if (rc) return rc;
+    }
+  return QXD_OK;
+}
+
+}  // namespace qxd

@@ -1,0 +1,170 @@
+"""GPU parity of SURVEY.md §8(f) row f3: the Schwarz alternating procedure (SAP) and the SAP-preconditioned GCR.
+
+The paper names the method and nothing else ("heavily preconditioned GCR ... Schwarz alternating procedure"),
+so the preconditioner is checked against a step-by-step restatement of include/qxd.h's definition built from the ORACLE's
+D_w (block restriction by masking, per-block minimal-residual steps, exact residual update by a full D_w apply), and the
+solver through the only thing that is unique: ||eta - D_ref psi|| / ||eta|| with the oracle's D_w over the whole lattice.
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import synth
+from test_gpu_parity import Case, relerr, to_np, F64, F32, F16
+
+pytestmark = pytest.mark.gpu
+
+GCR = 2
+
+
+def true_residual(ref, eta, psi):
+    return np.linalg.norm(np.ravel(eta) - np.ravel(ref.apply_Dw(psi))) / np.linalg.norm(np.ravel(eta))
+
+
+def block_map(c):
+    """(tile id, colour) of every site of the extended lattice in natural order, from the library's host-side introspection
+    of its site order (qxd_site_index): a block is one 128-index tile; its colour is the parity of its box coordinates."""
+    lib = c.B.load_library()
+    X = c.dims_ext
+    V = c.V
+    tile = np.empty(V, dtype=np.int64)
+    coords = np.stack(np.unravel_index(np.arange(V), X), axis=1).astype(np.int32)
+    cb, par = C.c_int(0), C.c_int(0)
+    for s in range(V):
+        x = (C.c_int * 4)(*coords[s])
+        assert lib.qxd_site_index(c.gpu.h, x, C.byref(cb), C.byref(par)) == 0
+        tile[s] = cb.value >> 7
+    # box of every tile on the indexed lattice (physical coordinates in the paired layout: both mirror images share a tile)
+    ci = coords.astype(np.int64).copy()
+    if c.gpu.cstar and c.pairing:
+        ci[:, 1] %= c.dims[1]
+    ntiles = tile.max() + 1
+    lo = np.full((ntiles, 4), 1 << 30)
+    hi = np.full((ntiles, 4), -1)
+    np.minimum.at(lo, tile, ci)
+    np.maximum.at(hi, tile, ci)
+    ext = (hi - lo + 1)
+    assert (ext == ext[0]).all() and (np.prod(ext[0]) * (2 if (c.gpu.cstar and c.pairing) else 1) == 256)
+    box = lo // ext[0]
+    nbox = box.max(axis=0) + 1
+    colour_t = (box * (nbox > 1)).sum(axis=1) & 1
+    return tile, colour_t[tile]
+
+
+def sap_reference(c, tile, colour, r_in, ncy, nmr):
+    """M_sap r_in as include/qxd.h defines it, with the oracle's D_w: for cy < ncy, for colour in (0, 1): on every block of the
+    colour nmr minimal-residual steps on P D_w P; psi += e; r -= D_w e (exact, by a full apply)."""
+    D = lambda v: c.ref.apply_Dw(v.reshape(c.psi_shape)).reshape(-1, 12)
+    psi = np.zeros((c.V, 12), dtype=complex)
+    r = r_in.reshape(-1, 12).astype(complex)
+    ntiles = tile.max() + 1
+    for _ in range(ncy):
+        for col in (0, 1):
+            mask = (colour == col)[:, None]
+            rho = r * mask
+            e = np.zeros_like(r)
+            for _ in range(nmr):
+                t = D(rho) * mask
+                num = np.zeros(ntiles, dtype=complex)
+                den = np.zeros(ntiles)
+                np.add.at(num, tile, np.sum(np.conj(t) * rho, axis=1))
+                np.add.at(den, tile, np.sum(np.abs(t) ** 2, axis=1))
+                alpha = np.where(den > 0, num / np.where(den > 0, den, 1.0), 0.0)[tile][:, None]
+                e += alpha * rho
+                rho -= alpha * t
+            psi += e
+            r = r - D(e)
+    return psi
+
+
+SAP_CASES = [
+    # dims, cstar, qed, pairing
+    ((8, 8, 8, 8), 0, False, False),
+    ((8, 8, 8, 8), 3, True, False),
+    ((8, 4, 8, 8), 3, True, True),
+    ((16, 8, 8, 8), 2, True, True),
+]
+
+
+@pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES)
+@pytest.mark.parametrize("prec,recon", [(F32, 18), (F32, 14), (F16, 18)])
+def test_sap_matches_stepwise_definition(dims, cstar, qed, pairing, prec, recon):
+    import torch
+    ncy, nmr = 3, 4
+    c = Case(dims, cstar, 1, qed, q=-1 / 3, kappa=0.125, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(4, ncy, nmr))
+    c.pairing = pairing
+    c.psi_shape = tuple(c.dims_ext) + (4, 3)
+    g, B = c.gpu, c.B
+    g.set_gauge_reconstruct(B.QXD_RECON_12 if recon == 14 else B.QXD_RECON_NONE, prec=prec)
+    tile, colour = block_map(c)
+    r_in = synth.gaussian_spinor(c.dims_ext, 71)
+    pin = g.spinor_pack(r_in, F32)
+    pout = torch.zeros_like(pin)
+    g.apply_sap(pin, pout, prec)
+    got = to_np(g.spinor_unpack(pout, F32)).reshape(-1, 12)
+    r32 = to_np(g.spinor_unpack(pin, F32)).reshape(-1, 12)          # the input as the device holds it (rounded to fp32)
+    exp = sap_reference(c, tile, colour, r32, ncy, nmr)
+    # fp32 arithmetic through 2 ncy (nmr + 1) block operators; binary16 storage of links and clover blocks (reading R13)
+    assert relerr(got, exp) < (1e-4 if prec == F32 else 5e-3), relerr(got, exp)
+    # the preconditioner does reduce the residual substantially
+    res = np.linalg.norm(r32 - c.ref.apply_Dw(got.reshape(c.psi_shape)).reshape(-1, 12)) / np.linalg.norm(r32)
+    assert res < 0.3, res
+    c.close()
+
+
+@pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES + [((8, 8, 8, 8), 3, True, True)])
+@pytest.mark.parametrize("sloppy", [F32, F16])
+def test_gcr_solve_small(dims, cstar, qed, pairing, sloppy):
+    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=0.125, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 4, 4))
+    eta = synth.gaussian_spinor(c.dims_ext, 5)
+    psi, info = c.gpu.solve(eta, 1e-10, algo=GCR, sloppy=sloppy)
+    assert info["status"] == 0, info
+    res = true_residual(c.ref, eta, to_np(psi).reshape(eta.shape))
+    assert res <= 1.05e-10, (res, info)
+    assert abs(res - info["true_res"]) <= 0.1 * res
+    assert info["n_reliable"] >= 2                 # fp32 cycles cannot reach 1e-10 without fp64 restarts
+    # GCR with the Schwarz preconditioner needs far fewer operator applications than CG on the normal equations
+    _, icg = c.gpu.solve(eta, 1e-10, algo=0, sloppy=F32)
+    assert info["iters"] < icg["iters"], (info, icg)
+    c.close()
+
+
+def test_gcr_argument_errors_and_zero_source():
+    import torch
+    c = Case((8, 8, 8, 8), 0, 1, False, precisions=(F64, F32))           # no Krylov space
+    eta = synth.gaussian_spinor(c.dims_ext, 5)
+    with pytest.raises(c.B.QxdError) as e:
+        c.gpu.solve(eta, 1e-10, algo=GCR, sloppy=F32)
+    assert e.value.status == c.B.QXD_EWORKSPACE
+    c.close()
+    c = Case((8, 8, 8, 8), 0, 1, False, precisions=(F64, F32), gcr=(4, 2, 4))
+    with pytest.raises(c.B.QxdError) as e:
+        c.gpu.solve(eta, 1e-10, algo=GCR, sloppy=F64)                     # block operator in fp64: not provided
+    assert e.value.status == c.B.QXD_EINVAL
+    psi, info = c.gpu.solve(np.zeros_like(eta), 1e-10, algo=GCR, sloppy=F32)
+    assert info["status"] == 0 and info["iters"] == 0 and float(psi.abs().max()) == 0.0
+    psi, info = c.gpu.solve(eta, 1e-10, algo=GCR, sloppy=F32, maxiter=3)
+    assert info["status"] == c.B.QXD_ENOCONV and info["iters"] == 3
+    res = true_residual(c.ref, eta, to_np(psi).reshape(eta.shape))
+    assert abs(res - info["true_res"]) < 1e-9 and res < 1.0
+    c.close()
+    # a lattice with an odd number of blocks in a direction has no two-colouring: rejected, not silently wrong
+    c = Case((12, 4, 4, 4), 0, 1, False, precisions=(F64, F32), gcr=(4, 2, 4))
+    with pytest.raises(c.B.QxdError) as e:
+        c.gpu.solve(synth.gaussian_spinor(c.dims_ext, 5), 1e-10, algo=GCR, sloppy=F32)
+    assert e.value.status == c.B.QXD_EINVAL
+    c.close()
+
+
+@pytest.mark.parametrize("sloppy", [F32, F16])
+def test_gcr_config_c2_full_size(sloppy):
+    """BASELINE config 2 at full size (32x16^3 QCD+QED C*, paired layout = the library default)."""
+    cfg = synth.config("c2")
+    c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], pairing=True, gcr=(16, 4, 4))
+    eta = synth.gaussian_spinor(c.dims_ext, 3)
+    psi, info = c.gpu.solve(eta, cfg["tol"], algo=GCR, sloppy=sloppy)
+    assert info["status"] == 0, info
+    assert true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05 * cfg["tol"]
+    c.close()
