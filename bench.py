@@ -529,6 +529,37 @@ def run_cuda(args, cfg):
             del etas, psis
         g.set_gauge_reconstruct(B.QXD_RECON_NONE)
 
+    # ---- row f3: SAP-preconditioned GCR on the full-lattice D_w (the solver family the paper measures), in a
+    # context of its own (the Krylov space is part of the workspace): library default layout, link formats as above
+    if not args.no_solve and args.gcr_nkv > 0:
+        g.close()
+        torch.cuda.empty_cache()
+        gp = (args.gcr_nkv, args.gcr_ncy, args.gcr_nmr)
+        g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=1, device=f"cuda:{local}", pairing=(True if pairing else None), gcr=gp)
+        Ud = torch.from_numpy(U).to(dev)
+        Ad = torch.from_numpy(A).to(dev) if A is not None else None
+        g.gauge_load(Ud, Ad, cfg["qel"])
+        g.set_quark(cfg["kappa"], cfg["q"])
+        g.clover_build(cfg["csw"], cfg["csw_qed"])
+        del Ud, Ad
+        g.set_gauge_reconstruct(B.QXD_RECON_12)
+        g.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=B.QXD_F16)
+        psi_d = torch.empty_like(eta_d)
+        pin = g.spinor_pack(eta_d, B.QXD_F32)
+        pout = torch.zeros_like(pin)
+        for name, sl in (("gcr_sap_fp64_fp16", B.QXD_F16), ("gcr_sap_fp64_fp32", B.QXD_F32)):
+            g.apply_sap(pin, pout, sl)
+            sap_ms = timed(lambda: g.apply_sap(pin, pout, sl), 10)
+            g.solve(eta_d, cfg["tol"], algo=B.QXD_GCR, sloppy=sl, maxiter=args.maxiter, psi=psi_d)     # warm-up (function attributes, clocks)
+            l0 = g.launch_count()
+            _, info = g.solve(eta_d, cfg["tol"], algo=B.QXD_GCR, sloppy=sl, maxiter=args.maxiter, psi=psi_d)
+            info.update({"launches": g.launch_count() - l0, "tol": cfg["tol"], "nkv": gp[0], "ncy": gp[1], "nmr": gp[2],
+                         "sap_ms_per_application": sap_ms, "sap_ms_per_half_step": sap_ms / (2 * gp[1]),
+                         "layout": "C*-paired" if pairing else "extended lattice", "block": "128-index tile, both parities (256 sites)",
+                         "true_res_oracle": oracle_residual(eta, psi_d)})
+            solves[name] = info
+        del psi_d, pin, pout
+
     # ---- CPU baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----------------------------
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -576,6 +607,9 @@ def main():
     ap.add_argument("--config", default="c3")
     ap.add_argument("--maxiter", type=int, default=20000)
     ap.add_argument("--nrhs", type=int, default=12, help="right-hand sides of the multi-RHS D_w / batched solve lines (row a10; 1 = skip)")
+    ap.add_argument("--gcr-nkv", type=int, default=16, help="Krylov vectors per GCR cycle (0 = skip the SAP-GCR solves)")
+    ap.add_argument("--gcr-ncy", type=int, default=4, help="SAP cycles per preconditioner application")
+    ap.add_argument("--gcr-nmr", type=int, default=5, help="minimal-residual steps per SAP block solve")
     ap.add_argument("--no-pairing", action="store_true", help="keep the extended-lattice layout for the solves (C* configs)")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

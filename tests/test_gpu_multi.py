@@ -85,17 +85,54 @@ def test_solve_multi_argument_errors():
     c1.close()
 
 
-def test_full_c4_twelve_rhs_batched_dslash_and_solve():
+class _Shared:
+    pass
+
+
+@pytest.fixture(scope="module")
+def c4_oracle():
+    """Oracle context of BASELINE config 4 (96x48^3 QCD, 10.6 M sites), built once for the module."""
+    from oracle import qxd_ref as R
+    cfg = synth.config("c4")
+    o = _Shared()
+    o.cfg = cfg
+    o.U = synth.su3_links(cfg["dims"], cfg["eps"], 1)
+    o.A = None
+    o.ref = R.Ref(*cfg["dims"], cfg["bc"])
+    o.ref.gauge_load(o.U, None, cfg["qel"])
+    o.ref.set_quark(cfg["kappa"], cfg["q"])
+    o.ref.clover_build(cfg["csw"], cfg["csw_qed"])
+    yield o
+
+
+def test_full_c4_gcr_sap_converges_where_bicgstab_does_not(c4_oracle):
+    """Row f3 at config 4: the SAP-preconditioned GCR reaches 1e-10 (whole-lattice residual with the oracle's D_w) on the
+    system on which BiCGstab on D-hat stalls (round 1: QXD_ENOCONV after 548 iterations, true residual 6e-3)."""
+    cfg = c4_oracle.cfg
+    c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32, F16), share=c4_oracle, gcr=(16, 4, 5))
+    eta = synth.gaussian_spinor(c.dims_ext, 51)
+    psi, info = c.gpu.solve(eta, cfg["tol"], algo=2, sloppy=F16, maxiter=2000)
+    assert info["status"] == 0 and info["true_res"] <= cfg["tol"], info
+    assert true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05 * cfg["tol"]
+    _, ib = c.gpu.solve(eta, cfg["tol"], algo=1, sloppy=F32, maxiter=2000)
+    assert ib["status"] in (0, c.B.QXD_ENOCONV)
+    if ib["status"] == 0:
+        assert ib["true_res"] <= cfg["tol"]
+    c.close()
+
+
+def test_full_c4_twelve_rhs_batched_dslash_and_solve(c4_oracle):
     """BASELINE config 4 AS STATED (96x48^3 QCD, 10.6 M sites): 12 Gaussian right-hand sides, the 12-RHS batched D_w in the
     launch configuration bench.py uses and the batched mixed fp64/fp32 solve of all 12 systems to 1e-10; every right-hand
     side is compared with the oracle over the WHOLE lattice (D_w: relative L2; solve: ||eta - D_ref psi|| / ||eta||).
     Sources are generated one at a time (a c4 spinor is 2 GB in fp64) and regenerated for the check."""
     import torch
-    cfg = synth.config("c4")
+    cfg = c4_oracle.cfg
     n = cfg["nrhs"]
     assert n == 12
     c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
-             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32), nrhs=n)
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32), nrhs=n, share=c4_oracle)
     g = c.gpu
     source = lambda k: synth.gaussian_spinor(c.dims_ext, 51 + k)
     # ---- batched D_w, 12 right-hand sides in one launch ----

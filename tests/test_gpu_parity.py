@@ -398,7 +398,8 @@ def c3_oracle():
 def full_c3_case(request, c3_oracle):
     cfg = c3_oracle.cfg
     c = Case(cfg["dims"], cfg["cstar"], cfg["antiperiodic"], cfg["qed"], q=cfg["q"], kappa=cfg["kappa"], csw=cfg["csw"],
-             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32, F16), pairing=request.param, share=c3_oracle)
+             csw_qed=cfg["csw_qed"], qel=cfg["qel"], eps=cfg["eps"], precisions=(F64, F32, F16), pairing=request.param, share=c3_oracle,
+             gcr=(16, 4, 5))
     c.o = c3_oracle
     c.psi = c3_oracle.psi
     yield c
@@ -444,9 +445,10 @@ def test_full_c3_gamma5_hermiticity_property(full_c3_case):
     assert abs(lhs - rhs) / abs(lhs) < 1e-12
 
 
-@pytest.mark.parametrize("algo,sloppy", [(0, F16), (0, F32), (1, F32), (1, F16)], ids=["cgne_fp16", "cgne_fp32", "bicgstab_fp32", "bicgstab_fp16"])
+@pytest.mark.parametrize("algo,sloppy", [(0, F16), (0, F32), (1, F32), (1, F16), (2, F16), (2, F32)],
+                         ids=["cgne_fp16", "cgne_fp32", "bicgstab_fp32", "bicgstab_fp16", "gcr_sap_fp16", "gcr_sap_fp32"])
 def test_full_c3_benched_solves_whole_lattice_residual(full_c3_case, algo, sloppy):
-    """The four solves bench.py times (link formats as there: 14 reals in fp64 / fp32, 18 in fp16), on both layouts:
+    """The solves bench.py times (link formats as there: 14 reals in fp64 / fp32, 18 in fp16), on both layouts:
     ||eta - D_ref psi|| / ||eta|| <= 1e-10 with the ORACLE's D_w over the whole lattice."""
     c = full_c3_case
     B = c.B
