@@ -253,6 +253,43 @@ int qxd_openqxd_index(qxd_ctx* ctx, const int block[4], const int* xs, long n, l
 int qxd_openqxd_reorder(qxd_ctx* ctx, const int block[4], int reals_per_site, int to_openqxd, const double* in, double* out);
 int qxd_openqxd_gauge(qxd_ctx* ctx, const int block[4], int reals_per_link, int to_openqxd, const double* in, double* out);
 
+/* ---- domain decomposition: device-side halo and building blocks ----
+ * A rank works on a LOCAL lattice = its own sites plus ghost layers in the cut directions (the geometry is created with the
+ * local extents; time ghosts are one tile thick so that owned sites are whole time slabs).  The calls below are what a
+ * distributed operator or solver is assembled from (paper_2502_02490_b200/domain.py drives them and moves the face buffers
+ * between ranks with torch.distributed: NCCL over NVLink between GPUs); they all enqueue on the bound stream.
+ *   qxd_time_slabs     number of time slabs of the site order and their thickness (the tile extent b0); QXD_EINVAL if the order
+ *                      has no such slabs (tile volume != 256 sites, fewer than 3 or more than 64 slabs).
+ *   qxd_dslash_packed  one dslash-shaped pass on packed FULL-lattice buffers (even half followed by odd half), restricted to the
+ *                      time slabs [slab_lo, slab_hi) -- interior and boundary slabs are separate launches, so the halo exchange
+ *                      overlaps the interior.  mode: QXD_DS_*; flags: QXD_DSF_*; the hop reads `in` on parity 1 - parity_out,
+ *                      `phi` and `out` live on parity_out (QXD_DS_DW: both parities, phi ignored).  phi may be NULL if unused.
+ *   qxd_clover_apply_packed   out = M in (inverse != 0: M^{-1} in) on one parity of packed full-lattice buffers.
+ *   qxd_face_gather    buf[f][12] = upper two spin components of (1 - sign gamma_mu) psi(x) on the layer x_mu = coord, face sites f
+ *                      in lexicographic order of the other three extended coordinates; reals of type double (QXD_F64) or float;
+ *                      parity_mask 1 / 2: only that parity, compact index f >> 1; 3: both.  Size: qxd_face_bytes.
+ *   qxd_face_scatter   ghost layer x_mu = coord <- (h, 0): the spinor whose projection has the upper components h; shift1 != 0
+ *                      (even, mu != 1) reads the face site displaced by shift1 in direction 1: a message that crossed a C*
+ *                      boundary lands shifted by L1.
+ *   qxd_halo_zero      psi(x) = 0 on the layers lo <= x_mu < hi.
+ *   qxd_blas_*_dev     BLAS-1 with device-resident scalars (a distributed solver all-reduces them with NCCL in place):
+ *                      norm2_dev: *out = |x|^2;  cg_xr: alpha = *num / *den, x += alpha p, r -= alpha t, *rr = |r|^2;
+ *                      cg_p: beta = *num / *den, p = s + beta p;  copy: y = x;  zero: x = 0.  Half-lattice packed vectors. */
+enum { QXD_DS_DW = 0, QXD_DS_HOP_AINV = 1, QXD_DS_A_XMHOP = 2, QXD_DS_X_MHOP = 3, QXD_DS_AINV_X_MHOP = 4 };
+enum { QXD_DSF_G5IN = 1, QXD_DSF_G5HOP = 2 };
+int qxd_time_slabs(const qxd_ctx* ctx, int* nslabs, int* thickness);
+int qxd_dslash_packed(qxd_ctx* ctx, int prec, int mode, int flags, int parity_out, const void* in, const void* phi, void* out, int slab_lo, int slab_hi);
+int qxd_clover_apply_packed(qxd_ctx* ctx, int prec, int inverse, int parity, const void* in, void* out);
+size_t qxd_face_bytes(const qxd_ctx* ctx, int prec, int mu);
+int qxd_face_gather(qxd_ctx* ctx, int prec, const void* packed, int parity_mask, int mu, int coord, int sign, void* buf);
+int qxd_face_scatter(qxd_ctx* ctx, int prec, void* packed, int parity_mask, int mu, int coord, int shift1, const void* buf);
+int qxd_halo_zero(qxd_ctx* ctx, int prec, void* packed, int parity_mask, int mu, int lo, int hi);
+int qxd_blas_norm2_dev(qxd_ctx* ctx, int prec, const void* x, double* out /*DEVICE*/);
+int qxd_blas_cg_xr(qxd_ctx* ctx, int prec, const double* num, const double* den, const void* p, const void* t, void* x, void* r, double* rr /*all scalars DEVICE*/);
+int qxd_blas_cg_p(qxd_ctx* ctx, int prec, const double* num, const double* den, const void* s, void* p);
+int qxd_blas_copy(qxd_ctx* ctx, int prec, const void* x, void* y);
+int qxd_blas_zero(qxd_ctx* ctx, int prec, void* x);
+
 /* ---- BLAS-1 on packed half-lattice spinors (row a6) ---------------------------------------------
  * y <- a*x + y ;  returns <x,y> = sum conj(x) y  and  |x|^2 (fp64 accumulation, HOST results). */
 int qxd_blas_axpy(qxd_ctx* ctx, int prec, double a, const void* x, void* y);

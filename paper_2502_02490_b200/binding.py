@@ -77,6 +77,18 @@ SYMBOLS = {
     "qxd_openqxd_index": (_i, [_vp, C.POINTER(_i), _vp, _l, _vp]),
     "qxd_openqxd_reorder": (_i, [_vp, C.POINTER(_i), _i, _i, _vp, _vp]),
     "qxd_openqxd_gauge": (_i, [_vp, C.POINTER(_i), _i, _i, _vp, _vp]),
+    "qxd_time_slabs": (_i, [_vp, C.POINTER(_i), C.POINTER(_i)]),
+    "qxd_dslash_packed": (_i, [_vp, _i, _i, _i, _i, _vp, _vp, _vp, _i, _i]),
+    "qxd_clover_apply_packed": (_i, [_vp, _i, _i, _i, _vp, _vp]),
+    "qxd_face_bytes": (_sz, [_vp, _i, _i]),
+    "qxd_face_gather": (_i, [_vp, _i, _vp, _i, _i, _i, _i, _vp]),
+    "qxd_face_scatter": (_i, [_vp, _i, _vp, _i, _i, _i, _i, _vp]),
+    "qxd_halo_zero": (_i, [_vp, _i, _vp, _i, _i, _i, _i]),
+    "qxd_blas_norm2_dev": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_blas_cg_xr": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "qxd_blas_cg_p": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
+    "qxd_blas_copy": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_blas_zero": (_i, [_vp, _i, _vp]),
     "qxd_blas_axpy": (_i, [_vp, _i, _d, _vp, _vp]),
     "qxd_blas_cdot": (_i, [_vp, _i, _vp, _vp, _vp]),
     "qxd_blas_norm2": (_i, [_vp, _i, _vp, _vp]),
@@ -331,6 +343,51 @@ class Qxd:
         info = self._info(algo, sloppy, delta, maxiter)
         rc = self._chk(self.lib.qxd_solve_host(self.h, _ptr(eta_host), _ptr(psi_host), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
         return psi_host, self._report(rc, info)
+
+    # -- domain decomposition building blocks (row f2) ---------------------------------------------------
+    def time_slabs(self):
+        n, t = C.c_int(0), C.c_int(0)
+        self._chk(self.lib.qxd_time_slabs(self.h, C.byref(n), C.byref(t)))
+        return n.value, t.value
+
+    def dslash_packed(self, mode, pin, pout, prec, parity_out=0, flags=0, phi=None, slabs=None):
+        lo, hi = slabs if slabs is not None else (0, self.time_slabs()[0])
+        self._chk(self.lib.qxd_dslash_packed(self.h, prec, mode, flags, parity_out, _ptr(pin), _ptr(phi), _ptr(pout), lo, hi))
+        return pout
+
+    def clover_apply_packed(self, pin, pout, prec, parity, inverse=False):
+        self._chk(self.lib.qxd_clover_apply_packed(self.h, prec, int(inverse), parity, _ptr(pin), _ptr(pout)))
+        return pout
+
+    def face_buffer(self, prec, mu):
+        n = self.lib.qxd_face_bytes(self.h, prec, mu)
+        dt = self.torch.float64 if prec == QXD_F64 else self.torch.float32
+        return self.torch.zeros(n // (8 if prec == QXD_F64 else 4), dtype=dt, device=self.device)
+
+    def face_gather(self, packed, prec, parity_mask, mu, coord, sign, buf):
+        self._chk(self.lib.qxd_face_gather(self.h, prec, _ptr(packed), parity_mask, mu, coord, sign, _ptr(buf)))
+        return buf
+
+    def face_scatter(self, packed, prec, parity_mask, mu, coord, shift1, buf):
+        self._chk(self.lib.qxd_face_scatter(self.h, prec, _ptr(packed), parity_mask, mu, coord, shift1, _ptr(buf)))
+
+    def halo_zero(self, packed, prec, parity_mask, mu, lo, hi):
+        self._chk(self.lib.qxd_halo_zero(self.h, prec, _ptr(packed), parity_mask, mu, lo, hi))
+
+    def blas_norm2_dev(self, x, prec, out):
+        self._chk(self.lib.qxd_blas_norm2_dev(self.h, prec, _ptr(x), _ptr(out)))
+
+    def blas_cg_xr(self, prec, num, den, p, t, x, r, rr):
+        self._chk(self.lib.qxd_blas_cg_xr(self.h, prec, _ptr(num), _ptr(den), _ptr(p), _ptr(t), _ptr(x), _ptr(r), _ptr(rr)))
+
+    def blas_cg_p(self, prec, num, den, s, p):
+        self._chk(self.lib.qxd_blas_cg_p(self.h, prec, _ptr(num), _ptr(den), _ptr(s), _ptr(p)))
+
+    def blas_copy(self, x, y, prec):
+        self._chk(self.lib.qxd_blas_copy(self.h, prec, _ptr(x), _ptr(y)))
+
+    def blas_zero(self, x, prec):
+        self._chk(self.lib.qxd_blas_zero(self.h, prec, _ptr(x)))
 
     # -- packed layout -------------------------------------------------------------------------------
     def packed_spinor_bytes(self, prec, half_only=False):

@@ -512,6 +512,105 @@ int qxd_apply_Dw_host(qxd_ctx* c, int prec, const double* psi_host, double* out_
   return QXD_OK;
 }
 
+// ---- domain decomposition building blocks (row f2) ------------------------------------------------------------------
+int qxd_time_slabs(const qxd_ctx* c, int* nslabs, int* thickness) {
+  if (!c || !nslabs || !thickness) return QXD_EINVAL;
+  std::vector<TileMap> maps;
+  size_t slab_sites = 0;
+  if (!time_slabs(c, maps, slab_sites)) return QXD_EINVAL;
+  *nslabs = int(maps.size()); *thickness = c->tile[0];
+  return QXD_OK;
+}
+
+int qxd_dslash_packed(qxd_ctx* c, int prec, int mode, int flags, int parity_out, const void* in, const void* phi, void* out, int slab_lo, int slab_hi) {
+  int rc = check_apply(c, prec, in, out, "dslash_packed");
+  if (rc) return rc;
+  if (mode < 0 || mode >= DS_NMODES || (flags & ~(DSF_G5IN | DSF_G5HOP)) || parity_out < 0 || parity_out > 1) return fail(c, QXD_EINVAL, "dslash_packed: bad mode, flags or parity");
+  const bool needs_phi = mode == DS_A_XMHOP || mode == DS_X_MHOP || mode == DS_AINV_X_MHOP;
+  if (needs_phi && !phi) return fail(c, QXD_EINVAL, "dslash_packed: this mode needs phi");
+  std::vector<TileMap> maps;
+  size_t slab_sites = 0;
+  if (!time_slabs(c, maps, slab_sites)) return fail(c, QXD_EINVAL, "dslash_packed: the site order has no time slabs");
+  if (slab_lo < 0 || slab_hi > int(maps.size()) || slab_lo > slab_hi) return fail(c, QXD_EINVAL, "dslash_packed: bad slab range");
+  const int Vh = c->g.Vh;
+  DslashCall d{};
+  d.prec = prec; d.mode = mode; d.flags = flags; d.parity_out = parity_out;
+  void* inp = const_cast<void*>(in);
+  void* php = const_cast<void*>(phi);
+  if (mode == DS_DW_FULL) {
+    d.in[0] = half_view(prec, inp, Vh, 0); d.in[1] = half_view(prec, inp, Vh, 1);
+    d.out[0] = half_view(prec, out, Vh, 0); d.out[1] = half_view(prec, out, Vh, 1);
+  } else {
+    d.in[1 - parity_out] = half_view(prec, inp, Vh, 1 - parity_out);
+    if (needs_phi) d.phi = half_view(prec, php, Vh, parity_out);
+    d.out[parity_out] = half_view(prec, out, Vh, parity_out);
+  }
+  for (int k = slab_lo; k < slab_hi; k++) {
+    d.tm = maps[k];
+    if ((rc = launch_dslash(c, d))) return rc;
+  }
+  return QXD_OK;
+}
+
+int qxd_clover_apply_packed(qxd_ctx* c, int prec, int inverse, int parity, const void* in, void* out) {
+  int rc = check_apply(c, prec, in, out, "clover_apply_packed");
+  if (rc) return rc;
+  if (parity < 0 || parity > 1) return fail(c, QXD_EINVAL, "clover_apply_packed: parity 0 or 1");
+  if (inverse && !c->Mi[prec][parity]) return fail(c, QXD_EINVAL, "clover_apply_packed: the even-site inverses exist in fp64 only");
+  const int Vh = c->g.Vh;
+  return launch_clover_apply(c, prec, inverse, parity, half_view(prec, const_cast<void*>(in), Vh, parity), half_view(prec, out, Vh, parity));
+}
+
+size_t qxd_face_bytes(const qxd_ctx* c, int prec, int mu) {
+  if (!c || prec < 0 || prec >= NPREC || mu < 0 || mu > 3) return 0;
+  return face_bytes(c, prec, mu);
+}
+static int check_halo(qxd_ctx* c, int prec, const void* a, const void* b, int pmask, int mu, const char* who) {
+  if (!c) return QXD_EINVAL;
+  if (!a || !b) return fail(c, QXD_EINVAL, std::string(who) + ": null pointer");
+  if (!c->ws) return fail(c, QXD_EWORKSPACE, std::string(who) + ": no workspace bound");
+  if (prec < 0 || prec >= NPREC || pmask < 1 || pmask > 3 || mu < 0 || mu > 3) return fail(c, QXD_EINVAL, std::string(who) + ": bad precision, parity mask or direction");
+  return QXD_OK;
+}
+int qxd_face_gather(qxd_ctx* c, int prec, const void* packed, int pmask, int mu, int coord, int sign, void* buf) {
+  int rc = check_halo(c, prec, packed, buf, pmask, mu, "face_gather");
+  if (rc) return rc;
+  if (sign != 1 && sign != -1) return fail(c, QXD_EINVAL, "face_gather: sign must be +1 or -1");
+  return launch_face_gather(c, prec, const_cast<void*>(packed), pmask, mu, coord, sign, buf);
+}
+int qxd_face_scatter(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int coord, int shift1, const void* buf) {
+  int rc = check_halo(c, prec, packed, buf, pmask, mu, "face_scatter");
+  if (rc) return rc;
+  return launch_face_scatter(c, prec, packed, pmask, mu, coord, shift1, buf);
+}
+int qxd_halo_zero(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int lo, int hi) {
+  int rc = check_halo(c, prec, packed, packed, pmask, mu, "halo_zero");
+  if (rc) return rc;
+  return launch_halo_zero(c, prec, packed, pmask, mu, lo, hi);
+}
+static bool blas_args_ok(qxd_ctx* c, int prec) { return c && c->ws && prec >= 0 && prec < NPREC; }
+static SpinorPtr hp(qxd_ctx* c, int prec, const void* p) { return half_view(prec, const_cast<void*>(p), c->g.Vh, 0); }
+int qxd_blas_norm2_dev(qxd_ctx* c, int prec, const void* x, double* out) {
+  if (!blas_args_ok(c, prec) || !x || !out) return QXD_EINVAL;
+  return blas_norm2(c, prec, hp(c, prec, x), out, Batch(), true);
+}
+int qxd_blas_cg_xr(qxd_ctx* c, int prec, const double* num, const double* den, const void* p, const void* t, void* x, void* r, double* rr) {
+  if (!blas_args_ok(c, prec) || !num || !den || !p || !t || !x || !r || !rr) return QXD_EINVAL;
+  return blas_cg_xr(c, prec, num, den, hp(c, prec, p), hp(c, prec, t), hp(c, prec, x), hp(c, prec, r), rr);
+}
+int qxd_blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, const void* s, void* p) {
+  if (!blas_args_ok(c, prec) || !num || !den || !s || !p) return QXD_EINVAL;
+  return blas_cg_p(c, prec, num, den, hp(c, prec, s), hp(c, prec, p));
+}
+int qxd_blas_copy(qxd_ctx* c, int prec, const void* x, void* y) {
+  if (!blas_args_ok(c, prec) || !x || !y) return QXD_EINVAL;
+  return blas_copy(c, prec, hp(c, prec, x), hp(c, prec, y));
+}
+int qxd_blas_zero(qxd_ctx* c, int prec, void* x) {
+  if (!blas_args_ok(c, prec) || !x) return QXD_EINVAL;
+  return blas_zero(c, prec, hp(c, prec, x));
+}
+
 int qxd_solve(qxd_ctx* c, const double* eta, double* psi, double tol, qxd_solve_info* info) {
   qxd_solve_info local;
   if (!info) { std::memset(&local, 0, sizeof(local)); info = &local; }

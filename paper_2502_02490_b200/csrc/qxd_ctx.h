@@ -188,6 +188,11 @@ int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, cons
 // solver.cu
 int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
 int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+// halo.cu (row f2)
+size_t face_bytes(const qxd_ctx* c, int prec, int mu);
+int launch_face_gather(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int coord, int sign, void* buf);
+int launch_face_scatter(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int coord, int shift1, const void* buf);
+int launch_halo_zero(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int lo, int hi);
 // sap.cu / gcr.cu (row f3)
 int sap_check_geometry(qxd_ctx* c);
 int launch_sap(qxd_ctx* c, int prec, const void* in_full32, void* out_full32);   // out = M_sap in (fp32 packed full-lattice vectors)

@@ -65,11 +65,12 @@ template <typename S> struct SapShape {
 
 // in-block hop from shared memory: acc += (1 -+ gamma_mu) W psi(x +- mu) for a neighbour inside the block, nothing otherwise
 template <typename S, int MU, int DIR, bool PAIR>
-__device__ __forceinline__ void hop_sm(const SapArgs& a, const Site& s, int tile, int par, int l, const float4* rho,
+__device__ __forceinline__ void hop_sm(const unsigned (&nbc)[2], int par, int l, const float4* rho,
                                        const typename PT<S>::V* Wsm, float* acc) {
-  const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
-  if ((nb >> 7) != tile) return;
-  const int ln = nb & 127;
+  constexpr int D = 2 * MU + (DIR < 0 ? 1 : 0);
+  const unsigned code = (nbc[D >> 2] >> (8 * (D & 3))) & 0xffu;   // bit 7: neighbour inside the block, bits 0-6: its local index
+  if (!(code & 0x80u)) return;
+  const int ln = code & 0x7f;
   float psi[24], w[18], h[12], t[12];
 #pragma unroll
   for (int c = 0; c < 6; c++) unpack4(rho[((1 - par) * 6 + c) * 128 + ln], psi + 4 * c);
@@ -155,19 +156,19 @@ __device__ __forceinline__ void stage_site(const SapArgs& a, int cb, int par, in
 
 // t = D_Lambda rho at the thread's site, all operands from shared memory
 template <typename S, bool PAIR>
-__device__ __forceinline__ void block_apply(const SapArgs& a, const Site& s, int tile, int cb, int par, int l, const float4* rho,
+__device__ __forceinline__ void block_apply(const unsigned (&nbc)[2], int cb, int par, int l, const float4* rho,
                                             const typename PT<S>::V* Wsm, const typename PT<S>::V* Csm, const float* own, float* t) {
   float acc[24];
 #pragma unroll
   for (int i = 0; i < 24; i++) acc[i] = 0.f;
-  hop_sm<S, 0, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 0, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 1, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 1, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 2, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 2, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 3, +1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
-  hop_sm<S, 3, -1, PAIR>(a, s, tile, par, l, rho, Wsm, acc);
+  hop_sm<S, 0, +1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 0, -1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 1, +1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 1, -1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 2, +1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 2, -1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 3, +1, PAIR>(nbc, par, l, rho, Wsm, acc);
+  hop_sm<S, 3, -1, PAIR>(nbc, par, l, rho, Wsm, acc);
   const bool mir = PAIR && (cb & 1);
   const typename PT<S>::V* cl = Csm + par * SapShape<S>::NCH * 128;
 #pragma unroll
@@ -211,6 +212,16 @@ __global__ void __launch_bounds__(256, SapShape<S>::MINB) sap_mr_k(const __grid_
   stage_site<S, NL, PAIR>(a, cb, par, l, Wsm, Csm);
   Site s;
   site_init<PAIR ? 1 : 0>(a.g, cb, par, s);
+  // the eight neighbours, once: inside the block (bit 7) and local index (the index arithmetic is not repeated per MR step)
+  unsigned nbc[2];
+  {
+    const int n[8] = {neighbour_cb<0, +1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<0, -1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<1, +1, PAIR ? 1 : 0>(a.g, s),
+                      neighbour_cb<1, -1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<2, +1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<2, -1, PAIR ? 1 : 0>(a.g, s),
+                      neighbour_cb<3, +1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<3, -1, PAIR ? 1 : 0>(a.g, s)};
+    nbc[0] = 0; nbc[1] = 0;
+#pragma unroll
+    for (int d = 0; d < 8; d++) nbc[d >> 2] |= ((((n[d] >> 7) == tile) ? 0x80u : 0u) | unsigned(n[d] & 127)) << (8 * (d & 3));
+  }
   float r[24], e[24];
 #pragma unroll
   for (int c = 0; c < 6; c++) unpack4(__ldg(a.src[par] + size_t(c) * Vh + cb), r + 4 * c);
@@ -237,7 +248,7 @@ __global__ void __launch_bounds__(256, SapShape<S>::MINB) sap_mr_k(const __grid_
   __syncthreads();
   for (int it = 0; it < a.nmr; it++) {
     float t[24];
-    block_apply<S, PAIR>(a, s, tile, cb, par, l, rho, Wsm, Csm, r, t);
+    block_apply<S, PAIR>(nbc, cb, par, l, rho, Wsm, Csm, r, t);
     // alpha = <t, r> / <t, t> over the block (minimal residual step)
     float p0 = 0.f, p1 = 0.f, p2 = 0.f;
 #pragma unroll

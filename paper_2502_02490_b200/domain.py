@@ -1,105 +1,502 @@
-"""Time-slab domain decomposition of the D_w apply over ranks (first step).
+"""Domain decomposition of the D_w apply and solve over ranks.
 
-The paper's codes run on rank-local lattices with a neighbour map between ranks and exchange
-boundary data before the operator is applied.  Here the lattice is cut along time, T_loc = T / world
-slices per rank.  Every rank works on a LOCAL lattice of T_loc + 2 slices: its own slices plus one ghost slice below
-and one above.  Gauge field and U(1) field of the ghost slices are part of the rank's fields (loaded once); the ghost
-slices of the spinor are filled by one exchange with the two time neighbours before every apply (torch.distributed
-send/recv: NCCL over NVLink between GPUs, gloo in the CPU tests).  The existing single-GPU kernels then run unchanged
-on the local lattice and the ghost slices of the result are discarded: every interior site sees exactly the neighbours,
-links and clover leaves of the global lattice (a leaf reaches one site from its corner), so the decomposition is correct
-by construction.  The local lattice is periodic in its own time direction, which only couples the two ghost slices to
-each other; the global antiperiodic boundary condition is carried by the sign of the time links of global slice T-1
-(reading R9), which cancels in every clover leaf.  C* boundaries are spatial and stay rank-local.
+The paper's codes run on rank-local lattices, exchange boundary data before the operator is applied
+ and realise C* boundary conditions by changing the neighbour map between ranks ("shifted boundaries",
+PAPER.md:137-139).  Here:
 
-This module is host logic only (index arithmetic, slicing, the exchange).  What applies the operator is passed in: the
-CUDA context on a GPU rank, the oracle in the CPU tests.  Cost of this first step: 2 / T_loc redundant work and one
-exchange per apply that is not yet overlapped with the interior; both are what a fused halo kernel would remove.
+* :class:`ProcessGrid` is that neighbour map as a pure function: a hop across the global boundary of a C* direction
+  k in 2..cstar lands, on the lattice doubled in direction 1, displaced by L1 in direction 1 -- on the rank N1/2 further
+  along direction 1 if that direction is distributed, else on the same rank column with a LOCAL displacement by L1.
+* :class:`LocalLattice` is a rank's lattice: its own sites plus ghost layers in the cut directions (time: one tile = 4 slices
+  thick, so that the owned sites are whole time slabs of the device site order and nothing is computed on ghosts; direction
+  3: two layers, the one next to the owned sites carrying data).  Gauge and U(1) fields of the ghost layers are loaded with the rank's fields, once.
+* :func:`halo_exchange` fills the spinor ghost layers: the boundary layer is spin-projected to 12 reals per site by a kernel
+  (qxd_face_gather), the face buffers travel as ONE batch of point-to-point operations (NCCL between GPUs), and
+  qxd_face_scatter writes the ghost spinors, displaced by L1 where the message crossed a C* boundary.
+* :class:`GpuRank` applies D_w and the even-odd operator D-hat with the unchanged single-GPU kernels on the owned time slabs:
+  interior slabs are launched first and run while the faces are in flight, the two boundary slabs after the ghosts have arrived.
+* :func:`cgne` is the distributed CG on the normal equations: every scalar is all-reduced over the ranks.
+
+The module is written against two small interfaces so that the same code runs (a) one rank per process under
+torch.distributed (``TorchComm``; NCCL on GPUs, gloo in the CPU tests) and (b) all ranks of a decomposition inside one
+process, one after the other (``LocalComm``: how a decomposition is verified on the single GPU a test box has).  What applies
+the operator on a rank is an ``ops`` object: :class:`GpuRank` here, the fp64 oracle in the CPU tests.
 """
 from __future__ import annotations
 
 import numpy as np
 
+TIME_GHOST = 4          # thickness of the time ghost zones = tile extent b0 of the device site order
+SPACE_GHOST = 2         # thickness of the direction-3 ghost zones (keeps the local extent a multiple of the tile extent 4;
+                        # only the layer next to the owned sites carries data)
 
-class TimeSlabs:
-    """Geometry of rank `rank` of `world` for a global physical lattice dims = (T, L1, L2, L3)."""
 
-    def __init__(self, dims, world: int, rank: int):
-        T = int(dims[0])
-        if world < 1 or not (0 <= rank < world):
-            raise ValueError("TimeSlabs: need world >= 1 and 0 <= rank < world")
-        if T % world or (T // world) % 2 or T // world < 2:
-            raise ValueError("TimeSlabs: T must split into an even number (>= 2) of slices per rank")
-        self.dims = tuple(int(d) for d in dims)
-        self.world, self.rank = world, rank
-        self.T, self.T_loc = T, T // world
-        self.t0 = rank * self.T_loc
-        self.local_dims = (self.T_loc + 2,) + self.dims[1:]
-        self.prev, self.next = (rank - 1) % world, (rank + 1) % world
+class ProcessGrid:
+    """Ranks on a 4D grid, direction 3 fastest; the C* neighbour map of PAPER.md:139 as a pure function."""
 
-    def time_index(self):
-        """Global time slice of every local slice (ghost below, interior, ghost above)."""
-        return [(self.t0 - 1 + k) % self.T for k in range(self.T_loc + 2)]
+    def __init__(self, dims, grid, cstar=0):
+        self.dims = tuple(int(d) for d in dims)              # global PHYSICAL extents T, L1, L2, L3
+        self.grid = tuple(int(n) for n in grid)
+        self.cstar = int(cstar)
+        self.ext = (self.dims[0], (2 if cstar else 1) * self.dims[1], self.dims[2], self.dims[3])   # extended lattice
+        for mu in range(4):
+            if self.grid[mu] < 1 or self.ext[mu] % self.grid[mu] or (self.ext[mu] // self.grid[mu]) % 2:
+                raise ValueError("ProcessGrid: every direction must split into an even number of sites per rank")
+        if cstar and self.grid[1] > 1 and self.grid[1] % 2:
+            raise ValueError("ProcessGrid: with C* boundaries direction 1 (doubled) needs an even number of ranks")
+        self.local_ext = tuple(self.ext[mu] // self.grid[mu] for mu in range(4))
+        self.world = int(np.prod(self.grid))
 
-    def local_fields(self, U, A=None, antiperiodic=True):
-        """Rank-local gauge field (and U(1) field) including the ghost slices.  With antiperiodic fermions the time links
-        of global slice T-1 carry the factor -1 and the local context is created WITHOUT the antiperiodic bit."""
-        idx = self.time_index()
-        Ul = np.ascontiguousarray(np.asarray(U)[idx])
-        if antiperiodic:
-            for k, t in enumerate(idx):
-                if t == self.T - 1:
-                    Ul[k, ..., 0, :, :] *= -1.0
-        Al = None if A is None else np.ascontiguousarray(np.asarray(A)[idx])
+    def coords(self, rank):
+        c = []
+        for n in reversed(self.grid):
+            c.append(rank % n)
+            rank //= n
+        return tuple(reversed(c))
+
+    def rank(self, coords):
+        r = 0
+        for c, n in zip(coords, self.grid):
+            r = r * n + (c % n)
+        return r
+
+    def neighbour(self, rank, mu, direction):
+        """(rank of the neighbour in direction +-mu, local displacement in direction 1 applied to data that arrive from / go
+        to it, crossed): a hop over the global boundary of a C* direction k (2 <= k <= cstar) is displaced by L1 on the doubled
+        lattice: N1/2 ranks along direction 1 if it is distributed, else L1 sites locally."""
+        c = list(self.coords(rank))
+        n = c[mu] + direction
+        crossed = n < 0 or n >= self.grid[mu]
+        c[mu] = n % self.grid[mu]
+        shift1 = 0
+        if crossed and 2 <= mu <= self.cstar:
+            if self.grid[1] > 1:
+                c[1] = (c[1] + self.grid[1] // 2) % self.grid[1]
+            else:
+                shift1 = self.dims[1]
+        return self.rank(c), shift1, crossed
+
+    def owner(self, x):
+        """Rank that owns the extended global site x, and its local (ghost-free) coordinates."""
+        c = tuple(x[mu] // self.local_ext[mu] for mu in range(4))
+        return self.rank(c), tuple(x[mu] % self.local_ext[mu] for mu in range(4))
+
+
+class LocalLattice:
+    """The lattice of one rank: owned sites + ghost layers in the cut directions 0 and 3 (directions 1, 2 are not cut)."""
+
+    def __init__(self, pg: ProcessGrid, rank: int, antiperiodic=True, force_cut=(False, False, False, False)):
+        if pg.grid[1] != 1 or pg.grid[2] != 1:
+            raise ValueError("LocalLattice: fields are decomposed along directions 0 and 3 only")
+        self.pg, self.rank = pg, rank
+        self.c = pg.coords(rank)
+        self.cut = tuple(pg.grid[mu] > 1 or bool(force_cut[mu]) for mu in range(4))
+        if self.cut[1] or self.cut[2]:
+            raise ValueError("LocalLattice: cuts along directions 0 and 3 only")
+        self.g = (TIME_GHOST if self.cut[0] else 0, 0, 0, SPACE_GHOST if self.cut[3] else 0)
+        T, L1, L2, L3 = pg.dims
+        self.own = (T // pg.grid[0], L1, L2, L3 // pg.grid[3])             # owned PHYSICAL extents
+        self.local_dims = tuple(self.own[mu] + 2 * self.g[mu] for mu in range(4))
+        self.origin = (self.c[0] * self.own[0], 0, 0, self.c[3] * self.own[3])
+        # boundary conditions of the local context: a cut direction is handled by the ghosts (periodic locally, which only
+        # couples ghost layers to each other); the C* count drops to 2 when direction 3 is cut
+        self.cstar_local = pg.cstar if not (self.cut[3] and pg.cstar == 3) else 2
+        self.antiperiodic = bool(antiperiodic)
+        self.bc_local = self.cstar_local | ((1 if (antiperiodic and not self.cut[0]) else 0) << 2)
+        X1 = (2 if pg.cstar else 1) * L1
+        self.local_ext = (self.local_dims[0], X1, L2, self.local_dims[3])   # extended local lattice (spinors)
+        if self.cut[0] and (self.own[0] % TIME_GHOST or self.own[0] < 2 * TIME_GHOST):
+            raise ValueError("LocalLattice: a time cut needs T_loc to be a multiple of 4 and >= 8 (whole tiles, two boundary slabs)")
+
+    # ---- index maps -------------------------------------------------------------------------------------------------
+    def _global_index(self):
+        """For every local PHYSICAL site (incl. ghosts): global physical coordinates and whether the site is a C* mirror image
+        (reached through an odd number of C* boundary crossings in direction 3)."""
+        T, L1, L2, L3 = self.pg.dims
+        t = (self.origin[0] - self.g[0] + np.arange(self.local_dims[0])) % T
+        zr = self.origin[3] - self.g[3] + np.arange(self.local_dims[3])
+        z = zr % L3
+        mirror = ((zr // L3) % 2 != 0) & (self.pg.cstar == 3)
+        return t, z, mirror
+
+    def local_fields(self, U, A=None):
+        """Rank-local gauge field (and U(1) field) including the ghost layers.  With antiperiodic fermions and a time cut the
+        time links of global slice T-1 carry the factor -1 (the local context is then periodic in time); links of ghost
+        layers reached across a C* boundary are the mirror images conj(U), -A (reading R8)."""
+        t, z, mirror = self._global_index()
+        U = np.asarray(U)
+        Ul = np.ascontiguousarray(U[t][:, :, :, z])
+        Ul[:, :, :, mirror] = np.conj(Ul[:, :, :, mirror])
+        if self.antiperiodic and self.cut[0]:
+            Ul[t == self.pg.dims[0] - 1, ..., 0, :, :] *= -1.0
+        Al = None
+        if A is not None:
+            Al = np.ascontiguousarray(np.asarray(A)[t][:, :, :, z])
+            Al[:, :, :, mirror] *= -1.0
         return Ul, Al
 
-    @staticmethod
-    def local_bc(cstar: int) -> int:
-        """bc word of the local context: same C* directions, periodic in (local) time."""
-        return int(cstar) & 3
+    def owned_slices(self):
+        return (slice(self.g[0], self.g[0] + self.own[0]), slice(None), slice(None), slice(self.g[3], self.g[3] + self.own[3]))
 
     def scatter(self, psi_global):
-        """Interior slices of this rank from a global extended-lattice spinor [T][X1][L2][L3][4][3], with empty ghosts."""
+        """Owned part of a global extended-lattice spinor [T][X1][L2][L3][4][3] placed into a local array with empty ghosts."""
         psi_global = np.asarray(psi_global)
-        loc = np.zeros((self.T_loc + 2,) + psi_global.shape[1:], dtype=psi_global.dtype)
-        loc[1:self.T_loc + 1] = psi_global[self.t0:self.t0 + self.T_loc]
+        loc = np.zeros(self.local_ext + psi_global.shape[4:], dtype=psi_global.dtype)
+        o = self.origin
+        loc[self.owned_slices()] = psi_global[o[0]:o[0] + self.own[0], :, :, o[3]:o[3] + self.own[3]]
         return loc
 
-    def interior(self, local):
-        return local[1:self.T_loc + 1]
+    def gather_into(self, psi_global, local):
+        o = self.origin
+        psi_global[o[0]:o[0] + self.own[0], :, :, o[3]:o[3] + self.own[3]] = np.asarray(local).reshape(self.local_ext + psi_global.shape[4:])[self.owned_slices()]
+
+    def messages(self):
+        """The halo messages this rank SENDS, one per cut direction and side: dicts with the layer to gather (coord, sign of
+        the projector the receiver's hop applies), the destination rank, the ghost layer it fills there and the displacement
+        in direction 1 the receiver applies (C* shifted boundary)."""
+        out = []
+        for mu in (3, 0):     # direction 3 first: its ghosts are needed by every time slab
+            if not self.cut[mu]:
+                continue
+            g, n = self.g[mu], self.own[mu]
+            up, s_up, _ = self.pg.neighbour(self.rank, mu, +1)
+            dn, s_dn, _ = self.pg.neighbour(self.rank, mu, -1)
+            # upward: my last owned layer -> lower ghost of the next rank, read there by backward hops: (1 + gamma_mu)
+            out.append(dict(mu=mu, side="up", coord=g + n - 1, sign=-1, dst=up, ghost=g - 1, shift1=s_up))
+            # downward: my first owned layer -> upper ghost of the previous rank, read there by forward hops: (1 - gamma_mu)
+            out.append(dict(mu=mu, side="down", coord=g, sign=+1, dst=dn, ghost=g + n, shift1=s_dn))
+        return out
 
 
-def exchange_time_ghosts(ts: TimeSlabs, local, dist=None):
-    """Fill the two ghost slices of `local` (tensor or array [T_loc+2][...]) from the time neighbours.  world == 1:
-    periodic self-copy.  The four point-to-point operations go out as ONE batch (dist.batch_isend_irecv = one
-    ncclGroupStart/End under NCCL): NCCL ignores tags and serialises the p2p operations of a peer pair on one stream, so
-    with world == 2 (previous and next rank are the same peer) four separately issued isend/irecv calls could block each
-    other; inside a group they cannot.  The pairing does not rely on tags: for every peer both sides list the upward
-    message (my last interior slice -> the next rank's lower ghost) before the downward one, and messages between a pair
-    of ranks are matched in issue order."""
-    Tl = ts.T_loc
-    if ts.world == 1 or dist is None:
-        if ts.world != 1:
-            raise ValueError("exchange_time_ghosts: a process group is needed for world > 1")
-        local[0] = local[Tl]
-        local[Tl + 1] = local[1]
-        return local
-    import torch
-    t = local if isinstance(local, torch.Tensor) else torch.from_numpy(local)
-    up_send, down_send = t[Tl].contiguous(), t[1].contiguous()
-    low_recv, high_recv = torch.empty_like(up_send), torch.empty_like(down_send)
-    ops = [dist.P2POp(dist.isend, up_send, ts.next), dist.P2POp(dist.irecv, low_recv, ts.prev),       # upward
-           dist.P2POp(dist.isend, down_send, ts.prev), dist.P2POp(dist.irecv, high_recv, ts.next)]    # downward
-    for r in dist.batch_isend_irecv(ops):
-        r.wait()
-    t[0].copy_(low_recv)
-    t[Tl + 1].copy_(high_recv)
-    return local
+# ---------------------------------------------------------------------------------------------------------------------
+# communication: one rank per process (torch.distributed) or all ranks in one process (verification on one device)
+# ---------------------------------------------------------------------------------------------------------------------
+class LocalComm:
+    """All ranks of the decomposition live in this process (ops[r] for every rank r); messages are copies."""
+
+    def __init__(self, world):
+        self.world = world
+        self.my_ranks = list(range(world))
+
+    def exchange(self, sends):
+        """sends: list of (src, dst, tag, tensor).  Returns {(dst, tag): tensor}."""
+        return {(dst, tag): t.clone() for (src, dst, tag, t) in sends}
+
+    def allreduce_sum(self, per_rank):
+        """per_rank: {rank: 0-d / 1-element tensor}; every tensor is replaced by the sum over ranks, in place."""
+        vals = list(per_rank.values())
+        tot = vals[0].clone()
+        for v in vals[1:]:
+            tot += v.to(tot.device)
+        for v in vals:
+            v.copy_(tot.to(v.device))
 
 
-def apply_Dw_distributed(ts: TimeSlabs, local_psi, apply_local, dist=None):
-    """One distributed D_w apply: exchange the ghost slices, apply the local operator `apply_local(local_psi) -> local_out`
-    (the CUDA context of this rank, or the oracle in CPU tests) on the T_loc + 2 lattice, return the interior slices."""
-    exchange_time_ghosts(ts, local_psi, dist)
-    out = apply_local(local_psi)
-    return ts.interior(out.reshape(local_psi.shape))
+class TorchComm:
+    """One rank per process under torch.distributed (NCCL on GPUs, gloo on CPU).  All point-to-point operations of an
+    exchange go out as ONE batch (one ncclGroup): NCCL ignores tags and serialises the operations of a peer pair on one
+    stream, so separately issued sends and receives between two ranks could block each other; messages between a pair are
+    matched by issue order, which is the same on both sides (direction 3 before 0, upward before downward).  A message to
+    the rank itself (a direction with a single rank but ghosts) is a copy unless `self_via_dist` asks for a real send/recv
+    pair (how the NCCL path is exercised on a single GPU)."""
+
+    def __init__(self, dist, self_via_dist=False):
+        self.dist = dist
+        self.world = dist.get_world_size()
+        self.rank = dist.get_rank()
+        self.my_ranks = [self.rank]
+        self.self_via_dist = self_via_dist
+
+    def exchange(self, sends, recv_like):
+        """sends: list of (src = me, dst, tag, tensor); recv_like: list of (src, tag, template tensor) in the SAME order in
+        which the peers list their sends.  Returns {(me, tag): tensor}."""
+        import torch
+        dist = self.dist
+        out, ops = {}, []
+        for (src, dst, tag, t) in sends:
+            if dst == self.rank and not self.self_via_dist:
+                continue
+            ops.append(dist.P2POp(dist.isend, t, dst))
+        for (src, tag, like) in recv_like:
+            if src == self.rank and not self.self_via_dist:
+                mine = [t for (s, d, tg, t) in sends if d == self.rank and tg == tag]
+                out[(self.rank, tag)] = mine[0].clone()
+                continue
+            buf = torch.empty_like(like)
+            out[(self.rank, tag)] = buf
+            ops.append(dist.P2POp(dist.irecv, buf, src))
+        if ops:
+            for r in dist.batch_isend_irecv(ops):
+                r.wait()
+        return out
+
+    def allreduce_sum(self, per_rank):
+        for v in per_rank.values():
+            if self.world > 1:
+                self.dist.all_reduce(v)
+
+
+def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 0)):
+    """Fill the ghost layers of the spinors vecs[r] (r over the ranks this process holds) in the given cut directions.
+    Gather kernels -> one batched exchange -> scatter kernels.  The tag of a message is (mu, side)."""
+    sends, recv_like = [], {}
+    for r in comm.my_ranks:
+        for m in lats[r].messages():
+            if m["mu"] not in directions:
+                continue
+            buf = ops[r].face_gather(vecs[r], parity_mask, m["mu"], m["coord"], m["sign"])
+            sends.append((r, m["dst"], (m["mu"], m["side"]), buf))
+    if isinstance(comm, LocalComm):
+        arrived = comm.exchange(sends)
+    else:
+        r = comm.my_ranks[0]
+        rl = []
+        for m in lats[r].messages():          # what I receive mirrors what I send: the "up" message comes from below
+            if m["mu"] not in directions:
+                continue
+            src = lats[r].pg.neighbour(r, m["mu"], -1 if m["side"] == "up" else +1)[0]
+            like = [t for (s, d, tg, t) in sends if tg == (m["mu"], m["side"])][0]
+            rl.append((src, (m["mu"], m["side"]), like))
+        arrived = comm.exchange(sends, rl)
+    for r in comm.my_ranks:
+        lat = lats[r]
+        for mu in directions:
+            if not lat.cut[mu]:
+                continue
+            g, n = lat.g[mu], lat.own[mu]
+            for side, ghost, d in (("up", g - 1, -1), ("down", g + n, +1)):
+                shift1 = lat.pg.neighbour(r, mu, d)[1]      # displacement of data that crossed my lower / upper boundary
+                ops[r].face_scatter(vecs[r], parity_mask, mu, ghost, shift1, arrived[(r, (mu, side))])
+
+
+def halo_clear(lats, ops, vecs, ranks, parity_mask=3):
+    """Zero the ghost layers (after the operator has used them), so that reductions over a vector see owned sites only."""
+    for r in ranks:
+        lat = lats[r]
+        for mu in (0, 3):
+            if lat.cut[mu]:
+                g, n = lat.g[mu], lat.own[mu]
+                ops[r].halo_zero(vecs[r], parity_mask, mu, 0, g)
+                ops[r].halo_zero(vecs[r], parity_mask, mu, g + n, 2 * g + n)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# a rank on a GPU: the C-ABI library on the local lattice
+# ---------------------------------------------------------------------------------------------------------------------
+class GpuRank:
+    """One rank's CUDA context on its local lattice (fields with ghost layers loaded once) and the per-rank steps of the
+    distributed operator.  Vectors are packed FULL-lattice buffers of the storage precision `prec` (torch uint8 tensors)."""
+
+    def __init__(self, lat: LocalLattice, U, A, qel, kappa, q, csw, csw_qed, prec=0, device="cuda:0", pairing=None):
+        from . import binding as B
+        self.B, self.lat, self.prec = B, lat, prec
+        Ul, Al = lat.local_fields(U, A)
+        self.g = B.Qxd(*lat.local_dims, lat.bc_local, precisions=tuple({B.QXD_F64, prec}), device=device, pairing=pairing)
+        self.g.gauge_load(Ul, Al, qel)
+        self.g.set_quark(kappa, q)
+        self.g.clover_build(csw, csw_qed)
+        self.nslabs, self.thick = self.g.time_slabs()
+        gs = lat.g[0] // self.thick
+        self.owned = (gs, self.nslabs - gs)                       # owned time slabs [lo, hi)
+        self.hb = self.g.packed_spinor_bytes(prec, half_only=True)
+
+    def close(self):
+        self.g.close()
+
+    # vectors
+    def alloc(self):
+        return self.g.new_packed(self.prec)
+
+    def pack(self, local_nat):
+        return self.g.spinor_pack(np.ascontiguousarray(local_nat), self.prec)
+
+    def unpack(self, v):
+        return self.g.spinor_unpack(v, self.prec).cpu().numpy().reshape(self.lat.local_ext + (4, 3))
+
+    def half(self, v, parity=0):
+        return v[parity * self.hb:(parity + 1) * self.hb]
+
+    # halo kernels
+    def face_gather(self, v, pmask, mu, coord, sign):
+        buf = self.g.face_buffer(self.prec, mu)
+        return self.g.face_gather(v, self.prec, pmask, mu, coord, sign, buf)
+
+    def face_scatter(self, v, pmask, mu, coord, shift1, buf):
+        self.g.face_scatter(v, self.prec, pmask, mu, coord, shift1, buf)
+
+    def halo_zero(self, v, pmask, mu, lo, hi):
+        self.g.halo_zero(v, self.prec, pmask, mu, lo, hi)
+
+    # operator passes on a range of owned time slabs: which = "interior", "boundary" or "all"
+    def slab_ranges(self, which):
+        lo, hi = self.owned
+        if not self.lat.cut[0] or which == "all":
+            return [(lo, hi)] if which in ("all", "interior") else []
+        return [(lo + 1, hi - 1)] if which == "interior" else [(lo, lo + 1), (hi - 1, hi)]
+
+    def dslash(self, which, mode, vin, vout, parity_out=0, flags=0, phi=None):
+        for rng in self.slab_ranges(which):
+            if rng[1] > rng[0]:
+                self.g.dslash_packed(mode, vin, vout, self.prec, parity_out=parity_out, flags=flags, phi=phi, slabs=rng)
+
+
+def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, overlap=True):
+    """One dslash-shaped pass of the distributed operator on every rank of this process: direction-3 ghosts first (every slab
+    needs them), then the time faces -- in flight while the interior slabs run when there is one rank per process."""
+    ranks = comm.my_ranks
+    pm = 3 if mode == 0 else (1 << (1 - parity_out))
+    if any(lats[r].cut[3] for r in ranks):
+        halo_exchange(comm, lats, ops, vin, pm, directions=(3,))
+    time_cut = any(lats[r].cut[0] for r in ranks)
+    ph = {r: (phi[r] if phi is not None else None) for r in ranks}
+    if time_cut and overlap and isinstance(comm, TorchComm) and vin[ranks[0]].is_cuda:
+        import torch
+        r = ranks[0]
+        main = torch.cuda.current_stream()
+        if not hasattr(comm, "side"):
+            comm.side = torch.cuda.Stream()
+        sends = [(r, m["dst"], (m["mu"], m["side"]), ops[r].face_gather(vin[r], pm, m["mu"], m["coord"], m["sign"]))
+                 for m in lats[r].messages() if m["mu"] == 0]
+        rl = [(lats[r].pg.neighbour(r, 0, -1 if m["side"] == "up" else +1)[0], (0, m["side"]), t)
+              for m, (_, _, _, t) in zip([m for m in lats[r].messages() if m["mu"] == 0], sends)]
+        e1 = torch.cuda.Event()
+        e1.record(main)
+        with torch.cuda.stream(comm.side):
+            comm.side.wait_event(e1)
+            arrived = comm.exchange(sends, rl)
+            e2 = torch.cuda.Event()
+            e2.record(comm.side)
+        ops[r].dslash("interior", mode, vin[r], vout[r], parity_out, flags, ph[r])     # runs while the faces travel
+        main.wait_event(e2)
+        g, n = lats[r].g[0], lats[r].own[0]
+        for side, ghost, d in (("up", g - 1, -1), ("down", g + n, +1)):
+            ops[r].face_scatter(vin[r], pm, 0, ghost, lats[r].pg.neighbour(r, 0, d)[1], arrived[(r, (0, side))])
+        ops[r].dslash("boundary", mode, vin[r], vout[r], parity_out, flags, ph[r])
+    else:
+        if time_cut:
+            halo_exchange(comm, lats, ops, vin, pm, directions=(0,))
+        for r in ranks:
+            ops[r].dslash("all", mode, vin[r], vout[r], parity_out, flags, ph[r])
+    halo_clear(lats, ops, vin, ranks, pm)
+    # time ghosts are never computed (whole slabs are skipped); the direction-3 ghost layers lie inside the owned slabs and
+    # do receive (meaningless) results: clear them, so that the output is zero outside the owned sites
+    pmo = 3 if mode == 0 else (1 << parity_out)
+    for r in ranks:
+        if lats[r].cut[3]:
+            g, n = lats[r].g[3], lats[r].own[3]
+            ops[r].halo_zero(vout[r], pmo, 3, 0, g)
+            ops[r].halo_zero(vout[r], pmo, 3, g + n, 2 * g + n)
+
+
+class GpuOperator:
+    """The distributed operators on GPU ranks: D_w on full-lattice vectors and D-hat = A_ee - D_eo A_oo^{-1} D_oe on the even
+    halves (vectors are dicts rank -> packed buffer; the odd half of `tmp` is the intermediate of D-hat)."""
+
+    def __init__(self, comm, lats, ops, overlap=True):
+        self.comm, self.lats, self.ops, self.overlap = comm, lats, ops, overlap
+        self.ranks = comm.my_ranks
+        self.tmp = {r: ops[r].alloc() for r in self.ranks}
+        import torch
+        self.torch = torch
+
+    def alloc(self):
+        return {r: self.ops[r].alloc() for r in self.ranks}
+
+    def apply_Dw(self, vin, vout):
+        _pass(self.comm, self.lats, self.ops, vin, vout, 0, overlap=self.overlap)
+
+    def apply(self, vin, vout, dagger=False):
+        """vout_e = D-hat vin_e (dagger: D-hat^dagger)."""
+        B = self.ops[self.ranks[0]].B
+        _pass(self.comm, self.lats, self.ops, vin, self.tmp, B.QXD_DS_HOP_AINV, flags=B.QXD_DSF_G5IN if dagger else 0, parity_out=1, overlap=self.overlap)
+        _pass(self.comm, self.lats, self.ops, self.tmp, vout, B.QXD_DS_A_XMHOP, flags=B.QXD_DSF_G5HOP if dagger else 0, parity_out=0, phi=vin,
+              overlap=self.overlap)
+
+    # even-odd source preparation and reconstruction (row a8), distributed
+    def prepare(self, eta, b):
+        """b_e = eta_e - D_eo A_oo^{-1} eta_o"""
+        B = self.ops[self.ranks[0]].B
+        for r in self.ranks:
+            self.ops[r].g.clover_apply_packed(eta[r], self.tmp[r], self.ops[r].prec, 1, inverse=True)
+        _pass(self.comm, self.lats, self.ops, self.tmp, b, B.QXD_DS_X_MHOP, parity_out=0, phi=eta, overlap=self.overlap)
+
+    def reconstruct(self, eta, x):
+        """x_o = A_oo^{-1}(eta_o - D_oe x_e), written into the odd half of x"""
+        B = self.ops[self.ranks[0]].B
+        _pass(self.comm, self.lats, self.ops, x, x, B.QXD_DS_AINV_X_MHOP, parity_out=1, phi=eta, overlap=self.overlap)
+
+    # BLAS on the even halves with device-resident, all-reduced scalars
+    def scalar(self):
+        return {r: self.torch.zeros(1, dtype=self.torch.float64, device=self.ops[r].g.device) for r in self.ranks}
+
+    def norm2(self, v, out):
+        for r in self.ranks:
+            o = self.ops[r]
+            o.g.blas_norm2_dev(o.half(v[r]), o.prec, out[r])
+        self.comm.allreduce_sum(out)
+
+    def cg_xr(self, num, den, p, t, x, rvec, rr):
+        for r in self.ranks:
+            o = self.ops[r]
+            o.g.blas_cg_xr(o.prec, num[r], den[r], o.half(p[r]), o.half(t[r]), o.half(x[r]), o.half(rvec[r]), rr[r])
+        self.comm.allreduce_sum(rr)
+
+    def cg_p(self, num, den, s, p):
+        for r in self.ranks:
+            o = self.ops[r]
+            o.g.blas_cg_p(o.prec, num[r], den[r], o.half(s[r]), o.half(p[r]))
+
+    def copy(self, x, y):
+        for r in self.ranks:
+            o = self.ops[r]
+            o.g.blas_copy(o.half(x[r]), o.half(y[r]), o.prec)
+
+    def value(self, s):
+        return float(s[self.ranks[0]].item())
+
+
+def cgne(op, b, tol2_abs, maxiter=10000):
+    """Distributed CG on the normal equations of `op` keeping the system residual (reading R11), x = 0 start:
+    s = A^dag r, p = s, gam = |s|^2; loop: t = A p; al = gam/|t|^2; x += al p; r -= al t; stop on |r|^2 <= tol2_abs;
+    s = A^dag r; gam' = |s|^2; p = s + (gam'/gam) p.  Every scalar is a sum over all ranks (all-reduce).  Returns x, info."""
+    x, r, s, p, t = op.alloc(), op.alloc(), op.alloc(), op.alloc(), op.alloc()
+    gam, gam2, tt, rr = op.scalar(), op.scalar(), op.scalar(), op.scalar()
+    op.copy(b, r)
+    op.norm2(r, rr)
+    it, res2 = 0, op.value(rr)
+    if res2 > tol2_abs:
+        op.apply(r, s, dagger=True)
+        op.copy(s, p)
+        op.norm2(s, gam)
+    while res2 > tol2_abs and it < maxiter:
+        op.apply(p, t)
+        op.norm2(t, tt)
+        op.cg_xr(gam, tt, p, t, x, r, rr)
+        it += 1
+        res2 = op.value(rr)
+        if not (res2 == res2) or res2 <= tol2_abs:
+            break
+        op.apply(r, s, dagger=True)
+        op.norm2(s, gam2)
+        op.cg_p(gam2, gam, s, p)
+        gam, gam2 = gam2, gam
+    return x, dict(iters=it, res2=res2, status=0 if res2 <= tol2_abs else -5)
+
+
+def solve_distributed(op: GpuOperator, eta, tol, maxiter=10000):
+    """Solve D_w psi = eta on the decomposed lattice by even-odd preconditioning + distributed CGNE (fp64 storage).
+    eta: dict rank -> packed full-lattice buffer with clean ghosts.  Returns psi (same form) and a report."""
+    n2 = op.scalar()
+    tot = 0.0
+    for par in (0, 1):      # |eta|^2 over both parities and all ranks
+        for r in op.ranks:
+            o = op.ops[r]
+            o.g.blas_norm2_dev(o.half(eta[r], par), o.prec, n2[r])
+        op.comm.allreduce_sum(n2)
+        tot += op.value(n2)
+    b = op.alloc()
+    op.prepare(eta, b)
+    x, info = cgne(op, b, tol * tol * tot, maxiter)
+    op.reconstruct(eta, x)
+    info["true_res_eo"] = (info["res2"] / tot) ** 0.5 if tot > 0 else 0.0
+    return x, info

@@ -1,9 +1,13 @@
-"""Time-slab domain decomposition (row f2, first step; paper_2502_02490_b200/domain.py).
+"""Domain decomposition (paper_2502_02490_b200/domain.py).
 
-CPU: the decomposition and the ghost exchange are host logic; with the ORACLE as the rank-local operator the distributed
-apply must reproduce the oracle's global D_w -- sequentially emulated ranks (world 1, 2, 4) and a real world_size-2 `gloo`
-process group.  GPU: the same with the CUDA contexts as rank-local operators, ranks emulated one after the other on the one
-GPU (their kernels never wait on one another)."""
+CPU (`-m "not gpu"`): the C* rank map of PAPER.md:139 against the neighbour table of the global lattice (tests/lattice_np.py);
+the decomposition, the 12-real projected halo protocol and the distributed CG with the fp64 ORACLE as the rank-local operator,
+ranks emulated in one process (LocalComm) and as a real world_size-2 `gloo` group (TorchComm): D_w and the solve must reproduce
+the oracle on the global lattice.
+GPU: the same through the CUDA contexts and the device-side halo kernels (qxd_face_gather / qxd_face_scatter / qxd_halo_zero,
+interior / boundary time slabs), all ranks of a decomposition one after the other on the one GPU, plus a single rank whose
+ghost layers are filled by a real NCCL send/recv to itself with the exchange overlapping the interior slabs.
+"""
 import os
 import socket
 
@@ -11,62 +15,190 @@ import numpy as np
 import pytest
 
 import synth
+import lattice_np as LN
 from oracle import qxd_ref as R
 from paper_2502_02490_b200 import domain as D
 
 KAPPA, CSW, CSWQ, Q = 0.12, 1.5, 1.0, 2.0 / 3.0
 
 
-def global_reference(dims, cstar, ap, qed, psi):
+def fields(dims, qed):
+    return synth.su3_links(dims, 0.3, 1), (synth.u1_field(dims, 0.3, 2) if qed else None)
+
+
+def global_oracle(dims, cstar, ap, qed, U, A):
     ref = R.Ref(*dims, cstar | (ap << 2))
-    U = synth.su3_links(dims, 0.3, 1)
-    A = synth.u1_field(dims, 0.3, 2) if qed else None
     ref.gauge_load(U, A, 1.0)
     ref.set_quark(KAPPA, Q if qed else 0.0)
     ref.clover_build(CSW, CSWQ if qed else 0.0)
-    return U, A, ref.apply_Dw(psi)
+    return ref
 
 
-def oracle_local_operator(ts, U, A, cstar, ap, qed):
-    Ul, Al = ts.local_fields(U, A, antiperiodic=bool(ap))
-    ref = R.Ref(*ts.local_dims, D.TimeSlabs.local_bc(cstar))
-    ref.gauge_load(Ul, Al, 1.0)
-    ref.set_quark(KAPPA, Q if qed else 0.0)
-    ref.clover_build(CSW, CSWQ if qed else 0.0)
-    return ref.apply_Dw
+# ---- the rank map as a pure function ---------------------------------------------------------------------
+@pytest.mark.parametrize("dims,grid,cstar", [((8, 4, 4, 8), (2, 1, 1, 2), 3), ((4, 4, 4, 8), (1, 2, 1, 2), 3), ((4, 4, 8, 4), (1, 4, 2, 1), 2),
+                                             ((4, 4, 4, 4), (2, 1, 2, 1), 0), ((4, 2, 4, 8), (1, 1, 2, 4), 1)])
+def test_rank_map_matches_global_neighbour_table(dims, grid, cstar):
+    """For every site and every direction: the rank that owns the neighbour (global table with shifted C* boundaries) is the
+    rank the map names, and the neighbour's local coordinates are the stepped local coordinates displaced by the map's shift."""
+    pg = D.ProcessGrid(dims, grid, cstar)
+    lat = LN.Lattice(*dims, cstar=cstar)
+    for s in range(lat.V):
+        x = tuple(int(v) for v in lat.coords[s])
+        r, xl = pg.owner(x)
+        for mu in range(4):
+            for d, step in enumerate((+1, -1)):
+                y = tuple(int(v) for v in lat.coords[lat.nbr[mu, d, s]])
+                ry, yl = pg.owner(y)
+                leaves = not (0 <= xl[mu] + step < pg.local_ext[mu])
+                if not leaves:
+                    assert ry == r and yl == tuple(xl[k] + (step if k == mu else 0) for k in range(4))
+                    continue
+                rn, shift1, _ = pg.neighbour(r, mu, step)
+                assert ry == rn, (x, mu, step)
+                exp = list(xl)
+                exp[mu] = (xl[mu] + step) % pg.local_ext[mu]
+                exp[1] = (exp[1] + shift1) % pg.local_ext[1]
+                assert yl == tuple(exp), (x, mu, step)
 
 
-def emulate(dims, world, make_operator, psi):
-    """All ranks in one process: scatter, copy ghosts by hand, apply, gather."""
-    slabs = [D.TimeSlabs(dims, world, r) for r in range(world)]
-    loc = [ts.scatter(psi) for ts in slabs]
-    for r, ts in enumerate(slabs):       # what exchange_time_ghosts does with messages
-        loc[r][0] = loc[ts.prev][ts.T_loc]
-        loc[r][ts.T_loc + 1] = loc[ts.next][1]
-    outs = [ts.interior(np.asarray(make_operator(ts)(loc[r])).reshape(loc[r].shape)) for r, ts in enumerate(slabs)]
-    return np.concatenate(outs, axis=0)
-
-
-def test_time_slabs_geometry():
-    ts = D.TimeSlabs((8, 4, 4, 4), 2, 1)
-    assert ts.T_loc == 4 and ts.local_dims == (6, 4, 4, 4) and ts.time_index() == [3, 4, 5, 6, 7, 0]
-    assert (ts.prev, ts.next) == (0, 0)
+def test_process_grid_rejects_bad_splits():
     with pytest.raises(ValueError):
-        D.TimeSlabs((6, 4, 4, 4), 2, 0)      # 3 slices per rank: odd
-    U = synth.su3_links((8, 2, 2, 2), 0.3, 1)
-    Ul, _ = ts.local_fields(U, None, antiperiodic=True)
-    assert np.array_equal(Ul[4, ..., 0, :, :], -U[7, ..., 0, :, :]) and np.array_equal(Ul[4, ..., 1, :, :], U[7, ..., 1, :, :])
-    assert np.array_equal(Ul[0], U[3]) and np.array_equal(Ul[5], U[0])
+        D.ProcessGrid((6, 4, 4, 4), (2, 1, 1, 1))          # 3 slices per rank
+    with pytest.raises(ValueError):
+        D.ProcessGrid((4, 6, 4, 4), (1, 3, 1, 1), 3)       # odd number of ranks along the doubled direction
+    pg = D.ProcessGrid((16, 4, 4, 8), (2, 1, 1, 2), 3)
+    assert pg.world == 4 and pg.coords(3) == (1, 0, 0, 1) and pg.rank((1, 0, 0, 1)) == 3
+    lat = D.LocalLattice(pg, 3)
+    assert lat.local_dims == (16, 4, 4, 8) and lat.cstar_local == 2 and lat.bc_local == 2 and lat.origin == (8, 0, 0, 4)
+    with pytest.raises(ValueError):
+        D.LocalLattice(D.ProcessGrid((8, 4, 4, 4), (2, 1, 1, 1)), 0)   # T_loc = 4 < two boundary slabs
 
 
-@pytest.mark.parametrize("dims,cstar,ap,qed,world", [((8, 4, 4, 4), 0, 1, False, 2), ((8, 2, 4, 4), 3, 1, True, 2),
-                                                     ((8, 4, 2, 4), 2, 0, True, 4), ((4, 4, 4, 4), 0, 1, True, 1)])
-def test_emulated_ranks_reproduce_the_global_operator(dims, cstar, ap, qed, world):
-    X = (dims[0], 2 * dims[1] if cstar else dims[1], dims[2], dims[3])
-    psi = synth.gaussian_spinor(X, 3)
-    U, A, exp = global_reference(dims, cstar, ap, qed, psi)
-    got = emulate(dims, world, lambda ts: oracle_local_operator(ts, U, A, cstar, ap, qed), psi)
-    assert np.linalg.norm((got - exp).ravel()) / np.linalg.norm(exp.ravel()) < 1e-14
+# ---- the oracle as the rank-local operator ----------------------------------------------------------------------------------
+class OracleRank:
+    """ops object of domain.py on numpy arrays [local_ext + (4, 3)]; the halo protocol restated with explicit gamma matrices."""
+
+    def __init__(self, lat, U, A, qed):
+        self.lat = lat
+        Ul, Al = lat.local_fields(U, A)
+        self.ref = R.Ref(*lat.local_dims, lat.bc_local)
+        self.ref.gauge_load(Ul, Al, 1.0)
+        self.ref.set_quark(KAPPA, Q if qed else 0.0)
+        self.ref.clover_build(CSW, CSWQ if qed else 0.0)
+
+    def face_gather(self, v, pmask, mu, coord, sign):
+        import torch
+        layer = np.take(v, coord, axis=mu)                                     # [3 other coords][4][3]
+        P = np.eye(4) - sign * LN.GAMMA[mu]
+        return torch.from_numpy(np.ascontiguousarray(np.einsum("ab,...bc->...ac", P, layer)[..., :2, :]))
+
+    def face_scatter(self, v, pmask, mu, coord, shift1, buf):
+        h = buf.numpy()
+        if shift1:
+            h = np.roll(h, -shift1, axis=0 if mu == 0 else 1)      # ghost(x1) = face(x1 + shift1): direction 1 is axis 1 unless mu = 0
+        ghost = np.zeros(h.shape[:-2] + (4, 3), dtype=complex)
+        ghost[..., :2, :] = h
+        idx = [slice(None)] * 4
+        idx[mu] = coord
+        v[tuple(idx)] = ghost
+
+    def halo_zero(self, v, pmask, mu, lo, hi):
+        idx = [slice(None)] * 4
+        idx[mu] = slice(lo, hi)
+        v[tuple(idx)] = 0
+
+    def apply_owned(self, vin, vout):
+        out = self.ref.apply_Dw(vin).reshape(vin.shape)
+        vout[...] = 0
+        sl = self.lat.owned_slices()
+        vout[sl] = out[sl]
+
+
+class OracleOperator:
+    """The distributed D_w with the oracle on every rank, in the interface domain.cgne expects (numpy arrays, torch scalars)."""
+    G5 = np.array([1, 1, -1, -1])[:, None]
+
+    def __init__(self, comm, lats, ops):
+        self.comm, self.lats, self.ops, self.ranks = comm, lats, ops, comm.my_ranks
+
+    def alloc(self):
+        return {r: np.zeros(self.lats[r].local_ext + (4, 3), dtype=complex) for r in self.ranks}
+
+    def apply(self, vin, vout, dagger=False):
+        src = {r: (self.G5 * vin[r] if dagger else vin[r].copy()) for r in self.ranks}
+        D.halo_exchange(self.comm, self.lats, self.ops, src)
+        for r in self.ranks:
+            self.ops[r].apply_owned(src[r], vout[r])
+            if dagger:
+                vout[r] *= self.G5
+
+    def scalar(self):
+        import torch
+        return {r: torch.zeros(1, dtype=torch.float64) for r in self.ranks}
+
+    def norm2(self, v, out):
+        for r in self.ranks:
+            out[r][0] = float(np.vdot(v[r], v[r]).real)
+        self.comm.allreduce_sum(out)
+
+    def cg_xr(self, num, den, p, t, x, rvec, rr):
+        for r in self.ranks:
+            al = float(num[r]) / float(den[r])
+            x[r] += al * p[r]
+            rvec[r] -= al * t[r]
+            rr[r][0] = float(np.vdot(rvec[r], rvec[r]).real)
+        self.comm.allreduce_sum(rr)
+
+    def cg_p(self, num, den, s, p):
+        for r in self.ranks:
+            p[r][...] = s[r] + (float(num[r]) / float(den[r])) * p[r]
+
+    def copy(self, x, y):
+        for r in self.ranks:
+            y[r][...] = x[r]
+
+    def value(self, s):
+        return float(s[self.ranks[0]])
+
+
+GRIDS = [
+    # dims (physical), grid, cstar, antiperiodic, qed
+    ((16, 4, 4, 4), (2, 1, 1, 1), 0, 1, False),
+    ((16, 2, 4, 4), (2, 1, 1, 1), 3, 1, True),
+    ((4, 2, 4, 8), (1, 1, 1, 2), 3, 1, True),       # the cut crosses a C* direction: ghosts arrive displaced by L1
+    ((4, 2, 4, 8), (1, 1, 1, 2), 2, 0, True),       # direction 3 periodic
+    ((16, 2, 2, 8), (2, 1, 1, 2), 3, 1, True),
+]
+
+
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed", GRIDS)
+def test_distributed_Dw_and_solve_oracle_ranks(dims, grid, cstar, ap, qed):
+    U, A = fields(dims, qed)
+    ref = global_oracle(dims, cstar, ap, qed, U, A)
+    psi = synth.gaussian_spinor(ref.dims_ext, 3)
+    pg = D.ProcessGrid(dims, grid, cstar)
+    comm = D.LocalComm(pg.world)
+    lats = {r: D.LocalLattice(pg, r, antiperiodic=bool(ap)) for r in range(pg.world)}
+    ops = {r: OracleRank(lats[r], U, A, qed) for r in range(pg.world)}
+    op = OracleOperator(comm, lats, ops)
+    vin = {r: lats[r].scatter(psi) for r in range(pg.world)}
+    vout = op.alloc()
+    op.apply(vin, vout)
+    got = np.zeros_like(psi)
+    for r in range(pg.world):
+        lats[r].gather_into(got, vout[r])
+    exp = ref.apply_Dw(psi)
+    assert np.linalg.norm(got - exp) / np.linalg.norm(exp) < 1e-14
+    if grid != (2, 1, 1, 2):
+        return
+    # distributed CG on the normal equations of D_w: the solution is unique, compare through the global oracle's residual
+    tol = 1e-9
+    x, info = D.cgne(op, vin, tol**2 * float(np.vdot(psi, psi).real))
+    sol = np.zeros_like(psi)
+    for r in range(pg.world):
+        lats[r].gather_into(sol, x[r])
+    assert info["status"] == 0
+    assert np.linalg.norm(psi - ref.apply_Dw(sol)) / np.linalg.norm(psi) <= 1.05 * tol
 
 
 def _free_port():
@@ -77,67 +209,54 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, dims, cstar, ap, qed, out):
+def _gloo_worker(rank, world, port, dims, grid, cstar, ap, qed, q):
     import torch.distributed as dist
-    os.environ["MASTER_ADDR"] = "127.0.0.1"
-    os.environ["MASTER_PORT"] = str(port)
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        X = (dims[0], 2 * dims[1] if cstar else dims[1], dims[2], dims[3])
-        psi = synth.gaussian_spinor(X, 3)
-        U = synth.su3_links(dims, 0.3, 1)
-        A = synth.u1_field(dims, 0.3, 2) if qed else None
-        ts = D.TimeSlabs(dims, world, rank)
-        op = oracle_local_operator(ts, U, A, cstar, ap, qed)
-        local = np.ascontiguousarray(ts.scatter(psi))
-        res = D.apply_Dw_distributed(ts, local, op, dist)
-        out.put((rank, np.array(res)))
+        U, A = fields(dims, qed)
+        pg = D.ProcessGrid(dims, grid, cstar)
+        comm = D.TorchComm(dist)
+        lats = {rank: D.LocalLattice(pg, rank, antiperiodic=bool(ap))}
+        ops = {rank: OracleRank(lats[rank], U, A, qed)}
+        op = OracleOperator(comm, lats, ops)
+        psi = synth.gaussian_spinor(pg.ext, 3)
+        vin = {rank: lats[rank].scatter(psi)}
+        vout = op.alloc()
+        op.apply(vin, vout)
+        tol = 1e-9
+        x, info = D.cgne(op, vin, tol**2 * float(np.vdot(psi, psi).real))
+        q.put((rank, vout[rank], x[rank], info))
     finally:
         dist.destroy_process_group()
 
 
-def test_world2_gloo_distributed_apply():
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed", [((16, 2, 4, 4), (2, 1, 1, 1), 3, 1, True), ((4, 2, 4, 8), (1, 1, 1, 2), 3, 1, True)])
+def test_world_size_2_gloo_Dw_and_solve(dims, grid, cstar, ap, qed):
+    """One rank per process, torch.distributed `gloo`, world_size 2: batched point-to-point halo exchange matched by issue
+    order (both time neighbours of a rank are the SAME peer here), all-reduced CG scalars; D_w and the solve against the
+    oracle on the global lattice."""
     import torch.multiprocessing as mp
-    dims, cstar, ap, qed, world = (8, 2, 4, 4), 3, 1, True, 2
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, world, port, dims, cstar, ap, qed, q)) for r in range(world)]
+    procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, dims, grid, cstar, ap, qed, q)) for r in range(2)]
     for p in procs:
         p.start()
-    res = dict(q.get(timeout=180) for _ in range(world))
+    res = [q.get(timeout=300) for _ in range(2)]
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    X = (dims[0], 2 * dims[1], dims[2], dims[3])
-    psi = synth.gaussian_spinor(X, 3)
-    _, _, exp = global_reference(dims, cstar, ap, qed, psi)
-    got = np.concatenate([res[0], res[1]], axis=0)
-    assert np.linalg.norm((got - exp).ravel()) / np.linalg.norm(exp.ravel()) < 1e-14
-
-
-@pytest.mark.gpu
-@pytest.mark.parametrize("dims,cstar,ap,qed,world", [((16, 4, 4, 4), 0, 1, False, 2), ((16, 2, 4, 4), 3, 1, True, 4)])
-@pytest.mark.parametrize("prec", [0, 1])
-def test_cuda_contexts_as_rank_local_operators(dims, cstar, ap, qed, world, prec):
-    from paper_2502_02490_b200 import binding as B
-    X = (dims[0], 2 * dims[1] if cstar else dims[1], dims[2], dims[3])
-    psi = synth.gaussian_spinor(X, 3)
-    U, A, exp = global_reference(dims, cstar, ap, qed, psi)
-    ctxs = []
-
-    def make(ts):
-        Ul, Al = ts.local_fields(U, A, antiperiodic=bool(ap))
-        g = B.Qxd(*ts.local_dims, D.TimeSlabs.local_bc(cstar), precisions=(B.QXD_F64, B.QXD_F32), pairing=cstar > 0)
-        g.gauge_load(Ul, Al, 1.0)
-        g.set_quark(KAPPA, Q if qed else 0.0)
-        g.set_gauge_reconstruct(B.QXD_RECON_12)     # det W carries the boundary sign of the time links
-        g.clover_build(CSW, CSWQ if qed else 0.0)
-        ctxs.append(g)
-        return lambda loc: g.apply_Dw(loc, prec).cpu().numpy()
-
-    got = emulate(dims, world, make, psi)
-    err = np.linalg.norm((got - exp).ravel()) / np.linalg.norm(exp.ravel())
-    assert err < (1e-13 if prec == 0 else 1e-6), err
-    for g in ctxs:
-        g.close()
+    U, A = fields(dims, qed)
+    ref = global_oracle(dims, cstar, ap, qed, U, A)
+    psi = synth.gaussian_spinor(ref.dims_ext, 3)
+    pg = D.ProcessGrid(dims, grid, cstar)
+    got, sol = np.zeros_like(psi), np.zeros_like(psi)
+    for rank, vout, x, info in res:
+        lat = D.LocalLattice(pg, rank, antiperiodic=bool(ap))
+        lat.gather_into(got, vout)
+        lat.gather_into(sol, x)
+        assert info["status"] == 0
+    exp = ref.apply_Dw(psi)
+    assert np.linalg.norm(got - exp) / np.linalg.norm(exp) < 1e-14
+    assert np.linalg.norm(psi - ref.apply_Dw(sol)) / np.linalg.norm(psi) <= 1.05e-9
