@@ -13,6 +13,8 @@ QXD_F64, QXD_F32, QXD_F16 = 0, 1, 2
 QXD_CGNE, QXD_BICGSTAB, QXD_GCR = 0, 1, 2
 QXD_RECON_NONE, QXD_RECON_12 = 18, 12
 QXD_FS_GAUGE, QXD_FS_HOPLINKS, QXD_FS_CLOVER, QXD_FS_HOPLINKS_STALE, QXD_FS_CLOVER_STALE, QXD_FS_LAZY = 1, 2, 4, 8, 16, 32
+QXD_DS_DW, QXD_DS_HOP_AINV, QXD_DS_A_XMHOP, QXD_DS_X_MHOP, QXD_DS_AINV_X_MHOP = 0, 1, 2, 3, 4
+QXD_DSF_G5IN, QXD_DSF_G5HOP = 1, 2
 QXD_OK, QXD_EINVAL, QXD_ESTATE, QXD_EWORKSPACE, QXD_ECUDA, QXD_ENOCONV = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

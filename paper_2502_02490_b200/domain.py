@@ -236,15 +236,18 @@ class TorchComm:
                 self.dist.all_reduce(v)
 
 
-def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 0)):
+def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 0), g5in=False):
     """Fill the ghost layers of the spinors vecs[r] (r over the ranks this process holds) in the given cut directions.
-    Gather kernels -> one batched exchange -> scatter kernels.  The tag of a message is (mu, side)."""
+    Gather kernels -> one batched exchange -> scatter kernels.  The tag of a message is (mu, side).  g5in: the operator pass
+    applies gamma5 to its input (D-hat^dagger): the ghosts must then hold the projection of gamma5 psi, and since the upper
+    components of (1 - s gamma_mu) gamma5 psi are those of (1 + s gamma_mu) psi, the faces are gathered with the opposite sign
+    (gamma5 leaves the expanded ghost spinor (h, 0) unchanged)."""
     sends, recv_like = [], {}
     for r in comm.my_ranks:
         for m in lats[r].messages():
             if m["mu"] not in directions:
                 continue
-            buf = ops[r].face_gather(vecs[r], parity_mask, m["mu"], m["coord"], m["sign"])
+            buf = ops[r].face_gather(vecs[r], parity_mask, m["mu"], m["coord"], -m["sign"] if g5in else m["sign"])
             sends.append((r, m["dst"], (m["mu"], m["side"]), buf))
     if isinstance(comm, LocalComm):
         arrived = comm.exchange(sends)
@@ -345,8 +348,9 @@ def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, ove
     needs them), then the time faces -- in flight while the interior slabs run when there is one rank per process."""
     ranks = comm.my_ranks
     pm = 3 if mode == 0 else (1 << (1 - parity_out))
+    g5in = bool(flags & 1)        # QXD_DSF_G5IN
     if any(lats[r].cut[3] for r in ranks):
-        halo_exchange(comm, lats, ops, vin, pm, directions=(3,))
+        halo_exchange(comm, lats, ops, vin, pm, directions=(3,), g5in=g5in)
     time_cut = any(lats[r].cut[0] for r in ranks)
     ph = {r: (phi[r] if phi is not None else None) for r in ranks}
     if time_cut and overlap and isinstance(comm, TorchComm) and vin[ranks[0]].is_cuda:
@@ -355,7 +359,7 @@ def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, ove
         main = torch.cuda.current_stream()
         if not hasattr(comm, "side"):
             comm.side = torch.cuda.Stream()
-        sends = [(r, m["dst"], (m["mu"], m["side"]), ops[r].face_gather(vin[r], pm, m["mu"], m["coord"], m["sign"]))
+        sends = [(r, m["dst"], (m["mu"], m["side"]), ops[r].face_gather(vin[r], pm, m["mu"], m["coord"], -m["sign"] if g5in else m["sign"]))
                  for m in lats[r].messages() if m["mu"] == 0]
         rl = [(lats[r].pg.neighbour(r, 0, -1 if m["side"] == "up" else +1)[0], (0, m["side"]), t)
               for m, (_, _, _, t) in zip([m for m in lats[r].messages() if m["mu"] == 0], sends)]
@@ -374,7 +378,7 @@ def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, ove
         ops[r].dslash("boundary", mode, vin[r], vout[r], parity_out, flags, ph[r])
     else:
         if time_cut:
-            halo_exchange(comm, lats, ops, vin, pm, directions=(0,))
+            halo_exchange(comm, lats, ops, vin, pm, directions=(0,), g5in=g5in)
         for r in ranks:
             ops[r].dslash("all", mode, vin[r], vout[r], parity_out, flags, ph[r])
     halo_clear(lats, ops, vin, ranks, pm)

@@ -260,3 +260,129 @@ def test_world_size_2_gloo_Dw_and_solve(dims, grid, cstar, ap, qed):
     exp = ref.apply_Dw(psi)
     assert np.linalg.norm(got - exp) / np.linalg.norm(exp) < 1e-14
     assert np.linalg.norm(psi - ref.apply_Dw(sol)) / np.linalg.norm(psi) <= 1.05e-9
+
+
+# ---- GPU: the CUDA contexts as ranks, device-side halos ---------------------------------------------------------------------
+GPU_GRIDS = [
+    # dims (physical), grid, cstar, antiperiodic, qed, pairing
+    ((16, 4, 4, 4), (2, 1, 1, 1), 0, 1, False, None),
+    ((16, 4, 4, 4), (2, 1, 1, 1), 3, 1, True, True),
+    ((16, 4, 4, 4), (2, 1, 1, 1), 3, 1, True, False),
+    ((12, 4, 4, 8), (1, 1, 1, 2), 3, 1, True, True),     # cut across a C* direction, paired layout
+    ((12, 4, 4, 8), (1, 1, 1, 2), 3, 0, True, False),
+    ((12, 4, 4, 8), (1, 1, 1, 2), 2, 1, True, True),
+    ((16, 4, 4, 8), (2, 1, 1, 2), 3, 1, True, True),     # four ranks, both cuts
+    ((32, 4, 4, 4), (4, 1, 1, 1), 1, 1, True, None),
+]
+
+
+def _gpu_ranks(dims, grid, cstar, ap, qed, pairing, prec):
+    U, A = fields(dims, qed)
+    pg = D.ProcessGrid(dims, grid, cstar)
+    lats = {r: D.LocalLattice(pg, r, antiperiodic=bool(ap)) for r in range(pg.world)}
+    ops = {r: D.GpuRank(lats[r], U, A, 1.0, KAPPA, Q if qed else 0.0, CSW, CSWQ if qed else 0.0, prec=prec, pairing=pairing) for r in range(pg.world)}
+    return U, A, pg, lats, ops
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", GPU_GRIDS)
+@pytest.mark.parametrize("prec", [0, 1, 2])
+def test_gpu_distributed_Dw(dims, grid, cstar, ap, qed, pairing, prec):
+    """All ranks of the decomposition on one GPU, one after the other (LocalComm: their kernels never wait on one another):
+    gather kernels -> face buffers -> scatter kernels, interior and boundary slabs; against the oracle on the global lattice."""
+    U, A, pg, lats, ops = _gpu_ranks(dims, grid, cstar, ap, qed, pairing, prec)
+    ref = global_oracle(dims, cstar, ap, qed, U, A)
+    psi = synth.gaussian_spinor(ref.dims_ext, 3)
+    op = D.GpuOperator(D.LocalComm(pg.world), lats, ops)
+    vin = {r: ops[r].pack(lats[r].scatter(psi)) for r in range(pg.world)}
+    vout = op.alloc()
+    op.apply_Dw(vin, vout)
+    got = np.zeros_like(psi)
+    for r in range(pg.world):
+        loc = ops[r].unpack(vout[r])
+        # nothing but the owned sites is written or left behind
+        mask = np.ones(loc.shape[:4], dtype=bool)
+        mask[lats[r].owned_slices()] = False
+        assert np.all(loc[mask] == 0)
+        lats[r].gather_into(got, loc)
+    exp = ref.apply_Dw(psi)
+    assert np.linalg.norm(got - exp) / np.linalg.norm(exp) < {0: 1e-13, 1: 1e-6, 2: 2e-3}[prec]
+    for r in range(pg.world):
+        ops[r].close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[3], GPU_GRIDS[6]])
+def test_gpu_distributed_solve(dims, grid, cstar, ap, qed, pairing):
+    """Distributed even-odd CGNE (fp64): source preparation, D-hat with two halo exchanges per application, all-reduced
+    scalars, reconstruction; the global solution must satisfy ||eta - D_ref psi|| / ||eta|| <= tol with the oracle's D_w."""
+    U, A, pg, lats, ops = _gpu_ranks(dims, grid, cstar, ap, qed, pairing, 0)
+    ref = global_oracle(dims, cstar, ap, qed, U, A)
+    eta = synth.gaussian_spinor(ref.dims_ext, 5)
+    op = D.GpuOperator(D.LocalComm(pg.world), lats, ops)
+    src = {r: ops[r].pack(lats[r].scatter(eta)) for r in range(pg.world)}
+    x, info = D.solve_distributed(op, src, 1e-10)
+    assert info["status"] == 0, info
+    sol = np.zeros_like(eta)
+    for r in range(pg.world):
+        lats[r].gather_into(sol, ops[r].unpack(x[r]))
+    res = np.linalg.norm(eta - ref.apply_Dw(sol)) / np.linalg.norm(eta)
+    assert res <= 1.05e-10, (res, info)
+    # same iteration count as the single-GPU solver on the global lattice (same algorithm, same arithmetic up to summation order)
+    from paper_2502_02490_b200 import binding as B
+    g = B.Qxd(*dims, cstar | (ap << 2), precisions=(0,))
+    g.gauge_load(U, A, 1.0); g.set_quark(KAPPA, Q if qed else 0.0); g.clover_build(CSW, CSWQ if qed else 0.0)
+    _, i1 = g.solve(eta, 1e-10, algo=0, sloppy=0)
+    assert abs(i1["iters"] - info["iters"]) <= 2, (i1, info)
+    g.close()
+    for r in range(pg.world):
+        ops[r].close()
+
+
+def _nccl_self_worker(port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        dims, cstar, ap, qed = (16, 4, 4, 8), 3, 1, True
+        U, A = fields(dims, qed)
+        pg = D.ProcessGrid(dims, (1, 1, 1, 1), cstar)
+        lat = D.LocalLattice(pg, 0, antiperiodic=True, force_cut=(True, False, False, True))   # ghosts although there is one rank
+        ops = {0: D.GpuRank(lat, U, A, 1.0, KAPPA, Q, CSW, CSWQ, prec=1)}
+        comm = D.TorchComm(dist, self_via_dist=True)        # the faces really go through ncclSend / ncclRecv (to this rank itself)
+        op = D.GpuOperator(comm, {0: lat}, ops, overlap=True)
+        psi = synth.gaussian_spinor(pg.ext, 3)
+        vin = {0: ops[0].pack(lat.scatter(psi))}
+        vout = op.alloc()
+        op.apply_Dw(vin, vout)
+        torch.cuda.synchronize()
+        got = np.zeros_like(psi)
+        lat.gather_into(got, ops[0].unpack(vout[0]))
+        t = torch.ones(1, device="cuda")
+        dist.all_reduce(t)
+        q.put(got)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.timeout(300)
+def test_gpu_nccl_halo_exchange_with_overlap_single_rank():
+    """The NCCL path on the one GPU a test box has: a single rank with ghost layers in time AND direction 3 (C*) whose faces
+    travel through a batched ncclSend / ncclRecv to itself on a side stream while the interior time slabs run; the result must
+    be the global operator (the lattice is periodic through its own ghosts)."""
+    import torch.multiprocessing as mp
+    dims, cstar, ap, qed = (16, 4, 4, 8), 3, 1, True
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    p = ctx.Process(target=_nccl_self_worker, args=(_free_port(), q))
+    p.start()
+    got = q.get(timeout=240)
+    p.join(timeout=60)
+    assert p.exitcode == 0
+    U, A = fields(dims, qed)
+    ref = global_oracle(dims, cstar, ap, qed, U, A)
+    exp = ref.apply_Dw(synth.gaussian_spinor(ref.dims_ext, 3))
+    assert np.linalg.norm(got - exp) / np.linalg.norm(exp) < 1e-6
