@@ -598,6 +598,96 @@ def run_cuda(args, cfg):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------------------
+# --decomp domain: the lattice cut into time slabs over the ranks (row f2), strong scaling
+# ---------------------------------------------------------------------------------------------------------
+def run_domain(args, cfg):
+    """One rank per GPU, the GLOBAL lattice of the config cut along time (paper_2502_02490_b200/domain.py): device-side
+    projected halos, faces exchanged by NCCL while the interior slabs run, all-reduced solver scalars.  With one rank the
+    ghost layers are kept and filled through a real NCCL send/recv to the rank itself, so that the N = 1 line measures the
+    cost of the halo path against the plain single-GPU apply.  value = global sites x 768 B / max-over-ranks time."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import synth as synth_mod
+    from paper_2502_02490_b200 import binding as B, domain as D, sharding
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the qxd hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world == 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29533")
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=dev)
+    pg = D.ProcessGrid(cfg["dims"], (world, 1, 1, 1), cfg["cstar"])
+    lat = D.LocalLattice(pg, rank, antiperiodic=bool(cfg["antiperiodic"]), force_cut=(True, False, False, False))
+    U = synth_mod.su3_links(cfg["dims"], cfg["eps"], 1)
+    A = synth_mod.u1_field(cfg["dims"], 0.3, 2) if cfg["qed"] else None
+    comm = D.TorchComm(dist, self_via_dist=True)
+    hp = B.QXD_F32
+    ops = {rank: D.GpuRank(lat, U, A, cfg["qel"], cfg["kappa"], cfg["q"], cfg["csw"], cfg["csw_qed"], prec=hp, device=f"cuda:{local}")}
+    op = D.GpuOperator(comm, {rank: lat}, ops, overlap=not args.no_overlap)
+    eta = synth_mod.gaussian_spinor(cfg["dims_ext"], 3)
+    vin = {rank: ops[rank].pack(lat.scatter(eta))}
+    vout = op.alloc()
+    V = int(np.prod(cfg["dims_ext"]))
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize(dev)
+    for _ in range(args.warmup):
+        op.apply_Dw(vin, vout)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = ops[rank].g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        op.apply_Dw(vin, vout)
+    e1.record()
+    e1.synchronize()
+    barrier()
+    launches = ops[rank].g.launch_count() - l0
+    ms_step = sharding.max_over_ranks(e0.elapsed_time(e1) / args.steps, dist, dev)
+    clocks = sampler.stop()
+    value = V * dw_bytes_per_site(hp) / (ms_step * 1e-3) / 1e9
+    peak, peak_src = measured_peak()
+    # distributed fp64 solve (even-odd CGNE, every scalar all-reduced)
+    solve = None
+    if not args.no_solve:
+        ops64 = {rank: D.GpuRank(lat, U, A, cfg["qel"], cfg["kappa"], cfg["q"], cfg["csw"], cfg["csw_qed"], prec=B.QXD_F64, device=f"cuda:{local}")}
+        op64 = D.GpuOperator(comm, {rank: lat}, ops64, overlap=not args.no_overlap)
+        src = {rank: ops64[rank].pack(lat.scatter(eta))}
+        barrier()
+        t0 = time.perf_counter()
+        x, info = D.solve_distributed(op64, src, cfg["tol"], maxiter=args.maxiter)
+        barrier()
+        solve = {"algo": "distributed even-odd CGNE, fp64", "seconds": sharding.max_over_ranks(time.perf_counter() - t0, dist, dev), "iters": info["iters"],
+                 "status": info["status"], "true_res": info["true_res_eo"], "tol": cfg["tol"]}
+        ops64[rank].close()
+    if rank == 0:
+        face = lat.local_ext[1] * lat.local_ext[2] * lat.local_ext[3]
+        line = {"metric": "Dw_apply_fp32_GBps", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": dict(config_object(cfg, V // world), parallelism=f"time-slab domain decomposition over {world} rank(s), "
+                               f"local lattice {lat.local_dims[0]} slices incl. 2 x {D.TIME_GHOST} ghost slices",
+                               sharding="lattice cut along time; halo = 2 faces x 12 reals per face site per apply, NCCL, overlapped with the interior slabs"),
+                "gflops": V * FLOP_PER_SITE / (ms_step * 1e-3) / 1e9,
+                "roofline": {"bound": "hbm", "achieved": value / world, "peak": peak, "unit": "GB/s", "frac": value / world / peak, "traffic": None,
+                             "peak_source": peak_src, "kernel": "dslash_k<float, DW_FULL> on interior + boundary time slabs",
+                             "algorithmic_bytes_per_launch": dw_bytes_per_site(hp) * V // world},
+                "e2e": {"value": None, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                        "note": "fields stay on the devices between applies; see the default (right-hand-side sharded) line for the host-pointer path"},
+                "halo_bytes_per_step_per_rank": 2 * face * 12 * 4, "gpu_launches": launches, "clocks": clocks, "solve": solve}
+        print(json.dumps(line), flush=True)
+    ops[rank].close()
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -610,6 +700,9 @@ def main():
     ap.add_argument("--gcr-nkv", type=int, default=16, help="Krylov vectors per GCR cycle (0 = skip the SAP-GCR solves)")
     ap.add_argument("--gcr-ncy", type=int, default=4, help="SAP cycles per preconditioner application")
     ap.add_argument("--gcr-nmr", type=int, default=5, help="minimal-residual steps per SAP block solve")
+    ap.add_argument("--decomp", default="rhs", choices=["rhs", "domain"], help="rhs: shard by right-hand side (weak scaling, the default); "
+                    "domain: cut the lattice along time over the ranks (strong scaling, row f2)")
+    ap.add_argument("--no-overlap", action="store_true", help="--decomp domain: exchange the faces before the interior slabs instead of during them")
     ap.add_argument("--no-pairing", action="store_true", help="keep the extended-lattice layout for the solves (C* configs)")
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -629,6 +722,8 @@ def main():
                     f"csw_qed={cfg['csw_qed']}, q={cfg['q']:.4f}")
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.decomp == "domain":
+        run_domain(args, cfg)
     else:
         run_cuda(args, cfg)
 
