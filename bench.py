@@ -290,6 +290,8 @@ def run_cuda(args, cfg):
     # ---- headline: K fp32 D_w applies, barrier + synchronize on both sides, max over ranks ---------------
     hp = B.QXD_F32
     pin, pout = packed[hp]
+    if args.dw_sweep:
+        g.set_dw_sweep(args.dw_sweep)     # experiment: the time-sweep kernel for the headline apply
     step = lambda: g.apply_Dw_packed(pin, pout, hp)
     for _ in range(args.warmup):
         step()
@@ -333,6 +335,7 @@ def run_cuda(args, cfg):
         sustained = {"applies": 100 * nblk, "seconds": evs[0].elapsed_time(evs[-1]) * 1e-3, "ms_per_step_median": ms_med,
                      "ms_per_step_min": per100[0], "ms_per_step_max": per100[-1], "value": gbs * world, "unit": "GB/s",
                      "frac": gbs / peak, "frac_of_nominal_8000": gbs / 8000.0, "clocks": ck}
+    g.set_dw_sweep(0)
     # the headline sampler ran through the --steps region and the sustained window of the same kernel (a 100 ms nvidia-smi
     # cadence cannot resolve a --steps region of a few ms by itself)
     clocks = sampler.stop()
@@ -700,6 +703,7 @@ def main():
     ap.add_argument("--gcr-nkv", type=int, default=16, help="Krylov vectors per GCR cycle (0 = skip the SAP-GCR solves)")
     ap.add_argument("--gcr-ncy", type=int, default=4, help="SAP cycles per preconditioner application")
     ap.add_argument("--gcr-nmr", type=int, default=5, help="minimal-residual steps per SAP block solve")
+    ap.add_argument("--dw-sweep", type=int, default=0, help="use the time-sweep D_w kernel with this segment length for the headline apply (0 = tile kernel)")
     ap.add_argument("--decomp", default="rhs", choices=["rhs", "domain"], help="rhs: shard by right-hand side (weak scaling, the default); "
                     "domain: cut the lattice along time over the ranks (strong scaling, row f2)")
     ap.add_argument("--no-overlap", action="store_true", help="--decomp domain: exchange the faces before the interior slabs instead of during them")

@@ -226,6 +226,12 @@ int qxd_spinor_pack(qxd_ctx* ctx, int prec, const double* nat /*DEVICE [V][4][3]
 int qxd_spinor_unpack(qxd_ctx* ctx, int prec, const void* packed, double* nat);
 int qxd_apply_Dw_packed(qxd_ctx* ctx, int prec, const void* in, void* out);
 int qxd_apply_Dhat_packed(qxd_ctx* ctx, int prec, const void* in_e, void* out_e, int dagger);
+/* Alternative kernel for qxd_apply_Dw_packed in fp32 (18-real links, extended-lattice layout, 4^4 tiles, extents multiples of
+ * (4, 8, 8, 4)): a CTA owns an 8 x 8 x 4 spatial footprint and sweeps tseg time slices, keeping the slices t-1, t, t+1 of its
+ * footprint in a shared-memory ring filled by cp.async two slices ahead, so that time neighbours and in-footprint spatial
+ * neighbours never go back to L2 / DRAM.  tseg = 0 (default): the tile kernel; tseg >= 2: the sweep kernel where
+ * it applies (silently the tile kernel elsewhere).  Same results up to the summation order of nothing: identical arithmetic. */
+int qxd_set_dw_sweep(qxd_ctx* ctx, int tseg);
 /* Multi-RHS D_w (row a10): in/out hold nrhs packed full-lattice spinors back to back, qxd_packed_spinor_bytes(prec,0)
  * apart.  One launch: the CTAs working on the same tile for different right-hand sides are consecutive, so the links
  * and clover blocks of a tile come from DRAM once and from L2 afterwards; every thread applies its site's links and

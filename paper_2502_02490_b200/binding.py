@@ -76,6 +76,7 @@ SYMBOLS = {
     "qxd_spinor_unpack": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dw_packed": (_i, [_vp, _i, _vp, _vp]),
     "qxd_apply_Dhat_packed": (_i, [_vp, _i, _vp, _vp, _i]),
+    "qxd_set_dw_sweep": (_i, [_vp, _i]),
     "qxd_openqxd_index": (_i, [_vp, C.POINTER(_i), _vp, _l, _vp]),
     "qxd_openqxd_reorder": (_i, [_vp, C.POINTER(_i), _i, _i, _vp, _vp]),
     "qxd_openqxd_gauge": (_i, [_vp, C.POINTER(_i), _i, _i, _vp, _vp]),
@@ -223,6 +224,9 @@ class Qxd:
         cnt = (C.c_long * 2)()
         self._chk(self.lib.qxd_field_status(self.h, C.byref(st), cnt))
         return st.value, cnt[0], cnt[1]
+
+    def set_dw_sweep(self, tseg):
+        self._chk(self.lib.qxd_set_dw_sweep(self.h, int(tseg)))
 
     def clover_stats(self):
         """(parity passes of the unpivoted block inversion, parity passes redone with the pivoted kernel)"""

@@ -380,7 +380,17 @@ int qxd_apply_Dw_packed(qxd_ctx* c, int prec, const void* in, void* out) {
   d.prec = prec; d.mode = DS_DW_FULL; d.flags = 0;
   d.in[0] = half_view(prec, const_cast<void*>(in), Vh, 0); d.in[1] = half_view(prec, const_cast<void*>(in), Vh, 1);
   d.out[0] = half_view(prec, out, Vh, 0); d.out[1] = half_view(prec, out, Vh, 1);
+  if (prec == 1 && c->dw_sweep_tseg > 0) {   // time-sweep kernel where it applies (fp32, 18-real links, extended layout, 4^4 tiles)
+    rc = launch_dw_sweep(c, d.in, d.out);
+    if (rc != QXD_EINVAL) return rc;
+  }
   return launch_dslash(c, d);
+}
+
+int qxd_set_dw_sweep(qxd_ctx* c, int tseg) {
+  if (!c || tseg < 0 || tseg == 1) return c ? fail(c, QXD_EINVAL, "set_dw_sweep: 0 (off) or a segment length >= 2") : QXD_EINVAL;
+  c->dw_sweep_tseg = tseg;
+  return QXD_OK;
 }
 
 int qxd_apply_Dw_multi_packed(qxd_ctx* c, int prec, int nrhs, const void* in, void* out) {

@@ -39,6 +39,7 @@ struct qxd_ctx {
   int prec_mask = 0, nrhs = 1;
   int link_reals[qxd::NPREC] = {18, 18, 18};     // per storage precision: stored reals per hopping link, 18 or 14 = rows 0,1 + det (qxd_set_gauge_reconstruct)
   int rhs_per_thread = 0;                        // multi-RHS dslash: right-hand sides per thread (0 = default)
+  int dw_sweep_tseg = 0;                         // > 0: the fp32 full-lattice D_w uses the time-sweep kernel with this segment length (qxd_set_dw_sweep)
   // state
   bool have_gauge = false, have_qed = false, have_quark = false, have_clover = false;
   // field-status manager (row f4): derived fields marked stale by a setter and regenerated at their first use
@@ -188,6 +189,8 @@ int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, cons
 // solver.cu
 int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
 int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+// dslash_sweep.cu
+int launch_dw_sweep(qxd_ctx* c, const SpinorPtr in[2], const SpinorPtr out[2]);
 // halo.cu (row f2)
 size_t face_bytes(const qxd_ctx* c, int prec, int mu);
 int launch_face_gather(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int coord, int sign, void* buf);

@@ -247,6 +247,26 @@ def test_blas(case, prec):
     assert relerr(got, ye + 0.37 * xe) < {F64: 1e-15, F32: 2e-7, F16: 1e-3}[prec]
 
 
+def test_dw_sweep_kernel_is_bit_identical():
+    """The time-sweep D_w kernel (qxd_set_dw_sweep; fp32, 18-real links, extended layout) does the arithmetic of the tile kernel
+    in the same order: bit-identical output for several segment lengths, with C* boundaries and a ragged last segment."""
+    import torch
+    for dims, cstar in (((16, 8, 8, 8), 0), ((12, 4, 8, 8), 3)):
+        c = Case(dims, cstar, 1, cstar > 0, precisions=(F64, F32), pairing=False)
+        psi = synth.gaussian_spinor(c.dims_ext, 3)
+        pin = c.gpu.spinor_pack(psi, F32)
+        ref = c.gpu.new_packed(F32)
+        c.gpu.apply_Dw_packed(pin, ref, F32)
+        for tseg in (2, 4, 8, 5):
+            c.gpu.set_dw_sweep(tseg)
+            out = c.gpu.new_packed(F32)
+            c.gpu.apply_Dw_packed(pin, out, F32)
+            assert torch.equal(out, ref), (dims, cstar, tseg)
+        c.gpu.set_dw_sweep(0)
+        assert relerr(to_np(c.gpu.spinor_unpack(ref, F32)).reshape(psi.shape), c.ref.apply_Dw(psi)) < TOL[F32]
+        c.close()
+
+
 def test_tiling_does_not_change_results():
     """Row a1: the tile shape only permutes sites in memory; results are identical for any legal tile."""
     dims = (4, 4, 4, 8)
