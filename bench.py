@@ -659,19 +659,27 @@ def run_domain(args, cfg):
     clocks = sampler.stop()
     value = V * dw_bytes_per_site(hp) / (ms_step * 1e-3) / 1e9
     peak, peak_src = measured_peak()
-    # distributed fp64 solve (even-odd CGNE, every scalar all-reduced)
+    # distributed solves: fp64 even-odd CGNE and the mixed fp64/fp32 one with reliable updates (every scalar all-reduced)
     solve = None
     if not args.no_solve:
-        ops64 = {rank: D.GpuRank(lat, U, A, cfg["qel"], cfg["kappa"], cfg["q"], cfg["csw"], cfg["csw_qed"], prec=B.QXD_F64, device=f"cuda:{local}")}
-        op64 = D.GpuOperator(comm, {rank: lat}, ops64, overlap=not args.no_overlap)
-        src = {rank: ops64[rank].pack(lat.scatter(eta))}
-        barrier()
-        t0 = time.perf_counter()
-        x, info = D.solve_distributed(op64, src, cfg["tol"], maxiter=args.maxiter)
-        barrier()
-        solve = {"algo": "distributed even-odd CGNE, fp64", "seconds": sharding.max_over_ranks(time.perf_counter() - t0, dist, dev), "iters": info["iters"],
-                 "status": info["status"], "true_res": info["true_res_eo"], "tol": cfg["tol"]}
-        ops64[rank].close()
+        hi = {rank: D.GpuRank(lat, U, A, cfg["qel"], cfg["kappa"], cfg["q"], cfg["csw"], cfg["csw_qed"], prec=B.QXD_F64, device=f"cuda:{local}",
+                              extra_precisions=(B.QXD_F32,))}
+        lo = {rank: hi[rank].with_prec(B.QXD_F32)}
+        op64 = D.GpuOperator(comm, {rank: lat}, hi, overlap=not args.no_overlap)
+        op32 = D.GpuOperator(comm, {rank: lat}, lo, overlap=not args.no_overlap)
+        src = {rank: hi[rank].pack(lat.scatter(eta))}
+        solve = {}
+        for name in ("cgne_fp64", "cgne_fp64_fp32"):
+            barrier()
+            t0 = time.perf_counter()
+            if name == "cgne_fp64":
+                x, info = D.solve_distributed(op64, src, cfg["tol"], maxiter=args.maxiter)
+            else:
+                x, info = D.solve_distributed_mixed(op64, op32, src, cfg["tol"], delta=0.1, maxiter=args.maxiter)
+            barrier()
+            solve[name] = {"algo": "distributed even-odd CGNE", "seconds": sharding.max_over_ranks(time.perf_counter() - t0, dist, dev), "iters": info["iters"],
+                           "status": info["status"], "true_res": info["true_res_eo"], "tol": cfg["tol"], "n_reliable": info.get("n_reliable")}
+        hi[rank].close()
     if rank == 0:
         face = lat.local_ext[1] * lat.local_ext[2] * lat.local_ext[3]
         line = {"metric": "Dw_apply_fp32_GBps", "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

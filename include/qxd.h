@@ -280,7 +280,8 @@ int qxd_openqxd_gauge(qxd_ctx* ctx, const int block[4], int reals_per_link, int 
  *   qxd_halo_zero      psi(x) = 0 on the layers lo <= x_mu < hi.
  *   qxd_blas_*_dev     BLAS-1 with device-resident scalars (a distributed solver all-reduces them with NCCL in place):
  *                      norm2_dev: *out = |x|^2;  cg_xr: alpha = *num / *den, x += alpha p, r -= alpha t, *rr = |r|^2;
- *                      cg_p: beta = *num / *den, p = s + beta p;  copy: y = x;  zero: x = 0.  Half-lattice packed vectors. */
+ *                      cg_p: beta = *num / *den, p = s + beta p;  copy: y = x;  zero: x = 0;  convert / acc_hi / sub_norm_dev: the steps of
+ *                      a reliable update (fp64 solution accumulation and true residual).  Half-lattice packed vectors. */
 enum { QXD_DS_DW = 0, QXD_DS_HOP_AINV = 1, QXD_DS_A_XMHOP = 2, QXD_DS_X_MHOP = 3, QXD_DS_AINV_X_MHOP = 4 };
 enum { QXD_DSF_G5IN = 1, QXD_DSF_G5HOP = 2 };
 int qxd_time_slabs(const qxd_ctx* ctx, int* nslabs, int* thickness);
@@ -295,6 +296,10 @@ int qxd_blas_cg_xr(qxd_ctx* ctx, int prec, const double* num, const double* den,
 int qxd_blas_cg_p(qxd_ctx* ctx, int prec, const double* num, const double* den, const void* s, void* p);
 int qxd_blas_copy(qxd_ctx* ctx, int prec, const void* x, void* y);
 int qxd_blas_zero(qxd_ctx* ctx, int prec, void* x);
+/* reliable-update building blocks: y (prec_to) = x (prec_from);  x_hi (fp64) += x_lo (prec), x_lo = 0;  r = b - t, *rr = |r|^2 */
+int qxd_blas_convert(qxd_ctx* ctx, int prec_from, const void* x, int prec_to, void* y);
+int qxd_blas_acc_hi(qxd_ctx* ctx, int prec, void* x_lo, void* x_hi);
+int qxd_blas_sub_norm_dev(qxd_ctx* ctx, int prec, const void* b, const void* t, void* r, double* rr /*DEVICE*/);
 
 /* ---- BLAS-1 on packed half-lattice spinors (row a6) ---------------------------------------------
  * y <- a*x + y ;  returns <x,y> = sum conj(x) y  and  |x|^2 (fp64 accumulation, HOST results). */

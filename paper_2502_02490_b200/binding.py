@@ -92,6 +92,9 @@ SYMBOLS = {
     "qxd_blas_cg_p": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
     "qxd_blas_copy": (_i, [_vp, _i, _vp, _vp]),
     "qxd_blas_zero": (_i, [_vp, _i, _vp]),
+    "qxd_blas_convert": (_i, [_vp, _i, _vp, _i, _vp]),
+    "qxd_blas_acc_hi": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_blas_sub_norm_dev": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
     "qxd_blas_axpy": (_i, [_vp, _i, _d, _vp, _vp]),
     "qxd_blas_cdot": (_i, [_vp, _i, _vp, _vp, _vp]),
     "qxd_blas_norm2": (_i, [_vp, _i, _vp, _vp]),
@@ -394,6 +397,15 @@ class Qxd:
 
     def blas_zero(self, x, prec):
         self._chk(self.lib.qxd_blas_zero(self.h, prec, _ptr(x)))
+
+    def blas_convert(self, x, prec_from, y, prec_to):
+        self._chk(self.lib.qxd_blas_convert(self.h, prec_from, _ptr(x), prec_to, _ptr(y)))
+
+    def blas_acc_hi(self, x_lo, prec, x_hi):
+        self._chk(self.lib.qxd_blas_acc_hi(self.h, prec, _ptr(x_lo), _ptr(x_hi)))
+
+    def blas_sub_norm_dev(self, b, t, r, prec, rr):
+        self._chk(self.lib.qxd_blas_sub_norm_dev(self.h, prec, _ptr(b), _ptr(t), _ptr(r), _ptr(rr)))
 
     # -- packed layout -------------------------------------------------------------------------------
     def packed_spinor_bytes(self, prec, half_only=False):

@@ -555,8 +555,8 @@ int qxd_dslash_packed(qxd_ctx* c, int prec, int mode, int flags, int parity_out,
     if (needs_phi) d.phi = half_view(prec, php, Vh, parity_out);
     d.out[parity_out] = half_view(prec, out, Vh, parity_out);
   }
-  for (int k = slab_lo; k < slab_hi; k++) {
-    d.tm = maps[k];
+  if (slab_hi > slab_lo) {   // ONE launch over all tiles; the CTAs whose time slab lies outside the range retire at once
+    d.t_lo = slab_lo * c->tile[0]; d.t_hi = slab_hi * c->tile[0];
     if ((rc = launch_dslash(c, d))) return rc;
   }
   return QXD_OK;
@@ -619,6 +619,18 @@ int qxd_blas_copy(qxd_ctx* c, int prec, const void* x, void* y) {
 int qxd_blas_zero(qxd_ctx* c, int prec, void* x) {
   if (!blas_args_ok(c, prec) || !x) return QXD_EINVAL;
   return blas_zero(c, prec, hp(c, prec, x));
+}
+int qxd_blas_convert(qxd_ctx* c, int prec_from, const void* x, int prec_to, void* y) {
+  if (!blas_args_ok(c, prec_from) || !blas_args_ok(c, prec_to) || !x || !y) return QXD_EINVAL;
+  return launch_convert_spinor(c, prec_from, hp(c, prec_from, x), prec_to, hp(c, prec_to, y));
+}
+int qxd_blas_acc_hi(qxd_ctx* c, int prec, void* x_lo, void* x_hi) {
+  if (!blas_args_ok(c, prec) || !x_lo || !x_hi) return QXD_EINVAL;
+  return blas_acc_hi(c, prec, hp(c, prec, x_lo), hp(c, 0, x_hi));
+}
+int qxd_blas_sub_norm_dev(qxd_ctx* c, int prec, const void* b, const void* t, void* r, double* rr) {
+  if (!blas_args_ok(c, prec) || !b || !t || !r || !rr) return QXD_EINVAL;
+  return blas_sub_norm(c, prec, hp(c, prec, b), hp(c, prec, t), hp(c, prec, r), rr);
 }
 
 int qxd_solve(qxd_ctx* c, const double* eta, double* psi, double tol, qxd_solve_info* info) {

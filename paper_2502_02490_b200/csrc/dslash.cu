@@ -55,6 +55,7 @@ int launch_dslash(qxd_ctx* c, const DslashCall& d) {
   a.nrhs = d.nrhs > 1 ? d.nrhs : 1; a.ngroups = 1;
   a.rs_in = d.rs_in; a.rs_phi = d.rs_phi; a.rs_out = d.rs_out;
   a.tm = d.tm;
+  a.t_lo = d.t_hi > 0 ? d.t_lo : 0; a.t_hi = d.t_hi > 0 ? d.t_hi : 0x7fffffff;
   if (a.nrhs > 64) return fail(c, QXD_EINVAL, "dslash: at most 64 right-hand sides per launch");
   a.R.partials = c->partials; a.R.result = d.norm_result; a.R.rstride = d.norm_stride;
   typedef int (*Dispatch)(qxd_ctx*, const DslashCall&, DslashArgs&);

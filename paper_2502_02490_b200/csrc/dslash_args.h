@@ -17,6 +17,7 @@ struct DslashArgs {
   size_t rs_in, rs_phi, rs_out;   // byte distance between consecutive right-hand sides
   Reducer R;
   TileMap tm;          // subset of tiles this launch works on (identity unless count > 0)
+  int t_lo, t_hi;      // only sites with t_lo <= x0 < t_hi are computed (time-slab ranges of the domain decomposition; default: all)
 };
 
 

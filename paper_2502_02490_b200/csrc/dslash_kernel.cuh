@@ -381,9 +381,13 @@ __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelSh
   for (int r = 0; r < R; r++)
 #pragma unroll
     for (int k = 0; k < NRED; k++) nrm[r][k] = 0.0;
-  if (cb < Vh) {
-    Site s;
+  Site s;
+  bool active = cb < Vh;
+  if (active) {
     site_init<PAIR ? 1 : 0>(a.g, cb, parity, s);
+    active = s.x[0] >= a.t_lo && s.x[0] < a.t_hi;   // time range of a slab-restricted launch (uniform over the CTA for whole slabs)
+  }
+  if (active) {
     C acc[R][24];
 #pragma unroll
     for (int r = 0; r < R; r++)

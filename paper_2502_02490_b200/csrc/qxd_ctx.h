@@ -148,6 +148,7 @@ struct DslashCall {
   size_t rs_in, rs_phi, rs_out;
   int norm_stride;
   TileMap tm;       // launch on a subset of the tiles (time slab); default: whole lattice
+  int t_lo, t_hi;   // t_hi > 0: compute only the sites with t_lo <= x0 < t_hi (CTAs outside the range retire at once)
 };
 int launch_dslash(qxd_ctx* c, const DslashCall& d);
 int launch_clover_apply(qxd_ctx* c, int prec, int inverse, int parity, const SpinorPtr& in, const SpinorPtr& out);

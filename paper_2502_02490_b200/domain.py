@@ -290,11 +290,11 @@ class GpuRank:
     """One rank's CUDA context on its local lattice (fields with ghost layers loaded once) and the per-rank steps of the
     distributed operator.  Vectors are packed FULL-lattice buffers of the storage precision `prec` (torch uint8 tensors)."""
 
-    def __init__(self, lat: LocalLattice, U, A, qel, kappa, q, csw, csw_qed, prec=0, device="cuda:0", pairing=None):
+    def __init__(self, lat: LocalLattice, U, A, qel, kappa, q, csw, csw_qed, prec=0, device="cuda:0", pairing=None, extra_precisions=()):
         from . import binding as B
         self.B, self.lat, self.prec = B, lat, prec
         Ul, Al = lat.local_fields(U, A)
-        self.g = B.Qxd(*lat.local_dims, lat.bc_local, precisions=tuple({B.QXD_F64, prec}), device=device, pairing=pairing)
+        self.g = B.Qxd(*lat.local_dims, lat.bc_local, precisions=tuple({B.QXD_F64, prec} | set(extra_precisions)), device=device, pairing=pairing)
         self.g.gauge_load(Ul, Al, qel)
         self.g.set_quark(kappa, q)
         self.g.clover_build(csw, csw_qed)
@@ -305,6 +305,14 @@ class GpuRank:
 
     def close(self):
         self.g.close()
+
+    def with_prec(self, prec):
+        """The same context seen through another bound storage precision (the sloppy operator of a mixed-precision solve)."""
+        import copy
+        o = copy.copy(self)
+        o.prec = prec
+        o.hb = self.g.packed_spinor_bytes(prec, half_only=True)
+        return o
 
     # vectors
     def alloc(self):
@@ -504,3 +512,83 @@ def solve_distributed(op: GpuOperator, eta, tol, maxiter=10000):
     op.reconstruct(eta, x)
     info["true_res_eo"] = (info["res2"] / tot) ** 0.5 if tot > 0 else 0.0
     return x, info
+
+
+def solve_distributed_mixed(op_hi: GpuOperator, op_lo: GpuOperator, eta, tol, delta=0.1, maxiter=10000):
+    """Mixed-precision distributed solve: the CG iteration on the normal equations of D-hat runs on the SLOPPY operator
+    op_lo (fp32 storage; same ranks and contexts as op_hi, see GpuRank.with_prec), the solution is accumulated and the true
+    residual recomputed with the fp64 operator op_hi whenever the iterated residual has dropped by `delta` since the last
+    update ("reliable updates", PAPER.md:207 ref [4]; the single-GPU loop of csrc/solver.cu with every scalar all-reduced and a
+    halo exchange inside every operator application).  Convergence is declared on the fp64 residual only."""
+    H, L = op_hi, op_lo
+    ranks = H.ranks
+    n2 = H.scalar()
+    tot = 0.0
+    for par in (0, 1):
+        for r in ranks:
+            o = H.ops[r]
+            o.g.blas_norm2_dev(o.half(eta[r], par), o.prec, n2[r])
+        H.comm.allreduce_sum(n2)
+        tot += H.value(n2)
+    stop2 = tol * tol * tot
+    b = H.alloc()
+    H.prepare(eta, b)
+    xhi, rhi, thi = H.alloc(), H.alloc(), H.alloc()
+    xlo, rlo, s, p, t = L.alloc(), L.alloc(), L.alloc(), L.alloc(), L.alloc()
+    gam, gam2, tt, rr, rrt = L.scalar(), L.scalar(), L.scalar(), L.scalar(), H.scalar()
+
+    def to_lo(src, dst):
+        for r in ranks:
+            oh, ol = H.ops[r], L.ops[r]
+            oh.g.blas_convert(oh.half(src[r]), oh.prec, ol.half(dst[r]), ol.prec)
+
+    def reliable():
+        for r in ranks:
+            oh, ol = H.ops[r], L.ops[r]
+            oh.g.blas_acc_hi(ol.half(xlo[r]), ol.prec, oh.half(xhi[r]))
+        H.apply(xhi, thi)
+        for r in ranks:
+            oh = H.ops[r]
+            oh.g.blas_sub_norm_dev(oh.half(b[r]), oh.half(thi[r]), oh.half(rhi[r]), oh.prec, rrt[r])
+        H.comm.allreduce_sum(rrt)
+        to_lo(rhi, rlo)
+        return H.value(rrt)
+
+    H.copy(b, rhi)
+    H.norm2(rhi, rrt)
+    rr_true = H.value(rrt)
+    to_lo(rhi, rlo)
+    it, nrel, maxr = 0, 0, rr_true ** 0.5
+    status = 0 if rr_true <= stop2 else -5
+    if status:
+        L.apply(rlo, s, dagger=True)
+        L.copy(s, p)
+        L.norm2(s, gam)
+    while status and it < maxiter:
+        L.apply(p, t)
+        L.norm2(t, tt)
+        L.cg_xr(gam, tt, p, t, xlo, rlo, rr)
+        it += 1
+        res2 = L.value(rr)
+        if not (res2 == res2):
+            break
+        rn = res2 ** 0.5
+        maxr = max(maxr, rn)
+        if rn < delta * maxr or res2 <= stop2:
+            rr_true = reliable()
+            nrel += 1
+            maxr = rr_true ** 0.5
+            if rr_true <= stop2:
+                status = 0
+                break
+        L.apply(rlo, s, dagger=True)
+        L.norm2(s, gam2)
+        L.cg_p(gam2, gam, s, p)
+        gam, gam2 = gam2, gam
+    if status:
+        rr_true = reliable()
+        nrel += 1
+        if rr_true <= stop2:
+            status = 0
+    H.reconstruct(eta, xhi)
+    return xhi, dict(iters=it, n_reliable=nrel, status=status, true_res_eo=(rr_true / tot) ** 0.5 if tot > 0 else 0.0)

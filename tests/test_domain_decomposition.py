@@ -339,6 +339,31 @@ def test_gpu_distributed_solve(dims, grid, cstar, ap, qed, pairing):
         ops[r].close()
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[6]])
+def test_gpu_distributed_mixed_precision_solve(dims, grid, cstar, ap, qed, pairing):
+    """fp32 sloppy operator with fp64 reliable updates on the decomposed lattice: reaches 1e-10 on the global oracle's residual."""
+    U, A = fields(dims, qed)
+    pg = D.ProcessGrid(dims, grid, cstar)
+    lats = {r: D.LocalLattice(pg, r, antiperiodic=bool(ap)) for r in range(pg.world)}
+    hi = {r: D.GpuRank(lats[r], U, A, 1.0, KAPPA, Q if qed else 0.0, CSW, CSWQ if qed else 0.0, prec=0, pairing=pairing, extra_precisions=(1,))
+          for r in range(pg.world)}
+    lo = {r: hi[r].with_prec(1) for r in range(pg.world)}
+    comm = D.LocalComm(pg.world)
+    ref = global_oracle(dims, cstar, ap, qed, U, A)
+    eta = synth.gaussian_spinor(ref.dims_ext, 5)
+    src = {r: hi[r].pack(lats[r].scatter(eta)) for r in range(pg.world)}
+    x, info = D.solve_distributed_mixed(D.GpuOperator(comm, lats, hi), D.GpuOperator(comm, lats, lo), src, 1e-10)
+    assert info["status"] == 0 and info["n_reliable"] >= 2, info
+    sol = np.zeros_like(eta)
+    for r in range(pg.world):
+        lats[r].gather_into(sol, hi[r].unpack(x[r]))
+    res = np.linalg.norm(eta - ref.apply_Dw(sol)) / np.linalg.norm(eta)
+    assert res <= 1.05e-10, (res, info)
+    for r in range(pg.world):
+        hi[r].close()
+
+
 def _nccl_self_worker(port, q):
     import torch
     import torch.distributed as dist
