@@ -206,6 +206,9 @@ int qxd_solve_host(qxd_ctx* ctx, const double* eta_host, double* psi_host, doubl
  * direction) are rejected with QXD_EINVAL by qxd_solve.
  * qxd_apply_sap: out = M_sap in on fp32 packed full-lattice spinors (test and bench entry point of the preconditioner). */
 int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
+/* Host-only introspection of the SAP block decomposition (no GPU needed; CPU tests of reading R21): block index (= cb >> 7) and
+ * colour (0 / 1) of the site (cb, parity).  QXD_EINVAL if the geometry admits no two-colouring (qxd_last_error says why). */
+int qxd_sap_block_of(qxd_ctx* ctx, int cb, int parity, int* block, int* colour);
 int qxd_apply_sap(qxd_ctx* ctx, int prec, const void* in /*DEVICE, packed fp32*/, void* out /*DEVICE, packed fp32*/);
 
 /* ---- batched solve (rows a7 + a10; "for many right-hand sides"; BASELINE config 4) -------------------

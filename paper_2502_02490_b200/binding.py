@@ -68,6 +68,7 @@ SYMBOLS = {
     "qxd_solve_host": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_set_gcr": (_i, [_vp, _i, _i, _i]),
     "qxd_apply_sap": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_sap_block_of": (_i, [_vp, _i, _i, C.POINTER(_i), C.POINTER(_i)]),
     "qxd_solve_multi": (_i, [_vp, _i, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_apply_Dw_multi_packed": (_i, [_vp, _i, _i, _vp, _vp]),
     "qxd_set_rhs_per_thread": (_i, [_vp, _i]),

@@ -651,6 +651,18 @@ int qxd_set_gcr(qxd_ctx* c, int nkv, int ncy, int nmr) {
   return QXD_OK;
 }
 
+int qxd_sap_block_of(qxd_ctx* c, int cb, int parity, int* block, int* colour) {
+  if (!c || !block || !colour || cb < 0 || cb >= c->g.Vh || parity < 0 || parity > 1) return QXD_EINVAL;
+  int rc = sap_check_geometry(c);
+  if (rc) return rc;
+  int x[4];
+  coords_int(c->g, c->g.pair ? (cb >> 1) : cb, parity, x);
+  int col = 0;
+  for (int mu = 0; mu < 4; mu++) if (c->sap_colmask[mu]) col += x[mu] >> c->sap_boxsh[mu];
+  *block = cb >> 7; *colour = col & 1;
+  return QXD_OK;
+}
+
 int qxd_apply_sap(qxd_ctx* c, int prec, const void* in, void* out) {
   int rc = check_apply(c, prec, in, out, "apply_sap");
   if (rc) return rc;

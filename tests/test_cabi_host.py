@@ -116,3 +116,54 @@ def test_site_order_bijection_and_neighbours(lib, dims, cstar, tile, block, pair
     assert lib.qxd_site_neighbour(h, 0, 0, 4, 1, C.byref(nb)) == -1
     assert lib.qxd_site_coords(h, V // 2, 0, I4()) == -1
     lib.qxd_geometry_destroy(h)
+
+
+@pytest.mark.parametrize("dims,cstar,pairing,ok", [
+    ((8, 8, 8, 8), 0, 0, True),
+    ((8, 8, 8, 8), 3, 0, True),       # extended layout, L1 / 4 even: the C* shift keeps the direction-1 colour
+    ((8, 4, 8, 8), 3, 0, False),      # L1 / 4 odd: a hop across a C* boundary would land on the same colour -> rejected
+    ((8, 4, 8, 8), 3, 1, True),       # paired layout: the shift is a flip of the mirror bit inside the block
+    ((16, 8, 4, 8), 2, 1, True),      # a single block in a C* direction (paired: the wrap stays inside the block)
+    ((12, 4, 4, 4), 0, 0, False),     # three blocks in time
+    ((4, 4, 4, 4), 0, 0, False),      # one tile: an odd number of tiles
+])
+def test_sap_blocks_are_two_coloured(lib, dims, cstar, pairing, ok):
+    """Reading R21 on the host (no GPU): blocks are the 128-index tiles of both parities; whenever a hop leaves a block it
+    lands on a block of the other colour, for every site and direction including the shifted C* wraps; geometries without
+    such a colouring are rejected."""
+    h = C.c_void_p()
+    assert lib.qxd_geometry_create(*dims, cstar | 4, C.byref(h)) == 0
+    if cstar:
+        assert lib.qxd_set_cstar_pairing(h, pairing) == 0
+    V = lib.qxd_volume(h)
+    blk, col, nb = C.c_int(), C.c_int(), C.c_int()
+    rc = lib.qxd_sap_block_of(h, 0, 0, C.byref(blk), C.byref(col))
+    if not ok:
+        assert rc == -1 and b"two-colouring" in lib.qxd_last_error(h)
+        lib.qxd_geometry_destroy(h)
+        return
+    assert rc == 0
+    info = {}
+    for p in (0, 1):
+        for cb in range(V // 2):
+            assert lib.qxd_sap_block_of(h, cb, p, C.byref(blk), C.byref(col)) == 0
+            assert blk.value == cb >> 7
+            info[(cb, p)] = (blk.value, col.value)
+    colour_of_block = {}
+    for (b, c) in info.values():
+        assert colour_of_block.setdefault(b, c) == c                       # one colour per block, both parities
+    counts = [list(colour_of_block.values()).count(k) for k in (0, 1)]
+    assert counts[0] == counts[1] == V // 512                              # half of the blocks each
+    for j in range(V // 512):                                              # the kernel's pairing of consecutive tiles
+        assert colour_of_block[2 * j] != colour_of_block[2 * j + 1]
+    crossings = 0
+    for (cb, p), (b, c) in info.items():
+        for mu in range(4):
+            for step in (+1, -1):
+                assert lib.qxd_site_neighbour(h, cb, p, mu, step, C.byref(nb)) == 0
+                b2, c2 = info[(nb.value, 1 - p)]
+                if b2 != b:
+                    crossings += 1
+                    assert c2 != c, (cb, p, mu, step)
+    assert crossings > 0
+    lib.qxd_geometry_destroy(h)
