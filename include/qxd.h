@@ -59,7 +59,7 @@ typedef enum {
 typedef enum { QXD_F64 = 0, QXD_F32 = 1, QXD_F16 = 2 } qxd_prec;
 #define QXD_PREC_MASK(p) (1 << (p))
 
-typedef enum { QXD_CGNE = 0, QXD_BICGSTAB = 1, QXD_GCR = 2 } qxd_algo;
+typedef enum { QXD_CGNE = 0, QXD_BICGSTAB = 1, QXD_GCR = 2, QXD_DFL_GCR = 3 } qxd_algo;
 
 /* Solver controls (in) and report (out).  Zero-initialise for defaults. */
 typedef struct {
@@ -206,6 +206,24 @@ int qxd_solve_host(qxd_ctx* ctx, const double* eta_host, double* psi_host, doubl
  * direction) are rejected with QXD_EINVAL by qxd_solve.
  * qxd_apply_sap: out = M_sap in on fp32 packed full-lattice spinors (test and bench entry point of the preconditioner). */
 int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
+/* Second level (deflated SAP-GCR on the CPU, multigrid GCR on the GPU): local-coherence deflation on the SAP blocks.
+ *   qxd_set_deflation    ns null vectors (even, <= 32; 0 = off), ninv smoothing passes in the setup (0 = default 4), nkc GCR steps of
+ *                        every coarse-grid solve (0 = default 16); before qxd_workspace_bind; needs qxd_set_gcr too.
+ *   qxd_deflation_setup  random_vectors: DEVICE, ns packed fp32 full-lattice spinors back to back (the caller draws them; any
+ *                        linearly independent set works).  Each is smoothed by ninv applications of M_sap (block operator in storage
+ *                        precision prec = QXD_F32 / QXD_F16), the set is orthonormalised block by block, and the coarse operator
+ *                        A_c = R D_w P (nine-point stencil of ns x ns complex matrices per block) is built.  Must be repeated after
+ *                        every change of the gauge field, the quark or the clover coefficients (else QXD_ESTATE).
+ *   qxd_solve            with algo = QXD_DFL_GCR: the flexible GCR of QXD_GCR with the two-level preconditioner
+ *                            z = P A_c^{-1} R r + M_sap (r - D_w P A_c^{-1} R r),   A_c^{-1} ~ nkc unpreconditioned GCR steps.
+ *   qxd_deflation_info   number of blocks, ns, and whether the setup is valid.
+ *   qxd_deflation_op     test entry: op 0  coarse = R fine;  1  fine = P coarse;  2  coarse_out = A_c coarse_in;  3  fine_out = two-level
+ *                        preconditioner applied to fine_in.  fine: DEVICE packed fp32 full-lattice spinor; coarse: DEVICE [nblocks][ns]
+ *                        complex fp32 (block index = checkerboard index >> 7). */
+int qxd_set_deflation(qxd_ctx* ctx, int ns, int ninv, int nkc);
+int qxd_deflation_setup(qxd_ctx* ctx, int prec, const void* random_vectors /*DEVICE*/);
+int qxd_deflation_info(const qxd_ctx* ctx, int* nblocks, int* ns, int* ready);
+int qxd_deflation_op(qxd_ctx* ctx, int op, const void* in, void* out);
 /* Host-only introspection of the SAP block decomposition (no GPU needed; CPU tests of reading R21): block index (= cb >> 7) and
  * colour (0 / 1) of the site (cb, parity).  QXD_EINVAL if the geometry admits no two-colouring (qxd_last_error says why). */
 int qxd_sap_block_of(qxd_ctx* ctx, int cb, int parity, int* block, int* colour);

@@ -10,7 +10,7 @@ import ctypes as C
 import os
 
 QXD_F64, QXD_F32, QXD_F16 = 0, 1, 2
-QXD_CGNE, QXD_BICGSTAB, QXD_GCR = 0, 1, 2
+QXD_CGNE, QXD_BICGSTAB, QXD_GCR, QXD_DFL_GCR = 0, 1, 2, 3
 QXD_RECON_NONE, QXD_RECON_12 = 18, 12
 QXD_FS_GAUGE, QXD_FS_HOPLINKS, QXD_FS_CLOVER, QXD_FS_HOPLINKS_STALE, QXD_FS_CLOVER_STALE, QXD_FS_LAZY = 1, 2, 4, 8, 16, 32
 QXD_DS_DW, QXD_DS_HOP_AINV, QXD_DS_A_XMHOP, QXD_DS_X_MHOP, QXD_DS_AINV_X_MHOP = 0, 1, 2, 3, 4
@@ -68,6 +68,10 @@ SYMBOLS = {
     "qxd_solve_host": (_i, [_vp, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_set_gcr": (_i, [_vp, _i, _i, _i]),
     "qxd_apply_sap": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_set_deflation": (_i, [_vp, _i, _i, _i]),
+    "qxd_deflation_setup": (_i, [_vp, _i, _vp]),
+    "qxd_deflation_info": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)]),
+    "qxd_deflation_op": (_i, [_vp, _i, _vp, _vp]),
     "qxd_sap_block_of": (_i, [_vp, _i, _i, C.POINTER(_i), C.POINTER(_i)]),
     "qxd_solve_multi": (_i, [_vp, _i, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_apply_Dw_multi_packed": (_i, [_vp, _i, _i, _vp, _vp]),
@@ -129,7 +133,8 @@ def _ptr(t):
 class Qxd:
     """One solver context (qxd_ctx): geometry, workspace, gauge field, quark, clover term."""
 
-    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=None, gcr=None):
+    def __init__(self, T, L1, L2, L3, bc, precisions=(QXD_F64,), nrhs=1, tile=None, block=None, device="cuda:0", pairing=None, gcr=None,
+                 deflation=None):
         import torch
         if not torch.cuda.is_available():
             raise QxdError(QXD_ECUDA, "no CUDA device: the qxd hot path has no CPU fallback")
@@ -153,6 +158,8 @@ class Qxd:
             self._chk(self.lib.qxd_set_block(self.h, *block))
         if gcr is not None:                     # (nkv, ncy, nmr): Krylov space and SAP parameters of QXD_GCR (row f3)
             self._chk(self.lib.qxd_set_gcr(self.h, *gcr))
+        if deflation is not None:               # (ns, ninv, nkc): null vectors, setup smoothing passes, coarse GCR steps (QXD_DFL_GCR)
+            self._chk(self.lib.qxd_set_deflation(self.h, *deflation))
         self.prec_mask = 0
         for p in precisions:
             self.prec_mask |= 1 << p
@@ -286,6 +293,19 @@ class Qxd:
         info = self._info(algo, sloppy, delta, maxiter)
         rc = self._chk(self.lib.qxd_solve(self.h, _ptr(eta), _ptr(psi), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
         return psi, self._report(rc, info)
+
+    def deflation_setup(self, random_vectors, prec=QXD_F16):
+        """random_vectors: ns packed fp32 full-lattice spinors back to back (uint8 tensor on the device)."""
+        self._chk(self.lib.qxd_deflation_setup(self.h, prec, _ptr(random_vectors)))
+
+    def deflation_info(self):
+        nb, ns, rd = C.c_int(0), C.c_int(0), C.c_int(0)
+        self._chk(self.lib.qxd_deflation_info(self.h, C.byref(nb), C.byref(ns), C.byref(rd)))
+        return nb.value, ns.value, bool(rd.value)
+
+    def deflation_op(self, op, tin, tout):
+        self._chk(self.lib.qxd_deflation_op(self.h, op, _ptr(tin), _ptr(tout)))
+        return tout
 
     def apply_sap(self, pin, pout, prec=QXD_F16):
         """pout = M_sap pin on fp32 packed full-lattice spinors; prec = storage precision of the block operator."""

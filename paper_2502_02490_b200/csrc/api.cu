@@ -96,7 +96,23 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
     g_r = k.take(f32); g_res = k.take(f32); g_corr = k.take(f32); g_r64 = k.take(f64); g_t64 = k.take(f64);
     gscal = k.take(4096 * 8);
   }
+  // two-level preconditioner (dfl.cu): ns + 2 fp32 full-lattice vectors, the coarse operator and the coarse-grid vectors
+  void* dphi[32] = {}; void* dcz[32] = {}; void* dcw[32] = {};
+  void* d_t1 = nullptr; void* d_t2 = nullptr; void* dAc = nullptr; void* dnbr = nullptr; void* dcb = nullptr; void* dcx = nullptr; void* dcr = nullptr;
+  void* dscal = nullptr; void* dDinv = nullptr;
+  if (c->dfl_ns > 0) {
+    const size_t f32 = 2 * half_bytes(1, Vh), nb = Vh / 128 > 0 ? Vh / 128 : 1, cv = nb * c->dfl_ns * 8;
+    for (int i = 0; i < c->dfl_ns; i++) dphi[i] = k.take(f32);
+    d_t1 = k.take(f32); d_t2 = k.take(f32);
+    dAc = k.take(nb * 9 * c->dfl_ns * c->dfl_ns * 8); dnbr = k.take(nb * 8 * 4); dDinv = k.take(nb * c->dfl_ns * c->dfl_ns * 8);
+    dcb = k.take(cv); dcx = k.take(cv); dcr = k.take(cv);
+    for (int i = 0; i < c->dfl_nkc; i++) { dcz[i] = k.take(cv); dcw[i] = k.take(cv); }
+    dscal = k.take(4096 * 8);
+  }
   if (assign) {
+    for (int i = 0; i < 32; i++) { c->dphi[i] = dphi[i]; c->dcz[i] = dcz[i]; c->dcw[i] = dcw[i]; }
+    c->d_t1 = d_t1; c->d_t2 = d_t2; c->dAc = dAc; c->dnbr = (int*)dnbr; c->dcb = dcb; c->dcx = dcx; c->dcr = dcr; c->dscal = (double*)dscal; c->dDinv = dDinv;
+    c->dfl_ready = false;
     for (int i = 0; i < 32; i++) { c->gz[i] = gz[i]; c->gw[i] = gw[i]; }
     c->g_r = g_r; c->g_res = g_res; c->g_corr = g_corr; c->g_r64 = g_r64; c->g_t64 = g_t64; c->gscal = (double*)gscal;
     for (int i = 0; i < 2; i++) c->mhi[i] = mhi[i];
@@ -300,7 +316,7 @@ int qxd_gauge_load(qxd_ctx* c, const double* U, const double* A, double qel) {
   c->have_qed = (A != nullptr);
   int rc = launch_gauge_pack(c, U, A);
   if (rc) return rc;
-  c->have_gauge = true;
+  c->have_gauge = true; c->dfl_ready = false;
   if (c->lazy) {   // the quark and clover parameters stay; what they produced is stale until its next use
     c->hop_stale = c->have_quark; c->clover_stale = c->have_clover;
   } else { c->have_quark = false; c->have_clover = false; }
@@ -311,7 +327,7 @@ int qxd_set_quark(qxd_ctx* c, double kappa, double q) {
   if (!c) return QXD_EINVAL;
   if (!c->have_gauge) return fail(c, QXD_ESTATE, "set_quark: load a gauge field first");
   if (!(kappa > 0.0)) return fail(c, QXD_EINVAL, "set_quark: kappa must be > 0");
-  c->kappa = kappa; c->q = q; c->m0 = 1.0 / (2.0 * kappa) - 4.0;
+  c->kappa = kappa; c->q = q; c->m0 = 1.0 / (2.0 * kappa) - 4.0; c->dfl_ready = false;
   if (c->lazy) {   // the clover term depends on m0 and q: stale too if its coefficients are known
     c->have_quark = true; c->hop_stale = true; c->clover_stale = c->have_clover;
     return QXD_OK;
@@ -342,7 +358,7 @@ int qxd_set_gauge_reconstruct(qxd_ctx* c, int recon) {
 int qxd_clover_build(qxd_ctx* c, double csw, double csw_qed) {
   if (!c) return QXD_EINVAL;
   if (!c->have_gauge || !c->have_quark) return fail(c, QXD_ESTATE, "clover_build: needs gauge_load and set_quark");
-  c->csw = csw; c->csw_qed = csw_qed;
+  c->csw = csw; c->csw_qed = csw_qed; c->dfl_ready = false;
   if (c->lazy) { c->have_clover = true; c->clover_stale = true; return QXD_OK; }
   int rc = refresh_clover(c);
   if (rc) return rc;
@@ -638,7 +654,7 @@ int qxd_solve(qxd_ctx* c, const double* eta, double* psi, double tol, qxd_solve_
   if (!info) { std::memset(&local, 0, sizeof(local)); info = &local; }
   int rc = check_apply(c, info->sloppy, eta, psi, "solve");
   if (rc) return rc;
-  if (info->algo == QXD_GCR) return solve_gcr(c, eta, psi, tol, info);
+  if (info->algo == QXD_GCR || info->algo == QXD_DFL_GCR) return solve_gcr(c, eta, psi, tol, info);
   if (info->algo != QXD_CGNE && info->algo != QXD_BICGSTAB) return fail(c, QXD_EINVAL, "solve: unknown algorithm");
   return solve_eo(c, eta, psi, tol, info);
 }
@@ -649,6 +665,38 @@ int qxd_set_gcr(qxd_ctx* c, int nkv, int ncy, int nmr) {
   if (nkv < 0 || nkv > 32 || ncy < 0 || nmr < 0) return fail(c, QXD_EINVAL, "set_gcr: 0 <= nkv <= 32, ncy >= 0, nmr >= 0");
   c->gcr_nkv = nkv; c->gcr_ncy = ncy > 0 ? ncy : 4; c->gcr_nmr = nmr > 0 ? nmr : 4;
   return QXD_OK;
+}
+
+int qxd_set_deflation(qxd_ctx* c, int ns, int ninv, int nkc) {
+  if (!c) return QXD_EINVAL;
+  if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_deflation must precede qxd_workspace_bind");
+  if (ns < 0 || ns > 32 || (ns & 1) || ninv < 0 || nkc < 0 || nkc > 32) return fail(c, QXD_EINVAL, "set_deflation: ns even in 0..32, ninv >= 0, 0 <= nkc <= 32");
+  c->dfl_ns = ns; c->dfl_ninv = ninv > 0 ? ninv : 4; c->dfl_nkc = nkc > 0 ? nkc : 16;
+  return QXD_OK;
+}
+int qxd_deflation_setup(qxd_ctx* c, int prec, const void* random_vectors) {
+  int rc = check_apply(c, prec, random_vectors, random_vectors, "deflation_setup");
+  if (rc) return rc;
+  if (c->dfl_ns < 2 || !c->dphi[0]) return fail(c, QXD_EWORKSPACE, "deflation_setup: call qxd_set_deflation before qxd_workspace_bind");
+  if (c->gcr_nkv < 1) return fail(c, QXD_EWORKSPACE, "deflation_setup: needs the SAP workspace (qxd_set_gcr)");
+  if (!prec_ok(c, 1) || (prec != 1 && prec != 2)) return fail(c, QXD_EINVAL, "deflation_setup: fp32 must be bound; block operator in fp32 or binary16");
+  return dfl_setup(c, prec, random_vectors);
+}
+int qxd_deflation_info(const qxd_ctx* c, int* nblocks, int* ns, int* ready) {
+  if (!c || !nblocks || !ns || !ready) return QXD_EINVAL;
+  *nblocks = c->g.Vh / 128; *ns = c->dfl_ns; *ready = c->dfl_ready ? 1 : 0;
+  return QXD_OK;
+}
+int qxd_deflation_op(qxd_ctx* c, int op, const void* in, void* out) {
+  if (!c || !in || !out) return QXD_EINVAL;
+  if (!c->dfl_ready) return fail(c, QXD_ESTATE, "deflation_op: call qxd_deflation_setup first");
+  switch (op) {
+    case 0: return dfl_restrict(c, in, out);
+    case 1: return dfl_prolong(c, in, out);
+    case 2: return dfl_coarse_apply(c, in, out);
+    case 3: return launch_dfl_precond(c, c->dfl_prec, in, out);
+    default: return fail(c, QXD_EINVAL, "deflation_op: 0 restrict, 1 prolong, 2 coarse operator, 3 two-level preconditioner");
+  }
 }
 
 int qxd_sap_block_of(qxd_ctx* c, int cb, int parity, int* block, int* colour) {

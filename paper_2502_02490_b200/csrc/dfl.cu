@@ -1,0 +1,378 @@
+// dfl.cu -- SURVEY.md §8(f) row f3, second level: the Schwarz-preconditioned GCR of sap.cu / gcr.cu with a coarse-grid
+// (deflation) correction, the ingredient that makes the paper's solvers "heavily preconditioned" (deflated SAP-GCR
+// on the CPU, multigrid GCR on the GPU).  Local-coherence deflation in the style of the host code's solver family:
+//
+//   setup   ns test vectors (random, passed in by the caller) are smoothed by ninv applications of M_sap, which damps the high
+//           modes of D_w and leaves an approximate low-mode space; the vectors are restricted to the SAP blocks (256 sites) and
+//           orthonormalised block by block: the deflation space is span{ P_b phi_i } (dimension ns per block);
+//           the coarse ("little") operator A_c = R D_w P is a nine-point stencil of ns x ns complex matrices (sap.cu).
+//   apply   z = P A_c^{-1} R r  +  M_sap (r - D_w P A_c^{-1} R r):  coarse-grid correction, then Schwarz smoothing of what is left;
+//           A_c^{-1} is nkc steps of GCR on the coarse grid, all coefficients on the device, no host round trip.
+//
+// R = P^dagger (block-wise inner products with the phi_i), P = block-wise linear combination.  Everything is fp32 (the block
+// operator of M_sap and of the coarse-operator build in the storage precision of the solve).  The outer solver is the flexible
+// GCR of gcr.cu: the preconditioner may be as inexact as it likes, convergence is declared on the fp64 residual only.
+#include "gcr_kernels.cuh"
+#include <cmath>
+
+namespace qxd {
+
+namespace {
+
+#define QXD_TRY(expr)        \
+  do {                       \
+    int rc__ = (expr);       \
+    if (rc__) return rc__;   \
+  } while (0)
+
+struct PhiList {
+  const float4* v[32];
+};
+// float4 index of chunk c of the thread's site (block b = blockIdx.x, 256 threads = 128 checkerboard indices x 2 parities)
+__device__ __forceinline__ size_t own_index(int Vh) { return size_t(threadIdx.x >> 7) * 6 * Vh + size_t(blockIdx.x) * 128 + (threadIdx.x & 127); }
+
+// out[b * ldo + j0 + j] = sum_{x in b} conj(u_{j0+j}(x)) . v(x),  j < NJ   (restriction, Gram-Schmidt coefficients, block norms)
+template <int NJ>
+__global__ void __launch_bounds__(256) dfl_block_dots_k(int Vh, PhiList U, int j0, const float4* __restrict__ v, float2* __restrict__ out, int ldo) {
+  __shared__ float red[8][2 * NJ];
+  const size_t own = own_index(Vh);
+  float y[24], part[2 * NJ];
+#pragma unroll
+  for (int c = 0; c < 6; c++) { const float4 t = __ldg(v + own + size_t(c) * Vh); y[4 * c] = t.x; y[4 * c + 1] = t.y; y[4 * c + 2] = t.z; y[4 * c + 3] = t.w; }
+#pragma unroll
+  for (int j = 0; j < NJ; j++) {
+    float re = 0.f, im = 0.f;
+#pragma unroll
+    for (int c = 0; c < 6; c++) {
+      const float4 u = __ldg(U.v[j0 + j] + own + size_t(c) * Vh);
+      re += u.x * y[4 * c]; re += u.y * y[4 * c + 1]; re += u.z * y[4 * c + 2]; re += u.w * y[4 * c + 3];
+      im += u.x * y[4 * c + 1]; im -= u.y * y[4 * c]; im += u.z * y[4 * c + 3]; im -= u.w * y[4 * c + 2];
+    }
+    part[2 * j] = re; part[2 * j + 1] = im;
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+  for (int k = 0; k < 2 * NJ; k++) {
+    float t = part[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) red[warp][k] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < 2 * NJ) {
+    float t = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; w++) t += red[w][threadIdx.x];
+    reinterpret_cast<float*>(out + size_t(blockIdx.x) * ldo + j0)[threadIdx.x] = t;
+  }
+}
+// v(x) = beta v(x) + sign sum_{j<n} c[b * ldc + j] u_j(x)      (Gram-Schmidt update: beta 1, sign -1; prolongation: beta 0, sign +1)
+__global__ void __launch_bounds__(256) dfl_block_axpy_k(int Vh, PhiList U, int n, const float2* __restrict__ coef, int ldc, float beta, float sign,
+                                                        float4* __restrict__ v) {
+  __shared__ float2 cs[32];
+  if (threadIdx.x < n) { const float2 t = coef[size_t(blockIdx.x) * ldc + threadIdx.x]; cs[threadIdx.x] = make_float2(sign * t.x, sign * t.y); }
+  __syncthreads();
+  const size_t own = own_index(Vh);
+  float4 y[6];
+#pragma unroll
+  for (int c = 0; c < 6; c++) {
+    y[c] = beta != 0.f ? v[own + size_t(c) * Vh] : make_float4(0.f, 0.f, 0.f, 0.f);
+    if (beta != 0.f && beta != 1.f) { y[c].x *= beta; y[c].y *= beta; y[c].z *= beta; y[c].w *= beta; }
+  }
+  for (int j = 0; j < n; j++) {
+    const float ar = cs[j].x, ai = cs[j].y;
+#pragma unroll
+    for (int c = 0; c < 6; c++) {
+      const float4 u = __ldg(U.v[j] + own + size_t(c) * Vh);
+      y[c].x += ar * u.x - ai * u.y; y[c].y += ar * u.y + ai * u.x;
+      y[c].z += ar * u.z - ai * u.w; y[c].w += ar * u.w + ai * u.z;
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 6; c++) v[own + size_t(c) * Vh] = y[c];
+}
+// v(x) /= sqrt(n2[b].x)  (block-wise normalisation; a vanishing block is left as it is)
+__global__ void __launch_bounds__(256) dfl_block_scale_k(int Vh, const float2* __restrict__ n2, int ld, float4* __restrict__ v) {
+  const float d = n2[size_t(blockIdx.x) * ld].x;
+  const float s = d > 0.f ? rsqrtf(d) : 1.f;
+  const size_t own = own_index(Vh);
+#pragma unroll
+  for (int c = 0; c < 6; c++) { float4 t = v[own + size_t(c) * Vh]; t.x *= s; t.y *= s; t.z *= s; t.w *= s; v[own + size_t(c) * Vh] = t; }
+}
+// flat helpers on packed full-lattice fp32 vectors
+__global__ void __launch_bounds__(256) dfl_scale_flat_k(size_t n4, const double* __restrict__ n2, float4* __restrict__ v) {
+  const float s = *n2 > 0.0 ? (float)(1.0 / sqrt(*n2)) : 1.f;
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    float4 t = v[i]; t.x *= s; t.y *= s; t.z *= s; t.w *= s; v[i] = t;
+  }
+}
+// z = a - b   /   z = a + b
+__global__ void __launch_bounds__(256) dfl_addsub_flat_k(size_t n4, const float4* __restrict__ a, const float4* __restrict__ b, float sign, float4* __restrict__ z) {
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const float4 x = a[i], y = b[i];
+    z[i] = make_float4(x.x + sign * y.x, x.y + sign * y.y, x.z + sign * y.z, x.w + sign * y.w);
+  }
+}
+// coarse operator: y[b][j] = sum_i A[b][0][j][i] x[b][i] + sum_{d<8} sum_i A[b][1+d][j][i] x[nbr[b][d]][i]; thread per (b, j)
+__global__ void __launch_bounds__(256) dfl_coarse_apply_k(int nblocks, int ns, const float2* __restrict__ A, const int* __restrict__ nbr,
+                                                          const float2* __restrict__ x, float2* __restrict__ y) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = t / ns, j = t - b * ns;
+  if (b >= nblocks) return;
+  float re = 0.f, im = 0.f;
+  for (int d = 0; d < 9; d++) {
+    const int nb = d == 0 ? b : nbr[b * 8 + d - 1];
+    if (nb < 0) continue;
+    const float2* row = A + ((size_t(b) * 9 + d) * ns + j) * ns;
+    const float2* xv = x + size_t(nb) * ns;
+    for (int i = 0; i < ns; i++) {
+      const float2 a = __ldg(row + i), v = __ldg(xv + i);
+      re += a.x * v.x - a.y * v.y; im += a.x * v.y + a.y * v.x;
+    }
+  }
+  y[t] = make_float2(re, im);
+}
+
+// Dinv[b] = A[b][0]^{-1} (ns x ns complex, Gauss-Jordan with partial pivoting, one thread per block; setup only)
+__global__ void __launch_bounds__(64) dfl_diag_inverse_k(int nblocks, int ns, const float2* __restrict__ A, float2* __restrict__ Dinv) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nblocks) return;
+  float2 m[32 * 32];
+  float2* inv = Dinv + size_t(b) * ns * ns;
+  const float2* src = A + size_t(b) * 9 * ns * ns;
+  for (int i = 0; i < ns * ns; i++) { m[i] = src[i]; inv[i] = make_float2((i / ns) == (i % ns) ? 1.f : 0.f, 0.f); }
+  for (int col = 0; col < ns; col++) {
+    int piv = col; float best = m[col * ns + col].x * m[col * ns + col].x + m[col * ns + col].y * m[col * ns + col].y;
+    for (int r = col + 1; r < ns; r++) { const float v = m[r * ns + col].x * m[r * ns + col].x + m[r * ns + col].y * m[r * ns + col].y; if (v > best) { best = v; piv = r; } }
+    if (!(best > 0.f)) continue;
+    if (piv != col) for (int j = 0; j < ns; j++) { float2 t = m[piv * ns + j]; m[piv * ns + j] = m[col * ns + j]; m[col * ns + j] = t; t = inv[piv * ns + j]; inv[piv * ns + j] = inv[col * ns + j]; inv[col * ns + j] = t; }
+    const float2 p = m[col * ns + col];
+    const float dr = p.x / best, di = -p.y / best;
+    for (int j = 0; j < ns; j++) {
+      float2 t = m[col * ns + j]; m[col * ns + j] = make_float2(t.x * dr - t.y * di, t.x * di + t.y * dr);
+      t = inv[col * ns + j]; inv[col * ns + j] = make_float2(t.x * dr - t.y * di, t.x * di + t.y * dr);
+    }
+    for (int r = 0; r < ns; r++) {
+      if (r == col) continue;
+      const float2 f = m[r * ns + col];
+      for (int j = 0; j < ns; j++) {
+        const float2 a = m[col * ns + j], c2 = inv[col * ns + j];
+        m[r * ns + j].x -= f.x * a.x - f.y * a.y; m[r * ns + j].y -= f.x * a.y + f.y * a.x;
+        inv[r * ns + j].x -= f.x * c2.x - f.y * c2.y; inv[r * ns + j].y -= f.x * c2.y + f.y * c2.x;
+      }
+    }
+  }
+}
+// y[b] = Dinv[b] x[b]  (block-Jacobi preconditioner of the coarse GCR); thread per (b, j)
+__global__ void __launch_bounds__(256) dfl_diag_apply_k(int nblocks, int ns, const float2* __restrict__ Dinv, const float2* __restrict__ x, float2* __restrict__ y) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int b = t / ns, j = t - b * ns;
+  if (b >= nblocks) return;
+  const float2* row = Dinv + (size_t(b) * ns + j) * ns;
+  const float2* xv = x + size_t(b) * ns;
+  float re = 0.f, im = 0.f;
+  for (int i = 0; i < ns; i++) { const float2 a = __ldg(row + i), v = __ldg(xv + i); re += a.x * v.x - a.y * v.y; im += a.x * v.y + a.y * v.x; }
+  y[t] = make_float2(re, im);
+}
+// minimal-residual step of the coarse correction on the fine grid: alpha = <t, r> / <t, t> (device, dots = (Re, Im) of <t, r> and |t|^2);
+// t <- r - alpha t  (the residual the Schwarz smoother starts from),  z <- alpha z
+__global__ void __launch_bounds__(256) dfl_mr_step_k(size_t n4, const double* __restrict__ dots, const float4* __restrict__ r, float4* __restrict__ t, float4* __restrict__ z) {
+  const double d = dots[2];
+  const float ar = d > 0.0 ? (float)(dots[0] / d) : 0.f, ai = d > 0.0 ? (float)(dots[1] / d) : 0.f;
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const float4 x = t[i], y = r[i], w = z[i];
+    t[i] = make_float4(y.x - (ar * x.x - ai * x.y), y.y - (ar * x.y + ai * x.x), y.z - (ar * x.z - ai * x.w), y.w - (ar * x.w + ai * x.z));
+    z[i] = make_float4(ar * w.x - ai * w.y, ar * w.y + ai * w.x, ar * w.z - ai * w.w, ar * w.w + ai * w.z);
+  }
+}
+// (Re <t, r>, Im <t, r>, |t|^2)
+__global__ void __launch_bounds__(256) dfl_mr_dots_k(size_t n4, const float4* __restrict__ t, const float4* __restrict__ r, Reducer R) {
+  double acc[3] = {0.0, 0.0, 0.0};
+  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
+    const float4 x = __ldg(t + i), y = __ldg(r + i);
+    float re = x.x * y.x; re += x.y * y.y; re += x.z * y.z; re += x.w * y.w;
+    float im = x.x * y.y; im -= x.y * y.x; im += x.z * y.w; im -= x.w * y.z;
+    float nn = x.x * x.x; nn += x.y * x.y; nn += x.z * x.z; nn += x.w * x.w;
+    acc[0] += (double)re; acc[1] += (double)im; acc[2] += (double)nn;
+  }
+  grid_reduce<3>(acc, R, blockIdx.x, gridDim.x, 0);
+}
+
+struct Dfl {
+  qxd_ctx* c;
+  int Vh, nb, ns;
+  size_t n4, nc4;     // float4 per fine / coarse vector
+  int nblk, nblkc;
+  PhiList phi() const { PhiList P; for (int i = 0; i < 32; i++) P.v[i] = static_cast<const float4*>(c->dphi[i]); return P; }
+  Reducer red(double* result) const { Reducer R; R.partials = c->partials; R.result = result; R.rstride = 0; return R; }
+};
+Dfl make_dfl(qxd_ctx* c) {
+  Dfl D;
+  D.c = c; D.Vh = c->g.Vh; D.nb = c->g.Vh / 128; D.ns = c->dfl_ns;
+  D.n4 = size_t(12) * D.Vh; D.nc4 = size_t(D.nb) * D.ns / 2;
+  D.nblk = D.Vh / 128 < 1 ? 1 : (D.Vh / 128 > 148 * 8 ? 148 * 8 : D.Vh / 128);
+  D.nblkc = int((D.nc4 + 255) / 256); if (D.nblkc > D.nblk) D.nblkc = D.nblk; if (D.nblkc < 1) D.nblkc = 1;
+  return D;
+}
+// out[b][0..ns) = R v  (block inner products with all null vectors)
+int restrict_to_coarse(const Dfl& D, const float4* v, float2* out) {
+  for (int j0 = 0; j0 < D.ns; j0 += 4) {
+    const int nj = D.ns - j0 < 4 ? D.ns - j0 : 4;
+    if (nj == 4) dfl_block_dots_k<4><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
+    else if (nj == 3) dfl_block_dots_k<3><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
+    else if (nj == 2) dfl_block_dots_k<2><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
+    else dfl_block_dots_k<1><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
+    QXD_LAUNCH_CHECK(D.c);
+  }
+  return QXD_OK;
+}
+
+// x = (approximately) A_c^{-1} b: nkc steps of unpreconditioned GCR on the coarse grid (z_k = current residual), every
+// coefficient on the device, one back substitution at the end; no host synchronisation.
+int coarse_solve(const Dfl& D, const float2* b, float2* x) {
+  qxd_ctx* c = D.c;
+  double* S = c->dscal;
+  double* tmp = S + 3000;
+  const int K = c->dfl_nkc;
+  VecList Z, W;
+  for (int k = 0; k < 32; k++) { Z.v[k] = static_cast<const float4*>(c->dcz[k]); W.v[k] = static_cast<const float4*>(c->dcw[k]); }
+  float4* r = static_cast<float4*>(c->dcr);
+  QXD_CUDA_OK(c, cudaMemcpyAsync(r, b, D.nc4 * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  for (int k = 0; k < K; k++) {
+    dfl_diag_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dDinv), reinterpret_cast<const float2*>(r),
+                                                                      static_cast<float2*>(c->dcz[k]));   // z_k = block-Jacobi r
+    QXD_LAUNCH_CHECK(c);
+    dfl_coarse_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), c->dnbr,
+                                                                        static_cast<const float2*>(c->dcz[k]), static_cast<float2*>(c->dcw[k]));
+    QXD_LAUNCH_CHECK(c);
+    float4* wk = static_cast<float4*>(c->dcw[k]);
+    for (int j0 = 0; j0 < k; j0 += 4) {
+      const int nj = k - j0 < 4 ? k - j0 : 4;
+      Reducer R = D.red(S + G_BR + (j0 * 32 + k) * 2);
+      R.rstride = 64;
+      if (nj == 4) gcr_dots_k<4><<<D.nblkc, 256, 0, c->stream>>>(D.nc4, W, j0, wk, R);
+      else if (nj == 3) gcr_dots_k<3><<<D.nblkc, 256, 0, c->stream>>>(D.nc4, W, j0, wk, R);
+      else if (nj == 2) gcr_dots_k<2><<<D.nblkc, 256, 0, c->stream>>>(D.nc4, W, j0, wk, R);
+      else gcr_dots_k<1><<<D.nblkc, 256, 0, c->stream>>>(D.nc4, W, j0, wk, R);
+      QXD_LAUNCH_CHECK(c);
+      reduce_finalize_k<2><<<dim3(1, nj), FINALIZE_THREADS, 0, c->stream>>>(R, D.nblkc);
+      QXD_LAUNCH_CHECK(c);
+    }
+    gcr_orth_k<<<D.nblkc, 256, 0, c->stream>>>(D.nc4, W, k, S + G_BR + k * 2, S + G_N2, wk, r, D.red(tmp));
+    QXD_LAUNCH_CHECK(c);
+    reduce_finalize_k<3><<<dim3(1, 1), FINALIZE_THREADS, 0, c->stream>>>(D.red(tmp), D.nblkc);
+    QXD_LAUNCH_CHECK(c);
+    gcr_store3_k<<<1, 1, 0, c->stream>>>(tmp, S + G_N2 + k, S + G_Q + 2 * k);
+    QXD_LAUNCH_CHECK(c);
+    gcr_update_r_k<<<D.nblkc, 256, 0, c->stream>>>(D.nc4, wk, S + G_Q + 2 * k, S + G_N2 + k, r, D.red(S + G_RR));
+    QXD_LAUNCH_CHECK(c);
+    reduce_finalize_k<1><<<dim3(1, 1), FINALIZE_THREADS, 0, c->stream>>>(D.red(S + G_RR), D.nblkc);
+    QXD_LAUNCH_CHECK(c);
+  }
+  gcr_backsub_k<<<1, 32, 0, c->stream>>>(K, S);
+  QXD_LAUNCH_CHECK(c);
+  gcr_update_x32_k<<<D.nblkc, 256, 0, c->stream>>>(D.nc4, Z, K, S + G_Y, reinterpret_cast<float4*>(x), 1);
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+int apply_Dw32(qxd_ctx* c, void* in, void* out) {
+  const int Vh = c->g.Vh;
+  DslashCall d{};
+  d.prec = 1; d.mode = DS_DW_FULL; d.flags = 0;
+  d.in[0] = half_view(1, in, Vh, 0); d.in[1] = half_view(1, in, Vh, 1);
+  d.out[0] = half_view(1, out, Vh, 0); d.out[1] = half_view(1, out, Vh, 1);
+  return launch_dslash(c, d);
+}
+
+}  // namespace
+
+// z = P A_c^{-1} R r + M_sap (r - D_w P A_c^{-1} R r);  r, z: fp32 packed full-lattice vectors; scratch: the context's d_t1, d_t2
+int launch_dfl_precond(qxd_ctx* c, int prec, const void* r, void* z) {
+  if (!c->dfl_ready) return fail(c, QXD_ESTATE, "deflated preconditioner: call qxd_deflation_setup first");
+  const Dfl D = make_dfl(c);
+  float2* cr = static_cast<float2*>(c->dcb);
+  float2* cx = static_cast<float2*>(c->dcx);
+  float4* z0 = static_cast<float4*>(z);
+  float4* t1 = static_cast<float4*>(c->d_t1);
+  float4* t2 = static_cast<float4*>(c->d_t2);
+  QXD_TRY(restrict_to_coarse(D, static_cast<const float4*>(r), cr));
+  QXD_TRY(coarse_solve(D, cr, cx));
+  dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), D.ns, cx, D.ns, 0.f, 1.f, z0);            // z0 = P cx
+  QXD_LAUNCH_CHECK(c);
+  QXD_TRY(apply_Dw32(c, z0, t1));                                                                            // t1 = D_w z0
+  dfl_addsub_flat_k<<<D.nblk, 256, 0, c->stream>>>(D.n4, static_cast<const float4*>(r), t1, -1.f, t1);      // t1 = r - D_w z0
+  QXD_LAUNCH_CHECK(c);
+  QXD_TRY(launch_sap(c, prec, t1, t2));                                                                      // t2 = M_sap t1
+  dfl_addsub_flat_k<<<D.nblk, 256, 0, c->stream>>>(D.n4, z0, t2, 1.f, z0);                                   // z = z0 + t2
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+// Setup: smooth the caller's ns random vectors with ninv applications of M_sap (normalising in between), orthonormalise them
+// block by block (Gram-Schmidt, twice), build the coarse operator.
+int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors) {
+  const Dfl D = make_dfl(c);
+  const size_t vb = 2 * half_bytes(1, D.Vh);
+  double* S = c->dscal;
+  float4* t2 = static_cast<float4*>(c->d_t2);
+  for (int i = 0; i < D.ns; i++) {
+    float4* v = static_cast<float4*>(c->dphi[i]);
+    QXD_CUDA_OK(c, cudaMemcpyAsync(v, static_cast<const char*>(random_vectors) + vb * i, vb, cudaMemcpyDeviceToDevice, c->stream));
+    for (int it = 0; it < c->dfl_ninv; it++) {
+      QXD_TRY(launch_sap(c, prec, v, t2));
+      VecList L; for (int k = 0; k < 32; k++) L.v[k] = t2;
+      gcr_dots_k<1><<<D.nblk, 256, 0, c->stream>>>(D.n4, L, 0, t2, D.red(S + 3900));
+      QXD_LAUNCH_CHECK(c);
+      reduce_finalize_k<2><<<dim3(1, 1), FINALIZE_THREADS, 0, c->stream>>>(D.red(S + 3900), D.nblk);
+      QXD_LAUNCH_CHECK(c);
+      dfl_scale_flat_k<<<D.nblk, 256, 0, c->stream>>>(D.n4, S + 3900, t2);
+      QXD_LAUNCH_CHECK(c);
+      QXD_CUDA_OK(c, cudaMemcpyAsync(v, t2, vb, cudaMemcpyDeviceToDevice, c->stream));
+    }
+  }
+  float2* coef = static_cast<float2*>(c->dcb);      // [nb][ns] scratch
+  for (int i = 0; i < D.ns; i++) {
+    float4* v = static_cast<float4*>(c->dphi[i]);
+    for (int pass = 0; pass < 2 && i > 0; pass++) {
+      for (int j0 = 0; j0 < i; j0 += 4) {
+        const int nj = i - j0 < 4 ? i - j0 : 4;
+        if (nj == 4) dfl_block_dots_k<4><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
+        else if (nj == 3) dfl_block_dots_k<3><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
+        else if (nj == 2) dfl_block_dots_k<2><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
+        else dfl_block_dots_k<1><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
+        QXD_LAUNCH_CHECK(c);
+      }
+      dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), i, coef, D.ns, 1.f, -1.f, v);
+      QXD_LAUNCH_CHECK(c);
+    }
+    PhiList self; for (int k = 0; k < 32; k++) self.v[k] = v;
+    dfl_block_dots_k<1><<<D.nb, 256, 0, c->stream>>>(D.Vh, self, 0, v, coef, D.ns);
+    QXD_LAUNCH_CHECK(c);
+    dfl_block_scale_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, coef, D.ns, v);     // coef[b * ns].x = |v|_b^2 (ldo = ns, j0 = 0)
+    QXD_LAUNCH_CHECK(c);
+  }
+  QXD_TRY(launch_coarse_build(c, prec, D.ns, c->dphi, c->dAc, c->dnbr));
+  dfl_diag_inverse_k<<<(D.nb + 63) / 64, 64, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), static_cast<float2*>(c->dDinv));
+  QXD_LAUNCH_CHECK(c);
+  c->dfl_ready = true; c->dfl_prec = prec;
+  return QXD_OK;
+}
+
+// test / bench entry points on the coarse level: y = R x (x fine), x = P y, y = A_c x
+int dfl_restrict(qxd_ctx* c, const void* fine, void* coarse) { const Dfl D = make_dfl(c); return restrict_to_coarse(D, static_cast<const float4*>(fine), static_cast<float2*>(coarse)); }
+int dfl_prolong(qxd_ctx* c, const void* coarse, void* fine) {
+  const Dfl D = make_dfl(c);
+  dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), D.ns, static_cast<const float2*>(coarse), D.ns, 0.f, 1.f, static_cast<float4*>(fine));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+int dfl_coarse_apply(qxd_ctx* c, const void* x, void* y) {
+  const Dfl D = make_dfl(c);
+  dfl_coarse_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), c->dnbr, static_cast<const float2*>(x),
+                                                                      static_cast<float2*>(y));
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+}  // namespace qxd

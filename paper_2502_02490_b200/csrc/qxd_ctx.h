@@ -79,6 +79,21 @@ struct qxd_ctx {
   void* g_t64 = nullptr;
   int sap_ok = -1, sap_boxsh[4] = {}, sap_colmask[4] = {};   // two-colouring of the SAP blocks (-1: not yet checked for the current site order)
   double* gscal = nullptr;                       // device scalars of the GCR cycle: coefficient matrix b[32][32] (complex), c[32], y[32], norms
+  // two-level (deflated) preconditioner of the GCR (dfl.cu): null vectors, coarse operator, coarse-grid vectors
+  int dfl_ns = 0, dfl_ninv = 4, dfl_nkc = 16, dfl_prec = 1;
+  bool dfl_ready = false;
+  void* dphi[32] = {};                           // fp32 packed full-lattice null vectors, block-orthonormal
+  void* d_t1 = nullptr;                          // fp32 fine-grid temporaries
+  void* d_t2 = nullptr;
+  void* dAc = nullptr;                           // coarse operator [nblocks][9][ns][ns] complex fp32
+  int* dnbr = nullptr;                           // neighbour blocks [nblocks][8]
+  void* dDinv = nullptr;                         // inverses of the diagonal coarse blocks [nblocks][ns][ns] (block-Jacobi preconditioner)
+  void* dcb = nullptr;                           // coarse vectors [nblocks][ns] complex fp32: right-hand side / scratch,
+  void* dcx = nullptr;                           //   solution,
+  void* dcr = nullptr;                           //   residual,
+  void* dcz[32] = {};                            //   Krylov vectors of the coarse GCR
+  void* dcw[32] = {};
+  double* dscal = nullptr;                       // device scalars of the coarse GCR (layout of gcr_kernels.cuh)
   // reductions
   double* partials = nullptr;
   double* scal = nullptr;                        // device scalars [64]
@@ -201,5 +216,12 @@ int launch_halo_zero(qxd_ctx* c, int prec, void* packed, int pmask, int mu, int 
 int sap_check_geometry(qxd_ctx* c);
 int launch_sap(qxd_ctx* c, int prec, const void* in_full32, void* out_full32);   // out = M_sap in (fp32 packed full-lattice vectors)
 int solve_gcr(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+int launch_coarse_build(qxd_ctx* c, int prec, int ns, void* const* phi, void* A, int* nbr);
+// dfl.cu (row f3, second level)
+int launch_dfl_precond(qxd_ctx* c, int prec, const void* r, void* z);
+int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors);
+int dfl_restrict(qxd_ctx* c, const void* fine, void* coarse);
+int dfl_prolong(qxd_ctx* c, const void* coarse, void* fine);
+int dfl_coarse_apply(qxd_ctx* c, const void* x, void* y);
 
 }  // namespace qxd

@@ -84,13 +84,14 @@ __device__ __forceinline__ void hop_sm(const unsigned (&nbc)[2], int par, int l,
 }
 // hop across the block boundary, from the stored corrections in global memory (prologue)
 template <typename S, int MU, int DIR, int NL, bool PAIR>
-__device__ __forceinline__ void hop_bnd(const SapArgs& a, const Site& s, int tile, int par, int l, const typename PT<S>::V* Wsm, float* acc) {
+__device__ __forceinline__ void hop_bnd(const SapArgs& a, const float4* __restrict__ nsrc, const Site& s, int tile, int par, int l,
+                                        const typename PT<S>::V* Wsm, float* acc) {
   const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
   if ((nb >> 7) == tile) return;
   const int Vh = a.g.Vh;
   float psi[24], w[18], h[12], t[12];
 #pragma unroll
-  for (int c = 0; c < 6; c++) unpack4(__ldg(a.corr[1 - par] + size_t(c) * Vh + nb), psi + 4 * c);
+  for (int c = 0; c < 6; c++) unpack4(__ldg(nsrc + size_t(c) * Vh + nb), psi + 4 * c);
   if (DIR > 0) lds_reals<S, 18 * MU, 18>(Wsm + par * SapShape<S>::NCH * 128, l, w);
   else {   // W_mu(x - mu): the forward link of the neighbour, from its global record
     int wi = nb;
@@ -230,14 +231,14 @@ __global__ void __launch_bounds__(256, SapShape<S>::MINB) sap_mr_k(const __grid_
     float acc[24];
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[i] = 0.f;
-    hop_bnd<S, 0, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 0, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 1, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 1, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 2, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 2, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 3, +1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
-    hop_bnd<S, 3, -1, NL, PAIR>(a, s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 0, +1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 0, -1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 1, +1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 1, -1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 2, +1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 2, -1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 3, +1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
+    hop_bnd<S, 3, -1, NL, PAIR>(a, a.corr[1 - par], s, tile, par, l, Wsm, acc);
 #pragma unroll
     for (int i = 0; i < 24; i++) r[i] += 0.5f * acc[i];
   }
@@ -296,6 +297,126 @@ int sap_launch_t(qxd_ctx* c, const SapArgs& a, int nblocks) {
     configured = true;
   }
   sap_mr_k<S, NL, PAIR><<<nblocks, 256, SapShape<S>::BYTES, c->stream>>>(a);
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
+// ---- coarse (little) Dirac operator of the two-level preconditioner (dfl.cu): for every block b and null vector phi_i the nine
+// block rows  A[b][0][j][i] = <phi_j, D_b phi_i>_b  (Dirichlet block operator) and  A[b][1+d][j][i] = <phi_j, H_d phi_i>_b  (the
+// hops that leave the block in direction d = 2 mu + (dir < 0), reading phi_i on the neighbouring block), built with the block
+// machinery of the Schwarz kernel: links and clover blocks of the block staged in shared memory, phi_i of the block in the ring
+// slot of the residual.  One CTA per block, all blocks.  Also records the neighbour block of every direction.
+struct CoarseArgs {
+  SapArgs a;
+  const float4* phi[32];   // null vectors: fp32 packed full lattice (parity 1 at +6 Vh float4)
+  int ns;
+  float2* A;               // [nblocks][9][ns][ns]
+  int* nbr;                // [nblocks][8], -1 where the block is its own neighbour in that direction
+};
+// sums of the 2 ns per-thread partials over the CTA -> dst[j] (float2), j < ns
+__device__ __forceinline__ void coarse_reduce_store(float (&part)[64], int ns, float* red /*[8][64]*/, float2* dst, int warp, int lane) {
+  for (int k = 0; k < 2 * ns; k++) {
+    float v = part[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) red[warp * 64 + k] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 2 * ns) {
+    float v = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; w++) v += red[w * 64 + threadIdx.x];
+    reinterpret_cast<float*>(dst)[threadIdx.x] = v;
+  }
+  __syncthreads();
+}
+template <typename S, int NL, bool PAIR>
+__global__ void __launch_bounds__(256, 1) coarse_build_k(const __grid_constant__ CoarseArgs ca) {
+  typedef typename PT<S>::V V;
+  const SapArgs& a = ca.a;
+  extern __shared__ __align__(16) unsigned char smem[];
+  float4* rho = reinterpret_cast<float4*>(smem);
+  V* Wsm = reinterpret_cast<V*>(smem + SapShape<S>::RHO);
+  V* Csm = reinterpret_cast<V*>(smem + SapShape<S>::RHO + SapShape<S>::REC);
+  __shared__ float red[8 * 64];
+  const int l = threadIdx.x & 127, par = threadIdx.x >> 7, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int Vh = a.g.Vh, ns = ca.ns;
+  const int tile = blockIdx.x;
+  const int cb = tile * 128 + l;
+  stage_site<S, NL, PAIR>(a, cb, par, l, Wsm, Csm);
+  Site s;
+  site_init<PAIR ? 1 : 0>(a.g, cb, par, s);
+  unsigned nbc[2];
+  int nbt[8];
+  {
+    const int n[8] = {neighbour_cb<0, +1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<0, -1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<1, +1, PAIR ? 1 : 0>(a.g, s),
+                      neighbour_cb<1, -1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<2, +1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<2, -1, PAIR ? 1 : 0>(a.g, s),
+                      neighbour_cb<3, +1, PAIR ? 1 : 0>(a.g, s), neighbour_cb<3, -1, PAIR ? 1 : 0>(a.g, s)};
+    nbc[0] = 0; nbc[1] = 0;
+#pragma unroll
+    for (int d = 0; d < 8; d++) {
+      nbt[d] = n[d] >> 7;
+      nbc[d >> 2] |= (((nbt[d] == tile) ? 0x80u : 0u) | unsigned(n[d] & 127)) << (8 * (d & 3));
+      if (nbt[d] != tile) ca.nbr[tile * 8 + d] = nbt[d];      // every face thread writes the same value
+    }
+  }
+  const size_t own = size_t(par) * 6 * Vh + cb;     // float4 index of chunk 0 of the own site in a packed full-lattice vector
+  for (int i = 0; i < ns; i++) {
+    float r[24], y[24], part[64];
+#pragma unroll
+    for (int c = 0; c < 6; c++) {
+      const float4 v = __ldg(ca.phi[i] + own + size_t(c) * Vh);
+      rho[(par * 6 + c) * 128 + l] = v;
+      unpack4(v, r + 4 * c);
+    }
+    __syncthreads();
+    const float4* nsrc = ca.phi[i] + size_t(1 - par) * 6 * Vh;
+#pragma unroll 1
+    for (int d = 0; d < 9; d++) {
+      if (d == 0) block_apply<S, PAIR>(nbc, cb, par, l, rho, Wsm, Csm, r, y);
+      else {
+#pragma unroll
+        for (int k = 0; k < 24; k++) y[k] = 0.f;
+        switch (d) {
+          case 1: hop_bnd<S, 0, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 2: hop_bnd<S, 0, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 3: hop_bnd<S, 1, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 4: hop_bnd<S, 1, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 5: hop_bnd<S, 2, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 6: hop_bnd<S, 2, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 7: hop_bnd<S, 3, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          default: hop_bnd<S, 3, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+        }
+#pragma unroll
+        for (int k = 0; k < 24; k++) y[k] *= -0.5f;          // H = -1/2 sum (1 -+ gamma) W psi
+      }
+      for (int j = 0; j < ns; j++) {                         // <phi_j, y> at this site
+        float re = 0.f, im = 0.f;
+#pragma unroll
+        for (int c = 0; c < 6; c++) {
+          const float4 u = __ldg(ca.phi[j] + own + size_t(c) * Vh);
+          re += u.x * y[4 * c]; re += u.y * y[4 * c + 1]; re += u.z * y[4 * c + 2]; re += u.w * y[4 * c + 3];
+          im += u.x * y[4 * c + 1]; im -= u.y * y[4 * c]; im += u.z * y[4 * c + 3]; im -= u.w * y[4 * c + 2];
+        }
+        part[2 * j] = re; part[2 * j + 1] = im;
+      }
+      // A[b][d][j][i]: row j, column i -> the reduction delivers a column; store transposed
+      __shared__ float2 col[32];
+      coarse_reduce_store(part, ns, red, col, warp, lane);
+      if (threadIdx.x < ns) ca.A[((size_t(tile) * 9 + d) * ns + threadIdx.x) * ns + i] = col[threadIdx.x];
+      __syncthreads();
+    }
+  }
+}
+template <typename S, int NL, bool PAIR>
+int coarse_build_t(qxd_ctx* c, const CoarseArgs& ca, int nblocks) {
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(coarse_build_k<S, NL, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SapShape<S>::BYTES);
+    if (e != cudaSuccess) return fail(c, QXD_ECUDA, std::string("coarse_build: cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+    configured = true;
+  }
+  coarse_build_k<S, NL, PAIR><<<nblocks, 256, SapShape<S>::BYTES, c->stream>>>(ca);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
@@ -391,6 +512,36 @@ int launch_sap(qxd_ctx* c, int prec, const void* in, void* out) {
       if (rc) return rc;
     }
   return QXD_OK;
+}
+
+
+// Coarse operator of the two-level preconditioner (dfl.cu): A[b][9][ns][ns] and the neighbour-block table, from the ns null
+// vectors phi (fp32 packed full-lattice), with the block operator in storage precision `prec` (fp32 or binary16).
+int launch_coarse_build(qxd_ctx* c, int prec, int ns, void* const* phi, void* A, int* nbr) {
+  if (prec != 1 && prec != 2) return fail(c, QXD_EINVAL, "coarse_build: block operator stored in fp32 or binary16");
+  int rc = sap_check_geometry(c);
+  if (rc) return rc;
+  const int nblocks = c->g.Vh / 128;
+  CoarseArgs ca;
+  ca.a.g = c->g;
+  for (int p = 0; p < 2; p++) {
+    ca.a.W[p] = c->W[prec][p]; ca.a.CL[p] = c->M[prec][p];
+    ca.a.src[p] = nullptr; ca.a.res[p] = nullptr; ca.a.corr[p] = nullptr; ca.a.psi[p] = nullptr;
+  }
+  for (int mu = 0; mu < 4; mu++) { ca.a.boxsh[mu] = c->sap_boxsh[mu]; ca.a.colmask[mu] = c->sap_colmask[mu]; }
+  ca.a.colour = 0; ca.a.prologue = 0; ca.a.init_psi = 0; ca.a.nmr = 0;
+  for (int i = 0; i < 32; i++) ca.phi[i] = i < ns ? static_cast<const float4*>(phi[i]) : nullptr;
+  ca.ns = ns; ca.A = static_cast<float2*>(A); ca.nbr = nbr;
+  QXD_CUDA_OK(c, cudaMemsetAsync(nbr, 0xff, size_t(nblocks) * 8 * sizeof(int), c->stream));
+  const int nl = c->link_reals[prec];
+  if (prec == 1) {
+    if (nl == 14) rc = c->g.pair ? coarse_build_t<float, 14, true>(c, ca, nblocks) : coarse_build_t<float, 14, false>(c, ca, nblocks);
+    else rc = c->g.pair ? coarse_build_t<float, 18, true>(c, ca, nblocks) : coarse_build_t<float, 18, false>(c, ca, nblocks);
+  } else {
+    if (nl == 14) rc = c->g.pair ? coarse_build_t<__half, 14, true>(c, ca, nblocks) : coarse_build_t<__half, 14, false>(c, ca, nblocks);
+    else rc = c->g.pair ? coarse_build_t<__half, 18, true>(c, ca, nblocks) : coarse_build_t<__half, 18, false>(c, ca, nblocks);
+  }
+  return rc;
 }
 
 }  // namespace qxd

@@ -168,3 +168,84 @@ def test_gcr_config_c2_full_size(sloppy):
     assert info["status"] == 0, info
     assert true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05 * cfg["tol"]
     c.close()
+
+
+# ---- second level: local-coherence deflation (qxd_set_deflation / qxd_deflation_setup / QXD_DFL_GCR) ---------------------------
+DFL_GCR = 3
+
+
+def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32):
+    import torch
+    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4), deflation=(ns, ninv, nkc))
+    g = c.gpu
+    rnd = torch.cat([g.spinor_pack(synth.gaussian_spinor(c.dims_ext, 100 + i), F32) for i in range(ns)])
+    g.deflation_setup(rnd, prec)
+    return c, rnd
+
+
+@pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES)
+def test_deflation_subspace_and_coarse_operator(dims, cstar, qed, pairing):
+    """R P = 1 on the coarse space (block-orthonormal null vectors), P R is a projector, and the stored nine-point coarse operator
+    equals R D_w P applied through the (oracle-verified) fp32 D_w kernel."""
+    import torch
+    c, _ = _dfl_case(dims, cstar, qed, pairing)
+    g = c.gpu
+    nb, ns, ready = g.deflation_info()
+    assert ready and nb == c.V // 256 and ns == 8
+    rng = np.random.default_rng(7)
+    cc = torch.from_numpy((rng.normal(size=(nb, ns)) + 1j * rng.normal(size=(nb, ns))).astype(np.complex64)).cuda()
+    fine = g.new_packed(F32)
+    g.deflation_op(1, cc, fine)                                   # P c
+    back = torch.empty_like(cc)
+    g.deflation_op(0, fine, back)                                 # R P c
+    assert float((back - cc).abs().max() / cc.abs().max()) < 2e-5
+    fine2 = g.new_packed(F32)
+    g.deflation_op(1, back, fine2)                                # P R P c = P c
+    a, b = to_np(g.spinor_unpack(fine, F32)), to_np(g.spinor_unpack(fine2, F32))
+    assert relerr(b, a) < 2e-5
+    dfine = g.new_packed(F32)
+    g.apply_Dw_packed(fine, dfine, F32)                           # D_w P c
+    ref_c = torch.empty_like(cc)
+    g.deflation_op(0, dfine, ref_c)                               # R D_w P c
+    got_c = torch.empty_like(cc)
+    g.deflation_op(2, cc, got_c)                                  # A_c c
+    assert float((got_c - ref_c).abs().max() / ref_c.abs().max()) < 1e-4
+    # and against the ORACLE's D_w: R D_ref P c with P c taken from the device
+    dref = c.ref.apply_Dw(a.reshape(tuple(c.dims_ext) + (4, 3)))
+    pd = g.spinor_pack(dref, F32)
+    ref2 = torch.empty_like(cc)
+    g.deflation_op(0, pd, ref2)
+    assert float((got_c - ref2).abs().max() / ref2.abs().max()) < 1e-4
+    c.close()
+
+
+@pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES)
+@pytest.mark.parametrize("sloppy", [F32, F16])
+def test_deflated_gcr_solve(dims, cstar, qed, pairing, sloppy):
+    """QXD_DFL_GCR: the two-level preconditioner is a contraction on the residual (|r - D_ref M r| < |r| with the oracle's D_w),
+    the solve reaches the oracle residual, and a change of the quark invalidates the setup (QXD_ESTATE) until it is redone."""
+    import torch
+    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy)
+    g = c.gpu
+    eta = synth.gaussian_spinor(c.dims_ext, 5)
+    pin = g.spinor_pack(eta, F32)
+    pz = g.new_packed(F32)
+    g.deflation_op(3, pin, pz)
+    r32 = to_np(g.spinor_unpack(pin, F32)).reshape(eta.shape)
+    z = to_np(g.spinor_unpack(pz, F32)).reshape(eta.shape)
+    contraction = np.linalg.norm(r32 - c.ref.apply_Dw(z)) / np.linalg.norm(r32)
+    assert contraction < 0.5, contraction
+    psi, info = g.solve(eta, 1e-10, algo=DFL_GCR, sloppy=sloppy)
+    assert info["status"] == 0, info
+    res = true_residual(c.ref, eta, to_np(psi).reshape(eta.shape))
+    assert res <= 1.05e-10, (res, info)
+    g.set_quark(0.124, 2 / 3 if qed else 0.0)
+    g.clover_build(1.5, 1.0 if qed else 0.0)
+    assert g.deflation_info()[2] is False
+    with pytest.raises(c.B.QxdError) as e:
+        g.solve(eta, 1e-10, algo=DFL_GCR, sloppy=sloppy)
+    assert e.value.status == c.B.QXD_ESTATE
+    g.deflation_setup(rnd, sloppy)                 # redone for the new quark: usable again
+    psi, info = g.solve(eta, 1e-10, algo=DFL_GCR, sloppy=sloppy)
+    assert info["status"] == 0
+    c.close()

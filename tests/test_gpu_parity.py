@@ -32,7 +32,7 @@ class Case:
     """Oracle context + CUDA context on identical seeded fields."""
 
     def __init__(self, dims, cstar, ap, qed, q=2 / 3, kappa=0.12, csw=1.5, csw_qed=1.0, qel=1.0, eps=0.3,
-                 precisions=(F64, F32, F16), tile=None, oracle_clover=True, nrhs=1, pairing=False, share=None, gcr=None):
+                 precisions=(F64, F32, F16), tile=None, oracle_clover=True, nrhs=1, pairing=False, share=None, gcr=None, deflation=None):
         from paper_2502_02490_b200 import binding as B
         self.B = B
         bc = cstar | (ap << 2)
@@ -51,7 +51,7 @@ class Case:
                 self.ref.clover_build(csw, self.csw_qed)
             else:
                 self.ref.set_csw(csw, self.csw_qed)
-        self.gpu = B.Qxd(*dims, bc, precisions=precisions, tile=tile, nrhs=nrhs, pairing=pairing, gcr=gcr)
+        self.gpu = B.Qxd(*dims, bc, precisions=precisions, tile=tile, nrhs=nrhs, pairing=pairing, gcr=gcr, deflation=deflation)
         self.gpu.gauge_load(self.U, self.A, qel)
         self.gpu.set_quark(kappa, self.q)
         self.gpu.clover_build(csw, self.csw_qed)
