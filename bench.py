@@ -538,7 +538,8 @@ def run_cuda(args, cfg):
         g.close()
         torch.cuda.empty_cache()
         gp = (args.gcr_nkv, args.gcr_ncy, args.gcr_nmr)
-        g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=1, device=f"cuda:{local}", pairing=(True if pairing else None), gcr=gp)
+        dp = (args.dfl_ns, args.dfl_ninv, args.dfl_nkc) if args.dfl_ns > 0 else None
+        g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=1, device=f"cuda:{local}", pairing=(True if pairing else None), gcr=gp, deflation=dp)
         Ud = torch.from_numpy(U).to(dev)
         Ad = torch.from_numpy(A).to(dev) if A is not None else None
         g.gauge_load(Ud, Ad, cfg["qel"])
@@ -561,6 +562,21 @@ def run_cuda(args, cfg):
                          "layout": "C*-paired" if pairing else "extended lattice", "block": "128-index tile, both parities (256 sites)",
                          "true_res_oracle": oracle_residual(eta, psi_d)})
             solves[name] = info
+        if dp is not None:   # second level: local-coherence deflation (setup per gauge field and quark, timed separately)
+            rnd = torch.cat([g.spinor_pack(torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 100 + i)).to(dev), B.QXD_F32) for i in range(dp[0])])
+            t0 = ev(); t1 = ev()
+            g.deflation_setup(rnd, B.QXD_F16)
+            t0.record()
+            g.deflation_setup(rnd, B.QXD_F16)
+            t1.record()
+            t1.synchronize()
+            g.solve(eta_d, cfg["tol"], algo=B.QXD_DFL_GCR, sloppy=B.QXD_F16, maxiter=args.maxiter, psi=psi_d)
+            _, info = g.solve(eta_d, cfg["tol"], algo=B.QXD_DFL_GCR, sloppy=B.QXD_F16, maxiter=args.maxiter, psi=psi_d)
+            info.update({"tol": cfg["tol"], "nkv": gp[0], "ncy": gp[1], "nmr": gp[2], "ns": dp[0], "ninv": dp[1], "nkc": dp[2],
+                         "setup_seconds": t0.elapsed_time(t1) * 1e-3, "layout": "C*-paired" if pairing else "extended lattice",
+                         "true_res_oracle": oracle_residual(eta, psi_d)})
+            solves["dfl_gcr_sap_fp64_fp16"] = info
+            del rnd
         del psi_d, pin, pout
 
     # ---- CPU baseline: the oracle on this box's host cores (rank 0, N = 1 only) ----------------------------
@@ -716,6 +732,9 @@ def main():
     ap.add_argument("--gcr-ncy", type=int, default=4, help="SAP cycles per preconditioner application")
     ap.add_argument("--gcr-nmr", type=int, default=5, help="minimal-residual steps per SAP block solve")
     ap.add_argument("--dw-sweep", type=int, default=0, help="use the time-sweep D_w kernel with this segment length for the headline apply (0 = tile kernel)")
+    ap.add_argument("--dfl-ns", type=int, default=24, help="null vectors of the deflated (two-level) GCR solve (0 = skip)")
+    ap.add_argument("--dfl-ninv", type=int, default=8, help="M_sap smoothing passes per null vector in the deflation setup")
+    ap.add_argument("--dfl-nkc", type=int, default=24, help="GCR steps of every coarse-grid solve")
     ap.add_argument("--decomp", default="rhs", choices=["rhs", "domain"], help="rhs: shard by right-hand side (weak scaling, the default); "
                     "domain: cut the lattice along time over the ranks (strong scaling, row f2)")
     ap.add_argument("--no-overlap", action="store_true", help="--decomp domain: exchange the faces before the interior slabs instead of during them")

@@ -208,7 +208,9 @@ int qxd_solve_host(qxd_ctx* ctx, const double* eta_host, double* psi_host, doubl
 int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
 /* Second level (deflated SAP-GCR on the CPU, multigrid GCR on the GPU): local-coherence deflation on the SAP blocks.
  *   qxd_set_deflation    ns null vectors (even, <= 32; 0 = off), ninv smoothing passes in the setup (0 = default 4), nkc GCR steps of
- *                        every coarse-grid solve (0 = default 16); before qxd_workspace_bind; needs qxd_set_gcr too.
+ *                        every coarse-grid solve (0 = default 16), nref rounds of adaptive refinement in the setup (every null
+ *                        vector replaced by the current two-level preconditioner applied to it, space and coarse operator rebuilt;
+ *                        needs ns <= 2 nkv); before qxd_workspace_bind; needs qxd_set_gcr too.
  *   qxd_deflation_setup  random_vectors: DEVICE, ns packed fp32 full-lattice spinors back to back (the caller draws them; any
  *                        linearly independent set works).  Each is smoothed by ninv applications of M_sap (block operator in storage
  *                        precision prec = QXD_F32 / QXD_F16), the set is orthonormalised block by block, and the coarse operator
@@ -220,7 +222,7 @@ int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
  *   qxd_deflation_op     test entry: op 0  coarse = R fine;  1  fine = P coarse;  2  coarse_out = A_c coarse_in;  3  fine_out = two-level
  *                        preconditioner applied to fine_in.  fine: DEVICE packed fp32 full-lattice spinor; coarse: DEVICE [nblocks][ns]
  *                        complex fp32 (block index = checkerboard index >> 7). */
-int qxd_set_deflation(qxd_ctx* ctx, int ns, int ninv, int nkc);
+int qxd_set_deflation(qxd_ctx* ctx, int ns, int ninv, int nkc, int nref);
 int qxd_deflation_setup(qxd_ctx* ctx, int prec, const void* random_vectors /*DEVICE*/);
 int qxd_deflation_info(const qxd_ctx* ctx, int* nblocks, int* ns, int* ready);
 int qxd_deflation_op(qxd_ctx* ctx, int op, const void* in, void* out);

@@ -667,11 +667,11 @@ int qxd_set_gcr(qxd_ctx* c, int nkv, int ncy, int nmr) {
   return QXD_OK;
 }
 
-int qxd_set_deflation(qxd_ctx* c, int ns, int ninv, int nkc) {
+int qxd_set_deflation(qxd_ctx* c, int ns, int ninv, int nkc, int nref) {
   if (!c) return QXD_EINVAL;
   if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_deflation must precede qxd_workspace_bind");
-  if (ns < 0 || ns > 32 || (ns & 1) || ninv < 0 || nkc < 0 || nkc > 32) return fail(c, QXD_EINVAL, "set_deflation: ns even in 0..32, ninv >= 0, 0 <= nkc <= 32");
-  c->dfl_ns = ns; c->dfl_ninv = ninv > 0 ? ninv : 4; c->dfl_nkc = nkc > 0 ? nkc : 16;
+  if (ns < 0 || ns > 32 || (ns & 1) || ninv < 0 || nkc < 0 || nkc > 32 || nref < 0) return fail(c, QXD_EINVAL, "set_deflation: ns even in 0..32, ninv >= 0, 0 <= nkc <= 32, nref >= 0");
+  c->dfl_ns = ns; c->dfl_ninv = ninv > 0 ? ninv : 4; c->dfl_nkc = nkc > 0 ? nkc : 16; c->dfl_nref = nref;
   return QXD_OK;
 }
 int qxd_deflation_setup(qxd_ctx* c, int prec, const void* random_vectors) {

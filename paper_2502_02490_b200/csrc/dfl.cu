@@ -309,28 +309,23 @@ int launch_dfl_precond(qxd_ctx* c, int prec, const void* r, void* z) {
   return QXD_OK;
 }
 
-// Setup: smooth the caller's ns random vectors with ninv applications of M_sap (normalising in between), orthonormalise them
-// block by block (Gram-Schmidt, twice), build the coarse operator.
-int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors) {
-  const Dfl D = make_dfl(c);
-  const size_t vb = 2 * half_bytes(1, D.Vh);
+namespace {
+// v <- v / |v| (global norm) on a packed full-lattice fp32 vector
+int normalise_flat(const Dfl& D, float4* v) {
+  qxd_ctx* c = D.c;
   double* S = c->dscal;
-  float4* t2 = static_cast<float4*>(c->d_t2);
-  for (int i = 0; i < D.ns; i++) {
-    float4* v = static_cast<float4*>(c->dphi[i]);
-    QXD_CUDA_OK(c, cudaMemcpyAsync(v, static_cast<const char*>(random_vectors) + vb * i, vb, cudaMemcpyDeviceToDevice, c->stream));
-    for (int it = 0; it < c->dfl_ninv; it++) {
-      QXD_TRY(launch_sap(c, prec, v, t2));
-      VecList L; for (int k = 0; k < 32; k++) L.v[k] = t2;
-      gcr_dots_k<1><<<D.nblk, 256, 0, c->stream>>>(D.n4, L, 0, t2, D.red(S + 3900));
-      QXD_LAUNCH_CHECK(c);
-      reduce_finalize_k<2><<<dim3(1, 1), FINALIZE_THREADS, 0, c->stream>>>(D.red(S + 3900), D.nblk);
-      QXD_LAUNCH_CHECK(c);
-      dfl_scale_flat_k<<<D.nblk, 256, 0, c->stream>>>(D.n4, S + 3900, t2);
-      QXD_LAUNCH_CHECK(c);
-      QXD_CUDA_OK(c, cudaMemcpyAsync(v, t2, vb, cudaMemcpyDeviceToDevice, c->stream));
-    }
-  }
+  VecList L; for (int k = 0; k < 32; k++) L.v[k] = v;
+  gcr_dots_k<1><<<D.nblk, 256, 0, c->stream>>>(D.n4, L, 0, v, D.red(S + 3900));
+  QXD_LAUNCH_CHECK(c);
+  reduce_finalize_k<2><<<dim3(1, 1), FINALIZE_THREADS, 0, c->stream>>>(D.red(S + 3900), D.nblk);
+  QXD_LAUNCH_CHECK(c);
+  dfl_scale_flat_k<<<D.nblk, 256, 0, c->stream>>>(D.n4, S + 3900, v);
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+// block-wise Gram-Schmidt (twice) of the null vectors, then the coarse operator and the inverses of its diagonal blocks
+int orthonormalise_and_build(const Dfl& D, int prec) {
+  qxd_ctx* c = D.c;
   float2* coef = static_cast<float2*>(c->dcb);      // [nb][ns] scratch
   for (int i = 0; i < D.ns; i++) {
     float4* v = static_cast<float4*>(c->dphi[i]);
@@ -355,7 +350,46 @@ int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors) {
   QXD_TRY(launch_coarse_build(c, prec, D.ns, c->dphi, c->dAc, c->dnbr));
   dfl_diag_inverse_k<<<(D.nb + 63) / 64, 64, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), static_cast<float2*>(c->dDinv));
   QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+}  // namespace
+
+// Setup: smooth the caller's ns random vectors with ninv applications of M_sap (normalising in between), orthonormalise them
+// block by block (Gram-Schmidt, twice), build the coarse operator.  Then nref rounds of adaptive refinement: every null vector
+// is replaced by the two-level preconditioner applied to it (which amplifies exactly what the current method still converges
+// slowly on), and the space and the coarse operator are rebuilt.
+int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors) {
+  const Dfl D = make_dfl(c);
+  const size_t vb = 2 * half_bytes(1, D.Vh);
+  float4* t2 = static_cast<float4*>(c->d_t2);
+  c->dfl_ready = false;
+  for (int i = 0; i < D.ns; i++) {
+    float4* v = static_cast<float4*>(c->dphi[i]);
+    QXD_CUDA_OK(c, cudaMemcpyAsync(v, static_cast<const char*>(random_vectors) + vb * i, vb, cudaMemcpyDeviceToDevice, c->stream));
+    for (int it = 0; it < c->dfl_ninv; it++) {
+      QXD_TRY(launch_sap(c, prec, v, t2));
+      QXD_TRY(normalise_flat(D, t2));
+      QXD_CUDA_OK(c, cudaMemcpyAsync(v, t2, vb, cudaMemcpyDeviceToDevice, c->stream));
+    }
+  }
+  QXD_TRY(orthonormalise_and_build(D, prec));
   c->dfl_ready = true; c->dfl_prec = prec;
+  for (int round = 0; round < c->dfl_nref; round++) {
+    // new vectors from the CURRENT two-level method, parked in the Krylov space of the fine-grid GCR until all are done
+    if (D.ns > 2 * c->gcr_nkv) return fail(c, QXD_EWORKSPACE, "deflation refinement needs ns <= 2 nkv scratch vectors (qxd_set_gcr)");
+    for (int i = 0; i < D.ns; i++) {
+      void* dst = i < c->gcr_nkv ? c->gz[i] : c->gw[i - c->gcr_nkv];
+      QXD_TRY(launch_dfl_precond(c, prec, c->dphi[i], dst));
+      QXD_TRY(normalise_flat(D, static_cast<float4*>(dst)));
+    }
+    for (int i = 0; i < D.ns; i++) {
+      void* src = i < c->gcr_nkv ? c->gz[i] : c->gw[i - c->gcr_nkv];
+      QXD_CUDA_OK(c, cudaMemcpyAsync(c->dphi[i], src, vb, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    c->dfl_ready = false;
+    QXD_TRY(orthonormalise_and_build(D, prec));
+    c->dfl_ready = true;
+  }
   return QXD_OK;
 }
 

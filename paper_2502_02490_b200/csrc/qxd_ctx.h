@@ -80,7 +80,7 @@ struct qxd_ctx {
   int sap_ok = -1, sap_boxsh[4] = {}, sap_colmask[4] = {};   // two-colouring of the SAP blocks (-1: not yet checked for the current site order)
   double* gscal = nullptr;                       // device scalars of the GCR cycle: coefficient matrix b[32][32] (complex), c[32], y[32], norms
   // two-level (deflated) preconditioner of the GCR (dfl.cu): null vectors, coarse operator, coarse-grid vectors
-  int dfl_ns = 0, dfl_ninv = 4, dfl_nkc = 16, dfl_prec = 1;
+  int dfl_ns = 0, dfl_ninv = 4, dfl_nkc = 16, dfl_nref = 0, dfl_prec = 1;
   bool dfl_ready = false;
   void* dphi[32] = {};                           // fp32 packed full-lattice null vectors, block-orthonormal
   void* d_t1 = nullptr;                          // fp32 fine-grid temporaries

@@ -174,9 +174,9 @@ def test_gcr_config_c2_full_size(sloppy):
 DFL_GCR = 3
 
 
-def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32):
+def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32, nref=0):
     import torch
-    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4), deflation=(ns, ninv, nkc))
+    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4), deflation=(ns, ninv, nkc, nref))
     g = c.gpu
     rnd = torch.cat([g.spinor_pack(synth.gaussian_spinor(c.dims_ext, 100 + i), F32) for i in range(ns)])
     g.deflation_setup(rnd, prec)
@@ -225,7 +225,7 @@ def test_deflated_gcr_solve(dims, cstar, qed, pairing, sloppy):
     """QXD_DFL_GCR: the two-level preconditioner is a contraction on the residual (|r - D_ref M r| < |r| with the oracle's D_w),
     the solve reaches the oracle residual, and a change of the quark invalidates the setup (QXD_ESTATE) until it is redone."""
     import torch
-    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy)
+    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy, nref=1 if sloppy == F32 else 0)
     g = c.gpu
     eta = synth.gaussian_spinor(c.dims_ext, 5)
     pin = g.spinor_pack(eta, F32)
