@@ -536,10 +536,30 @@ def run_cuda(args, cfg):
     # context of its own (the Krylov space is part of the workspace): library default layout, link formats as above
     if not args.no_solve and args.gcr_nkv > 0:
         g.close()
+        packed = None                     # the packed sweep spinors of the first context are not needed any more
         torch.cuda.empty_cache()
         gp = (args.gcr_nkv, args.gcr_ncy, args.gcr_nmr)
         dp = (args.dfl_ns, args.dfl_ninv, args.dfl_nkc) if args.dfl_ns > 0 else None
-        g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=1, device=f"cuda:{local}", pairing=(True if pairing else None), gcr=gp, deflation=dp)
+        # the Krylov space and the deflation space are part of the workspace: take the largest number of null vectors that
+        # leaves room for the test vectors of the setup (the largest lattices run with fewer, or without the second level)
+        g = None
+        for ns_try in ([dp[0], 16, 8] if dp else []) + [0]:
+            dtry = (ns_try, dp[1], dp[2]) if (dp and ns_try > 0) else None
+            try:
+                g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=1, device=f"cuda:{local}", pairing=(True if pairing else None), gcr=gp, deflation=dtry)
+                free = torch.cuda.mem_get_info(dev)[0]
+                need = g.packed_spinor_bytes(B.QXD_F32) * ns_try + 5 * g.packed_spinor_bytes(B.QXD_F64)
+                if free >= need:
+                    break
+                g.close()
+                g = None
+                torch.cuda.empty_cache()
+            except torch.OutOfMemoryError:
+                g = None
+                torch.cuda.empty_cache()
+        if dp is not None and dtry != dp:
+            solves["dfl_gcr_sap_fp64_fp16_note"] = f"device memory: {dp[0]} null vectors requested, {ns_try} used"
+        dp = dtry
         Ud = torch.from_numpy(U).to(dev)
         Ad = torch.from_numpy(A).to(dev) if A is not None else None
         g.gauge_load(Ud, Ad, cfg["qel"])
@@ -563,7 +583,10 @@ def run_cuda(args, cfg):
                          "true_res_oracle": oracle_residual(eta, psi_d)})
             solves[name] = info
         if dp is not None:   # second level: local-coherence deflation (setup per gauge field and quark, timed separately)
-            rnd = torch.cat([g.spinor_pack(torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 100 + i)).to(dev), B.QXD_F32) for i in range(dp[0])])
+            nbv = g.packed_spinor_bytes(B.QXD_F32)
+            rnd = torch.empty(dp[0] * nbv, dtype=torch.uint8, device=dev)
+            for i in range(dp[0]):
+                g.spinor_pack(torch.from_numpy(synth_mod.gaussian_spinor(cfg["dims_ext"], 100 + i)).to(dev), B.QXD_F32, packed=rnd[i * nbv:(i + 1) * nbv])
             t0 = ev(); t1 = ev()
             g.deflation_setup(rnd, B.QXD_F16)
             t0.record()
