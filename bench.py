@@ -345,7 +345,7 @@ def run_cuda(args, cfg):
     sweep = {}
     nrep = max(10, min(args.steps, 50))
     for nl, tag in ((18, ""), (14, "_recon12")):
-        if args.no_sweep:
+        if args.no_sweep or args.only_multi:
             break
         g.set_gauge_reconstruct(B.QXD_RECON_12 if nl == 14 else B.QXD_RECON_NONE)
         for p in precs:
@@ -371,7 +371,7 @@ def run_cuda(args, cfg):
 
     # ---- multi-RHS D_w (row a10): links and clover blocks read once for a batch of right-hand sides --------
     multi = {}
-    if args.nrhs > 1 and not args.no_sweep:
+    if args.nrhs > 1 and (not args.no_sweep or args.only_multi):
         n = args.nrhs
         for p in (B.QXD_F32, B.QXD_F16):
             nb = g.packed_spinor_bytes(p)
@@ -382,7 +382,15 @@ def run_cuda(args, cfg):
             ms = timed(lambda: g.apply_Dw_multi_packed(pin, pout, p, n), max(3, nrep // 5))
             reals = 48 + 144.0 / n
             multi[PREC_NAME[p]] = {"nrhs": n, "ms_per_rhs": ms / n, "GBps": reals * PREC_BYTES[p] * V * n / ms / 1e6,
-                                   "Gflops": FLOP_PER_SITE * V * n / ms / 1e6, "speedup_vs_single": sweep[PREC_NAME[p]]["Dw_ms"] * n / ms}
+                                   "Gflops": FLOP_PER_SITE * V * n / ms / 1e6, "speedup_vs_single": (sweep[PREC_NAME[p]]["Dw_ms"] * n / ms) if PREC_NAME[p] in sweep else None}
+            if n % 4 == 0:      # experimental layout: right-hand sides across lanes (csrc/dslash_ilv.cu)
+                qin = torch.empty_like(pin)
+                g.multi_interleave(pin, qin, p, n, True)
+                for _ in range(2):
+                    g.apply_Dw_multi_interleaved(qin, pout, p, n)
+                ms_i = timed(lambda: g.apply_Dw_multi_interleaved(qin, pout, p, n), max(3, nrep // 5))
+                multi[PREC_NAME[p]]["ms_per_rhs_interleaved"] = ms_i / n
+                del qin
             del pin, pout
 
     # ---- end to end through the host-pointer C-ABI call (H2D + pack + apply + unpack + D2H every step) ------
@@ -422,7 +430,7 @@ def run_cuda(args, cfg):
         setup_ms["clover_build_invert_paired"] = ep0.elapsed_time(ep1)
         del Ud, Ad
         for nl, tag in ((18, "_paired"), (14, "_paired_recon12")):
-            if args.no_sweep:
+            if args.no_sweep or args.only_multi:
                 break
             g.set_gauge_reconstruct(B.QXD_RECON_12 if nl == 14 else B.QXD_RECON_NONE)
             for p in precs:
@@ -765,6 +773,7 @@ def main():
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the precision sweep (short runs under ncu)")
+    ap.add_argument("--only-multi", action="store_true", help="of the sweep, run only the multi-RHS D_w lines (short runs under ncu)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-pointer end-to-end loops (short runs under ncu)")
     ap.add_argument("--sustain-s", type=float, default=1.0, help="seconds of back-to-back applies for the `sustained` figure (0 = skip)")
     ap.add_argument("--no-oracle-residual", action="store_true", help="skip the oracle's whole-lattice true residual of the solves")

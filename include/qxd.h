@@ -261,6 +261,13 @@ int qxd_set_dw_sweep(qxd_ctx* ctx, int tseg);
  * clover blocks to r right-hand sides (qxd_set_rhs_per_thread: 0 = library default (1), 1..3; fp64 always 1). */
 int qxd_apply_Dw_multi_packed(qxd_ctx* ctx, int prec, int nrhs, const void* in, void* out);
 int qxd_set_rhs_per_thread(qxd_ctx* ctx, int r);
+/* EXPERIMENTAL variant of qxd_apply_Dw_multi_packed with the right-hand sides ACROSS LANES (csrc/dslash_ilv.cu): nrhs (a
+ * multiple of 4) spinors are stored in groups of four, chunk c of site cb of right-hand side j of a group at vector index
+ * (c Vh + cb) 4 + j, so that the four lanes of a site share every link and clover load.  qxd_multi_interleave converts between
+ * nrhs plain packed spinors (back to back) and that layout (to_interleaved != 0) or back; same total size.  Same arithmetic per
+ * site and right-hand side as the plain batch: identical results. */
+int qxd_multi_interleave(qxd_ctx* ctx, int prec, int nrhs, void* plain /*DEVICE*/, void* interleaved /*DEVICE*/, int to_interleaved);
+int qxd_apply_Dw_multi_interleaved(qxd_ctx* ctx, int prec, int nrhs, const void* in, void* out);
 
 /* ---- openQxD field orders (§2, §4.1) ---------------------------------
  * The paper's host code keeps its fields in its own order; these calls convert between that order and the natural

@@ -76,6 +76,8 @@ SYMBOLS = {
     "qxd_solve_multi": (_i, [_vp, _i, _vp, _vp, _d, C.POINTER(SolveInfo)]),
     "qxd_apply_Dw_multi_packed": (_i, [_vp, _i, _i, _vp, _vp]),
     "qxd_set_rhs_per_thread": (_i, [_vp, _i]),
+    "qxd_multi_interleave": (_i, [_vp, _i, _i, _vp, _vp, _i]),
+    "qxd_apply_Dw_multi_interleaved": (_i, [_vp, _i, _i, _vp, _vp]),
     "qxd_packed_spinor_bytes": (_sz, [_vp, _i, _i]),
     "qxd_spinor_pack": (_i, [_vp, _i, _vp, _vp]),
     "qxd_spinor_unpack": (_i, [_vp, _i, _vp, _vp]),
@@ -236,6 +238,13 @@ class Qxd:
         cnt = (C.c_long * 2)()
         self._chk(self.lib.qxd_field_status(self.h, C.byref(st), cnt))
         return st.value, cnt[0], cnt[1]
+
+    def multi_interleave(self, plain, interleaved, prec, nrhs, to_interleaved=True):
+        self._chk(self.lib.qxd_multi_interleave(self.h, prec, nrhs, _ptr(plain), _ptr(interleaved), int(bool(to_interleaved))))
+
+    def apply_Dw_multi_interleaved(self, pin, pout, prec, nrhs):
+        self._chk(self.lib.qxd_apply_Dw_multi_interleaved(self.h, prec, nrhs, _ptr(pin), _ptr(pout)))
+        return pout
 
     def set_dw_sweep(self, tseg):
         self._chk(self.lib.qxd_set_dw_sweep(self.h, int(tseg)))

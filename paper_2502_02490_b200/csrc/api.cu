@@ -423,6 +423,17 @@ int qxd_apply_Dw_multi_packed(qxd_ctx* c, int prec, int nrhs, const void* in, vo
   return launch_dslash(c, d);
 }
 
+int qxd_apply_Dw_multi_interleaved(qxd_ctx* c, int prec, int nrhs, const void* in, void* out) {
+  int rc = check_apply(c, prec, in, out, "apply_Dw_multi_interleaved");
+  if (rc) return rc;
+  if (nrhs < 4 || nrhs > 64) return fail(c, QXD_EINVAL, "apply_Dw_multi_interleaved: nrhs must be a multiple of 4 in 4..64");
+  return launch_dw_ilv(c, prec, nrhs, in, out);
+}
+int qxd_multi_interleave(qxd_ctx* c, int prec, int nrhs, void* plain, void* interleaved, int to_interleaved) {
+  if (!c || !plain || !interleaved || prec < 0 || prec >= NPREC || !c->ws) return c ? fail(c, QXD_EINVAL, "multi_interleave: bad argument") : QXD_EINVAL;
+  return launch_ilv_convert(c, prec, nrhs, plain, interleaved, to_interleaved);
+}
+
 int qxd_set_rhs_per_thread(qxd_ctx* c, int r) {
   if (!c || r < 0 || r > 3) return c ? fail(c, QXD_EINVAL, "set_rhs_per_thread: 0 (default), 1, 2 or 3") : QXD_EINVAL;
   c->rhs_per_thread = r;

@@ -205,6 +205,9 @@ int blas_copy(qxd_ctx* c, int prec, const SpinorPtr& x, const SpinorPtr& y, cons
 // solver.cu
 int solve_eo(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
 int solve_eo_multi(qxd_ctx* c, int nrhs, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info);
+// dslash_ilv.cu
+int launch_dw_ilv(qxd_ctx* c, int prec, int nrhs, const void* in, void* out);
+int launch_ilv_convert(qxd_ctx* c, int prec, int nrhs, void* plain, void* ilv, int to_ilv);
 // dslash_sweep.cu
 int launch_dw_sweep(qxd_ctx* c, const SpinorPtr in[2], const SpinorPtr out[2]);
 // halo.cu (row f2)

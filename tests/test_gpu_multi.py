@@ -40,6 +40,34 @@ def test_apply_Dw_multi(dims, cstar, qed, nrhs, prec, rpt):
     c.close()
 
 
+@pytest.mark.parametrize("dims,cstar,qed,pairing", [((8, 4, 4, 8), 0, False, False), ((8, 4, 4, 8), 3, True, False), ((8, 4, 4, 8), 3, True, True),
+                                                    ((6, 4, 6, 10), 2, True, True)])
+@pytest.mark.parametrize("prec", [F64, F32, F16])
+@pytest.mark.parametrize("recon", [18, 14])
+def test_apply_Dw_multi_interleaved_is_bit_identical(dims, cstar, qed, pairing, prec, recon):
+    """Experimental layout of row a10 (right-hand sides across lanes, csrc/dslash_ilv.cu): interleave -> batched D_w -> de-interleave
+    must equal the plain batch bit for bit (same arithmetic per site and right-hand side), which is itself compared with the oracle
+    in test_apply_Dw_multi; ragged tile tail (Vh = 720 x 2) and both link formats included."""
+    import torch
+    c = Case(dims, cstar, 1, qed, nrhs=8, pairing=pairing)
+    g = c.gpu
+    g.set_gauge_reconstruct(c.B.QXD_RECON_12 if recon == 14 else c.B.QXD_RECON_NONE)
+    n = 8
+    nb = g.packed_spinor_bytes(prec)
+    pin = torch.zeros(n * nb, dtype=torch.uint8, device="cuda")
+    for k in range(n):
+        g.spinor_pack(synth.gaussian_spinor(c.dims_ext, 11 + k), prec, packed=pin[k * nb:(k + 1) * nb])
+    pout, qin, qout, back = (torch.zeros_like(pin) for _ in range(4))
+    g.apply_Dw_multi_packed(pin, pout, prec, n)
+    g.multi_interleave(pin, qin, prec, n, True)
+    g.apply_Dw_multi_interleaved(qin, qout, prec, n)
+    g.multi_interleave(back, qout, prec, n, False)
+    assert torch.equal(back, pout)
+    with pytest.raises(c.B.QxdError):
+        g.apply_Dw_multi_interleaved(qin, qout, prec, 6)          # not a multiple of 4
+    c.close()
+
+
 @pytest.mark.parametrize("sloppy", [F32, F16])
 @pytest.mark.parametrize("rpt", [0, 2])
 def test_solve_multi(sloppy, rpt):
