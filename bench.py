@@ -40,7 +40,7 @@ FALLBACK_HBM_GBS = 6650.0               # /opt/skills/guides/B200_PROFILING.md f
 # keyed by what the capture was taken on: (config, storage precision, stored reals per link, layout).  Any other
 # combination reports "traffic": null (a capture of another lattice says nothing about this one).
 NCU_TRAFFIC = {
-    ("c3", 1, 18, "extended"): (3688878848, "profiles/r2e_dw_sweep_vs_tile_c3.md"),   # 3.267301 GB read + 0.421578 GB write (tile kernel)
+    ("c3", 1, 18, "extended"): (3663867392, "profiles/r2e_dw_sweep_vs_tile_c3.md"),   # 3.256693 GB read + 0.407175 GB write (tile kernel, final tree)
 }
 
 
