@@ -309,10 +309,82 @@ __device__ __forceinline__ void hop_use(const HopRegs<S, R, NL>& d, typename PT<
     else reconstruct<MU, DIR, PT<S>::ID == 2>(t, acc[r], (C)d.scale[r]);
   }
 }
-// all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one
+// EXPERIMENT (QXD_ASYNC_RING = depth >= 3, off by default): the hops in flight wait in a per-thread shared-memory ring filled by
+// cp.async instead of in registers, so that `depth` hops (not two) are outstanding per thread.
+#ifndef QXD_ASYNC_RING
+#define QXD_ASYNC_RING 0
+#endif
+__device__ __forceinline__ void ring_cp16(void* smem, const void* gmem) {
+  unsigned sa = static_cast<unsigned>(__cvta_generic_to_shared(smem));
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void ring_cp4(void* smem, const void* gmem) {
+  unsigned sa = static_cast<unsigned>(__cvta_generic_to_shared(smem));
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gmem) : "memory");
+}
+template <int N> __device__ __forceinline__ void ring_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+template <typename S, int NL, int DEPTH> struct HopRing {
+  typedef typename PT<S>::V V;
+  static constexpr int NCH = HopRegs<S, 1, NL>::NPSI + HopRegs<S, 1, NL>::NWC;
+  V v[DEPTH][NCH][128];
+  float scale[DEPTH][128];
+};
+template <typename S, int H, int NL, bool PAIR, int DEPTH>
+__device__ __forceinline__ void ring_issue(const DslashArgs& a, const Site& s, int cb, int parity, HopRing<S, NL, DEPTH>& ring, float (&wsgn)[DEPTH]) {
+  typedef typename PT<S>::V V;
+  constexpr int MU = H >> 1, DIR = (H & 1) ? -1 : +1, SLOT = H % DEPTH;
+  typedef LinkChunks<MU, S, NL> LC;
+  const int Vh = a.g.Vh, t = threadIdx.x & 127;
+  const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
+  const V* p = reinterpret_cast<const V*>(a.in[1 - parity].data);
+#pragma unroll
+  for (int c = 0; c < HopRegs<S, 1, NL>::NPSI; c++) ring_cp16(&ring.v[SLOT][c][t], p + size_t(c) * Vh + nb);
+  if (PT<S>::ID == 2) ring_cp4(&ring.scale[SLOT][t], a.in[1 - parity].scale + nb);
+  const V* w = reinterpret_cast<const V*>(DIR > 0 ? a.W[parity] : a.W[1 - parity]);
+  int wi = DIR > 0 ? cb : nb;
+  wsgn[SLOT] = 1.f;
+  if (PAIR) { wsgn[SLOT] = (wi & 1) ? -1.f : 1.f; wi >>= 1; }
+  const int Vs = PAIR ? a.g.Vg : Vh;
+#pragma unroll
+  for (int c = 0; c < LC::N; c++) ring_cp16(&ring.v[SLOT][HopRegs<S, 1, NL>::NPSI + c][t], w + size_t(LC::C0 + c) * Vs + wi);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+}
+template <typename S, int H, bool G5IN, int NL, bool PAIR, int DEPTH>
+__device__ __forceinline__ void ring_step(const DslashArgs& a, const Site& s, int cb, int parity, HopRing<S, NL, DEPTH>& ring, float (&wsgn)[DEPTH],
+                                          typename PT<S>::C (*acc)[24]) {
+  constexpr int MU = H >> 1, DIR = (H & 1) ? -1 : +1, SLOT = H % DEPTH;
+  typedef LinkChunks<MU, S, NL> LC;
+  ring_wait<(7 - H < DEPTH - 1) ? 7 - H : DEPTH - 1>();
+  const int t = threadIdx.x & 127;
+  HopRegs<S, 1, NL> d;
+#pragma unroll
+  for (int c = 0; c < HopRegs<S, 1, NL>::NPSI; c++) d.psi[0][c] = ring.v[SLOT][c][t];
+#pragma unroll
+  for (int c = 0; c < LC::N; c++) d.w[c] = ring.v[SLOT][HopRegs<S, 1, NL>::NPSI + c][t];
+  d.scale[0] = PT<S>::ID == 2 ? ring.scale[SLOT][t] : 1.f;
+  d.wsgn = wsgn[SLOT];
+  if constexpr (H + DEPTH < 8) ring_issue<S, H + DEPTH, NL, PAIR, DEPTH>(a, s, cb, parity, ring, wsgn);
+  hop_use<S, MU, DIR, G5IN, 1, NL, PAIR>(d, acc);
+}
+// all eight hops; PIPE = 2: two hops in flight (software pipeline), PIPE = 1: one; PIPE >= 3: cp.async ring of that depth
 template <typename S, bool G5IN, int R, int PIPE, int NL, bool PAIR>
 __device__ __forceinline__ void hop_all(const DslashArgs& a, const Site& s, int cb, int parity, int rhs0, typename PT<S>::C (*acc)[24]) {
-  if (PIPE == 2) {
+  if constexpr (PIPE >= 3) {
+    __shared__ HopRing<S, NL, PIPE> ring;
+    float wsgn[PIPE];
+    ring_issue<S, 0, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn);
+    ring_issue<S, 1, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn);
+    ring_issue<S, 2, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn);
+    if constexpr (PIPE >= 4) ring_issue<S, 3, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn);
+    ring_step<S, 0, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 1, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 2, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 3, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 4, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 5, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 6, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+    ring_step<S, 7, G5IN, NL, PAIR, PIPE>(a, s, cb, parity, ring, wsgn, acc);
+  } else if (PIPE == 2) {
     HopRegs<S, R, NL> d0, d1;
     hop_issue<S, 0, +1, R, NL, PAIR>(a, s, cb, parity, rhs0, d0);
     hop_issue<S, 0, -1, R, NL, PAIR>(a, s, cb, parity, rhs0, d1);
@@ -361,7 +433,7 @@ template <typename S, int R, bool FULL, int NL> struct KernelShape {
   static constexpr int THREADS = (FULL && !SPLIT) ? 256 : 128;
   // CTAs per SM the register budget is sized for
   static constexpr int MINB = SPLIT ? (sizeof(S) == 8 ? 2 : 4) : sizeof(S) == 8 ? 1 : (R == 1 ? (FULL ? 2 : 4) : (R == 2 ? (FULL ? 1 : 3) : (FULL ? 1 : 2)));
-  static constexpr int PIPE = (R == 1) ? 2 : 1;   // hops in flight per thread
+  static constexpr int PIPE = (QXD_ASYNC_RING >= 3 && R == 1 && !FULL && sizeof(S) == 2) ? QXD_ASYNC_RING : (R == 1) ? 2 : 1;   // hops in flight per thread
 };
 template <typename S, int PHI, int POST, bool NEG, int FLAGS, bool FULL, int R, int NL, bool PAIR>
 __global__ void __launch_bounds__(KernelShape<S, R, FULL, NL>::THREADS, KernelShape<S, R, FULL, NL>::MINB) dslash_k(const __grid_constant__ DslashArgs a) {
