@@ -62,64 +62,74 @@ __device__ __forceinline__ void m3_adj_mul(const double* a, const double* b, dou
 
 struct GaugePtrs { const void* U[2]; const void* A[2]; };
 
-// links and A of the site s; in the paired layout the records are those of the physical site and the mirror image
-// (s.m = 1) takes U^* and -A (reading R8)
-template <int MU>
-__device__ __forceinline__ void link_at(const GaugePtrs& P, const Geom& g, const Site& s, double* m) {
-  load_reals<double, 18 * MU, 18>(P.U[site_parity(s)], g.Vg, s.idx2 >> 1, m);
-  if (s.m) {
+// links and A of a site; in the paired layout the records are those of the physical site and the mirror image
+// (mirror bit = 1) takes U^* and -A (reading R8).  The plaquette arithmetic keeps only a handle of a neighbour site alive
+// (record index, parity, mirror bit), and the plane (mu, nu) is a run-time argument: six unrolled template instances of
+// the 12 matrix products were ~250 KB of code, and the kernel spent its time waiting for instructions
+// (ncu: stall_no_instruction 11.5 per issue).
+__device__ __forceinline__ int site_ref(const Site& s) { return ((s.idx2 >> 1) << 2) | (site_parity(s) << 1) | s.m; }
+__device__ __forceinline__ void link_ref(const GaugePtrs& P, const Geom& g, int mu, int ref, double* m) {
+  const double2* p = reinterpret_cast<const double2*>(P.U[(ref >> 1) & 1]) + size_t(9 * mu) * g.Vg + (ref >> 2);
+  const double sg = (ref & 1) ? -1.0 : 1.0;
 #pragma unroll
-    for (int k = 0; k < 9; k++) m[2 * k + 1] = -m[2 * k + 1];
+  for (int c = 0; c < 9; c++) {
+    const double2 v = __ldg(p + size_t(c) * g.Vg);
+    m[2 * c] = v.x; m[2 * c + 1] = sg * v.y;
   }
 }
-template <int MU>
-__device__ __forceinline__ double a_at(const GaugePtrs& P, const Geom& g, const Site& s) {
-  double a;
-  load_reals<double, MU, 1>(P.A[site_parity(s)], g.Vg, s.idx2 >> 1, &a);
+__device__ __forceinline__ double a_at(const GaugePtrs& P, const Geom& g, int mu, const Site& s) {
+  const double a = __ldg(reinterpret_cast<const double*>(P.A[site_parity(s)]) + (size_t(mu >> 1) * g.Vg + (s.idx2 >> 1)) * 2 + (mu & 1));
   return s.m ? -a : a;
 }
-template <int MU, int NU>
-__device__ __forceinline__ double phi_at(const GaugePtrs& P, const Geom& g, const Site& y) {
+__device__ __forceinline__ double phi_at(const GaugePtrs& P, const Geom& g, int mu, int nu, const Site& y) {
   Site ypm, ypn;
-  site_step(g, y, MU, +1, ypm);
-  site_step(g, y, NU, +1, ypn);
-  return a_at<MU>(P, g, y) + a_at<NU>(P, g, ypm) - a_at<MU>(P, g, ypn) - a_at<NU>(P, g, y);
+  site_step(g, y, mu, +1, ypm);
+  site_step(g, y, nu, +1, ypn);
+  return a_at(P, g, mu, y) + a_at(P, g, nu, ypm) - a_at(P, g, mu, ypn) - a_at(P, g, nu, y);
 }
 
 // X_{mu nu}(x) = csw F-hat_{mu nu} + q csw_qed A-hat_{mu nu} 1   (anti-Hermitian 3x3)
-template <int MU, int NU>
-__device__ void plane_X(const GaugePtrs& P, const Geom& g, const Site& x, double csw, double qcq, double qel, int use_a, double* X) {
-  Site xpm, xpn, xmm, xmn, xmmpn, xmmmn, xpmmn;
-  site_step(g, x, MU, +1, xpm); site_step(g, x, NU, +1, xpn);
-  site_step(g, x, MU, -1, xmm); site_step(g, x, NU, -1, xmn);
-  site_step(g, xmm, NU, +1, xmmpn); site_step(g, xmm, NU, -1, xmmmn); site_step(g, xpm, NU, -1, xpmmn);
+__device__ __forceinline__ void plane_X(const GaugePtrs& P, const Geom& g, const Site& x, int mu, int nu, double csw, double qcq, double qel,
+                                        int use_a, double* X) {
+  int r_x, r_pm, r_pn, r_mm, r_mn, r_mmpn, r_mmmn, r_pmmn;
+  {
+    Site y, z;
+    r_x = site_ref(x);
+    site_step(g, x, mu, +1, y); r_pm = site_ref(y);
+    site_step(g, y, nu, -1, z); r_pmmn = site_ref(z);
+    site_step(g, x, nu, +1, y); r_pn = site_ref(y);
+    site_step(g, x, nu, -1, y); r_mn = site_ref(y);
+    site_step(g, x, mu, -1, y); r_mm = site_ref(y);
+    site_step(g, y, nu, +1, z); r_mmpn = site_ref(z);
+    site_step(g, y, nu, -1, z); r_mmmn = site_ref(z);
+  }
   double Q[18];
 #pragma unroll
   for (int i = 0; i < 18; i++) Q[i] = 0.0;
   if (csw != 0.0) {
     m3 a, b, t1, t2, t3;
     // leaf 1: U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
-    link_at<MU>(P, g, x, a); link_at<NU>(P, g, xpm, b); m3_mul(a, b, t1);
-    link_at<MU>(P, g, xpn, a); m3_mul_adj(t1, a, t2);
-    link_at<NU>(P, g, x, a); m3_mul_adj(t2, a, t3);
+    link_ref(P, g, mu, r_x, a); link_ref(P, g, nu, r_pm, b); m3_mul(a, b, t1);
+    link_ref(P, g, mu, r_pn, a); m3_mul_adj(t1, a, t2);
+    link_ref(P, g, nu, r_x, a); m3_mul_adj(t2, a, t3);
 #pragma unroll
     for (int i = 0; i < 18; i++) Q[i] += t3[i];
     // leaf 2: U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
-    link_at<NU>(P, g, x, a); link_at<MU>(P, g, xmmpn, b); m3_mul_adj(a, b, t1);
-    link_at<NU>(P, g, xmm, a); m3_mul_adj(t1, a, t2);
-    link_at<MU>(P, g, xmm, a); m3_mul(t2, a, t3);
+    link_ref(P, g, nu, r_x, a); link_ref(P, g, mu, r_mmpn, b); m3_mul_adj(a, b, t1);
+    link_ref(P, g, nu, r_mm, a); m3_mul_adj(t1, a, t2);
+    link_ref(P, g, mu, r_mm, a); m3_mul(t2, a, t3);
 #pragma unroll
     for (int i = 0; i < 18; i++) Q[i] += t3[i];
     // leaf 3: U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
-    link_at<NU>(P, g, xmmmn, a); link_at<MU>(P, g, xmm, b); m3_mul(a, b, t1);   // (U_nu(x-mu-nu) U_mu(x-mu))
-    link_at<MU>(P, g, xmmmn, a); m3_adj_mul(t1, a, t2);                          // ^dag * U_mu(x-mu-nu)
-    link_at<NU>(P, g, xmn, a); m3_mul(t2, a, t3);
+    link_ref(P, g, nu, r_mmmn, a); link_ref(P, g, mu, r_mm, b); m3_mul(a, b, t1);   // (U_nu(x-mu-nu) U_mu(x-mu))
+    link_ref(P, g, mu, r_mmmn, a); m3_adj_mul(t1, a, t2);                           // ^dag * U_mu(x-mu-nu)
+    link_ref(P, g, nu, r_mn, a); m3_mul(t2, a, t3);
 #pragma unroll
     for (int i = 0; i < 18; i++) Q[i] += t3[i];
     // leaf 4: U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
-    link_at<NU>(P, g, xmn, a); link_at<MU>(P, g, xmn, b); m3_adj_mul(a, b, t1);
-    link_at<NU>(P, g, xpmmn, a); m3_mul(t1, a, t2);
-    link_at<MU>(P, g, x, a); m3_mul_adj(t2, a, t3);
+    link_ref(P, g, nu, r_mn, a); link_ref(P, g, mu, r_mn, b); m3_adj_mul(a, b, t1);
+    link_ref(P, g, nu, r_pmmn, a); m3_mul(t1, a, t2);
+    link_ref(P, g, mu, r_x, a); m3_mul_adj(t2, a, t3);
 #pragma unroll
     for (int i = 0; i < 18; i++) Q[i] += t3[i];
   }
@@ -133,20 +143,21 @@ __device__ void plane_X(const GaugePtrs& P, const Geom& g, const Site& x, double
     }
   if (use_a && qcq != 0.0) {
     // A-hat = (i/(4 qel)) sum over the four leaves of sin(qel Phi)
-    double s = sin(qel * phi_at<MU, NU>(P, g, x)) + sin(qel * phi_at<MU, NU>(P, g, xmm)) + sin(qel * phi_at<MU, NU>(P, g, xmn)) +
-               sin(qel * phi_at<MU, NU>(P, g, xmmmn));
+    Site xmm, xmn, xmmmn;
+    site_step(g, x, mu, -1, xmm); site_step(g, x, nu, -1, xmn); site_step(g, xmm, nu, -1, xmmmn);
+    double s = sin(qel * phi_at(P, g, mu, nu, x)) + sin(qel * phi_at(P, g, mu, nu, xmm)) + sin(qel * phi_at(P, g, mu, nu, xmn)) +
+               sin(qel * phi_at(P, g, mu, nu, xmmmn));
     double ah = qcq * s / (4.0 * qel);
     X[1] += ah; X[9] += ah; X[17] += ah;  // imaginary parts of the diagonal
   }
 }
 
-// add sign_p*(i/2) X to Cp and sign_m*(i/2) X to Cm
-__device__ __forceinline__ void acc_C(const double* X, double sp, double sm, double* Cp, double* Cm) {
+// C += sign * (i/2) X
+__device__ __forceinline__ void acc_C(const double* X, double sign, double* C) {
 #pragma unroll
   for (int k = 0; k < 9; k++) {
-    double re = -0.5 * X[2 * k + 1], im = 0.5 * X[2 * k];  // (i/2) X
-    Cp[2 * k] += sp * re; Cp[2 * k + 1] += sp * im;
-    Cm[2 * k] += sm * re; Cm[2 * k + 1] += sm * im;
+    C[2 * k] += sign * (-0.5 * X[2 * k + 1]);
+    C[2 * k + 1] += sign * (0.5 * X[2 * k]);
   }
 }
 
@@ -178,30 +189,49 @@ __device__ __forceinline__ void block_from_C(double diag, const double* C1, cons
     }
 }
 
-__global__ void __launch_bounds__(64) clover_build_k(Geom g, GaugePtrs P, double diag, double csw, double qcq, double qel, int use_a,
-                                                     void* M0, void* M1) {
-  int cb = blockIdx.x * blockDim.x + threadIdx.x;   // index of the clover record (physical site in the paired layout)
-  int parity = blockIdx.y;
-  if (cb >= g.Vg) return;
-  Site x;
-  site_init(g, g.pair ? 2 * cb : cb, parity, x);
-  double out[72];
-  double Cp[3][18], Cm[3][18];
+// One thread per (site, plane): the six anti-Hermitian X_{mu nu} of a site are built by six warps of the CTA (a warp = one
+// plane of 32 consecutive sites, so the template choice is warp-uniform and the link loads coalesce), parked in shared memory,
+// and two threads per site then assemble the two chirality blocks.  (One thread per site held 2 x 54 accumulators next to
+// the plane arithmetic: 255 registers and 428 B of spills.)
+constexpr int CB_SITES = 32;
+__global__ void __launch_bounds__(6 * CB_SITES, 2) clover_build_k(Geom g, GaugePtrs P, double diag, double csw, double qcq, double qel, int use_a,
+                                                                void* M0, void* M1) {
+  __shared__ double Xs[6][18][CB_SITES];
+  const int lane = threadIdx.x & (CB_SITES - 1), pl = threadIdx.x / CB_SITES;
+  const int cb = blockIdx.x * CB_SITES + lane;   // index of the clover record (physical site in the paired layout)
+  const int parity = blockIdx.y;
+  const bool act = cb < g.Vg;
+  if (act) {
+    Site x;
+    site_init(g, g.pair ? 2 * cb : cb, parity, x);
+    double X[18];
+    // planes in the order E_1 = X_01, B_1 = X_23, E_2 = X_02, X_13 = -B_2, E_3 = X_03, B_3 = X_12
+    const int mu = (0x101020 >> (4 * pl)) & 3, nu = (0x233231 >> (4 * pl)) & 3;
+    plane_X(P, g, x, mu, nu, csw, qcq, qel, use_a, X);
 #pragma unroll
-  for (int k = 0; k < 3; k++)
+    for (int i = 0; i < 18; i++) Xs[pl][i][lane] = X[i];
+  }
+  __syncthreads();
+  if (!act || pl >= 2) return;
+  // chirality block pl (0: C^+, 1: C^-).  E_k = X_{0k}: C^+ += (i/2) E, C^- -= (i/2) E;  B_k: C^+- -= (i/2) B  (B_2 = -X_13)
+  double C[3][18], X[18];
 #pragma unroll
-    for (int i = 0; i < 18; i++) { Cp[k][i] = 0.0; Cm[k][i] = 0.0; }
-  double X[18];
-  // E_k = X_{0k}:  C^+ += (i/2) E, C^- -= (i/2) E ;  B_k:  C^+- -= (i/2) B
-  plane_X<0, 1>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, -1.0, Cp[0], Cm[0]);
-  plane_X<2, 3>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, -1.0, -1.0, Cp[0], Cm[0]);   // B_1 = X_23
-  plane_X<0, 2>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, -1.0, Cp[1], Cm[1]);
-  plane_X<1, 3>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, +1.0, Cp[1], Cm[1]);   // B_2 = X_31 = -X_13
-  plane_X<0, 3>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, +1.0, -1.0, Cp[2], Cm[2]);
-  plane_X<1, 2>(P, g, x, csw, qcq, qel, use_a, X); acc_C(X, -1.0, -1.0, Cp[2], Cm[2]);   // B_3 = X_12
-  block_from_C(diag, Cp[0], Cp[1], Cp[2], out);
-  block_from_C(diag, Cm[0], Cm[1], Cm[2], out + 36);
-  store_record<double, 72>(parity ? M1 : M0, g.Vg, cb, out);
+  for (int k = 0; k < 3; k++) {
+#pragma unroll
+    for (int i = 0; i < 18; i++) C[k][i] = 0.0;
+#pragma unroll
+    for (int i = 0; i < 18; i++) X[i] = Xs[2 * k][i][lane];
+    acc_C(X, pl == 0 ? +1.0 : -1.0, C[k]);
+#pragma unroll
+    for (int i = 0; i < 18; i++) X[i] = Xs[2 * k + 1][i][lane];
+    acc_C(X, k == 1 ? +1.0 : -1.0, C[k]);
+  }
+  double out[36];
+  block_from_C(diag, C[0], C[1], C[2], out);
+  typedef PT<double>::V V;
+  V* q = reinterpret_cast<V*>(parity ? M1 : M0);
+#pragma unroll
+  for (int k = 0; k < 18; k++) q[size_t(18 * pl + k) * g.Vg + cb] = make_double2(out[2 * k], out[2 * k + 1]);
 }
 
 // Fast path of the block inversion: in-place Gauss-Jordan WITHOUT pivoting, fully unrolled so that the 6x6 complex matrix
@@ -332,9 +362,9 @@ __global__ void __launch_bounds__(64) clover_invert_k(int Vh, const void* M, voi
 int launch_clover_build(qxd_ctx* c) {
   GaugePtrs P;
   P.U[0] = c->Ug[0]; P.U[1] = c->Ug[1]; P.A[0] = c->Ag[0]; P.A[1] = c->Ag[1];
-  dim3 gr((c->g.Vg + 63) / 64, 2);
+  dim3 gr((c->g.Vg + CB_SITES - 1) / CB_SITES, 2);
   double diag = 4.0 + c->m0;
-  clover_build_k<<<gr, 64, 0, c->stream>>>(c->g, P, diag, c->csw, c->q * c->csw_qed, c->qel, c->have_qed ? 1 : 0, c->M[0][0], c->M[0][1]);
+  clover_build_k<<<gr, 6 * CB_SITES, 0, c->stream>>>(c->g, P, diag, c->csw, c->q * c->csw_qed, c->qel, c->have_qed ? 1 : 0, c->M[0][0], c->M[0][1]);
   QXD_LAUNCH_CHECK(c);
   int* flag = reinterpret_cast<int*>(c->scal + 60);
   QXD_CUDA_OK(c, cudaMemsetAsync(flag, 0, 2 * sizeof(int), c->stream));
