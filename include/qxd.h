@@ -217,10 +217,15 @@ int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
  *                        A_c = R D_w P (nine-point stencil of ns x ns complex matrices per block) is built.  Must be repeated after
  *                        every change of the gauge field, the quark or the clover coefficients (else QXD_ESTATE).
  *   qxd_solve            with algo = QXD_DFL_GCR: the flexible GCR of QXD_GCR with the two-level preconditioner
- *                            z = P A_c^{-1} R r + M_sap (r - D_w P A_c^{-1} R r),   A_c^{-1} ~ nkc unpreconditioned GCR steps.
+ *                            z = P A_c^{-1} R r + M_sap (r - D_w P A_c^{-1} R r),   A_c^{-1} ~ nkc GCR steps on the even-odd
+ *                        (Schur) form of the coarse system: the blocks are two-coloured and the nine-point operator only joins
+ *                        opposite colours, so x_e solves (1 - Dinv_e H_eo Dinv_o H_oe) x_e = Dinv_e (b_e - H_eo Dinv_o b_o) and
+ *                        x_o = Dinv_o (b_o - H_oe x_e); the hop matrices and the inverses Dinv of the diagonal blocks are read
+ *                        from a binary16 copy (a preconditioner: the outer flexible GCR absorbs the rounding).
  *   qxd_deflation_info   number of blocks, ns, and whether the setup is valid.
- *   qxd_deflation_op     test entry: op 0  coarse = R fine;  1  fine = P coarse;  2  coarse_out = A_c coarse_in;  3  fine_out = two-level
- *                        preconditioner applied to fine_in.  fine: DEVICE packed fp32 full-lattice spinor; coarse: DEVICE [nblocks][ns]
+ *   qxd_deflation_op     test entry: op 0  coarse = R fine;  1  fine = P coarse;  2  coarse_out = A_c coarse_in (fp32 operator);
+ *                        3  fine_out = two-level preconditioner applied to fine_in;  4  coarse_out = the coarse solver applied to
+ *                        coarse_in (~ A_c^{-1} coarse_in).  fine: DEVICE packed fp32 full-lattice spinor; coarse: DEVICE [nblocks][ns]
  *                        complex fp32 (block index = checkerboard index >> 7). */
 int qxd_set_deflation(qxd_ctx* ctx, int ns, int ninv, int nkc, int nref);
 int qxd_deflation_setup(qxd_ctx* ctx, int prec, const void* random_vectors /*DEVICE*/);

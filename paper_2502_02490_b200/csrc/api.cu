@@ -99,19 +99,21 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
   // two-level preconditioner (dfl.cu): ns + 2 fp32 full-lattice vectors, the coarse operator and the coarse-grid vectors
   void* dphi[32] = {}; void* dcz[32] = {}; void* dcw[32] = {};
   void* d_t1 = nullptr; void* d_t2 = nullptr; void* dAc = nullptr; void* dnbr = nullptr; void* dcb = nullptr; void* dcx = nullptr; void* dcr = nullptr;
-  void* dscal = nullptr; void* dDinv = nullptr;
+  void* dscal = nullptr; void* dDinv = nullptr; void* dAh = nullptr; void* dcol = nullptr; void* dcs = nullptr; void* dct = nullptr;
   if (c->dfl_ns > 0) {
     const size_t f32 = 2 * half_bytes(1, Vh), nb = Vh / 128 > 0 ? Vh / 128 : 1, cv = nb * c->dfl_ns * 8;
     for (int i = 0; i < c->dfl_ns; i++) dphi[i] = k.take(f32);
     d_t1 = k.take(f32); d_t2 = k.take(f32);
     dAc = k.take(nb * 9 * c->dfl_ns * c->dfl_ns * 8); dnbr = k.take(nb * 8 * 4); dDinv = k.take(nb * c->dfl_ns * c->dfl_ns * 8);
-    dcb = k.take(cv); dcx = k.take(cv); dcr = k.take(cv);
+    dcb = k.take(cv); dcx = k.take(cv); dcr = k.take(cv); dcs = k.take(cv); dct = k.take(cv);
+    dAh = k.take(nb * 9 * c->dfl_ns * c->dfl_ns * 4); dcol = k.take(nb * 4);
     for (int i = 0; i < c->dfl_nkc; i++) { dcz[i] = k.take(cv); dcw[i] = k.take(cv); }
     dscal = k.take(4096 * 8);
   }
   if (assign) {
     for (int i = 0; i < 32; i++) { c->dphi[i] = dphi[i]; c->dcz[i] = dcz[i]; c->dcw[i] = dcw[i]; }
     c->d_t1 = d_t1; c->d_t2 = d_t2; c->dAc = dAc; c->dnbr = (int*)dnbr; c->dcb = dcb; c->dcx = dcx; c->dcr = dcr; c->dscal = (double*)dscal; c->dDinv = dDinv;
+    c->dAh = dAh; c->dcol = (int*)dcol; c->dcs = dcs; c->dct = dct;
     c->dfl_ready = false;
     for (int i = 0; i < 32; i++) { c->gz[i] = gz[i]; c->gw[i] = gw[i]; }
     c->g_r = g_r; c->g_res = g_res; c->g_corr = g_corr; c->g_r64 = g_r64; c->g_t64 = g_t64; c->gscal = (double*)gscal;
@@ -706,7 +708,8 @@ int qxd_deflation_op(qxd_ctx* c, int op, const void* in, void* out) {
     case 1: return dfl_prolong(c, in, out);
     case 2: return dfl_coarse_apply(c, in, out);
     case 3: return launch_dfl_precond(c, c->dfl_prec, in, out);
-    default: return fail(c, QXD_EINVAL, "deflation_op: 0 restrict, 1 prolong, 2 coarse operator, 3 two-level preconditioner");
+    case 4: return dfl_coarse_solve(c, in, out);
+    default: return fail(c, QXD_EINVAL, "deflation_op: 0 restrict, 1 prolong, 2 coarse operator, 3 two-level preconditioner, 4 coarse solve");
   }
 }
 

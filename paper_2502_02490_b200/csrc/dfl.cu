@@ -14,6 +14,7 @@
 // GCR of gcr.cu: the preconditioner may be as inexact as it likes, convergence is declared on the fp64 residual only.
 #include "gcr_kernels.cuh"
 #include <cmath>
+#include <vector>
 
 namespace qxd {
 
@@ -174,6 +175,66 @@ __global__ void __launch_bounds__(256) dfl_diag_apply_k(int nblocks, int ns, con
   for (int i = 0; i < ns; i++) { const float2 a = __ldg(row + i), v = __ldg(xv + i); re += a.x * v.x - a.y * v.y; im += a.x * v.y + a.y * v.x; }
   y[t] = make_float2(re, im);
 }
+// ---- even-odd (Schur) form of the coarse system ------------------------------------------------------------------------
+// The blocks are two-coloured and every hop of the nine-point operator joins blocks of opposite colours, so with A_c = D + H
+// (D the diagonal blocks) the coarse system splits as on the fine grid:
+//     (1 - Dinv_e H_eo Dinv_o H_oe) x_e = Dinv_e (b_e - H_eo Dinv_o b_o),      x_o = Dinv_o (b_o - H_oe x_e).
+// k GCR steps on the left-hand operator span the same space as 2k steps on the block-Jacobi preconditioned full operator, at
+// half the matrix traffic each; the matrices are read from a transposed binary16 copy (thread j of a block reads column j:
+// 4 ns contiguous bytes per row for the block's ns threads).
+__global__ void __launch_bounds__(256) dfl_pack16_k(int nblocks, int ns, const float2* __restrict__ A, const float2* __restrict__ Dinv, __half2* __restrict__ Ah) {
+  const size_t n = size_t(nblocks) * 9 * ns * ns;
+  for (size_t t = size_t(blockIdx.x) * blockDim.x + threadIdx.x; t < n; t += size_t(gridDim.x) * blockDim.x) {
+    const int j = int(t % ns), i = int((t / ns) % ns), slot = int((t / (size_t(ns) * ns)) % 9);
+    const size_t b = t / (size_t(9) * ns * ns);
+    const float2 v = slot < 8 ? A[((b * 9 + 1 + slot) * ns + j) * ns + i] : Dinv[(b * ns + j) * ns + i];
+    Ah[t] = __floats2half2_rn(v.x, v.y);
+  }
+}
+// y[b] = (u ? u[b] : 0) + sign * Dinv[b] sum_d A[b][1+d] x[nbr[b][d]] on the blocks of `colour`, 0 on the others.
+// One CTA per pair of blocks (2k, 2k+1) -- they have opposite colours (sap_check_geometry) -- of 8 ns threads: thread (d, j)
+// forms row j of hop d of the active block (ns loads of 4 bytes, contiguous over j), the eight partial sums meet in shared
+// memory, the first ns threads multiply by Dinv and write both blocks (zeros for the other colour).
+__global__ void __launch_bounds__(256) dfl_eo_hop_k(int ns, int colour, float sign, const __half2* __restrict__ Ah, const int* __restrict__ nbr,
+                                                    const int* __restrict__ col, const float2* __restrict__ x, const float2* __restrict__ u, float2* __restrict__ y) {
+  __shared__ float2 part[8 * 32];
+  __shared__ float2 t[32];
+  const int d = threadIdx.x / ns, j = threadIdx.x - d * ns;
+  const int b = 2 * blockIdx.x + (col[2 * blockIdx.x] != colour ? 1 : 0);
+  float re = 0.f, im = 0.f;
+  const int nb = nbr[b * 8 + d];
+  if (nb >= 0) {
+    const __half2* At = Ah + ((size_t(b) * 9 + d) * ns) * ns + j;
+    const float2* xv = x + size_t(nb) * ns;
+#pragma unroll 8
+    for (int i = 0; i < ns; i++) {
+      const float2 a = __half22float2(At[size_t(i) * ns]), v = __ldg(xv + i);
+      re += a.x * v.x - a.y * v.y; im += a.x * v.y + a.y * v.x;
+    }
+  }
+  part[d * 32 + j] = make_float2(re, im);
+  __syncthreads();
+  if (threadIdx.x < ns) {
+    float2 a = part[j];
+#pragma unroll
+    for (int k = 1; k < 8; k++) { a.x += part[k * 32 + j].x; a.y += part[k * 32 + j].y; }
+    t[j] = a;
+  }
+  __syncthreads();
+  if (threadIdx.x < ns) {
+    const __half2* Dt = Ah + ((size_t(b) * 9 + 8) * ns) * ns + j;
+    re = 0.f; im = 0.f;
+#pragma unroll 8
+    for (int i = 0; i < ns; i++) {
+      const float2 a = __half22float2(Dt[size_t(i) * ns]), v = t[i];
+      re += a.x * v.x - a.y * v.y; im += a.x * v.y + a.y * v.x;
+    }
+    float2 o = u ? u[size_t(b) * ns + j] : make_float2(0.f, 0.f);
+    o.x += sign * re; o.y += sign * im;
+    y[size_t(b) * ns + j] = o;
+    y[size_t(b ^ 1) * ns + j] = make_float2(0.f, 0.f);
+  }
+}
 // minimal-residual step of the coarse correction on the fine grid: alpha = <t, r> / <t, t> (device, dots = (Re, Im) of <t, r> and |t|^2);
 // t <- r - alpha t  (the residual the Schwarz smoother starts from),  z <- alpha z
 __global__ void __launch_bounds__(256) dfl_mr_step_k(size_t n4, const double* __restrict__ dots, const float4* __restrict__ r, float4* __restrict__ t, float4* __restrict__ z) {
@@ -227,8 +288,13 @@ int restrict_to_coarse(const Dfl& D, const float4* v, float2* out) {
   return QXD_OK;
 }
 
-// x = (approximately) A_c^{-1} b: nkc steps of unpreconditioned GCR on the coarse grid (z_k = current residual), every
-// coefficient on the device, one back substitution at the end; no host synchronisation.
+int eo_hop(const Dfl& D, int colour, float sign, const float2* x, const float2* u, float2* y) {
+  dfl_eo_hop_k<<<D.nb / 2, 8 * D.ns, 0, D.c->stream>>>(D.ns, colour, sign, static_cast<const __half2*>(D.c->dAh), D.c->dnbr, D.c->dcol, x, u, y);
+  QXD_LAUNCH_CHECK(D.c);
+  return QXD_OK;
+}
+// x = (approximately) A_c^{-1} b: nkc GCR steps on the even-odd (Schur) form of the coarse system (z_k = current residual),
+// every coefficient on the device, one back substitution at the end; no host synchronisation.
 int coarse_solve(const Dfl& D, const float2* b, float2* x) {
   qxd_ctx* c = D.c;
   double* S = c->dscal;
@@ -237,14 +303,15 @@ int coarse_solve(const Dfl& D, const float2* b, float2* x) {
   VecList Z, W;
   for (int k = 0; k < 32; k++) { Z.v[k] = static_cast<const float4*>(c->dcz[k]); W.v[k] = static_cast<const float4*>(c->dcw[k]); }
   float4* r = static_cast<float4*>(c->dcr);
-  QXD_CUDA_OK(c, cudaMemcpyAsync(r, b, D.nc4 * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));
+  float2* s = static_cast<float2*>(c->dcs);
+  float2* t = static_cast<float2*>(c->dct);
+  dfl_diag_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dDinv), b, s);   // s = Dinv b
+  QXD_LAUNCH_CHECK(c);
+  QXD_TRY(eo_hop(D, 0, -1.f, s, s, reinterpret_cast<float2*>(r)));                                   // r = s_e - Dinv_e H_eo s_o
   for (int k = 0; k < K; k++) {
-    dfl_diag_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dDinv), reinterpret_cast<const float2*>(r),
-                                                                      static_cast<float2*>(c->dcz[k]));   // z_k = block-Jacobi r
-    QXD_LAUNCH_CHECK(c);
-    dfl_coarse_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), c->dnbr,
-                                                                        static_cast<const float2*>(c->dcz[k]), static_cast<float2*>(c->dcw[k]));
-    QXD_LAUNCH_CHECK(c);
+    QXD_CUDA_OK(c, cudaMemcpyAsync(c->dcz[k], r, D.nc4 * sizeof(float4), cudaMemcpyDeviceToDevice, c->stream));   // z_k = r
+    QXD_TRY(eo_hop(D, 1, +1.f, static_cast<const float2*>(c->dcz[k]), nullptr, t));                                 // t_o = Dinv_o H_oe z_k
+    QXD_TRY(eo_hop(D, 0, -1.f, t, static_cast<const float2*>(c->dcz[k]), static_cast<float2*>(c->dcw[k])));         // w_k = z_k - Dinv_e H_eo t_o
     float4* wk = static_cast<float4*>(c->dcw[k]);
     for (int j0 = 0; j0 < k; j0 += 4) {
       const int nj = k - j0 < 4 ? k - j0 : 4;
@@ -271,7 +338,10 @@ int coarse_solve(const Dfl& D, const float2* b, float2* x) {
   }
   gcr_backsub_k<<<1, 32, 0, c->stream>>>(K, S);
   QXD_LAUNCH_CHECK(c);
-  gcr_update_x32_k<<<D.nblkc, 256, 0, c->stream>>>(D.nc4, Z, K, S + G_Y, reinterpret_cast<float4*>(x), 1);
+  gcr_update_x32_k<<<D.nblkc, 256, 0, c->stream>>>(D.nc4, Z, K, S + G_Y, reinterpret_cast<float4*>(x), 1);          // x_e
+  QXD_LAUNCH_CHECK(c);
+  QXD_TRY(eo_hop(D, 1, -1.f, x, s, t));                                                                // t_o = s_o - Dinv_o H_oe x_e
+  dfl_addsub_flat_k<<<D.nblkc, 256, 0, c->stream>>>(D.nc4, reinterpret_cast<const float4*>(x), reinterpret_cast<const float4*>(t), 1.f, reinterpret_cast<float4*>(x));
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
@@ -350,6 +420,15 @@ int orthonormalise_and_build(const Dfl& D, int prec) {
   QXD_TRY(launch_coarse_build(c, prec, D.ns, c->dphi, c->dAc, c->dnbr));
   dfl_diag_inverse_k<<<(D.nb + 63) / 64, 64, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), static_cast<float2*>(c->dDinv));
   QXD_LAUNCH_CHECK(c);
+  dfl_pack16_k<<<148 * 8, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), static_cast<const float2*>(c->dDinv), static_cast<__half2*>(c->dAh));
+  QXD_LAUNCH_CHECK(c);
+  std::vector<int> col(D.nb);
+  for (int b = 0; b < D.nb; b++) {
+    int blk;
+    QXD_TRY(qxd_sap_block_of(c, b * 128, 0, &blk, &col[b]));
+  }
+  QXD_CUDA_OK(c, cudaMemcpyAsync(c->dcol, col.data(), sizeof(int) * D.nb, cudaMemcpyHostToDevice, c->stream));
+  QXD_CUDA_OK(c, cudaStreamSynchronize(c->stream));   // col leaves scope
   return QXD_OK;
 }
 }  // namespace
@@ -401,6 +480,7 @@ int dfl_prolong(qxd_ctx* c, const void* coarse, void* fine) {
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
+int dfl_coarse_solve(qxd_ctx* c, const void* b, void* x) { const Dfl D = make_dfl(c); return coarse_solve(D, static_cast<const float2*>(b), static_cast<float2*>(x)); }
 int dfl_coarse_apply(qxd_ctx* c, const void* x, void* y) {
   const Dfl D = make_dfl(c);
   dfl_coarse_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), c->dnbr, static_cast<const float2*>(x),

@@ -88,6 +88,10 @@ struct qxd_ctx {
   void* dAc = nullptr;                           // coarse operator [nblocks][9][ns][ns] complex fp32
   int* dnbr = nullptr;                           // neighbour blocks [nblocks][8]
   void* dDinv = nullptr;                         // inverses of the diagonal coarse blocks [nblocks][ns][ns] (block-Jacobi preconditioner)
+  void* dAh = nullptr;                           // binary16 transposed copy for the even-odd coarse solver: [nblocks][9][ns][ns] half2, slot d < 8 = (A_c[1+d])^T, slot 8 = Dinv^T
+  int* dcol = nullptr;                           // colour (0 / 1) of every block
+  void* dcs = nullptr;                           // coarse scratch vectors of the even-odd solver
+  void* dct = nullptr;
   void* dcb = nullptr;                           // coarse vectors [nblocks][ns] complex fp32: right-hand side / scratch,
   void* dcx = nullptr;                           //   solution,
   void* dcr = nullptr;                           //   residual,
@@ -226,5 +230,6 @@ int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors);
 int dfl_restrict(qxd_ctx* c, const void* fine, void* coarse);
 int dfl_prolong(qxd_ctx* c, const void* coarse, void* fine);
 int dfl_coarse_apply(qxd_ctx* c, const void* x, void* y);
+int dfl_coarse_solve(qxd_ctx* c, const void* b, void* x);
 
 }  // namespace qxd

@@ -13,6 +13,7 @@ from .fields import (  # noqa: F401
     uniform01,
     normal,
     su3_links,
+    su3_links_smooth,
     u1_field,
     gaussian_spinor,
     random_su3,

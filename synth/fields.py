@@ -28,6 +28,7 @@ FIELD_U1 = 2
 FIELD_SPINOR = 3
 FIELD_GAUGE_TRAFO = 4
 FIELD_U1_TRAFO = 5
+FIELD_SU3_SMOOTH = 6
 
 
 def splitmix64(z):
@@ -150,6 +151,43 @@ def su3_links(dims, eps: float, seed: int = 1, chunk: int = 1 << 14):
         out[a:b] = _su3_from_counter(a, b - a, eps, seed, FIELD_SU3)
 
     _chunked(n, chunk, fill)
+    return out.reshape(T, L1, L2, L3, 4, 3, 3)
+
+
+def su3_links_smooth(dims, eps: float, seed: int = 1, corr: int = 4):
+    """SU(3) links whose generators vary smoothly over ``corr`` lattice spacings (periodic).
+
+    ``U_mu(x) = exp(i eps H_mu(x))`` with the eight real components of every ``H_mu`` drawn as unit
+    normals on the coarse lattice ``dims / corr`` and interpolated multilinearly in all four
+    directions.  The plain ``su3_links`` field is white noise at the lattice scale; this one
+    has the long-range order of a weakly coupled field, which is what deflation and multigrid
+    methods rely on ("local coherence" of the low modes).  Same layout as ``su3_links``.
+    """
+    T, L1, L2, L3 = dims
+    cd = tuple(d // corr for d in dims)
+    if any(c * corr != d or c < 1 for c, d in zip(cd, dims)):
+        raise ValueError("dims must be multiples of corr")
+    nc = int(np.prod(cd)) * 4
+    idx = (np.arange(nc, dtype=np.uint64)[None, :] * np.uint64(18) + np.arange(18, dtype=np.uint64)[:, None])
+    g = normal(seed, FIELD_SU3_SMOOTH, idx).reshape(18, *cd, 4)
+    for ax, d in enumerate(dims):                     # multilinear interpolation, one direction at a time
+        pos = np.arange(d) / corr
+        i0 = np.floor(pos).astype(np.int64) % cd[ax]
+        i1 = (i0 + 1) % cd[ax]
+        w = (pos - np.floor(pos)).reshape([-1 if k == ax + 1 else 1 for k in range(g.ndim)])
+        g = np.take(g, i0, axis=ax + 1) * (1.0 - w) + np.take(g, i1, axis=ax + 1) * w
+    n = T * L1 * L2 * L3 * 4
+    g = g.reshape(3, 3, 2, n)
+    G = g[:, :, 0] + 1j * g[:, :, 1]
+    H = 0.5 * (G + np.conj(np.swapaxes(G, 0, 1)))
+    tr = (H[0, 0] + H[1, 1] + H[2, 2]).real / 3.0
+    for i in range(3):
+        H[i, i] -= tr
+    out = np.empty((n, 3, 3), dtype=np.complex128)
+    chunk = 1 << 16
+    for a in range(0, n, chunk):
+        b = min(n, a + chunk)
+        out[a:b] = np.moveaxis(_reunitarise(_expm_i_herm(H[:, :, a:b], eps)), -1, 0)
     return out.reshape(T, L1, L2, L3, 4, 3, 3)
 
 
