@@ -342,6 +342,30 @@ int qxd_blas_axpy(qxd_ctx* ctx, int prec, double a, const void* x, void* y);
 int qxd_blas_cdot(qxd_ctx* ctx, int prec, const void* x, const void* y, double* re_im /*HOST [2]*/);
 int qxd_blas_norm2(qxd_ctx* ctx, int prec, const void* x, double* out /*HOST*/);
 
+/* ---- allocation-free entry point (noalloc.cu) -------------------------------------------------------------------------
+ * For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): the norm reduction of the solvers (row a6, the |r|^2 of every iteration: PAPER.md:45) on a flat array, with
+ * its per-CTA partial sums in a file-scope __device__ array of the library instead of the caller's workspace.  Needs no
+ * context and no workspace, and calls no cudaMalloc / cudaFree / allocating library routine.
+ *   qxd_norm2_noalloc      *out = sum_{k < nreals} x[k]^2, accumulated in fp64.  prec: QXD_F64 (x: const double*) or QXD_F32
+ *                          (x: const float*); QXD_F16 -> QXD_EINVAL.  x: DEVICE, nreals reals (any packed fp64 / fp32 spinor of
+ *                          this library is such an array: 24 Vh reals per half lattice); out: DEVICE, one double, written by
+ *                          the GPU in stream order (no host synchronisation); stream: a cudaStream_t, NULL = the default
+ *                          stream.  nreals = 0 gives 0 (x may then be NULL).  nreals > qxd_noalloc_max_reals() = 268 435 456 (65 536 partial sums
+ *                          of 4096 reals, 512 KB of static device memory per GPU that loads the library) -> QXD_EINVAL, with
+ *                          the limit in qxd_noalloc_last_error().  The result is independent of the launch configuration
+ *                          (fixed chunks, fixed order).  All calls on a device share the one scratch array, which keeps the
+ *                          last call's partial sums (none of them is read again: every call overwrites what it uses): calls
+ *                          in one stream are safe, calls that OVERLAP on the GPU (different streams, no ordering) race.
+ *   qxd_noalloc_init       set-up of the current device (looks up the device address of the scratch array); once per device,
+ *                          with that device current, outside any graph capture.  qxd_norm2_noalloc does it on its first call
+ *                          on a device if it was not done.
+ *   qxd_noalloc_last_error message of the last failure of these calls in this thread. */
+int qxd_noalloc_init(void);
+size_t qxd_noalloc_max_reals(void);
+const char* qxd_noalloc_last_error(void);
+int qxd_norm2_noalloc(int prec, const void* x /*DEVICE*/, size_t nreals, double* out /*DEVICE*/, void* stream);
+
 /* Number of kernel launches issued by this context so far (bench.py's gpu_launches). */
 long qxd_launch_count(const qxd_ctx* ctx);
 const char* qxd_last_error(const qxd_ctx* ctx);

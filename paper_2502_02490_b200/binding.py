@@ -95,6 +95,10 @@ SYMBOLS = {
     "qxd_face_scatter": (_i, [_vp, _i, _vp, _i, _i, _i, _i, _vp]),
     "qxd_halo_zero": (_i, [_vp, _i, _vp, _i, _i, _i, _i]),
     "qxd_blas_norm2_dev": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_noalloc_init": (_i, []),
+    "qxd_noalloc_max_reals": (_sz, []),
+    "qxd_noalloc_last_error": (C.c_char_p, []),
+    "qxd_norm2_noalloc": (_i, [_i, _vp, _sz, _vp, _vp]),
     "qxd_blas_cg_xr": (_i, [_vp, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "qxd_blas_cg_p": (_i, [_vp, _i, _vp, _vp, _vp, _vp]),
     "qxd_blas_copy": (_i, [_vp, _i, _vp, _vp]),
@@ -130,6 +134,35 @@ def load_library():
 
 def _ptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def noalloc_max_reals():
+    return int(load_library().qxd_noalloc_max_reals())
+
+
+def norm2_noalloc(x, out, stream=None):
+    """out[0] = sum of the squares of the reals of ``x`` (qxd_norm2_noalloc: no context, no workspace, no allocation; the
+    partial sums live in a static device array of the library).  x: contiguous CUDA tensor, float64 or float32 (complex
+    tensors count their real and imaginary parts); out: CUDA float64 tensor with at least one element, written in stream
+    order.  Calls that overlap on the GPU race on the shared scratch (include/qxd.h)."""
+    import torch
+    lib = load_library()
+    if not (x.is_cuda and out.is_cuda and x.is_contiguous() and out.dtype == torch.float64 and out.numel() >= 1):
+        raise QxdError(QXD_EINVAL, "norm2_noalloc: x and out must be contiguous CUDA tensors, out float64")
+    if x.is_complex():
+        x = torch.view_as_real(x)
+    if x.dtype == torch.float64:
+        prec = QXD_F64
+    elif x.dtype == torch.float32:
+        prec = QXD_F32
+    else:
+        raise QxdError(QXD_EINVAL, "norm2_noalloc: float64 or float32 data")
+    s = stream if stream is not None else torch.cuda.current_stream(x.device)
+    with torch.cuda.device(x.device):
+        rc = lib.qxd_norm2_noalloc(prec, _ptr(x), x.numel(), _ptr(out), C.c_void_p(s.cuda_stream))
+    if rc != QXD_OK:
+        raise QxdError(rc, lib.qxd_noalloc_last_error().decode())
+    return out
 
 
 class Qxd:
