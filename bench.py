@@ -765,7 +765,7 @@ def main():
     ap.add_argument("--dw-sweep", type=int, default=0, help="use the time-sweep D_w kernel with this segment length for the headline apply (0 = tile kernel)")
     ap.add_argument("--dfl-ns", type=int, default=24, help="null vectors of the deflated (two-level) GCR solve (0 = skip)")
     ap.add_argument("--dfl-ninv", type=int, default=8, help="M_sap smoothing passes per null vector in the deflation setup")
-    ap.add_argument("--dfl-nkc", type=int, default=24, help="GCR steps of every coarse-grid solve")
+    ap.add_argument("--dfl-nkc", type=int, default=12, help="GCR steps of every coarse-grid solve")
     ap.add_argument("--decomp", default="rhs", choices=["rhs", "domain"], help="rhs: shard by right-hand side (weak scaling, the default); "
                     "domain: cut the lattice along time over the ranks (strong scaling, row f2)")
     ap.add_argument("--no-overlap", action="store_true", help="--decomp domain: exchange the faces before the interior slabs instead of during them")
