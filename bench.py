@@ -607,6 +607,45 @@ def run_cuda(args, cfg):
                          "setup_seconds": t0.elapsed_time(t1) * 1e-3, "layout": "C*-paired" if pairing else "extended lattice",
                          "true_res_oracle": oracle_residual(eta, psi_d)})
             solves["dfl_gcr_sap_fp64_fp16"] = info
+            # ---- the regime the second level is for: the same lattice, couplings and U(1) field with SU(3)
+            # links that have long-range order (synth.su3_links_smooth), just below the critical hopping parameter
+            nck = args.nc_kappa if args.nc_kappa is not None else (0.1238 if cfg["name"] == "c3" else 0.0)
+            if nck > 0:
+                Us = synth_mod.su3_links_smooth(cfg["dims"], 0.7, 1, 4)
+                Ud = torch.from_numpy(Us).to(dev)
+                Ad = torch.from_numpy(A).to(dev) if A is not None else None
+                g.gauge_load(Ud, Ad, cfg["qel"])
+                g.set_quark(nck, cfg["q"])
+                g.clover_build(cfg["csw"], cfg["csw_qed"])
+                del Ud, Ad
+                g.set_gauge_reconstruct(B.QXD_RECON_12)
+                g.set_gauge_reconstruct(B.QXD_RECON_NONE, prec=B.QXD_F16)
+                oref2 = None
+                if want_oracle:
+                    from oracle import qxd_ref as R
+                    oref2 = R.Ref(*cfg["dims"], cfg["bc"])
+                    oref2.gauge_load(Us, A, cfg["qel"])
+                    oref2.set_quark(nck, cfg["q"])
+                    oref2.clover_build(cfg["csw"], cfg["csw_qed"])
+                nc = {"workload": f"{cfg['name']} geometry, couplings and U(1) field; SU(3) links = synth.su3_links_smooth(eps 0.7, every 4 sites); kappa {nck}",
+                      "tol": cfg["tol"], "maxiter": 3000}
+                t0 = ev(); t1 = ev()
+                t0.record()
+                g.deflation_setup(rnd, B.QXD_F16)
+                t1.record()
+                t1.synchronize()
+                for name, algo in (("cgne_fp64_fp16", B.QXD_CGNE), ("bicgstab_fp64_fp16", B.QXD_BICGSTAB), ("gcr_sap_fp64_fp16", B.QXD_GCR),
+                                   ("dfl_gcr_sap_fp64_fp16", B.QXD_DFL_GCR)):
+                    reps = 1 if algo == B.QXD_CGNE else 2          # CGNE runs into maxiter here (seconds): once is enough
+                    for _ in range(reps):
+                        _, info = g.solve(eta_d, cfg["tol"], algo=algo, sloppy=B.QXD_F16, maxiter=3000, psi=psi_d)
+                    if oref2 is not None and info["status"] == 0:
+                        r = eta.reshape(-1) - oref2.apply_Dw(psi_d.cpu().numpy()).reshape(-1)
+                        info["true_res_oracle"] = float(np.linalg.norm(r) / np.linalg.norm(eta.reshape(-1)))
+                    nc[name] = info
+                nc["dfl_gcr_sap_fp64_fp16"].update({"ns": dp[0], "ninv": dp[1], "nkc": dp[2], "setup_seconds": t0.elapsed_time(t1) * 1e-3})
+                solves["near_critical"] = nc
+                del oref2, Us
             del rnd
         del psi_d, pin, pout
 
@@ -766,6 +805,8 @@ def main():
     ap.add_argument("--dfl-ns", type=int, default=24, help="null vectors of the deflated (two-level) GCR solve (0 = skip)")
     ap.add_argument("--dfl-ninv", type=int, default=8, help="M_sap smoothing passes per null vector in the deflation setup")
     ap.add_argument("--dfl-nkc", type=int, default=12, help="GCR steps of every coarse-grid solve")
+    ap.add_argument("--nc-kappa", type=float, default=None,
+                    help="hopping parameter of the near-critical solver comparison on smooth links (default: 0.1238 at c3, skipped elsewhere; 0 = skip)")
     ap.add_argument("--decomp", default="rhs", choices=["rhs", "domain"], help="rhs: shard by right-hand side (weak scaling, the default); "
                     "domain: cut the lattice along time over the ranks (strong scaling, row f2)")
     ap.add_argument("--no-overlap", action="store_true", help="--decomp domain: exchange the faces before the interior slabs instead of during them")
