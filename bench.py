@@ -551,8 +551,8 @@ def run_cuda(args, cfg):
         # the Krylov space and the deflation space are part of the workspace: take the largest number of null vectors that
         # leaves room for the test vectors of the setup (the largest lattices run with fewer, or without the second level)
         g = None
-        for ns_try in ([dp[0], 16, 8] if dp else []) + [0]:
-            dtry = (ns_try, dp[1], dp[2]) if (dp and ns_try > 0) else None
+        for ns_try in ([n for n in (dp[0], 16, 8) if n <= dp[0]] if dp else []) + [0]:
+            dtry = (ns_try, dp[1], dp[2], 0, args.dfl_chiral) if (dp and ns_try > 0) else None
             try:
                 g = B.Qxd(*cfg["dims"], cfg["bc"], precisions=precs, nrhs=1, device=f"cuda:{local}", pairing=(True if pairing else None), gcr=gp, deflation=dtry)
                 free = torch.cuda.mem_get_info(dev)[0]
@@ -565,7 +565,7 @@ def run_cuda(args, cfg):
             except torch.OutOfMemoryError:
                 g = None
                 torch.cuda.empty_cache()
-        if dp is not None and dtry != dp:
+        if dp is not None and (dtry is None or dtry[0] != dp[0]):
             solves["dfl_gcr_sap_fp64_fp16_note"] = f"device memory: {dp[0]} null vectors requested, {ns_try} used"
         dp = dtry
         Ud = torch.from_numpy(U).to(dev)
@@ -603,7 +603,7 @@ def run_cuda(args, cfg):
             t1.synchronize()
             g.solve(eta_d, cfg["tol"], algo=B.QXD_DFL_GCR, sloppy=B.QXD_F16, maxiter=args.maxiter, psi=psi_d)
             _, info = g.solve(eta_d, cfg["tol"], algo=B.QXD_DFL_GCR, sloppy=B.QXD_F16, maxiter=args.maxiter, psi=psi_d)
-            info.update({"tol": cfg["tol"], "nkv": gp[0], "ncy": gp[1], "nmr": gp[2], "ns": dp[0], "ninv": dp[1], "nkc": dp[2],
+            info.update({"tol": cfg["tol"], "nkv": gp[0], "ncy": gp[1], "nmr": gp[2], "ns": dp[0], "ninv": dp[1], "nkc": dp[2], "chirality_split": dp[4],
                          "setup_seconds": t0.elapsed_time(t1) * 1e-3, "layout": "C*-paired" if pairing else "extended lattice",
                          "true_res_oracle": oracle_residual(eta, psi_d)})
             solves["dfl_gcr_sap_fp64_fp16"] = info
@@ -643,7 +643,7 @@ def run_cuda(args, cfg):
                         r = eta.reshape(-1) - oref2.apply_Dw(psi_d.cpu().numpy()).reshape(-1)
                         info["true_res_oracle"] = float(np.linalg.norm(r) / np.linalg.norm(eta.reshape(-1)))
                     nc[name] = info
-                nc["dfl_gcr_sap_fp64_fp16"].update({"ns": dp[0], "ninv": dp[1], "nkc": dp[2], "setup_seconds": t0.elapsed_time(t1) * 1e-3})
+                nc["dfl_gcr_sap_fp64_fp16"].update({"ns": dp[0], "ninv": dp[1], "nkc": dp[2], "chirality_split": dp[4], "setup_seconds": t0.elapsed_time(t1) * 1e-3})
                 solves["near_critical"] = nc
                 del oref2, Us
             del rnd
@@ -802,7 +802,8 @@ def main():
     ap.add_argument("--gcr-ncy", type=int, default=4, help="SAP cycles per preconditioner application")
     ap.add_argument("--gcr-nmr", type=int, default=5, help="minimal-residual steps per SAP block solve")
     ap.add_argument("--dw-sweep", type=int, default=0, help="use the time-sweep D_w kernel with this segment length for the headline apply (0 = tile kernel)")
-    ap.add_argument("--dfl-ns", type=int, default=24, help="null vectors of the deflated (two-level) GCR solve (0 = skip)")
+    ap.add_argument("--dfl-ns", type=int, default=16, help="null vectors of the deflated (two-level) GCR solve (0 = skip)")
+    ap.add_argument("--dfl-chiral", type=int, default=1, help="1: null vectors split by chirality (2 ns coarse degrees of freedom per block; ns <= 16)")
     ap.add_argument("--dfl-ninv", type=int, default=8, help="M_sap smoothing passes per null vector in the deflation setup")
     ap.add_argument("--dfl-nkc", type=int, default=12, help="GCR steps of every coarse-grid solve")
     ap.add_argument("--nc-kappa", type=float, default=None,

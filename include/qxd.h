@@ -211,6 +211,12 @@ int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
  *                        every coarse-grid solve (0 = default 16), nref rounds of adaptive refinement in the setup (every null
  *                        vector replaced by the current two-level preconditioner applied to it, space and coarse operator rebuilt;
  *                        needs ns <= 2 nkv); before qxd_workspace_bind; needs qxd_set_gcr too.
+ *   qxd_set_deflation_chirality   on = 1: every null vector is split into its two chirality components (upper / lower two spin
+ *                        components in the chiral basis of reading R3), the aggregation of the multigrid solvers the paper's GPU runs
+ *                        use: the deflation space is span{P_b P_chi phi_i}, 2 ns complex dimensions per block for ns smoothed
+ *                        vectors (ns <= 16), and gamma5 maps it onto itself.  Before qxd_workspace_bind.  Default 0.  With the split
+ *                        qxd_deflation_info reports 2 ns and the coarse vectors of qxd_deflation_op are [nblocks][2 ns], index
+ *                        2 i + chi.
  *   qxd_deflation_setup  random_vectors: DEVICE, ns packed fp32 full-lattice spinors back to back (the caller draws them; any
  *                        linearly independent set works).  Each is smoothed by ninv applications of M_sap (block operator in storage
  *                        precision prec = QXD_F32 / QXD_F16), the set is orthonormalised block by block, and the coarse operator
@@ -228,6 +234,7 @@ int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
  *                        coarse_in (~ A_c^{-1} coarse_in).  fine: DEVICE packed fp32 full-lattice spinor; coarse: DEVICE [nblocks][ns]
  *                        complex fp32 (block index = checkerboard index >> 7). */
 int qxd_set_deflation(qxd_ctx* ctx, int ns, int ninv, int nkc, int nref);
+int qxd_set_deflation_chirality(qxd_ctx* ctx, int on);
 int qxd_deflation_setup(qxd_ctx* ctx, int prec, const void* random_vectors /*DEVICE*/);
 int qxd_deflation_info(const qxd_ctx* ctx, int* nblocks, int* ns, int* ready);
 int qxd_deflation_op(qxd_ctx* ctx, int op, const void* in, void* out);

@@ -69,6 +69,7 @@ SYMBOLS = {
     "qxd_set_gcr": (_i, [_vp, _i, _i, _i]),
     "qxd_apply_sap": (_i, [_vp, _i, _vp, _vp]),
     "qxd_set_deflation": (_i, [_vp, _i, _i, _i, _i]),
+    "qxd_set_deflation_chirality": (_i, [_vp, _i]),
     "qxd_deflation_setup": (_i, [_vp, _i, _vp]),
     "qxd_deflation_info": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)]),
     "qxd_deflation_op": (_i, [_vp, _i, _vp, _vp]),
@@ -194,8 +195,10 @@ class Qxd:
         if gcr is not None:                     # (nkv, ncy, nmr): Krylov space and SAP parameters of QXD_GCR (row f3)
             self._chk(self.lib.qxd_set_gcr(self.h, *gcr))
         if deflation is not None:               # (ns, ninv, nkc[, nref]): null vectors, setup smoothing passes, coarse GCR steps, refinement rounds
-            d = tuple(deflation) + (0,) * (4 - len(deflation))
-            self._chk(self.lib.qxd_set_deflation(self.h, *d))
+            d = tuple(deflation) + (0,) * (5 - len(deflation))       # fifth entry: 1 = split the null vectors by chirality
+            if d[4]:
+                self._chk(self.lib.qxd_set_deflation_chirality(self.h, 1))
+            self._chk(self.lib.qxd_set_deflation(self.h, *d[:4]))
         self.prec_mask = 0
         for p in precisions:
             self.prec_mask |= 1 << p

@@ -101,12 +101,13 @@ size_t carve(qxd_ctx* c, char* base, int prec_mask, int nrhs, bool assign) {
   void* d_t1 = nullptr; void* d_t2 = nullptr; void* dAc = nullptr; void* dnbr = nullptr; void* dcb = nullptr; void* dcx = nullptr; void* dcr = nullptr;
   void* dscal = nullptr; void* dDinv = nullptr; void* dAh = nullptr; void* dcol = nullptr; void* dcs = nullptr; void* dct = nullptr;
   if (c->dfl_ns > 0) {
-    const size_t f32 = 2 * half_bytes(1, Vh), nb = Vh / 128 > 0 ? Vh / 128 : 1, cv = nb * c->dfl_ns * 8;
+    const size_t ncd = size_t(c->dfl_ns) * (c->dfl_chiral ? 2 : 1);   // coarse dimension per block
+    const size_t f32 = 2 * half_bytes(1, Vh), nb = Vh / 128 > 0 ? Vh / 128 : 1, cv = nb * ncd * 8;
     for (int i = 0; i < c->dfl_ns; i++) dphi[i] = k.take(f32);
     d_t1 = k.take(f32); d_t2 = k.take(f32);
-    dAc = k.take(nb * 9 * c->dfl_ns * c->dfl_ns * 8); dnbr = k.take(nb * 8 * 4); dDinv = k.take(nb * c->dfl_ns * c->dfl_ns * 8);
+    dAc = k.take(nb * 9 * ncd * ncd * 8); dnbr = k.take(nb * 8 * 4); dDinv = k.take(nb * ncd * ncd * 8);
     dcb = k.take(cv); dcx = k.take(cv); dcr = k.take(cv); dcs = k.take(cv); dct = k.take(cv);
-    dAh = k.take(nb * 9 * c->dfl_ns * c->dfl_ns * 4); dcol = k.take(nb * 4);
+    dAh = k.take(nb * 9 * ncd * ncd * 4); dcol = k.take(nb * 4);
     for (int i = 0; i < c->dfl_nkc; i++) { dcz[i] = k.take(cv); dcw[i] = k.take(cv); }
     dscal = k.take(4096 * 8);
   }
@@ -684,7 +685,16 @@ int qxd_set_deflation(qxd_ctx* c, int ns, int ninv, int nkc, int nref) {
   if (!c) return QXD_EINVAL;
   if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_deflation must precede qxd_workspace_bind");
   if (ns < 0 || ns > 32 || (ns & 1) || ninv < 0 || nkc < 0 || nkc > 32 || nref < 0) return fail(c, QXD_EINVAL, "set_deflation: ns even in 0..32, ninv >= 0, 0 <= nkc <= 32, nref >= 0");
+  if (c->dfl_chiral && ns > 16) return fail(c, QXD_EINVAL, "set_deflation: at most 16 null vectors with the chirality split");
   c->dfl_ns = ns; c->dfl_ninv = ninv > 0 ? ninv : 4; c->dfl_nkc = nkc > 0 ? nkc : 16; c->dfl_nref = nref;
+  return QXD_OK;
+}
+int qxd_set_deflation_chirality(qxd_ctx* c, int on) {
+  if (!c) return QXD_EINVAL;
+  if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_deflation_chirality must precede qxd_workspace_bind");
+  if (on != 0 && on != 1) return fail(c, QXD_EINVAL, "set_deflation_chirality: 0 or 1");
+  if (on && c->dfl_ns > 16) return fail(c, QXD_EINVAL, "set_deflation_chirality: at most 16 null vectors (32 coarse degrees of freedom per block)");
+  c->dfl_chiral = on;
   return QXD_OK;
 }
 int qxd_deflation_setup(qxd_ctx* c, int prec, const void* random_vectors) {
@@ -697,7 +707,7 @@ int qxd_deflation_setup(qxd_ctx* c, int prec, const void* random_vectors) {
 }
 int qxd_deflation_info(const qxd_ctx* c, int* nblocks, int* ns, int* ready) {
   if (!c || !nblocks || !ns || !ready) return QXD_EINVAL;
-  *nblocks = c->g.Vh / 128; *ns = c->dfl_ns; *ready = c->dfl_ready ? 1 : 0;
+  *nblocks = c->g.Vh / 128; *ns = c->dfl_ns * (c->dfl_chiral ? 2 : 1); *ready = c->dfl_ready ? 1 : 0;
   return QXD_OK;
 }
 int qxd_deflation_op(qxd_ctx* c, int op, const void* in, void* out) {

@@ -32,46 +32,58 @@ struct PhiList {
 // float4 index of chunk c of the thread's site (block b = blockIdx.x, 256 threads = 128 checkerboard indices x 2 parities)
 __device__ __forceinline__ size_t own_index(int Vh) { return size_t(threadIdx.x >> 7) * 6 * Vh + size_t(blockIdx.x) * 128 + (threadIdx.x & 127); }
 
-// out[b * ldo + j0 + j] = sum_{x in b} conj(u_{j0+j}(x)) . v(x),  j < NJ   (restriction, Gram-Schmidt coefficients, block norms)
+// out[b * ldo + j0 + j] = sum_{x in b} conj(u_{j0+j}(x)) . v(x),  j < NJ   (restriction, Gram-Schmidt coefficients, block norms).
+// ch = 1 (chirality split): the sums over the upper (reals 0..11) and the lower (12..23) spin components are kept apart,
+// out[b * ldo + 2 (j0 + j) + chi].
 template <int NJ>
-__global__ void __launch_bounds__(256) dfl_block_dots_k(int Vh, PhiList U, int j0, const float4* __restrict__ v, float2* __restrict__ out, int ldo) {
-  __shared__ float red[8][2 * NJ];
+__global__ void __launch_bounds__(256) dfl_block_dots_k(int Vh, PhiList U, int j0, const float4* __restrict__ v, float2* __restrict__ out, int ldo, int ch) {
+  __shared__ float red[8][4 * NJ];
   const size_t own = own_index(Vh);
-  float y[24], part[2 * NJ];
+  float y[24], part[4 * NJ];
 #pragma unroll
   for (int c = 0; c < 6; c++) { const float4 t = __ldg(v + own + size_t(c) * Vh); y[4 * c] = t.x; y[4 * c + 1] = t.y; y[4 * c + 2] = t.z; y[4 * c + 3] = t.w; }
 #pragma unroll
   for (int j = 0; j < NJ; j++) {
-    float re = 0.f, im = 0.f;
+    float re[2] = {0.f, 0.f}, im[2] = {0.f, 0.f};
 #pragma unroll
     for (int c = 0; c < 6; c++) {
       const float4 u = __ldg(U.v[j0 + j] + own + size_t(c) * Vh);
-      re += u.x * y[4 * c]; re += u.y * y[4 * c + 1]; re += u.z * y[4 * c + 2]; re += u.w * y[4 * c + 3];
-      im += u.x * y[4 * c + 1]; im -= u.y * y[4 * c]; im += u.z * y[4 * c + 3]; im -= u.w * y[4 * c + 2];
+      const int h = c / 3;
+      re[h] += u.x * y[4 * c]; re[h] += u.y * y[4 * c + 1]; re[h] += u.z * y[4 * c + 2]; re[h] += u.w * y[4 * c + 3];
+      im[h] += u.x * y[4 * c + 1]; im[h] -= u.y * y[4 * c]; im[h] += u.z * y[4 * c + 3]; im[h] -= u.w * y[4 * c + 2];
     }
-    part[2 * j] = re; part[2 * j + 1] = im;
+    part[4 * j] = re[0]; part[4 * j + 1] = im[0]; part[4 * j + 2] = re[1]; part[4 * j + 3] = im[1];
   }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
-  for (int k = 0; k < 2 * NJ; k++) {
+  for (int k = 0; k < 4 * NJ; k++) {
     float t = part[k];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
     if (lane == 0) red[warp][k] = t;
   }
   __syncthreads();
-  if (threadIdx.x < 2 * NJ) {
+  if (ch) {
+    if (threadIdx.x < 4 * NJ) {
+      float t = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; w++) t += red[w][threadIdx.x];
+      reinterpret_cast<float*>(out + size_t(blockIdx.x) * ldo + 2 * j0)[threadIdx.x] = t;
+    }
+  } else if (threadIdx.x < 2 * NJ) {
+    const int k = 4 * (threadIdx.x >> 1) + (threadIdx.x & 1);
     float t = 0.f;
 #pragma unroll
-    for (int w = 0; w < 8; w++) t += red[w][threadIdx.x];
+    for (int w = 0; w < 8; w++) t += red[w][k] + red[w][k + 2];
     reinterpret_cast<float*>(out + size_t(blockIdx.x) * ldo + j0)[threadIdx.x] = t;
   }
 }
 // v(x) = beta v(x) + sign sum_{j<n} c[b * ldc + j] u_j(x)      (Gram-Schmidt update: beta 1, sign -1; prolongation: beta 0, sign +1)
+// ch = 1: the upper spin components take c[b * ldc + 2 j], the lower ones c[b * ldc + 2 j + 1]  (n <= 16)
 __global__ void __launch_bounds__(256) dfl_block_axpy_k(int Vh, PhiList U, int n, const float2* __restrict__ coef, int ldc, float beta, float sign,
-                                                        float4* __restrict__ v) {
+                                                        float4* __restrict__ v, int ch) {
   __shared__ float2 cs[32];
-  if (threadIdx.x < n) { const float2 t = coef[size_t(blockIdx.x) * ldc + threadIdx.x]; cs[threadIdx.x] = make_float2(sign * t.x, sign * t.y); }
+  if (threadIdx.x < (ch ? 2 * n : n)) { const float2 t = coef[size_t(blockIdx.x) * ldc + threadIdx.x]; cs[threadIdx.x] = make_float2(sign * t.x, sign * t.y); }
   __syncthreads();
   const size_t own = own_index(Vh);
   float4 y[6];
@@ -81,9 +93,10 @@ __global__ void __launch_bounds__(256) dfl_block_axpy_k(int Vh, PhiList U, int n
     if (beta != 0.f && beta != 1.f) { y[c].x *= beta; y[c].y *= beta; y[c].z *= beta; y[c].w *= beta; }
   }
   for (int j = 0; j < n; j++) {
-    const float ar = cs[j].x, ai = cs[j].y;
+    const float2 cu = ch ? cs[2 * j] : cs[j], cl = ch ? cs[2 * j + 1] : cs[j];
 #pragma unroll
     for (int c = 0; c < 6; c++) {
+      const float ar = c < 3 ? cu.x : cl.x, ai = c < 3 ? cu.y : cl.y;
       const float4 u = __ldg(U.v[j] + own + size_t(c) * Vh);
       y[c].x += ar * u.x - ai * u.y; y[c].y += ar * u.y + ai * u.x;
       y[c].z += ar * u.z - ai * u.w; y[c].w += ar * u.w + ai * u.z;
@@ -92,13 +105,13 @@ __global__ void __launch_bounds__(256) dfl_block_axpy_k(int Vh, PhiList U, int n
 #pragma unroll
   for (int c = 0; c < 6; c++) v[own + size_t(c) * Vh] = y[c];
 }
-// v(x) /= sqrt(n2[b].x)  (block-wise normalisation; a vanishing block is left as it is)
-__global__ void __launch_bounds__(256) dfl_block_scale_k(int Vh, const float2* __restrict__ n2, int ld, float4* __restrict__ v) {
-  const float d = n2[size_t(blockIdx.x) * ld].x;
-  const float s = d > 0.f ? rsqrtf(d) : 1.f;
+// v(x) /= sqrt(n2[b].x)  (block-wise normalisation; a vanishing block is left as it is); ch = 1: n2[b] and n2[b + 1] for the two chiralities
+__global__ void __launch_bounds__(256) dfl_block_scale_k(int Vh, const float2* __restrict__ n2, int ld, float4* __restrict__ v, int ch) {
+  const float du = n2[size_t(blockIdx.x) * ld].x, dl = ch ? n2[size_t(blockIdx.x) * ld + 1].x : du;
+  const float su = du > 0.f ? rsqrtf(du) : 1.f, sl = dl > 0.f ? rsqrtf(dl) : 1.f;
   const size_t own = own_index(Vh);
 #pragma unroll
-  for (int c = 0; c < 6; c++) { float4 t = v[own + size_t(c) * Vh]; t.x *= s; t.y *= s; t.z *= s; t.w *= s; v[own + size_t(c) * Vh] = t; }
+  for (int c = 0; c < 6; c++) { const float sc = c < 3 ? su : sl; float4 t = v[own + size_t(c) * Vh]; t.x *= sc; t.y *= sc; t.z *= sc; t.w *= sc; v[own + size_t(c) * Vh] = t; }
 }
 // flat helpers on packed full-lattice fp32 vectors
 __global__ void __launch_bounds__(256) dfl_scale_flat_k(size_t n4, const double* __restrict__ n2, float4* __restrict__ v) {
@@ -261,7 +274,7 @@ __global__ void __launch_bounds__(256) dfl_mr_dots_k(size_t n4, const float4* __
 
 struct Dfl {
   qxd_ctx* c;
-  int Vh, nb, ns;
+  int Vh, nb, ns, nc, ch;   // ns null vectors; nc = coarse degrees of freedom per block (2 ns with the chirality split)
   size_t n4, nc4;     // float4 per fine / coarse vector
   int nblk, nblkc;
   PhiList phi() const { PhiList P; for (int i = 0; i < 32; i++) P.v[i] = static_cast<const float4*>(c->dphi[i]); return P; }
@@ -269,8 +282,8 @@ struct Dfl {
 };
 Dfl make_dfl(qxd_ctx* c) {
   Dfl D;
-  D.c = c; D.Vh = c->g.Vh; D.nb = c->g.Vh / 128; D.ns = c->dfl_ns;
-  D.n4 = size_t(12) * D.Vh; D.nc4 = size_t(D.nb) * D.ns / 2;
+  D.c = c; D.Vh = c->g.Vh; D.nb = c->g.Vh / 128; D.ns = c->dfl_ns; D.ch = c->dfl_chiral ? 1 : 0; D.nc = D.ns * (1 + D.ch);
+  D.n4 = size_t(12) * D.Vh; D.nc4 = size_t(D.nb) * D.nc / 2;
   D.nblk = D.Vh / 128 < 1 ? 1 : (D.Vh / 128 > 148 * 8 ? 148 * 8 : D.Vh / 128);
   D.nblkc = int((D.nc4 + 255) / 256); if (D.nblkc > D.nblk) D.nblkc = D.nblk; if (D.nblkc < 1) D.nblkc = 1;
   return D;
@@ -279,17 +292,17 @@ Dfl make_dfl(qxd_ctx* c) {
 int restrict_to_coarse(const Dfl& D, const float4* v, float2* out) {
   for (int j0 = 0; j0 < D.ns; j0 += 4) {
     const int nj = D.ns - j0 < 4 ? D.ns - j0 : 4;
-    if (nj == 4) dfl_block_dots_k<4><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
-    else if (nj == 3) dfl_block_dots_k<3><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
-    else if (nj == 2) dfl_block_dots_k<2><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
-    else dfl_block_dots_k<1><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.ns);
+    if (nj == 4) dfl_block_dots_k<4><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.nc, D.ch);
+    else if (nj == 3) dfl_block_dots_k<3><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.nc, D.ch);
+    else if (nj == 2) dfl_block_dots_k<2><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.nc, D.ch);
+    else dfl_block_dots_k<1><<<D.nb, 256, 0, D.c->stream>>>(D.Vh, D.phi(), j0, v, out, D.nc, D.ch);
     QXD_LAUNCH_CHECK(D.c);
   }
   return QXD_OK;
 }
 
 int eo_hop(const Dfl& D, int colour, float sign, const float2* x, const float2* u, float2* y) {
-  dfl_eo_hop_k<<<D.nb / 2, 8 * D.ns, 0, D.c->stream>>>(D.ns, colour, sign, static_cast<const __half2*>(D.c->dAh), D.c->dnbr, D.c->dcol, x, u, y);
+  dfl_eo_hop_k<<<D.nb / 2, 8 * D.nc, 0, D.c->stream>>>(D.nc, colour, sign, static_cast<const __half2*>(D.c->dAh), D.c->dnbr, D.c->dcol, x, u, y);
   QXD_LAUNCH_CHECK(D.c);
   return QXD_OK;
 }
@@ -305,7 +318,7 @@ int coarse_solve(const Dfl& D, const float2* b, float2* x) {
   float4* r = static_cast<float4*>(c->dcr);
   float2* s = static_cast<float2*>(c->dcs);
   float2* t = static_cast<float2*>(c->dct);
-  dfl_diag_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dDinv), b, s);   // s = Dinv b
+  dfl_diag_apply_k<<<(D.nb * D.nc + 255) / 256, 256, 0, c->stream>>>(D.nb, D.nc, static_cast<const float2*>(c->dDinv), b, s);   // s = Dinv b
   QXD_LAUNCH_CHECK(c);
   QXD_TRY(eo_hop(D, 0, -1.f, s, s, reinterpret_cast<float2*>(r)));                                   // r = s_e - Dinv_e H_eo s_o
   for (int k = 0; k < K; k++) {
@@ -368,7 +381,7 @@ int launch_dfl_precond(qxd_ctx* c, int prec, const void* r, void* z) {
   float4* t2 = static_cast<float4*>(c->d_t2);
   QXD_TRY(restrict_to_coarse(D, static_cast<const float4*>(r), cr));
   QXD_TRY(coarse_solve(D, cr, cx));
-  dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), D.ns, cx, D.ns, 0.f, 1.f, z0);            // z0 = P cx
+  dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), D.ns, cx, D.nc, 0.f, 1.f, z0, D.ch);            // z0 = P cx
   QXD_LAUNCH_CHECK(c);
   QXD_TRY(apply_Dw32(c, z0, t1));                                                                            // t1 = D_w z0
   dfl_addsub_flat_k<<<D.nblk, 256, 0, c->stream>>>(D.n4, static_cast<const float4*>(r), t1, -1.f, t1);      // t1 = r - D_w z0
@@ -402,25 +415,25 @@ int orthonormalise_and_build(const Dfl& D, int prec) {
     for (int pass = 0; pass < 2 && i > 0; pass++) {
       for (int j0 = 0; j0 < i; j0 += 4) {
         const int nj = i - j0 < 4 ? i - j0 : 4;
-        if (nj == 4) dfl_block_dots_k<4><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
-        else if (nj == 3) dfl_block_dots_k<3><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
-        else if (nj == 2) dfl_block_dots_k<2><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
-        else dfl_block_dots_k<1><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.ns);
+        if (nj == 4) dfl_block_dots_k<4><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.nc, D.ch);
+        else if (nj == 3) dfl_block_dots_k<3><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.nc, D.ch);
+        else if (nj == 2) dfl_block_dots_k<2><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.nc, D.ch);
+        else dfl_block_dots_k<1><<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), j0, v, coef, D.nc, D.ch);
         QXD_LAUNCH_CHECK(c);
       }
-      dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), i, coef, D.ns, 1.f, -1.f, v);
+      dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), i, coef, D.nc, 1.f, -1.f, v, D.ch);
       QXD_LAUNCH_CHECK(c);
     }
     PhiList self; for (int k = 0; k < 32; k++) self.v[k] = v;
-    dfl_block_dots_k<1><<<D.nb, 256, 0, c->stream>>>(D.Vh, self, 0, v, coef, D.ns);
+    dfl_block_dots_k<1><<<D.nb, 256, 0, c->stream>>>(D.Vh, self, 0, v, coef, D.nc, D.ch);
     QXD_LAUNCH_CHECK(c);
-    dfl_block_scale_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, coef, D.ns, v);     // coef[b * ns].x = |v|_b^2 (ldo = ns, j0 = 0)
+    dfl_block_scale_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, coef, D.nc, v, D.ch);     // coef[b * nc (+ 1)].x = |v|_b^2 (per chirality)
     QXD_LAUNCH_CHECK(c);
   }
   QXD_TRY(launch_coarse_build(c, prec, D.ns, c->dphi, c->dAc, c->dnbr));
-  dfl_diag_inverse_k<<<(D.nb + 63) / 64, 64, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), static_cast<float2*>(c->dDinv));
+  dfl_diag_inverse_k<<<(D.nb + 63) / 64, 64, 0, c->stream>>>(D.nb, D.nc, static_cast<const float2*>(c->dAc), static_cast<float2*>(c->dDinv));
   QXD_LAUNCH_CHECK(c);
-  dfl_pack16_k<<<148 * 8, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), static_cast<const float2*>(c->dDinv), static_cast<__half2*>(c->dAh));
+  dfl_pack16_k<<<148 * 8, 256, 0, c->stream>>>(D.nb, D.nc, static_cast<const float2*>(c->dAc), static_cast<const float2*>(c->dDinv), static_cast<__half2*>(c->dAh));
   QXD_LAUNCH_CHECK(c);
   std::vector<int> col(D.nb);
   for (int b = 0; b < D.nb; b++) {
@@ -476,14 +489,14 @@ int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors) {
 int dfl_restrict(qxd_ctx* c, const void* fine, void* coarse) { const Dfl D = make_dfl(c); return restrict_to_coarse(D, static_cast<const float4*>(fine), static_cast<float2*>(coarse)); }
 int dfl_prolong(qxd_ctx* c, const void* coarse, void* fine) {
   const Dfl D = make_dfl(c);
-  dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), D.ns, static_cast<const float2*>(coarse), D.ns, 0.f, 1.f, static_cast<float4*>(fine));
+  dfl_block_axpy_k<<<D.nb, 256, 0, c->stream>>>(D.Vh, D.phi(), D.ns, static_cast<const float2*>(coarse), D.nc, 0.f, 1.f, static_cast<float4*>(fine), D.ch);
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;
 }
 int dfl_coarse_solve(qxd_ctx* c, const void* b, void* x) { const Dfl D = make_dfl(c); return coarse_solve(D, static_cast<const float2*>(b), static_cast<float2*>(x)); }
 int dfl_coarse_apply(qxd_ctx* c, const void* x, void* y) {
   const Dfl D = make_dfl(c);
-  dfl_coarse_apply_k<<<(D.nb * D.ns + 255) / 256, 256, 0, c->stream>>>(D.nb, D.ns, static_cast<const float2*>(c->dAc), c->dnbr, static_cast<const float2*>(x),
+  dfl_coarse_apply_k<<<(D.nb * D.nc + 255) / 256, 256, 0, c->stream>>>(D.nb, D.nc, static_cast<const float2*>(c->dAc), c->dnbr, static_cast<const float2*>(x),
                                                                       static_cast<float2*>(y));
   QXD_LAUNCH_CHECK(c);
   return QXD_OK;

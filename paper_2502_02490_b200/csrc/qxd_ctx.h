@@ -81,6 +81,7 @@ struct qxd_ctx {
   double* gscal = nullptr;                       // device scalars of the GCR cycle: coefficient matrix b[32][32] (complex), c[32], y[32], norms
   // two-level (deflated) preconditioner of the GCR (dfl.cu): null vectors, coarse operator, coarse-grid vectors
   int dfl_ns = 0, dfl_ninv = 4, dfl_nkc = 16, dfl_nref = 0, dfl_prec = 1;
+  int dfl_chiral = 0;                            // 1: null vectors split by chirality, coarse dimension per block = 2 ns (qxd_set_deflation_chirality)
   bool dfl_ready = false;
   void* dphi[32] = {};                           // fp32 packed full-lattice null vectors, block-orthonormal
   void* d_t1 = nullptr;                          // fp32 fine-grid temporaries

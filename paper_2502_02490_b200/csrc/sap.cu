@@ -85,13 +85,17 @@ __device__ __forceinline__ void hop_sm(const unsigned (&nbc)[2], int par, int l,
 // hop across the block boundary, from the stored corrections in global memory (prologue)
 template <typename S, int MU, int DIR, int NL, bool PAIR>
 __device__ __forceinline__ void hop_bnd(const SapArgs& a, const float4* __restrict__ nsrc, const Site& s, int tile, int par, int l,
-                                        const typename PT<S>::V* Wsm, float* acc) {
+                                        const typename PT<S>::V* Wsm, float* acc, int chmask = 0 /* 1 / 2: upper / lower chirality of the source only */) {
   const int nb = neighbour_cb<MU, DIR, PAIR ? 1 : 0>(a.g, s);
   if ((nb >> 7) == tile) return;
   const int Vh = a.g.Vh;
   float psi[24], w[18], h[12], t[12];
 #pragma unroll
   for (int c = 0; c < 6; c++) unpack4(__ldg(nsrc + size_t(c) * Vh + nb), psi + 4 * c);
+  if (chmask) {
+#pragma unroll
+    for (int k = 0; k < 12; k++) psi[(chmask == 1 ? 12 : 0) + k] = 0.f;
+  }
   if (DIR > 0) lds_reals<S, 18 * MU, 18>(Wsm + par * SapShape<S>::NCH * 128, l, w);
   else {   // W_mu(x - mu): the forward link of the neighbour, from its global record
     int wi = nb;
@@ -309,12 +313,13 @@ int sap_launch_t(qxd_ctx* c, const SapArgs& a, int nblocks) {
 struct CoarseArgs {
   SapArgs a;
   const float4* phi[32];   // null vectors: fp32 packed full lattice (parity 1 at +6 Vh float4)
-  int ns;
-  float2* A;               // [nblocks][9][ns][ns]
+  int ns;                  // null vectors
+  int ch;                  // 1: every null vector is split into its two chirality components (coarse dimension nc = 2 ns, index 2 i + chi)
+  float2* A;               // [nblocks][9][nc][nc]
   int* nbr;                // [nblocks][8], -1 where the block is its own neighbour in that direction
 };
 // sums of the 2 ns per-thread partials over the CTA -> dst[j] (float2), j < ns
-__device__ __forceinline__ void coarse_reduce_store(float (&part)[64], int ns, float* red /*[8][64]*/, float2* dst, int warp, int lane) {
+__device__ __forceinline__ void coarse_reduce_store(float (&part)[64], int ns /* coarse dimension */, float* red /*[8][64]*/, float2* dst, int warp, int lane) {
   for (int k = 0; k < 2 * ns; k++) {
     float v = part[k];
 #pragma unroll
@@ -361,11 +366,14 @@ __global__ void __launch_bounds__(256, 1) coarse_build_k(const __grid_constant__
     }
   }
   const size_t own = size_t(par) * 6 * Vh + cb;     // float4 index of chunk 0 of the own site in a packed full-lattice vector
-  for (int i = 0; i < ns; i++) {
+  const int ch = ca.ch, nc = ch ? 2 * ns : ns;
+  for (int ic = 0; ic < nc; ic++) {                 // column of the coarse operator: null vector i, chirality chi (ch) or all of it
+    const int i = ch ? (ic >> 1) : ic, chm = ch ? 1 + (ic & 1) : 0;
     float r[24], y[24], part[64];
 #pragma unroll
     for (int c = 0; c < 6; c++) {
-      const float4 v = __ldg(ca.phi[i] + own + size_t(c) * Vh);
+      float4 v = __ldg(ca.phi[i] + own + size_t(c) * Vh);
+      if ((chm == 1 && c >= 3) || (chm == 2 && c < 3)) v = make_float4(0.f, 0.f, 0.f, 0.f);
       rho[(par * 6 + c) * 128 + l] = v;
       unpack4(v, r + 4 * c);
     }
@@ -378,32 +386,34 @@ __global__ void __launch_bounds__(256, 1) coarse_build_k(const __grid_constant__
 #pragma unroll
         for (int k = 0; k < 24; k++) y[k] = 0.f;
         switch (d) {
-          case 1: hop_bnd<S, 0, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          case 2: hop_bnd<S, 0, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          case 3: hop_bnd<S, 1, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          case 4: hop_bnd<S, 1, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          case 5: hop_bnd<S, 2, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          case 6: hop_bnd<S, 2, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          case 7: hop_bnd<S, 3, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
-          default: hop_bnd<S, 3, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y); break;
+          case 1: hop_bnd<S, 0, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          case 2: hop_bnd<S, 0, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          case 3: hop_bnd<S, 1, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          case 4: hop_bnd<S, 1, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          case 5: hop_bnd<S, 2, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          case 6: hop_bnd<S, 2, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          case 7: hop_bnd<S, 3, +1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
+          default: hop_bnd<S, 3, -1, NL, PAIR>(a, nsrc, s, tile, par, l, Wsm, y, chm); break;
         }
 #pragma unroll
         for (int k = 0; k < 24; k++) y[k] *= -0.5f;          // H = -1/2 sum (1 -+ gamma) W psi
       }
-      for (int j = 0; j < ns; j++) {                         // <phi_j, y> at this site
-        float re = 0.f, im = 0.f;
+      for (int j = 0; j < ns; j++) {                         // <phi_j, y> at this site, upper and lower chirality apart
+        float re[2] = {0.f, 0.f}, im[2] = {0.f, 0.f};
 #pragma unroll
         for (int c = 0; c < 6; c++) {
           const float4 u = __ldg(ca.phi[j] + own + size_t(c) * Vh);
-          re += u.x * y[4 * c]; re += u.y * y[4 * c + 1]; re += u.z * y[4 * c + 2]; re += u.w * y[4 * c + 3];
-          im += u.x * y[4 * c + 1]; im -= u.y * y[4 * c]; im += u.z * y[4 * c + 3]; im -= u.w * y[4 * c + 2];
+          const int h = c / 3;
+          re[h] += u.x * y[4 * c]; re[h] += u.y * y[4 * c + 1]; re[h] += u.z * y[4 * c + 2]; re[h] += u.w * y[4 * c + 3];
+          im[h] += u.x * y[4 * c + 1]; im[h] -= u.y * y[4 * c]; im[h] += u.z * y[4 * c + 3]; im[h] -= u.w * y[4 * c + 2];
         }
-        part[2 * j] = re; part[2 * j + 1] = im;
+        if (ch) { part[4 * j] = re[0]; part[4 * j + 1] = im[0]; part[4 * j + 2] = re[1]; part[4 * j + 3] = im[1]; }
+        else { part[2 * j] = re[0] + re[1]; part[2 * j + 1] = im[0] + im[1]; }
       }
-      // A[b][d][j][i]: row j, column i -> the reduction delivers a column; store transposed
+      // A[b][d][row][ic]: the reduction delivers a column; store transposed
       __shared__ float2 col[32];
-      coarse_reduce_store(part, ns, red, col, warp, lane);
-      if (threadIdx.x < ns) ca.A[((size_t(tile) * 9 + d) * ns + threadIdx.x) * ns + i] = col[threadIdx.x];
+      coarse_reduce_store(part, nc, red, col, warp, lane);
+      if (threadIdx.x < nc) ca.A[((size_t(tile) * 9 + d) * nc + threadIdx.x) * nc + ic] = col[threadIdx.x];
       __syncthreads();
     }
   }
@@ -531,7 +541,7 @@ int launch_coarse_build(qxd_ctx* c, int prec, int ns, void* const* phi, void* A,
   for (int mu = 0; mu < 4; mu++) { ca.a.boxsh[mu] = c->sap_boxsh[mu]; ca.a.colmask[mu] = c->sap_colmask[mu]; }
   ca.a.colour = 0; ca.a.prologue = 0; ca.a.init_psi = 0; ca.a.nmr = 0;
   for (int i = 0; i < 32; i++) ca.phi[i] = i < ns ? static_cast<const float4*>(phi[i]) : nullptr;
-  ca.ns = ns; ca.A = static_cast<float2*>(A); ca.nbr = nbr;
+  ca.ns = ns; ca.ch = c->dfl_chiral ? 1 : 0; ca.A = static_cast<float2*>(A); ca.nbr = nbr;
   QXD_CUDA_OK(c, cudaMemsetAsync(nbr, 0xff, size_t(nblocks) * 8 * sizeof(int), c->stream));
   const int nl = c->link_reals[prec];
   if (prec == 1) {

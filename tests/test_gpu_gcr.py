@@ -174,9 +174,9 @@ def test_gcr_config_c2_full_size(sloppy):
 DFL_GCR = 3
 
 
-def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32, nref=0):
+def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32, nref=0, chiral=0):
     import torch
-    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4), deflation=(ns, ninv, nkc, nref))
+    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4), deflation=(ns, ninv, nkc, nref, chiral))
     g = c.gpu
     rnd = torch.cat([g.spinor_pack(synth.gaussian_spinor(c.dims_ext, 100 + i), F32) for i in range(ns)])
     g.deflation_setup(rnd, prec)
@@ -184,14 +184,16 @@ def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec
 
 
 @pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES)
-def test_deflation_subspace_and_coarse_operator(dims, cstar, qed, pairing):
+@pytest.mark.parametrize("chiral", [0, 1])
+def test_deflation_subspace_and_coarse_operator(dims, cstar, qed, pairing, chiral):
     """R P = 1 on the coarse space (block-orthonormal null vectors), P R is a projector, and the stored nine-point coarse operator
-    equals R D_w P applied through the (oracle-verified) fp32 D_w kernel."""
+    equals R D_w P applied through the (oracle-verified) fp32 D_w kernel.  chiral = 1: null vectors split by chirality (2 ns
+    coarse degrees of freedom per block); then gamma5 maps the deflation space onto itself."""
     import torch
-    c, _ = _dfl_case(dims, cstar, qed, pairing)
+    c, _ = _dfl_case(dims, cstar, qed, pairing, chiral=chiral)
     g = c.gpu
     nb, ns, ready = g.deflation_info()
-    assert ready and nb == c.V // 256 and ns == 8
+    assert ready and nb == c.V // 256 and ns == 8 * (1 + chiral)
     rng = np.random.default_rng(7)
     cc = torch.from_numpy((rng.normal(size=(nb, ns)) + 1j * rng.normal(size=(nb, ns))).astype(np.complex64)).cuda()
     fine = g.new_packed(F32)
@@ -216,18 +218,25 @@ def test_deflation_subspace_and_coarse_operator(dims, cstar, qed, pairing):
     ref2 = torch.empty_like(cc)
     g.deflation_op(0, pd, ref2)
     assert float((got_c - ref2).abs().max() / ref2.abs().max()) < 1e-4
+    if chiral:     # gamma5 P c = P c' with c'[2 i + chi] = (+1, -1)[chi] c[2 i + chi]   (chiral basis: gamma5 = diag(1, 1, -1, -1))
+        g5 = a.reshape(tuple(c.dims_ext) + (4, 3)).copy()
+        g5[..., 2:, :] *= -1
+        sgn = torch.tensor([1.0, -1.0], device="cuda").repeat(ns // 2)
+        g.deflation_op(1, (cc * sgn).contiguous(), fine2)
+        assert relerr(to_np(g.spinor_unpack(fine2, F32)), g5) < 2e-6
     c.close()
 
 
 @pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES)
-def test_coarse_solve_even_odd(dims, cstar, qed, pairing):
+@pytest.mark.parametrize("chiral", [0, 1])
+def test_coarse_solve_even_odd(dims, cstar, qed, pairing, chiral):
     """The coarse-grid solver (GCR on the even-odd Schur form of the nine-point operator, matrices read in binary16): the
     residual b - A_c x, evaluated with the fp32 coarse operator that the previous test ties to R D_w P, falls with the number of
     steps down to the rounding of the binary16 copy; x = 0 for b = 0."""
     import torch
     res = []
     for nkc in (4, 32):
-        c, _ = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=nkc)
+        c, _ = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=nkc, chiral=chiral)
         g = c.gpu
         nb, ns, _ = g.deflation_info()
         rng = np.random.default_rng(11)
@@ -277,12 +286,12 @@ def test_deflation_pays_on_a_smooth_field():
 
 
 @pytest.mark.parametrize("dims,cstar,qed,pairing", SAP_CASES)
-@pytest.mark.parametrize("sloppy", [F32, F16])
-def test_deflated_gcr_solve(dims, cstar, qed, pairing, sloppy):
+@pytest.mark.parametrize("sloppy,chiral", [(F32, 0), (F16, 0), (F16, 1)])
+def test_deflated_gcr_solve(dims, cstar, qed, pairing, sloppy, chiral):
     """QXD_DFL_GCR: the two-level preconditioner is a contraction on the residual (|r - D_ref M r| < |r| with the oracle's D_w),
     the solve reaches the oracle residual, and a change of the quark invalidates the setup (QXD_ESTATE) until it is redone."""
     import torch
-    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy, nref=1 if sloppy == F32 else 0)
+    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy, nref=1 if sloppy == F32 else 0, chiral=chiral)
     g = c.gpu
     eta = synth.gaussian_spinor(c.dims_ext, 5)
     pin = g.spinor_pack(eta, F32)
