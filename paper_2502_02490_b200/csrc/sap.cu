@@ -318,16 +318,23 @@ struct CoarseArgs {
   float2* A;               // [nblocks][9][nc][nc]
   int* nbr;                // [nblocks][8], -1 where the block is its own neighbour in that direction
 };
-// sums of the 2 ns per-thread partials over the CTA -> dst[j] (float2), j < ns
-__device__ __forceinline__ void coarse_reduce_store(float (&part)[64], int ns /* coarse dimension */, float* red /*[8][64]*/, float2* dst, int warp, int lane) {
-  for (int k = 0; k < 2 * ns; k++) {
-    float v = part[k];
+// sums of the 64 per-thread partials over the CTA -> dst[0..32) (float2).  Within a warp a transposing butterfly: at the step
+// with lane offset o every lane keeps one half of its values and hands the other half to its partner (32 + 16 + 8 + 4 + 2
+// shuffles instead of 64 x 5); lane l ends up with the warp sums of values 2 l and 2 l + 1.
+__device__ __forceinline__ void coarse_reduce_store(float (&part)[64], float* red /*[8][64]*/, float2* dst, int warp, int lane) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) red[warp * 64 + k] = v;
+  for (int h = 32, o = 16; h >= 2; h >>= 1, o >>= 1) {
+    const bool up = (lane & o) != 0;
+#pragma unroll
+    for (int k = 0; k < h; k++) {
+      const float send = up ? part[k] : part[k + h];
+      const float keep = up ? part[k + h] : part[k];
+      part[k] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+    }
   }
+  reinterpret_cast<float2*>(red)[warp * 32 + lane] = make_float2(part[0], part[1]);
   __syncthreads();
-  if (threadIdx.x < 2 * ns) {
+  if (threadIdx.x < 64) {
     float v = 0.f;
 #pragma unroll
     for (int w = 0; w < 8; w++) v += red[w * 64 + threadIdx.x];
@@ -398,21 +405,29 @@ __global__ void __launch_bounds__(256, 1) coarse_build_k(const __grid_constant__
 #pragma unroll
         for (int k = 0; k < 24; k++) y[k] *= -0.5f;          // H = -1/2 sum (1 -+ gamma) W psi
       }
-      for (int j = 0; j < ns; j++) {                         // <phi_j, y> at this site, upper and lower chirality apart
-        float re[2] = {0.f, 0.f}, im[2] = {0.f, 0.f};
+      // <phi_j, y> at this site, upper and lower chirality apart.  Out-of-block hops: y = 0 except on the face of direction d
+      bool act = true;
+      if (d > 0) act = ((nbc[(d - 1) >> 2] >> (8 * ((d - 1) & 3))) & 0x80u) == 0;
 #pragma unroll
-        for (int c = 0; c < 6; c++) {
-          const float4 u = __ldg(ca.phi[j] + own + size_t(c) * Vh);
-          const int h = c / 3;
-          re[h] += u.x * y[4 * c]; re[h] += u.y * y[4 * c + 1]; re[h] += u.z * y[4 * c + 2]; re[h] += u.w * y[4 * c + 3];
-          im[h] += u.x * y[4 * c + 1]; im[h] -= u.y * y[4 * c]; im[h] += u.z * y[4 * c + 3]; im[h] -= u.w * y[4 * c + 2];
+      for (int k = 0; k < 64; k++) part[k] = 0.f;
+#pragma unroll
+      for (int j = 0; j < 32; j++) {
+        if (j < ns && act) {
+          float re[2] = {0.f, 0.f}, im[2] = {0.f, 0.f};
+#pragma unroll
+          for (int c = 0; c < 6; c++) {
+            const float4 u = __ldg(ca.phi[j] + own + size_t(c) * Vh);
+            const int h = c / 3;
+            re[h] += u.x * y[4 * c]; re[h] += u.y * y[4 * c + 1]; re[h] += u.z * y[4 * c + 2]; re[h] += u.w * y[4 * c + 3];
+            im[h] += u.x * y[4 * c + 1]; im[h] -= u.y * y[4 * c]; im[h] += u.z * y[4 * c + 3]; im[h] -= u.w * y[4 * c + 2];
+          }
+          if (ch) { if (j < 16) { part[4 * j] = re[0]; part[4 * j + 1] = im[0]; part[4 * j + 2] = re[1]; part[4 * j + 3] = im[1]; } }
+          else { part[2 * j] = re[0] + re[1]; part[2 * j + 1] = im[0] + im[1]; }
         }
-        if (ch) { part[4 * j] = re[0]; part[4 * j + 1] = im[0]; part[4 * j + 2] = re[1]; part[4 * j + 3] = im[1]; }
-        else { part[2 * j] = re[0] + re[1]; part[2 * j + 1] = im[0] + im[1]; }
       }
       // A[b][d][row][ic]: the reduction delivers a column; store transposed
       __shared__ float2 col[32];
-      coarse_reduce_store(part, nc, red, col, warp, lane);
+      coarse_reduce_store(part, red, col, warp, lane);
       if (threadIdx.x < nc) ca.A[((size_t(tile) * 9 + d) * nc + threadIdx.x) * nc + ic] = col[threadIdx.x];
       __syncthreads();
     }
