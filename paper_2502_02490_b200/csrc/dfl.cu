@@ -5,9 +5,12 @@
 //   setup   ns test vectors (random, passed in by the caller) are smoothed by ninv applications of M_sap, which damps the high
 //           modes of D_w and leaves an approximate low-mode space; the vectors are restricted to the SAP blocks (256 sites) and
 //           orthonormalised block by block: the deflation space is span{ P_b phi_i } (dimension ns per block);
-//           the coarse ("little") operator A_c = R D_w P is a nine-point stencil of ns x ns complex matrices (sap.cu).
+//           with the chirality split (qxd_set_deflation_chirality) every phi_i gives two basis vectors per block, its upper and
+//           lower spin components: dimension nc = 2 ns per block, coarse index 2 i + chi;
+//           the coarse ("little") operator A_c = R D_w P is a nine-point stencil of nc x nc complex matrices (sap.cu).
 //   apply   z = P A_c^{-1} R r  +  M_sap (r - D_w P A_c^{-1} R r):  coarse-grid correction, then Schwarz smoothing of what is left;
-//           A_c^{-1} is nkc steps of GCR on the coarse grid, all coefficients on the device, no host round trip.
+//           A_c^{-1} is nkc steps of GCR on the even-odd (Schur) form of the coarse system, matrices in binary16, all coefficients
+//           on the device, no host round trip.
 //
 // R = P^dagger (block-wise inner products with the phi_i), P = block-wise linear combination.  Everything is fp32 (the block
 // operator of M_sap and of the coarse-operator build in the storage precision of the solve).  The outer solver is the flexible
@@ -248,30 +251,6 @@ __global__ void __launch_bounds__(256) dfl_eo_hop_k(int ns, int colour, float si
     y[size_t(b ^ 1) * ns + j] = make_float2(0.f, 0.f);
   }
 }
-// minimal-residual step of the coarse correction on the fine grid: alpha = <t, r> / <t, t> (device, dots = (Re, Im) of <t, r> and |t|^2);
-// t <- r - alpha t  (the residual the Schwarz smoother starts from),  z <- alpha z
-__global__ void __launch_bounds__(256) dfl_mr_step_k(size_t n4, const double* __restrict__ dots, const float4* __restrict__ r, float4* __restrict__ t, float4* __restrict__ z) {
-  const double d = dots[2];
-  const float ar = d > 0.0 ? (float)(dots[0] / d) : 0.f, ai = d > 0.0 ? (float)(dots[1] / d) : 0.f;
-  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
-    const float4 x = t[i], y = r[i], w = z[i];
-    t[i] = make_float4(y.x - (ar * x.x - ai * x.y), y.y - (ar * x.y + ai * x.x), y.z - (ar * x.z - ai * x.w), y.w - (ar * x.w + ai * x.z));
-    z[i] = make_float4(ar * w.x - ai * w.y, ar * w.y + ai * w.x, ar * w.z - ai * w.w, ar * w.w + ai * w.z);
-  }
-}
-// (Re <t, r>, Im <t, r>, |t|^2)
-__global__ void __launch_bounds__(256) dfl_mr_dots_k(size_t n4, const float4* __restrict__ t, const float4* __restrict__ r, Reducer R) {
-  double acc[3] = {0.0, 0.0, 0.0};
-  for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n4; i += size_t(gridDim.x) * blockDim.x) {
-    const float4 x = __ldg(t + i), y = __ldg(r + i);
-    float re = x.x * y.x; re += x.y * y.y; re += x.z * y.z; re += x.w * y.w;
-    float im = x.x * y.y; im -= x.y * y.x; im += x.z * y.w; im -= x.w * y.z;
-    float nn = x.x * x.x; nn += x.y * x.y; nn += x.z * x.z; nn += x.w * x.w;
-    acc[0] += (double)re; acc[1] += (double)im; acc[2] += (double)nn;
-  }
-  grid_reduce<3>(acc, R, blockIdx.x, gridDim.x, 0);
-}
-
 struct Dfl {
   qxd_ctx* c;
   int Vh, nb, ns, nc, ch;   // ns null vectors; nc = coarse degrees of freedom per block (2 ns with the chirality split)
