@@ -629,11 +629,15 @@ def run_cuda(args, cfg):
                     oref2.clover_build(cfg["csw"], cfg["csw_qed"])
                 nc = {"workload": f"{cfg['name']} geometry, couplings and U(1) field; SU(3) links = synth.su3_links_smooth(eps 0.7, every 4 sites); kappa {nck}",
                       "tol": cfg["tol"], "maxiter": 3000}
+                # here the inverse-iteration refinement of the deflation space pays (it does not on the white-noise links: DESIGN.md 6a)
+                refine = (args.nc_nref, args.nc_refk) if dp[0] <= 2 * (gp[0] - args.nc_refk) else (0, 1)
+                g.set_deflation_refine(*refine)
                 t0 = ev(); t1 = ev()
                 t0.record()
                 g.deflation_setup(rnd, B.QXD_F16)
                 t1.record()
                 t1.synchronize()
+                g.set_deflation_refine(0, 1)
                 for name, algo in (("cgne_fp64_fp16", B.QXD_CGNE), ("bicgstab_fp64_fp16", B.QXD_BICGSTAB), ("gcr_sap_fp64_fp16", B.QXD_GCR),
                                    ("dfl_gcr_sap_fp64_fp16", B.QXD_DFL_GCR)):
                     reps = 1 if algo == B.QXD_CGNE else 2          # CGNE runs into maxiter here (seconds): once is enough
@@ -643,7 +647,8 @@ def run_cuda(args, cfg):
                         r = eta.reshape(-1) - oref2.apply_Dw(psi_d.cpu().numpy()).reshape(-1)
                         info["true_res_oracle"] = float(np.linalg.norm(r) / np.linalg.norm(eta.reshape(-1)))
                     nc[name] = info
-                nc["dfl_gcr_sap_fp64_fp16"].update({"ns": dp[0], "ninv": dp[1], "nkc": dp[2], "chirality_split": dp[4], "setup_seconds": t0.elapsed_time(t1) * 1e-3})
+                nc["dfl_gcr_sap_fp64_fp16"].update({"ns": dp[0], "ninv": dp[1], "nkc": dp[2], "chirality_split": dp[4], "refinement_rounds": refine[0],
+                                                    "gcr_steps_per_refinement_solve": refine[1], "setup_seconds": t0.elapsed_time(t1) * 1e-3})
                 solves["near_critical"] = nc
                 del oref2, Us
             del rnd
@@ -806,6 +811,8 @@ def main():
     ap.add_argument("--dfl-chiral", type=int, default=1, help="1: null vectors split by chirality (2 ns coarse degrees of freedom per block; ns <= 16)")
     ap.add_argument("--dfl-ninv", type=int, default=8, help="M_sap smoothing passes per null vector in the deflation setup")
     ap.add_argument("--dfl-nkc", type=int, default=12, help="GCR steps of every coarse-grid solve")
+    ap.add_argument("--nc-nref", type=int, default=2, help="refinement rounds of the deflation space in the near-critical comparison")
+    ap.add_argument("--nc-refk", type=int, default=4, help="deflated GCR steps of every refinement solve there")
     ap.add_argument("--nc-kappa", type=float, default=None,
                     help="hopping parameter of the near-critical solver comparison on smooth links (default: 0.1238 at c3, skipped elsewhere; 0 = skip)")
     ap.add_argument("--decomp", default="rhs", choices=["rhs", "domain"], help="rhs: shard by right-hand side (weak scaling, the default); "

@@ -217,6 +217,13 @@ int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
  *                        vectors (ns <= 16), and gamma5 maps it onto itself.  Before qxd_workspace_bind.  Default 0.  With the split
  *                        qxd_deflation_info reports 2 ns and the coarse vectors of qxd_deflation_op are [nblocks][2 ns], index
  *                        2 i + chi.
+ *   qxd_set_deflation_refine   nref refinement rounds (replaces the nref of qxd_set_deflation) and what a round does to every null
+ *                        vector: steps = 1 (default) applies the current two-level preconditioner once; steps > 1 is an inverse
+ *                        iteration, phi_i <- `steps` steps of the deflated flexible GCR on D_w x = phi_i in fp32 (no convergence
+ *                        test, no host round trip); after every round the space is re-orthonormalised and the coarse operator
+ *                        rebuilt.  Needs ns <= 2 (nkv - steps) (checked by qxd_deflation_setup, QXD_EWORKSPACE).  May be called at
+ *                        any time; takes effect at the next qxd_deflation_setup.  Pays where D_w is close to singular with a
+ *                        well-defined sign of the real parts of its spectrum; off by default.
  *   qxd_deflation_setup  random_vectors: DEVICE, ns packed fp32 full-lattice spinors back to back (the caller draws them; any
  *                        linearly independent set works).  Each is smoothed by ninv applications of M_sap (block operator in storage
  *                        precision prec = QXD_F32 / QXD_F16), the set is orthonormalised block by block, and the coarse operator
@@ -235,6 +242,7 @@ int qxd_set_gcr(qxd_ctx* ctx, int nkv, int ncy, int nmr);
  *                        complex fp32 (block index = checkerboard index >> 7). */
 int qxd_set_deflation(qxd_ctx* ctx, int ns, int ninv, int nkc, int nref);
 int qxd_set_deflation_chirality(qxd_ctx* ctx, int on);
+int qxd_set_deflation_refine(qxd_ctx* ctx, int nref, int steps);
 int qxd_deflation_setup(qxd_ctx* ctx, int prec, const void* random_vectors /*DEVICE*/);
 int qxd_deflation_info(const qxd_ctx* ctx, int* nblocks, int* ns, int* ready);
 int qxd_deflation_op(qxd_ctx* ctx, int op, const void* in, void* out);

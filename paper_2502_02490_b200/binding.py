@@ -70,6 +70,7 @@ SYMBOLS = {
     "qxd_apply_sap": (_i, [_vp, _i, _vp, _vp]),
     "qxd_set_deflation": (_i, [_vp, _i, _i, _i, _i]),
     "qxd_set_deflation_chirality": (_i, [_vp, _i]),
+    "qxd_set_deflation_refine": (_i, [_vp, _i, _i]),
     "qxd_deflation_setup": (_i, [_vp, _i, _vp]),
     "qxd_deflation_info": (_i, [_vp, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)]),
     "qxd_deflation_op": (_i, [_vp, _i, _vp, _vp]),
@@ -195,10 +196,12 @@ class Qxd:
         if gcr is not None:                     # (nkv, ncy, nmr): Krylov space and SAP parameters of QXD_GCR (row f3)
             self._chk(self.lib.qxd_set_gcr(self.h, *gcr))
         if deflation is not None:               # (ns, ninv, nkc[, nref]): null vectors, setup smoothing passes, coarse GCR steps, refinement rounds
-            d = tuple(deflation) + (0,) * (5 - len(deflation))       # fifth entry: 1 = split the null vectors by chirality
+            d = tuple(deflation) + (0,) * (6 - len(deflation))       # fifth entry: 1 = split the null vectors by chirality; sixth: GCR steps of a refinement solve
             if d[4]:
                 self._chk(self.lib.qxd_set_deflation_chirality(self.h, 1))
             self._chk(self.lib.qxd_set_deflation(self.h, *d[:4]))
+            if d[5] > 1:
+                self.set_deflation_refine(d[3], d[5])
         self.prec_mask = 0
         for p in precisions:
             self.prec_mask |= 1 << p
@@ -339,6 +342,10 @@ class Qxd:
         info = self._info(algo, sloppy, delta, maxiter)
         rc = self._chk(self.lib.qxd_solve(self.h, _ptr(eta), _ptr(psi), float(tol), C.byref(info)), allow=(QXD_ENOCONV,))
         return psi, self._report(rc, info)
+
+    def set_deflation_refine(self, nref, steps=1):
+        """nref refinement rounds of the deflation space at the next deflation_setup; steps > 1: inverse iteration by that many deflated GCR steps."""
+        self._chk(self.lib.qxd_set_deflation_refine(self.h, nref, steps))
 
     def deflation_setup(self, random_vectors, prec=QXD_F16):
         """random_vectors: ns packed fp32 full-lattice spinors back to back (uint8 tensor on the device)."""

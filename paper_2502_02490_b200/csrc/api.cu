@@ -689,6 +689,12 @@ int qxd_set_deflation(qxd_ctx* c, int ns, int ninv, int nkc, int nref) {
   c->dfl_ns = ns; c->dfl_ninv = ninv > 0 ? ninv : 4; c->dfl_nkc = nkc > 0 ? nkc : 16; c->dfl_nref = nref;
   return QXD_OK;
 }
+int qxd_set_deflation_refine(qxd_ctx* c, int nref, int steps) {
+  if (!c) return QXD_EINVAL;
+  if (nref < 0 || steps < 1 || steps > 16) return fail(c, QXD_EINVAL, "set_deflation_refine: nref >= 0, 1 <= steps <= 16");
+  c->dfl_nref = nref; c->dfl_refk = steps;
+  return QXD_OK;
+}
 int qxd_set_deflation_chirality(qxd_ctx* c, int on) {
   if (!c) return QXD_EINVAL;
   if (c->ws) return fail(c, QXD_ESTATE, "qxd_set_deflation_chirality must precede qxd_workspace_bind");

@@ -447,14 +447,20 @@ int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors) {
   c->dfl_ready = true; c->dfl_prec = prec;
   for (int round = 0; round < c->dfl_nref; round++) {
     // new vectors from the CURRENT two-level method, parked in the Krylov space of the fine-grid GCR until all are done
-    if (D.ns > 2 * c->gcr_nkv) return fail(c, QXD_EWORKSPACE, "deflation refinement needs ns <= 2 nkv scratch vectors (qxd_set_gcr)");
+    // refk = 1: phi_i <- M_2level phi_i; refk > 1: inverse iteration, phi_i <- refk steps of the deflated GCR on D_w x = phi_i
+    // (Krylov vectors [0, refk) of the fine-grid solver; the new vectors wait in the upper part of the Krylov space)
+    const int refk = c->dfl_refk > 1 ? c->dfl_refk : 0, park = c->gcr_nkv - refk;
+    if (D.ns > 2 * park) return fail(c, QXD_EWORKSPACE, "deflation refinement needs ns <= 2 (nkv - steps) scratch vectors (qxd_set_gcr)");
     for (int i = 0; i < D.ns; i++) {
-      void* dst = i < c->gcr_nkv ? c->gz[i] : c->gw[i - c->gcr_nkv];
-      QXD_TRY(launch_dfl_precond(c, prec, c->dphi[i], dst));
+      void* dst = i < park ? c->gz[refk + i] : c->gw[refk + i - park];
+      if (refk) {
+        QXD_CUDA_OK(c, cudaMemcpyAsync(c->g_r, c->dphi[i], vb, cudaMemcpyDeviceToDevice, c->stream));
+        QXD_TRY(gcr_cycle32(c, prec, true, refk, dst));
+      } else QXD_TRY(launch_dfl_precond(c, prec, c->dphi[i], dst));
       QXD_TRY(normalise_flat(D, static_cast<float4*>(dst)));
     }
     for (int i = 0; i < D.ns; i++) {
-      void* src = i < c->gcr_nkv ? c->gz[i] : c->gw[i - c->gcr_nkv];
+      void* src = i < park ? c->gz[refk + i] : c->gw[refk + i - park];
       QXD_CUDA_OK(c, cudaMemcpyAsync(c->dphi[i], src, vb, cudaMemcpyDeviceToDevice, c->stream));
     }
     c->dfl_ready = false;

@@ -78,6 +78,57 @@ struct Gcr {
 
 }  // namespace
 
+// K steps of the flexible GCR in fp32 without any host round trip (the inverse iteration of the deflation setup, dfl.cu):
+// on entry c->g_r holds the right-hand side b (it is overwritten with the residual), on exit x ~ D_w^{-1} b.  Uses the Krylov
+// vectors gz / gw [0, K) and the scalars of the solver; no convergence test.
+int gcr_cycle32(qxd_ctx* c, int pprec, bool use_dfl, int K, void* x) {
+  const int Vh = c->g.Vh;
+  if (K < 1 || K > c->gcr_nkv) return fail(c, QXD_EINVAL, "gcr_cycle32: 1 <= K <= nkv");
+  Gcr G;
+  G.c = c; G.n4 = size_t(12) * Vh;
+  G.nblk = Vh / 128 < 1 ? 1 : (Vh / 128 > 148 * 8 ? 148 * 8 : Vh / 128);
+  double* S = c->gscal;
+  double* tmp = S + 3000;
+  float4* r32 = static_cast<float4*>(c->g_r);
+  VecList Z, W;
+  for (int k = 0; k < 32; k++) { Z.v[k] = static_cast<const float4*>(c->gz[k]); W.v[k] = static_cast<const float4*>(c->gw[k]); }
+  for (int k = 0; k < K; k++) {
+    if (use_dfl) QXD_TRY(launch_dfl_precond(c, pprec, c->g_r, c->gz[k]));
+    else QXD_TRY(launch_sap(c, pprec, c->g_r, c->gz[k]));
+    DslashCall d{};
+    d.prec = 1; d.mode = DS_DW_FULL; d.flags = 0;
+    d.in[0] = half_view(1, c->gz[k], Vh, 0); d.in[1] = half_view(1, c->gz[k], Vh, 1);
+    d.out[0] = half_view(1, c->gw[k], Vh, 0); d.out[1] = half_view(1, c->gw[k], Vh, 1);
+    QXD_TRY(launch_dslash(c, d));
+    float4* wk = static_cast<float4*>(c->gw[k]);
+    for (int j0 = 0; j0 < k; j0 += 4) {
+      const int nj = k - j0 < 4 ? k - j0 : 4;
+      Reducer R = G.red(S + G_BR + (j0 * 32 + k) * 2);
+      R.rstride = 64;
+      if (nj == 4) gcr_dots_k<4><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+      else if (nj == 3) gcr_dots_k<3><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+      else if (nj == 2) gcr_dots_k<2><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+      else gcr_dots_k<1><<<G.nblk, 256, 0, c->stream>>>(G.n4, W, j0, wk, R);
+      QXD_LAUNCH_CHECK(c);
+      reduce_finalize_k<2><<<dim3(1, nj), FINALIZE_THREADS, 0, c->stream>>>(R, G.nblk);
+      QXD_LAUNCH_CHECK(c);
+    }
+    gcr_orth_k<<<G.nblk, 256, 0, c->stream>>>(G.n4, W, k, S + G_BR + k * 2, S + G_N2, wk, r32, G.red(tmp));
+    QXD_LAUNCH_CHECK(c);
+    QXD_TRY(G.finalize<3>(tmp));
+    gcr_store3_k<<<1, 1, 0, c->stream>>>(tmp, S + G_N2 + k, S + G_Q + 2 * k);
+    QXD_LAUNCH_CHECK(c);
+    gcr_update_r_k<<<G.nblk, 256, 0, c->stream>>>(G.n4, wk, S + G_Q + 2 * k, S + G_N2 + k, r32, G.red(S + G_RR));
+    QXD_LAUNCH_CHECK(c);
+    QXD_TRY(G.finalize<1>(S + G_RR));
+  }
+  gcr_backsub_k<<<1, 32, 0, c->stream>>>(K, S);
+  QXD_LAUNCH_CHECK(c);
+  gcr_update_x32_k<<<G.nblk, 256, 0, c->stream>>>(G.n4, Z, K, S + G_Y, static_cast<float4*>(x), 1);
+  QXD_LAUNCH_CHECK(c);
+  return QXD_OK;
+}
+
 int solve_gcr(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qxd_solve_info* info) {
   const int Vh = c->g.Vh;
   const int pprec = info->sloppy;   // storage precision of the SAP block operator

@@ -81,6 +81,7 @@ struct qxd_ctx {
   double* gscal = nullptr;                       // device scalars of the GCR cycle: coefficient matrix b[32][32] (complex), c[32], y[32], norms
   // two-level (deflated) preconditioner of the GCR (dfl.cu): null vectors, coarse operator, coarse-grid vectors
   int dfl_ns = 0, dfl_ninv = 4, dfl_nkc = 16, dfl_nref = 0, dfl_prec = 1;
+  int dfl_refk = 1;                              // GCR steps of every inverse-iteration solve of the refinement rounds (1 = one preconditioner application)
   int dfl_chiral = 0;                            // 1: null vectors split by chirality, coarse dimension per block = 2 ns (qxd_set_deflation_chirality)
   bool dfl_ready = false;
   void* dphi[32] = {};                           // fp32 packed full-lattice null vectors, block-orthonormal
@@ -227,6 +228,7 @@ int solve_gcr(qxd_ctx* c, const double* eta_nat, double* psi_nat, double tol, qx
 int launch_coarse_build(qxd_ctx* c, int prec, int ns, void* const* phi, void* A, int* nbr);
 // dfl.cu (row f3, second level)
 int launch_dfl_precond(qxd_ctx* c, int prec, const void* r, void* z);
+int gcr_cycle32(qxd_ctx* c, int pprec, bool use_dfl, int K, void* x);
 int dfl_setup(qxd_ctx* c, int prec, const void* random_vectors);
 int dfl_restrict(qxd_ctx* c, const void* fine, void* coarse);
 int dfl_prolong(qxd_ctx* c, const void* coarse, void* fine);

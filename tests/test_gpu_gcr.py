@@ -174,9 +174,10 @@ def test_gcr_config_c2_full_size(sloppy):
 DFL_GCR = 3
 
 
-def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32, nref=0, chiral=0):
+def _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=3, nkc=12, kappa=0.125, prec=F32, nref=0, chiral=0, refk=1):
     import torch
-    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4), deflation=(ns, ninv, nkc, nref, chiral))
+    c = Case(dims, cstar, 1, qed, q=2 / 3, kappa=kappa, csw=1.5, csw_qed=1.0, eps=0.2, pairing=pairing, gcr=(8, 3, 4),
+             deflation=(ns, ninv, nkc, nref, chiral, refk))
     g = c.gpu
     rnd = torch.cat([g.spinor_pack(synth.gaussian_spinor(c.dims_ext, 100 + i), F32) for i in range(ns)])
     g.deflation_setup(rnd, prec)
@@ -291,7 +292,10 @@ def test_deflated_gcr_solve(dims, cstar, qed, pairing, sloppy, chiral):
     """QXD_DFL_GCR: the two-level preconditioner is a contraction on the residual (|r - D_ref M r| < |r| with the oracle's D_w),
     the solve reaches the oracle residual, and a change of the quark invalidates the setup (QXD_ESTATE) until it is redone."""
     import torch
-    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy, nref=1 if sloppy == F32 else 0, chiral=chiral)
+    # refinement of the deflation space: one application of the two-level preconditioner per vector (fp32 case), an inverse
+    # iteration of 3 deflated GCR steps per vector (chirality-split case), none (fp16 case)
+    c, rnd = _dfl_case(dims, cstar, qed, pairing, ns=8, ninv=4, nkc=16, kappa=0.125, prec=sloppy, nref=1 if (sloppy == F32 or chiral) else 0,
+                       chiral=chiral, refk=3 if chiral else 1)
     g = c.gpu
     eta = synth.gaussian_spinor(c.dims_ext, 5)
     pin = g.spinor_pack(eta, F32)
