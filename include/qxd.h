@@ -344,6 +344,10 @@ int qxd_halo_zero(qxd_ctx* ctx, int prec, void* packed, int parity_mask, int mu,
 int qxd_blas_norm2_dev(qxd_ctx* ctx, int prec, const void* x, double* out /*DEVICE*/);
 int qxd_blas_cg_xr(qxd_ctx* ctx, int prec, const double* num, const double* den, const void* p, const void* t, void* x, void* r, double* rr /*all scalars DEVICE*/);
 int qxd_blas_cg_p(qxd_ctx* ctx, int prec, const double* num, const double* den, const void* s, void* p);
+/* binary16 operator with fp32 Krylov vectors (the form the single-GPU solver uses, reading R12): x32 += alpha p16, r32 -= alpha t16,
+ * r16 = half(r32), *rr = |r32|^2   and   p32 = s16 + beta p32, p16 = half(p32);  alpha, beta = *num / *den (DEVICE scalars). */
+int qxd_blas_cg_xr_h(qxd_ctx* ctx, const double* num, const double* den, const void* p16, const void* t16, void* x32, void* r32, void* r16, double* rr);
+int qxd_blas_cg_p_h(qxd_ctx* ctx, const double* num, const double* den, const void* s16, void* p32, void* p16);
 int qxd_blas_copy(qxd_ctx* ctx, int prec, const void* x, void* y);
 int qxd_blas_zero(qxd_ctx* ctx, int prec, void* x);
 /* reliable-update building blocks: y (prec_to) = x (prec_from);  x_hi (fp64) += x_lo (prec), x_lo = 0;  r = b - t, *rr = |r|^2 */

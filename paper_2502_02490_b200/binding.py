@@ -97,6 +97,8 @@ SYMBOLS = {
     "qxd_face_scatter": (_i, [_vp, _i, _vp, _i, _i, _i, _i, _vp]),
     "qxd_halo_zero": (_i, [_vp, _i, _vp, _i, _i, _i, _i]),
     "qxd_blas_norm2_dev": (_i, [_vp, _i, _vp, _vp]),
+    "qxd_blas_cg_xr_h": (_i, [_vp] * 9),
+    "qxd_blas_cg_p_h": (_i, [_vp] * 6),
     "qxd_noalloc_init": (_i, []),
     "qxd_noalloc_max_reals": (_sz, []),
     "qxd_noalloc_last_error": (C.c_char_p, []),
@@ -462,6 +464,12 @@ class Qxd:
 
     def blas_cg_xr(self, prec, num, den, p, t, x, r, rr):
         self._chk(self.lib.qxd_blas_cg_xr(self.h, prec, _ptr(num), _ptr(den), _ptr(p), _ptr(t), _ptr(x), _ptr(r), _ptr(rr)))
+
+    def blas_cg_xr_h(self, num, den, p16, t16, x32, r32, r16, rr):
+        self._chk(self.lib.qxd_blas_cg_xr_h(self.h, _ptr(num), _ptr(den), _ptr(p16), _ptr(t16), _ptr(x32), _ptr(r32), _ptr(r16), _ptr(rr)))
+
+    def blas_cg_p_h(self, num, den, s16, p32, p16):
+        self._chk(self.lib.qxd_blas_cg_p_h(self.h, _ptr(num), _ptr(den), _ptr(s16), _ptr(p32), _ptr(p16)))
 
     def blas_cg_p(self, prec, num, den, s, p):
         self._chk(self.lib.qxd_blas_cg_p(self.h, prec, _ptr(num), _ptr(den), _ptr(s), _ptr(p)))

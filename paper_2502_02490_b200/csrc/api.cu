@@ -642,6 +642,18 @@ int qxd_blas_cg_p(qxd_ctx* c, int prec, const double* num, const double* den, co
   if (!blas_args_ok(c, prec) || !num || !den || !s || !p) return QXD_EINVAL;
   return blas_cg_p(c, prec, num, den, hp(c, prec, s), hp(c, prec, p));
 }
+int qxd_blas_cg_xr_h(qxd_ctx* c, const double* num, const double* den, const void* p16, const void* t16, void* x32, void* r32, void* r16, double* rr) {
+  if (!blas_args_ok(c, 1) || !blas_args_ok(c, 2) || !num || !den || !p16 || !t16 || !x32 || !r32 || !r16 || !rr) return QXD_EINVAL;
+  SpinorPtr x = hp(c, 1, x32), r = hp(c, 1, r32);
+  x.scale = nullptr; r.scale = nullptr;
+  return blas_cg_xr_h(c, num, den, hp(c, 2, p16), hp(c, 2, t16), x, r, hp(c, 2, r16), rr);
+}
+int qxd_blas_cg_p_h(qxd_ctx* c, const double* num, const double* den, const void* s16, void* p32, void* p16) {
+  if (!blas_args_ok(c, 1) || !blas_args_ok(c, 2) || !num || !den || !s16 || !p32 || !p16) return QXD_EINVAL;
+  SpinorPtr p = hp(c, 1, p32);
+  p.scale = nullptr;
+  return blas_cg_p_h(c, num, den, hp(c, 2, s16), p, hp(c, 2, p16));
+}
 int qxd_blas_copy(qxd_ctx* c, int prec, const void* x, void* y) {
   if (!blas_args_ok(c, prec) || !x || !y) return QXD_EINVAL;
   return blas_copy(c, prec, hp(c, prec, x), hp(c, prec, y));

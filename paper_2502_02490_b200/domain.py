@@ -514,12 +514,18 @@ def solve_distributed(op: GpuOperator, eta, tol, maxiter=10000):
     return x, info
 
 
-def solve_distributed_mixed(op_hi: GpuOperator, op_lo: GpuOperator, eta, tol, delta=0.1, maxiter=10000):
+def solve_distributed_mixed(op_hi: GpuOperator, op_lo: GpuOperator, eta, tol, delta=0.1, maxiter=10000, op_vec: GpuOperator = None):
     """Mixed-precision distributed solve: the CG iteration on the normal equations of D-hat runs on the SLOPPY operator
     op_lo (fp32 storage; same ranks and contexts as op_hi, see GpuRank.with_prec), the solution is accumulated and the true
     residual recomputed with the fp64 operator op_hi whenever the iterated residual has dropped by `delta` since the last
     update ("reliable updates", PAPER.md:207 ref [4]; the single-GPU loop of csrc/solver.cu with every scalar all-reduced and a
-    halo exchange inside every operator application).  Convergence is declared on the fp64 residual only."""
+    halo exchange inside every operator application).  Convergence is declared on the fp64 residual only.
+
+    op_vec (fp32 view of the same contexts) with a binary16 op_lo: the Krylov vectors x, r, p stay in fp32 and only the operator's
+    inputs and outputs (p16, r16, s, t: what travels in the halos) are binary16 -- the form of the single-GPU solver (reading R12;
+    rounding x, r, p themselves to binary16 costs 2.8 x the iterations)."""
+    if op_vec is not None:
+        return _solve_distributed_h16(op_hi, op_lo, op_vec, eta, tol, delta, maxiter)
     H, L = op_hi, op_lo
     ranks = H.ranks
     n2 = H.scalar()
@@ -584,6 +590,90 @@ def solve_distributed_mixed(op_hi: GpuOperator, op_lo: GpuOperator, eta, tol, de
         L.apply(rlo, s, dagger=True)
         L.norm2(s, gam2)
         L.cg_p(gam2, gam, s, p)
+        gam, gam2 = gam2, gam
+    if status:
+        rr_true = reliable()
+        nrel += 1
+        if rr_true <= stop2:
+            status = 0
+    H.reconstruct(eta, xhi)
+    return xhi, dict(iters=it, n_reliable=nrel, status=status, true_res_eo=(rr_true / tot) ** 0.5 if tot > 0 else 0.0)
+
+
+def _solve_distributed_h16(H: GpuOperator, L: GpuOperator, V: GpuOperator, eta, tol, delta, maxiter):
+    """solve_distributed_mixed with a binary16 operator L and fp32 Krylov vectors (allocated through V)."""
+    ranks = H.ranks
+    n2 = H.scalar()
+    tot = 0.0
+    for par in (0, 1):
+        for r in ranks:
+            o = H.ops[r]
+            o.g.blas_norm2_dev(o.half(eta[r], par), o.prec, n2[r])
+        H.comm.allreduce_sum(n2)
+        tot += H.value(n2)
+    stop2 = tol * tol * tot
+    b = H.alloc()
+    H.prepare(eta, b)
+    xhi, rhi, thi = H.alloc(), H.alloc(), H.alloc()
+    xlo, rlo, p = V.alloc(), V.alloc(), V.alloc()                 # fp32
+    r16, p16, s, t = L.alloc(), L.alloc(), L.alloc(), L.alloc()   # binary16
+    gam, gam2, tt, rr, rrt = L.scalar(), L.scalar(), L.scalar(), L.scalar(), H.scalar()
+
+    def convert(src, osrc, dst, odst):
+        for r in ranks:
+            a, c = osrc.ops[r], odst.ops[r]
+            a.g.blas_convert(a.half(src[r]), a.prec, c.half(dst[r]), c.prec)
+
+    def reliable():
+        for r in ranks:
+            oh, ov = H.ops[r], V.ops[r]
+            oh.g.blas_acc_hi(ov.half(xlo[r]), ov.prec, oh.half(xhi[r]))
+        H.apply(xhi, thi)
+        for r in ranks:
+            oh = H.ops[r]
+            oh.g.blas_sub_norm_dev(oh.half(b[r]), oh.half(thi[r]), oh.half(rhi[r]), oh.prec, rrt[r])
+        H.comm.allreduce_sum(rrt)
+        convert(rhi, H, rlo, V)
+        convert(rhi, H, r16, L)
+        return H.value(rrt)
+
+    H.copy(b, rhi)
+    H.norm2(rhi, rrt)
+    rr_true = H.value(rrt)
+    convert(rhi, H, rlo, V)
+    convert(rhi, H, r16, L)
+    it, nrel, maxr = 0, 0, rr_true ** 0.5
+    status = 0 if rr_true <= stop2 else -5
+    if status:
+        L.apply(r16, s, dagger=True)
+        convert(s, L, p, V)
+        L.copy(s, p16)
+        L.norm2(s, gam)
+    while status and it < maxiter:
+        L.apply(p16, t)
+        L.norm2(t, tt)
+        for r in ranks:
+            ol, ov = L.ops[r], V.ops[r]
+            ol.g.blas_cg_xr_h(gam[r], tt[r], ol.half(p16[r]), ol.half(t[r]), ov.half(xlo[r]), ov.half(rlo[r]), ol.half(r16[r]), rr[r])
+        L.comm.allreduce_sum(rr)
+        it += 1
+        res2 = L.value(rr)
+        if not (res2 == res2):
+            break
+        rn = res2 ** 0.5
+        maxr = max(maxr, rn)
+        if rn < delta * maxr or res2 <= stop2:
+            rr_true = reliable()
+            nrel += 1
+            maxr = rr_true ** 0.5
+            if rr_true <= stop2:
+                status = 0
+                break
+        L.apply(r16, s, dagger=True)
+        L.norm2(s, gam2)
+        for r in ranks:
+            ol, ov = L.ops[r], V.ops[r]
+            ol.g.blas_cg_p_h(gam2[r], gam[r], ol.half(s[r]), ov.half(p[r]), ol.half(p16[r]))
         gam, gam2 = gam2, gam
     if status:
         rr_true = reliable()

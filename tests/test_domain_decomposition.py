@@ -340,20 +340,24 @@ def test_gpu_distributed_solve(dims, grid, cstar, ap, qed, pairing):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("sloppy", [1, 2], ids=["fp32", "fp16"])
 @pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[6]])
-def test_gpu_distributed_mixed_precision_solve(dims, grid, cstar, ap, qed, pairing):
-    """fp32 sloppy operator with fp64 reliable updates on the decomposed lattice: reaches 1e-10 on the global oracle's residual."""
+def test_gpu_distributed_mixed_precision_solve(dims, grid, cstar, ap, qed, pairing, sloppy):
+    """fp32 / binary16 sloppy operator (halos, Krylov vectors and all) with fp64 reliable updates on the decomposed lattice:
+    reaches 1e-10 on the global oracle's residual."""
     U, A = fields(dims, qed)
     pg = D.ProcessGrid(dims, grid, cstar)
     lats = {r: D.LocalLattice(pg, r, antiperiodic=bool(ap)) for r in range(pg.world)}
-    hi = {r: D.GpuRank(lats[r], U, A, 1.0, KAPPA, Q if qed else 0.0, CSW, CSWQ if qed else 0.0, prec=0, pairing=pairing, extra_precisions=(1,))
+    hi = {r: D.GpuRank(lats[r], U, A, 1.0, KAPPA, Q if qed else 0.0, CSW, CSWQ if qed else 0.0, prec=0, pairing=pairing, extra_precisions=(1, sloppy))
           for r in range(pg.world)}
-    lo = {r: hi[r].with_prec(1) for r in range(pg.world)}
+    lo = {r: hi[r].with_prec(sloppy) for r in range(pg.world)}
+    vec = {r: hi[r].with_prec(1) for r in range(pg.world)}
     comm = D.LocalComm(pg.world)
     ref = global_oracle(dims, cstar, ap, qed, U, A)
     eta = synth.gaussian_spinor(ref.dims_ext, 5)
     src = {r: hi[r].pack(lats[r].scatter(eta)) for r in range(pg.world)}
-    x, info = D.solve_distributed_mixed(D.GpuOperator(comm, lats, hi), D.GpuOperator(comm, lats, lo), src, 1e-10)
+    x, info = D.solve_distributed_mixed(D.GpuOperator(comm, lats, hi), D.GpuOperator(comm, lats, lo), src, 1e-10,
+                                        op_vec=D.GpuOperator(comm, lats, vec) if sloppy == 2 else None)
     assert info["status"] == 0 and info["n_reliable"] >= 2, info
     sol = np.zeros_like(eta)
     for r in range(pg.world):
