@@ -8,8 +8,8 @@ PAPER.md:137-139).  Here:
   k in 2..cstar lands, on the lattice doubled in direction 1, displaced by L1 in direction 1 -- on the rank N1/2 further
   along direction 1 if that direction is distributed, else on the same rank column with a LOCAL displacement by L1.
 * :class:`LocalLattice` is a rank's lattice: its own sites plus ghost layers in the cut directions (time: one tile = 4 slices
-  thick, so that the owned sites are whole time slabs of the device site order and nothing is computed on ghosts; direction
-  3: two layers, the one next to the owned sites carrying data).  Gauge and U(1) fields of the ghost layers are loaded with the rank's fields, once.
+  thick, so that the owned sites are whole time slabs of the device site order and nothing is computed on ghosts; directions
+  2 and 3: two layers, the one next to the owned sites carrying data).  Gauge and U(1) fields of the ghost layers are loaded with the rank's fields, once.
 * :func:`halo_exchange` fills the spinor ghost layers: the boundary layer is spin-projected to 12 reals per site by a kernel
   (qxd_face_gather), the face buffers travel as ONE batch of point-to-point operations (NCCL between GPUs), and
   qxd_face_scatter writes the ghost spinors, displaced by L1 where the message crossed a C* boundary.
@@ -27,7 +27,7 @@ from __future__ import annotations
 import numpy as np
 
 TIME_GHOST = 4          # thickness of the time ghost zones = tile extent b0 of the device site order
-SPACE_GHOST = 2         # thickness of the direction-3 ghost zones (keeps the local extent a multiple of the tile extent 4;
+SPACE_GHOST = 2         # thickness of the ghost zones of directions 2 and 3 (keeps the local extent a multiple of the tile extent 4;
                         # only the layer next to the owned sites carries data)
 
 
@@ -83,79 +83,90 @@ class ProcessGrid:
 
 
 class LocalLattice:
-    """The lattice of one rank: owned sites + ghost layers in the cut directions 0 and 3 (directions 1, 2 are not cut)."""
+    """The lattice of one rank: owned sites + ghost layers in the cut directions 0, 2 and 3 (direction 1, the doubled one, is not cut)."""
 
     def __init__(self, pg: ProcessGrid, rank: int, antiperiodic=True, force_cut=(False, False, False, False)):
-        if pg.grid[1] != 1 or pg.grid[2] != 1:
-            raise ValueError("LocalLattice: fields are decomposed along directions 0 and 3 only")
+        if pg.grid[1] != 1:
+            raise ValueError("LocalLattice: fields are decomposed along directions 0, 2 and 3 only")
         self.pg, self.rank = pg, rank
         self.c = pg.coords(rank)
         self.cut = tuple(pg.grid[mu] > 1 or bool(force_cut[mu]) for mu in range(4))
-        if self.cut[1] or self.cut[2]:
-            raise ValueError("LocalLattice: cuts along directions 0 and 3 only")
-        self.g = (TIME_GHOST if self.cut[0] else 0, 0, 0, SPACE_GHOST if self.cut[3] else 0)
+        if self.cut[1]:
+            raise ValueError("LocalLattice: cuts along directions 0, 2 and 3 only")
+        self.g = (TIME_GHOST if self.cut[0] else 0, 0, SPACE_GHOST if self.cut[2] else 0, SPACE_GHOST if self.cut[3] else 0)
         T, L1, L2, L3 = pg.dims
-        self.own = (T // pg.grid[0], L1, L2, L3 // pg.grid[3])             # owned PHYSICAL extents
+        self.own = (T // pg.grid[0], L1, L2 // pg.grid[2], L3 // pg.grid[3])             # owned PHYSICAL extents
         self.local_dims = tuple(self.own[mu] + 2 * self.g[mu] for mu in range(4))
-        self.origin = (self.c[0] * self.own[0], 0, 0, self.c[3] * self.own[3])
+        self.origin = (self.c[0] * self.own[0], 0, self.c[2] * self.own[2], self.c[3] * self.own[3])
         # boundary conditions of the local context: a cut direction is handled by the ghosts (periodic locally, which only
-        # couples ghost layers to each other); the C* count drops to 2 when direction 3 is cut
-        self.cstar_local = pg.cstar if not (self.cut[3] and pg.cstar == 3) else 2
+        # couples ghost layers to each other).  The library's C* directions are 1..cstar, so the uncut C* directions must
+        # still be a prefix: cutting direction 3 drops the count to 2, cutting 2 (and 3, if it is a C* direction) to 1
+        cs = pg.cstar
+        if cs == 3 and self.cut[2] and not self.cut[3]:
+            raise ValueError("LocalLattice: with cstar = 3 a cut along direction 2 needs direction 3 cut too (force_cut) -- "
+                             "the local C* directions must be 1..k")
+        if cs >= 2 and self.cut[2]:
+            cs = 1
+        elif cs == 3 and self.cut[3]:
+            cs = 2
+        self.cstar_local = cs
         self.antiperiodic = bool(antiperiodic)
         self.bc_local = self.cstar_local | ((1 if (antiperiodic and not self.cut[0]) else 0) << 2)
         X1 = (2 if pg.cstar else 1) * L1
-        self.local_ext = (self.local_dims[0], X1, L2, self.local_dims[3])   # extended local lattice (spinors)
+        self.local_ext = (self.local_dims[0], X1, self.local_dims[2], self.local_dims[3])   # extended local lattice (spinors)
         if self.cut[0] and (self.own[0] % TIME_GHOST or self.own[0] < 2 * TIME_GHOST):
             raise ValueError("LocalLattice: a time cut needs T_loc to be a multiple of 4 and >= 8 (whole tiles, two boundary slabs)")
 
     # ---- index maps -------------------------------------------------------------------------------------------------
     def _global_index(self):
         """For every local PHYSICAL site (incl. ghosts): global physical coordinates and whether the site is a C* mirror image
-        (reached through an odd number of C* boundary crossings in direction 3)."""
+        (reached through an odd number of C* boundary crossings in directions 2 and 3): mirror[y, z]."""
         T, L1, L2, L3 = self.pg.dims
         t = (self.origin[0] - self.g[0] + np.arange(self.local_dims[0])) % T
+        yr = self.origin[2] - self.g[2] + np.arange(self.local_dims[2])
         zr = self.origin[3] - self.g[3] + np.arange(self.local_dims[3])
-        z = zr % L3
-        mirror = ((zr // L3) % 2 != 0) & (self.pg.cstar == 3)
-        return t, z, mirror
+        y, z = yr % L2, zr % L3
+        my = ((yr // L2) % 2 != 0) & (self.pg.cstar >= 2)
+        mz = ((zr // L3) % 2 != 0) & (self.pg.cstar == 3)
+        return t, y, z, my[:, None] ^ mz[None, :]
 
     def local_fields(self, U, A=None):
         """Rank-local gauge field (and U(1) field) including the ghost layers.  With antiperiodic fermions and a time cut the
         time links of global slice T-1 carry the factor -1 (the local context is then periodic in time); links of ghost
         layers reached across a C* boundary are the mirror images conj(U), -A (reading R8)."""
-        t, z, mirror = self._global_index()
+        t, y, z, mirror = self._global_index()
         U = np.asarray(U)
-        Ul = np.ascontiguousarray(U[t][:, :, :, z])
-        Ul[:, :, :, mirror] = np.conj(Ul[:, :, :, mirror])
+        Ul = np.ascontiguousarray(U[t][:, :, y][:, :, :, z])
+        Ul[:, :, mirror] = np.conj(Ul[:, :, mirror])
         if self.antiperiodic and self.cut[0]:
             Ul[t == self.pg.dims[0] - 1, ..., 0, :, :] *= -1.0
         Al = None
         if A is not None:
-            Al = np.ascontiguousarray(np.asarray(A)[t][:, :, :, z])
-            Al[:, :, :, mirror] *= -1.0
+            Al = np.ascontiguousarray(np.asarray(A)[t][:, :, y][:, :, :, z])
+            Al[:, :, mirror] *= -1.0
         return Ul, Al
 
     def owned_slices(self):
-        return (slice(self.g[0], self.g[0] + self.own[0]), slice(None), slice(None), slice(self.g[3], self.g[3] + self.own[3]))
+        return (slice(self.g[0], self.g[0] + self.own[0]), slice(None), slice(self.g[2], self.g[2] + self.own[2]), slice(self.g[3], self.g[3] + self.own[3]))
 
     def scatter(self, psi_global):
         """Owned part of a global extended-lattice spinor [T][X1][L2][L3][4][3] placed into a local array with empty ghosts."""
         psi_global = np.asarray(psi_global)
         loc = np.zeros(self.local_ext + psi_global.shape[4:], dtype=psi_global.dtype)
         o = self.origin
-        loc[self.owned_slices()] = psi_global[o[0]:o[0] + self.own[0], :, :, o[3]:o[3] + self.own[3]]
+        loc[self.owned_slices()] = psi_global[o[0]:o[0] + self.own[0], :, o[2]:o[2] + self.own[2], o[3]:o[3] + self.own[3]]
         return loc
 
     def gather_into(self, psi_global, local):
         o = self.origin
-        psi_global[o[0]:o[0] + self.own[0], :, :, o[3]:o[3] + self.own[3]] = np.asarray(local).reshape(self.local_ext + psi_global.shape[4:])[self.owned_slices()]
+        psi_global[o[0]:o[0] + self.own[0], :, o[2]:o[2] + self.own[2], o[3]:o[3] + self.own[3]] = np.asarray(local).reshape(self.local_ext + psi_global.shape[4:])[self.owned_slices()]
 
     def messages(self):
         """The halo messages this rank SENDS, one per cut direction and side: dicts with the layer to gather (coord, sign of
         the projector the receiver's hop applies), the destination rank, the ghost layer it fills there and the displacement
         in direction 1 the receiver applies (C* shifted boundary)."""
         out = []
-        for mu in (3, 0):     # direction 3 first: its ghosts are needed by every time slab
+        for mu in (3, 2, 0):     # the spatial directions first: their ghosts are needed by every time slab
             if not self.cut[mu]:
                 continue
             g, n = self.g[mu], self.own[mu]
@@ -196,7 +207,7 @@ class TorchComm:
     """One rank per process under torch.distributed (NCCL on GPUs, gloo on CPU).  All point-to-point operations of an
     exchange go out as ONE batch (one ncclGroup): NCCL ignores tags and serialises the operations of a peer pair on one
     stream, so separately issued sends and receives between two ranks could block each other; messages between a pair are
-    matched by issue order, which is the same on both sides (direction 3 before 0, upward before downward).  A message to
+    matched by issue order, which is the same on both sides (directions 3, 2, 0, upward before downward).  A message to
     the rank itself (a direction with a single rank but ghosts) is a copy unless `self_via_dist` asks for a real send/recv
     pair (how the NCCL path is exercised on a single GPU)."""
 
@@ -236,7 +247,7 @@ class TorchComm:
                 self.dist.all_reduce(v)
 
 
-def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 0), g5in=False):
+def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 2, 0), g5in=False):
     """Fill the ghost layers of the spinors vecs[r] (r over the ranks this process holds) in the given cut directions.
     Gather kernels -> one batched exchange -> scatter kernels.  The tag of a message is (mu, side).  g5in: the operator pass
     applies gamma5 to its input (D-hat^dagger): the ghosts must then hold the projection of gamma5 psi, and since the upper
@@ -276,7 +287,7 @@ def halo_clear(lats, ops, vecs, ranks, parity_mask=3):
     """Zero the ghost layers (after the operator has used them), so that reductions over a vector see owned sites only."""
     for r in ranks:
         lat = lats[r]
-        for mu in (0, 3):
+        for mu in (0, 2, 3):
             if lat.cut[mu]:
                 g, n = lat.g[mu], lat.own[mu]
                 ops[r].halo_zero(vecs[r], parity_mask, mu, 0, g)
@@ -352,13 +363,13 @@ class GpuRank:
 
 
 def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, overlap=True):
-    """One dslash-shaped pass of the distributed operator on every rank of this process: direction-3 ghosts first (every slab
+    """One dslash-shaped pass of the distributed operator on every rank of this process: ghosts of directions 3 and 2 first (every slab
     needs them), then the time faces -- in flight while the interior slabs run when there is one rank per process."""
     ranks = comm.my_ranks
     pm = 3 if mode == 0 else (1 << (1 - parity_out))
     g5in = bool(flags & 1)        # QXD_DSF_G5IN
-    if any(lats[r].cut[3] for r in ranks):
-        halo_exchange(comm, lats, ops, vin, pm, directions=(3,), g5in=g5in)
+    if any(lats[r].cut[2] or lats[r].cut[3] for r in ranks):
+        halo_exchange(comm, lats, ops, vin, pm, directions=(3, 2), g5in=g5in)
     time_cut = any(lats[r].cut[0] for r in ranks)
     ph = {r: (phi[r] if phi is not None else None) for r in ranks}
     if time_cut and overlap and isinstance(comm, TorchComm) and vin[ranks[0]].is_cuda:
@@ -390,14 +401,15 @@ def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, ove
         for r in ranks:
             ops[r].dslash("all", mode, vin[r], vout[r], parity_out, flags, ph[r])
     halo_clear(lats, ops, vin, ranks, pm)
-    # time ghosts are never computed (whole slabs are skipped); the direction-3 ghost layers lie inside the owned slabs and
+    # time ghosts are never computed (whole slabs are skipped); the ghost layers of directions 2 and 3 lie inside the owned slabs and
     # do receive (meaningless) results: clear them, so that the output is zero outside the owned sites
     pmo = 3 if mode == 0 else (1 << parity_out)
     for r in ranks:
-        if lats[r].cut[3]:
-            g, n = lats[r].g[3], lats[r].own[3]
-            ops[r].halo_zero(vout[r], pmo, 3, 0, g)
-            ops[r].halo_zero(vout[r], pmo, 3, g + n, 2 * g + n)
+        for mu in (2, 3):
+            if lats[r].cut[mu]:
+                g, n = lats[r].g[mu], lats[r].own[mu]
+                ops[r].halo_zero(vout[r], pmo, mu, 0, g)
+                ops[r].halo_zero(vout[r], pmo, mu, g + n, 2 * g + n)
 
 
 class GpuOperator:

@@ -61,6 +61,18 @@ def test_rank_map_matches_global_neighbour_table(dims, grid, cstar):
                 assert yl == tuple(exp), (x, mu, step)
 
 
+def test_direction_2_cut_needs_prefix_of_cstar_directions():
+    """The library's C* directions are 1..cstar: with cstar = 3 a rank lattice cut along 2 but not along 3 cannot be expressed
+    (its local C* directions would be 1 and 3); with ghost zones in direction 3 as well it can (local cstar 1)."""
+    pg = D.ProcessGrid((4, 2, 8, 4), (1, 1, 2, 1), 3)
+    with pytest.raises(ValueError):
+        D.LocalLattice(pg, 0)
+    lat = D.LocalLattice(pg, 0, force_cut=(False, False, False, True))
+    assert lat.cstar_local == 1 and lat.local_dims == (4, 2, 8, 8) and lat.cut == (False, False, True, True)
+    assert D.LocalLattice(D.ProcessGrid((4, 2, 8, 4), (1, 1, 2, 1), 2), 0).cstar_local == 1
+    assert D.LocalLattice(D.ProcessGrid((4, 2, 4, 8), (1, 1, 1, 2), 3), 0).cstar_local == 2
+
+
 def test_process_grid_rejects_bad_splits():
     with pytest.raises(ValueError):
         D.ProcessGrid((6, 4, 4, 4), (2, 1, 1, 1))          # 3 slices per rank
@@ -168,6 +180,9 @@ GRIDS = [
     ((4, 2, 4, 8), (1, 1, 1, 2), 3, 1, True),       # the cut crosses a C* direction: ghosts arrive displaced by L1
     ((4, 2, 4, 8), (1, 1, 1, 2), 2, 0, True),       # direction 3 periodic
     ((16, 2, 2, 8), (2, 1, 1, 2), 3, 1, True),
+    ((4, 2, 8, 4), (1, 1, 2, 1), 2, 1, True),       # cut along direction 2, a C* direction (the cut of the round-1 review)
+    ((4, 4, 8, 4), (1, 1, 2, 1), 0, 1, False),
+    ((4, 2, 8, 8), (1, 1, 2, 2), 3, 0, True),       # directions 2 and 3 cut, both C*: four ranks
 ]
 
 
@@ -273,6 +288,9 @@ GPU_GRIDS = [
     ((12, 4, 4, 8), (1, 1, 1, 2), 2, 1, True, True),
     ((16, 4, 4, 8), (2, 1, 1, 2), 3, 1, True, True),     # four ranks, both cuts
     ((32, 4, 4, 4), (4, 1, 1, 1), 1, 1, True, None),
+    ((12, 4, 8, 4), (1, 1, 2, 1), 2, 1, True, True),     # cut along direction 2 (C*), paired layout
+    ((12, 4, 8, 8), (1, 1, 2, 2), 3, 1, True, False),    # directions 2 and 3
+    ((16, 4, 8, 4), (2, 1, 2, 1), 2, 0, True, True),     # time and direction 2
 ]
 
 
@@ -312,7 +330,7 @@ def test_gpu_distributed_Dw(dims, grid, cstar, ap, qed, pairing, prec):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[3], GPU_GRIDS[6]])
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[3], GPU_GRIDS[6], GPU_GRIDS[8], GPU_GRIDS[10]])
 def test_gpu_distributed_solve(dims, grid, cstar, ap, qed, pairing):
     """Distributed even-odd CGNE (fp64): source preparation, D-hat with two halo exchanges per application, all-reduced
     scalars, reconstruction; the global solution must satisfy ||eta - D_ref psi|| / ||eta|| <= tol with the oracle's D_w."""
