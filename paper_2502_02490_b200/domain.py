@@ -7,7 +7,7 @@ PAPER.md:137-139).  Here:
 * :class:`ProcessGrid` is that neighbour map as a pure function: a hop across the global boundary of a C* direction
   k in 2..cstar lands, on the lattice doubled in direction 1, displaced by L1 in direction 1 -- on the rank N1/2 further
   along direction 1 if that direction is distributed, else on the same rank column with a LOCAL displacement by L1.
-* :class:`LocalLattice` is a rank's lattice: its own sites plus ghost layers in the cut directions (time: one tile = 4 slices
+* :class:`LocalLattice` is a rank's lattice: its own sites plus ghost layers in the cut directions, any of the four (time: one tile = 4 slices
   thick, so that the owned sites are whole time slabs of the device site order and nothing is computed on ghosts; directions
   2 and 3: two layers, the one next to the owned sites carrying data).  Gauge and U(1) fields of the ghost layers are loaded with the rank's fields, once.
 * :func:`halo_exchange` fills the spinor ghost layers: the boundary layer is spin-projected to 12 reals per site by a kernel
@@ -83,90 +83,110 @@ class ProcessGrid:
 
 
 class LocalLattice:
-    """The lattice of one rank: owned sites + ghost layers in the cut directions 0, 2 and 3 (direction 1, the doubled one, is not cut)."""
+    """The lattice of one rank: owned sites + ghost layers in the cut directions.
+
+    Directions 0, 2, 3: the rank keeps the whole doubled direction 1 and its context is a C* lattice of its own.  A cut along
+    direction 1 (the paper's layout: the mirror half of the doubled lattice lives on OTHER ranks) makes the
+    local lattice an ordinary periodic one: direction 1 and every C* direction get ghost zones, the hop across the global
+    boundary of a C* direction arrives from the rank N1/2 further along direction 1 (ProcessGrid.neighbour), and the gauge
+    field of the sites with extended coordinate x1 >= L1 is the mirror image conj(U), -A."""
 
     def __init__(self, pg: ProcessGrid, rank: int, antiperiodic=True, force_cut=(False, False, False, False)):
-        if pg.grid[1] != 1:
-            raise ValueError("LocalLattice: fields are decomposed along directions 0, 2 and 3 only")
         self.pg, self.rank = pg, rank
         self.c = pg.coords(rank)
-        self.cut = tuple(pg.grid[mu] > 1 or bool(force_cut[mu]) for mu in range(4))
-        if self.cut[1]:
-            raise ValueError("LocalLattice: cuts along directions 0, 2 and 3 only")
-        self.g = (TIME_GHOST if self.cut[0] else 0, 0, SPACE_GHOST if self.cut[2] else 0, SPACE_GHOST if self.cut[3] else 0)
+        cut = [pg.grid[mu] > 1 or bool(force_cut[mu]) for mu in range(4)]
+        if cut[1] and not pg.cstar:
+            raise ValueError("LocalLattice: direction 1 is cut only on C* lattices (use directions 0, 2, 3 otherwise)")
+        if cut[1]:
+            for mu in range(2, pg.cstar + 1):      # their wrap leaves the rank: they need ghost zones whatever grid[mu] is
+                cut[mu] = True
+        self.cut = tuple(cut)
+        self.g = (TIME_GHOST if cut[0] else 0, SPACE_GHOST if cut[1] else 0, SPACE_GHOST if cut[2] else 0, SPACE_GHOST if cut[3] else 0)
         T, L1, L2, L3 = pg.dims
-        self.own = (T // pg.grid[0], L1, L2 // pg.grid[2], L3 // pg.grid[3])             # owned PHYSICAL extents
+        X1 = (2 if pg.cstar else 1) * L1
+        # owned extents: PHYSICAL in the directions of a C* context, EXTENDED in direction 1 when it is cut (the context is then periodic)
+        self.own = (T // pg.grid[0], X1 // pg.grid[1] if cut[1] else L1, L2 // pg.grid[2], L3 // pg.grid[3])
         self.local_dims = tuple(self.own[mu] + 2 * self.g[mu] for mu in range(4))
-        self.origin = (self.c[0] * self.own[0], 0, self.c[2] * self.own[2], self.c[3] * self.own[3])
+        self.origin = (self.c[0] * self.own[0], self.c[1] * self.own[1] if cut[1] else 0, self.c[2] * self.own[2], self.c[3] * self.own[3])
         # boundary conditions of the local context: a cut direction is handled by the ghosts (periodic locally, which only
         # couples ghost layers to each other).  The library's C* directions are 1..cstar, so the uncut C* directions must
-        # still be a prefix: cutting direction 3 drops the count to 2, cutting 2 (and 3, if it is a C* direction) to 1
+        # still be a prefix: cutting direction 3 drops the count to 2, cutting 2 (and 3, if it is a C* direction) to 1,
+        # cutting 1 to 0
         cs = pg.cstar
-        if cs == 3 and self.cut[2] and not self.cut[3]:
+        if cut[1]:
+            cs = 0
+        elif cs == 3 and cut[2] and not cut[3]:
             raise ValueError("LocalLattice: with cstar = 3 a cut along direction 2 needs direction 3 cut too (force_cut) -- "
                              "the local C* directions must be 1..k")
-        if cs >= 2 and self.cut[2]:
+        elif cs >= 2 and cut[2]:
             cs = 1
-        elif cs == 3 and self.cut[3]:
+        elif cs == 3 and cut[3]:
             cs = 2
         self.cstar_local = cs
         self.antiperiodic = bool(antiperiodic)
-        self.bc_local = self.cstar_local | ((1 if (antiperiodic and not self.cut[0]) else 0) << 2)
-        X1 = (2 if pg.cstar else 1) * L1
-        self.local_ext = (self.local_dims[0], X1, self.local_dims[2], self.local_dims[3])   # extended local lattice (spinors)
-        if self.cut[0] and (self.own[0] % TIME_GHOST or self.own[0] < 2 * TIME_GHOST):
+        self.bc_local = self.cstar_local | ((1 if (antiperiodic and not cut[0]) else 0) << 2)
+        self.local_ext = (self.local_dims[0], self.local_dims[1] if cut[1] else X1, self.local_dims[2], self.local_dims[3])   # extended local lattice (spinors)
+        if cut[0] and (self.own[0] % TIME_GHOST or self.own[0] < 2 * TIME_GHOST):
             raise ValueError("LocalLattice: a time cut needs T_loc to be a multiple of 4 and >= 8 (whole tiles, two boundary slabs)")
 
     # ---- index maps -------------------------------------------------------------------------------------------------
     def _global_index(self):
-        """For every local PHYSICAL site (incl. ghosts): global physical coordinates and whether the site is a C* mirror image
-        (reached through an odd number of C* boundary crossings in directions 2 and 3): mirror[y, z]."""
+        """For every local site of the context's lattice (incl. ghosts): global PHYSICAL coordinates and whether the site is a
+        C* mirror image: mirror[x1, y, z] (x1 in the mirror half of the doubled lattice when direction 1 is cut, XOR an odd
+        number of C* boundary crossings in directions 2 and 3)."""
         T, L1, L2, L3 = self.pg.dims
         t = (self.origin[0] - self.g[0] + np.arange(self.local_dims[0])) % T
+        if self.cut[1]:
+            x1e = (self.origin[1] - self.g[1] + np.arange(self.local_dims[1])) % (2 * L1)
+            x1, m1 = x1e % L1, x1e >= L1
+        else:
+            x1, m1 = np.arange(L1), np.zeros(L1, dtype=bool)
         yr = self.origin[2] - self.g[2] + np.arange(self.local_dims[2])
         zr = self.origin[3] - self.g[3] + np.arange(self.local_dims[3])
         y, z = yr % L2, zr % L3
         my = ((yr // L2) % 2 != 0) & (self.pg.cstar >= 2)
         mz = ((zr // L3) % 2 != 0) & (self.pg.cstar == 3)
-        return t, y, z, my[:, None] ^ mz[None, :]
+        return t, x1, y, z, m1[:, None, None] ^ my[None, :, None] ^ mz[None, None, :]
 
     def local_fields(self, U, A=None):
         """Rank-local gauge field (and U(1) field) including the ghost layers.  With antiperiodic fermions and a time cut the
-        time links of global slice T-1 carry the factor -1 (the local context is then periodic in time); links of ghost
-        layers reached across a C* boundary are the mirror images conj(U), -A (reading R8)."""
-        t, y, z, mirror = self._global_index()
+        time links of global slice T-1 carry the factor -1 (the local context is then periodic in time); links of sites
+        that are C* mirror images are conj(U), -A (reading R8)."""
+        t, x1, y, z, mirror = self._global_index()
         U = np.asarray(U)
-        Ul = np.ascontiguousarray(U[t][:, :, y][:, :, :, z])
-        Ul[:, :, mirror] = np.conj(Ul[:, :, mirror])
+        Ul = np.ascontiguousarray(U[t][:, x1][:, :, y][:, :, :, z])
+        Ul[:, mirror] = np.conj(Ul[:, mirror])
         if self.antiperiodic and self.cut[0]:
             Ul[t == self.pg.dims[0] - 1, ..., 0, :, :] *= -1.0
         Al = None
         if A is not None:
-            Al = np.ascontiguousarray(np.asarray(A)[t][:, :, y][:, :, :, z])
-            Al[:, :, mirror] *= -1.0
+            Al = np.ascontiguousarray(np.asarray(A)[t][:, x1][:, :, y][:, :, :, z])
+            Al[:, mirror] *= -1.0
         return Ul, Al
 
     def owned_slices(self):
-        return (slice(self.g[0], self.g[0] + self.own[0]), slice(None), slice(self.g[2], self.g[2] + self.own[2]), slice(self.g[3], self.g[3] + self.own[3]))
+        return tuple(slice(self.g[mu], self.g[mu] + self.own[mu]) if self.cut[mu] else slice(None) for mu in range(4))
+
+    def _global_slices(self):
+        o = self.origin
+        return tuple(slice(o[mu], o[mu] + self.own[mu]) if self.cut[mu] else slice(None) for mu in range(4))
 
     def scatter(self, psi_global):
         """Owned part of a global extended-lattice spinor [T][X1][L2][L3][4][3] placed into a local array with empty ghosts."""
         psi_global = np.asarray(psi_global)
         loc = np.zeros(self.local_ext + psi_global.shape[4:], dtype=psi_global.dtype)
-        o = self.origin
-        loc[self.owned_slices()] = psi_global[o[0]:o[0] + self.own[0], :, o[2]:o[2] + self.own[2], o[3]:o[3] + self.own[3]]
+        loc[self.owned_slices()] = psi_global[self._global_slices()]
         return loc
 
     def gather_into(self, psi_global, local):
-        o = self.origin
-        psi_global[o[0]:o[0] + self.own[0], :, o[2]:o[2] + self.own[2], o[3]:o[3] + self.own[3]] = np.asarray(local).reshape(self.local_ext + psi_global.shape[4:])[self.owned_slices()]
+        psi_global[self._global_slices()] = np.asarray(local).reshape(self.local_ext + psi_global.shape[4:])[self.owned_slices()]
 
     def messages(self):
         """The halo messages this rank SENDS, one per cut direction and side: dicts with the layer to gather (coord, sign of
         the projector the receiver's hop applies), the destination rank, the ghost layer it fills there and the displacement
         in direction 1 the receiver applies (C* shifted boundary)."""
         out = []
-        for mu in (3, 2, 0):     # the spatial directions first: their ghosts are needed by every time slab
+        for mu in (3, 2, 1, 0):     # the spatial directions first: their ghosts are needed by every time slab
             if not self.cut[mu]:
                 continue
             g, n = self.g[mu], self.own[mu]
@@ -247,7 +267,7 @@ class TorchComm:
                 self.dist.all_reduce(v)
 
 
-def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 2, 0), g5in=False):
+def halo_exchange(comm, lats, ops, vecs, parity_mask=3, directions=(3, 2, 1, 0), g5in=False):
     """Fill the ghost layers of the spinors vecs[r] (r over the ranks this process holds) in the given cut directions.
     Gather kernels -> one batched exchange -> scatter kernels.  The tag of a message is (mu, side).  g5in: the operator pass
     applies gamma5 to its input (D-hat^dagger): the ghosts must then hold the projection of gamma5 psi, and since the upper
@@ -287,7 +307,7 @@ def halo_clear(lats, ops, vecs, ranks, parity_mask=3):
     """Zero the ghost layers (after the operator has used them), so that reductions over a vector see owned sites only."""
     for r in ranks:
         lat = lats[r]
-        for mu in (0, 2, 3):
+        for mu in (0, 1, 2, 3):
             if lat.cut[mu]:
                 g, n = lat.g[mu], lat.own[mu]
                 ops[r].halo_zero(vecs[r], parity_mask, mu, 0, g)
@@ -368,8 +388,8 @@ def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, ove
     ranks = comm.my_ranks
     pm = 3 if mode == 0 else (1 << (1 - parity_out))
     g5in = bool(flags & 1)        # QXD_DSF_G5IN
-    if any(lats[r].cut[2] or lats[r].cut[3] for r in ranks):
-        halo_exchange(comm, lats, ops, vin, pm, directions=(3, 2), g5in=g5in)
+    if any(lats[r].cut[1] or lats[r].cut[2] or lats[r].cut[3] for r in ranks):
+        halo_exchange(comm, lats, ops, vin, pm, directions=(3, 2, 1), g5in=g5in)
     time_cut = any(lats[r].cut[0] for r in ranks)
     ph = {r: (phi[r] if phi is not None else None) for r in ranks}
     if time_cut and overlap and isinstance(comm, TorchComm) and vin[ranks[0]].is_cuda:
@@ -405,7 +425,7 @@ def _pass(comm, lats, ops, vin, vout, mode, flags=0, parity_out=0, phi=None, ove
     # do receive (meaningless) results: clear them, so that the output is zero outside the owned sites
     pmo = 3 if mode == 0 else (1 << parity_out)
     for r in ranks:
-        for mu in (2, 3):
+        for mu in (1, 2, 3):
             if lats[r].cut[mu]:
                 g, n = lats[r].g[mu], lats[r].own[mu]
                 ops[r].halo_zero(vout[r], pmo, mu, 0, g)

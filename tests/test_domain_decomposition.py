@@ -71,6 +71,10 @@ def test_direction_2_cut_needs_prefix_of_cstar_directions():
     assert lat.cstar_local == 1 and lat.local_dims == (4, 2, 8, 8) and lat.cut == (False, False, True, True)
     assert D.LocalLattice(D.ProcessGrid((4, 2, 8, 4), (1, 1, 2, 1), 2), 0).cstar_local == 1
     assert D.LocalLattice(D.ProcessGrid((4, 2, 4, 8), (1, 1, 1, 2), 3), 0).cstar_local == 2
+    lat = D.LocalLattice(D.ProcessGrid((4, 4, 4, 4), (1, 2, 1, 1), 3), 1)      # direction 1 cut: every C* direction gets ghosts
+    assert lat.cstar_local == 0 and lat.cut == (False, True, True, True) and lat.local_dims == (4, 8, 8, 8) and lat.origin == (0, 4, 0, 0)
+    with pytest.raises(ValueError):
+        D.LocalLattice(D.ProcessGrid((4, 4, 4, 4), (1, 2, 1, 1), 0), 0)
 
 
 def test_process_grid_rejects_bad_splits():
@@ -183,6 +187,9 @@ GRIDS = [
     ((4, 2, 8, 4), (1, 1, 2, 1), 2, 1, True),       # cut along direction 2, a C* direction (the cut of the round-1 review)
     ((4, 4, 8, 4), (1, 1, 2, 1), 0, 1, False),
     ((4, 2, 8, 8), (1, 1, 2, 2), 3, 0, True),       # directions 2 and 3 cut, both C*: four ranks
+    ((4, 4, 4, 4), (1, 2, 1, 1), 3, 1, True),       # direction 1 cut: the mirror half lives on the other rank
+    ((4, 4, 4, 4), (1, 2, 1, 1), 1, 0, True),
+    ((4, 4, 4, 8), (1, 4, 1, 2), 2, 1, True),       # eight ranks: a C* hop in direction 2 lands N1/2 = 2 ranks further along direction 1
 ]
 
 
@@ -291,6 +298,8 @@ GPU_GRIDS = [
     ((12, 4, 8, 4), (1, 1, 2, 1), 2, 1, True, True),     # cut along direction 2 (C*), paired layout
     ((12, 4, 8, 8), (1, 1, 2, 2), 3, 1, True, False),    # directions 2 and 3
     ((16, 4, 8, 4), (2, 1, 2, 1), 2, 0, True, True),     # time and direction 2
+    ((12, 4, 4, 4), (1, 2, 1, 1), 3, 1, True, None),     # direction 1 cut: periodic local lattices, C* through the rank map alone
+    ((16, 8, 4, 4), (2, 2, 1, 1), 1, 1, True, None),     # time and direction 1
 ]
 
 
@@ -330,7 +339,7 @@ def test_gpu_distributed_Dw(dims, grid, cstar, ap, qed, pairing, prec):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[3], GPU_GRIDS[6], GPU_GRIDS[8], GPU_GRIDS[10]])
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed,pairing", [GPU_GRIDS[1], GPU_GRIDS[3], GPU_GRIDS[6], GPU_GRIDS[8], GPU_GRIDS[10], GPU_GRIDS[11], GPU_GRIDS[12]])
 def test_gpu_distributed_solve(dims, grid, cstar, ap, qed, pairing):
     """Distributed even-odd CGNE (fp64): source preparation, D-hat with two halo exchanges per application, all-reduced
     scalars, reconstruction; the global solution must satisfy ||eta - D_ref psi|| / ||eta|| <= tol with the oracle's D_w."""
