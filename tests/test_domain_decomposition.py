@@ -253,7 +253,8 @@ def _gloo_worker(rank, world, port, dims, grid, cstar, ap, qed, q):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("dims,grid,cstar,ap,qed", [((16, 2, 4, 4), (2, 1, 1, 1), 3, 1, True), ((4, 2, 4, 8), (1, 1, 1, 2), 3, 1, True)])
+@pytest.mark.parametrize("dims,grid,cstar,ap,qed", [((16, 2, 4, 4), (2, 1, 1, 1), 3, 1, True), ((4, 2, 4, 8), (1, 1, 1, 2), 3, 1, True),
+                                                    ((4, 4, 4, 4), (1, 2, 1, 1), 3, 1, True)])
 def test_world_size_2_gloo_Dw_and_solve(dims, grid, cstar, ap, qed):
     """One rank per process, torch.distributed `gloo`, world_size 2: batched point-to-point halo exchange matched by issue
     order (both time neighbours of a rank are the SAME peer here), all-reduced CG scalars; D_w and the solve against the
