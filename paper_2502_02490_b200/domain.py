@@ -517,11 +517,11 @@ def cgne(op, b, tol2_abs, maxiter=10000):
         op.norm2(t, tt)
         op.cg_xr(gam, tt, p, t, x, r, rr)
         it += 1
+        op.apply(r, s, dagger=True)        # enqueued before the host reads |r|^2: the device does not idle on the round trip
+        op.norm2(s, gam2)
         res2 = op.value(rr)
         if not (res2 == res2) or res2 <= tol2_abs:
             break
-        op.apply(r, s, dagger=True)
-        op.norm2(s, gam2)
         op.cg_p(gam2, gam, s, p)
         gam, gam2 = gam2, gam
     return x, dict(iters=it, res2=res2, status=0 if res2 <= tol2_abs else -5)
@@ -607,6 +607,10 @@ def solve_distributed_mixed(op_hi: GpuOperator, op_lo: GpuOperator, eta, tol, de
         L.norm2(t, tt)
         L.cg_xr(gam, tt, p, t, xlo, rlo, rr)
         it += 1
+        # s = A^dag r is enqueued BEFORE the host reads |r|^2 (as in csrc/solver.cu): the device never idles on the round trip;
+        # the work is only wasted in the iterations that do a reliable update
+        L.apply(rlo, s, dagger=True)
+        L.norm2(s, gam2)
         res2 = L.value(rr)
         if not (res2 == res2):
             break
@@ -619,8 +623,8 @@ def solve_distributed_mixed(op_hi: GpuOperator, op_lo: GpuOperator, eta, tol, de
             if rr_true <= stop2:
                 status = 0
                 break
-        L.apply(rlo, s, dagger=True)
-        L.norm2(s, gam2)
+            L.apply(rlo, s, dagger=True)
+            L.norm2(s, gam2)
         L.cg_p(gam2, gam, s, p)
         gam, gam2 = gam2, gam
     if status:
@@ -689,6 +693,8 @@ def _solve_distributed_h16(H: GpuOperator, L: GpuOperator, V: GpuOperator, eta, 
             ol.g.blas_cg_xr_h(gam[r], tt[r], ol.half(p16[r]), ol.half(t[r]), ov.half(xlo[r]), ov.half(rlo[r]), ol.half(r16[r]), rr[r])
         L.comm.allreduce_sum(rr)
         it += 1
+        L.apply(r16, s, dagger=True)          # enqueued before the host reads |r|^2 (see solve_distributed_mixed)
+        L.norm2(s, gam2)
         res2 = L.value(rr)
         if not (res2 == res2):
             break
@@ -701,8 +707,8 @@ def _solve_distributed_h16(H: GpuOperator, L: GpuOperator, V: GpuOperator, eta, 
             if rr_true <= stop2:
                 status = 0
                 break
-        L.apply(r16, s, dagger=True)
-        L.norm2(s, gam2)
+            L.apply(r16, s, dagger=True)
+            L.norm2(s, gam2)
         for r in ranks:
             ol, ov = L.ops[r], V.ops[r]
             ol.g.blas_cg_p_h(gam2[r], gam[r], ol.half(s[r]), ov.half(p[r]), ol.half(p16[r]))
