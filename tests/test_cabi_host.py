@@ -167,3 +167,28 @@ def test_sap_blocks_are_two_coloured(lib, dims, cstar, pairing, ok):
                     assert c2 != c, (cb, p, mu, step)
     assert crossings > 0
     lib.qxd_geometry_destroy(h)
+
+
+def test_solver_space_setters_check_their_arguments(lib):
+    """qxd_set_gcr / qxd_set_deflation / qxd_set_deflation_chirality / qxd_set_deflation_refine: host-side argument checks (no GPU
+    needed: the solver spaces are only carved at qxd_workspace_bind)."""
+    h = C.c_void_p()
+    assert lib.qxd_geometry_create(8, 8, 8, 8, 4, C.byref(h)) == 0
+    assert lib.qxd_set_gcr(h, 16, 4, 5) == 0
+    assert lib.qxd_set_gcr(h, 33, 4, 5) == -1
+    assert lib.qxd_set_deflation(h, 24, 8, 12, 0) == 0
+    assert lib.qxd_set_deflation(h, 7, 8, 12, 0) == -1                 # odd number of null vectors
+    assert lib.qxd_set_deflation(h, 34, 8, 12, 0) == -1
+    assert lib.qxd_set_deflation_chirality(h, 1) == -1                 # 24 vectors would be 48 coarse degrees of freedom per block
+    assert b"16" in lib.qxd_last_error(h)
+    assert lib.qxd_set_deflation(h, 16, 8, 12, 0) == 0
+    assert lib.qxd_set_deflation_chirality(h, 1) == 0
+    assert lib.qxd_set_deflation(h, 18, 8, 12, 0) == -1                # and the other way round
+    assert lib.qxd_set_deflation_chirality(h, 2) == -1
+    assert lib.qxd_set_deflation_refine(h, 2, 4) == 0
+    assert lib.qxd_set_deflation_refine(h, -1, 4) == -1
+    assert lib.qxd_set_deflation_refine(h, 1, 0) == -1 and lib.qxd_set_deflation_refine(h, 1, 17) == -1
+    nb, ns, ready = C.c_int(), C.c_int(), C.c_int()
+    assert lib.qxd_deflation_info(h, C.byref(nb), C.byref(ns), C.byref(ready)) == 0
+    assert (nb.value, ns.value, ready.value) == (8 * 8 * 8 * 8 // 256, 32, 0)
+    assert lib.qxd_geometry_destroy(h) == 0
