@@ -255,6 +255,37 @@ def test_coarse_solve_even_odd(dims, cstar, qed, pairing, chiral):
     assert res[0] < 0.5 and res[1] < 5e-3 and res[1] < 0.1 * res[0], res
 
 
+@pytest.mark.parametrize("ns,chiral", [(2, 0), (2, 1), (16, 1), (32, 0)])
+def test_coarse_level_at_the_extreme_sizes(ns, chiral):
+    """The smallest and the largest coarse dimensions per block (2 and 32; CTA shapes of the coarse kernels depend on it): R P = 1,
+    A_c c = R D_w P c through the fp32 D_w kernel, the coarse solver reduces the residual, and the solve converges."""
+    import torch
+    dims, cstar, qed, pairing = SAP_CASES[0]
+    c, _ = _dfl_case(dims, cstar, qed, pairing, ns=ns, ninv=2, nkc=16, chiral=chiral)
+    g = c.gpu
+    nb, nc, ready = g.deflation_info()
+    assert ready and nc == ns * (1 + chiral)
+    rng = np.random.default_rng(3)
+    cc = torch.from_numpy((rng.normal(size=(nb, nc)) + 1j * rng.normal(size=(nb, nc))).astype(np.complex64)).cuda()
+    fine, back = g.new_packed(F32), torch.empty_like(cc)
+    g.deflation_op(1, cc, fine)
+    g.deflation_op(0, fine, back)
+    assert float((back - cc).abs().max() / cc.abs().max()) < 5e-5
+    dfine, ref_c, got_c = g.new_packed(F32), torch.empty_like(cc), torch.empty_like(cc)
+    g.apply_Dw_packed(fine, dfine, F32)
+    g.deflation_op(0, dfine, ref_c)
+    g.deflation_op(2, cc, got_c)
+    assert float((got_c - ref_c).abs().max() / ref_c.abs().max()) < 2e-4
+    x, ax = torch.empty_like(cc), torch.empty_like(cc)
+    g.deflation_op(4, cc, x)
+    g.deflation_op(2, x, ax)
+    assert float(torch.linalg.vector_norm(cc - ax) / torch.linalg.vector_norm(cc)) < 2e-2
+    eta = synth.gaussian_spinor(c.dims_ext, 5)
+    psi, info = g.solve(eta, 1e-10, algo=DFL_GCR, sloppy=F16)
+    assert info["status"] == 0 and true_residual(c.ref, eta, to_np(psi).reshape(eta.shape)) <= 1.05e-10
+    c.close()
+
+
 def test_deflation_pays_on_a_smooth_field():
     """On links with long-range order (synth.su3_links_smooth) close to the critical hopping parameter the low modes are locally
     coherent: the deflated solver must need clearly fewer GCR steps than the plain Schwarz-preconditioned one, both reaching the
